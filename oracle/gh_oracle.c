@@ -1,0 +1,642 @@
+/* gh_oracle.c — CPU ORACLE.  TEST INFRASTRUCTURE, NOT PRODUCT.
+ *
+ * A plain, slow, obviously-correct implementation of what the hot path of
+ * arXiv 1804.09101 computes: spectral derivatives on Chebyshev^3 blocks and
+ * Chebyshev x Y_lm shells, the pointwise right-hand side of the first-order
+ * generalized-harmonic (GH) Einstein system, the SSP-RK3 update and the
+ * constraint norms.  Only tests/, __graft_entry__.smoke() and bench.py's
+ * cpu_baseline / --impl reference legs may call it.  It shares no code with
+ * paper_1804_09101_b200/csrc (no headers, tables, helpers); the CUDA path must
+ * never call it.
+ *
+ * How it differs from the CUDA path on purpose:
+ *   - derivatives are MODAL: explicit-sum transforms to Chebyshev / Y_lm
+ *     coefficients, recurrence-based differentiation, explicit-sum synthesis
+ *     (Eqs. 14-18; Eqs. 23-24) — never a
+ *     cached differentiation matrix;
+ *   - the GH right-hand side is written as index loops over FULL 4x4 and
+ *     3x4x4 arrays with no symmetry exploitation;
+ *   - arithmetic is `long double` (x87 80-bit) by default, because an FP64
+ *     recurrence-based derivative is itself only ~1e-11 accurate at N>=32
+ *     (SURVEY.md §7 hard part 1) and cannot referee a 1e-11 bar.  Compile with
+ *     -DORA_DOUBLE for the timed CPU baseline (same source, Real=double).
+ *
+ * The paper never prints the evolved equations (it says "the Einstein equations
+ * in their generalized harmonic formulation", first order in
+ * "about 50 fundamental variables").  The system coded in
+ * ora_rhs_point() is the standard first-order GH system of the paper's ref.
+ * [34] lineage (Lindblom, Scheel, Kidder, Owen, Rinne 2006) as written out in
+ * SURVEY.md §8(c) O5 / DESIGN.md "Readings" S1.
+ *
+ * Parity pins (tests/test_oracle_*.py): monomials, the textbook CGL matrix,
+ * Gauss-Legendre exactness, Y_lm orthonormality / Unsold / closed forms,
+ * Cartesian polynomials on shells, Kerr-Schild lapse/shift closed forms,
+ * stationarity of exact Kerr-Schild data with analytic derivatives, the harmonic
+ * gauge wave, homogeneous damping-term cases, RK3 order.  PARITY UNPINNED (pure
+ * conventions, fixed by DESIGN.md): the normalisation of the constraint norms
+ * (unweighted RMS over points and components) and the default gamma's.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#ifdef ORA_DOUBLE
+typedef double real;
+#define R_SQRT sqrt
+#define R_COS cos
+#define R_SIN sin
+#define R_ACOS acos
+#define R_FABS fabs
+#define R_PI 3.14159265358979323846
+#else
+typedef long double real;
+#define R_SQRT sqrtl
+#define R_COS cosl
+#define R_SIN sinl
+#define R_ACOS acosl
+#define R_FABS fabsl
+#define R_PI 3.14159265358979323846264338327950288L
+#endif
+
+typedef struct {
+  int32_t kind;      /* 0 = shell (I1 x S2), 1 = block (I1^3) */
+  int32_t n[3];      /* shell: {N_r, L, unused}; block: {N_x, N_y, N_z} */
+  double lo[3], hi[3]; /* shell: lo[0]=r_in, hi[0]=r_out; block: corners */
+  double center[3];  /* shell centre */
+  int32_t face[6];   /* 1 = FROZEN. shell: [0]=inner,[1]=outer; block: -x,+x,-y,+y,-z,+z */
+  double gamma[3];   /* constraint damping gamma0, gamma1, gamma2 */
+} ora_subdomain;
+
+int ora_real_bytes(void) { return (int)sizeof(real); }
+
+/* ---------------------------------------------------------------------- */
+/* grid                                                                   */
+/* ---------------------------------------------------------------------- */
+static void dims(const ora_subdomain* sd, int* n0, int* n1, int* n2) {
+  if (sd->kind == 0) { *n0 = sd->n[0]; *n1 = sd->n[1] + 1; *n2 = 2 * (sd->n[1] + 1); }
+  else { *n0 = sd->n[0]; *n1 = sd->n[1]; *n2 = sd->n[2]; }
+}
+
+int64_t ora_num_points(const ora_subdomain* sd) {
+  int a, b, c; dims(sd, &a, &b, &c); return (int64_t)a * b * c;
+}
+
+/* Chebyshev-Gauss-Lobatto nodes x_j = -cos(pi j/(N-1)), ascending. */
+static void cgl_nodes(int N, real* x) {
+  for (int j = 0; j < N; ++j) x[j] = -R_COS(R_PI * (real)j / (real)(N - 1));
+}
+void ora_cheb_nodes(int N, double* x) {
+  real* t = malloc(sizeof(real) * N); cgl_nodes(N, t);
+  for (int j = 0; j < N; ++j) x[j] = (double)t[j];
+  free(t);
+}
+
+/* Legendre P_n(x) and P_n'(x) by the three-term recurrence. */
+static void legendre(int n, real x, real* p, real* dp) {
+  real p0 = 1, p1 = x;
+  if (n == 0) { *p = 1; *dp = 0; return; }
+  for (int k = 2; k <= n; ++k) { real pk = ((2 * k - 1) * x * p1 - (k - 1) * p0) / k; p0 = p1; p1 = pk; }
+  *p = p1; *dp = n * (x * p1 - p0) / (x * x - 1);
+}
+
+/* Gauss-Legendre: cos(theta_j) = roots of P_{L+1} by Newton, theta ascending;
+ * w_j = 2 / ((1-x_j^2) P'_{L+1}(x_j)^2). */
+static void gl_nodes(int L, real* ct, real* w) {
+  int n = L + 1;
+  for (int j = 0; j < n; ++j) {
+    real x = R_COS(R_PI * ((real)j + 0.75L) / ((real)n + 0.5L)); /* descending in x = ascending in theta */
+    real p, dp;
+    for (int it = 0; it < 100; ++it) { legendre(n, x, &p, &dp); real dx = p / dp; x -= dx; if (R_FABS(dx) < 1e-19L) break; }
+    legendre(n, x, &p, &dp);
+    ct[j] = x; w[j] = 2 / ((1 - x * x) * dp * dp);
+  }
+}
+void ora_gl_nodes(int L, double* theta, double* w) {
+  int n = L + 1; real* c = malloc(sizeof(real) * n); real* ww = malloc(sizeof(real) * n);
+  gl_nodes(L, c, ww);
+  for (int j = 0; j < n; ++j) { theta[j] = (double)R_ACOS(c[j]); w[j] = (double)ww[j]; }
+  free(c); free(ww);
+}
+
+/* Coordinates xyz[3][P]; shells ordered (r slowest, theta, phi fastest), blocks (x,y,z). */
+void ora_coords(const ora_subdomain* sd, double* xyz) {
+  int n0, n1, n2; dims(sd, &n0, &n1, &n2); int64_t P = (int64_t)n0 * n1 * n2;
+  if (sd->kind == 0) {
+    int L = sd->n[1];
+    real* xr = malloc(sizeof(real) * n0); cgl_nodes(n0, xr);
+    real* ct = malloc(sizeof(real) * n1); real* w = malloc(sizeof(real) * n1); gl_nodes(L, ct, w);
+    for (int i = 0; i < n0; ++i) for (int j = 0; j < n1; ++j) for (int k = 0; k < n2; ++k) {
+      real r = (real)sd->lo[0] + ((real)sd->hi[0] - (real)sd->lo[0]) * (xr[i] + 1) / 2;
+      real st = R_SQRT(1 - ct[j] * ct[j]); real ph = 2 * R_PI * (real)k / (real)n2;
+      int64_t p = ((int64_t)i * n1 + j) * n2 + k;
+      xyz[p] = (double)((real)sd->center[0] + r * st * R_COS(ph));
+      xyz[P + p] = (double)((real)sd->center[1] + r * st * R_SIN(ph));
+      xyz[2 * P + p] = (double)((real)sd->center[2] + r * ct[j]);
+    }
+    free(xr); free(ct); free(w);
+  } else {
+    real* x[3]; int nn[3] = {n0, n1, n2};
+    for (int d = 0; d < 3; ++d) { x[d] = malloc(sizeof(real) * nn[d]); cgl_nodes(nn[d], x[d]); }
+    for (int i = 0; i < n0; ++i) for (int j = 0; j < n1; ++j) for (int k = 0; k < n2; ++k) {
+      int64_t p = ((int64_t)i * n1 + j) * n2 + k; int idx[3] = {i, j, k};
+      for (int d = 0; d < 3; ++d)
+        xyz[d * P + p] = (double)((real)sd->lo[d] + ((real)sd->hi[d] - (real)sd->lo[d]) * (x[d][idx[d]] + 1) / 2);
+    }
+    for (int d = 0; d < 3; ++d) free(x[d]);
+  }
+}
+
+/* ---------------------------------------------------------------------- */
+/* O1 — Chebyshev derivative of one line (Eqs. 14-18)   */
+/* ---------------------------------------------------------------------- */
+/* T_k(x_j) = (-1)^k cos(pi j k/(N-1)); argument reduced in integers. */
+static real cheb_T(int N, int k, int j) {
+  int64_t m = ((int64_t)j * k) % (2 * (int64_t)(N - 1));
+  real v = R_COS(R_PI * (real)m / (real)(N - 1));
+  return (k & 1) ? -v : v;
+}
+
+/* u, du have stride `st`; derivative w.r.t. the reference coordinate x in [-1,1]. */
+static void cheb_line(int N, const real* u, int64_t st, real* du, int64_t dst) {
+  real* ut = malloc(sizeof(real) * N); real* dt = malloc(sizeof(real) * (N + 1));
+  /* (a) PhysToSpec, Eq. 17: u~_k = (2/(N-1)) (1/c_k) sum_j (1/c_j) u_j T_k(x_j) */
+  for (int k = 0; k < N; ++k) {
+    real s = 0;
+    for (int j = 0; j < N; ++j) { real cj = (j == 0 || j == N - 1) ? 2 : 1; s += u[j * st] * cheb_T(N, k, j) / cj; }
+    real ck = (k == 0 || k == N - 1) ? 2 : 1;
+    ut[k] = 2 * s / ((real)(N - 1) * ck);
+  }
+  /* (b) modal derivative, Eq. 18, by the downward recurrence
+   *     c_{k-1} u'~_{k-1} = u'~_{k+1} + 2 k u~_k,  c_0 = 2 else 1 */
+  dt[N] = 0; dt[N - 1] = 0;
+  for (int k = N - 1; k >= 1; --k) { real c = (k - 1 == 0) ? 2 : 1; dt[k - 1] = (dt[k + 1] + 2 * (real)k * ut[k]) / c; }
+  /* (c) SpecToPhys, Eq. 16 */
+  for (int j = 0; j < N; ++j) { real s = 0; for (int k = 0; k < N; ++k) s += dt[k] * cheb_T(N, k, j); du[j * dst] = s; }
+  free(ut); free(dt);
+}
+
+void ora_cheb_derivative_line(int N, const double* u, double* du) {
+  real* a = malloc(sizeof(real) * N); real* b = malloc(sizeof(real) * N);
+  for (int j = 0; j < N; ++j) a[j] = u[j];
+  cheb_line(N, a, 1, b, 1);
+  for (int j = 0; j < N; ++j) du[j] = (double)b[j];
+  free(a); free(b);
+}
+
+/* ---------------------------------------------------------------------- */
+/* O2 — shell angular derivatives through Y_lm         */
+/* ---------------------------------------------------------------------- */
+typedef struct {
+  int L, nth, nph;
+  real *ct, *w;        /* cos(theta_j), GL weights */
+  real *pb, *dpb;      /* Pbar_lm(theta_j), dPbar_lm/dtheta: index [(l*(L+1)+m)*nth + j], m<=l */
+  real *cs, *sn;       /* cos(m phi_k), sin(m phi_k): [m*nph + k] */
+} ylm_table;
+
+/* Orthonormalised associated Legendre functions Pbar_lm (so that Y_lm = Pbar_lm e^{i m phi}
+ * is orthonormal on the sphere, Condon-Shortley phase), by the standard recurrences. */
+static void pbar_all(int L, real ct, real* pb, real* dpb) {
+  int n = L + 1; real st = R_SQRT(1 - ct * ct);
+  for (int i = 0; i < n * n; ++i) { pb[i] = 0; dpb[i] = 0; }
+  pb[0] = R_SQRT(1 / (4 * R_PI));
+  for (int m = 1; m <= L; ++m) pb[m * n + m] = -R_SQRT((real)(2 * m + 1) / (real)(2 * m)) * st * pb[(m - 1) * n + (m - 1)];
+  for (int m = 0; m < L; ++m) pb[(m + 1) * n + m] = R_SQRT((real)(2 * m + 3)) * ct * pb[m * n + m];
+  for (int m = 0; m <= L; ++m) for (int l = m + 2; l <= L; ++l) {
+    real a = R_SQRT((real)(4 * l * l - 1) / (real)(l * l - m * m));
+    real b = R_SQRT((real)((l - 1) * (l - 1) - m * m) / (real)(4 * (l - 1) * (l - 1) - 1));
+    pb[l * n + m] = a * (ct * pb[(l - 1) * n + m] - b * pb[(l - 2) * n + m]);
+  }
+  /* sin(theta) dPbar_lm/dtheta = l cos(theta) Pbar_lm - sqrt((2l+1)/(2l-1) (l^2-m^2)) Pbar_{l-1,m} */
+  for (int l = 0; l <= L; ++l) for (int m = 0; m <= l; ++m) {
+    real prev = (l - 1 >= m) ? pb[(l - 1) * n + m] : 0;
+    real f = (l > 0) ? R_SQRT((real)(2 * l + 1) / (real)(2 * l - 1) * (real)(l * l - m * m)) : 0;
+    dpb[l * n + m] = ((real)l * ct * pb[l * n + m] - f * prev) / st;
+  }
+}
+
+static ylm_table* ylm_build(int L) {
+  ylm_table* t = malloc(sizeof(ylm_table));
+  int n = L + 1; t->L = L; t->nth = n; t->nph = 2 * n;
+  t->ct = malloc(sizeof(real) * n); t->w = malloc(sizeof(real) * n); gl_nodes(L, t->ct, t->w);
+  t->pb = malloc(sizeof(real) * n * n * n); t->dpb = malloc(sizeof(real) * n * n * n);
+  real* a = malloc(sizeof(real) * n * n); real* b = malloc(sizeof(real) * n * n);
+  for (int j = 0; j < n; ++j) {
+    pbar_all(L, t->ct[j], a, b);
+    for (int i = 0; i < n * n; ++i) { t->pb[(int64_t)i * n + j] = a[i]; t->dpb[(int64_t)i * n + j] = b[i]; }
+  }
+  free(a); free(b);
+  t->cs = malloc(sizeof(real) * n * t->nph); t->sn = malloc(sizeof(real) * n * t->nph);
+  for (int m = 0; m <= L; ++m) for (int k = 0; k < t->nph; ++k) {
+    int64_t q = ((int64_t)m * k) % t->nph; real ang = 2 * R_PI * (real)q / (real)t->nph;
+    t->cs[m * t->nph + k] = R_COS(ang); t->sn[m * t->nph + k] = R_SIN(ang);
+  }
+  return t;
+}
+static void ylm_free(ylm_table* t) { free(t->ct); free(t->w); free(t->pb); free(t->dpb); free(t->cs); free(t->sn); free(t); }
+
+/* Pbar_lm and dPbar_lm/dtheta at one colatitude, [l*(L+1)+m] (for the pins). */
+void ora_pbar(int L, double theta, double* pb, double* dpb) {
+  int n = L + 1; real* a = malloc(sizeof(real) * n * n); real* b = malloc(sizeof(real) * n * n);
+  pbar_all(L, R_COS((real)theta), a, b);
+  for (int i = 0; i < n * n; ++i) { pb[i] = (double)a[i]; dpb[i] = (double)b[i]; }
+  free(a); free(b);
+}
+
+/* One (theta,phi) plane u[nth][nph] (strides given) -> out0 = d/dtheta, out1 = d/dphi,
+ * or (mode 1) out0 = the projection synthesis(analysis(u)).
+ *   a_lm = sum_{j,k} w_j (2 pi/N_phi) conj(Y_lm(theta_j,phi_k)) u_jk,  0<=l<=L, 0<=m<=l
+ *   real u:  u = sum_l [ a_l0 Y_l0 + 2 Re sum_{m>0} a_lm Y_lm ]  (a_{l,-m} = (-1)^m conj a_lm)
+ *   d_theta u = same with dPbar/dtheta;  d_phi u = same with (i m) a_lm.
+ * Explicit quadruple loops, Eq. 23-24 / SURVEY O2; both derivatives go through a_lm (S8). */
+static void shell_plane(const ylm_table* t, const real* u, real* out0, real* out1, int mode) {
+  int L = t->L, n = t->nth, nph = t->nph;
+  real* are = calloc((size_t)n * n, sizeof(real)); real* aim = calloc((size_t)n * n, sizeof(real));
+  real dphi = 2 * R_PI / (real)nph;
+  for (int l = 0; l <= L; ++l) for (int m = 0; m <= l; ++m) {
+    real sr = 0, si = 0; const real* pb = t->pb + (int64_t)(l * n + m) * n;
+    for (int j = 0; j < n; ++j) for (int k = 0; k < nph; ++k) {
+      real f = t->w[j] * dphi * pb[j] * u[j * nph + k];
+      sr += f * t->cs[m * nph + k]; si -= f * t->sn[m * nph + k];
+    }
+    are[l * n + m] = sr; aim[l * n + m] = si;
+  }
+  for (int j = 0; j < n; ++j) for (int k = 0; k < nph; ++k) {
+    real s0 = 0, s1 = 0;
+    for (int l = 0; l <= L; ++l) for (int m = 0; m <= l; ++m) {
+      real fac = (m == 0) ? 1 : 2; real ar = are[l * n + m], ai = aim[l * n + m];
+      real c = t->cs[m * nph + k], s = t->sn[m * nph + k];
+      real re = ar * c - ai * s;            /* Re(a e^{i m phi}) */
+      real im = ar * s + ai * c;            /* Im(a e^{i m phi}) */
+      if (mode == 0) {
+        s0 += fac * t->dpb[(int64_t)(l * n + m) * n + j] * re;
+        s1 += fac * t->pb[(int64_t)(l * n + m) * n + j] * (-(real)m * im);   /* Re(i m a e^{i m phi}) */
+      } else {
+        s0 += fac * t->pb[(int64_t)(l * n + m) * n + j] * re;
+      }
+    }
+    out0[j * nph + k] = s0; if (mode == 0) out1[j * nph + k] = s1;
+  }
+  free(are); free(aim);
+}
+
+void ora_shell_angular(int L, const double* u, double* dth, double* dph) {
+  ylm_table* t = ylm_build(L); int np = t->nth * t->nph;
+  real* a = malloc(sizeof(real) * np); real* b = malloc(sizeof(real) * np); real* c = malloc(sizeof(real) * np);
+  for (int i = 0; i < np; ++i) a[i] = u[i];
+  shell_plane(t, a, b, c, 0);
+  for (int i = 0; i < np; ++i) { dth[i] = (double)b[i]; dph[i] = (double)c[i]; }
+  free(a); free(b); free(c); ylm_free(t);
+}
+void ora_shell_project(int L, const double* u, double* out) {
+  ylm_table* t = ylm_build(L); int np = t->nth * t->nph;
+  real* a = malloc(sizeof(real) * np); real* b = malloc(sizeof(real) * np);
+  for (int i = 0; i < np; ++i) a[i] = u[i];
+  shell_plane(t, a, b, NULL, 1);
+  for (int i = 0; i < np; ++i) out[i] = (double)b[i];
+  free(a); free(b); ylm_free(t);
+}
+
+/* ---------------------------------------------------------------------- */
+/* O3 — Cartesian gradient of ncomp scalar fields on one subdomain        */
+/* ---------------------------------------------------------------------- */
+/* u[ncomp][P] (real) -> g[3][ncomp][P] = d/dx, d/dy, d/dz. */
+static void gradient_real(const ora_subdomain* sd, int ncomp, const real* u, real* g) {
+  int n0, n1, n2; dims(sd, &n0, &n1, &n2); int64_t P = (int64_t)n0 * n1 * n2;
+  if (sd->kind == 1) {
+    /* blocks: O1 along x, y, z with the affine map factor 2/(hi-lo) (Eq. 22) */
+    int nn[3] = {n0, n1, n2}; int64_t st[3] = {(int64_t)n1 * n2, n2, 1};
+#pragma omp parallel for schedule(dynamic)
+    for (int c = 0; c < ncomp; ++c) for (int d = 0; d < 3; ++d) {
+      real sc = 2 / ((real)sd->hi[d] - (real)sd->lo[d]);
+      int e = (d + 1) % 3, f = (d + 2) % 3;
+      for (int a = 0; a < nn[e]; ++a) for (int b = 0; b < nn[f]; ++b) {
+        int64_t off = a * st[e] + b * st[f];
+        real* out = g + ((int64_t)d * ncomp + c) * P + off;
+        cheb_line(nn[d], u + (int64_t)c * P + off, st[d], out, st[d]);
+        for (int i = 0; i < nn[d]; ++i) out[i * st[d]] *= sc;
+      }
+    }
+    return;
+  }
+  /* shells: O1 in r, O2 in (theta,phi), then Eq. 8 with the spherical Jacobian */
+  int L = sd->n[1]; ylm_table* t = ylm_build(L); int64_t np = (int64_t)n1 * n2;
+  real* xr = malloc(sizeof(real) * n0); cgl_nodes(n0, xr);
+  real sc = 2 / ((real)sd->hi[0] - (real)sd->lo[0]);
+#pragma omp parallel for schedule(dynamic)
+  for (int c = 0; c < ncomp; ++c) {
+    const real* uc = u + (int64_t)c * P;
+    real* dr = malloc(sizeof(real) * P); real* dth = malloc(sizeof(real) * P); real* dph = malloc(sizeof(real) * P);
+    for (int64_t q = 0; q < np; ++q) { cheb_line(n0, uc + q, np, dr + q, np); }
+    for (int64_t p = 0; p < P; ++p) dr[p] *= sc;
+    for (int i = 0; i < n0; ++i) shell_plane(t, uc + i * np, dth + i * np, dph + i * np, 0);
+    for (int i = 0; i < n0; ++i) {
+      real r = (real)sd->lo[0] + ((real)sd->hi[0] - (real)sd->lo[0]) * (xr[i] + 1) / 2;
+      for (int j = 0; j < n1; ++j) for (int k = 0; k < n2; ++k) {
+        real ct = t->ct[j], st = R_SQRT(1 - ct * ct); real ph = 2 * R_PI * (real)k / (real)n2;
+        real cp = R_COS(ph), sp = R_SIN(ph); int64_t p = i * np + (int64_t)j * n2 + k;
+        real a = dr[p], b = dth[p], e = dph[p];
+        g[((int64_t)0 * ncomp + c) * P + p] = st * cp * a + (ct * cp / r) * b - (sp / (r * st)) * e;
+        g[((int64_t)1 * ncomp + c) * P + p] = st * sp * a + (ct * sp / r) * b + (cp / (r * st)) * e;
+        g[((int64_t)2 * ncomp + c) * P + p] = ct * a - (st / r) * b;
+      }
+    }
+    free(dr); free(dth); free(dph);
+  }
+  free(xr); ylm_free(t);
+}
+
+void ora_gradient(const ora_subdomain* sd, int ncomp, const double* u, double* g) {
+  int64_t P = ora_num_points(sd);
+  real* a = malloc(sizeof(real) * ncomp * P); real* b = malloc(sizeof(real) * 3 * ncomp * P);
+  for (int64_t i = 0; i < ncomp * P; ++i) a[i] = u[i];
+  gradient_real(sd, ncomp, a, b);
+  for (int64_t i = 0; i < 3 * ncomp * P; ++i) g[i] = (double)b[i];
+  free(a); free(b);
+}
+
+/* ---------------------------------------------------------------------- */
+/* O4 — geometry at a point                                               */
+/* ---------------------------------------------------------------------- */
+typedef struct { real ginv[3][3], lapse, shift[3], psiinv[4][4], tup[4], tdn[4]; } geom;
+
+static int geometry(const real psi[4][4], geom* G) {
+  real g[3][3]; for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) g[i][j] = psi[i + 1][j + 1];
+  real c00 = g[1][1] * g[2][2] - g[1][2] * g[2][1], c01 = g[1][2] * g[2][0] - g[1][0] * g[2][2], c02 = g[1][0] * g[2][1] - g[1][1] * g[2][0];
+  real det = g[0][0] * c00 + g[0][1] * c01 + g[0][2] * c02;
+  if (!(det > 0)) return 1;
+  /* g^{ij} = cofactor(j,i)/det */
+  G->ginv[0][0] = c00 / det; G->ginv[1][0] = c01 / det; G->ginv[2][0] = c02 / det;
+  G->ginv[0][1] = (g[0][2] * g[2][1] - g[0][1] * g[2][2]) / det;
+  G->ginv[1][1] = (g[0][0] * g[2][2] - g[0][2] * g[2][0]) / det;
+  G->ginv[2][1] = (g[0][1] * g[2][0] - g[0][0] * g[2][1]) / det;
+  G->ginv[0][2] = (g[0][1] * g[1][2] - g[0][2] * g[1][1]) / det;
+  G->ginv[1][2] = (g[0][2] * g[1][0] - g[0][0] * g[1][2]) / det;
+  G->ginv[2][2] = (g[0][0] * g[1][1] - g[0][1] * g[1][0]) / det;
+  real n2 = -psi[0][0];
+  for (int i = 0; i < 3; ++i) { real s = 0; for (int j = 0; j < 3; ++j) s += G->ginv[i][j] * psi[0][j + 1]; G->shift[i] = s; }
+  for (int i = 0; i < 3; ++i) n2 += G->shift[i] * psi[0][i + 1];
+  if (!(n2 > 0)) return 1;
+  G->lapse = R_SQRT(n2);
+  G->psiinv[0][0] = -1 / n2;
+  for (int i = 0; i < 3; ++i) { G->psiinv[0][i + 1] = G->shift[i] / n2; G->psiinv[i + 1][0] = G->shift[i] / n2; }
+  for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) G->psiinv[i + 1][j + 1] = G->ginv[i][j] - G->shift[i] * G->shift[j] / n2;
+  G->tup[0] = 1 / G->lapse; for (int i = 0; i < 3; ++i) G->tup[i + 1] = -G->shift[i] / G->lapse;
+  G->tdn[0] = -G->lapse; G->tdn[1] = G->tdn[2] = G->tdn[3] = 0;
+  return 0;
+}
+
+/* psi[16] -> ginv[9], lapse, shift[3], psiinv[16]; returns 1 if non-physical. */
+int ora_geometry_point(const double* psi, double* ginv, double* lapse, double* shift, double* psiinv) {
+  real p[4][4]; geom G; for (int a = 0; a < 4; ++a) for (int b = 0; b < 4; ++b) p[a][b] = psi[a * 4 + b];
+  if (geometry(p, &G)) return 1;
+  for (int i = 0; i < 3; ++i) { shift[i] = (double)G.shift[i]; for (int j = 0; j < 3; ++j) ginv[i * 3 + j] = (double)G.ginv[i][j]; }
+  *lapse = (double)G.lapse;
+  for (int a = 0; a < 4; ++a) for (int b = 0; b < 4; ++b) psiinv[a * 4 + b] = (double)G.psiinv[a][b];
+  return 0;
+}
+
+/* ---------------------------------------------------------------------- */
+/* O5 — GH right-hand side at a point; O8 — constraints at a point        */
+/* ---------------------------------------------------------------------- */
+typedef struct {
+  real psi[4][4], Pi[4][4], Phi[3][4][4];
+  real dpsi[3][4][4], dPi[3][4][4], dPhi[3][3][4][4]; /* spectral d_k: dPhi[k][i][a][b] = d_k Phi_iab */
+  real H[4], dH[3][4];                                /* dH[i][b] = d_i H_b ; d_0 H_b = 0 */
+} point_in;
+
+/* Christoffels of the first kind from the FIRST-ORDER variables:
+ * d_0 psi = -N Pi + N^i Phi_i, d_i psi = Phi_i (SURVEY O5 "two meanings of d psi"). */
+static void christoffel(const point_in* in, const geom* G, real Gam[4][4][4], real Gam1[4]) {
+  real D[4][4][4];
+  for (int a = 0; a < 4; ++a) for (int b = 0; b < 4; ++b) {
+    real s = -G->lapse * in->Pi[a][b];
+    for (int i = 0; i < 3; ++i) s += G->shift[i] * in->Phi[i][a][b];
+    D[0][a][b] = s;
+    for (int i = 0; i < 3; ++i) D[i + 1][a][b] = in->Phi[i][a][b];
+  }
+  for (int a = 0; a < 4; ++a) for (int b = 0; b < 4; ++b) for (int c = 0; c < 4; ++c)
+    Gam[a][b][c] = (D[b][a][c] + D[c][a][b] - D[a][b][c]) / 2;
+  for (int a = 0; a < 4; ++a) { real s = 0; for (int b = 0; b < 4; ++b) for (int c = 0; c < 4; ++c) s += G->psiinv[b][c] * Gam[a][b][c]; Gam1[a] = s; }
+}
+
+static int rhs_point(const point_in* in, const real gam[3], real dtpsi[4][4], real dtPi[4][4], real dtPhi[3][4][4]) {
+  geom G; if (geometry(in->psi, &G)) return 1;
+  real g0 = gam[0], g1 = gam[1], g2 = gam[2], N = G.lapse;
+  real Gam[4][4][4], Gam1[4], C[4]; christoffel(in, &G, Gam, Gam1);
+  for (int a = 0; a < 4; ++a) C[a] = in->H[a] + Gam1[a];
+  real dH4[4][4]; for (int b = 0; b < 4; ++b) { dH4[0][b] = 0; for (int i = 0; i < 3; ++i) dH4[i + 1][b] = in->dH[i][b]; }
+  real tC = 0; for (int c = 0; c < 4; ++c) tC += G.tup[c] * C[c];
+  real ttPi = 0; for (int c = 0; c < 4; ++c) for (int d = 0; d < 4; ++d) ttPi += G.tup[c] * G.tup[d] * in->Pi[c][d];
+  for (int a = 0; a < 4; ++a) for (int b = 0; b < 4; ++b) {
+    real sdpsi = 0, sPhi = 0, sdPi = 0;
+    for (int k = 0; k < 3; ++k) { sdpsi += G.shift[k] * in->dpsi[k][a][b]; sPhi += G.shift[k] * in->Phi[k][a][b]; sdPi += G.shift[k] * in->dPi[k][a][b]; }
+    dtpsi[a][b] = (1 + g1) * sdpsi - N * in->Pi[a][b] - g1 * sPhi;
+    real gdPhi = 0; for (int k = 0; k < 3; ++k) for (int i = 0; i < 3; ++i) gdPhi += G.ginv[k][i] * in->dPhi[k][i][a][b];
+    real quad = 0;
+    for (int c = 0; c < 4; ++c) for (int d = 0; d < 4; ++d) {
+      real t = 0;
+      for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) t += G.ginv[i][j] * in->Phi[i][c][a] * in->Phi[j][d][b];
+      t -= in->Pi[c][a] * in->Pi[d][b];
+      for (int e = 0; e < 4; ++e) for (int f = 0; f < 4; ++f) t -= G.psiinv[e][f] * Gam[a][c][e] * Gam[b][d][f];
+      quad += G.psiinv[c][d] * t;
+    }
+    real nabH = (dH4[a][b] + dH4[b][a]) / 2;
+    for (int c = 0; c < 4; ++c) for (int d = 0; d < 4; ++d) nabH -= G.psiinv[c][d] * Gam[d][a][b] * in->H[c];
+    real tPigPhi = 0;
+    for (int c = 0; c < 4; ++c) for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) tPigPhi += G.tup[c] * in->Pi[c][i + 1] * G.ginv[i][j] * in->Phi[j][a][b];
+    dtPi[a][b] = sdPi - N * gdPhi + g1 * g2 * sdpsi + 2 * N * quad - 2 * N * nabH - N * ttPi * in->Pi[a][b] / 2 - N * tPigPhi
+               + N * g0 * (G.tdn[b] * C[a] + G.tdn[a] * C[b] - in->psi[a][b] * tC) - g1 * g2 * sPhi;
+    for (int i = 0; i < 3; ++i) {
+      real sdPhi = 0; for (int k = 0; k < 3; ++k) sdPhi += G.shift[k] * in->dPhi[k][i][a][b];
+      real ttPhi = 0; for (int c = 0; c < 4; ++c) for (int d = 0; d < 4; ++d) ttPhi += G.tup[c] * G.tup[d] * in->Phi[i][c][d];
+      real gtPP = 0;
+      for (int j = 0; j < 3; ++j) for (int k = 0; k < 3; ++k) for (int c = 0; c < 4; ++c) gtPP += G.ginv[j][k] * G.tup[c] * in->Phi[i][j + 1][c] * in->Phi[k][a][b];
+      dtPhi[i][a][b] = sdPhi - N * in->dPi[i][a][b] + N * g2 * in->dpsi[i][a][b] + N * ttPhi * in->Pi[a][b] / 2 + N * gtPP - N * g2 * in->Phi[i][a][b];
+    }
+  }
+  return 0;
+}
+
+/* C_a[4], C_iab[3][4][4], C_ijab[3][3][4][4] */
+static int constraints_point(const point_in* in, real Ca[4], real Ciab[3][4][4], real Cijab[3][3][4][4]) {
+  geom G; if (geometry(in->psi, &G)) return 1;
+  real Gam[4][4][4], Gam1[4]; christoffel(in, &G, Gam, Gam1);
+  for (int a = 0; a < 4; ++a) Ca[a] = in->H[a] + Gam1[a];
+  for (int i = 0; i < 3; ++i) for (int a = 0; a < 4; ++a) for (int b = 0; b < 4; ++b) Ciab[i][a][b] = in->dpsi[i][a][b] - in->Phi[i][a][b];
+  for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) for (int a = 0; a < 4; ++a) for (int b = 0; b < 4; ++b)
+    Cijab[i][j][a][b] = in->dPhi[i][j][a][b] - in->dPhi[j][i][a][b];
+  return 0;
+}
+
+/* Flat double interface to one point, FULL (unsymmetrised) arrays, row-major:
+ * psi[16], Pi[16], Phi[48], dpsi[48], dPi[48], dPhi[144] ([k][i][a][b]), H[4], dH[12] ([i][b]). */
+static void load_point(point_in* in, const double* psi, const double* Pi, const double* Phi, const double* dpsi,
+                       const double* dPi, const double* dPhi, const double* H, const double* dH) {
+  for (int a = 0; a < 4; ++a) for (int b = 0; b < 4; ++b) { in->psi[a][b] = psi[a * 4 + b]; in->Pi[a][b] = Pi[a * 4 + b]; }
+  for (int i = 0; i < 3; ++i) for (int a = 0; a < 4; ++a) for (int b = 0; b < 4; ++b) {
+    in->Phi[i][a][b] = Phi[(i * 4 + a) * 4 + b]; in->dpsi[i][a][b] = dpsi[(i * 4 + a) * 4 + b]; in->dPi[i][a][b] = dPi[(i * 4 + a) * 4 + b];
+    for (int k = 0; k < 3; ++k) in->dPhi[k][i][a][b] = dPhi[((k * 3 + i) * 4 + a) * 4 + b];
+  }
+  for (int a = 0; a < 4; ++a) in->H[a] = H[a];
+  for (int i = 0; i < 3; ++i) for (int b = 0; b < 4; ++b) in->dH[i][b] = dH[i * 4 + b];
+}
+
+int ora_rhs_point(const double* psi, const double* Pi, const double* Phi, const double* dpsi, const double* dPi,
+                  const double* dPhi, const double* H, const double* dH, const double* gamma,
+                  double* dtpsi, double* dtPi, double* dtPhi) {
+  point_in in; load_point(&in, psi, Pi, Phi, dpsi, dPi, dPhi, H, dH);
+  real g[3] = {gamma[0], gamma[1], gamma[2]}, a[4][4], b[4][4], c[3][4][4];
+  if (rhs_point(&in, g, a, b, c)) return 1;
+  for (int x = 0; x < 4; ++x) for (int y = 0; y < 4; ++y) { dtpsi[x * 4 + y] = (double)a[x][y]; dtPi[x * 4 + y] = (double)b[x][y];
+    for (int i = 0; i < 3; ++i) dtPhi[(i * 4 + x) * 4 + y] = (double)c[i][x][y]; }
+  return 0;
+}
+
+int ora_constraints_point(const double* psi, const double* Pi, const double* Phi, const double* dpsi, const double* dPhi,
+                          const double* H, double* Ca, double* Ciab, double* Cijab) {
+  static const double z48[48] = {0}, z12[12] = {0};
+  point_in in; load_point(&in, psi, Pi, Phi, dpsi, z48, dPhi, H, z12);
+  real a[4], b[3][4][4], c[3][3][4][4];
+  if (constraints_point(&in, a, b, c)) return 1;
+  for (int x = 0; x < 4; ++x) Ca[x] = (double)a[x];
+  for (int i = 0; i < 3; ++i) for (int x = 0; x < 4; ++x) for (int y = 0; y < 4; ++y) { Ciab[(i * 4 + x) * 4 + y] = (double)b[i][x][y];
+    for (int j = 0; j < 3; ++j) Cijab[((i * 3 + j) * 4 + x) * 4 + y] = (double)c[i][j][x][y]; }
+  return 0;
+}
+
+/* ---------------------------------------------------------------------- */
+/* subdomain level: storage is the packed 50-component order              */
+/*   s(a,b), a<=b: 00,01,02,03,11,12,13,22,23,33 -> 0..9                  */
+/*   psi: c=s; Pi: c=10+s; Phi_iab: c=20+10 i+s                           */
+/* (the oracle unpacks to FULL arrays before doing any tensor algebra)    */
+/* ---------------------------------------------------------------------- */
+static const int SYM[4][4] = {{0, 1, 2, 3}, {1, 4, 5, 6}, {2, 5, 7, 8}, {3, 6, 8, 9}};
+
+static void fill_point(point_in* in, const real* u, const real* g, const real* H, const real* gH, int64_t P, int64_t p) {
+  for (int a = 0; a < 4; ++a) for (int b = 0; b < 4; ++b) {
+    int s = SYM[a][b];
+    in->psi[a][b] = u[(int64_t)s * P + p]; in->Pi[a][b] = u[(int64_t)(10 + s) * P + p];
+    for (int i = 0; i < 3; ++i) in->Phi[i][a][b] = u[(int64_t)(20 + 10 * i + s) * P + p];
+    for (int k = 0; k < 3; ++k) {
+      in->dpsi[k][a][b] = g[((int64_t)k * 50 + s) * P + p]; in->dPi[k][a][b] = g[((int64_t)k * 50 + 10 + s) * P + p];
+      for (int i = 0; i < 3; ++i) in->dPhi[k][i][a][b] = g[((int64_t)k * 50 + 20 + 10 * i + s) * P + p];
+    }
+  }
+  for (int a = 0; a < 4; ++a) { in->H[a] = H[(int64_t)a * P + p]; for (int i = 0; i < 3; ++i) in->dH[i][a] = gH[((int64_t)i * 4 + a) * P + p]; }
+}
+
+/* O6: is point p on a FROZEN face? */
+static int frozen(const ora_subdomain* sd, int64_t p) {
+  int n0, n1, n2; dims(sd, &n0, &n1, &n2);
+  int k = (int)(p % n2), j = (int)((p / n2) % n1), i = (int)(p / ((int64_t)n1 * n2));
+  if (sd->kind == 0) return (i == 0 && sd->face[0] == 1) || (i == n0 - 1 && sd->face[1] == 1);
+  return (i == 0 && sd->face[0] == 1) || (i == n0 - 1 && sd->face[1] == 1) || (j == 0 && sd->face[2] == 1) ||
+         (j == n1 - 1 && sd->face[3] == 1) || (k == 0 && sd->face[4] == 1) || (k == n2 - 1 && sd->face[5] == 1);
+}
+
+/* real-typed core: u[50][P], H[4][P], gH[12][P] ([i][a]) -> dtu[50][P]. Returns #non-physical points. */
+static int rhs_real(const ora_subdomain* sd, const real* u, const real* H, const real* gH, real* dtu) {
+  int64_t P = ora_num_points(sd);
+  real* g = malloc(sizeof(real) * 150 * P);
+  gradient_real(sd, 50, u, g);
+  real gam[3] = {sd->gamma[0], sd->gamma[1], sd->gamma[2]};
+  int bad = 0;
+#pragma omp parallel for schedule(static) reduction(+ : bad)
+  for (int64_t p = 0; p < P; ++p) {
+    point_in in; fill_point(&in, u, g, H, gH, P, p);
+    real a[4][4], b[4][4], c[3][4][4];
+    if (rhs_point(&in, gam, a, b, c)) { bad += 1; memset(a, 0, sizeof a); memset(b, 0, sizeof b); memset(c, 0, sizeof c); }
+    int fz = frozen(sd, p);
+    for (int x = 0; x < 4; ++x) for (int y = x; y < 4; ++y) {
+      int s = SYM[x][y];
+      dtu[(int64_t)s * P + p] = fz ? 0 : a[x][y]; dtu[(int64_t)(10 + s) * P + p] = fz ? 0 : b[x][y];
+      for (int i = 0; i < 3; ++i) dtu[(int64_t)(20 + 10 * i + s) * P + p] = fz ? 0 : c[i][x][y];
+    }
+  }
+  free(g);
+  return bad;
+}
+
+/* Full-array (16+16+48) RHS output, for the symmetry pin: out[80][P] = dtpsi[16], dtPi[16], dtPhi[48]. */
+int ora_rhs_subdomain_full(const ora_subdomain* sd, const double* u, const double* H, const double* dH, double* out) {
+  int64_t P = ora_num_points(sd);
+  real* ur = malloc(sizeof(real) * 50 * P); real* Hr = malloc(sizeof(real) * 4 * P); real* gH = malloc(sizeof(real) * 12 * P);
+  for (int64_t i = 0; i < 50 * P; ++i) ur[i] = u[i];
+  for (int64_t i = 0; i < 4 * P; ++i) Hr[i] = H[i];
+  if (dH) for (int64_t i = 0; i < 12 * P; ++i) gH[i] = dH[i]; else gradient_real(sd, 4, Hr, gH);
+  real* g = malloc(sizeof(real) * 150 * P); gradient_real(sd, 50, ur, g);
+  real gam[3] = {sd->gamma[0], sd->gamma[1], sd->gamma[2]}; int bad = 0;
+  for (int64_t p = 0; p < P; ++p) {
+    point_in in; fill_point(&in, ur, g, Hr, gH, P, p); real a[4][4], b[4][4], c[3][4][4];
+    if (rhs_point(&in, gam, a, b, c)) { bad++; continue; }
+    for (int x = 0; x < 4; ++x) for (int y = 0; y < 4; ++y) { out[(int64_t)(x * 4 + y) * P + p] = (double)a[x][y]; out[(int64_t)(16 + x * 4 + y) * P + p] = (double)b[x][y];
+      for (int i = 0; i < 3; ++i) out[(int64_t)(32 + (i * 4 + x) * 4 + y) * P + p] = (double)c[i][x][y]; }
+  }
+  free(ur); free(Hr); free(gH); free(g); return bad;
+}
+
+/* u[50][P], H[4][P], dH[12][P] or NULL (then d_i H_a = O3 applied to H_a) -> dtu[50][P] */
+int ora_rhs_subdomain(const ora_subdomain* sd, const double* u, const double* H, const double* dH, double* dtu) {
+  int64_t P = ora_num_points(sd);
+  real* ur = malloc(sizeof(real) * 50 * P); real* Hr = malloc(sizeof(real) * 4 * P); real* gH = malloc(sizeof(real) * 12 * P);
+  real* out = malloc(sizeof(real) * 50 * P);
+  for (int64_t i = 0; i < 50 * P; ++i) ur[i] = u[i];
+  for (int64_t i = 0; i < 4 * P; ++i) Hr[i] = H[i];
+  if (dH) for (int64_t i = 0; i < 12 * P; ++i) gH[i] = dH[i]; else gradient_real(sd, 4, Hr, gH);
+  int bad = rhs_real(sd, ur, Hr, gH, out);
+  for (int64_t i = 0; i < 50 * P; ++i) dtu[i] = (double)out[i];
+  free(ur); free(Hr); free(gH); free(out);
+  return bad;
+}
+
+/* O7 — nsteps of Shu-Osher SSP-RK3, state kept in `real` across steps:
+ *   u1 = u0 + dt k(u0); u2 = 3/4 u0 + 1/4 (u1 + dt k(u1)); u_new = 1/3 u0 + 2/3 (u2 + dt k(u2)) */
+int ora_rk3_subdomain(const ora_subdomain* sd, double* u, const double* H, const double* dH, double dt, int nsteps) {
+  int64_t P = ora_num_points(sd), n = 50 * P;
+  real* u0 = malloc(sizeof(real) * n); real* us = malloc(sizeof(real) * n); real* k = malloc(sizeof(real) * n);
+  real* Hr = malloc(sizeof(real) * 4 * P); real* gH = malloc(sizeof(real) * 12 * P);
+  for (int64_t i = 0; i < n; ++i) u0[i] = u[i];
+  for (int64_t i = 0; i < 4 * P; ++i) Hr[i] = H[i];
+  if (dH) for (int64_t i = 0; i < 12 * P; ++i) gH[i] = dH[i]; else gradient_real(sd, 4, Hr, gH);
+  real h = dt; int bad = 0;
+  for (int s = 0; s < nsteps; ++s) {
+    bad += rhs_real(sd, u0, Hr, gH, k);
+    for (int64_t i = 0; i < n; ++i) us[i] = u0[i] + h * k[i];
+    bad += rhs_real(sd, us, Hr, gH, k);
+    for (int64_t i = 0; i < n; ++i) us[i] = (3 * u0[i] + (us[i] + h * k[i])) / 4;
+    bad += rhs_real(sd, us, Hr, gH, k);
+    for (int64_t i = 0; i < n; ++i) u0[i] = (u0[i] + 2 * (us[i] + h * k[i])) / 3;
+  }
+  for (int64_t i = 0; i < n; ++i) u[i] = (double)u0[i];
+  free(u0); free(us); free(k); free(Hr); free(gH);
+  return bad;
+}
+
+/* O8 — constraints on one subdomain.
+ * sums[3] = sum of squares over points and UNIQUE components of C_a (4), C_iab (30: a<=b),
+ * C_ijab (30: i<j, a<=b); maxs[3] = max |.|.  Optional per-point fields Cfield[64][P]:
+ * rows 0..3 C_a; 4+10 i+s C_iab; 34+10 q+s C_ijab with q = 0,1,2 for (i,j) = (0,1),(0,2),(1,2).
+ * Domain norms: rms = sqrt(sum_over_subdomains(sums)/(P_total n_comp)). */
+int ora_constraints_subdomain(const ora_subdomain* sd, const double* u, const double* H, double* sums, double* maxs, double* Cfield) {
+  int64_t P = ora_num_points(sd);
+  real* ur = malloc(sizeof(real) * 50 * P); real* Hr = malloc(sizeof(real) * 4 * P); real* gH = calloc(12 * P, sizeof(real));
+  for (int64_t i = 0; i < 50 * P; ++i) ur[i] = u[i];
+  for (int64_t i = 0; i < 4 * P; ++i) Hr[i] = H[i];
+  real* g = malloc(sizeof(real) * 150 * P); gradient_real(sd, 50, ur, g);
+  real S[3] = {0, 0, 0}, M[3] = {0, 0, 0}; int bad = 0;
+  static const int PI_[3] = {0, 0, 1}, PJ_[3] = {1, 2, 2};
+  for (int64_t p = 0; p < P; ++p) {
+    point_in in; fill_point(&in, ur, g, Hr, gH, P, p); real a[4], b[3][4][4], c[3][3][4][4];
+    if (constraints_point(&in, a, b, c)) { bad++; continue; }
+    for (int x = 0; x < 4; ++x) { S[0] += a[x] * a[x]; if (R_FABS(a[x]) > M[0]) M[0] = R_FABS(a[x]); if (Cfield) Cfield[(int64_t)x * P + p] = (double)a[x]; }
+    for (int x = 0; x < 4; ++x) for (int y = x; y < 4; ++y) {
+      int s = SYM[x][y];
+      for (int i = 0; i < 3; ++i) { real v = b[i][x][y]; S[1] += v * v; if (R_FABS(v) > M[1]) M[1] = R_FABS(v); if (Cfield) Cfield[(int64_t)(4 + 10 * i + s) * P + p] = (double)v; }
+      for (int q = 0; q < 3; ++q) { real v = c[PI_[q]][PJ_[q]][x][y]; S[2] += v * v; if (R_FABS(v) > M[2]) M[2] = R_FABS(v); if (Cfield) Cfield[(int64_t)(34 + 10 * q + s) * P + p] = (double)v; }
+    }
+  }
+  for (int q = 0; q < 3; ++q) { sums[q] = (double)S[q]; maxs[q] = (double)M[q]; }
+  free(ur); free(Hr); free(gH); free(g);
+  return bad;
+}

@@ -1,0 +1,254 @@
+"""ctypes front end of the CPU oracle (oracle/gh_oracle.c).  TEST INFRASTRUCTURE.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+legs may import this.  It imports nothing from paper_1804_09101_b200.
+
+Two builds of the same C source: ``real = long double`` (parity; default) and
+``real = double`` (``precision="double"``, the timed CPU baseline).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+import threading
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "gh_oracle.c")
+_LOCK = threading.Lock()
+
+
+def build(force: bool = False) -> dict:
+    """Compile liboracle_ld.so (long double) and liboracle_d.so (double) with gcc."""
+    out = {}
+    for tag, flags in (("ld", []), ("d", ["-DORA_DOUBLE"])):
+        so = os.path.join(_HERE, f"liboracle_{tag}.so")
+        if force or not os.path.exists(so) or os.path.getmtime(so) < os.path.getmtime(_SRC):
+            tmp = so + f".tmp{os.getpid()}"
+            cmd = ["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-fopenmp", "-fno-fast-math", *flags, _SRC, "-o", tmp, "-lm"]
+            subprocess.run(cmd, check=True)
+            os.replace(tmp, so)
+        out[tag] = so
+    return out
+
+
+class Subdomain(C.Structure):
+    _fields_ = [
+        ("kind", C.c_int32),
+        ("n", C.c_int32 * 3),
+        ("lo", C.c_double * 3),
+        ("hi", C.c_double * 3),
+        ("center", C.c_double * 3),
+        ("face", C.c_int32 * 6),
+        ("gamma", C.c_double * 3),
+    ]
+
+
+def make_subdomain(d: dict) -> Subdomain:
+    """d: {'kind': 'shell'|'block', 'n': [..], 'lo': [..], 'hi': [..], 'center': [..], 'face': [..], 'gamma': [..]}"""
+    s = Subdomain()
+    s.kind = 0 if d["kind"] == "shell" else 1
+    n = list(d["n"]) + [0] * (3 - len(d["n"]))
+    lo = list(d["lo"]) + [0.0] * (3 - len(d["lo"]))
+    hi = list(d["hi"]) + [0.0] * (3 - len(d["hi"]))
+    face = list(d.get("face", [])) + [0] * (6 - len(d.get("face", [])))
+    for i in range(3):
+        s.n[i] = int(n[i])
+        s.lo[i] = float(lo[i])
+        s.hi[i] = float(hi[i])
+        s.center[i] = float(d.get("center", [0, 0, 0])[i])
+        s.gamma[i] = float(d.get("gamma", [1.0, -1.0, 1.0])[i])
+    for i in range(6):
+        s.face[i] = int(face[i])
+    return s
+
+
+_dp = np.ctypeslib.ndpointer(dtype=np.float64, flags="C_CONTIGUOUS")
+
+
+class Oracle:
+    def __init__(self, precision: str = "long double", threads: int | None = None):
+        with _LOCK:
+            libs = build()
+        self.precision = precision
+        self.lib = C.CDLL(libs["ld" if precision == "long double" else "d"])
+        L = self.lib
+        L.ora_real_bytes.restype = C.c_int
+        L.ora_num_points.restype = C.c_int64
+        L.ora_num_points.argtypes = [C.POINTER(Subdomain)]
+        L.ora_cheb_nodes.argtypes = [C.c_int, _dp]
+        L.ora_gl_nodes.argtypes = [C.c_int, _dp, _dp]
+        L.ora_coords.argtypes = [C.POINTER(Subdomain), _dp]
+        L.ora_cheb_derivative_line.argtypes = [C.c_int, _dp, _dp]
+        L.ora_pbar.argtypes = [C.c_int, C.c_double, _dp, _dp]
+        L.ora_shell_angular.argtypes = [C.c_int, _dp, _dp, _dp]
+        L.ora_shell_project.argtypes = [C.c_int, _dp, _dp]
+        L.ora_gradient.argtypes = [C.POINTER(Subdomain), C.c_int, _dp, _dp]
+        L.ora_geometry_point.argtypes = [_dp, _dp, _dp, _dp, _dp]
+        L.ora_geometry_point.restype = C.c_int
+        L.ora_rhs_point.argtypes = [_dp] * 12
+        L.ora_rhs_point.restype = C.c_int
+        L.ora_constraints_point.argtypes = [_dp] * 9
+        L.ora_constraints_point.restype = C.c_int
+        L.ora_rhs_subdomain.argtypes = [C.POINTER(Subdomain), _dp, _dp, C.c_void_p, _dp]
+        L.ora_rhs_subdomain.restype = C.c_int
+        L.ora_rhs_subdomain_full.argtypes = [C.POINTER(Subdomain), _dp, _dp, C.c_void_p, _dp]
+        L.ora_rhs_subdomain_full.restype = C.c_int
+        L.ora_rk3_subdomain.argtypes = [C.POINTER(Subdomain), _dp, _dp, C.c_void_p, C.c_double, C.c_int]
+        L.ora_rk3_subdomain.restype = C.c_int
+        L.ora_constraints_subdomain.argtypes = [C.POINTER(Subdomain), _dp, _dp, _dp, _dp, C.c_void_p]
+        L.ora_constraints_subdomain.restype = C.c_int
+        self.threads = threads
+        if threads is not None:
+            try:
+                omp = C.CDLL("libgomp.so.1")
+                omp.omp_set_num_threads(int(threads))
+            except OSError:
+                pass
+
+    # ---- grids -------------------------------------------------------
+    def num_points(self, sd: dict) -> int:
+        return int(self.lib.ora_num_points(C.byref(make_subdomain(sd))))
+
+    def cheb_nodes(self, N: int) -> np.ndarray:
+        x = np.empty(N)
+        self.lib.ora_cheb_nodes(N, x)
+        return x
+
+    def gl_nodes(self, L: int):
+        th, w = np.empty(L + 1), np.empty(L + 1)
+        self.lib.ora_gl_nodes(L, th, w)
+        return th, w
+
+    def coords(self, sd: dict) -> np.ndarray:
+        s = make_subdomain(sd)
+        P = int(self.lib.ora_num_points(C.byref(s)))
+        xyz = np.empty((3, P))
+        self.lib.ora_coords(C.byref(s), xyz)
+        return xyz
+
+    # ---- O1 / O2 / O3 ------------------------------------------------
+    def cheb_derivative_line(self, u: np.ndarray) -> np.ndarray:
+        u = np.ascontiguousarray(u, dtype=np.float64)
+        du = np.empty_like(u)
+        self.lib.ora_cheb_derivative_line(u.shape[0], u, du)
+        return du
+
+    def pbar(self, L: int, theta: float):
+        n = L + 1
+        pb, dpb = np.empty((n, n)), np.empty((n, n))
+        self.lib.ora_pbar(L, float(theta), pb, dpb)
+        return pb, dpb
+
+    def shell_angular(self, L: int, u: np.ndarray):
+        u = np.ascontiguousarray(u, dtype=np.float64)
+        assert u.shape == (L + 1, 2 * L + 2)
+        a, b = np.empty_like(u), np.empty_like(u)
+        self.lib.ora_shell_angular(L, u, a, b)
+        return a, b
+
+    def shell_project(self, L: int, u: np.ndarray) -> np.ndarray:
+        u = np.ascontiguousarray(u, dtype=np.float64)
+        out = np.empty_like(u)
+        self.lib.ora_shell_project(L, u, out)
+        return out
+
+    def gradient(self, sd: dict, u: np.ndarray) -> np.ndarray:
+        """u[ncomp,P] -> g[3,ncomp,P] (Cartesian d/dx, d/dy, d/dz)."""
+        s = make_subdomain(sd)
+        u = np.ascontiguousarray(u, dtype=np.float64)
+        g = np.empty((3,) + u.shape)
+        self.lib.ora_gradient(C.byref(s), u.shape[0], u, g)
+        return g
+
+    # ---- O4 / O5 / O8 at a point (full arrays) ------------------------
+    def geometry_point(self, psi: np.ndarray):
+        ginv, lapse, shift, psiinv = np.empty((3, 3)), np.empty(1), np.empty(3), np.empty((4, 4))
+        bad = self.lib.ora_geometry_point(np.ascontiguousarray(psi, dtype=np.float64), ginv, lapse, shift, psiinv)
+        if bad:
+            raise ValueError("non-physical metric")
+        return ginv, float(lapse[0]), shift, psiinv
+
+    def rhs_point(self, psi, Pi, Phi, dpsi, dPi, dPhi, H, dH, gamma):
+        c = lambda a: np.ascontiguousarray(a, dtype=np.float64)
+        o1, o2, o3 = np.empty((4, 4)), np.empty((4, 4)), np.empty((3, 4, 4))
+        bad = self.lib.ora_rhs_point(c(psi), c(Pi), c(Phi), c(dpsi), c(dPi), c(dPhi), c(H), c(dH), c(gamma), o1, o2, o3)
+        if bad:
+            raise ValueError("non-physical metric")
+        return o1, o2, o3
+
+    def constraints_point(self, psi, Pi, Phi, dpsi, dPhi, H):
+        c = lambda a: np.ascontiguousarray(a, dtype=np.float64)
+        o1, o2, o3 = np.empty(4), np.empty((3, 4, 4)), np.empty((3, 3, 4, 4))
+        bad = self.lib.ora_constraints_point(c(psi), c(Pi), c(Phi), c(dpsi), c(dPhi), c(H), o1, o2, o3)
+        if bad:
+            raise ValueError("non-physical metric")
+        return o1, o2, o3
+
+    # ---- subdomain level (packed 50-component storage) ---------------
+    @staticmethod
+    def _opt(a):
+        if a is None:
+            return None, None
+        a = np.ascontiguousarray(a, dtype=np.float64)
+        return a, a.ctypes.data_as(C.c_void_p)
+
+    def rhs(self, sd: dict, u, H, dH=None) -> np.ndarray:
+        s = make_subdomain(sd)
+        u = np.ascontiguousarray(u, dtype=np.float64)
+        H = np.ascontiguousarray(H, dtype=np.float64)
+        keep, ptr = self._opt(dH)
+        out = np.empty_like(u)
+        bad = self.lib.ora_rhs_subdomain(C.byref(s), u, H, ptr, out)
+        if bad:
+            raise ValueError(f"{bad} non-physical points")
+        return out
+
+    def rhs_full(self, sd: dict, u, H, dH=None) -> np.ndarray:
+        s = make_subdomain(sd)
+        u = np.ascontiguousarray(u, dtype=np.float64)
+        H = np.ascontiguousarray(H, dtype=np.float64)
+        keep, ptr = self._opt(dH)
+        out = np.zeros((80, u.shape[1]))
+        bad = self.lib.ora_rhs_subdomain_full(C.byref(s), u, H, ptr, out)
+        if bad:
+            raise ValueError(f"{bad} non-physical points")
+        return out
+
+    def rk3(self, sd: dict, u, H, dt: float, nsteps: int = 1, dH=None) -> np.ndarray:
+        s = make_subdomain(sd)
+        u = np.array(u, dtype=np.float64, order="C", copy=True)
+        H = np.ascontiguousarray(H, dtype=np.float64)
+        keep, ptr = self._opt(dH)
+        bad = self.lib.ora_rk3_subdomain(C.byref(s), u, H, ptr, float(dt), int(nsteps))
+        if bad:
+            raise ValueError(f"{bad} non-physical points")
+        return u
+
+    def constraints(self, sd: dict, u, H, fields: bool = False):
+        """-> (sums[3], maxs[3], Cfield[64,P] or None) for one subdomain."""
+        s = make_subdomain(sd)
+        u = np.ascontiguousarray(u, dtype=np.float64)
+        H = np.ascontiguousarray(H, dtype=np.float64)
+        sums, maxs = np.empty(3), np.empty(3)
+        Cf = np.zeros((64, u.shape[1])) if fields else None
+        ptr = Cf.ctypes.data_as(C.c_void_p) if fields else None
+        bad = self.lib.ora_constraints_subdomain(C.byref(s), u, H, sums, maxs, ptr)
+        if bad:
+            raise ValueError(f"{bad} non-physical points")
+        return sums, maxs, Cf
+
+    def constraint_norms(self, sds, us, Hs) -> np.ndarray:
+        """Domain norms [3][2] = (rms, max) for C_a, C_iab, C_ijab (unweighted)."""
+        S = np.zeros(3)
+        M = np.zeros(3)
+        P = 0
+        for sd, u, H in zip(sds, us, Hs):
+            s, m, _ = self.constraints(sd, u, H)
+            S += s
+            M = np.maximum(M, m)
+            P += u.shape[1]
+        ncomp = np.array([4.0, 30.0, 30.0])
+        return np.stack([np.sqrt(S / (P * ncomp)), M], axis=1)

@@ -1,0 +1,27 @@
+import os
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+
+def pytest_configure(config):
+    config.addinivalue_line("markers", "gpu: needs a CUDA device (B200); parity tests through the C ABI")
+    config.addinivalue_line("markers", "slow: long-running oracle comparison")
+
+
+@pytest.fixture(scope="session")
+def oracle():
+    from oracle.gh_oracle import Oracle
+
+    return Oracle("long double")
+
+
+@pytest.fixture(scope="session")
+def oracle_double():
+    from oracle.gh_oracle import Oracle
+
+    return Oracle("double")
