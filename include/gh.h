@@ -1,0 +1,165 @@
+/* gh.h — C ABI of the B200-native generalized-harmonic (GH) right-hand-side library.
+ *
+ * The data-parallel hot path of arXiv 1804.09101 (Lewis & Pfeiffer, "GPU-Accelerated
+ * Simulations of Isolated Black Holes"): evaluating the evolution right-hand side of the
+ * first-order generalized-harmonic Einstein system (§1, "about 50 fundamental
+ * variables" PAPER.md:81 §2.1) on spectral subdomains — spherical shells I1 x S2
+ * (Chebyshev radial x Y_lm angular, Eqs. 23-24) and blocks I1^3
+ * (Chebyshev^3, Eqs. 20-22) — followed by a Runge-Kutta stage update and
+ * a constraint-norm reduction.  The paper never prints the evolved equations; the system
+ * implemented is written out in DESIGN.md ("Readings", S1) and SURVEY.md §8(c) O5.
+ *
+ * Conventions common to every call
+ * --------------------------------
+ * - All floating point is IEEE FP64.  No torch types: plain pointers and sizes.  Each pointer
+ *   argument is documented as HOST or DEVICE; arguments with an `on_device` flag may be either.
+ * - Field layout (structure of arrays):  u[c * comp_stride + offsets[s] + local],  c < 50,
+ *   with local = (i0 * n1 + i1) * n2 + i2, last index fastest (the paper's row-major order,
+ *   PAPER.md:397-401).  Shells: (i0,i1,i2) = (r, theta, phi), n1 = L+1 Gauss-Legendre
+ *   colatitudes (ascending theta), n2 = 2L+2 uniform longitudes phi_k = 2 pi k / n2, radial
+ *   Chebyshev-Gauss-Lobatto nodes r = lo + (hi-lo)(x+1)/2, x_j = -cos(pi j/(N_r-1)).
+ *   Blocks: (x, y, z), CGL nodes on every axis.  Padding entries between subdomains are ignored
+ *   on input and left untouched on output.
+ * - Component order: s(a,b), a <= b: 00,01,02,03,11,12,13,22,23,33 -> 0..9;
+ *   psi_ab: c = s;  Pi_ab: c = 10+s;  Phi_iab: c = 20 + 10 i + s  (i = 0,1,2 = x,y,z).
+ *   Tensor components are Cartesian on every subdomain, shells included.
+ * - Ownership: the caller owns the device workspace and the CUDA stream; the library owns only
+ *   the host-side handle.  After gh_domain_create the library never allocates or frees device
+ *   memory (allocation is "extremely expensive", §3.2).  Work is enqueued on the
+ *   stream given at creation; calls that return host data synchronise that stream.
+ * - Errors: every call returns a gh_status; nothing throws across the boundary; a message is
+ *   available from gh_last_error().  There is NO CPU fallback: without a usable CUDA device
+ *   every compute call returns GH_ERR_CUDA.
+ */
+#ifndef GH_H_
+#define GH_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GH_NCOMP 50
+
+typedef struct gh_domain gh_domain; /* opaque; host struct owned by the library */
+
+typedef enum {
+  GH_OK = 0,
+  GH_ERR_ARG = 1,       /* bad descriptor / NULL pointer / unsupported size */
+  GH_ERR_WORKSPACE = 2, /* workspace too small or misaligned (needs 256-byte alignment) */
+  GH_ERR_CUDA = 3,      /* CUDA runtime error (message has the CUDA error string) */
+  GH_ERR_STATE = 4,     /* call out of order (e.g. gh_rhs before gh_set_fields) */
+  GH_ERR_SINGULAR = 5   /* non-physical data met on the device: det g_ij <= 0 or lapse^2 <= 0 */
+} gh_status;
+
+typedef enum { GH_SHELL = 0, GH_BLOCK = 1 } gh_kind;
+typedef enum { GH_FACE_FREE = 0, GH_FACE_FROZEN = 1 } gh_face;
+
+/* One spectral subdomain (PAPER.md:371 I1^3 blocks, PAPER.md:386 I1 x S2 shells). */
+typedef struct {
+  int32_t kind;      /* gh_kind */
+  int32_t n[3];      /* shell: {N_r, L, 0} (N_theta = L+1, N_phi = 2L+2); block: {N_x, N_y, N_z}; N >= 2 */
+  double lo[3], hi[3]; /* shell: lo[0] = r_in, hi[0] = r_out (rest unused); block: corner coordinates */
+  double center[3];  /* shell centre (blocks: ignored) */
+  int32_t face[6];   /* gh_face. shell: [0] = inner, [1] = outer; block: -x,+x,-y,+y,-z,+z */
+  double gamma[3];   /* constraint-damping gamma0, gamma1, gamma2, constant on the subdomain */
+} gh_subdomain_desc;
+
+/* Limits of this build. */
+#define GH_MAX_CHEB_N 64  /* largest N on a Chebyshev axis */
+#define GH_MAX_L 47       /* largest shell L (angular planes are staged in shared memory) */
+
+/* Bytes of device workspace gh_domain_create needs for these subdomains; 0 on invalid input.
+ * Pure host query, no CUDA call.  descs: HOST. */
+size_t gh_workspace_bytes(const gh_subdomain_desc* descs, int32_t n_sub);
+
+/* Build the domain (A0 + A1 of DESIGN.md): validates the descriptors, builds on the host in
+ * long double the Chebyshev-Gauss-Lobatto differentiation matrices (Eq. 22, PAPER.md:379-384;
+ * negative-sum trick), the Gauss-Legendre nodes/weights, the real-Fourier analysis/synthesis
+ * matrices and the per-m Legendre composites that realise Eq. 24 axis by axis,
+ * lays out the structure-of-arrays field store in `dev_workspace` and uploads tables once.
+ *   descs: HOST, n_sub >= 1.   dev_workspace: DEVICE, 256-byte aligned, `bytes` >= gh_workspace_bytes.
+ *   cuda_stream: a cudaStream_t (NULL = the legacy default stream).   out: HOST, receives the handle.
+ * The workspace must stay valid and untouched by the caller until gh_domain_destroy. */
+gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_sub, void* dev_workspace, size_t bytes,
+                           void* cuda_stream, gh_domain** out);
+
+/* Frees the host handle only (the workspace belongs to the caller).  NULL is a no-op. */
+void gh_domain_destroy(gh_domain* dom);
+
+/* Layout query.  n_points: HOST, total grid points P (unpadded).  comp_stride: HOST, distance in doubles
+ * between components (= padded P).  offsets: HOST, n_sub+1 entries, start of each subdomain inside a
+ * component (multiples of 16 doubles), last = comp_stride.  Any pointer may be NULL. */
+gh_status gh_domain_layout(const gh_domain* dom, int64_t* n_points, int64_t* comp_stride, int64_t* offsets);
+
+/* Grid coordinates xyz[3][comp_stride] (x, y, z of every point; padding = 0).  HOST or DEVICE per flag. */
+gh_status gh_domain_coords(const gh_domain* dom, double* xyz, int on_device);
+
+/* Set / get the evolved fields u[50][comp_stride] and the time.  HOST or DEVICE per flag.
+ * gh_get_fields to HOST synchronises and reports GH_ERR_SINGULAR if the device flag was raised. */
+gh_status gh_set_fields(gh_domain* dom, const double* u, int on_device, double t);
+gh_status gh_get_fields(const gh_domain* dom, double* u, int on_device, double* t);
+
+/* Gauge source H_a: H[4][comp_stride] and optionally its Cartesian gradient dH[12][comp_stride]
+ * ([i*4+a] = d_i H_a).  dH == NULL: the library differentiates H once with its own spectral derivative.
+ * d_t H_a = 0 (frozen gauge source, reading S3).  Default before the call: H = 0, dH = 0. */
+gh_status gh_set_gauge_source(gh_domain* dom, const double* H, const double* dH, int on_device);
+
+/* Right-hand side of the current state: dtu[50][comp_stride] = d_t (psi, Pi, Phi).
+ * Steps A2-A6 of DESIGN.md: Chebyshev-line derivatives (Eq. 22), shell angular derivatives through
+ * the l <= L projection (Eq. 24), logical->Cartesian Jacobian (Eq. 8), the fused
+ * pointwise GH algebra, and zeroing on FROZEN faces.  dtu: HOST or DEVICE per flag (HOST synchronises). */
+gh_status gh_rhs(gh_domain* dom, double* dtu, int on_device);
+
+/* Spectral Cartesian gradient of the current state (debug / parity entry, A2-A4):
+ * du[3][50][comp_stride], du[(k*50+c)*comp_stride + p] = d_k u_c.  HOST or DEVICE per flag. */
+gh_status gh_gradient(gh_domain* dom, double* du, int on_device);
+
+/* One full Shu-Osher SSP-RK3 step of size dt (A7; "method of lines", reading S4):
+ *   u1 = u0 + dt k(u0);  u2 = 3/4 u0 + 1/4 (u1 + dt k(u1));  u_new = 1/3 u0 + 2/3 (u2 + dt k(u2)).
+ * Asynchronous on the domain's stream; advances the stored time by dt. */
+gh_status gh_rk_step(gh_domain* dom, double dt);
+
+/* Constraint norms of the current state (A8): out[3][2] = {rms, max} for C_a (4 components),
+ * C_iab = d_i psi_ab - Phi_iab (30), C_ijab = d_i Phi_jab - d_j Phi_iab (30 independent);
+ * rms = sqrt(sum over points and components / (P * n_comp)), unweighted (reading S16).
+ * per_sub: NULL or HOST [n_sub][3][2], the same per subdomain.  out: HOST.  Synchronises; reports
+ * GH_ERR_SINGULAR if the device flag was raised. */
+gh_status gh_constraint_norms(gh_domain* dom, double* out, double* per_sub);
+
+/* Per-kernel device time of the most recent gh_rhs / gh_rk_step / gh_constraint_norms, in
+ * milliseconds, measured with CUDA events on the domain's stream when profiling is enabled with
+ * gh_set_profiling(dom, 1) (off by default: event records cost launch latency).
+ * ms: HOST [GH_NUM_KERNELS] accumulated since the last call to gh_profile_reset; counts likewise. */
+#define GH_NUM_KERNELS 8
+enum { GH_K_CHEB = 0, GH_K_SHELL_ANG = 1, GH_K_RHS = 2, GH_K_RK = 3, GH_K_CONSTRAINTS = 4, GH_K_REDUCE = 5, GH_K_JAC = 6, GH_K_OTHER = 7 };
+gh_status gh_set_profiling(gh_domain* dom, int enabled);
+gh_status gh_profile_read(gh_domain* dom, double* ms, int64_t* counts);
+gh_status gh_profile_reset(gh_domain* dom);
+const char* gh_kernel_name(int k);
+
+/* Number of kernel launches issued by the library on this domain since creation. */
+int64_t gh_launch_count(const gh_domain* dom);
+
+/* Message for the last non-OK status on this domain (or for a failed create when dom == NULL). */
+const char* gh_last_error(const gh_domain* dom);
+
+/* ---- host-side basis builder, exposed for tests (no CUDA) --------------------------------- */
+/* CGL nodes x[N] and differentiation matrix D[N*N] (row-major, D[i*N+j]) on [-1,1]. */
+gh_status gh_basis_cheb(int32_t N, double* x, double* D);
+/* Gauss-Legendre colatitudes theta[L+1] (ascending) and weights w[L+1]. */
+gh_status gh_basis_gauss_legendre(int32_t L, double* theta, double* w);
+/* Shell angular matrices for band limit L, n_t = L+1, n_p = 2L+2, n_q = 2L+1:
+ *   Fa[n_q*n_p]: analysis, row q: q=0..L cos(m phi_k) (m=q), q=L+1..2L sin(m phi_k) (m=q-L), normalised
+ *                so that Fs*Fa is the projector onto modes m <= L;
+ *   Fs[n_p*n_q]: synthesis;
+ *   Th[(L+1)*n_t*n_t]: per-m composite d/dtheta o projection, Th[m][j'][j];
+ *   Pr[(L+1)*n_t*n_t]: per-m projector onto l <= L.   Any pointer may be NULL. */
+gh_status gh_basis_shell(int32_t L, double* Fa, double* Fs, double* Th, double* Pr);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GH_H_ */

@@ -1,0 +1,35 @@
+// basis.h — host-side basis-matrix builder (step A0 of DESIGN.md).  Internal to the library.
+//
+// Everything here runs once per domain on the host in long double and is rounded to double at the end
+// ("extra function calls needed to build the matrix ... can be ignored", §3.4).
+#pragma once
+#include <vector>
+
+namespace ghb {
+
+typedef long double ld;
+
+// Chebyshev-Gauss-Lobatto nodes x_j = -cos(pi j/(N-1)) (ascending) and the collocation differentiation
+// matrix D (row-major N x N) on [-1,1]: the "cached matrix" of PAPER.md:357-384 (Eqs. 19-22), built
+// analytically instead of by delta-tracing.  Diagonal by the negative-sum trick.
+void cheb_nodes(int N, std::vector<ld>& x);
+void cheb_diff_matrix(int N, std::vector<ld>& D);
+
+// Gauss-Legendre nodes: cos(theta_j) descending (theta ascending), weights; n = L+1 points.
+void gauss_legendre(int L, std::vector<ld>& ct, std::vector<ld>& w);
+
+// Shell angular matrices for band limit L (n_t = L+1, n_p = 2L+2, n_q = 2L+1), all row-major:
+//   Fa [n_q][n_p]  real-Fourier analysis: rows q=0..L cos(m phi_k) (m=q), rows q=L+1..2L sin(m phi_k) (m=q-L)
+//   Fs [n_p][n_q]  synthesis of u            from the (cos, sin) coefficients
+//   Fp [n_p][n_q]  synthesis of d u / d phi  from the same coefficients
+//   Th [L+1][n_t][n_t]  per-m:  d/dtheta of the projection onto l<=L, Th[m][j'][j]
+//   Pr [L+1][n_t][n_t]  per-m:  the projection itself
+// Together Fs*Th*Fa and Fp*Pr*Fa are the dense Theta and Phi matrices of Eq. 24.
+struct ShellBasis {
+  int L, nt, np, nq;
+  std::vector<ld> ct, st, w;  // cos/sin(theta_j), GL weights
+  std::vector<ld> Fa, Fs, Fp, Th, Pr;
+};
+void shell_basis(int L, ShellBasis& B);
+
+}  // namespace ghb

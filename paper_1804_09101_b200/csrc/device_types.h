@@ -1,0 +1,51 @@
+// device_types.h — plain structs shared by the host API (gh_lib.cu) and the kernels (kernels.cuh).
+#pragma once
+#include <stdint.h>
+
+namespace ghd {
+
+constexpr int NCOMP = 50;
+constexpr int TILE_PTS = 128;   // points per CTA of the pointwise kernels (K_rhs, K_con, K_jac)
+
+// One spectral subdomain as the kernels see it.
+struct SubDev {
+  int32_t kind;            // 0 shell, 1 block
+  int32_t n0, n1, n2;      // logical extents, n2 fastest (shell: N_r, L+1, 2L+2)
+  int64_t off;             // start inside a component (multiple of 16 doubles)
+  int32_t P;               // n0*n1*n2
+  int32_t face[6];         // 1 = FROZEN
+  double gamma[3];
+  // shells only: offsets (in doubles) into the table memory
+  int32_t t_rinv;          // 1/r_i               [n0]
+  int32_t t_ct, t_st;      // cos/sin(theta_j)     [n1]
+  int32_t t_cp, t_sp;      // cos/sin(phi_k)       [n2]
+  int32_t pad_;
+};
+
+// One tile of Chebyshev lines: out[a, col] = sum_i Dt[i][a] in[i, col] for `ncols` columns (A2, Eq. 22).
+// Element (i, col) lives at  base + i*stride_i + (col / col_inner)*outer_stride + (col % col_inner).
+struct ChebItem {
+  int64_t base;
+  int64_t stride_i;
+  int64_t outer_stride;
+  int32_t N;
+  int32_t col_inner;
+  int32_t col0;
+  int32_t ncols;
+  int32_t dmat;     // offset (doubles) of Dt[N][apitch], already multiplied by 2/(hi-lo)
+  int32_t apitch;   // N rounded up to a multiple of 8
+  int32_t axis;     // which logical-derivative slot the result goes to
+  int32_t pad_;
+};
+
+// One batch of angular planes of one shell (A3, Eq. 24): planes [plane0, plane0+nplanes) of component
+// `blockIdx.y`; plane ir starts at off + ir * n1*n2.
+struct AngItem {
+  int64_t off;
+  int32_t L;
+  int32_t plane0;
+  int32_t nplanes;
+  int32_t m_Fa, m_Fs, m_Fp, m_Th, m_Pr;   // offsets (doubles) of the shell matrices in the table memory
+};
+
+}  // namespace ghd

@@ -1,0 +1,433 @@
+// gh_lib.cu — the C ABI of include/gh.h: host-side domain planning (A0, A1) and kernel launches (A2-A8).
+// No torch, no CPU fallback: every compute call needs a CUDA device and returns GH_ERR_CUDA without one.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <string>
+#include <utility>
+#include <vector>
+
+#include "../../include/gh.h"
+#include "basis.h"
+#include "device_types.h"
+#include "kernels_deriv.cuh"
+#include "kernels_point.cuh"
+
+using namespace ghd;
+
+namespace {
+
+constexpr int CHEB_TPB = 64, CHEB_CPT = 4, CHEB_CT = CHEB_TPB * CHEB_CPT;   // lines per K_cheb tile
+constexpr int ANG_TPB = 256;
+constexpr size_t ANG_SMEM_TARGET = 100 * 1024;   // planes per K_ang CTA are chosen to stay under this
+constexpr size_t SMEM_MAX = 227 * 1024;
+
+thread_local std::string g_create_error;
+
+inline int64_t round_up(int64_t v, int64_t m) { return (v + m - 1) / m * m; }
+
+struct Carve {   // bump allocator over the caller's workspace (256-byte granularity)
+  size_t pos = 0;
+  size_t take(size_t bytes) { size_t p = pos; pos += (size_t)round_up((int64_t)bytes, 256); return p; }
+};
+
+struct Plan {
+  int n_sub = 0;
+  std::vector<gh_subdomain_desc> descs;
+  std::vector<int64_t> offsets;          // n_sub+1
+  std::vector<int32_t> tile_first;       // n_sub+1
+  int64_t P = 0, S = 0;
+  int n_tiles = 0;
+  size_t table_doubles = 0;
+  int n_cheb_items = 0, n_cheb_items_r = 0, n_ang_items = 0;
+  size_t cheb_smem = 0, ang_smem = 0;
+  std::vector<int> ang_pb;               // planes per CTA for each subdomain (0 for blocks)
+  // workspace offsets (bytes)
+  size_t o_ua, o_ub, o_k, o_du, o_H, o_dH, o_tables, o_subs, o_tiles, o_cheb, o_ang, o_part, o_persub, o_flag, total;
+};
+
+inline void sub_dims(const gh_subdomain_desc& d, int& n0, int& n1, int& n2) {
+  if (d.kind == GH_SHELL) { n0 = d.n[0]; n1 = d.n[1] + 1; n2 = 2 * d.n[1] + 2; }
+  else { n0 = d.n[0]; n1 = d.n[1]; n2 = d.n[2]; }
+}
+
+inline size_t ang_plane_smem(int L) { return (size_t)(L + 1) * ((2 * L + 2) + 2 * (2 * L + 1)) * sizeof(double); }
+inline size_t shell_matrix_doubles(int L) {
+  size_t nt = L + 1, np = 2 * L + 2, nq = 2 * L + 1;
+  return 3 * nq * np + 2 * (size_t)(L + 1) * nt * nt;
+}
+
+bool validate(const gh_subdomain_desc* descs, int32_t n_sub, std::string& err) {
+  char buf[256];
+  if (!descs || n_sub < 1) { err = "descs is NULL or n_sub < 1"; return false; }
+  for (int s = 0; s < n_sub; ++s) {
+    const gh_subdomain_desc& d = descs[s];
+    if (d.kind == GH_SHELL) {
+      if (d.n[0] < 2 || d.n[0] > GH_MAX_CHEB_N || d.n[1] < 1 || d.n[1] > GH_MAX_L) {
+        snprintf(buf, sizeof buf, "subdomain %d: shell needs 2 <= N_r <= %d and 1 <= L <= %d", s, GH_MAX_CHEB_N, GH_MAX_L);
+        err = buf; return false;
+      }
+      if (!(d.lo[0] > 0.0) || !(d.hi[0] > d.lo[0])) { snprintf(buf, sizeof buf, "subdomain %d: shell needs 0 < r_in < r_out", s); err = buf; return false; }
+    } else if (d.kind == GH_BLOCK) {
+      for (int a = 0; a < 3; ++a) {
+        if (d.n[a] < 2 || d.n[a] > GH_MAX_CHEB_N) { snprintf(buf, sizeof buf, "subdomain %d: block needs 2 <= N <= %d on every axis", s, GH_MAX_CHEB_N); err = buf; return false; }
+        if (!(d.hi[a] > d.lo[a])) { snprintf(buf, sizeof buf, "subdomain %d: block needs lo < hi on every axis", s); err = buf; return false; }
+      }
+    } else { snprintf(buf, sizeof buf, "subdomain %d: unknown kind %d", s, d.kind); err = buf; return false; }
+    for (int f = 0; f < 6; ++f)
+      if (d.face[f] != GH_FACE_FREE && d.face[f] != GH_FACE_FROZEN) { snprintf(buf, sizeof buf, "subdomain %d: bad face flag", s); err = buf; return false; }
+    for (int g = 0; g < 3; ++g)
+      if (!std::isfinite(d.gamma[g])) { snprintf(buf, sizeof buf, "subdomain %d: non-finite gamma", s); err = buf; return false; }
+  }
+  return true;
+}
+
+// Sizes and offsets of everything; pure host arithmetic (shared by gh_workspace_bytes and gh_domain_create).
+bool make_plan(const gh_subdomain_desc* descs, int32_t n_sub, Plan& pl, std::string& err) {
+  if (!validate(descs, n_sub, err)) return false;
+  pl.n_sub = n_sub;
+  pl.descs.assign(descs, descs + n_sub);
+  pl.offsets.assign(n_sub + 1, 0);
+  pl.tile_first.assign(n_sub + 1, 0);
+  pl.ang_pb.assign(n_sub, 0);
+  std::map<int, int> seenL;
+  size_t tab = 0;
+  int64_t off = 0, tiles = 0;
+  for (int s = 0; s < n_sub; ++s) {
+    const gh_subdomain_desc& d = descs[s];
+    int n0, n1, n2; sub_dims(d, n0, n1, n2);
+    const int64_t Ps = (int64_t)n0 * n1 * n2;
+    if (Ps > (int64_t)1 << 30) { err = "subdomain too large"; return false; }
+    pl.offsets[s] = off; off += round_up(Ps, 16);
+    pl.tile_first[s] = (int32_t)tiles; tiles += (Ps + TILE_PTS - 1) / TILE_PTS;
+    pl.P += Ps;
+    const int naxes = d.kind == GH_SHELL ? 1 : 3;
+    for (int a = 0; a < naxes; ++a) {
+      const int N = d.n[a];
+      const int nn[3] = {n0, n1, n2};
+      (void)nn;
+      tab += (size_t)N * round_up(N, 8);
+      const int64_t cols = Ps / N;
+      const int items = (int)((cols + CHEB_CT - 1) / CHEB_CT);
+      pl.n_cheb_items += items;
+      pl.cheb_smem = std::max(pl.cheb_smem, ((size_t)N * round_up(N, 8) + (size_t)N * (CHEB_CT + 1)) * sizeof(double));
+    }
+    if (d.kind == GH_SHELL) {
+      const int L = d.n[1];
+      tab += (size_t)round_up(n0, 2) + 2 * (size_t)round_up(n1, 2) + 2 * (size_t)round_up(n2, 2);
+      if (!seenL.count(L)) { seenL[L] = 1; tab += shell_matrix_doubles(L); }
+      const size_t per = ang_plane_smem(L);
+      int pb = (int)std::max<size_t>(1, ANG_SMEM_TARGET / per);
+      pb = std::min(pb, n0);
+      if (per * pb > SMEM_MAX) { err = "shell L too large for shared memory"; return false; }
+      pl.ang_pb[s] = pb;
+      pl.n_ang_items += (n0 + pb - 1) / pb;
+      pl.ang_smem = std::max(pl.ang_smem, per * pb);
+    }
+  }
+  if (tiles > 0x7fffffff) { err = "domain too large"; return false; }
+  pl.offsets[n_sub] = off; pl.S = off;
+  pl.tile_first[n_sub] = (int32_t)tiles; pl.n_tiles = (int)tiles;
+  pl.table_doubles = tab;
+  if (pl.cheb_smem > SMEM_MAX) { err = "Chebyshev N too large for shared memory"; return false; }
+  Carve c;
+  const size_t comp = (size_t)pl.S * sizeof(double);
+  pl.o_ua = c.take(NCOMP * comp); pl.o_ub = c.take(NCOMP * comp); pl.o_k = c.take(NCOMP * comp);
+  pl.o_du = c.take(3 * NCOMP * comp); pl.o_H = c.take(4 * comp); pl.o_dH = c.take(12 * comp);
+  pl.o_tables = c.take(pl.table_doubles * sizeof(double));
+  pl.o_subs = c.take((size_t)n_sub * sizeof(SubDev));
+  pl.o_tiles = c.take((size_t)(n_sub + 1) * sizeof(int32_t));
+  pl.o_cheb = c.take((size_t)pl.n_cheb_items * sizeof(ChebItem));
+  pl.o_ang = c.take((size_t)std::max(1, pl.n_ang_items) * sizeof(AngItem));
+  pl.o_part = c.take((size_t)pl.n_tiles * 6 * sizeof(double));
+  pl.o_persub = c.take((size_t)n_sub * 6 * sizeof(double));
+  pl.o_flag = c.take(256);
+  pl.total = c.pos;
+  return true;
+}
+
+}  // namespace
+
+struct gh_domain {
+  Plan pl;
+  char* ws = nullptr;
+  cudaStream_t stream = nullptr;
+  double *ua = nullptr, *ub = nullptr, *k = nullptr, *du = nullptr, *H = nullptr, *dH = nullptr, *tables = nullptr;
+  SubDev* subs = nullptr;
+  int32_t* tiles = nullptr;
+  ChebItem* cheb = nullptr;
+  AngItem* ang = nullptr;
+  double *part = nullptr, *persub = nullptr;
+  int* flag = nullptr;
+  std::vector<SubDev> h_subs;
+  bool has_fields = false, has_shell = false, has_block = false;
+  double t = 0.0;
+  int64_t launches = 0;
+  std::string err;
+  // profiling
+  bool prof = false;
+  struct Pending { cudaEvent_t a, b; int cls; };
+  std::vector<Pending> pending;
+  std::vector<cudaEvent_t> pool;
+  double prof_ms[GH_NUM_KERNELS] = {0};
+  int64_t prof_n[GH_NUM_KERNELS] = {0};
+};
+
+namespace {
+
+gh_status fail(gh_domain* d, gh_status st, const std::string& msg) {
+  if (d) d->err = msg; else g_create_error = msg;
+  return st;
+}
+#define GH_CUDA(d, call)                                                                              \
+  do {                                                                                                \
+    cudaError_t e_ = (call);                                                                          \
+    if (e_ != cudaSuccess) return fail(d, GH_ERR_CUDA, std::string(#call ": ") + cudaGetErrorString(e_)); \
+  } while (0)
+
+cudaEvent_t get_event(gh_domain* d) {
+  if (!d->pool.empty()) { cudaEvent_t e = d->pool.back(); d->pool.pop_back(); return e; }
+  cudaEvent_t e; cudaEventCreate(&e); return e;
+}
+struct ProfScope {   // brackets one launch with events when profiling is on; always counts the launch
+  gh_domain* d; int cls; cudaEvent_t a = nullptr, b = nullptr;
+  ProfScope(gh_domain* d_, int cls_) : d(d_), cls(cls_) {
+    d->launches += 1;
+    if (d->prof) { a = get_event(d); b = get_event(d); cudaEventRecord(a, d->stream); }
+  }
+  ~ProfScope() { if (d->prof) { cudaEventRecord(b, d->stream); d->pending.push_back({a, b, cls}); } }
+};
+void drain_profile(gh_domain* d) {
+  if (d->pending.empty()) return;
+  cudaStreamSynchronize(d->stream);
+  for (auto& p : d->pending) {
+    float ms = 0; cudaEventElapsedTime(&ms, p.a, p.b);
+    d->prof_ms[p.cls] += ms; d->prof_n[p.cls] += 1;
+    d->pool.push_back(p.a); d->pool.push_back(p.b);
+  }
+  d->pending.clear();
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------------------
+// host-side basis builder entry points (no CUDA)
+// ------------------------------------------------------------------------------------------------------
+extern "C" gh_status gh_basis_cheb(int32_t N, double* x, double* D) {
+  if (N < 2) return GH_ERR_ARG;
+  std::vector<ghb::ld> xv, Dv;
+  ghb::cheb_nodes(N, xv); ghb::cheb_diff_matrix(N, Dv);
+  if (x) for (int j = 0; j < N; ++j) x[j] = (double)xv[j];
+  if (D) for (size_t e = 0; e < (size_t)N * N; ++e) D[e] = (double)Dv[e];
+  return GH_OK;
+}
+
+extern "C" gh_status gh_basis_gauss_legendre(int32_t L, double* theta, double* w) {
+  if (L < 0) return GH_ERR_ARG;
+  std::vector<ghb::ld> ct, wv;
+  ghb::gauss_legendre(L, ct, wv);
+  for (int j = 0; j <= L; ++j) { if (theta) theta[j] = (double)acosl(ct[j]); if (w) w[j] = (double)wv[j]; }
+  return GH_OK;
+}
+
+extern "C" gh_status gh_basis_shell(int32_t L, double* Fa, double* Fs, double* Th, double* Pr) {
+  if (L < 1) return GH_ERR_ARG;
+  ghb::ShellBasis B; ghb::shell_basis(L, B);
+  if (Fa) for (size_t e = 0; e < B.Fa.size(); ++e) Fa[e] = (double)B.Fa[e];
+  if (Fs) for (size_t e = 0; e < B.Fs.size(); ++e) Fs[e] = (double)B.Fs[e];
+  if (Th) for (size_t e = 0; e < B.Th.size(); ++e) Th[e] = (double)B.Th[e];
+  if (Pr) for (size_t e = 0; e < B.Pr.size(); ++e) Pr[e] = (double)B.Pr[e];
+  return GH_OK;
+}
+
+extern "C" size_t gh_workspace_bytes(const gh_subdomain_desc* descs, int32_t n_sub) {
+  Plan pl; std::string err;
+  if (!make_plan(descs, n_sub, pl, err)) { g_create_error = err; return 0; }
+  return pl.total;
+}
+
+// ------------------------------------------------------------------------------------------------------
+// gh_domain_create: A0 (tables) + A1 (store layout, work lists), one upload
+// ------------------------------------------------------------------------------------------------------
+extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_sub, void* dev_workspace, size_t bytes,
+                                      void* cuda_stream, gh_domain** out) {
+  if (!out) return fail(nullptr, GH_ERR_ARG, "out is NULL");
+  *out = nullptr;
+  Plan pl; std::string err;
+  if (!make_plan(descs, n_sub, pl, err)) return fail(nullptr, GH_ERR_ARG, err);
+  if (!dev_workspace || ((uintptr_t)dev_workspace & 255) != 0) return fail(nullptr, GH_ERR_WORKSPACE, "workspace is NULL or not 256-byte aligned");
+  if (bytes < pl.total) return fail(nullptr, GH_ERR_WORKSPACE, "workspace too small: need " + std::to_string(pl.total) + " bytes");
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return fail(nullptr, GH_ERR_CUDA, "no CUDA device (this library has no CPU fallback)"); }
+
+  gh_domain* d = new gh_domain();
+  d->pl = pl; d->ws = (char*)dev_workspace; d->stream = (cudaStream_t)cuda_stream;
+  char* w = d->ws;
+  d->ua = (double*)(w + pl.o_ua); d->ub = (double*)(w + pl.o_ub); d->k = (double*)(w + pl.o_k);
+  d->du = (double*)(w + pl.o_du); d->H = (double*)(w + pl.o_H); d->dH = (double*)(w + pl.o_dH);
+  d->tables = (double*)(w + pl.o_tables); d->subs = (SubDev*)(w + pl.o_subs); d->tiles = (int32_t*)(w + pl.o_tiles);
+  d->cheb = (ChebItem*)(w + pl.o_cheb); d->ang = (AngItem*)(w + pl.o_ang);
+  d->part = (double*)(w + pl.o_part); d->persub = (double*)(w + pl.o_persub); d->flag = (int*)(w + pl.o_flag);
+
+  // ---- tables and work lists on the host ----
+  std::vector<double> tab(pl.table_doubles, 0.0);
+  std::vector<ChebItem> cheb; cheb.reserve(pl.n_cheb_items);
+  std::vector<ChebItem> cheb_r;   // radial items of shells are kept with the others; the list is one launch
+  std::vector<AngItem> ang; ang.reserve(pl.n_ang_items);
+  d->h_subs.resize(n_sub);
+  size_t tp = 0;
+  std::map<int, std::vector<ghb::ld>> Dcache;        // N -> unscaled D
+  struct ShellOff { int Fa, Fs, Fp, Th, Pr; };
+  std::map<int, ShellOff> Lcache;
+  for (int s = 0; s < n_sub; ++s) {
+    const gh_subdomain_desc& de = descs[s];
+    SubDev& sd = d->h_subs[s];
+    memset(&sd, 0, sizeof sd);
+    int n0, n1, n2; sub_dims(de, n0, n1, n2);
+    sd.kind = de.kind; sd.n0 = n0; sd.n1 = n1; sd.n2 = n2; sd.off = pl.offsets[s]; sd.P = n0 * n1 * n2;
+    for (int f = 0; f < 6; ++f) sd.face[f] = de.face[f];
+    for (int g = 0; g < 3; ++g) sd.gamma[g] = de.gamma[g];
+    const int naxes = de.kind == GH_SHELL ? 1 : 3;
+    const int64_t nn[3] = {n0, n1, n2};
+    const int64_t strides[3] = {(int64_t)n1 * n2, n2, 1};
+    for (int a = 0; a < naxes; ++a) {
+      const int N = (int)nn[a];
+      if (!Dcache.count(N)) ghb::cheb_diff_matrix(N, Dcache[N]);
+      const std::vector<ghb::ld>& D = Dcache[N];
+      const int ap = (int)round_up(N, 8);
+      const ghb::ld scale = 2 / ((ghb::ld)de.hi[a] - (ghb::ld)de.lo[a]);   // affine map factor of Eq. 22
+      const int dm = (int)tp;
+      for (int i = 0; i < N; ++i)
+        for (int o = 0; o < N; ++o) tab[tp + (size_t)i * ap + o] = (double)(scale * D[(size_t)o * N + i]);   // Dt[i][o]
+      tp += (size_t)N * ap;
+      const int64_t cols = sd.P / N;
+      for (int64_t c0 = 0; c0 < cols; c0 += CHEB_CT) {
+        ChebItem it; memset(&it, 0, sizeof it);
+        it.base = sd.off; it.stride_i = strides[a]; it.N = N; it.dmat = dm; it.apitch = ap; it.axis = a;
+        it.col0 = (int)c0; it.ncols = (int)std::min<int64_t>(CHEB_CT, cols - c0);
+        if (a == 0) { it.col_inner = (int)(nn[1] * nn[2]); it.outer_stride = 0; }
+        else if (a == 1) { it.col_inner = (int)nn[2]; it.outer_stride = nn[1] * nn[2]; }
+        else { it.col_inner = 1; it.outer_stride = nn[2]; }
+        cheb.push_back(it);
+      }
+    }
+    if (de.kind == GH_SHELL) {
+      d->has_shell = true;
+      const int L = de.n[1];
+      if (!Lcache.count(L)) {
+        ghb::ShellBasis B; ghb::shell_basis(L, B);
+        ShellOff o;
+        auto put = [&](const std::vector<ghb::ld>& v) { int at = (int)tp; for (size_t e = 0; e < v.size(); ++e) tab[tp + e] = (double)v[e]; tp += v.size(); return at; };
+        o.Fa = put(B.Fa); o.Fs = put(B.Fs); o.Fp = put(B.Fp); o.Th = put(B.Th); o.Pr = put(B.Pr);
+        Lcache[L] = o;
+      }
+      const ShellOff& o = Lcache[L];
+      // coordinate tables of this shell (for the Jacobian of Eq. 8)
+      std::vector<ghb::ld> xr, ct, wv;
+      ghb::cheb_nodes(n0, xr); ghb::gauss_legendre(L, ct, wv);
+      sd.t_rinv = (int)tp;
+      for (int i = 0; i < n0; ++i) {
+        ghb::ld r = (ghb::ld)de.lo[0] + ((ghb::ld)de.hi[0] - (ghb::ld)de.lo[0]) * (xr[i] + 1) / 2;
+        tab[tp + i] = (double)(1 / r);
+      }
+      tp += round_up(n0, 2);
+      sd.t_ct = (int)tp; for (int j = 0; j < n1; ++j) tab[tp + j] = (double)ct[j]; tp += round_up(n1, 2);
+      sd.t_st = (int)tp; for (int j = 0; j < n1; ++j) tab[tp + j] = (double)sqrtl((1 - ct[j]) * (1 + ct[j])); tp += round_up(n1, 2);
+      const ghb::ld PI_L = 3.14159265358979323846264338327950288L;
+      sd.t_cp = (int)tp; for (int k = 0; k < n2; ++k) tab[tp + k] = (double)cosl(2 * PI_L * k / n2); tp += round_up(n2, 2);
+      sd.t_sp = (int)tp; for (int k = 0; k < n2; ++k) tab[tp + k] = (double)sinl(2 * PI_L * k / n2); tp += round_up(n2, 2);
+      const int pb = pl.ang_pb[s];
+      for (int p0 = 0; p0 < n0; p0 += pb) {
+        AngItem it; memset(&it, 0, sizeof it);
+        it.off = sd.off; it.L = L; it.plane0 = p0; it.nplanes = std::min(pb, n0 - p0);
+        it.m_Fa = o.Fa; it.m_Fs = o.Fs; it.m_Fp = o.Fp; it.m_Th = o.Th; it.m_Pr = o.Pr;
+        ang.push_back(it);
+      }
+    } else {
+      d->has_block = true;
+    }
+  }
+  if (tp != pl.table_doubles || (int)cheb.size() != pl.n_cheb_items || (int)ang.size() != pl.n_ang_items) {
+    delete d; return fail(nullptr, GH_ERR_STATE, "internal: plan and build disagree");
+  }
+
+  // ---- one-time upload; zero the store so that padding is zero ----
+  cudaStream_t st = d->stream;
+#define GH_CREATE_CUDA(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { std::string m = std::string(#call ": ") + cudaGetErrorString(e_); delete d; return fail(nullptr, GH_ERR_CUDA, m); } } while (0)
+  GH_CREATE_CUDA(cudaMemsetAsync(d->ws, 0, pl.o_tables, st));
+  GH_CREATE_CUDA(cudaMemsetAsync(d->part, 0, pl.total - pl.o_part, st));
+  GH_CREATE_CUDA(cudaMemcpyAsync(d->tables, tab.data(), tab.size() * sizeof(double), cudaMemcpyHostToDevice, st));
+  GH_CREATE_CUDA(cudaMemcpyAsync(d->subs, d->h_subs.data(), (size_t)n_sub * sizeof(SubDev), cudaMemcpyHostToDevice, st));
+  GH_CREATE_CUDA(cudaMemcpyAsync(d->tiles, pl.tile_first.data(), (size_t)(n_sub + 1) * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+  GH_CREATE_CUDA(cudaMemcpyAsync(d->cheb, cheb.data(), cheb.size() * sizeof(ChebItem), cudaMemcpyHostToDevice, st));
+  if (!ang.empty()) GH_CREATE_CUDA(cudaMemcpyAsync(d->ang, ang.data(), ang.size() * sizeof(AngItem), cudaMemcpyHostToDevice, st));
+  GH_CREATE_CUDA(cudaStreamSynchronize(st));   // host staging vectors die at return
+  GH_CREATE_CUDA(cudaFuncSetAttribute(k_cheb<CHEB_TPB, CHEB_CPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.cheb_smem));
+  if (pl.ang_smem) GH_CREATE_CUDA(cudaFuncSetAttribute(k_ang<ANG_TPB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.ang_smem));
+#undef GH_CREATE_CUDA
+  *out = d;
+  return GH_OK;
+}
+
+extern "C" void gh_domain_destroy(gh_domain* d) {
+  if (!d) return;
+  for (auto& p : d->pending) { cudaEventDestroy(p.a); cudaEventDestroy(p.b); }
+  for (auto e : d->pool) cudaEventDestroy(e);
+  delete d;
+}
+
+extern "C" gh_status gh_domain_layout(const gh_domain* d, int64_t* n_points, int64_t* comp_stride, int64_t* offsets) {
+  if (!d) return GH_ERR_ARG;
+  if (n_points) *n_points = d->pl.P;
+  if (comp_stride) *comp_stride = d->pl.S;
+  if (offsets) for (int s = 0; s <= d->pl.n_sub; ++s) offsets[s] = d->pl.offsets[s];
+  return GH_OK;
+}
+
+extern "C" gh_status gh_domain_coords(const gh_domain* cd, double* xyz, int on_device) {
+  gh_domain* d = const_cast<gh_domain*>(cd);
+  if (!d || !xyz) return fail(d, GH_ERR_ARG, "NULL argument");
+  const int64_t S = d->pl.S;
+  std::vector<double> h((size_t)3 * S, 0.0);
+  const ghb::ld PI_L = 3.14159265358979323846264338327950288L;
+  for (int s = 0; s < d->pl.n_sub; ++s) {
+    const gh_subdomain_desc& de = d->pl.descs[s];
+    int n0, n1, n2; sub_dims(de, n0, n1, n2);
+    const int64_t off = d->pl.offsets[s];
+    if (de.kind == GH_SHELL) {
+      std::vector<ghb::ld> xr, ct, wv; ghb::cheb_nodes(n0, xr); ghb::gauss_legendre(de.n[1], ct, wv);
+      for (int i = 0; i < n0; ++i) {
+        const ghb::ld r = (ghb::ld)de.lo[0] + ((ghb::ld)de.hi[0] - (ghb::ld)de.lo[0]) * (xr[i] + 1) / 2;
+        for (int j = 0; j < n1; ++j) {
+          const ghb::ld st = sqrtl((1 - ct[j]) * (1 + ct[j]));
+          for (int k = 0; k < n2; ++k) {
+            const ghb::ld ph = 2 * PI_L * k / n2;
+            const int64_t p = off + ((int64_t)i * n1 + j) * n2 + k;
+            h[p] = (double)((ghb::ld)de.center[0] + r * st * cosl(ph));
+            h[S + p] = (double)((ghb::ld)de.center[1] + r * st * sinl(ph));
+            h[2 * S + p] = (double)((ghb::ld)de.center[2] + r * ct[j]);
+          }
+        }
+      }
+    } else {
+      std::vector<ghb::ld> x[3];
+      for (int a = 0; a < 3; ++a) ghb::cheb_nodes(de.n[a], x[a]);
+      for (int i = 0; i < n0; ++i) for (int j = 0; j < n1; ++j) for (int k = 0; k < n2; ++k) {
+        const int64_t p = off + ((int64_t)i * n1 + j) * n2 + k; const int id[3] = {i, j, k};
+        for (int a = 0; a < 3; ++a)
+          h[(size_t)a * S + p] = (double)((ghb::ld)de.lo[a] + ((ghb::ld)de.hi[a] - (ghb::ld)de.lo[a]) * (x[a][id[a]] + 1) / 2);
+      }
+    }
+  }
+  if (on_device) {
+    GH_CUDA(d, cudaMemcpyAsync(xyz, h.data(), h.size() * sizeof(double), cudaMemcpyHostToDevice, d->stream));
+    GH_CUDA(d, cudaStreamSynchronize(d->stream));
+  } else {
+    memcpy(xyz, h.data(), h.size() * sizeof(double));
+  }
+  return GH_OK;
+}

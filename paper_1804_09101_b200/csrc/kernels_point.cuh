@@ -1,0 +1,545 @@
+// kernels_point.cuh — pointwise kernels: fused Jacobian + GH right-hand side + face mask (A4-A6),
+// RK stage update (A7), constraints + reduction (A8).
+//
+// The evolved system is the first-order generalized-harmonic Einstein system the paper evolves
+// ("the Einstein equations in their generalized harmonic formulation"; "about 50 fundamental
+// variables"); the paper does not print it, reading S1 writes it out:
+//   dt psi_ab  = (1+g1) N^k d_k psi_ab - N Pi_ab - g1 N^i Phi_iab
+//   dt Pi_ab   = N^k d_k Pi_ab - N g^{ki} d_k Phi_iab + g1 g2 N^k (d_k psi_ab - Phi_kab)
+//                + 2N psi^{cd} ( g^{ij} Phi_ica Phi_jdb - Pi_ca Pi_db - psi^{ef} Gam_ace Gam_bdf )
+//                - 2N nabla_(a H_b) - 1/2 N t^c t^d Pi_cd Pi_ab - N t^c Pi_ci g^{ij} Phi_jab
+//                + N g0 ( t_b C_a + t_a C_b - psi_ab t^c C_c )
+//   dt Phi_iab = N^k d_k Phi_iab - N d_i Pi_ab + N g2 (d_i psi_ab - Phi_iab)
+//                + 1/2 N t^c t^d Phi_icd Pi_ab + N g^{jk} t^c Phi_ijc Phi_kab
+// with Gam_abc built from the first-order variables (d_0 psi = -N Pi + N^i Phi_i, d_i psi = Phi_i).
+#pragma once
+#include "device_types.h"
+#include "kernels_deriv.cuh"
+
+namespace ghd {
+
+// index of the symmetric pair (a,b) in the packed order 00,01,02,03,11,12,13,22,23,33
+__host__ __device__ constexpr int SI(int a, int b) {
+  return a <= b ? (a * 4 - (a * (a - 1)) / 2 + b - a) : (b * 4 - (b * (b - 1)) / 2 + a - b);
+}
+// index of the spatial symmetric pair (i,j), i,j in 0..2, packed xx,xy,xz,yy,yz,zz
+__host__ __device__ constexpr int S3(int i, int j) {
+  return i <= j ? (i * 3 - (i * (i - 1)) / 2 + j - i) : (j * 3 - (j * (j - 1)) / 2 + i - j);
+}
+
+struct Geom {
+  double gi[6];     // g^{ij}
+  double sh[3];     // N^i
+  double N;         // lapse
+  double pinv[10];  // psi^{ab}
+  double tu[4];     // t^a = (1/N, -N^i/N)
+};
+
+// O4 of DESIGN.md.  Returns false on non-physical data (det g_ij <= 0 or N^2 <= 0).
+__device__ __forceinline__ bool geometry(const double (&psi)[10], Geom& G) {
+  const double gxx = psi[SI(1, 1)], gxy = psi[SI(1, 2)], gxz = psi[SI(1, 3)];
+  const double gyy = psi[SI(2, 2)], gyz = psi[SI(2, 3)], gzz = psi[SI(3, 3)];
+  const double cxx = gyy * gzz - gyz * gyz, cxy = gyz * gxz - gxy * gzz, cxz = gxy * gyz - gyy * gxz;
+  const double det = gxx * cxx + gxy * cxy + gxz * cxz;
+  const double idet = 1.0 / det;
+  G.gi[S3(0, 0)] = cxx * idet;
+  G.gi[S3(0, 1)] = cxy * idet;
+  G.gi[S3(0, 2)] = cxz * idet;
+  G.gi[S3(1, 1)] = (gxx * gzz - gxz * gxz) * idet;
+  G.gi[S3(1, 2)] = (gxy * gxz - gxx * gyz) * idet;
+  G.gi[S3(2, 2)] = (gxx * gyy - gxy * gxy) * idet;
+  double n2 = -psi[SI(0, 0)];
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    double s = 0.0;
+#pragma unroll
+    for (int j = 0; j < 3; ++j) s = fma(G.gi[S3(i, j)], psi[SI(0, j + 1)], s);
+    G.sh[i] = s;
+  }
+#pragma unroll
+  for (int i = 0; i < 3; ++i) n2 = fma(G.sh[i], psi[SI(0, i + 1)], n2);
+  const bool ok = (det > 0.0) && (n2 > 0.0);
+  const double in2 = 1.0 / n2;
+  G.N = sqrt(n2);
+  G.pinv[SI(0, 0)] = -in2;
+#pragma unroll
+  for (int i = 0; i < 3; ++i) G.pinv[SI(0, i + 1)] = G.sh[i] * in2;
+#pragma unroll
+  for (int i = 0; i < 3; ++i)
+#pragma unroll
+    for (int j = i; j < 3; ++j) G.pinv[SI(i + 1, j + 1)] = G.gi[S3(i, j)] - G.sh[i] * G.sh[j] * in2;
+  const double iN = 1.0 / G.N;
+  G.tu[0] = iN;
+#pragma unroll
+  for (int i = 0; i < 3; ++i) G.tu[i + 1] = -G.sh[i] * iN;
+  return ok;
+}
+
+// Christoffel symbols of the first kind from the first-order variables, as 4 symmetric matrices
+// Gam[a][SI(b,c)] = 1/2 (D_b psi_ac + D_c psi_ab - D_a psi_bc),  D_0 = -N Pi + N^i Phi_i,  D_i = Phi_i.
+__device__ __forceinline__ void christoffel(const Geom& G, const double (&Pi)[10], const double (&Phi)[3][10],
+                                            double (&Gam)[4][10]) {
+  double D0[10];
+#pragma unroll
+  for (int s = 0; s < 10; ++s) {
+    double v = -G.N * Pi[s];
+#pragma unroll
+    for (int i = 0; i < 3; ++i) v = fma(G.sh[i], Phi[i][s], v);
+    D0[s] = v;
+  }
+#define GH_D(c, s) ((c) == 0 ? D0[s] : Phi[(c) - 1][s])
+#pragma unroll
+  for (int a = 0; a < 4; ++a)
+#pragma unroll
+    for (int b = 0; b < 4; ++b)
+#pragma unroll
+      for (int c = b; c < 4; ++c)
+        Gam[a][SI(b, c)] = 0.5 * (GH_D(b, SI(a, c)) + GH_D(c, SI(a, b)) - GH_D(a, SI(b, c)));
+#undef GH_D
+}
+
+// full contraction of two symmetric 4x4 matrices X^{bc} Y_bc in packed storage
+__device__ __forceinline__ double symdot(const double (&X)[10], const double (&Y)[10]) {
+  double s = 0.0;
+#pragma unroll
+  for (int b = 0; b < 4; ++b)
+#pragma unroll
+    for (int c = b; c < 4; ++c) s = fma((b == c ? 1.0 : 2.0) * X[SI(b, c)], Y[SI(b, c)], s);
+  return s;
+}
+
+// Quantities of the algebraic part that the per-(ab) assembly needs.
+struct Alg {
+  double S[10];    // W_ab - (Pi psi^-1 Pi)_ab - T_ab + H^d Gam_dab
+  double C[4];     // C_a = H_a + Gam_a
+  double tC;       // t^c C_c
+  double ttPi;     // t^c t^d Pi_cd
+  double p[3];     // t^c Pi_ci
+  double s[3];     // t^c t^d Phi_icd
+  double w[3][3];  // w[i][j] = t^c Phi_i(j+1)c
+};
+
+__device__ __forceinline__ void algebraic(const Geom& G, const double (&Pi)[10], const double (&Phi)[3][10],
+                                          const double (&H)[4], Alg& A) {
+  double Gam[4][10];
+  christoffel(G, Pi, Phi, Gam);
+  double Hup[4];
+#pragma unroll
+  for (int d = 0; d < 4; ++d) {
+    double v = 0.0;
+#pragma unroll
+    for (int c = 0; c < 4; ++c) v = fma(G.pinv[SI(d, c)], H[c], v);
+    Hup[d] = v;
+  }
+#pragma unroll
+  for (int a = 0; a < 4; ++a) A.C[a] = H[a] + symdot(G.pinv, Gam[a]);
+  A.tC = 0.0;
+#pragma unroll
+  for (int a = 0; a < 4; ++a) A.tC = fma(G.tu[a], A.C[a], A.tC);
+  // H^d Gam_dab
+#pragma unroll
+  for (int s = 0; s < 10; ++s) {
+    double v = 0.0;
+#pragma unroll
+    for (int d = 0; d < 4; ++d) v = fma(Hup[d], Gam[d][s], v);
+    A.S[s] = v;
+  }
+  // - T_ab,  T_ab = psi^{cd} psi^{ef} Gam_ace Gam_bdf = R_a^{df} Gam_bdf,  R_a = psi^-1 Gam_a psi^-1
+#pragma unroll
+  for (int a = 0; a < 4; ++a) {
+    double Y[4][4];  // Y[d][e] = psi^{dc} Gam_a[c][e]
+#pragma unroll
+    for (int d = 0; d < 4; ++d)
+#pragma unroll
+      for (int e = 0; e < 4; ++e) {
+        double v = 0.0;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) v = fma(G.pinv[SI(d, c)], Gam[a][SI(c, e)], v);
+        Y[d][e] = v;
+      }
+    double R[10];
+#pragma unroll
+    for (int d = 0; d < 4; ++d)
+#pragma unroll
+      for (int f = d; f < 4; ++f) {
+        double v = 0.0;
+#pragma unroll
+        for (int e = 0; e < 4; ++e) v = fma(Y[d][e], G.pinv[SI(e, f)], v);
+        R[SI(d, f)] = v;
+      }
+#pragma unroll
+    for (int b = a; b < 4; ++b) A.S[SI(a, b)] -= symdot(R, Gam[b]);
+  }
+  // - Pi_ac psi^{cd} Pi_db
+  {
+    double Q[4][4];  // Q[c][b] = psi^{cd} Pi_db
+#pragma unroll
+    for (int c = 0; c < 4; ++c)
+#pragma unroll
+      for (int b = 0; b < 4; ++b) {
+        double v = 0.0;
+#pragma unroll
+        for (int d = 0; d < 4; ++d) v = fma(G.pinv[SI(c, d)], Pi[SI(d, b)], v);
+        Q[c][b] = v;
+      }
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+#pragma unroll
+      for (int b = a; b < 4; ++b) {
+        double v = 0.0;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) v = fma(Pi[SI(a, c)], Q[c][b], v);
+        A.S[SI(a, b)] -= v;
+      }
+  }
+  // + W_ab = g^{ij} Phi_iac psi^{cd} Phi_jdb = sum_i (Phi^i psi^-1 Phi_i)_ab,  Phi^i = g^{ij} Phi_j
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    double Z[4][4];  // Z[c][b] = psi^{cd} Phi_i,db
+#pragma unroll
+    for (int c = 0; c < 4; ++c)
+#pragma unroll
+      for (int b = 0; b < 4; ++b) {
+        double v = 0.0;
+#pragma unroll
+        for (int d = 0; d < 4; ++d) v = fma(G.pinv[SI(c, d)], Phi[i][SI(d, b)], v);
+        Z[c][b] = v;
+      }
+#pragma unroll
+    for (int a = 0; a < 4; ++a) {
+      double up[4];  // Phi^i_ac, c = 0..3
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        double v = 0.0;
+#pragma unroll
+        for (int j = 0; j < 3; ++j) v = fma(G.gi[S3(i, j)], Phi[j][SI(a, c)], v);
+        up[c] = v;
+      }
+#pragma unroll
+      for (int b = a; b < 4; ++b) {
+        double v = 0.0;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) v = fma(up[c], Z[c][b], v);
+        A.S[SI(a, b)] += v;
+      }
+    }
+  }
+  // small contractions with the normal t^a
+  A.ttPi = 0.0;
+#pragma unroll
+  for (int c = 0; c < 4; ++c)
+#pragma unroll
+    for (int d = 0; d < 4; ++d) A.ttPi = fma(G.tu[c] * G.tu[d], Pi[SI(c, d)], A.ttPi);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    double v = 0.0, u = 0.0;
+#pragma unroll
+    for (int c = 0; c < 4; ++c) v = fma(G.tu[c], Pi[SI(c, i + 1)], v);
+    A.p[i] = v;
+#pragma unroll
+    for (int c = 0; c < 4; ++c)
+#pragma unroll
+      for (int d = 0; d < 4; ++d) u = fma(G.tu[c] * G.tu[d], Phi[i][SI(c, d)], u);
+    A.s[i] = u;
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+      double x = 0.0;
+#pragma unroll
+      for (int c = 0; c < 4; ++c) x = fma(G.tu[c], Phi[i][SI(j + 1, c)], x);
+      A.w[i][j] = x;
+    }
+  }
+}
+
+
+// ---------------------------------------------------------------------------------------------------------
+// K_rhs.  One thread per grid point, TILE_PTS points per CTA, tiles never straddle subdomains.
+// Reads 50 fields + 150 logical derivatives + 4 H_a + 12 d_iH_a once, writes 50 once (2 152 B/point).
+// Stage 1: psi -> geometry; stage 2: Pi, Phi -> algebraic part (Gam, quadratic sources, C_a);
+// stage 3: per symmetric pair (ab) stream in its 15 derivatives (Jacobian applied on the fly for shells),
+// assemble the 5 outputs and store.  FROZEN faces get zeros (A6).
+// ---------------------------------------------------------------------------------------------------------
+template <bool SHELL>
+__device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __restrict__ tables, int local,
+                                          const double* __restrict__ u, const double* __restrict__ du,
+                                          const double* __restrict__ Hs, const double* __restrict__ dHs,
+                                          double* __restrict__ k, int64_t S, int* __restrict__ flag) {
+  const int64_t p = sd.off + local;
+  double psi[10], Pi[10], Phi[3][10], H[4];
+#pragma unroll
+  for (int s = 0; s < 10; ++s) psi[s] = u[(int64_t)s * S + p];
+#pragma unroll
+  for (int s = 0; s < 10; ++s) Pi[s] = u[(int64_t)(10 + s) * S + p];
+#pragma unroll
+  for (int i = 0; i < 3; ++i)
+#pragma unroll
+    for (int s = 0; s < 10; ++s) Phi[i][s] = u[(int64_t)(20 + 10 * i + s) * S + p];
+#pragma unroll
+  for (int a = 0; a < 4; ++a) H[a] = Hs[(int64_t)a * S + p];
+
+  // face mask (A6)
+  bool frozen;
+  {
+    const int i2 = local % sd.n2, t = local / sd.n2, i1 = t % sd.n1, i0 = t / sd.n1;
+    frozen = (i0 == 0 && sd.face[0] == 1) || (i0 == sd.n0 - 1 && sd.face[1] == 1);
+    if (!SHELL)
+      frozen = frozen || (i1 == 0 && sd.face[2] == 1) || (i1 == sd.n1 - 1 && sd.face[3] == 1) ||
+               (i2 == 0 && sd.face[4] == 1) || (i2 == sd.n2 - 1 && sd.face[5] == 1);
+  }
+
+  Geom G;
+  const bool ok = geometry(psi, G);
+  if (!ok) atomicOr(flag, 1);
+  if (!ok || frozen) {
+#pragma unroll 1
+    for (int c = 0; c < NCOMP; ++c) k[(int64_t)c * S + p] = 0.0;
+    return;
+  }
+  Alg A;
+  algebraic(G, Pi, Phi, H, A);
+
+  ShellJac J;
+  if (SHELL) J = shell_jac(sd, tables, local);
+  const double g0 = sd.gamma[0], g1 = sd.gamma[1], g2 = sd.gamma[2], N = G.N;
+  const int64_t DS = (int64_t)NCOMP * S;   // stride between derivative directions
+
+#pragma unroll
+  for (int a = 0; a < 4; ++a)
+#pragma unroll
+    for (int b = a; b < 4; ++b) {
+      const int s = SI(a, b);
+      // d[c5][k]: Cartesian derivative k of component (psi, Pi, Phi_x, Phi_y, Phi_z)_ab
+      double d[5][3];
+#pragma unroll
+      for (int c5 = 0; c5 < 5; ++c5) {
+        const double* q = du + (int64_t)(10 * c5 + s) * S + p;
+        const double l0 = q[0], l1 = q[DS], l2 = q[2 * DS];
+        if (SHELL) {
+          d[c5][0] = J.xr * l0 + J.xt * l1 + J.xp * l2;
+          d[c5][1] = J.yr * l0 + J.yt * l1 + J.yp * l2;
+          d[c5][2] = J.zr * l0 + J.zt * l1;
+        } else {
+          d[c5][0] = l0; d[c5][1] = l1; d[c5][2] = l2;
+        }
+      }
+      double sdpsi = 0.0, sdPi = 0.0, sPhi = 0.0;
+#pragma unroll
+      for (int kk = 0; kk < 3; ++kk) {
+        sdpsi = fma(G.sh[kk], d[0][kk], sdpsi);
+        sdPi = fma(G.sh[kk], d[1][kk], sdPi);
+        sPhi = fma(G.sh[kk], Phi[kk][s], sPhi);
+      }
+      k[(int64_t)s * S + p] = (1.0 + g1) * sdpsi - N * Pi[s] - g1 * sPhi;
+
+      double gdPhi = 0.0;   // g^{ki} d_k Phi_iab
+#pragma unroll
+      for (int kk = 0; kk < 3; ++kk)
+#pragma unroll
+        for (int i = 0; i < 3; ++i) gdPhi = fma(G.gi[S3(kk, i)], d[2 + i][kk], gdPhi);
+      double up[3];         // Phi^j_ab = g^{jk} Phi_kab
+#pragma unroll
+      for (int j = 0; j < 3; ++j) {
+        double v = 0.0;
+#pragma unroll
+        for (int kk = 0; kk < 3; ++kk) v = fma(G.gi[S3(j, kk)], Phi[kk][s], v);
+        up[j] = v;
+      }
+      // 1/2 (d_a H_b + d_b H_a), d_0 H = 0 ; dHs[(i*4+b)] = d_i H_b
+      double symdH = 0.0;
+      if (a > 0) symdH += dHs[(int64_t)((a - 1) * 4 + b) * S + p];
+      if (b > 0) symdH += dHs[(int64_t)((b - 1) * 4 + a) * S + p];
+      symdH *= 0.5;
+      double pup = 0.0;
+#pragma unroll
+      for (int i = 0; i < 3; ++i) pup = fma(A.p[i], up[i], pup);
+      // t_a = (-N, 0, 0, 0)
+      const double tbCa = (b == 0 ? -N * A.C[a] : 0.0), taCb = (a == 0 ? -N * A.C[b] : 0.0);
+      double r = sdPi - N * gdPhi + g1 * g2 * (sdpsi - sPhi) + 2.0 * N * (A.S[s] - symdH) - 0.5 * N * A.ttPi * Pi[s] -
+                 N * pup + N * g0 * (tbCa + taCb - psi[s] * A.tC);
+      k[(int64_t)(10 + s) * S + p] = r;
+#pragma unroll
+      for (int i = 0; i < 3; ++i) {
+        double sdPhi = 0.0, wup = 0.0;
+#pragma unroll
+        for (int kk = 0; kk < 3; ++kk) sdPhi = fma(G.sh[kk], d[2 + i][kk], sdPhi);
+#pragma unroll
+        for (int j = 0; j < 3; ++j) wup = fma(A.w[i][j], up[j], wup);
+        k[(int64_t)(20 + 10 * i + s) * S + p] =
+            sdPhi - N * d[1][i] + N * g2 * (d[0][i] - Phi[i][s]) + 0.5 * N * A.s[i] * Pi[s] + N * wup;
+      }
+    }
+}
+
+__global__ void __launch_bounds__(TILE_PTS, 2)
+k_rhs(const SubDev* __restrict__ subs, const int32_t* __restrict__ tile_first, int n_sub,
+      const double* __restrict__ tables, const double* __restrict__ u, const double* __restrict__ du,
+      const double* __restrict__ Hs, const double* __restrict__ dHs, double* __restrict__ k, int64_t S,
+      int* __restrict__ flag) {
+  __shared__ SubDev sd_s;
+  __shared__ int tile0_s;
+  if (threadIdx.x == 0) {
+    const int s = find_sub(tile_first, n_sub, blockIdx.x);
+    sd_s = subs[s];
+    tile0_s = tile_first[s];
+  }
+  __syncthreads();
+  const SubDev& sd = sd_s;
+  const int local = (blockIdx.x - tile0_s) * TILE_PTS + threadIdx.x;
+  if (local >= sd.P) return;
+  if (sd.kind == 0) rhs_point<true>(sd, tables, local, u, du, Hs, dHs, k, S, flag);
+  else rhs_point<false>(sd, tables, local, u, du, Hs, dHs, k, S, flag);
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// K_rk (A7): one stage of Shu-Osher SSP-RK3 written as  out = a*u0 + b*(us + dt*k)  over the whole store
+// (padding included; it is zero and stays zero).  Stage 1: a=0,b=1 (u0 not read).
+// ---------------------------------------------------------------------------------------------------------
+template <bool READ_U0>
+__global__ void __launch_bounds__(256)
+k_rk(const double2* __restrict__ u0, const double2* __restrict__ us, const double2* __restrict__ k,
+     double2* __restrict__ out, double a, double b, double dt, int64_t n2) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n2; i += (int64_t)gridDim.x * blockDim.x) {
+    const double2 s = us[i], kk = k[i];
+    double2 r;
+    r.x = b * fma(dt, kk.x, s.x);
+    r.y = b * fma(dt, kk.y, s.y);
+    if (READ_U0) {
+      const double2 o = u0[i];
+      r.x = fma(a, o.x, r.x);
+      r.y = fma(a, o.y, r.y);
+    }
+    out[i] = r;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// K_con (A8): constraints at a point, then warp-shuffle + block reduction to per-tile partials
+// part[tile][6] = {sum C_a^2, sum C_iab^2, sum C_ijab^2, max|C_a|, max|C_iab|, max|C_ijab|};
+// K_con_reduce folds the tiles of each subdomain in a fixed order (deterministic).
+// ---------------------------------------------------------------------------------------------------------
+template <bool SHELL>
+__device__ __forceinline__ void con_point(const SubDev& sd, const double* __restrict__ tables, int local,
+                                          const double* __restrict__ u, const double* __restrict__ du,
+                                          const double* __restrict__ Hs, int64_t S, int* __restrict__ flag,
+                                          double (&acc)[6]) {
+  const int64_t p = sd.off + local;
+  double psi[10], Pi[10], Phi[3][10], H[4];
+#pragma unroll
+  for (int s = 0; s < 10; ++s) psi[s] = u[(int64_t)s * S + p];
+#pragma unroll
+  for (int s = 0; s < 10; ++s) Pi[s] = u[(int64_t)(10 + s) * S + p];
+#pragma unroll
+  for (int i = 0; i < 3; ++i)
+#pragma unroll
+    for (int s = 0; s < 10; ++s) Phi[i][s] = u[(int64_t)(20 + 10 * i + s) * S + p];
+#pragma unroll
+  for (int a = 0; a < 4; ++a) H[a] = Hs[(int64_t)a * S + p];
+  Geom G;
+  if (!geometry(psi, G)) { atomicOr(flag, 1); return; }
+  {
+    double Gam[4][10];
+    christoffel(G, Pi, Phi, Gam);
+#pragma unroll
+    for (int a = 0; a < 4; ++a) {
+      const double c = H[a] + symdot(G.pinv, Gam[a]);
+      acc[0] = fma(c, c, acc[0]);
+      acc[3] = fmax(acc[3], fabs(c));
+    }
+  }
+  ShellJac J;
+  if (SHELL) J = shell_jac(sd, tables, local);
+  const int64_t DS = (int64_t)NCOMP * S;
+#pragma unroll 1
+  for (int s = 0; s < 10; ++s) {
+    double d[4][3];   // Cartesian derivatives of psi_ab, Phi_xab, Phi_yab, Phi_zab
+#pragma unroll
+    for (int c4 = 0; c4 < 4; ++c4) {
+      const int comp = (c4 == 0) ? s : 10 + 10 * c4 + s;
+      const double* q = du + (int64_t)comp * S + p;
+      const double l0 = q[0], l1 = q[DS], l2 = q[2 * DS];
+      if (SHELL) {
+        d[c4][0] = J.xr * l0 + J.xt * l1 + J.xp * l2;
+        d[c4][1] = J.yr * l0 + J.yt * l1 + J.yp * l2;
+        d[c4][2] = J.zr * l0 + J.zt * l1;
+      } else {
+        d[c4][0] = l0; d[c4][1] = l1; d[c4][2] = l2;
+      }
+    }
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      const double c = d[0][i] - u[(int64_t)(20 + 10 * i + s) * S + p];
+      acc[1] = fma(c, c, acc[1]);
+      acc[4] = fmax(acc[4], fabs(c));
+    }
+    // C_ijab = d_i Phi_jab - d_j Phi_iab for (i,j) = (0,1), (0,2), (1,2)
+    const double c01 = d[2][0] - d[1][1], c02 = d[3][0] - d[1][2], c12 = d[3][1] - d[2][2];
+    acc[2] = fma(c01, c01, acc[2]); acc[2] = fma(c02, c02, acc[2]); acc[2] = fma(c12, c12, acc[2]);
+    acc[5] = fmax(acc[5], fmax(fabs(c01), fmax(fabs(c02), fabs(c12))));
+  }
+}
+
+__global__ void __launch_bounds__(TILE_PTS)
+k_con(const SubDev* __restrict__ subs, const int32_t* __restrict__ tile_first, int n_sub,
+      const double* __restrict__ tables, const double* __restrict__ u, const double* __restrict__ du,
+      const double* __restrict__ Hs, int64_t S, int* __restrict__ flag, double* __restrict__ part) {
+  __shared__ SubDev sd_s;
+  __shared__ int tile0_s;
+  __shared__ double red[TILE_PTS / 32][6];
+  if (threadIdx.x == 0) {
+    const int s = find_sub(tile_first, n_sub, blockIdx.x);
+    sd_s = subs[s];
+    tile0_s = tile_first[s];
+  }
+  __syncthreads();
+  const SubDev& sd = sd_s;
+  const int local = (blockIdx.x - tile0_s) * TILE_PTS + threadIdx.x;
+  double acc[6] = {0, 0, 0, 0, 0, 0};
+  if (local < sd.P) {
+    if (sd.kind == 0) con_point<true>(sd, tables, local, u, du, Hs, S, flag, acc);
+    else con_point<false>(sd, tables, local, u, du, Hs, S, flag, acc);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+    for (int q = 0; q < 3; ++q) acc[q] += __shfl_xor_sync(0xffffffffu, acc[q], o);
+#pragma unroll
+    for (int q = 3; q < 6; ++q) acc[q] = fmax(acc[q], __shfl_xor_sync(0xffffffffu, acc[q], o));
+  }
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (lane == 0)
+#pragma unroll
+    for (int q = 0; q < 6; ++q) red[warp][q] = acc[q];
+  __syncthreads();
+  if (threadIdx.x < 6) {
+    const int q = threadIdx.x;
+    double v = red[0][q];
+    for (int w = 1; w < TILE_PTS / 32; ++w) v = (q < 3) ? v + red[w][q] : fmax(v, red[w][q]);
+    part[(int64_t)blockIdx.x * 6 + q] = v;
+  }
+}
+
+// one warp per subdomain: per_sub[s][6] from its tiles, in tile order
+__global__ void __launch_bounds__(32)
+k_con_reduce(const int32_t* __restrict__ tile_first, const double* __restrict__ part, double* __restrict__ per_sub) {
+  const int s = blockIdx.x, lane = threadIdx.x;
+  const int t0 = tile_first[s], t1 = tile_first[s + 1];
+  double acc[6] = {0, 0, 0, 0, 0, 0};
+  for (int t = t0 + lane; t < t1; t += 32) {
+#pragma unroll
+    for (int q = 0; q < 3; ++q) acc[q] += part[(int64_t)t * 6 + q];
+#pragma unroll
+    for (int q = 3; q < 6; ++q) acc[q] = fmax(acc[q], part[(int64_t)t * 6 + q]);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+    for (int q = 0; q < 3; ++q) acc[q] += __shfl_xor_sync(0xffffffffu, acc[q], o);
+#pragma unroll
+    for (int q = 3; q < 6; ++q) acc[q] = fmax(acc[q], __shfl_xor_sync(0xffffffffu, acc[q], o));
+  }
+  if (lane == 0)
+#pragma unroll
+    for (int q = 0; q < 6; ++q) per_sub[(int64_t)s * 6 + q] = acc[q];
+}
+
+}  // namespace ghd
