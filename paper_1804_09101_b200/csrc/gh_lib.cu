@@ -431,3 +431,231 @@ extern "C" gh_status gh_domain_coords(const gh_domain* cd, double* xyz, int on_d
   }
   return GH_OK;
 }
+
+// ------------------------------------------------------------------------------------------------------
+// launch helpers
+// ------------------------------------------------------------------------------------------------------
+namespace {
+
+gh_status check_flag(gh_domain* d) {   // stream must be synchronised by the caller's preceding copy
+  int h = 0;
+  GH_CUDA(d, cudaMemcpyAsync(&h, d->flag, sizeof(int), cudaMemcpyDeviceToHost, d->stream));
+  GH_CUDA(d, cudaStreamSynchronize(d->stream));
+  if (h) {
+    cudaMemsetAsync(d->flag, 0, sizeof(int), d->stream);
+    return fail(d, GH_ERR_SINGULAR, "non-physical data on the device: det g_ij <= 0 or lapse^2 <= 0");
+  }
+  return GH_OK;
+}
+
+// A2 + A3: logical derivatives of `ncomp` components of `in` into out[3][ncomp][S]
+// (blocks: d/dx, d/dy, d/dz already Cartesian; shells: d/dr, d/dtheta, d/dphi).
+gh_status launch_derivs(gh_domain* d, const double* in, double* out, int ncomp) {
+  const Plan& pl = d->pl;
+  {
+    ProfScope ps(d, GH_K_CHEB);
+    k_cheb<CHEB_TPB, CHEB_CPT><<<dim3(pl.n_cheb_items, ncomp), CHEB_TPB, pl.cheb_smem, d->stream>>>(
+        d->cheb, d->tables, in, out, pl.S, ncomp);
+  }
+  if (pl.n_ang_items) {
+    ProfScope ps(d, GH_K_SHELL_ANG);
+    k_ang<ANG_TPB><<<dim3(pl.n_ang_items, ncomp), ANG_TPB, pl.ang_smem, d->stream>>>(d->ang, d->tables, in, out, pl.S, ncomp);
+  }
+  GH_CUDA(d, cudaGetLastError());
+  return GH_OK;
+}
+
+// A2-A6 on state `u`, result into `k` (device pointers)
+gh_status launch_rhs(gh_domain* d, const double* u, double* k) {
+  gh_status st = launch_derivs(d, u, d->du, NCOMP);
+  if (st != GH_OK) return st;
+  {
+    ProfScope ps(d, GH_K_RHS);
+    k_rhs<<<d->pl.n_tiles, TILE_PTS, 0, d->stream>>>(d->subs, d->tiles, d->pl.n_sub, d->tables, u, d->du, d->H, d->dH, k,
+                                                     d->pl.S, d->flag);
+  }
+  GH_CUDA(d, cudaGetLastError());
+  return GH_OK;
+}
+
+gh_status launch_jac(gh_domain* d, double* g, int ncomp) {
+  if (!d->has_shell) return GH_OK;
+  ProfScope ps(d, GH_K_JAC);
+  k_jac<<<d->pl.n_tiles, TILE_PTS, 0, d->stream>>>(d->subs, d->tiles, d->pl.n_sub, d->tables, g, d->pl.S, ncomp);
+  GH_CUDA(d, cudaGetLastError());
+  return GH_OK;
+}
+
+gh_status launch_rk(gh_domain* d, const double* u0, const double* us, const double* k, double* out, double a, double b, double dt) {
+  const int64_t n2 = (int64_t)NCOMP * d->pl.S / 2;   // S is a multiple of 16
+  int dev = 0, sms = 148;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  const int64_t want = (n2 + 255) / 256;
+  const int grid = (int)std::min<int64_t>(want, (int64_t)sms * 8);
+  ProfScope ps(d, GH_K_RK);
+  if (a == 0.0)
+    k_rk<false><<<grid, 256, 0, d->stream>>>(nullptr, (const double2*)us, (const double2*)k, (double2*)out, a, b, dt, n2);
+  else
+    k_rk<true><<<grid, 256, 0, d->stream>>>((const double2*)u0, (const double2*)us, (const double2*)k, (double2*)out, a, b, dt, n2);
+  GH_CUDA(d, cudaGetLastError());
+  return GH_OK;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------------------
+// state in / out
+// ------------------------------------------------------------------------------------------------------
+extern "C" gh_status gh_set_fields(gh_domain* d, const double* u, int on_device, double t) {
+  if (!d || !u) return fail(d, GH_ERR_ARG, "NULL argument");
+  const size_t bytes = (size_t)NCOMP * d->pl.S * sizeof(double);
+  GH_CUDA(d, cudaMemcpyAsync(d->ua, u, bytes, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, d->stream));
+  if (!on_device) GH_CUDA(d, cudaStreamSynchronize(d->stream));
+  d->t = t; d->has_fields = true;
+  return GH_OK;
+}
+
+extern "C" gh_status gh_get_fields(const gh_domain* cd, double* u, int on_device, double* t) {
+  gh_domain* d = const_cast<gh_domain*>(cd);
+  if (!d || !u) return fail(d, GH_ERR_ARG, "NULL argument");
+  if (!d->has_fields) return fail(d, GH_ERR_STATE, "gh_get_fields before gh_set_fields");
+  const size_t bytes = (size_t)NCOMP * d->pl.S * sizeof(double);
+  GH_CUDA(d, cudaMemcpyAsync(u, d->ua, bytes, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, d->stream));
+  if (t) *t = d->t;
+  if (!on_device) return check_flag(d);
+  return GH_OK;
+}
+
+extern "C" gh_status gh_set_gauge_source(gh_domain* d, const double* H, const double* dH, int on_device) {
+  if (!d || !H) return fail(d, GH_ERR_ARG, "NULL argument");
+  const size_t comp = (size_t)d->pl.S * sizeof(double);
+  const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+  GH_CUDA(d, cudaMemcpyAsync(d->H, H, 4 * comp, kind, d->stream));
+  if (dH) {
+    GH_CUDA(d, cudaMemcpyAsync(d->dH, dH, 12 * comp, kind, d->stream));
+  } else {
+    gh_status st = launch_derivs(d, d->H, d->dH, 4);
+    if (st != GH_OK) return st;
+    st = launch_jac(d, d->dH, 4);
+    if (st != GH_OK) return st;
+  }
+  if (!on_device) GH_CUDA(d, cudaStreamSynchronize(d->stream));
+  return GH_OK;
+}
+
+// ------------------------------------------------------------------------------------------------------
+// compute entry points
+// ------------------------------------------------------------------------------------------------------
+extern "C" gh_status gh_rhs(gh_domain* d, double* dtu, int on_device) {
+  if (!d || !dtu) return fail(d, GH_ERR_ARG, "NULL argument");
+  if (!d->has_fields) return fail(d, GH_ERR_STATE, "gh_rhs before gh_set_fields");
+  if (on_device) return launch_rhs(d, d->ua, dtu);
+  gh_status st = launch_rhs(d, d->ua, d->k);
+  if (st != GH_OK) return st;
+  GH_CUDA(d, cudaMemcpyAsync(dtu, d->k, (size_t)NCOMP * d->pl.S * sizeof(double), cudaMemcpyDeviceToHost, d->stream));
+  return check_flag(d);
+}
+
+extern "C" gh_status gh_gradient(gh_domain* d, double* du, int on_device) {
+  if (!d || !du) return fail(d, GH_ERR_ARG, "NULL argument");
+  if (!d->has_fields) return fail(d, GH_ERR_STATE, "gh_gradient before gh_set_fields");
+  double* tgt = on_device ? du : d->du;
+  gh_status st = launch_derivs(d, d->ua, tgt, NCOMP);
+  if (st != GH_OK) return st;
+  st = launch_jac(d, tgt, NCOMP);
+  if (st != GH_OK) return st;
+  if (!on_device) {
+    GH_CUDA(d, cudaMemcpyAsync(du, d->du, (size_t)3 * NCOMP * d->pl.S * sizeof(double), cudaMemcpyDeviceToHost, d->stream));
+    GH_CUDA(d, cudaStreamSynchronize(d->stream));
+  }
+  return GH_OK;
+}
+
+extern "C" gh_status gh_rk_step(gh_domain* d, double dt) {
+  if (!d) return GH_ERR_ARG;
+  if (!d->has_fields) return fail(d, GH_ERR_STATE, "gh_rk_step before gh_set_fields");
+  if (!std::isfinite(dt)) return fail(d, GH_ERR_ARG, "dt is not finite");
+  gh_status st;
+  // u1 = u0 + dt k(u0)
+  if ((st = launch_rhs(d, d->ua, d->k)) != GH_OK) return st;
+  if ((st = launch_rk(d, nullptr, d->ua, d->k, d->ub, 0.0, 1.0, dt)) != GH_OK) return st;
+  // u2 = 3/4 u0 + 1/4 (u1 + dt k(u1))
+  if ((st = launch_rhs(d, d->ub, d->k)) != GH_OK) return st;
+  if ((st = launch_rk(d, d->ua, d->ub, d->k, d->ub, 0.75, 0.25, dt)) != GH_OK) return st;
+  // u_new = 1/3 u0 + 2/3 (u2 + dt k(u2))
+  if ((st = launch_rhs(d, d->ub, d->k)) != GH_OK) return st;
+  if ((st = launch_rk(d, d->ua, d->ub, d->k, d->ua, 1.0 / 3.0, 2.0 / 3.0, dt)) != GH_OK) return st;
+  d->t += dt;
+  return GH_OK;
+}
+
+extern "C" gh_status gh_constraint_norms(gh_domain* d, double* out, double* per_sub) {
+  if (!d || !out) return fail(d, GH_ERR_ARG, "NULL argument");
+  if (!d->has_fields) return fail(d, GH_ERR_STATE, "gh_constraint_norms before gh_set_fields");
+  const Plan& pl = d->pl;
+  gh_status st = launch_derivs(d, d->ua, d->du, NCOMP);
+  if (st != GH_OK) return st;
+  {
+    ProfScope ps(d, GH_K_CONSTRAINTS);
+    k_con<<<pl.n_tiles, TILE_PTS, 0, d->stream>>>(d->subs, d->tiles, pl.n_sub, d->tables, d->ua, d->du, d->H, pl.S, d->flag, d->part);
+  }
+  {
+    ProfScope ps(d, GH_K_REDUCE);
+    k_con_reduce<<<pl.n_sub, 32, 0, d->stream>>>(d->tiles, d->part, d->persub);
+  }
+  GH_CUDA(d, cudaGetLastError());
+  std::vector<double> h((size_t)pl.n_sub * 6);
+  GH_CUDA(d, cudaMemcpyAsync(h.data(), d->persub, h.size() * sizeof(double), cudaMemcpyDeviceToHost, d->stream));
+  st = check_flag(d);   // synchronises
+  if (st != GH_OK) return st;
+  static const double ncomp[3] = {4.0, 30.0, 30.0};
+  double sum[3] = {0, 0, 0}, mx[3] = {0, 0, 0};
+  for (int s = 0; s < pl.n_sub; ++s) {
+    int n0, n1, n2; sub_dims(pl.descs[s], n0, n1, n2);
+    const double Ps = (double)n0 * n1 * n2;
+    for (int q = 0; q < 3; ++q) {
+      sum[q] += h[(size_t)s * 6 + q];
+      mx[q] = std::max(mx[q], h[(size_t)s * 6 + 3 + q]);
+      if (per_sub) {
+        per_sub[(size_t)s * 6 + 2 * q] = std::sqrt(h[(size_t)s * 6 + q] / (Ps * ncomp[q]));
+        per_sub[(size_t)s * 6 + 2 * q + 1] = h[(size_t)s * 6 + 3 + q];
+      }
+    }
+  }
+  for (int q = 0; q < 3; ++q) { out[2 * q] = std::sqrt(sum[q] / ((double)pl.P * ncomp[q])); out[2 * q + 1] = mx[q]; }
+  return GH_OK;
+}
+
+// ------------------------------------------------------------------------------------------------------
+// profiling / bookkeeping
+// ------------------------------------------------------------------------------------------------------
+extern "C" gh_status gh_set_profiling(gh_domain* d, int enabled) {
+  if (!d) return GH_ERR_ARG;
+  drain_profile(d);
+  d->prof = enabled != 0;
+  return GH_OK;
+}
+
+extern "C" gh_status gh_profile_read(gh_domain* d, double* ms, int64_t* counts) {
+  if (!d) return GH_ERR_ARG;
+  drain_profile(d);
+  for (int k = 0; k < GH_NUM_KERNELS; ++k) { if (ms) ms[k] = d->prof_ms[k]; if (counts) counts[k] = d->prof_n[k]; }
+  return GH_OK;
+}
+
+extern "C" gh_status gh_profile_reset(gh_domain* d) {
+  if (!d) return GH_ERR_ARG;
+  drain_profile(d);
+  for (int k = 0; k < GH_NUM_KERNELS; ++k) { d->prof_ms[k] = 0; d->prof_n[k] = 0; }
+  return GH_OK;
+}
+
+extern "C" const char* gh_kernel_name(int k) {
+  static const char* names[GH_NUM_KERNELS] = {"k_cheb", "k_ang", "k_rhs", "k_rk", "k_con", "k_con_reduce", "k_jac", "other"};
+  return (k >= 0 && k < GH_NUM_KERNELS) ? names[k] : "?";
+}
+
+extern "C" int64_t gh_launch_count(const gh_domain* d) { return d ? d->launches : 0; }
+
+extern "C" const char* gh_last_error(const gh_domain* d) { return d ? d->err.c_str() : g_create_error.c_str(); }

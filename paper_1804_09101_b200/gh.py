@@ -1,0 +1,331 @@
+"""Thin Python binding of the C ABI in include/gh.h (argument marshalling only).
+
+Every step of the path runs in the CUDA kernels of libgh.so.  PyTorch is used for device memory
+(the workspace and I/O tensors) and the CUDA stream, nothing else.  There is no CPU fallback: if
+libgh.so is missing the import of the library fails loudly (``GHError``), and without a CUDA
+device ``gh_domain_create`` returns GH_ERR_CUDA.
+
+The module-level functions carry the names of the C entry points; ``Domain`` is a convenience
+wrapper that owns the workspace tensor and the handle.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libgh.so")
+
+GH_NCOMP = 50
+GH_NUM_KERNELS = 8
+GH_OK, GH_ERR_ARG, GH_ERR_WORKSPACE, GH_ERR_CUDA, GH_ERR_STATE, GH_ERR_SINGULAR = range(6)
+STATUS_NAMES = ["GH_OK", "GH_ERR_ARG", "GH_ERR_WORKSPACE", "GH_ERR_CUDA", "GH_ERR_STATE", "GH_ERR_SINGULAR"]
+
+# every symbol include/gh.h declares (checked by tests/test_abi.py)
+EXPORTS = [
+    "gh_workspace_bytes", "gh_domain_create", "gh_domain_destroy", "gh_domain_layout", "gh_domain_coords",
+    "gh_set_fields", "gh_get_fields", "gh_set_gauge_source", "gh_rhs", "gh_gradient", "gh_rk_step",
+    "gh_constraint_norms", "gh_set_profiling", "gh_profile_read", "gh_profile_reset", "gh_kernel_name",
+    "gh_launch_count", "gh_last_error", "gh_basis_cheb", "gh_basis_gauss_legendre", "gh_basis_shell",
+]
+
+
+class GHError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(f"{STATUS_NAMES[status] if 0 <= status < 6 else status}: {message}")
+        self.status = status
+
+
+class gh_subdomain_desc(C.Structure):
+    _fields_ = [
+        ("kind", C.c_int32),
+        ("n", C.c_int32 * 3),
+        ("lo", C.c_double * 3),
+        ("hi", C.c_double * 3),
+        ("center", C.c_double * 3),
+        ("face", C.c_int32 * 6),
+        ("gamma", C.c_double * 3),
+    ]
+
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """Load libgh.so (built in-tree by paper_1804_09101_b200.build).  Raises if it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise GHError(GH_ERR_STATE, f"{LIB_PATH} is missing: run `python -m paper_1804_09101_b200.build` "
+                                    "(there is no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    vp, dp, ip = C.c_void_p, C.c_void_p, C.c_int
+    descp = C.POINTER(gh_subdomain_desc)
+    L.gh_workspace_bytes.restype = C.c_size_t
+    L.gh_workspace_bytes.argtypes = [descp, C.c_int32]
+    L.gh_domain_create.argtypes = [descp, C.c_int32, vp, C.c_size_t, vp, C.POINTER(vp)]
+    L.gh_domain_destroy.restype = None
+    L.gh_domain_destroy.argtypes = [vp]
+    L.gh_domain_layout.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
+    L.gh_domain_coords.argtypes = [vp, dp, ip]
+    L.gh_set_fields.argtypes = [vp, dp, ip, C.c_double]
+    L.gh_get_fields.argtypes = [vp, dp, ip, C.POINTER(C.c_double)]
+    L.gh_set_gauge_source.argtypes = [vp, dp, dp, ip]
+    L.gh_rhs.argtypes = [vp, dp, ip]
+    L.gh_gradient.argtypes = [vp, dp, ip]
+    L.gh_rk_step.argtypes = [vp, C.c_double]
+    L.gh_constraint_norms.argtypes = [vp, dp, dp]
+    L.gh_set_profiling.argtypes = [vp, ip]
+    L.gh_profile_read.argtypes = [vp, dp, dp]
+    L.gh_profile_reset.argtypes = [vp]
+    L.gh_kernel_name.restype = C.c_char_p
+    L.gh_kernel_name.argtypes = [ip]
+    L.gh_launch_count.restype = C.c_int64
+    L.gh_launch_count.argtypes = [vp]
+    L.gh_last_error.restype = C.c_char_p
+    L.gh_last_error.argtypes = [vp]
+    L.gh_basis_cheb.argtypes = [C.c_int32, dp, dp]
+    L.gh_basis_gauss_legendre.argtypes = [C.c_int32, dp, dp]
+    L.gh_basis_shell.argtypes = [C.c_int32, dp, dp, dp, dp]
+    _lib = L
+    return L
+
+
+def make_descs(descs):
+    """list of descriptor dicts (configs.py) -> ctypes array of gh_subdomain_desc."""
+    arr = (gh_subdomain_desc * len(descs))()
+    for s, d in enumerate(descs):
+        e = arr[s]
+        e.kind = 0 if d["kind"] == "shell" else 1
+        n = list(d["n"]) + [0] * (3 - len(d["n"]))
+        lo = list(d["lo"]) + [0.0] * (3 - len(d["lo"]))
+        hi = list(d["hi"]) + [0.0] * (3 - len(d["hi"]))
+        ce = list(d.get("center", [0.0, 0.0, 0.0]))
+        fa = list(d.get("face", [])) + [0] * (6 - len(d.get("face", [])))
+        ga = list(d.get("gamma", [1.0, -1.0, 1.0]))
+        for i in range(3):
+            e.n[i], e.lo[i], e.hi[i], e.center[i], e.gamma[i] = int(n[i]), float(lo[i]), float(hi[i]), float(ce[i]), float(ga[i])
+        for i in range(6):
+            e.face[i] = int(fa[i])
+    return arr
+
+
+def _ptr(a):
+    """Raw address + on_device flag of a numpy array (HOST) or a torch CUDA tensor (DEVICE)."""
+    if a is None:
+        return None, 0
+    if isinstance(a, np.ndarray):
+        if a.dtype != np.float64 or not a.flags["C_CONTIGUOUS"]:
+            raise ValueError("host buffers must be C-contiguous float64")
+        return a.ctypes.data, 0
+    import torch
+
+    if isinstance(a, torch.Tensor):
+        if a.dtype != torch.float64 or not a.is_contiguous():
+            raise ValueError("tensors must be contiguous float64")
+        return a.data_ptr(), (1 if a.is_cuda else 0)
+    raise TypeError(type(a))
+
+
+def _check(status: int, handle=None):
+    if status != GH_OK:
+        msg = lib().gh_last_error(handle)
+        raise GHError(status, msg.decode() if msg else "")
+
+
+# ---- same-name wrappers of the C entry points ---------------------------------------------------
+def gh_workspace_bytes(descs) -> int:
+    arr = make_descs(descs)
+    n = lib().gh_workspace_bytes(arr, len(descs))
+    if n == 0:
+        _check(GH_ERR_ARG, None)
+    return int(n)
+
+
+def gh_domain_create(descs, workspace_ptr: int, nbytes: int, stream: int):
+    arr = make_descs(descs)
+    h = C.c_void_p()
+    _check(lib().gh_domain_create(arr, len(descs), workspace_ptr, nbytes, stream, C.byref(h)), None)
+    return h
+
+
+def gh_domain_destroy(h):
+    lib().gh_domain_destroy(h)
+
+
+def gh_domain_layout(h, n_sub: int):
+    P, S = C.c_int64(), C.c_int64()
+    off = (C.c_int64 * (n_sub + 1))()
+    _check(lib().gh_domain_layout(h, C.byref(P), C.byref(S), off), h)
+    return int(P.value), int(S.value), [int(v) for v in off]
+
+
+def gh_domain_coords(h, xyz):
+    p, dev = _ptr(xyz)
+    _check(lib().gh_domain_coords(h, p, dev), h)
+
+
+def gh_set_fields(h, u, t: float = 0.0):
+    p, dev = _ptr(u)
+    _check(lib().gh_set_fields(h, p, dev, float(t)), h)
+
+
+def gh_get_fields(h, u) -> float:
+    p, dev = _ptr(u)
+    t = C.c_double()
+    _check(lib().gh_get_fields(h, p, dev, C.byref(t)), h)
+    return float(t.value)
+
+
+def gh_set_gauge_source(h, H, dH=None):
+    p, dev = _ptr(H)
+    q, dev2 = _ptr(dH)
+    if dH is not None and dev != dev2:
+        raise ValueError("H and dH must live on the same side")
+    _check(lib().gh_set_gauge_source(h, p, q, dev), h)
+
+
+def gh_rhs(h, dtu):
+    p, dev = _ptr(dtu)
+    _check(lib().gh_rhs(h, p, dev), h)
+
+
+def gh_gradient(h, du):
+    p, dev = _ptr(du)
+    _check(lib().gh_gradient(h, p, dev), h)
+
+
+def gh_rk_step(h, dt: float):
+    _check(lib().gh_rk_step(h, float(dt)), h)
+
+
+def gh_constraint_norms(h, n_sub: int, per_sub: bool = False):
+    out = np.zeros((3, 2))
+    ps = np.zeros((n_sub, 3, 2)) if per_sub else None
+    _check(lib().gh_constraint_norms(h, out.ctypes.data, ps.ctypes.data if per_sub else None), h)
+    return (out, ps) if per_sub else out
+
+
+def gh_basis_cheb(N: int):
+    x, D = np.zeros(N), np.zeros((N, N))
+    _check(lib().gh_basis_cheb(N, x.ctypes.data, D.ctypes.data), None)
+    return x, D
+
+
+def gh_basis_gauss_legendre(L: int):
+    th, w = np.zeros(L + 1), np.zeros(L + 1)
+    _check(lib().gh_basis_gauss_legendre(L, th.ctypes.data, w.ctypes.data), None)
+    return th, w
+
+
+def gh_basis_shell(L: int):
+    nt, npp, nq = L + 1, 2 * L + 2, 2 * L + 1
+    Fa, Fs = np.zeros((nq, npp)), np.zeros((npp, nq))
+    Th, Pr = np.zeros((L + 1, nt, nt)), np.zeros((L + 1, nt, nt))
+    _check(lib().gh_basis_shell(L, Fa.ctypes.data, Fs.ctypes.data, Th.ctypes.data, Pr.ctypes.data), None)
+    return Fa, Fs, Th, Pr
+
+
+# ---- convenience wrapper -------------------------------------------------------------------------
+class Domain:
+    """Owns the device workspace (a torch uint8 tensor) and the gh_domain handle."""
+
+    def __init__(self, descs, device: str = "cuda:0", stream=None):
+        import torch
+
+        self.torch = torch
+        self.descs = list(descs)
+        self.n_sub = len(self.descs)
+        self.device = torch.device(device)
+        nbytes = gh_workspace_bytes(self.descs)
+        self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        base = self.workspace.data_ptr()
+        aligned = (base + 255) // 256 * 256
+        with torch.cuda.device(self.device):
+            self.stream = stream if stream is not None else torch.cuda.current_stream()
+            self.h = gh_domain_create(self.descs, aligned, nbytes, self.stream.cuda_stream)
+        self.P, self.S, self.offsets = gh_domain_layout(self.h, self.n_sub)
+        self.sizes = [self._npts(d) for d in self.descs]
+
+    @staticmethod
+    def _npts(d):
+        if d["kind"] == "shell":
+            return d["n"][0] * (d["n"][1] + 1) * (2 * d["n"][1] + 2)
+        return d["n"][0] * d["n"][1] * d["n"][2]
+
+    def close(self):
+        if getattr(self, "h", None) is not None:
+            gh_domain_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # layout helpers (host, numpy): per-subdomain lists <-> the padded [C][S] store
+    def pack(self, parts) -> np.ndarray:
+        ncomp = parts[0].shape[0]
+        out = np.zeros((ncomp, self.S))
+        for s, a in enumerate(parts):
+            out[:, self.offsets[s]:self.offsets[s] + self.sizes[s]] = a
+        return out
+
+    def unpack(self, arr):
+        arr = np.asarray(arr)
+        return [np.ascontiguousarray(arr[..., self.offsets[s]:self.offsets[s] + self.sizes[s]]) for s in range(self.n_sub)]
+
+    def coords(self):
+        xyz = np.zeros((3, self.S))
+        gh_domain_coords(self.h, xyz)
+        return self.unpack(xyz)
+
+    def empty(self, *lead):
+        return self.torch.empty(*lead, self.S, dtype=self.torch.float64, device=self.device)
+
+    def set_fields(self, u, t: float = 0.0):
+        gh_set_fields(self.h, u, t)
+
+    def get_fields(self, out=None):
+        out = np.zeros((GH_NCOMP, self.S)) if out is None else out
+        gh_get_fields(self.h, out)
+        return out
+
+    def set_gauge_source(self, H, dH=None):
+        gh_set_gauge_source(self.h, H, dH)
+
+    def rhs(self, out=None):
+        out = np.zeros((GH_NCOMP, self.S)) if out is None else out
+        gh_rhs(self.h, out)
+        return out
+
+    def gradient(self, out=None):
+        out = np.zeros((3, GH_NCOMP, self.S)) if out is None else out
+        gh_gradient(self.h, out)
+        return out
+
+    def rk_step(self, dt: float):
+        gh_rk_step(self.h, dt)
+
+    def constraint_norms(self, per_sub: bool = False):
+        return gh_constraint_norms(self.h, self.n_sub, per_sub)
+
+    def set_profiling(self, on: bool):
+        _check(lib().gh_set_profiling(self.h, int(on)), self.h)
+
+    def profile_reset(self):
+        _check(lib().gh_profile_reset(self.h), self.h)
+
+    def profile_read(self):
+        ms = np.zeros(GH_NUM_KERNELS)
+        cnt = np.zeros(GH_NUM_KERNELS, dtype=np.int64)
+        _check(lib().gh_profile_read(self.h, ms.ctypes.data, cnt.ctypes.data), self.h)
+        names = [lib().gh_kernel_name(k).decode() for k in range(GH_NUM_KERNELS)]
+        return {names[k]: (float(ms[k]), int(cnt[k])) for k in range(GH_NUM_KERNELS)}
+
+    def launch_count(self) -> int:
+        return int(lib().gh_launch_count(self.h))

@@ -1,0 +1,138 @@
+"""GPU parity: the CUDA path (through the C ABI) against the long-double CPU oracle, element by element, on the
+same seeded inputs.  Bar (BASELINE.json north_star, reading S15): max |gpu - oracle| <= 1e-11 * max(||X||inf,
+||d_t X||inf) per field X in (psi, Pi, Phi)."""
+import numpy as np
+import pytest
+
+from paper_1804_09101_b200 import configs, gh
+from domain_util import assert_parity, build_case, field_errors
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-11
+
+
+def _domain(descs, Hs, us):
+    dom = gh.Domain(descs)
+    dom.set_gauge_source(dom.pack(Hs))
+    dom.set_fields(dom.pack(us), 0.0)
+    return dom
+
+
+def _mini_mixed():
+    """a shell with ragged tiles next to a non-cubic block: exercises padding, multiple tiles and tails."""
+    return {"id": 7, "spin": 0.3, "amplitude": 1e-3,
+            "descs": [configs.shell(7, 5, 2.2, 4.0, face=(0, 1), gamma=[3.0, -1.0, 2.0]),
+                      configs.block([9, 6, 11], (3.0, -1.0, -2.0), (5.0, 1.5, 1.0), face=(1, 0, 0, 1, 0, 0), gamma=[0.5, -0.3, 0.7]),
+                      configs.shell(5, 9, 4.0, 9.0, face=(1, 1), center=(0.1, -0.2, 0.05))]}
+
+
+CASES = {"c1": configs.c1, "c2": configs.c2, "mixed": _mini_mixed}
+
+
+@pytest.fixture(scope="module", params=list(CASES))
+def case(request, oracle):
+    cfg = CASES[request.param]()
+    descs, coords, us, Hs = build_case(cfg, oracle)
+    dom = _domain(descs, Hs, us)
+    yield request.param, cfg, descs, coords, us, Hs, dom
+    dom.close()
+
+
+def test_layout_and_coords(case, oracle):
+    name, cfg, descs, coords, us, Hs, dom = case
+    assert dom.P == sum(c.shape[1] for c in coords)
+    assert all(o % 16 == 0 for o in dom.offsets) and dom.S == dom.offsets[-1]
+    for xyz_gpu, xyz in zip(dom.coords(), coords):
+        assert np.max(np.abs(xyz_gpu - xyz)) <= 4e-15 * max(1.0, np.max(np.abs(xyz)))
+
+
+def test_fields_round_trip(case):
+    name, cfg, descs, coords, us, Hs, dom = case
+    back = dom.unpack(dom.get_fields())
+    for a, b in zip(back, us):
+        assert np.array_equal(a, b)
+
+
+def test_gradient_parity(case, oracle):
+    name, cfg, descs, coords, us, Hs, dom = case
+    g = dom.gradient()
+    for s, d in enumerate(descs):
+        ref = oracle.gradient(d, us[s])
+        got = g[:, :, dom.offsets[s]:dom.offsets[s] + dom.sizes[s]]
+        for k in range(3):
+            assert_parity(got[k], ref[k], state=us[s], tol=TOL, what=f"{name} sub {s} d_{k}")
+
+
+def test_rhs_parity(case, oracle):
+    name, cfg, descs, coords, us, Hs, dom = case
+    k = dom.unpack(dom.rhs())
+    for s, d in enumerate(descs):
+        ref = oracle.rhs(d, us[s], Hs[s])
+        assert_parity(k[s], ref, state=us[s], tol=TOL, what=f"{name} sub {s} rhs")
+        # frozen faces are exactly zero on both sides
+        assert np.array_equal(k[s] == 0.0, ref == 0.0) or np.all((ref == 0.0) <= (k[s] == 0.0))
+
+
+def test_rhs_device_output_matches_host_output(case):
+    name, cfg, descs, coords, us, Hs, dom = case
+    host = dom.rhs()
+    dev = dom.empty(50)
+    dev.zero_()
+    dom.rhs(dev)
+    got = dev.cpu().numpy()
+    for s in range(dom.n_sub):
+        sl = slice(dom.offsets[s], dom.offsets[s] + dom.sizes[s])
+        assert np.array_equal(got[:, sl], host[:, sl])
+
+
+def test_rk_step_parity(case, oracle):
+    name, cfg, descs, coords, us, Hs, dom = case
+    dt = 0.25 * configs.min_spacing(descs)
+    dom.set_fields(dom.pack(us), 0.0)
+    dom.rk_step(dt)
+    new = dom.unpack(dom.get_fields())
+    for s, d in enumerate(descs):
+        ref = oracle.rk3(d, us[s], Hs[s], dt, 1)
+        assert_parity(new[s], ref, tol=TOL, what=f"{name} sub {s} rk3")
+        # the step must actually have moved the state by about dt * rhs
+        assert np.max(np.abs(ref - us[s])) > 0
+    dom.set_fields(dom.pack(us), 0.0)
+
+
+def test_constraint_norms_parity(case, oracle):
+    name, cfg, descs, coords, us, Hs, dom = case
+    dom.set_fields(dom.pack(us), 0.0)
+    got, per = dom.constraint_norms(per_sub=True)
+    ref = oracle.constraint_norms(descs, us, Hs)
+    # norms of O(amplitude) quantities: compare relative to the norm, with an absolute floor from the derivative rounding
+    floor = 1e-11 * max(np.max(np.abs(u)) for u in us)
+    assert np.all(np.abs(got - ref) <= 1e-9 * np.abs(ref) + floor), (got, ref)
+    for s, d in enumerate(descs):
+        sums, maxs, _ = oracle.constraints(d, us[s], Hs[s])
+        rms = np.sqrt(sums / (us[s].shape[1] * np.array([4.0, 30.0, 30.0])))
+        assert np.all(np.abs(per[s, :, 0] - rms) <= 1e-9 * rms + floor)
+        assert np.all(np.abs(per[s, :, 1] - maxs) <= 1e-9 * maxs + floor)
+
+
+def test_singular_data_raises_flag(oracle):
+    cfg = configs.c1()
+    descs, coords, us, Hs = build_case(cfg, oracle)
+    dom = _domain(descs, Hs, us)
+    bad = [u.copy() for u in us]
+    bad[0][0, 5] = +3.0      # psi_tt > 0 with small shift: lapse^2 <= 0 at one point
+    dom.set_fields(dom.pack(bad), 0.0)
+    with pytest.raises(gh.GHError) as e:
+        dom.rhs()
+    assert e.value.status == gh.GH_ERR_SINGULAR
+    dom.set_fields(dom.pack(us), 0.0)
+    dom.rhs()    # flag was cleared
+    dom.close()
+
+
+def test_state_errors():
+    dom = gh.Domain(configs.c1()["descs"])
+    with pytest.raises(gh.GHError) as e:
+        dom.rhs()
+    assert e.value.status == gh.GH_ERR_STATE
+    dom.close()
