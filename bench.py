@@ -1,0 +1,489 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the GH right-hand-side hot path (arXiv 1804.09101) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload c4|c3|c2|c1]
+
+Metric (BASELINE.json): GH RHS grid-point evaluations per second, FP64.  One "step" is one pass of the whole
+hot path (rows A2-A8) over the workload: one `gh_rk_step` (3 x [Chebyshev + angular derivatives,
+fused Jacobian + pointwise RHS + face mask] + 3 fused RK3 stage updates) followed by one `gh_constraint_norms`
+(derivatives + constraint kernel + reduction).  value = 3 * P * K / T: only the three RHS evaluations of the RK3
+step are counted as "evaluations"; the constraint pass is extra work inside the timed region.
+
+Default workload: C4 (BASELINE.json configs[3], the production-like isolated-BH domain: 40 shells + 24 cube
+blocks, spin 0.9, replicated to >= 4M points, reading S13) - the configuration the HBM-roofline part of the
+metric is meaningful on (C1/C2 are L2-resident latency cases).  All inputs are seeded and synthetic
+(analytic Kerr-Schild data + smooth seeded perturbations).
+
+N > 1 (torchrun): the path does not shard inside one call ("replicas only"): every rank runs its own
+replica of the workload on its own GPU, no data-path collective; value = N * 3 * P * K / max-over-ranks(T).
+
+`--impl reference` times the CPU oracle (oracle/, test infrastructure, as it stands) on a bounded sample of the
+same workload on the host cores; rank 0 only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "gh_rhs_grid_point_evals_per_s"
+UNIT = "points/s"
+
+# algorithmic traffic per grid point and launch, DESIGN.md §5
+BYTES_RHS_PT = (50 + 150 + 4 + 12 + 50) * 8      # k_rhs: 216 reads (+ table lookups, cached) + 50 writes = 2 128 B
+BYTES_RK_PT = {True: (3 + 1) * 50 * 8, False: (2 + 1) * 50 * 8}   # k_rk: u0?, u_s, k -> out
+FLOP_RHS_PT = 4391                                # SURVEY.md §8(a) A4+A5 instrumented count
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+# FP64 FMA-pipe peak for the derivative kernels: 148 SMs x 64 DFMA lanes x 2 flop x clock.  Quoted at
+# the max SM clock; the clock actually held is in the "clocks" key.
+def fp64_peak_tflops(sm_mhz: float = 1965.0) -> float:
+    return 148 * 64 * 2 * sm_mhz * 1e6 / 1e12
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# workload construction (host, numpy; seeded)
+# ------------------------------------------------------------------------------------------------------------------
+def make_config(name: str, min_points: int):
+    from paper_1804_09101_b200 import configs
+
+    if name == "c4":
+        cfg = configs.c4(min_points=min_points)
+        base = configs.c4(replicate=False)
+        label = (f"C4 production-like isolated-BH domain: {cfg['replicas']} x (40 shells N_r 12..24, L 12..32 + 24 cube "
+                 f"blocks N 16..32), Kerr-Schild a=0.9, perturbation 1e-5, one RK3 step + constraint norms")
+        return cfg, base, label
+    if name == "c3":
+        cfg = configs.c3()
+        return cfg, cfg, "C3 isolated Kerr BH a=0.7: 8 shells N_r=16 L=16, perturbation 1e-5, RK3 step + constraint norms"
+    if name == "c2":
+        cfg = configs.c2()
+        cfg["dt"] = 0.25 * configs.min_spacing(cfg["descs"])
+        return cfg, cfg, "C2 one 24^3 block, a=0.5 (L2-resident latency case)"
+    if name == "c1":
+        cfg = configs.c1()
+        cfg["dt"] = 0.25 * configs.min_spacing(cfg["descs"])
+        return cfg, cfg, "C1 one shell N_r=8 L=8, a=0 (L2-resident latency case)"
+    raise SystemExit(f"unknown workload {name}")
+
+
+def base_inputs(base_cfg, coords):
+    from paper_1804_09101_b200 import inputs
+
+    return inputs.initial_data(base_cfg["descs"], coords, base_cfg["spin"], base_cfg["amplitude"], base_cfg["id"])
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# clocks during the timed region (B200_PROFILING.md "clocks line")
+# ------------------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    QUERY = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.gpu = gpu_index
+        self.proc = None
+        self.lines = []
+        self.thread = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.gpu), f"--query-gpu={self.QUERY}", "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+            return
+        self.thread = threading.Thread(target=self._pump, daemon=True)
+        self.thread.start()
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        if self.thread is not None:
+            self.thread.join(timeout=2)
+        sm, smax, power, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); smax.append(float(f[1])); power.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(smax)), "power_w_max": float(max(power)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# the CPU oracle, timed on a bounded sample (cpu_baseline leg and --impl reference)
+# ------------------------------------------------------------------------------------------------------------------
+def oracle_sample(base_cfg, budget_points: int = 60_000):
+    """Pick subdomains of the workload (alternating shells / blocks, in order) until ~budget_points points."""
+    from paper_1804_09101_b200 import configs
+
+    descs = base_cfg["descs"]
+    shells = [s for s, d in enumerate(descs) if d["kind"] == "shell"]
+    blocks = [s for s, d in enumerate(descs) if d["kind"] == "block"]
+    order = []
+    for i in range(max(len(shells), len(blocks))):
+        if i < len(shells):
+            order.append(shells[i])
+        if i < len(blocks):
+            order.append(blocks[i])
+    pick, pts = [], 0
+    for s in order:
+        pick.append(s)
+        pts += configs.num_points(descs[s])
+        if pts >= budget_points:
+            break
+    return pick, pts
+
+
+def time_oracle(base_cfg, pick, steps: int, warmup: int):
+    """One 'step' = one oracle RHS evaluation (Real=double build, OpenMP) of every picked subdomain."""
+    from oracle.gh_oracle import Oracle
+    from paper_1804_09101_b200 import inputs
+
+    ora = Oracle("double")
+    descs = [base_cfg["descs"][s] for s in pick]
+    coords = [ora.coords(d) for d in descs]
+    us, Hs = [], []
+    for s, d, xyz in zip(pick, descs, coords):
+        u, H = inputs.initial_data([d], [xyz], base_cfg["spin"], base_cfg["amplitude"], base_cfg["id"])
+        us.append(u[0]); Hs.append(H[0])
+    pts = sum(u.shape[1] for u in us)
+    for _ in range(warmup):
+        ora.rhs(descs[0], us[0], Hs[0])
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        for d, u, H in zip(descs, us, Hs):
+            ora.rhs(d, u, H)
+    dt = time.perf_counter() - t0
+    try:
+        cores = len(os.sched_getaffinity(0))
+    except AttributeError:
+        cores = os.cpu_count() or 1
+    omp = os.environ.get("OMP_NUM_THREADS")
+    if omp:
+        cores = min(cores, int(omp))
+    return pts * steps / dt, dt / steps, cores, pts
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# algorithmic work per launch of each kernel, from the descriptors
+# ------------------------------------------------------------------------------------------------------------------
+def kernel_work(descs):
+    from paper_1804_09101_b200 import configs
+
+    P = sum(configs.num_points(d) for d in descs)
+    Ps = sum(configs.num_points(d) for d in descs if d["kind"] == "shell")
+    Pb = P - Ps
+    cheb_flop = ang_flop = 0.0
+    for d in descs:
+        p = configs.num_points(d)
+        if d["kind"] == "shell":
+            cheb_flop += 50.0 * p * (2 * d["n"][0] - 1)
+            ang_flop += 50.0 * p * 8 * (2 * d["n"][1] + 1)     # S1 + S2 + S3 of K_ang: 8 (2L+1) flop / point / component
+        else:
+            cheb_flop += 50.0 * p * sum(2 * n - 1 for n in d["n"])
+    return {
+        "P": P,
+        "k_rhs": {"bytes": float(BYTES_RHS_PT) * P, "flop": float(FLOP_RHS_PT) * P, "bound": "hbm"},
+        "k_rk": {"bytes": None, "flop": 200.0 * P, "bound": "hbm"},       # bytes depend on the stage, filled by the caller
+        "k_con": {"bytes": (50 + 120 + 4) * 8.0 * P, "flop": 1200.0 * P, "bound": "hbm"},
+        "k_cheb": {"bytes": 8.0 * (50 * Ps + 50 * Ps + 50 * Pb + 150 * Pb), "flop": cheb_flop, "bound": "alu"},
+        "k_ang": {"bytes": 8.0 * (50 + 100) * Ps, "flop": ang_flop, "bound": "alu"},
+    }
+
+
+def read_traffic(kernel: str, P: int):
+    """dram bytes per launch of `kernel` from the committed ncu summary profiles/ncu_traffic.csv
+    (columns: kernel,P,dram_bytes_per_launch; see profiles/README.md), if taken on this workload size; else None."""
+    p = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
+    if not os.path.exists(p):
+        return None
+    with open(p) as f:
+        for ln in f:
+            c = [x.strip() for x in ln.split(",")]
+            if len(c) >= 3 and c[0] == kernel:
+                try:
+                    if int(c[1]) == int(P):
+                        return float(c[2])
+                except ValueError:
+                    continue
+    return None
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# our arm
+# ------------------------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+
+    from paper_1804_09101_b200 import build as _build
+    from paper_1804_09101_b200 import gh
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the library has no CPU fallback (use --impl reference for the oracle)")
+    if rank == 0:
+        _build.build()
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_
+
+        dist = dist_
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
+        dist.barrier()
+    torch.cuda.set_device(local_rank)
+    dev = f"cuda:{local_rank}"
+
+    cfg, base, label = make_config(args.workload, args.min_points)
+    descs = cfg["descs"]
+    nbase = len(base["descs"])
+    reps = len(descs) // nbase
+    dom = gh.Domain(descs, device=dev)
+    P, S = dom.P, dom.S
+
+    # inputs: analytic data evaluated on the library's own grid (gh_domain_coords) for the base subdomain set,
+    # replicated (reading S13); every rank builds the same arrays (replicas)
+    coords = dom.coords()[:nbase]
+    us_b, Hs_b = base_inputs(base, coords)
+    u_host = torch.zeros(50, S, dtype=torch.float64).pin_memory()
+    H_host = np.zeros((4, S))
+    un = u_host.numpy()
+    for s in range(len(descs)):
+        o, n = dom.offsets[s], dom.sizes[s]
+        un[:, o:o + n] = us_b[s % nbase]
+        H_host[:, o:o + n] = Hs_b[s % nbase]
+    dom.set_gauge_source(H_host)
+    u_dev = torch.empty(50, S, dtype=torch.float64, device=dev)
+    u_dev.copy_(u_host)
+    dt = float(cfg["dt"])
+    work = kernel_work(descs)
+
+    def sync_all():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    def step():
+        dom.rk_step(dt)
+        return dom.constraint_norms()
+
+    # ---- device-resident timing -----------------------------------------------------------------------------
+    dom.set_fields(u_dev, 0.0)
+    for _ in range(args.warmup):
+        step()
+    dom.set_fields(u_dev, 0.0)
+    dom.set_profiling(True)
+    dom.profile_reset()
+    l0 = dom.launch_count()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    sync_all()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        norms = step()
+    e1.record()
+    sync_all()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop()
+    launches = dom.launch_count() - l0
+    prof = dom.profile_read()
+    dom.set_profiling(False)
+    if not np.all(np.isfinite(norms)):
+        raise SystemExit("bench.py: non-finite constraint norms after the timed region")
+
+    # ---- end to end through the C ABI with HOST buffers (pinned): H2D of the state, step, D2H of the state --------
+    out_host = torch.empty(50, S, dtype=torch.float64).pin_memory()
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    for _ in range(2):
+        dom.set_fields(u_host, 0.0); step(); dom.get_fields(out_host)
+    sync_all()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        dom.set_fields(u_host, 0.0)
+        step()
+        dom.get_fields(out_host)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    if not bool(torch.isfinite(out_host).all()):
+        raise SystemExit("bench.py: non-finite state after the e2e region")
+
+    tmax, e2emax = ms, e2e_s / e2e_steps
+    if dist is not None:
+        t = torch.tensor([ms, e2e_s / e2e_steps], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        tmax, e2emax = float(t[0]), float(t[1])
+    if rank != 0:
+        dom.close()
+        if dist is not None:
+            dist.barrier(); dist.destroy_process_group()
+        return
+    return finish_ours(args, world, label, cfg, descs, reps, P, S, tmax, e2emax, e2e_steps, launches, prof, work, clocks,
+                       norms, base, dom, dist)
+
+
+def finish_ours(args, world, label, cfg, descs, reps, P, S, ms, e2e_step_s, e2e_steps, launches, prof, work, clocks,
+                norms, base, dom, dist):
+    hbm_peak, peak_src = load_peaks()
+    steps = args.steps
+    value = world * 3.0 * P * steps / (ms * 1e-3)
+    # per-kernel numbers from the CUDA events the library records around each launch on its own stream
+    work["k_rk"]["bytes"] = P * (BYTES_RK_PT[False] + 2 * BYTES_RK_PT[True]) / 3.0
+    total_kernel_ms = sum(v[0] for v in prof.values()) or 1.0
+    kernels = {}
+    for name, (kms, cnt) in prof.items():
+        if cnt == 0:
+            continue
+        per = kms / cnt
+        e = {"launches_per_step": cnt / steps, "ms_per_launch": per, "share_of_kernel_time": kms / total_kernel_ms}
+        w = work.get(name)
+        if w:
+            e["achieved_GBps"] = w["bytes"] / (per * 1e-3) / 1e9
+            e["achieved_TFLOPs"] = w["flop"] / (per * 1e-3) / 1e12
+            e["bound"] = w["bound"]
+        kernels[name] = e
+    top = max((k for k in kernels if k in work), key=lambda k: kernels[k]["share_of_kernel_time"])
+    fp64_peak = fp64_peak_tflops()
+    if work[top]["bound"] == "hbm":
+        roof = {"kernel": top, "bound": "hbm", "achieved": kernels[top]["achieved_GBps"], "peak": hbm_peak, "unit": "GB/s",
+                "frac": kernels[top]["achieved_GBps"] / hbm_peak, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": work[top]["bytes"], "traffic": read_traffic(top, P)}
+    else:
+        roof = {"kernel": top, "bound": "alu", "achieved": kernels[top]["achieved_TFLOPs"], "peak": fp64_peak, "unit": "TFLOP/s",
+                "frac": kernels[top]["achieved_TFLOPs"] / fp64_peak,
+                "peak_source": "derived: 148 SM x 64 FP64 FMA lanes x 2 x 1.965 GHz (DESIGN.md §5)",
+                "algorithmic_flop_per_launch": work[top]["flop"], "traffic": read_traffic(top, P)}
+    # the fused RHS kernel is the one north_star sets a target for: always report it too
+    roof_rhs = None
+    if "k_rhs" in kernels:
+        roof_rhs = {"achieved": kernels["k_rhs"]["achieved_GBps"], "peak": hbm_peak, "unit": "GB/s",
+                    "frac": kernels["k_rhs"]["achieved_GBps"] / hbm_peak, "frac_of_8TBps_nominal": kernels["k_rhs"]["achieved_GBps"] / 8000.0,
+                    "traffic": read_traffic("k_rhs", P)}
+
+    cpu = None
+    if not args.no_cpu_baseline:
+        pick, _ = oracle_sample(base, args.cpu_points)
+        v, s_per, cores, pts = time_oracle(base, pick, 1, 1)
+        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": f"one oracle RHS evaluation (Real=double build, OpenMP) of subdomains {pick} of the workload's base set "
+                         f"({pts} points, {s_per:.1f} s)"}
+
+    h2d = 50 * S * 8
+    d2h = 50 * S * 8 + 6 * 8
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": args.warmup,
+        "ms_per_step": ms / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": label, "points_per_gpu": P, "subdomains": len(descs), "replicas_of_base_set": reps,
+                   "components": 50, "dt": float(cfg["dt"]), "rhs_evals_per_step": 3,
+                   "step": "gh_rk_step + gh_constraint_norms", "parallelism": "replicas only" if world > 1 else "single GPU",
+                   "l2": f"inputs larger than L2: the step streams {316 * S * 8 / 1e9:.2f} GB of state/derivative arrays (L2 126 MB)",
+                   "per_launch_events": "on (library CUDA events around every kernel launch, inside the timed region)"},
+        "rk_steps_per_s": world * steps / (ms * 1e-3),
+        "gpu_launches": int(launches),
+        "roofline": roof, "roofline_k_rhs": roof_rhs, "kernels": kernels,
+        "cpu_baseline": cpu,
+        "e2e": {"value": world * 3.0 * P / e2e_step_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "steps": e2e_steps, "ms_per_step": e2e_step_s * 1e3,
+                "path": "gh_set_fields(HOST pinned) + gh_rk_step + gh_constraint_norms + gh_get_fields(HOST pinned)"},
+        "clocks": clocks,
+        "constraint_norms_after": [[float(x) for x in r] for r in np.asarray(norms)],
+    }
+    print(json.dumps(out))
+    sys.stdout.flush()
+    dom.close()
+    if dist is not None:
+        dist.barrier(); dist.destroy_process_group()
+    return out
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# reference arm: the CPU oracle as it stands
+# ------------------------------------------------------------------------------------------------------------------
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import gh_oracle
+
+    gh_oracle.build()
+    cfg, base, label = make_config(args.workload, args.min_points)
+    pick, _ = oracle_sample(base, args.ref_points)
+    v, s_per, cores, pts = time_oracle(base, pick, args.steps, min(args.warmup, 1))
+    sample = (f"each step = one oracle RHS evaluation (Real=double build, OpenMP) of subdomains {pick} of the workload's base set "
+              f"({pts} points)")
+    out = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": s_per * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "dtype": "f64", "data": "synthetic", "config": {"workload": label, "sample": sample},
+           "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+           "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c4", choices=["c1", "c2", "c3", "c4"])
+    ap.add_argument("--min-points", type=int, default=4_000_000, help="C4: replicate the base set until P >= this")
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--cpu-points", type=int, default=250_000, help="points in the cpu_baseline sample (~10-30 s)")
+    ap.add_argument("--ref-points", type=int, default=60_000, help="points per step of --impl reference")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -283,7 +283,7 @@ def shell_perturbation(r_lo, r_hi, center, xyz, amplitude, seed, kmax=4, lmax=4)
     out = np.empty((N_COMP, r.shape[0]))
     for c in range(N_COMP):
         coef = rng.uniform(K * S).reshape(K, S)
-        f = np.einsum("ks,kp,sp->p", coef, T, Y)
+        f = ((coef @ Y) * T).sum(0)          # sum_k T_k(x) sum_s c_ks Y_s
         out[c] = f * (amplitude / np.max(np.abs(f)))
     return out
 
@@ -298,7 +298,9 @@ def block_perturbation(lo, hi, xyz, amplitude, seed, deg=6) -> np.ndarray:
     out = np.empty((N_COMP, xyz.shape[1]))
     for c in range(N_COMP):
         coef = rng.uniform(n * n * n).reshape(n, n, n)
-        f = np.einsum("ijk,ip,jp,kp->p", coef, T[0], T[1], T[2])
+        f = (coef.reshape(n * n, n) @ T[2]).reshape(n, n, -1)   # sum over k
+        f = (f * T[1][None]).sum(1)                               # sum over j
+        f = (f * T[0]).sum(0)                                     # sum over i
         out[c] = f * (amplitude / np.max(np.abs(f)))
     return out
 
