@@ -45,7 +45,10 @@ struct AngItem {
   int32_t L;
   int32_t plane0;
   int32_t nplanes;
-  int32_t m_Fa, m_Fs, m_Fp, m_Th, m_Pr;   // offsets (doubles) of the shell matrices in the table memory
+  int32_t nb_alloc;              // planes the shared-memory layout is sized for (>= nplanes)
+  int32_t m_Fa, m_Fs, m_TP;      // offsets (doubles) in the table memory: Fa [nq][np], Fs [np][nq], and the per-m
+                                 // [Th_m ; m Pr_m] matrices in DMMA fragment order [m][part][m_tile][k_step][32]
+  int32_t pad_;
 };
 
 }  // namespace ghd

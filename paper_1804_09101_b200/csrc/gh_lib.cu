@@ -23,7 +23,8 @@ namespace {
 
 constexpr int CHEB_TPB = 64, CHEB_CPT = 4, CHEB_CT = CHEB_TPB * CHEB_CPT;   // lines per K_cheb tile
 constexpr int ANG_TPB = 256;
-constexpr size_t ANG_SMEM_TARGET = 100 * 1024;   // planes per K_ang CTA are chosen to stay under this
+constexpr size_t ANG_SMEM_2CTA = 113 * 1024;     // K_ang shared memory that still lets two CTAs share an SM
+constexpr int ANG_NB_MAX = 8;                    // planes per K_ang CTA (S2 holds 2*nb <= 16 columns per m)
 constexpr size_t SMEM_MAX = 227 * 1024;
 
 thread_local std::string g_create_error;
@@ -44,8 +45,10 @@ struct Plan {
   int n_tiles = 0;
   size_t table_doubles = 0;
   int n_cheb_items = 0, n_cheb_items_r = 0, n_ang_items = 0;
-  size_t cheb_smem = 0, ang_smem = 0;
+  int n_ang_class[2] = {0, 0};           // K_ang items per shared-memory class (0: two CTAs per SM, 1: one)
+  size_t cheb_smem = 0, ang_smem[2] = {0, 0};
   std::vector<int> ang_pb;               // planes per CTA for each subdomain (0 for blocks)
+  std::vector<int> ang_class;            // shared-memory class of each shell
   // workspace offsets (bytes)
   size_t o_ua, o_ub, o_k, o_du, o_H, o_dH, o_tables, o_subs, o_tiles, o_cheb, o_ang, o_part, o_persub, o_flag, total;
 };
@@ -55,10 +58,18 @@ inline void sub_dims(const gh_subdomain_desc& d, int& n0, int& n1, int& n2) {
   else { n0 = d.n[0]; n1 = d.n[1]; n2 = d.n[2]; }
 }
 
-inline size_t ang_plane_smem(int L) { return (size_t)(L + 1) * ((2 * L + 2) + 2 * (2 * L + 1)) * sizeof(double); }
+// K_ang shared memory for nb planes of band limit L: X and Y ([nb][plane stride]) + F ([n_phi rounded to 8][pitch])
+inline size_t ang_smem_bytes(int L, int nb) {
+  const size_t np8 = (size_t)((2 * L + 2 + 7) / 8 * 8);
+  return (2 * (size_t)nb * ang_plane_stride(L) + np8 * ang_pitch(L)) * sizeof(double);
+}
+inline size_t shell_tp_doubles(int L) {   // [m][part][m_tile][k_step][32], see AngItem
+  const size_t nt = L + 1, mtn = (nt + 7) / 8, ks = (nt + 3) / 4;
+  return (size_t)(L + 1) * 2 * mtn * ks * 32;
+}
 inline size_t shell_matrix_doubles(int L) {
-  size_t nt = L + 1, np = 2 * L + 2, nq = 2 * L + 1;
-  return 3 * nq * np + 2 * (size_t)(L + 1) * nt * nt;
+  size_t np = 2 * L + 2, nq = 2 * L + 1;
+  return 2 * nq * np + shell_tp_doubles(L);
 }
 
 bool validate(const gh_subdomain_desc* descs, int32_t n_sub, std::string& err) {
@@ -94,6 +105,7 @@ bool make_plan(const gh_subdomain_desc* descs, int32_t n_sub, Plan& pl, std::str
   pl.offsets.assign(n_sub + 1, 0);
   pl.tile_first.assign(n_sub + 1, 0);
   pl.ang_pb.assign(n_sub, 0);
+  pl.ang_class.assign(n_sub, 0);
   std::map<int, int> seenL;
   size_t tab = 0;
   int64_t off = 0, tiles = 0;
@@ -120,13 +132,16 @@ bool make_plan(const gh_subdomain_desc* descs, int32_t n_sub, Plan& pl, std::str
       const int L = d.n[1];
       tab += (size_t)round_up(n0, 2) + 2 * (size_t)round_up(n1, 2) + 2 * (size_t)round_up(n2, 2);
       if (!seenL.count(L)) { seenL[L] = 1; tab += shell_matrix_doubles(L); }
-      const size_t per = ang_plane_smem(L);
-      int pb = (int)std::max<size_t>(1, ANG_SMEM_TARGET / per);
-      pb = std::min(pb, n0);
-      if (per * pb > SMEM_MAX) { err = "shell L too large for shared memory"; return false; }
-      pl.ang_pb[s] = pb;
-      pl.n_ang_items += (n0 + pb - 1) / pb;
-      pl.ang_smem = std::max(pl.ang_smem, per * pb);
+      // planes per CTA: the most (<= 8) that keep two CTAs on an SM if that is at least 4, else the most that fit
+      int pb = 0, cls = 0;
+      for (int nb = ANG_NB_MAX; nb >= 4; --nb) if (ang_smem_bytes(L, nb) <= ANG_SMEM_2CTA) { pb = nb; break; }
+      if (!pb) { cls = 1; for (int nb = ANG_NB_MAX; nb >= 1; --nb) if (ang_smem_bytes(L, nb) <= SMEM_MAX) { pb = nb; break; } }
+      if (!pb) { err = "shell L too large for shared memory"; return false; }
+      const int chunks = (n0 + pb - 1) / pb;
+      pb = (n0 + chunks - 1) / chunks;            // near-equal chunks
+      pl.ang_pb[s] = pb; pl.ang_class[s] = cls;
+      pl.n_ang_items += chunks; pl.n_ang_class[cls] += chunks;
+      pl.ang_smem[cls] = std::max(pl.ang_smem[cls], ang_smem_bytes(L, pb));
     }
   }
   if (tiles > 0x7fffffff) { err = "domain too large"; return false; }
@@ -277,11 +292,11 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
   std::vector<double> tab(pl.table_doubles, 0.0);
   std::vector<ChebItem> cheb; cheb.reserve(pl.n_cheb_items);
   std::vector<ChebItem> cheb_r;   // radial items of shells are kept with the others; the list is one launch
-  std::vector<AngItem> ang; ang.reserve(pl.n_ang_items);
+  std::vector<AngItem> ang, ang1; ang.reserve(pl.n_ang_items);   // class 0 items, class 1 items (appended below)
   d->h_subs.resize(n_sub);
   size_t tp = 0;
   std::map<int, std::vector<ghb::ld>> Dcache;        // N -> unscaled D
-  struct ShellOff { int Fa, Fs, Fp, Th, Pr; };
+  struct ShellOff { int Fa, Fs, TP; };
   std::map<int, ShellOff> Lcache;
   for (int s = 0; s < n_sub; ++s) {
     const gh_subdomain_desc& de = descs[s];
@@ -322,7 +337,24 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
         ghb::ShellBasis B; ghb::shell_basis(L, B);
         ShellOff o;
         auto put = [&](const std::vector<ghb::ld>& v) { int at = (int)tp; for (size_t e = 0; e < v.size(); ++e) tab[tp + e] = (double)v[e]; tp += v.size(); return at; };
-        o.Fa = put(B.Fa); o.Fs = put(B.Fs); o.Fp = put(B.Fp); o.Th = put(B.Th); o.Pr = put(B.Pr);
+        o.Fa = put(B.Fa); o.Fs = put(B.Fs);
+        // [Th_m ; m Pr_m] in DMMA fragment order: lane (g = lane/4, t = lane%4) of fragment (m_tile, k_step)
+        // holds element (row 8 m_tile + g, column 4 k_step + t); rows / columns beyond n_theta are zero
+        {
+          const int nt = L + 1, mtn = (nt + 7) / 8, ksn = (nt + 3) / 4;
+          std::vector<ghb::ld> TP(shell_tp_doubles(L), 0);
+          size_t e = 0;
+          for (int m = 0; m <= L; ++m)
+            for (int part = 0; part < 2; ++part)
+              for (int mt = 0; mt < mtn; ++mt)
+                for (int ks = 0; ks < ksn; ++ks)
+                  for (int lane = 0; lane < 32; ++lane, ++e) {
+                    const int row = mt * 8 + lane / 4, col = ks * 4 + lane % 4;
+                    if (row < nt && col < nt)
+                      TP[e] = part == 0 ? B.Th[((size_t)m * nt + row) * nt + col] : (ghb::ld)m * B.Pr[((size_t)m * nt + row) * nt + col];
+                  }
+          o.TP = put(TP);
+        }
         Lcache[L] = o;
       }
       const ShellOff& o = Lcache[L];
@@ -343,14 +375,15 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
       const int pb = pl.ang_pb[s];
       for (int p0 = 0; p0 < n0; p0 += pb) {
         AngItem it; memset(&it, 0, sizeof it);
-        it.off = sd.off; it.L = L; it.plane0 = p0; it.nplanes = std::min(pb, n0 - p0);
-        it.m_Fa = o.Fa; it.m_Fs = o.Fs; it.m_Fp = o.Fp; it.m_Th = o.Th; it.m_Pr = o.Pr;
-        ang.push_back(it);
+        it.off = sd.off; it.L = L; it.plane0 = p0; it.nplanes = std::min(pb, n0 - p0); it.nb_alloc = pb;
+        it.m_Fa = o.Fa; it.m_Fs = o.Fs; it.m_TP = o.TP;
+        (pl.ang_class[s] ? ang1 : ang).push_back(it);
       }
     } else {
       d->has_block = true;
     }
   }
+  ang.insert(ang.end(), ang1.begin(), ang1.end());
   if (tp != pl.table_doubles || (int)cheb.size() != pl.n_cheb_items || (int)ang.size() != pl.n_ang_items) {
     delete d; return fail(nullptr, GH_ERR_STATE, "internal: plan and build disagree");
   }
@@ -367,7 +400,7 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
   if (!ang.empty()) GH_CREATE_CUDA(cudaMemcpyAsync(d->ang, ang.data(), ang.size() * sizeof(AngItem), cudaMemcpyHostToDevice, st));
   GH_CREATE_CUDA(cudaStreamSynchronize(st));   // host staging vectors die at return
   GH_CREATE_CUDA(cudaFuncSetAttribute(k_cheb<CHEB_TPB, CHEB_CPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.cheb_smem));
-  if (pl.ang_smem) GH_CREATE_CUDA(cudaFuncSetAttribute(k_ang<ANG_TPB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.ang_smem));
+  if (pl.n_ang_items) GH_CREATE_CUDA(cudaFuncSetAttribute(k_ang<ANG_TPB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max(pl.ang_smem[0], pl.ang_smem[1])));
 #undef GH_CREATE_CUDA
   *out = d;
   return GH_OK;
@@ -457,9 +490,10 @@ gh_status launch_derivs(gh_domain* d, const double* in, double* out, int ncomp) 
     k_cheb<CHEB_TPB, CHEB_CPT><<<dim3(pl.n_cheb_items, ncomp), CHEB_TPB, pl.cheb_smem, d->stream>>>(
         d->cheb, d->tables, in, out, pl.S, ncomp);
   }
-  if (pl.n_ang_items) {
+  for (int cls = 0, first = 0; cls < 2; first += pl.n_ang_class[cls], ++cls) {
+    if (!pl.n_ang_class[cls]) continue;
     ProfScope ps(d, GH_K_SHELL_ANG);
-    k_ang<ANG_TPB><<<dim3(pl.n_ang_items, ncomp), ANG_TPB, pl.ang_smem, d->stream>>>(d->ang, d->tables, in, out, pl.S, ncomp);
+    k_ang<ANG_TPB><<<dim3(pl.n_ang_class[cls], ncomp), ANG_TPB, pl.ang_smem[cls], d->stream>>>(d->ang + first, d->tables, in, out, pl.S, ncomp);
   }
   GH_CUDA(d, cudaGetLastError());
   return GH_OK;

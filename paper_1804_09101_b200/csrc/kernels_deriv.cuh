@@ -93,84 +93,229 @@ k_cheb(const ChebItem* __restrict__ items, const double* __restrict__ tables, co
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// K_ang.  grid = (n_items, ncomp).  One CTA: `nplanes` (theta,phi) planes of one component of one shell.
-//   S1  C[b][j][q]  = sum_k U[b][j][k] Fa[q][k]                        (real DFT, Nyquist dropped)
-//   S2  A[b][j'][q] = sum_j Th[m(q)][j'][j] C[b][j][q],  B likewise with Pr[m(q)]
-//   S3  d_theta u[b][j'][k] = sum_q A[b][j'][q] Fs[k][q],   d_phi u[b][j'][k] = sum_q B[b][j'][q] Fp[k][q]
-// Shared memory: U (reused for A after S1), C, B.
+// K_ang.  grid = (n_items, ncomp), TPB = 256 (8 warps).  One CTA: `nb` (theta,phi) planes of one component of
+// one shell, kept in shared memory through three stages, each a small GEMM executed by warps with the FP64
+// tensor-core instruction mma.sync.m8n8k4 (DMMA: measured 37.1 TFLOP/s on B200 against 33.8 for register-
+// resident DFMA, at 1/8 of the issue slots; profiles/fp64_peak_r01.md):
+//   S1  C[r][q]       = sum_k  U[r][k] Fa[q][k]            rows r = (plane b, theta j); real DFT, Nyquist dropped
+//   S2  A[b][j'][q]   = sum_j  Th_m[j'][j] C[b][j][q]      m = m(q);  in place over C
+//       B'[b][j'][q~] = +-sum_j (m Pr_m)[j'][j] C[b][j][q]  q~ = the cos<->sin partner of q:  d/dphi in coefficient space
+//   S3  d_theta u[r][k] = sum_q A[r][q] Fs[k][q],   d_phi u[r][k] = sum_q B'[r][q] Fs[k][q]
+// Shared memory: X (U, later B'), Y (C, later A), F (Fa, later Fs).  Row (b, j) of X / Y starts at b*ps + j*pitch
+// doubles; pitch = 4 mod 8 and ps = 1 mod 16 make every fragment load conflict-free.
+// The per-m matrices [Th_m ; m Pr_m] are read from global memory (L2) in fragment order: one coalesced 256-byte
+// load per 8x4 fragment, prefetched one k-step ahead.
 // ---------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
+  asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+      : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+__host__ __device__ inline int ang_pitch(int L) {   // row pitch (doubles): >= n_phi rounded to 4, and = 4 mod 8
+  int p = (2 * L + 2 + 3) / 4 * 4;
+  return (p % 8 == 0) ? p + 4 : p;
+}
+__host__ __device__ inline int ang_plane_stride(int L) {   // plane stride (doubles): = 1 mod 16
+  return ((L + 1) * ang_pitch(L) + 15) / 16 * 16 + 1;
+}
+
+constexpr int ANG_NTC = 6;   // n-tiles per warp unit in S1 / S3
+
 template <int TPB>
 __global__ void __launch_bounds__(TPB)
 k_ang(const AngItem* __restrict__ items, const double* __restrict__ tables, const double* __restrict__ in,
       double* __restrict__ out, int64_t S, int ncomp) {
   extern __shared__ __align__(16) double sm[];
+  constexpr int NW = TPB / 32;
   const AngItem it = items[blockIdx.x];
-  const int comp = blockIdx.y, tid = threadIdx.x;
+  const int comp = blockIdx.y, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int g = lane >> 2, tl = lane & 3;
   const int L = it.L, nt = L + 1, np = 2 * L + 2, nq = 2 * L + 1, plane = nt * np;
-  const int nb = it.nplanes;
+  const int nb = it.nplanes, R = nb * nt;
+  const int pitch = ang_pitch(L), ps = ang_plane_stride(L);
+  const int NP8 = (np + 7) & ~7, NQ8 = (nq + 7) & ~7;
   const int64_t goff = it.off + (int64_t)it.plane0 * plane;
   const double* __restrict__ src = in + (int64_t)comp * S + goff;
   double* __restrict__ dth = out + ((int64_t)1 * ncomp + comp) * S + goff;
   double* __restrict__ dph = out + ((int64_t)2 * ncomp + comp) * S + goff;
-  const double* __restrict__ Fa = tables + it.m_Fa;
-  const double* __restrict__ Fs = tables + it.m_Fs;
-  const double* __restrict__ Fp = tables + it.m_Fp;
-  const double* __restrict__ Th = tables + it.m_Th;
-  const double* __restrict__ Pr = tables + it.m_Pr;
 
-  const int rows = nb * nt;
-  double* U = sm;                       // [rows][np]   (later A: [rows][nq])
-  double* Cc = U + (size_t)rows * np;    // [rows][nq]
-  double* Bb = Cc + (size_t)rows * nq;   // [rows][nq]
+  double* X = sm;                          // [nb][ps]
+  double* Y = X + (size_t)it.nb_alloc * ps;   // [nb][ps]
+  double* F = Y + (size_t)it.nb_alloc * ps;   // [NP8][pitch]
 
-  for (int e = tid; e < rows * np; e += TPB) U[e] = src[e];
-  __syncthreads();
-
-  // S1: analysis in phi
-  for (int e = tid; e < rows * nq; e += TPB) {
-    int r = e / nq, q = e - r * nq;
-    const double* u = U + (size_t)r * np;
-    const double* f = Fa + (size_t)q * np;
-    double s = 0.0;
-    for (int k = 0; k < np; ++k) s = fma(u[k], __ldg(f + k), s);
-    Cc[e] = s;
+  // ---- stage 0: U -> X (pad columns zero), Fa -> F (pad rows / columns zero) ----
+  {
+    const int hp = pitch >> 1;
+    for (int e = tid; e < R * hp; e += TPB) {
+      const int r = e / hp, k = (e - r * hp) * 2;
+      const int b = r / nt, j = r - b * nt;
+      double2 v = make_double2(0.0, 0.0);
+      if (k < np) v = *reinterpret_cast<const double2*>(src + (size_t)r * np + k);
+      double* d = X + (size_t)b * ps + j * pitch + k;
+      d[0] = v.x; d[1] = v.y;
+    }
+    const double* __restrict__ Fa = tables + it.m_Fa;
+    for (int e = tid; e < NQ8 * pitch; e += TPB) {
+      const int q = e / pitch, k = e - q * pitch;
+      F[e] = (q < nq && k < np) ? __ldg(Fa + (size_t)q * np + k) : 0.0;
+    }
   }
   __syncthreads();
 
-  // S2: per-m Legendre composites along theta
-  double* Aa = U;
-  for (int e = tid; e < rows * nq; e += TPB) {
-    int r = e / nq, q = e - r * nq;
-    int b = r / nt, jo = r - b * nt;
-    int m = (q <= L) ? q : q - L;
-    const double* th = Th + ((size_t)m * nt + jo) * nt;
-    const double* pr = Pr + ((size_t)m * nt + jo) * nt;
-    const double* c = Cc + (size_t)b * nt * nq + q;
-    double sa = 0.0, sb = 0.0;
-    for (int j = 0; j < nt; ++j) {
-      double v = c[(size_t)j * nq];
-      sa = fma(__ldg(th + j), v, sa);
-      sb = fma(__ldg(pr + j), v, sb);
+  const int MT1 = (R + 7) >> 3;
+  // ---- S1: C = U Fa^T ----
+  {
+    const int KS = (np + 3) >> 2, NT = NQ8 >> 3;
+    const int nch = (NT + ANG_NTC - 1) / ANG_NTC, per = (NT + nch - 1) / nch;
+    for (int u = warp; u < MT1 * nch; u += NW) {
+      const int mt = u / nch, ch = u - mt * nch;
+      const int n0 = ch * per, nn = min(per, NT - n0);
+      const int r = mt * 8 + g;
+      const bool rok = r < R;
+      const int rb = rok ? (r / nt) : 0, rj = rok ? (r - rb * nt) : 0;
+      const double* ap = X + (size_t)rb * ps + rj * pitch + tl;
+      const double* bp = F + (size_t)(n0 * 8 + g) * pitch + tl;
+      double acc[ANG_NTC][2];
+#pragma unroll
+      for (int n = 0; n < ANG_NTC; ++n) acc[n][0] = acc[n][1] = 0.0;
+      for (int ks = 0; ks < KS; ++ks) {
+        const double a = rok ? ap[ks * 4] : 0.0;
+#pragma unroll
+        for (int n = 0; n < ANG_NTC; ++n)
+          if (n < nn) dmma884(acc[n][0], acc[n][1], a, bp[(size_t)n * 8 * pitch + ks * 4]);
+      }
+      // C fragment: row g, columns 2 tl, 2 tl + 1 of each n-tile
+      const int r2 = mt * 8 + g;
+      if (r2 < R) {
+        double* yp = Y + (size_t)rb * ps + rj * pitch;
+#pragma unroll
+        for (int n = 0; n < ANG_NTC; ++n)
+          if (n < nn) {
+            const int c = (n0 + n) * 8 + 2 * tl;
+            if (c < pitch) yp[c] = acc[n][0];
+            if (c + 1 < pitch) yp[c + 1] = acc[n][1];
+          }
+      }
     }
-    Aa[e] = sa;
-    Bb[e] = sb;
   }
   __syncthreads();
 
-  // S3: synthesis in phi
-  for (int e = tid; e < rows * np; e += TPB) {
-    int r = e / np, k = e - r * np;
-    const double* a = Aa + (size_t)r * nq;
-    const double* b = Bb + (size_t)r * nq;
-    const double* fs = Fs + (size_t)k * nq;
-    const double* fp = Fp + (size_t)k * nq;
-    double s0 = 0.0, s1 = 0.0;
-    for (int q = 0; q < nq; ++q) {
-      s0 = fma(a[q], __ldg(fs + q), s0);
-      s1 = fma(b[q], __ldg(fp + q), s1);
+  // ---- Fs -> F (the buffer is free once S1 is done; S2 does not touch it) ----
+  {
+    const double* __restrict__ Fs = tables + it.m_Fs;
+    for (int e = tid; e < NP8 * pitch; e += TPB) {
+      const int k = e / pitch, q = e - k * pitch;
+      F[e] = (k < np && q < nq) ? __ldg(Fs + (size_t)k * nq + q) : 0.0;
     }
-    dth[e] = s0;
-    dph[e] = s1;
+  }
+  // ---- S2: per m, [A ; B'] = [Th_m ; m Pr_m] C_m over the columns (t, b), t = cos / sin, b = plane ----
+  {
+    const int MTn = (nt + 7) >> 3, KS = (nt + 3) >> 2;        // <= 6, <= 12
+    const double* __restrict__ TP = tables + it.m_TP;
+    for (int m = warp; m <= L; m += NW) {
+      const int ncols = (m == 0) ? nb : 2 * nb;               // <= 16
+      const int NTn = (ncols + 7) >> 3;                       // 1 or 2
+      // B fragment columns of this lane: n = 8 n_tile + g  ->  (t, b)
+      int boff[2]; bool bok[2];
+#pragma unroll
+      for (int n = 0; n < 2; ++n) {
+        const int c = n * 8 + g;
+        bok[n] = c < ncols;
+        const int t = bok[n] ? c / nb : 0, b = bok[n] ? c - t * nb : 0;
+        boff[n] = b * ps + (t ? L + m : m);
+      }
+      // part 1 first (m Pr_m -> X), then part 0 (Th_m -> Y, in place over the C_m it has just been read from)
+#pragma unroll 1
+      for (int p = 1; p >= 0; --p) {
+        double acc[6][2][2];
+#pragma unroll
+        for (int mt = 0; mt < 6; ++mt)
+#pragma unroll
+          for (int n = 0; n < 2; ++n) acc[mt][n][0] = acc[mt][n][1] = 0.0;
+        const double* __restrict__ tp = TP + ((size_t)(m * 2 + p) * MTn * KS) * 32 + lane;   // [mt][ks][32]
+        double an[6];
+#pragma unroll
+        for (int mt = 0; mt < 6; ++mt) an[mt] = (mt < MTn) ? __ldg(tp + (size_t)(mt * KS) * 32) : 0.0;
+        for (int ks = 0; ks < KS; ++ks) {
+          double a[6];
+#pragma unroll
+          for (int mt = 0; mt < 6; ++mt) a[mt] = an[mt];
+          if (ks + 1 < KS) {
+#pragma unroll
+            for (int mt = 0; mt < 6; ++mt)
+              if (mt < MTn) an[mt] = __ldg(tp + (size_t)(mt * KS + ks + 1) * 32);
+          }
+          const int j = ks * 4 + tl;
+          double bf[2];
+#pragma unroll
+          for (int n = 0; n < 2; ++n) bf[n] = (bok[n] && j < nt) ? Y[boff[n] + j * pitch] : 0.0;
+#pragma unroll
+          for (int mt = 0; mt < 6; ++mt)
+            if (mt < MTn) {
+              dmma884(acc[mt][0][0], acc[mt][0][1], a[mt], bf[0]);
+              if (NTn > 1) dmma884(acc[mt][1][0], acc[mt][1][1], a[mt], bf[1]);
+            }
+        }
+        __syncwarp();   // every lane has read its C_m entries before any lane overwrites them
+#pragma unroll
+        for (int mt = 0; mt < 6; ++mt) {
+          const int jo = mt * 8 + g;
+          if (mt < MTn && jo < nt) {
+#pragma unroll
+            for (int n = 0; n < 2; ++n)
+#pragma unroll
+              for (int e = 0; e < 2; ++e) {
+                const int c = n * 8 + 2 * tl + e;
+                if (c < ncols) {
+                  const int t = c / nb, b = c - t * nb;
+                  const int row = b * ps + jo * pitch;
+                  const double v = acc[mt][n][e];
+                  if (p == 0) Y[row + (t ? L + m : m)] = v;          // A: same coefficient slot
+                  else if (m == 0) X[row] = 0.0;                      // d/dphi of the m = 0 mode
+                  else if (t == 0) X[row + L + m] = -v;               // sin slot <- -m (Pr C_cos)
+                  else X[row + m] = v;                                // cos slot <- +m (Pr C_sin)
+                }
+              }
+          }
+        }
+      }
+    }
+  }
+  __syncthreads();
+
+  // ---- S3: [d_theta u ; d_phi u] = [A ; B'] Fs^T, stored straight from the accumulator fragments ----
+  {
+    const int KS = (nq + 3) >> 2, NT = NP8 >> 3;
+    const int nch = (NT + ANG_NTC - 1) / ANG_NTC, per = (NT + nch - 1) / nch;
+    for (int u = warp; u < 2 * MT1 * nch; u += NW) {
+      const int mt2 = u / nch, ch = u - mt2 * nch;
+      const int part = mt2 >= MT1, mt = part ? mt2 - MT1 : mt2;
+      const int n0 = ch * per, nn = min(per, NT - n0);
+      const int r = mt * 8 + g;
+      const bool rok = r < R;
+      const int rb = rok ? (r / nt) : 0, rj = rok ? (r - rb * nt) : 0;
+      const double* ap = (part ? X : Y) + (size_t)rb * ps + rj * pitch;
+      const double* bp = F + (size_t)(n0 * 8 + g) * pitch + tl;
+      double acc[ANG_NTC][2];
+#pragma unroll
+      for (int n = 0; n < ANG_NTC; ++n) acc[n][0] = acc[n][1] = 0.0;
+      for (int ks = 0; ks < KS; ++ks) {
+        const int q = ks * 4 + tl;
+        const double a = (rok && q < nq) ? ap[q] : 0.0;
+#pragma unroll
+        for (int n = 0; n < ANG_NTC; ++n)
+          if (n < nn) dmma884(acc[n][0], acc[n][1], a, bp[(size_t)n * 8 * pitch + ks * 4]);
+      }
+      if (rok) {
+        double* gp = (part ? dph : dth) + (size_t)r * np;
+#pragma unroll
+        for (int n = 0; n < ANG_NTC; ++n)
+          if (n < nn) {
+            const int c = (n0 + n) * 8 + 2 * tl;
+            if (c < np) *reinterpret_cast<double2*>(gp + c) = make_double2(acc[n][0], acc[n][1]);
+          }
+      }
+    }
   }
 }
 
