@@ -22,7 +22,7 @@ struct SubDev {
   int32_t pad_;
 };
 
-// One tile of Chebyshev lines: out[a, col] = sum_i Dt[i][a] in[i, col] for `ncols` columns (A2, Eq. 22).
+// One tile of Chebyshev lines: out[a, col] = sum_i D[a][i] in[i, col] for `ncols` columns (A2, Eq. 22).
 // Element (i, col) lives at  base + i*stride_i + (col / col_inner)*outer_stride + (col % col_inner).
 struct ChebItem {
   int64_t base;
@@ -32,8 +32,8 @@ struct ChebItem {
   int32_t col_inner;
   int32_t col0;
   int32_t ncols;
-  int32_t dmat;     // offset (doubles) of Dt[N][apitch], already multiplied by 2/(hi-lo)
-  int32_t apitch;   // N rounded up to a multiple of 8
+  int32_t dmat;     // offset (doubles) of D, multiplied by 2/(hi-lo), in DMMA A-fragment order [m_tile][k_step][32]
+  int32_t pad0_;
   int32_t axis;     // which logical-derivative slot the result goes to
   int32_t pad_;
 };

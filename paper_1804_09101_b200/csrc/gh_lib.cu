@@ -21,7 +21,12 @@ using namespace ghd;
 
 namespace {
 
-constexpr int CHEB_TPB = 64, CHEB_CPT = 4, CHEB_CT = CHEB_TPB * CHEB_CPT;   // lines per K_cheb tile
+constexpr int CHEB_TPB = 128;                     // K_cheb: 4 warps
+constexpr int CHEB_NTW0 = 4, CHEB_NTW1 = 2;       // n-tiles per warp: class 0 (N <= 32), class 1 (N <= 64)
+constexpr int CHEB_CT0 = (CHEB_TPB / 32) * 8 * CHEB_NTW0, CHEB_CT1 = (CHEB_TPB / 32) * 8 * CHEB_NTW1;   // columns per CTA
+inline int cheb_class(int N) { return N <= 32 ? 0 : 1; }
+inline int cheb_ct(int N) { return cheb_class(N) ? CHEB_CT1 : CHEB_CT0; }
+inline size_t cheb_frag_doubles(int N) { return (size_t)((N + 7) / 8) * ((N + 3) / 4) * 32; }   // D in fragment order
 constexpr int ANG_TPB = 256;
 constexpr size_t ANG_SMEM_2CTA = 113 * 1024;     // K_ang shared memory that still lets two CTAs share an SM
 constexpr int ANG_NB_MAX = 8;                    // planes per K_ang CTA (S2 holds 2*nb <= 16 columns per m)
@@ -44,7 +49,7 @@ struct Plan {
   int64_t P = 0, S = 0;
   int n_tiles = 0;
   size_t table_doubles = 0;
-  int n_cheb_items = 0, n_cheb_items_r = 0, n_ang_items = 0;
+  int n_cheb_items = 0, n_cheb_class[2] = {0, 0}, n_ang_items = 0;
   int n_ang_class[2] = {0, 0};           // K_ang items per shared-memory class (0: two CTAs per SM, 1: one)
   size_t cheb_smem = 0, ang_smem[2] = {0, 0};
   std::vector<int> ang_pb;               // planes per CTA for each subdomain (0 for blocks)
@@ -122,11 +127,11 @@ bool make_plan(const gh_subdomain_desc* descs, int32_t n_sub, Plan& pl, std::str
       const int N = d.n[a];
       const int nn[3] = {n0, n1, n2};
       (void)nn;
-      tab += (size_t)N * round_up(N, 8);
+      tab += cheb_frag_doubles(N);
       const int64_t cols = Ps / N;
-      const int items = (int)((cols + CHEB_CT - 1) / CHEB_CT);
-      pl.n_cheb_items += items;
-      pl.cheb_smem = std::max(pl.cheb_smem, ((size_t)N * round_up(N, 8) + (size_t)N * (CHEB_CT + 1)) * sizeof(double));
+      const int items = (int)((cols + cheb_ct(N) - 1) / cheb_ct(N));
+      pl.n_cheb_items += items; pl.n_cheb_class[cheb_class(N)] += items;
+      pl.cheb_smem = std::max(pl.cheb_smem, cheb_frag_doubles(N) * sizeof(double));
     }
     if (d.kind == GH_SHELL) {
       const int L = d.n[1];
@@ -290,8 +295,7 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
 
   // ---- tables and work lists on the host ----
   std::vector<double> tab(pl.table_doubles, 0.0);
-  std::vector<ChebItem> cheb; cheb.reserve(pl.n_cheb_items);
-  std::vector<ChebItem> cheb_r;   // radial items of shells are kept with the others; the list is one launch
+  std::vector<ChebItem> cheb, cheb1; cheb.reserve(pl.n_cheb_items);   // class 0 items, class 1 items (appended below)
   std::vector<AngItem> ang, ang1; ang.reserve(pl.n_ang_items);   // class 0 items, class 1 items (appended below)
   d->h_subs.resize(n_sub);
   size_t tp = 0;
@@ -313,21 +317,30 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
       const int N = (int)nn[a];
       if (!Dcache.count(N)) ghb::cheb_diff_matrix(N, Dcache[N]);
       const std::vector<ghb::ld>& D = Dcache[N];
-      const int ap = (int)round_up(N, 8);
       const ghb::ld scale = 2 / ((ghb::ld)de.hi[a] - (ghb::ld)de.lo[a]);   // affine map factor of Eq. 22
       const int dm = (int)tp;
-      for (int i = 0; i < N; ++i)
-        for (int o = 0; o < N; ++o) tab[tp + (size_t)i * ap + o] = (double)(scale * D[(size_t)o * N + i]);   // Dt[i][o]
-      tp += (size_t)N * ap;
+      // scaled D in DMMA A-fragment order: lane (g = lane/4, t = lane%4) of fragment (m_tile, k_step) holds
+      // D[8 m_tile + g][4 k_step + t]; rows / columns beyond N are zero
+      {
+        const int mtn = (N + 7) / 8, ksn = (N + 3) / 4;
+        for (int mt = 0; mt < mtn; ++mt)
+          for (int ks = 0; ks < ksn; ++ks)
+            for (int lane = 0; lane < 32; ++lane) {
+              const int row = mt * 8 + lane / 4, col = ks * 4 + lane % 4;
+              tab[tp + ((size_t)mt * ksn + ks) * 32 + lane] = (row < N && col < N) ? (double)(scale * D[(size_t)row * N + col]) : 0.0;
+            }
+      }
+      tp += cheb_frag_doubles(N);
       const int64_t cols = sd.P / N;
-      for (int64_t c0 = 0; c0 < cols; c0 += CHEB_CT) {
+      const int ct = cheb_ct(N);
+      for (int64_t c0 = 0; c0 < cols; c0 += ct) {
         ChebItem it; memset(&it, 0, sizeof it);
-        it.base = sd.off; it.stride_i = strides[a]; it.N = N; it.dmat = dm; it.apitch = ap; it.axis = a;
-        it.col0 = (int)c0; it.ncols = (int)std::min<int64_t>(CHEB_CT, cols - c0);
+        it.base = sd.off; it.stride_i = strides[a]; it.N = N; it.dmat = dm; it.axis = a;
+        it.col0 = (int)c0; it.ncols = (int)std::min<int64_t>(ct, cols - c0);
         if (a == 0) { it.col_inner = (int)(nn[1] * nn[2]); it.outer_stride = 0; }
         else if (a == 1) { it.col_inner = (int)nn[2]; it.outer_stride = nn[1] * nn[2]; }
         else { it.col_inner = 1; it.outer_stride = nn[2]; }
-        cheb.push_back(it);
+        (cheb_class(N) ? cheb1 : cheb).push_back(it);
       }
     }
     if (de.kind == GH_SHELL) {
@@ -384,6 +397,7 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
     }
   }
   ang.insert(ang.end(), ang1.begin(), ang1.end());
+  cheb.insert(cheb.end(), cheb1.begin(), cheb1.end());
   if (tp != pl.table_doubles || (int)cheb.size() != pl.n_cheb_items || (int)ang.size() != pl.n_ang_items) {
     delete d; return fail(nullptr, GH_ERR_STATE, "internal: plan and build disagree");
   }
@@ -399,7 +413,6 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
   GH_CREATE_CUDA(cudaMemcpyAsync(d->cheb, cheb.data(), cheb.size() * sizeof(ChebItem), cudaMemcpyHostToDevice, st));
   if (!ang.empty()) GH_CREATE_CUDA(cudaMemcpyAsync(d->ang, ang.data(), ang.size() * sizeof(AngItem), cudaMemcpyHostToDevice, st));
   GH_CREATE_CUDA(cudaStreamSynchronize(st));   // host staging vectors die at return
-  GH_CREATE_CUDA(cudaFuncSetAttribute(k_cheb<CHEB_TPB, CHEB_CPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.cheb_smem));
   if (pl.n_ang_items) GH_CREATE_CUDA(cudaFuncSetAttribute(k_ang<ANG_TPB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max(pl.ang_smem[0], pl.ang_smem[1])));
 #undef GH_CREATE_CUDA
   *out = d;
@@ -485,10 +498,15 @@ gh_status check_flag(gh_domain* d) {   // stream must be synchronised by the cal
 // (blocks: d/dx, d/dy, d/dz already Cartesian; shells: d/dr, d/dtheta, d/dphi).
 gh_status launch_derivs(gh_domain* d, const double* in, double* out, int ncomp) {
   const Plan& pl = d->pl;
-  {
+  if (pl.n_cheb_class[0]) {
     ProfScope ps(d, GH_K_CHEB);
-    k_cheb<CHEB_TPB, CHEB_CPT><<<dim3(pl.n_cheb_items, ncomp), CHEB_TPB, pl.cheb_smem, d->stream>>>(
+    k_cheb<CHEB_TPB, 4, 8, CHEB_NTW0><<<dim3(pl.n_cheb_class[0], ncomp), CHEB_TPB, pl.cheb_smem, d->stream>>>(
         d->cheb, d->tables, in, out, pl.S, ncomp);
+  }
+  if (pl.n_cheb_class[1]) {
+    ProfScope ps(d, GH_K_CHEB);
+    k_cheb<CHEB_TPB, 8, 16, CHEB_NTW1><<<dim3(pl.n_cheb_class[1], ncomp), CHEB_TPB, pl.cheb_smem, d->stream>>>(
+        d->cheb + pl.n_cheb_class[0], d->tables, in, out, pl.S, ncomp);
   }
   for (int cls = 0, first = 0; cls < 2; first += pl.n_ang_class[cls], ++cls) {
     if (!pl.n_ang_class[cls]) continue;

@@ -9,85 +9,96 @@
 namespace ghd {
 
 // ---------------------------------------------------------------------------------------------------------
-// K_cheb.  grid = (n_items, ncomp).  One CTA: a tile of up to TPB*CPT lines ("columns") of one component,
-// staged in shared memory T[i][col] (odd pitch: conflict-free both for the transposing fill of unit-stride
-// lines and for the per-column reads).  Each thread owns CPT columns and produces 8 outputs per column per
-// pass: per i one broadcast read of 8 matrix entries (4 x LDS.128) and CPT x LDS.64 feed 8*CPT DFMAs, which
-// keeps the shared-memory pipe under the FP64 pipe.
+// K_cheb.  grid = (n_items, ncomp), TPB threads.  out[a, col] = sum_i D[a][i] u[i, col] as a GEMM on the FP64 tensor
+// cores (mma.sync.m8n8k4, DMMA: 37.1 TFLOP/s measured against 33.9 for DFMA, profiles/r01_fp64_peak.md), M = a,
+// K = i, N = col.  One warp owns 8*NTW columns of one component and ALL of M and K, so every input element is
+// loaded exactly once, straight from global memory into its B-fragment register (lane (g, tl) of k-step ks holds
+// u[i = 4 ks + tl][col = 8 n + g]: per request 4 rows x 64 B for the strided axes, 8 lines x 32 B for the
+// unit-stride axis - whole 32-byte sectors either way), and every output leaves from its accumulator fragment
+// (row a = 8 mt + g, columns 8 n + 2 tl, +1).  No shared-memory staging of the data and no transposes; shared memory
+// only holds the differentiation matrix in A-fragment order (one conflict-free LDS.64 per fragment).  All K-steps of
+// a warp tile are loaded before the first DMMA, which keeps KS*NTW*256 B per warp in flight.
+// MTM / KSM: compile-time bounds on the m-tiles (N <= 8 MTM) and k-steps (N <= 4 KSM) of the class.
 // ---------------------------------------------------------------------------------------------------------
-template <int TPB, int CPT>
+__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
+  asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+      : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+template <int TPB, int MTM, int KSM, int NTW>
 __global__ void __launch_bounds__(TPB)
 k_cheb(const ChebItem* __restrict__ items, const double* __restrict__ tables, const double* __restrict__ in,
        double* __restrict__ out, int64_t S, int ncomp) {
-  extern __shared__ __align__(16) double sm[];
+  extern __shared__ __align__(16) double sm[];   // D in fragment order [mt][ks][32]
   const ChebItem it = items[blockIdx.x];
-  const int comp = blockIdx.y, tid = threadIdx.x;
+  const int comp = blockIdx.y, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int g = lane >> 2, tl = lane & 3;
   const double* __restrict__ src = in + (int64_t)comp * S + it.base;
   double* __restrict__ dst = out + ((int64_t)it.axis * ncomp + comp) * S + it.base;
-  const int N = it.N, ap = it.apitch, ncols = it.ncols;
-  constexpr int PITCH = TPB * CPT + 1;
-  double* Dt = sm;            // [N][ap]
-  double* T = sm + N * ap;    // [N][PITCH]
+  const int N = it.N, MTn = (N + 7) >> 3, KS = (N + 3) >> 2, ncols = it.ncols;
+  const int64_t si = it.stride_i;
 
-  for (int e = tid; e < N * ap; e += TPB) Dt[e] = tables[it.dmat + e];
-  if (it.stride_i == 1) {
-    // unit-stride lines (last logical axis): memory runs along i, consecutive threads take consecutive i
-    for (int e = tid; e < N * ncols; e += TPB) {
-      int c = e / N, i = e - c * N;
-      int col = it.col0 + c;
-      int64_t ca = (int64_t)(col / it.col_inner) * it.outer_stride + (col % it.col_inner);
-      T[i * PITCH + c] = src[ca + i];
-    }
-  } else {
-    for (int e = tid; e < N * ncols; e += TPB) {
-      int i = e / ncols, c = e - i * ncols;
-      int col = it.col0 + c;
-      int64_t ca = (int64_t)(col / it.col_inner) * it.outer_stride + (col % it.col_inner);
-      T[i * PITCH + c] = src[(int64_t)i * it.stride_i + ca];
-    }
+  for (int e = tid; e < MTn * KS * 32; e += TPB) sm[e] = __ldg(tables + it.dmat + e);
+
+  // B fragments of the whole warp tile (independent of shared memory: issued before the barrier)
+  const int wc0 = warp * (8 * NTW);
+  int64_t caddr[NTW];
+  bool cok[NTW];
+#pragma unroll
+  for (int n = 0; n < NTW; ++n) {
+    const int c = wc0 + n * 8 + g;
+    cok[n] = c < ncols;
+    const int col = it.col0 + (cok[n] ? c : 0);
+    const int q = col / it.col_inner;
+    caddr[n] = (int64_t)q * it.outer_stride + (col - q * it.col_inner);
   }
+  double b[KSM][NTW];
+#pragma unroll
+  for (int ks = 0; ks < KSM; ++ks)
+    if (ks < KS) {
+      const int i = ks * 4 + tl;
+#pragma unroll
+      for (int n = 0; n < NTW; ++n) b[ks][n] = (cok[n] && i < N) ? src[caddr[n] + (int64_t)i * si] : 0.0;
+    }
   __syncthreads();
+  if (wc0 >= ncols) return;
 
-  int64_t caddr[CPT];
-  bool valid[CPT];
+  double acc[MTM][NTW][2];
 #pragma unroll
-  for (int q = 0; q < CPT; ++q) {
-    int c = tid + q * TPB;
-    valid[q] = c < ncols;
-    int col = it.col0 + (valid[q] ? c : 0);
-    caddr[q] = (int64_t)(col / it.col_inner) * it.outer_stride + (col % it.col_inner);
-  }
-
-  for (int a0 = 0; a0 < N; a0 += 8) {
-    double acc[CPT][8];
+  for (int mt = 0; mt < MTM; ++mt)
 #pragma unroll
-    for (int q = 0; q < CPT; ++q)
+    for (int n = 0; n < NTW; ++n) acc[mt][n][0] = acc[mt][n][1] = 0.0;
 #pragma unroll
-      for (int a = 0; a < 8; ++a) acc[q][a] = 0.0;
-    const double* drow = Dt + a0;
-    const double* trow = T + tid;
-#pragma unroll 2
-    for (int i = 0; i < N; ++i) {
-      const double2 d0 = *reinterpret_cast<const double2*>(drow + 0);
-      const double2 d1 = *reinterpret_cast<const double2*>(drow + 2);
-      const double2 d2 = *reinterpret_cast<const double2*>(drow + 4);
-      const double2 d3 = *reinterpret_cast<const double2*>(drow + 6);
-      const double d[8] = {d0.x, d0.y, d1.x, d1.y, d2.x, d2.y, d3.x, d3.y};
+  for (int ks = 0; ks < KSM; ++ks)
+    if (ks < KS) {
 #pragma unroll
-      for (int q = 0; q < CPT; ++q) {
-        const double t = trow[q * TPB];
+      for (int mt = 0; mt < MTM; ++mt)
+        if (mt < MTn) {
+          const double a = sm[(mt * KS + ks) * 32 + lane];
 #pragma unroll
-        for (int a = 0; a < 8; ++a) acc[q][a] = fma(d[a], t, acc[q][a]);
-      }
-      drow += ap;
-      trow += PITCH;
+          for (int n = 0; n < NTW; ++n) dmma884(acc[mt][n][0], acc[mt][n][1], a, b[ks][n]);
+        }
     }
+
+  // C fragments: row a = 8 mt + g, columns 8 n + 2 tl and + 1; their addresses come from the lanes that loaded them
+  const bool pair = (si != 1) && ((it.col_inner & 1) == 0);
 #pragma unroll
-    for (int q = 0; q < CPT; ++q) {
-      if (!valid[q]) continue;
+  for (int n = 0; n < NTW; ++n) {
+    const int64_t c0a = __shfl_sync(0xffffffffu, caddr[n], (2 * tl) * 4);
+    const int64_t c1a = __shfl_sync(0xffffffffu, caddr[n], (2 * tl + 1) * 4);
+    const int c = wc0 + n * 8 + 2 * tl;
+    const bool ok0 = c < ncols, ok1 = c + 1 < ncols;
 #pragma unroll
-      for (int a = 0; a < 8; ++a)
-        if (a0 + a < N) dst[(int64_t)(a0 + a) * it.stride_i + caddr[q]] = acc[q][a];
+    for (int mt = 0; mt < MTM; ++mt) {
+      const int a = mt * 8 + g;
+      if (mt < MTn && a < N) {
+        if (pair && ok1) {
+          *reinterpret_cast<double2*>(dst + c0a + (int64_t)a * si) = make_double2(acc[mt][n][0], acc[mt][n][1]);
+        } else {
+          if (ok0) dst[c0a + (int64_t)a * si] = acc[mt][n][0];
+          if (ok1) dst[c1a + (int64_t)a * si] = acc[mt][n][1];
+        }
+      }
     }
   }
 }
@@ -106,11 +117,6 @@ k_cheb(const ChebItem* __restrict__ items, const double* __restrict__ tables, co
 // The per-m matrices [Th_m ; m Pr_m] are read from global memory (L2) in fragment order: one coalesced 256-byte
 // load per 8x4 fragment, prefetched one k-step ahead.
 // ---------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
-  asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
-      : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
-}
-
 __host__ __device__ inline int ang_pitch(int L) {   // row pitch (doubles): >= n_phi rounded to 4, and = 4 mod 8
   int p = (2 * L + 2 + 3) / 4 * 4;
   return (p % 8 == 0) ? p + 4 : p;
