@@ -46,8 +46,8 @@ struct AngItem {
   int32_t plane0;
   int32_t nplanes;
   int32_t nb_alloc;              // planes the shared-memory layout is sized for (>= nplanes)
-  int32_t m_Fa, m_Fs, m_TP;      // offsets (doubles) in the table memory: Fa [nq][np], Fs [np][nq], and the per-m
-                                 // [Th_m ; m Pr_m] matrices in DMMA fragment order [m][part][m_tile][k_step][32]
+  int32_t m_Fa, m_Fs, m_T;       // offsets (doubles) in the table memory, all in DMMA fragment order: Fa [k_step][n_tile][32],
+                                 // Fs [k_step][n_tile][32], stacked per-m matrices [Th_m ; m Pr_m] as [m][k_step][m_tile][32]
   int32_t pad_;
 };
 

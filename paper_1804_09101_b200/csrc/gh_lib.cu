@@ -64,18 +64,14 @@ inline void sub_dims(const gh_subdomain_desc& d, int& n0, int& n1, int& n2) {
 }
 
 // K_ang shared memory for nb planes of band limit L: X and Y ([nb][plane stride]) + F ([n_phi rounded to 8][pitch])
-inline size_t ang_smem_bytes(int L, int nb) {
-  const size_t np8 = (size_t)((2 * L + 2 + 7) / 8 * 8);
-  return (2 * (size_t)nb * ang_plane_stride(L) + np8 * ang_pitch(L)) * sizeof(double);
+inline size_t ang_smem_bytes(int L, int nb) { return ang_smem_doubles(L, nb) * sizeof(double); }
+inline size_t shell_fa_doubles(int L) { return (size_t)((2 * L + 2 + 3) / 4) * ((2 * L + 1 + 7) / 8) * 32; }   // [k_step][n_tile][32]
+inline size_t shell_fs_doubles(int L) { return (size_t)((2 * L + 1 + 3) / 4) * ((2 * L + 2 + 7) / 8) * 32; }
+inline size_t shell_t_doubles(int L) {    // [m][k_step][m_tile][32], stacked [Th_m ; m Pr_m], see AngItem
+  const size_t nt = L + 1, mtn = (2 * nt + 7) / 8, ks = (nt + 3) / 4;
+  return (size_t)(L + 1) * ks * mtn * 32;
 }
-inline size_t shell_tp_doubles(int L) {   // [m][part][m_tile][k_step][32], see AngItem
-  const size_t nt = L + 1, mtn = (nt + 7) / 8, ks = (nt + 3) / 4;
-  return (size_t)(L + 1) * 2 * mtn * ks * 32;
-}
-inline size_t shell_matrix_doubles(int L) {
-  size_t np = 2 * L + 2, nq = 2 * L + 1;
-  return 2 * nq * np + shell_tp_doubles(L);
-}
+inline size_t shell_matrix_doubles(int L) { return shell_fa_doubles(L) + shell_fs_doubles(L) + shell_t_doubles(L); }
 
 bool validate(const gh_subdomain_desc* descs, int32_t n_sub, std::string& err) {
   char buf[256];
@@ -300,7 +296,7 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
   d->h_subs.resize(n_sub);
   size_t tp = 0;
   std::map<int, std::vector<ghb::ld>> Dcache;        // N -> unscaled D
-  struct ShellOff { int Fa, Fs, TP; };
+  struct ShellOff { int Fa, Fs, T; };
   std::map<int, ShellOff> Lcache;
   for (int s = 0; s < n_sub; ++s) {
     const gh_subdomain_desc& de = descs[s];
@@ -350,23 +346,38 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
         ghb::ShellBasis B; ghb::shell_basis(L, B);
         ShellOff o;
         auto put = [&](const std::vector<ghb::ld>& v) { int at = (int)tp; for (size_t e = 0; e < v.size(); ++e) tab[tp + e] = (double)v[e]; tp += v.size(); return at; };
-        o.Fa = put(B.Fa); o.Fs = put(B.Fs);
-        // [Th_m ; m Pr_m] in DMMA fragment order: lane (g = lane/4, t = lane%4) of fragment (m_tile, k_step)
-        // holds element (row 8 m_tile + g, column 4 k_step + t); rows / columns beyond n_theta are zero
+        // all three operands in DMMA fragment order, zero padded to whole tiles; lane = 4 g + t
         {
-          const int nt = L + 1, mtn = (nt + 7) / 8, ksn = (nt + 3) / 4;
-          std::vector<ghb::ld> TP(shell_tp_doubles(L), 0);
-          size_t e = 0;
-          for (int m = 0; m <= L; ++m)
-            for (int part = 0; part < 2; ++part)
-              for (int mt = 0; mt < mtn; ++mt)
-                for (int ks = 0; ks < ksn; ++ks)
-                  for (int lane = 0; lane < 32; ++lane, ++e) {
-                    const int row = mt * 8 + lane / 4, col = ks * 4 + lane % 4;
-                    if (row < nt && col < nt)
-                      TP[e] = part == 0 ? B.Th[((size_t)m * nt + row) * nt + col] : (ghb::ld)m * B.Pr[((size_t)m * nt + row) * nt + col];
-                  }
-          o.TP = put(TP);
+          const int np = 2 * L + 2, nq = 2 * L + 1, nt = L + 1;
+          // Fa as the B operand of S1: fragment (k_step, n_tile): element (k = 4 ks + t, n = 8 nt_ + g) = Fa[q = n][k]
+          const int ksp = (np + 3) / 4, ntq = (nq + 7) / 8;
+          std::vector<ghb::ld> FA(shell_fa_doubles(L), 0);
+          for (int ks = 0; ks < ksp; ++ks) for (int n = 0; n < ntq; ++n) for (int lane = 0; lane < 32; ++lane) {
+            const int k = ks * 4 + lane % 4, q = n * 8 + lane / 4;
+            if (k < np && q < nq) FA[((size_t)ks * ntq + n) * 32 + lane] = B.Fa[(size_t)q * np + k];
+          }
+          o.Fa = put(FA);
+          // Fs as the B operand of S3: element (k = q = 4 ks + t, n = phi index 8 nt_ + g) = Fs[phi][q]
+          const int ksq = (nq + 3) / 4, ntp = (np + 7) / 8;
+          std::vector<ghb::ld> FS(shell_fs_doubles(L), 0);
+          for (int ks = 0; ks < ksq; ++ks) for (int n = 0; n < ntp; ++n) for (int lane = 0; lane < 32; ++lane) {
+            const int q = ks * 4 + lane % 4, k = n * 8 + lane / 4;
+            if (q < nq && k < np) FS[((size_t)ks * ntp + n) * 32 + lane] = B.Fs[(size_t)k * nq + q];
+          }
+          o.Fs = put(FS);
+          // stacked [Th_m ; m Pr_m] (2 nt x nt) as the A operand of S2: element (row = 8 mt + g, col = 4 ks + t)
+          const int mtn = (2 * nt + 7) / 8, ks2 = (nt + 3) / 4;
+          std::vector<ghb::ld> T(shell_t_doubles(L), 0);
+          for (int m = 0; m <= L; ++m) for (int ks = 0; ks < ks2; ++ks) for (int mt = 0; mt < mtn; ++mt) for (int lane = 0; lane < 32; ++lane) {
+            const int row = mt * 8 + lane / 4, col = ks * 4 + lane % 4;
+            ghb::ld v = 0;
+            if (col < nt) {
+              if (row < nt) v = B.Th[((size_t)m * nt + row) * nt + col];
+              else if (row < 2 * nt) v = (ghb::ld)m * B.Pr[((size_t)m * nt + (row - nt)) * nt + col];
+            }
+            T[(((size_t)m * ks2 + ks) * mtn + mt) * 32 + lane] = v;
+          }
+          o.T = put(T);
         }
         Lcache[L] = o;
       }
@@ -389,7 +400,7 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
       for (int p0 = 0; p0 < n0; p0 += pb) {
         AngItem it; memset(&it, 0, sizeof it);
         it.off = sd.off; it.L = L; it.plane0 = p0; it.nplanes = std::min(pb, n0 - p0); it.nb_alloc = pb;
-        it.m_Fa = o.Fa; it.m_Fs = o.Fs; it.m_TP = o.TP;
+        it.m_Fa = o.Fa; it.m_Fs = o.Fs; it.m_T = o.T;
         (pl.ang_class[s] ? ang1 : ang).push_back(it);
       }
     } else {

@@ -104,28 +104,179 @@ k_cheb(const ChebItem* __restrict__ items, const double* __restrict__ tables, co
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// K_ang.  grid = (n_items, ncomp), TPB = 256 (8 warps).  One CTA: `nb` (theta,phi) planes of one component of
-// one shell, kept in shared memory through three stages, each a small GEMM executed by warps with the FP64
-// tensor-core instruction mma.sync.m8n8k4 (DMMA: measured 37.1 TFLOP/s on B200 against 33.8 for register-
-// resident DFMA, at 1/8 of the issue slots; profiles/fp64_peak_r01.md):
-//   S1  C[r][q]       = sum_k  U[r][k] Fa[q][k]            rows r = (plane b, theta j); real DFT, Nyquist dropped
-//   S2  A[b][j'][q]   = sum_j  Th_m[j'][j] C[b][j][q]      m = m(q);  in place over C
-//       B'[b][j'][q~] = +-sum_j (m Pr_m)[j'][j] C[b][j][q]  q~ = the cos<->sin partner of q:  d/dphi in coefficient space
+// K_ang.  grid = (n_items, ncomp).  One CTA: `nb` (theta,phi) planes of one component of one shell, kept in shared
+// memory through three GEMM stages on the FP64 tensor cores (mma.sync.m8n8k4):
+//   S1  C[r][q]        = sum_k  U[r][k] Fa[q][k]             rows r = (plane b, theta j); real DFT, Nyquist dropped
+//   S2  [A ; B'](m)    = [Th_m ; m Pr_m] C_m                  per m, columns (t = cos/sin, plane b); A in place over C,
+//                                                             B' into the cos<->sin partner slot with sign: d/dphi
 //   S3  d_theta u[r][k] = sum_q A[r][q] Fs[k][q],   d_phi u[r][k] = sum_q B'[r][q] Fs[k][q]
-// Shared memory: X (U, later B'), Y (C, later A), F (Fa, later Fs).  Row (b, j) of X / Y starts at b*ps + j*pitch
-// doubles; pitch = 4 mod 8 and ps = 1 mod 16 make every fragment load conflict-free.
-// The per-m matrices [Th_m ; m Pr_m] are read from global memory (L2) in fragment order: one coalesced 256-byte
-// load per 8x4 fragment, prefetched one k-step ahead.
+// Every matrix operand is stored in DMMA fragment order, zero padded to whole tiles ([k_step][tile][32 lanes]: one
+// conflict-free LDS.64 / coalesced 256-byte LDG per fragment, tile offsets are immediates), so the inner loops carry
+// no bounds predicate: about 2-3 issued instructions per DMMA.  Fa / Fs fragments live in shared memory; the per-m
+// stacked matrices [Th_m ; m Pr_m] stream from L2 one k-step ahead.  Planes: X (U, later B') and Y (C, later A), row
+// (b, j) at b*ps + j*pitch doubles; pitch = 4 mod 8 and ps = 1 mod 16 keep the data-fragment loads conflict-free.
+// Rows beyond the tile range read a zeroed row.  Outputs go straight from the S3 accumulators to global memory.
 // ---------------------------------------------------------------------------------------------------------
-__host__ __device__ inline int ang_pitch(int L) {   // row pitch (doubles): >= n_phi rounded to 4, and = 4 mod 8
-  int p = (2 * L + 2 + 3) / 4 * 4;
+__host__ __device__ inline int ang_pitch(int L) {   // row pitch (doubles): >= 8*ceil(n_q/8) and 4*ceil(n_phi/4), = 4 mod 8
+  const int a = (2 * L + 1 + 7) / 8 * 8, b = (2 * L + 2 + 3) / 4 * 4;
+  int p = a > b ? a : b;
   return (p % 8 == 0) ? p + 4 : p;
 }
-__host__ __device__ inline int ang_plane_stride(int L) {   // plane stride (doubles): = 1 mod 16
-  return ((L + 1) * ang_pitch(L) + 15) / 16 * 16 + 1;
+__host__ __device__ inline int ang_plane_stride(int L) {   // plane stride (doubles): rows padded to 4, = 1 mod 16
+  return ((L + 1 + 3) / 4 * 4 * ang_pitch(L) + 15) / 16 * 16 + 1;
+}
+// shared memory (doubles) of K_ang for nb planes: X, Y, one zero row, F fragments, row-offset table (ints)
+__host__ __device__ inline size_t ang_f_doubles(int L) {
+  const size_t np = 2 * L + 2, nq = 2 * L + 1;
+  const size_t fa = ((np + 3) / 4) * ((nq + 7) / 8) * 32, fs = ((nq + 3) / 4) * ((np + 7) / 8) * 32;
+  return fa > fs ? fa : fs;
+}
+__host__ __device__ inline size_t ang_smem_doubles(int L, int nb) {
+  const size_t rows = (size_t)nb * (L + 1);
+  return 2 * (size_t)nb * ang_plane_stride(L) + ang_pitch(L) + 16 + ang_f_doubles(L) + ((rows + 8) * sizeof(int) + 7) / 8;
 }
 
-constexpr int ANG_NTC = 6;   // n-tiles per warp unit in S1 / S3
+__device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gsrc));
+}
+__device__ __forceinline__ void cp_async16(double* smem_dst, const double* gsrc) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N)); }
+
+// S1 unit: one m-tile (8 rows) x NTC n-tiles.  ap: this lane's A row (+ tl); bp: F fragments of the first n-tile (+ lane)
+template <int NTC>
+__device__ __forceinline__ void ang_s1_unit(const double* __restrict__ ap, const double* __restrict__ bp, int KS, int NT,
+                                            double* __restrict__ yrow, int c0, int pitch, bool rok) {
+  double acc[NTC][2];
+#pragma unroll
+  for (int n = 0; n < NTC; ++n) acc[n][0] = acc[n][1] = 0.0;
+  const int bstep = NT * 32;
+#pragma unroll 2
+  for (int ks = 0; ks < KS; ++ks) {
+    const double a = ap[0];
+#pragma unroll
+    for (int n = 0; n < NTC; ++n) dmma884(acc[n][0], acc[n][1], a, bp[n * 32]);
+    ap += 4; bp += bstep;
+  }
+  if (rok) {
+#pragma unroll
+    for (int n = 0; n < NTC; ++n) {
+      const int c = c0 + n * 8;
+      if (c < pitch) { yrow[c] = acc[n][0]; yrow[c + 1] = acc[n][1]; }
+    }
+  }
+}
+
+// S3 unit: one m-tile x NTC n-tiles, both parts (theta from Y, phi from X) sharing the Fs fragments
+template <int NTC>
+__device__ __forceinline__ void ang_s3_unit(const double* __restrict__ a0p, const double* __restrict__ a1p,
+                                            const double* __restrict__ bp, int KS, int NT, double* __restrict__ g0,
+                                            double* __restrict__ g1, int c0, int np, bool rok) {
+  double acc0[NTC][2], acc1[NTC][2];
+#pragma unroll
+  for (int n = 0; n < NTC; ++n) acc0[n][0] = acc0[n][1] = acc1[n][0] = acc1[n][1] = 0.0;
+  const int bstep = NT * 32;
+#pragma unroll 2
+  for (int ks = 0; ks < KS; ++ks) {
+    const double a0 = a0p[0], a1 = a1p[0];
+#pragma unroll
+    for (int n = 0; n < NTC; ++n) {
+      const double b = bp[n * 32];
+      dmma884(acc0[n][0], acc0[n][1], a0, b);
+      dmma884(acc1[n][0], acc1[n][1], a1, b);
+    }
+    a0p += 4; a1p += 4; bp += bstep;
+  }
+  if (rok) {
+#pragma unroll
+    for (int n = 0; n < NTC; ++n) {
+      const int c = c0 + n * 8;
+      if (c < np) {
+        *reinterpret_cast<double2*>(g0 + c) = make_double2(acc0[n][0], acc0[n][1]);
+        *reinterpret_cast<double2*>(g1 + c) = make_double2(acc1[n][0], acc1[n][1]);
+      }
+    }
+  }
+}
+
+// S2 unit: mode m, n-tile `ntile` of its columns; MT2 m-tiles of the stacked matrix [Th_m ; m Pr_m]
+template <int MT2>
+__device__ __forceinline__ void ang_s2_unit(const double* __restrict__ tp /* T_m fragments + lane */, int KS2,
+                                            double* __restrict__ X, double* __restrict__ Y, int m, int ntile, int nb,
+                                            int L, int pitch, int ps, int g, int tl) {
+  const int nt = L + 1, ncols = (m == 0) ? nb : 2 * nb;
+  // B fragment column of this lane
+  const int cb = ntile * 8 + g;
+  const bool bok = cb < ncols;
+  const int tb = (bok && cb >= nb) ? 1 : 0, bb = bok ? cb - tb * nb : 0;
+  const double* __restrict__ yp = Y + bb * ps + (tb ? L + m : m) + tl * pitch;
+  double acc[MT2][2];
+#pragma unroll
+  for (int mt = 0; mt < MT2; ++mt) acc[mt][0] = acc[mt][1] = 0.0;
+  double an[MT2];
+#pragma unroll
+  for (int mt = 0; mt < MT2; ++mt) an[mt] = __ldg(tp + mt * 32);
+  const int ystep = 4 * pitch;
+#pragma unroll 1
+  for (int ks = 0; ks < KS2; ++ks) {
+    double a[MT2];
+#pragma unroll
+    for (int mt = 0; mt < MT2; ++mt) a[mt] = an[mt];
+    tp += MT2 * 32;
+    if (ks + 1 < KS2) {
+#pragma unroll
+      for (int mt = 0; mt < MT2; ++mt) an[mt] = __ldg(tp + mt * 32);
+    }
+    const double yv = yp[0];
+    const double b = bok ? yv : 0.0;
+    yp += ystep;
+#pragma unroll
+    for (int mt = 0; mt < MT2; ++mt) dmma884(acc[mt][0], acc[mt][1], a[mt], b);
+  }
+  __syncwarp();   // every lane has read its C_m entries before any lane overwrites them
+  // C fragment: stacked row 8 mt + g, columns 8 ntile + 2 tl + e
+  int coff[2]; int ctt[2]; bool cok[2];
+#pragma unroll
+  for (int e = 0; e < 2; ++e) {
+    const int c = ntile * 8 + 2 * tl + e;
+    cok[e] = c < ncols;
+    ctt[e] = (cok[e] && c >= nb) ? 1 : 0;
+    coff[e] = (cok[e] ? c - ctt[e] * nb : 0) * ps;
+  }
+#pragma unroll
+  for (int mt = 0; mt < MT2; ++mt) {
+    const int rr = mt * 8 + g;
+    if (rr < 2 * nt) {
+      const bool phi = rr >= nt;
+      const int jo = (phi ? rr - nt : rr) * pitch;
+#pragma unroll
+      for (int e = 0; e < 2; ++e)
+        if (cok[e]) {
+          const double v = acc[mt][e];
+          const int row = coff[e] + jo;
+          if (!phi) Y[row + (ctt[e] ? L + m : m)] = v;            // A: same coefficient slot
+          else if (m == 0) X[row] = 0.0;                           // d/dphi of the m = 0 mode
+          else if (ctt[e] == 0) X[row + L + m] = -v;               // sin slot <- -m (Pr C_cos)
+          else X[row + m] = v;                                     // cos slot <- +m (Pr C_sin)
+        }
+    }
+  }
+}
+
+#define GH_NTC_SWITCH(nn, CALL)                       \
+  switch (nn) {                                        \
+    case 1: CALL(1); break;                            \
+    case 2: CALL(2); break;                            \
+    case 3: CALL(3); break;                            \
+    case 4: CALL(4); break;                            \
+    default: CALL(5); break;                           \
+  }
+
+constexpr int ANG_NTC = 5;   // most n-tiles per warp unit in S1 / S3
 
 template <int TPB>
 __global__ void __launch_bounds__(TPB)
@@ -139,188 +290,126 @@ k_ang(const AngItem* __restrict__ items, const double* __restrict__ tables, cons
   const int L = it.L, nt = L + 1, np = 2 * L + 2, nq = 2 * L + 1, plane = nt * np;
   const int nb = it.nplanes, R = nb * nt;
   const int pitch = ang_pitch(L), ps = ang_plane_stride(L);
-  const int NP8 = (np + 7) & ~7, NQ8 = (nq + 7) & ~7;
+  const int KSp = (np + 3) >> 2, KSq = (nq + 3) >> 2, NTq = (nq + 7) >> 3, NTp = (np + 7) >> 3;
   const int64_t goff = it.off + (int64_t)it.plane0 * plane;
   const double* __restrict__ src = in + (int64_t)comp * S + goff;
   double* __restrict__ dth = out + ((int64_t)1 * ncomp + comp) * S + goff;
   double* __restrict__ dph = out + ((int64_t)2 * ncomp + comp) * S + goff;
 
-  double* X = sm;                          // [nb][ps]
-  double* Y = X + (size_t)it.nb_alloc * ps;   // [nb][ps]
-  double* F = Y + (size_t)it.nb_alloc * ps;   // [NP8][pitch]
+  double* X = sm;                               // [nb][ps]
+  double* Y = X + (size_t)it.nb_alloc * ps;     // [nb][ps]
+  double* Z = Y + (size_t)it.nb_alloc * ps;     // zero row [pitch + 16]
+  double* F = Z + pitch + 16;                   // Fa fragments, later Fs fragments
+  int* rowoff = reinterpret_cast<int*>(F + ang_f_doubles(L));   // [R rounded up to 8]: offset of row r in X / Y; pad rows -> Z
+  const int zoff = (int)(Z - X);                // offset of the zero row relative to X (also used relative to Y: see below)
 
-  // ---- stage 0: U -> X (pad columns zero), Fa -> F (pad rows / columns zero) ----
+  // ---- stage 0: U -> X and Fa fragments -> F by cp.async; zero the K-padding; row-offset table ----
   {
-    const int hp = pitch >> 1;
-    for (int e = tid; e < R * hp; e += TPB) {
-      const int r = e / hp, k = (e - r * hp) * 2;
+    for (int e = tid; e < R * np; e += TPB) {
+      const int r = e / np, k = e - r * np;
       const int b = r / nt, j = r - b * nt;
-      double2 v = make_double2(0.0, 0.0);
-      if (k < np) v = *reinterpret_cast<const double2*>(src + (size_t)r * np + k);
-      double* d = X + (size_t)b * ps + j * pitch + k;
-      d[0] = v.x; d[1] = v.y;
+      cp_async8(X + (size_t)b * ps + j * pitch + k, src + e);
     }
     const double* __restrict__ Fa = tables + it.m_Fa;
-    for (int e = tid; e < NQ8 * pitch; e += TPB) {
-      const int q = e / pitch, k = e - q * pitch;
-      F[e] = (q < nq && k < np) ? __ldg(Fa + (size_t)q * np + k) : 0.0;
+    const int nfa = KSp * NTq * 32;
+    for (int e = tid * 2; e < nfa; e += TPB * 2) cp_async16(F + e, Fa + e);
+    cp_async_commit();
+    const int R8 = (R + 7) & ~7;
+    for (int r = tid; r < R8; r += TPB) {
+      const int b = r / nt, j = r - b * nt;
+      rowoff[r] = (r < R) ? b * ps + j * pitch : zoff;
     }
+    for (int e = tid; e < pitch + 16; e += TPB) Z[e] = 0.0;
+    // U columns [np, pitch) of every row (K padding of S1, finite values for S3), rows [nt, 4*ceil(nt/4)) of Y (K padding of S2)
+    const int padc = pitch - np;
+    for (int e = tid; e < R * padc; e += TPB) {
+      const int r = e / padc, k = np + (e - r * padc);
+      const int b = r / nt, j = r - b * nt;
+      X[(size_t)b * ps + j * pitch + k] = 0.0;
+    }
+    const int ntp = (nt + 3) & ~3, padr = (ntp - nt) * pitch;
+    for (int e = tid; e < nb * padr; e += TPB) {
+      const int b = e / padr;
+      Y[(size_t)b * ps + nt * pitch + (e - b * padr)] = 0.0;
+    }
+    cp_async_wait<0>();
   }
   __syncthreads();
 
   const int MT1 = (R + 7) >> 3;
   // ---- S1: C = U Fa^T ----
   {
-    const int KS = (np + 3) >> 2, NT = NQ8 >> 3;
-    const int nch = (NT + ANG_NTC - 1) / ANG_NTC, per = (NT + nch - 1) / nch;
+    const int nch = (NTq + ANG_NTC - 1) / ANG_NTC, per = (NTq + nch - 1) / nch;
     for (int u = warp; u < MT1 * nch; u += NW) {
       const int mt = u / nch, ch = u - mt * nch;
-      const int n0 = ch * per, nn = min(per, NT - n0);
+      const int n0 = ch * per, nn = min(per, NTq - n0);
       const int r = mt * 8 + g;
-      const bool rok = r < R;
-      const int rb = rok ? (r / nt) : 0, rj = rok ? (r - rb * nt) : 0;
-      const double* ap = X + (size_t)rb * ps + rj * pitch + tl;
-      const double* bp = F + (size_t)(n0 * 8 + g) * pitch + tl;
-      double acc[ANG_NTC][2];
-#pragma unroll
-      for (int n = 0; n < ANG_NTC; ++n) acc[n][0] = acc[n][1] = 0.0;
-      for (int ks = 0; ks < KS; ++ks) {
-        const double a = rok ? ap[ks * 4] : 0.0;
-#pragma unroll
-        for (int n = 0; n < ANG_NTC; ++n)
-          if (n < nn) dmma884(acc[n][0], acc[n][1], a, bp[(size_t)n * 8 * pitch + ks * 4]);
-      }
-      // C fragment: row g, columns 2 tl, 2 tl + 1 of each n-tile
-      const int r2 = mt * 8 + g;
-      if (r2 < R) {
-        double* yp = Y + (size_t)rb * ps + rj * pitch;
-#pragma unroll
-        for (int n = 0; n < ANG_NTC; ++n)
-          if (n < nn) {
-            const int c = (n0 + n) * 8 + 2 * tl;
-            if (c < pitch) yp[c] = acc[n][0];
-            if (c + 1 < pitch) yp[c + 1] = acc[n][1];
-          }
-      }
+      const int ro = rowoff[r];
+      const double* ap = X + ro + tl;
+      const double* bp = F + n0 * 32 + lane;
+      double* yrow = Y + ro;
+      const int c0 = n0 * 8 + 2 * tl;
+#define GH_CALL(K) ang_s1_unit<K>(ap, bp, KSp, NTq, yrow, c0, pitch, r < R)
+      GH_NTC_SWITCH(nn, GH_CALL)
+#undef GH_CALL
     }
   }
   __syncthreads();
 
-  // ---- Fs -> F (the buffer is free once S1 is done; S2 does not touch it) ----
+  // ---- Fs fragments -> F (free once S1 is done; S2 does not touch it) ----
   {
     const double* __restrict__ Fs = tables + it.m_Fs;
-    for (int e = tid; e < NP8 * pitch; e += TPB) {
-      const int k = e / pitch, q = e - k * pitch;
-      F[e] = (k < np && q < nq) ? __ldg(Fs + (size_t)k * nq + q) : 0.0;
-    }
+    const int nfs = KSq * NTp * 32;
+    for (int e = tid * 2; e < nfs; e += TPB * 2) cp_async16(F + e, Fs + e);
+    cp_async_commit();
   }
-  // ---- S2: per m, [A ; B'] = [Th_m ; m Pr_m] C_m over the columns (t, b), t = cos / sin, b = plane ----
+  // ---- S2: per m and n-tile of its columns ----
   {
-    const int MTn = (nt + 7) >> 3, KS = (nt + 3) >> 2;        // <= 6, <= 12
-    const double* __restrict__ TP = tables + it.m_TP;
-    for (int m = warp; m <= L; m += NW) {
-      const int ncols = (m == 0) ? nb : 2 * nb;               // <= 16
-      const int NTn = (ncols + 7) >> 3;                       // 1 or 2
-      // B fragment columns of this lane: n = 8 n_tile + g  ->  (t, b)
-      int boff[2]; bool bok[2];
-#pragma unroll
-      for (int n = 0; n < 2; ++n) {
-        const int c = n * 8 + g;
-        bok[n] = c < ncols;
-        const int t = bok[n] ? c / nb : 0, b = bok[n] ? c - t * nb : 0;
-        boff[n] = b * ps + (t ? L + m : m);
-      }
-      // part 1 first (m Pr_m -> X), then part 0 (Th_m -> Y, in place over the C_m it has just been read from)
-#pragma unroll 1
-      for (int p = 1; p >= 0; --p) {
-        double acc[6][2][2];
-#pragma unroll
-        for (int mt = 0; mt < 6; ++mt)
-#pragma unroll
-          for (int n = 0; n < 2; ++n) acc[mt][n][0] = acc[mt][n][1] = 0.0;
-        const double* __restrict__ tp = TP + ((size_t)(m * 2 + p) * MTn * KS) * 32 + lane;   // [mt][ks][32]
-        double an[6];
-#pragma unroll
-        for (int mt = 0; mt < 6; ++mt) an[mt] = (mt < MTn) ? __ldg(tp + (size_t)(mt * KS) * 32) : 0.0;
-        for (int ks = 0; ks < KS; ++ks) {
-          double a[6];
-#pragma unroll
-          for (int mt = 0; mt < 6; ++mt) a[mt] = an[mt];
-          if (ks + 1 < KS) {
-#pragma unroll
-            for (int mt = 0; mt < 6; ++mt)
-              if (mt < MTn) an[mt] = __ldg(tp + (size_t)(mt * KS + ks + 1) * 32);
-          }
-          const int j = ks * 4 + tl;
-          double bf[2];
-#pragma unroll
-          for (int n = 0; n < 2; ++n) bf[n] = (bok[n] && j < nt) ? Y[boff[n] + j * pitch] : 0.0;
-#pragma unroll
-          for (int mt = 0; mt < 6; ++mt)
-            if (mt < MTn) {
-              dmma884(acc[mt][0][0], acc[mt][0][1], a[mt], bf[0]);
-              if (NTn > 1) dmma884(acc[mt][1][0], acc[mt][1][1], a[mt], bf[1]);
-            }
-        }
-        __syncwarp();   // every lane has read its C_m entries before any lane overwrites them
-#pragma unroll
-        for (int mt = 0; mt < 6; ++mt) {
-          const int jo = mt * 8 + g;
-          if (mt < MTn && jo < nt) {
-#pragma unroll
-            for (int n = 0; n < 2; ++n)
-#pragma unroll
-              for (int e = 0; e < 2; ++e) {
-                const int c = n * 8 + 2 * tl + e;
-                if (c < ncols) {
-                  const int t = c / nb, b = c - t * nb;
-                  const int row = b * ps + jo * pitch;
-                  const double v = acc[mt][n][e];
-                  if (p == 0) Y[row + (t ? L + m : m)] = v;          // A: same coefficient slot
-                  else if (m == 0) X[row] = 0.0;                      // d/dphi of the m = 0 mode
-                  else if (t == 0) X[row + L + m] = -v;               // sin slot <- -m (Pr C_cos)
-                  else X[row + m] = v;                                // cos slot <- +m (Pr C_sin)
-                }
-              }
-          }
-        }
+    const int MT2 = (2 * nt + 7) >> 3, KS2 = (nt + 3) >> 2;
+    const int NTn = (2 * nb + 7) >> 3;
+    const double* __restrict__ T = tables + it.m_T + lane;
+    for (int u = warp; u < (L + 1) * NTn; u += NW) {
+      const int m = u / NTn, ntile = u - m * NTn;
+      if (m == 0 && ntile * 8 >= nb) continue;
+      const double* tp = T + (size_t)m * KS2 * MT2 * 32;
+      switch (MT2) {
+        case 1: ang_s2_unit<1>(tp, KS2, X, Y, m, ntile, nb, L, pitch, ps, g, tl); break;
+        case 2: ang_s2_unit<2>(tp, KS2, X, Y, m, ntile, nb, L, pitch, ps, g, tl); break;
+        case 3: ang_s2_unit<3>(tp, KS2, X, Y, m, ntile, nb, L, pitch, ps, g, tl); break;
+        case 4: ang_s2_unit<4>(tp, KS2, X, Y, m, ntile, nb, L, pitch, ps, g, tl); break;
+        case 5: ang_s2_unit<5>(tp, KS2, X, Y, m, ntile, nb, L, pitch, ps, g, tl); break;
+        case 6: ang_s2_unit<6>(tp, KS2, X, Y, m, ntile, nb, L, pitch, ps, g, tl); break;
+        case 7: ang_s2_unit<7>(tp, KS2, X, Y, m, ntile, nb, L, pitch, ps, g, tl); break;
+        case 8: ang_s2_unit<8>(tp, KS2, X, Y, m, ntile, nb, L, pitch, ps, g, tl); break;
+        case 9: ang_s2_unit<9>(tp, KS2, X, Y, m, ntile, nb, L, pitch, ps, g, tl); break;
+        case 10: ang_s2_unit<10>(tp, KS2, X, Y, m, ntile, nb, L, pitch, ps, g, tl); break;
+        case 11: ang_s2_unit<11>(tp, KS2, X, Y, m, ntile, nb, L, pitch, ps, g, tl); break;
+        default: ang_s2_unit<12>(tp, KS2, X, Y, m, ntile, nb, L, pitch, ps, g, tl); break;
       }
     }
   }
+  cp_async_wait<0>();
   __syncthreads();
 
   // ---- S3: [d_theta u ; d_phi u] = [A ; B'] Fs^T, stored straight from the accumulator fragments ----
   {
-    const int KS = (nq + 3) >> 2, NT = NP8 >> 3;
-    const int nch = (NT + ANG_NTC - 1) / ANG_NTC, per = (NT + nch - 1) / nch;
-    for (int u = warp; u < 2 * MT1 * nch; u += NW) {
-      const int mt2 = u / nch, ch = u - mt2 * nch;
-      const int part = mt2 >= MT1, mt = part ? mt2 - MT1 : mt2;
-      const int n0 = ch * per, nn = min(per, NT - n0);
+    const int nch = (NTp + ANG_NTC - 1) / ANG_NTC, per = (NTp + nch - 1) / nch;
+    const int yx = (int)(Y - X);
+    for (int u = warp; u < MT1 * nch; u += NW) {
+      const int mt = u / nch, ch = u - mt * nch;
+      const int n0 = ch * per, nn = min(per, NTp - n0);
       const int r = mt * 8 + g;
       const bool rok = r < R;
-      const int rb = rok ? (r / nt) : 0, rj = rok ? (r - rb * nt) : 0;
-      const double* ap = (part ? X : Y) + (size_t)rb * ps + rj * pitch;
-      const double* bp = F + (size_t)(n0 * 8 + g) * pitch + tl;
-      double acc[ANG_NTC][2];
-#pragma unroll
-      for (int n = 0; n < ANG_NTC; ++n) acc[n][0] = acc[n][1] = 0.0;
-      for (int ks = 0; ks < KS; ++ks) {
-        const int q = ks * 4 + tl;
-        const double a = (rok && q < nq) ? ap[q] : 0.0;
-#pragma unroll
-        for (int n = 0; n < ANG_NTC; ++n)
-          if (n < nn) dmma884(acc[n][0], acc[n][1], a, bp[(size_t)n * 8 * pitch + ks * 4]);
-      }
-      if (rok) {
-        double* gp = (part ? dph : dth) + (size_t)r * np;
-#pragma unroll
-        for (int n = 0; n < ANG_NTC; ++n)
-          if (n < nn) {
-            const int c = (n0 + n) * 8 + 2 * tl;
-            if (c < np) *reinterpret_cast<double2*>(gp + c) = make_double2(acc[n][0], acc[n][1]);
-          }
-      }
+      const int ro = rowoff[r];
+      const double* a1p = X + ro + tl;                             // B'
+      const double* a0p = rok ? a1p + yx : a1p;                     // A (pad rows: the zero row for both)
+      const double* bp = F + n0 * 32 + lane;
+      const int c0 = n0 * 8 + 2 * tl;
+      double* g0 = dth + (size_t)r * np;
+      double* g1 = dph + (size_t)r * np;
+#define GH_CALL(K) ang_s3_unit<K>(a0p, a1p, bp, KSq, NTp, g0, g1, c0, np, rok)
+      GH_NTC_SWITCH(nn, GH_CALL)
+#undef GH_CALL
     }
   }
 }
