@@ -22,12 +22,13 @@ using namespace ghd;
 namespace {
 
 constexpr int CHEB_TPB = 128;                     // K_cheb: 4 warps
+constexpr int CHEB_COMP_WALK = 5;                 // components one K_cheb CTA walks over
 constexpr int CHEB_NTW0 = 4, CHEB_NTW1 = 2;       // n-tiles per warp: class 0 (N <= 32), class 1 (N <= 64)
 constexpr int CHEB_CT0 = (CHEB_TPB / 32) * 8 * CHEB_NTW0, CHEB_CT1 = (CHEB_TPB / 32) * 8 * CHEB_NTW1;   // columns per CTA
 inline int cheb_class(int N) { return N <= 32 ? 0 : 1; }
 inline int cheb_ct(int N) { return cheb_class(N) ? CHEB_CT1 : CHEB_CT0; }
 inline size_t cheb_frag_doubles(int N) { return (size_t)((N + 7) / 8) * ((N + 3) / 4) * 32; }   // D in fragment order
-constexpr int ANG_TPB = 256;
+constexpr int ANG_TPB0 = 256, ANG_TPB1 = 512;    // K_ang threads: class 0 (two CTAs per SM), class 1 (one CTA per SM)
 constexpr size_t ANG_SMEM_2CTA = 113 * 1024;     // K_ang shared memory that still lets two CTAs share an SM
 constexpr int ANG_NB_MAX = 8;                    // planes per K_ang CTA (S2 holds 2*nb <= 16 columns per m)
 constexpr size_t SMEM_MAX = 227 * 1024;
@@ -64,6 +65,17 @@ inline void sub_dims(const gh_subdomain_desc& d, int& n0, int& n1, int& n2) {
 }
 
 // K_ang shared memory for nb planes of band limit L: X and Y ([nb][plane stride]) + F ([n_phi rounded to 8][pitch])
+// n-chunks per m-tile that minimise (rounds over the warps) x (DMMAs per unit + fixed cost); w = DMMAs per n-tile and k-step
+inline int ang_best_nch(int NT, int MT1, int NW, int w) {
+  int best = 0; double bc = 1e300;
+  for (int nch = (NT + ANG_NTC - 1) / ANG_NTC; nch <= NT; ++nch) {
+    const int per = (NT + nch - 1) / nch;
+    if ((NT + per - 1) / per != nch) continue;          // same chunking the kernel derives from nch
+    const double cost = (double)((MT1 * nch + NW - 1) / NW) * (w * per + 0.6);
+    if (cost < bc) { bc = cost; best = nch; }
+  }
+  return best;
+}
 inline size_t ang_smem_bytes(int L, int nb) { return ang_smem_doubles(L, nb) * sizeof(double); }
 inline size_t shell_fa_doubles(int L) { return (size_t)((2 * L + 2 + 3) / 4) * ((2 * L + 1 + 7) / 8) * 32; }   // [k_step][n_tile][32]
 inline size_t shell_fs_doubles(int L) { return (size_t)((2 * L + 1 + 3) / 4) * ((2 * L + 2 + 7) / 8) * 32; }
@@ -401,6 +413,11 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
         AngItem it; memset(&it, 0, sizeof it);
         it.off = sd.off; it.L = L; it.plane0 = p0; it.nplanes = std::min(pb, n0 - p0); it.nb_alloc = pb;
         it.m_Fa = o.Fa; it.m_Fs = o.Fs; it.m_T = o.T;
+        {
+          const int NW = (pl.ang_class[s] ? ANG_TPB1 : ANG_TPB0) / 32, MT1 = (it.nplanes * (L + 1) + 7) / 8;
+          it.nch1 = (int16_t)ang_best_nch((2 * L + 1 + 7) / 8, MT1, NW, 1);
+          it.nch3 = (int16_t)ang_best_nch((2 * L + 2 + 7) / 8, MT1, NW, 2);
+        }
         (pl.ang_class[s] ? ang1 : ang).push_back(it);
       }
     } else {
@@ -424,7 +441,8 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
   GH_CREATE_CUDA(cudaMemcpyAsync(d->cheb, cheb.data(), cheb.size() * sizeof(ChebItem), cudaMemcpyHostToDevice, st));
   if (!ang.empty()) GH_CREATE_CUDA(cudaMemcpyAsync(d->ang, ang.data(), ang.size() * sizeof(AngItem), cudaMemcpyHostToDevice, st));
   GH_CREATE_CUDA(cudaStreamSynchronize(st));   // host staging vectors die at return
-  if (pl.n_ang_items) GH_CREATE_CUDA(cudaFuncSetAttribute(k_ang<ANG_TPB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max(pl.ang_smem[0], pl.ang_smem[1])));
+  if (pl.n_ang_class[0]) GH_CREATE_CUDA(cudaFuncSetAttribute(k_ang<ANG_TPB0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.ang_smem[0]));
+  if (pl.n_ang_class[1]) GH_CREATE_CUDA(cudaFuncSetAttribute(k_ang<ANG_TPB1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.ang_smem[1]));
 #undef GH_CREATE_CUDA
   *out = d;
   return GH_OK;
@@ -509,20 +527,25 @@ gh_status check_flag(gh_domain* d) {   // stream must be synchronised by the cal
 // (blocks: d/dx, d/dy, d/dz already Cartesian; shells: d/dr, d/dtheta, d/dphi).
 gh_status launch_derivs(gh_domain* d, const double* in, double* out, int ncomp) {
   const Plan& pl = d->pl;
+  // each K_cheb CTA walks over ncomp / cheb_gy components (amortises its launch and matrix load)
+  const int cheb_gy = (ncomp % CHEB_COMP_WALK == 0) ? ncomp / CHEB_COMP_WALK : ncomp;
   if (pl.n_cheb_class[0]) {
     ProfScope ps(d, GH_K_CHEB);
-    k_cheb<CHEB_TPB, 4, 8, CHEB_NTW0><<<dim3(pl.n_cheb_class[0], ncomp), CHEB_TPB, pl.cheb_smem, d->stream>>>(
+    k_cheb<CHEB_TPB, 4, 8, CHEB_NTW0><<<dim3(pl.n_cheb_class[0], cheb_gy), CHEB_TPB, pl.cheb_smem, d->stream>>>(
         d->cheb, d->tables, in, out, pl.S, ncomp);
   }
   if (pl.n_cheb_class[1]) {
     ProfScope ps(d, GH_K_CHEB);
-    k_cheb<CHEB_TPB, 8, 16, CHEB_NTW1><<<dim3(pl.n_cheb_class[1], ncomp), CHEB_TPB, pl.cheb_smem, d->stream>>>(
+    k_cheb<CHEB_TPB, 8, 16, CHEB_NTW1><<<dim3(pl.n_cheb_class[1], cheb_gy), CHEB_TPB, pl.cheb_smem, d->stream>>>(
         d->cheb + pl.n_cheb_class[0], d->tables, in, out, pl.S, ncomp);
   }
   for (int cls = 0, first = 0; cls < 2; first += pl.n_ang_class[cls], ++cls) {
     if (!pl.n_ang_class[cls]) continue;
     ProfScope ps(d, GH_K_SHELL_ANG);
-    k_ang<ANG_TPB><<<dim3(pl.n_ang_class[cls], ncomp), ANG_TPB, pl.ang_smem[cls], d->stream>>>(d->ang + first, d->tables, in, out, pl.S, ncomp);
+    if (cls == 0)
+      k_ang<ANG_TPB0><<<dim3(pl.n_ang_class[0], ncomp), ANG_TPB0, pl.ang_smem[0], d->stream>>>(d->ang + first, d->tables, in, out, pl.S, ncomp);
+    else
+      k_ang<ANG_TPB1><<<dim3(pl.n_ang_class[1], ncomp), ANG_TPB1, pl.ang_smem[1], d->stream>>>(d->ang + first, d->tables, in, out, pl.S, ncomp);
   }
   GH_CUDA(d, cudaGetLastError());
   return GH_OK;

@@ -26,23 +26,21 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
 }
 
 template <int TPB, int MTM, int KSM, int NTW>
-__global__ void __launch_bounds__(TPB)
+__global__ void __launch_bounds__(TPB, 3)
 k_cheb(const ChebItem* __restrict__ items, const double* __restrict__ tables, const double* __restrict__ in,
        double* __restrict__ out, int64_t S, int ncomp) {
   extern __shared__ __align__(16) double sm[];   // D in fragment order [mt][ks][32]
   const ChebItem it = items[blockIdx.x];
-  const int comp = blockIdx.y, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int g = lane >> 2, tl = lane & 3;
-  const double* __restrict__ src = in + (int64_t)comp * S + it.base;
-  double* __restrict__ dst = out + ((int64_t)it.axis * ncomp + comp) * S + it.base;
   const int N = it.N, MTn = (N + 7) >> 3, KS = (N + 3) >> 2, ncols = it.ncols;
-  const int64_t si = it.stride_i;
+  const int si0 = (int)it.stride_i;   // offsets inside a subdomain fit 32 bits (P_s <= 2^30)
 
   for (int e = tid; e < MTn * KS * 32; e += TPB) sm[e] = __ldg(tables + it.dmat + e);
 
-  // B fragments of the whole warp tile (independent of shared memory: issued before the barrier)
+  // column addresses of this lane's B fragments (loads) and C fragments (stores)
   const int wc0 = warp * (8 * NTW);
-  int64_t caddr[NTW];
+  int caddr[NTW];
   bool cok[NTW];
 #pragma unroll
   for (int n = 0; n < NTW; ++n) {
@@ -50,53 +48,69 @@ k_cheb(const ChebItem* __restrict__ items, const double* __restrict__ tables, co
     cok[n] = c < ncols;
     const int col = it.col0 + (cok[n] ? c : 0);
     const int q = col / it.col_inner;
-    caddr[n] = (int64_t)q * it.outer_stride + (col - q * it.col_inner);
+    caddr[n] = q * (int)it.outer_stride + (col - q * it.col_inner);
   }
-  double b[KSM][NTW];
+  const bool pair = (si0 != 1) && ((it.col_inner & 1) == 0);
+  int c0a[NTW], c1a[NTW];
 #pragma unroll
-  for (int ks = 0; ks < KSM; ++ks)
-    if (ks < KS) {
-      const int i = ks * 4 + tl;
-#pragma unroll
-      for (int n = 0; n < NTW; ++n) b[ks][n] = (cok[n] && i < N) ? src[caddr[n] + (int64_t)i * si] : 0.0;
-    }
+  for (int n = 0; n < NTW; ++n) {
+    c0a[n] = __shfl_sync(0xffffffffu, caddr[n], (2 * tl) * 4);
+    c1a[n] = __shfl_sync(0xffffffffu, caddr[n], (2 * tl + 1) * 4);
+  }
+
   __syncthreads();
   if (wc0 >= ncols) return;
 
-  double acc[MTM][NTW][2];
+  // the CTA walks over components blockIdx.y, blockIdx.y + gridDim.y, ... (one launch and one matrix load for all of them)
+#pragma unroll 1
+  for (int comp = blockIdx.y; comp < ncomp; comp += gridDim.y) {
+    // B fragments of the whole warp tile.  (si is laundered so that the compiler recomputes the 2 x KS x NTW element
+    // offsets per component instead of keeping them all live across the loop: that costs 40 registers and a CTA per SM)
+    int si = si0;
+    asm volatile("" : "+r"(si));
+    double b[KSM][NTW];
+    {
+      const double* __restrict__ src = in + (int64_t)comp * S + it.base;
 #pragma unroll
-  for (int mt = 0; mt < MTM; ++mt)
+      for (int ks = 0; ks < KSM; ++ks)
+        if (ks < KS) {
+          const int i = ks * 4 + tl;
 #pragma unroll
-    for (int n = 0; n < NTW; ++n) acc[mt][n][0] = acc[mt][n][1] = 0.0;
-#pragma unroll
-  for (int ks = 0; ks < KSM; ++ks)
-    if (ks < KS) {
-#pragma unroll
-      for (int mt = 0; mt < MTM; ++mt)
-        if (mt < MTn) {
-          const double a = sm[(mt * KS + ks) * 32 + lane];
-#pragma unroll
-          for (int n = 0; n < NTW; ++n) dmma884(acc[mt][n][0], acc[mt][n][1], a, b[ks][n]);
+          for (int n = 0; n < NTW; ++n) b[ks][n] = (cok[n] && i < N) ? src[caddr[n] + i * si] : 0.0;
         }
     }
-
-  // C fragments: row a = 8 mt + g, columns 8 n + 2 tl and + 1; their addresses come from the lanes that loaded them
-  const bool pair = (si != 1) && ((it.col_inner & 1) == 0);
+    double acc[MTM][NTW][2];
 #pragma unroll
-  for (int n = 0; n < NTW; ++n) {
-    const int64_t c0a = __shfl_sync(0xffffffffu, caddr[n], (2 * tl) * 4);
-    const int64_t c1a = __shfl_sync(0xffffffffu, caddr[n], (2 * tl + 1) * 4);
-    const int c = wc0 + n * 8 + 2 * tl;
-    const bool ok0 = c < ncols, ok1 = c + 1 < ncols;
+    for (int mt = 0; mt < MTM; ++mt)
 #pragma unroll
-    for (int mt = 0; mt < MTM; ++mt) {
-      const int a = mt * 8 + g;
-      if (mt < MTn && a < N) {
-        if (pair && ok1) {
-          *reinterpret_cast<double2*>(dst + c0a + (int64_t)a * si) = make_double2(acc[mt][n][0], acc[mt][n][1]);
-        } else {
-          if (ok0) dst[c0a + (int64_t)a * si] = acc[mt][n][0];
-          if (ok1) dst[c1a + (int64_t)a * si] = acc[mt][n][1];
+      for (int n = 0; n < NTW; ++n) acc[mt][n][0] = acc[mt][n][1] = 0.0;
+#pragma unroll
+    for (int ks = 0; ks < KSM; ++ks)
+      if (ks < KS) {
+#pragma unroll
+        for (int mt = 0; mt < MTM; ++mt)
+          if (mt < MTn) {
+            const double a = sm[(mt * KS + ks) * 32 + lane];
+#pragma unroll
+            for (int n = 0; n < NTW; ++n) dmma884(acc[mt][n][0], acc[mt][n][1], a, b[ks][n]);
+          }
+      }
+    // C fragments: row a = 8 mt + g, columns 8 n + 2 tl and + 1
+    double* __restrict__ dst = out + ((int64_t)it.axis * ncomp + comp) * S + it.base;
+#pragma unroll
+    for (int n = 0; n < NTW; ++n) {
+      const int c = wc0 + n * 8 + 2 * tl;
+      const bool ok0 = c < ncols, ok1 = c + 1 < ncols;
+#pragma unroll
+      for (int mt = 0; mt < MTM; ++mt) {
+        const int a = mt * 8 + g;
+        if (mt < MTn && a < N) {
+          if (pair && ok1) {
+            *reinterpret_cast<double2*>(dst + c0a[n] + a * si) = make_double2(acc[mt][n][0], acc[mt][n][1]);
+          } else {
+            if (ok0) dst[c0a[n] + a * si] = acc[mt][n][0];
+            if (ok1) dst[c1a[n] + a * si] = acc[mt][n][1];
+          }
         }
       }
     }
@@ -339,7 +353,7 @@ k_ang(const AngItem* __restrict__ items, const double* __restrict__ tables, cons
   const int MT1 = (R + 7) >> 3;
   // ---- S1: C = U Fa^T ----
   {
-    const int nch = (NTq + ANG_NTC - 1) / ANG_NTC, per = (NTq + nch - 1) / nch;
+    const int nch = it.nch1, per = (NTq + nch - 1) / nch;
     for (int u = warp; u < MT1 * nch; u += NW) {
       const int mt = u / nch, ch = u - mt * nch;
       const int n0 = ch * per, nn = min(per, NTq - n0);
@@ -393,7 +407,7 @@ k_ang(const AngItem* __restrict__ items, const double* __restrict__ tables, cons
 
   // ---- S3: [d_theta u ; d_phi u] = [A ; B'] Fs^T, stored straight from the accumulator fragments ----
   {
-    const int nch = (NTp + ANG_NTC - 1) / ANG_NTC, per = (NTp + nch - 1) / nch;
+    const int nch = it.nch3, per = (NTp + nch - 1) / nch;
     const int yx = (int)(Y - X);
     for (int u = warp; u < MT1 * nch; u += NW) {
       const int mt = u / nch, ch = u - mt * nch;
