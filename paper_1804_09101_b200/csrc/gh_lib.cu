@@ -441,6 +441,9 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
   GH_CREATE_CUDA(cudaMemcpyAsync(d->cheb, cheb.data(), cheb.size() * sizeof(ChebItem), cudaMemcpyHostToDevice, st));
   if (!ang.empty()) GH_CREATE_CUDA(cudaMemcpyAsync(d->ang, ang.data(), ang.size() * sizeof(AngItem), cudaMemcpyHostToDevice, st));
   GH_CREATE_CUDA(cudaStreamSynchronize(st));   // host staging vectors die at return
+  GH_CREATE_CUDA(cudaFuncSetAttribute(k_rhs<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RHS_SMEM_BYTES));
+  GH_CREATE_CUDA(cudaFuncSetAttribute(k_rhs<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RHS_SMEM_BYTES));
+  GH_CREATE_CUDA(cudaFuncSetAttribute(k_rhs<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RHS_SMEM_BYTES));
   if (pl.n_ang_class[0]) GH_CREATE_CUDA(cudaFuncSetAttribute(k_ang<ANG_TPB0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.ang_smem[0]));
   if (pl.n_ang_class[1]) GH_CREATE_CUDA(cudaFuncSetAttribute(k_ang<ANG_TPB1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.ang_smem[1]));
 #undef GH_CREATE_CUDA
@@ -551,14 +554,22 @@ gh_status launch_derivs(gh_domain* d, const double* in, double* out, int ncomp) 
   return GH_OK;
 }
 
-// A2-A6 on state `u`, result into `k` (device pointers)
-gh_status launch_rhs(gh_domain* d, const double* u, double* k) {
+// A2-A6 on state `u`; rk_mode 0: d_t u into `out`; 1 / 2: the fused RK stage (A7)  out = a u0 + b (u + dt d_t u)
+// (mode 1: a = 0, u0 unused).  `out` may alias u or u0.
+gh_status launch_rhs(gh_domain* d, const double* u, double* out, int rk_mode = 0, const double* u0 = nullptr, double a = 0.0,
+                     double b = 1.0, double dt = 0.0) {
   gh_status st = launch_derivs(d, u, d->du, NCOMP);
   if (st != GH_OK) return st;
   {
     ProfScope ps(d, GH_K_RHS);
-    k_rhs<<<d->pl.n_tiles, TILE_PTS, 0, d->stream>>>(d->subs, d->tiles, d->pl.n_sub, d->tables, u, d->du, d->H, d->dH, k,
-                                                     d->pl.S, d->flag);
+    const RkArgs rk{u0, a, b, dt};
+    const int grid = d->pl.n_tiles;
+    if (rk_mode == 0)
+      k_rhs<0><<<grid, TILE_PTS, RHS_SMEM_BYTES, d->stream>>>(d->subs, d->tiles, d->pl.n_sub, d->tables, u, d->du, d->H, d->dH, out, rk, d->pl.S, d->flag);
+    else if (rk_mode == 1)
+      k_rhs<1><<<grid, TILE_PTS, RHS_SMEM_BYTES, d->stream>>>(d->subs, d->tiles, d->pl.n_sub, d->tables, u, d->du, d->H, d->dH, out, rk, d->pl.S, d->flag);
+    else
+      k_rhs<2><<<grid, TILE_PTS, RHS_SMEM_BYTES, d->stream>>>(d->subs, d->tiles, d->pl.n_sub, d->tables, u, d->du, d->H, d->dH, out, rk, d->pl.S, d->flag);
   }
   GH_CUDA(d, cudaGetLastError());
   return GH_OK;
@@ -568,22 +579,6 @@ gh_status launch_jac(gh_domain* d, double* g, int ncomp) {
   if (!d->has_shell) return GH_OK;
   ProfScope ps(d, GH_K_JAC);
   k_jac<<<d->pl.n_tiles, TILE_PTS, 0, d->stream>>>(d->subs, d->tiles, d->pl.n_sub, d->tables, g, d->pl.S, ncomp);
-  GH_CUDA(d, cudaGetLastError());
-  return GH_OK;
-}
-
-gh_status launch_rk(gh_domain* d, const double* u0, const double* us, const double* k, double* out, double a, double b, double dt) {
-  const int64_t n2 = (int64_t)NCOMP * d->pl.S / 2;   // S is a multiple of 16
-  int dev = 0, sms = 148;
-  cudaGetDevice(&dev);
-  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  const int64_t want = (n2 + 255) / 256;
-  const int grid = (int)std::min<int64_t>(want, (int64_t)sms * 8);
-  ProfScope ps(d, GH_K_RK);
-  if (a == 0.0)
-    k_rk<false><<<grid, 256, 0, d->stream>>>(nullptr, (const double2*)us, (const double2*)k, (double2*)out, a, b, dt, n2);
-  else
-    k_rk<true><<<grid, 256, 0, d->stream>>>((const double2*)u0, (const double2*)us, (const double2*)k, (double2*)out, a, b, dt, n2);
   GH_CUDA(d, cudaGetLastError());
   return GH_OK;
 }
@@ -663,15 +658,13 @@ extern "C" gh_status gh_rk_step(gh_domain* d, double dt) {
   if (!d->has_fields) return fail(d, GH_ERR_STATE, "gh_rk_step before gh_set_fields");
   if (!std::isfinite(dt)) return fail(d, GH_ERR_ARG, "dt is not finite");
   gh_status st;
-  // u1 = u0 + dt k(u0)
-  if ((st = launch_rhs(d, d->ua, d->k)) != GH_OK) return st;
-  if ((st = launch_rk(d, nullptr, d->ua, d->k, d->ub, 0.0, 1.0, dt)) != GH_OK) return st;
-  // u2 = 3/4 u0 + 1/4 (u1 + dt k(u1))
-  if ((st = launch_rhs(d, d->ub, d->k)) != GH_OK) return st;
-  if ((st = launch_rk(d, d->ua, d->ub, d->k, d->ub, 0.75, 0.25, dt)) != GH_OK) return st;
-  // u_new = 1/3 u0 + 2/3 (u2 + dt k(u2))
-  if ((st = launch_rhs(d, d->ub, d->k)) != GH_OK) return st;
-  if ((st = launch_rk(d, d->ua, d->ub, d->k, d->ua, 1.0 / 3.0, 2.0 / 3.0, dt)) != GH_OK) return st;
+  // the stage update (A7) is the epilogue of the fused RHS kernel: d_t u never goes to memory
+  // u1 = u0 + dt k(u0)                      (ua -> ub)
+  if ((st = launch_rhs(d, d->ua, d->ub, 1, nullptr, 0.0, 1.0, dt)) != GH_OK) return st;
+  // u2 = 3/4 u0 + 1/4 (u1 + dt k(u1))       (ub -> ub, in place)
+  if ((st = launch_rhs(d, d->ub, d->ub, 2, d->ua, 0.75, 0.25, dt)) != GH_OK) return st;
+  // u_new = 1/3 u0 + 2/3 (u2 + dt k(u2))    (ub -> ua, over u0)
+  if ((st = launch_rhs(d, d->ub, d->ua, 2, d->ua, 1.0 / 3.0, 2.0 / 3.0, dt)) != GH_OK) return st;
   d->t += dt;
   return GH_OK;
 }

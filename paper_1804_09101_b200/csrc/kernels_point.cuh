@@ -258,13 +258,75 @@ __device__ __forceinline__ void algebraic(const Geom& G, const double (&Pi)[10],
 // Stage 1: psi -> geometry; stage 2: Pi, Phi -> algebraic part (Gam, quadratic sources, C_a);
 // stage 3: per symmetric pair (ab) stream in its 15 derivatives (Jacobian applied on the fly for shells),
 // assemble the 5 outputs and store.  FROZEN faces get zeros (A6).
+//
+// A7 fused: with RK != 0 the kernel does not store d_t u but the Shu-Osher stage update
+//   out = a u0 + b (u + dt d_t u)        (RK = 1: a = 0, u0 not read;  RK = 2: u0 read)
+// using the field values it already holds in registers, which saves writing and re-reading d_t u and re-reading u
+// (1 200 B/point/stage).  `out` may alias `u` or `u0` (in-place stages): every field of the point is in registers
+// before the first store, and u / u0 / out are deliberately NOT __restrict__ so that the compiler cannot re-load them.
 // ---------------------------------------------------------------------------------------------------------
-template <bool SHELL>
+struct RkArgs { const double* u0; double a, b, dt; };
+
+template <int RK>
+__device__ __forceinline__ void rhs_store(double* out, const RkArgs& rk, int64_t idx, double dtu, double us, double u0v) {
+  if (RK == 0) { out[idx] = dtu; return; }
+  double r = rk.b * fma(rk.dt, dtu, us);
+  if (RK == 2) r = fma(rk.a, u0v, r);
+  out[idx] = r;
+}
+
+// Stage-3 operands of the symmetric pair s = (a,b): its 15 logical derivatives and up to 2 gauge-source gradients.
+// Each thread copies ITS OWN point's values with cp.async into its own column of a shared-memory ring
+// ring[slot][RHS_RING_ROWS][TILE_PTS] and later reads them back itself, so no block-level synchronisation is needed:
+// the loads of pairs s .. s+RHS_RING-1 are in flight while the algebra of stage 2 and the assembly of earlier pairs
+// run, which is what an HBM-bound kernel with 255 registers per thread (8 warps per SM) cannot get from the warp
+// scheduler alone.
+constexpr int RHS_RING = 4, RHS_RING_ROWS = 22;   // 15 derivatives + 2 gauge-source gradients + 5 u0 values (RK = 2)
+constexpr size_t RHS_SMEM_BYTES = (size_t)RHS_RING * RHS_RING_ROWS * TILE_PTS * sizeof(double);
+
+template <int PAIR, int RK>
+__device__ __forceinline__ void rhs_prefetch(double* __restrict__ slot /* + tid */, const double* __restrict__ du,
+                                             const double* __restrict__ dHs, const double* u0, int64_t S, int64_t p) {
+  constexpr int a = PAIR < 4 ? 0 : PAIR < 7 ? 1 : PAIR < 9 ? 2 : 3;
+  constexpr int b = PAIR < 4 ? PAIR : PAIR < 7 ? PAIR - 3 : PAIR < 9 ? PAIR - 5 : 3;
+  const int64_t DS = (int64_t)NCOMP * S;
+#pragma unroll
+  for (int c5 = 0; c5 < 5; ++c5)
+#pragma unroll
+    for (int kk = 0; kk < 3; ++kk)
+      cp_async8(slot + (c5 * 3 + kk) * TILE_PTS, du + kk * DS + (int64_t)(10 * c5 + PAIR) * S + p);
+  if (a > 0) cp_async8(slot + 15 * TILE_PTS, dHs + (int64_t)((a - 1) * 4 + b) * S + p);
+  if (b > 0) cp_async8(slot + 16 * TILE_PTS, dHs + (int64_t)((b - 1) * 4 + a) * S + p);
+  if (RK == 2) {
+#pragma unroll
+    for (int c5 = 0; c5 < 5; ++c5) cp_async8(slot + (17 + c5) * TILE_PTS, u0 + (int64_t)(10 * c5 + PAIR) * S + p);
+  }
+  cp_async_commit();
+}
+
+template <bool SHELL, int RK>
 __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __restrict__ tables, int local,
-                                          const double* __restrict__ u, const double* __restrict__ du,
+                                          const double* u, const double* __restrict__ du,
                                           const double* __restrict__ Hs, const double* __restrict__ dHs,
-                                          double* __restrict__ k, int64_t S, int* __restrict__ flag) {
+                                          double* k, const RkArgs& rk, int64_t S, int* __restrict__ flag,
+                                          double* __restrict__ ring /* + tid */) {
   const int64_t p = sd.off + local;
+  // face mask (A6)
+  bool frozen;
+  {
+    const int i2 = local % sd.n2, t = local / sd.n2, i1 = t % sd.n1, i0 = t / sd.n1;
+    frozen = (i0 == 0 && sd.face[0] == 1) || (i0 == sd.n0 - 1 && sd.face[1] == 1);
+    if (!SHELL)
+      frozen = frozen || (i1 == 0 && sd.face[2] == 1) || (i1 == sd.n1 - 1 && sd.face[3] == 1) ||
+               (i2 == 0 && sd.face[4] == 1) || (i2 == sd.n2 - 1 && sd.face[5] == 1);
+  }
+  constexpr int SLOT = RHS_RING_ROWS * TILE_PTS;
+  if (!frozen) {
+    rhs_prefetch<0, RK>(ring + 0 * SLOT, du, dHs, rk.u0, S, p);
+    rhs_prefetch<1, RK>(ring + 1 * SLOT, du, dHs, rk.u0, S, p);
+    rhs_prefetch<2, RK>(ring + 2 * SLOT, du, dHs, rk.u0, S, p);
+    rhs_prefetch<3, RK>(ring + 3 * SLOT, du, dHs, rk.u0, S, p);
+  }
   double psi[10], Pi[10], Phi[3][10], H[4];
 #pragma unroll
   for (int s = 0; s < 10; ++s) psi[s] = u[(int64_t)s * S + p];
@@ -277,22 +339,20 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
 #pragma unroll
   for (int a = 0; a < 4; ++a) H[a] = Hs[(int64_t)a * S + p];
 
-  // face mask (A6)
-  bool frozen;
-  {
-    const int i2 = local % sd.n2, t = local / sd.n2, i1 = t % sd.n1, i0 = t / sd.n1;
-    frozen = (i0 == 0 && sd.face[0] == 1) || (i0 == sd.n0 - 1 && sd.face[1] == 1);
-    if (!SHELL)
-      frozen = frozen || (i1 == 0 && sd.face[2] == 1) || (i1 == sd.n1 - 1 && sd.face[3] == 1) ||
-               (i2 == 0 && sd.face[4] == 1) || (i2 == sd.n2 - 1 && sd.face[5] == 1);
-  }
-
   Geom G;
   const bool ok = geometry(psi, G);
   if (!ok) atomicOr(flag, 1);
   if (!ok || frozen) {
-#pragma unroll 1
-    for (int c = 0; c < NCOMP; ++c) k[(int64_t)c * S + p] = 0.0;
+    cp_async_wait<0>();   // nothing of this thread may still be landing in shared memory when the CTA retires
+#pragma unroll
+    for (int s = 0; s < 10; ++s) {
+      // (frozen points issued no prefetch: u0 comes straight from memory; read before the store, same address when in place)
+      rhs_store<RK>(k, rk, (int64_t)s * S + p, 0.0, psi[s], RK == 2 ? rk.u0[(int64_t)s * S + p] : 0.0);
+      rhs_store<RK>(k, rk, (int64_t)(10 + s) * S + p, 0.0, Pi[s], RK == 2 ? rk.u0[(int64_t)(10 + s) * S + p] : 0.0);
+#pragma unroll
+      for (int i = 0; i < 3; ++i)
+        rhs_store<RK>(k, rk, (int64_t)(20 + 10 * i + s) * S + p, 0.0, Phi[i][s], RK == 2 ? rk.u0[(int64_t)(20 + 10 * i + s) * S + p] : 0.0);
+    }
     return;
   }
   Alg A;
@@ -301,19 +361,23 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
   ShellJac J;
   if (SHELL) J = shell_jac(sd, tables, local);
   const double g0 = sd.gamma[0], g1 = sd.gamma[1], g2 = sd.gamma[2], N = G.N;
-  const int64_t DS = (int64_t)NCOMP * S;   // stride between derivative directions
 
 #pragma unroll
   for (int a = 0; a < 4; ++a)
 #pragma unroll
     for (int b = a; b < 4; ++b) {
       const int s = SI(a, b);
+      // groups committed so far: min(10, s + RHS_RING); group s must have landed
+      if (s + RHS_RING <= 10) cp_async_wait<RHS_RING - 1>();
+      else if (s == 7) cp_async_wait<2>();
+      else if (s == 8) cp_async_wait<1>();
+      else cp_async_wait<0>();
+      const double* __restrict__ slot = ring + (s % RHS_RING) * SLOT;
       // d[c5][k]: Cartesian derivative k of component (psi, Pi, Phi_x, Phi_y, Phi_z)_ab
       double d[5][3];
 #pragma unroll
       for (int c5 = 0; c5 < 5; ++c5) {
-        const double* q = du + (int64_t)(10 * c5 + s) * S + p;
-        const double l0 = q[0], l1 = q[DS], l2 = q[2 * DS];
+        const double l0 = slot[(c5 * 3 + 0) * TILE_PTS], l1 = slot[(c5 * 3 + 1) * TILE_PTS], l2 = slot[(c5 * 3 + 2) * TILE_PTS];
         if (SHELL) {
           d[c5][0] = J.xr * l0 + J.xt * l1 + J.xp * l2;
           d[c5][1] = J.yr * l0 + J.yt * l1 + J.yp * l2;
@@ -322,6 +386,11 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
           d[c5][0] = l0; d[c5][1] = l1; d[c5][2] = l2;
         }
       }
+      double u0v[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+      if (RK == 2) {
+#pragma unroll
+        for (int c5 = 0; c5 < 5; ++c5) u0v[c5] = slot[(17 + c5) * TILE_PTS];
+      }
       double sdpsi = 0.0, sdPi = 0.0, sPhi = 0.0;
 #pragma unroll
       for (int kk = 0; kk < 3; ++kk) {
@@ -329,7 +398,7 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
         sdPi = fma(G.sh[kk], d[1][kk], sdPi);
         sPhi = fma(G.sh[kk], Phi[kk][s], sPhi);
       }
-      k[(int64_t)s * S + p] = (1.0 + g1) * sdpsi - N * Pi[s] - g1 * sPhi;
+      rhs_store<RK>(k, rk, (int64_t)s * S + p, (1.0 + g1) * sdpsi - N * Pi[s] - g1 * sPhi, psi[s], u0v[0]);
 
       double gdPhi = 0.0;   // g^{ki} d_k Phi_iab
 #pragma unroll
@@ -346,9 +415,16 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
       }
       // 1/2 (d_a H_b + d_b H_a), d_0 H = 0 ; dHs[(i*4+b)] = d_i H_b
       double symdH = 0.0;
-      if (a > 0) symdH += dHs[(int64_t)((a - 1) * 4 + b) * S + p];
-      if (b > 0) symdH += dHs[(int64_t)((b - 1) * 4 + a) * S + p];
+      if (a > 0) symdH += slot[15 * TILE_PTS];
+      if (b > 0) symdH += slot[16 * TILE_PTS];
       symdH *= 0.5;
+      // the slot's values are in registers: refill it with pair s + RHS_RING
+      if (s == 0) rhs_prefetch<4, RK>(ring + 0 * SLOT, du, dHs, rk.u0, S, p);
+      if (s == 1) rhs_prefetch<5, RK>(ring + 1 * SLOT, du, dHs, rk.u0, S, p);
+      if (s == 2) rhs_prefetch<6, RK>(ring + 2 * SLOT, du, dHs, rk.u0, S, p);
+      if (s == 3) rhs_prefetch<7, RK>(ring + 3 * SLOT, du, dHs, rk.u0, S, p);
+      if (s == 4) rhs_prefetch<8, RK>(ring + 0 * SLOT, du, dHs, rk.u0, S, p);
+      if (s == 5) rhs_prefetch<9, RK>(ring + 1 * SLOT, du, dHs, rk.u0, S, p);
       double pup = 0.0;
 #pragma unroll
       for (int i = 0; i < 3; ++i) pup = fma(A.p[i], up[i], pup);
@@ -356,7 +432,7 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
       const double tbCa = (b == 0 ? -N * A.C[a] : 0.0), taCb = (a == 0 ? -N * A.C[b] : 0.0);
       double r = sdPi - N * gdPhi + g1 * g2 * (sdpsi - sPhi) + 2.0 * N * (A.S[s] - symdH) - 0.5 * N * A.ttPi * Pi[s] -
                  N * pup + N * g0 * (tbCa + taCb - psi[s] * A.tC);
-      k[(int64_t)(10 + s) * S + p] = r;
+      rhs_store<RK>(k, rk, (int64_t)(10 + s) * S + p, r, Pi[s], u0v[1]);
 #pragma unroll
       for (int i = 0; i < 3; ++i) {
         double sdPhi = 0.0, wup = 0.0;
@@ -364,17 +440,19 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
         for (int kk = 0; kk < 3; ++kk) sdPhi = fma(G.sh[kk], d[2 + i][kk], sdPhi);
 #pragma unroll
         for (int j = 0; j < 3; ++j) wup = fma(A.w[i][j], up[j], wup);
-        k[(int64_t)(20 + 10 * i + s) * S + p] =
-            sdPhi - N * d[1][i] + N * g2 * (d[0][i] - Phi[i][s]) + 0.5 * N * A.s[i] * Pi[s] + N * wup;
+        rhs_store<RK>(k, rk, (int64_t)(20 + 10 * i + s) * S + p,
+                      sdPhi - N * d[1][i] + N * g2 * (d[0][i] - Phi[i][s]) + 0.5 * N * A.s[i] * Pi[s] + N * wup, Phi[i][s], u0v[2 + i]);
       }
     }
 }
 
+template <int RK>
 __global__ void __launch_bounds__(TILE_PTS, 2)
 k_rhs(const SubDev* __restrict__ subs, const int32_t* __restrict__ tile_first, int n_sub,
-      const double* __restrict__ tables, const double* __restrict__ u, const double* __restrict__ du,
-      const double* __restrict__ Hs, const double* __restrict__ dHs, double* __restrict__ k, int64_t S,
+      const double* __restrict__ tables, const double* u, const double* __restrict__ du,
+      const double* __restrict__ Hs, const double* __restrict__ dHs, double* k, RkArgs rk, int64_t S,
       int* __restrict__ flag) {
+  extern __shared__ __align__(16) double ring_s[];   // [RHS_RING][RHS_RING_ROWS][TILE_PTS]
   __shared__ SubDev sd_s;
   __shared__ int tile0_s;
   if (threadIdx.x == 0) {
@@ -386,30 +464,8 @@ k_rhs(const SubDev* __restrict__ subs, const int32_t* __restrict__ tile_first, i
   const SubDev& sd = sd_s;
   const int local = (blockIdx.x - tile0_s) * TILE_PTS + threadIdx.x;
   if (local >= sd.P) return;
-  if (sd.kind == 0) rhs_point<true>(sd, tables, local, u, du, Hs, dHs, k, S, flag);
-  else rhs_point<false>(sd, tables, local, u, du, Hs, dHs, k, S, flag);
-}
-
-// ---------------------------------------------------------------------------------------------------------
-// K_rk (A7): one stage of Shu-Osher SSP-RK3 written as  out = a*u0 + b*(us + dt*k)  over the whole store
-// (padding included; it is zero and stays zero).  Stage 1: a=0,b=1 (u0 not read).
-// ---------------------------------------------------------------------------------------------------------
-template <bool READ_U0>
-__global__ void __launch_bounds__(256)
-k_rk(const double2* __restrict__ u0, const double2* __restrict__ us, const double2* __restrict__ k,
-     double2* __restrict__ out, double a, double b, double dt, int64_t n2) {
-  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n2; i += (int64_t)gridDim.x * blockDim.x) {
-    const double2 s = us[i], kk = k[i];
-    double2 r;
-    r.x = b * fma(dt, kk.x, s.x);
-    r.y = b * fma(dt, kk.y, s.y);
-    if (READ_U0) {
-      const double2 o = u0[i];
-      r.x = fma(a, o.x, r.x);
-      r.y = fma(a, o.y, r.y);
-    }
-    out[i] = r;
-  }
+  if (sd.kind == 0) rhs_point<true, RK>(sd, tables, local, u, du, Hs, dHs, k, rk, S, flag, ring_s + threadIdx.x);
+  else rhs_point<false, RK>(sd, tables, local, u, du, Hs, dHs, k, rk, S, flag, ring_s + threadIdx.x);
 }
 
 // ---------------------------------------------------------------------------------------------------------
