@@ -386,11 +386,6 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
           d[c5][0] = l0; d[c5][1] = l1; d[c5][2] = l2;
         }
       }
-      double u0v[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
-      if (RK == 2) {
-#pragma unroll
-        for (int c5 = 0; c5 < 5; ++c5) u0v[c5] = slot[(17 + c5) * TILE_PTS];
-      }
       double sdpsi = 0.0, sdPi = 0.0, sPhi = 0.0;
 #pragma unroll
       for (int kk = 0; kk < 3; ++kk) {
@@ -398,7 +393,7 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
         sdPi = fma(G.sh[kk], d[1][kk], sdPi);
         sPhi = fma(G.sh[kk], Phi[kk][s], sPhi);
       }
-      rhs_store<RK>(k, rk, (int64_t)s * S + p, (1.0 + g1) * sdpsi - N * Pi[s] - g1 * sPhi, psi[s], u0v[0]);
+      rhs_store<RK>(k, rk, (int64_t)s * S + p, (1.0 + g1) * sdpsi - N * Pi[s] - g1 * sPhi, psi[s], RK == 2 ? slot[17 * TILE_PTS] : 0.0);
 
       double gdPhi = 0.0;   // g^{ki} d_k Phi_iab
 #pragma unroll
@@ -418,13 +413,6 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
       if (a > 0) symdH += slot[15 * TILE_PTS];
       if (b > 0) symdH += slot[16 * TILE_PTS];
       symdH *= 0.5;
-      // the slot's values are in registers: refill it with pair s + RHS_RING
-      if (s == 0) rhs_prefetch<4, RK>(ring + 0 * SLOT, du, dHs, rk.u0, S, p);
-      if (s == 1) rhs_prefetch<5, RK>(ring + 1 * SLOT, du, dHs, rk.u0, S, p);
-      if (s == 2) rhs_prefetch<6, RK>(ring + 2 * SLOT, du, dHs, rk.u0, S, p);
-      if (s == 3) rhs_prefetch<7, RK>(ring + 3 * SLOT, du, dHs, rk.u0, S, p);
-      if (s == 4) rhs_prefetch<8, RK>(ring + 0 * SLOT, du, dHs, rk.u0, S, p);
-      if (s == 5) rhs_prefetch<9, RK>(ring + 1 * SLOT, du, dHs, rk.u0, S, p);
       double pup = 0.0;
 #pragma unroll
       for (int i = 0; i < 3; ++i) pup = fma(A.p[i], up[i], pup);
@@ -432,7 +420,7 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
       const double tbCa = (b == 0 ? -N * A.C[a] : 0.0), taCb = (a == 0 ? -N * A.C[b] : 0.0);
       double r = sdPi - N * gdPhi + g1 * g2 * (sdpsi - sPhi) + 2.0 * N * (A.S[s] - symdH) - 0.5 * N * A.ttPi * Pi[s] -
                  N * pup + N * g0 * (tbCa + taCb - psi[s] * A.tC);
-      rhs_store<RK>(k, rk, (int64_t)(10 + s) * S + p, r, Pi[s], u0v[1]);
+      rhs_store<RK>(k, rk, (int64_t)(10 + s) * S + p, r, Pi[s], RK == 2 ? slot[18 * TILE_PTS] : 0.0);
 #pragma unroll
       for (int i = 0; i < 3; ++i) {
         double sdPhi = 0.0, wup = 0.0;
@@ -441,8 +429,16 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
 #pragma unroll
         for (int j = 0; j < 3; ++j) wup = fma(A.w[i][j], up[j], wup);
         rhs_store<RK>(k, rk, (int64_t)(20 + 10 * i + s) * S + p,
-                      sdPhi - N * d[1][i] + N * g2 * (d[0][i] - Phi[i][s]) + 0.5 * N * A.s[i] * Pi[s] + N * wup, Phi[i][s], u0v[2 + i]);
+                      sdPhi - N * d[1][i] + N * g2 * (d[0][i] - Phi[i][s]) + 0.5 * N * A.s[i] * Pi[s] + N * wup, Phi[i][s], RK == 2 ? slot[(19 + i) * TILE_PTS] : 0.0);
       }
+      // every value of the slot has been consumed: refill it with pair s + RHS_RING
+      if (s == 0) rhs_prefetch<4, RK>(ring + 0 * SLOT, du, dHs, rk.u0, S, p);
+      if (s == 1) rhs_prefetch<5, RK>(ring + 1 * SLOT, du, dHs, rk.u0, S, p);
+      if (s == 2) rhs_prefetch<6, RK>(ring + 2 * SLOT, du, dHs, rk.u0, S, p);
+      if (s == 3) rhs_prefetch<7, RK>(ring + 3 * SLOT, du, dHs, rk.u0, S, p);
+      if (s == 4) rhs_prefetch<8, RK>(ring + 0 * SLOT, du, dHs, rk.u0, S, p);
+      if (s == 5) rhs_prefetch<9, RK>(ring + 1 * SLOT, du, dHs, rk.u0, S, p);
+
     }
 }
 
