@@ -5,7 +5,7 @@
 
 Metric (BASELINE.json): GH RHS grid-point evaluations per second, FP64.  One "step" is one pass of the whole
 hot path (rows A2-A8) over the workload: one `gh_rk_step` (3 x [Chebyshev + angular derivatives,
-fused Jacobian + pointwise RHS + face mask] + 3 fused RK3 stage updates) followed by one `gh_constraint_norms`
+fused Jacobian + pointwise RHS + face mask + RK3 stage update as its epilogue]) followed by one `gh_constraint_norms`
 (derivatives + constraint kernel + reduction).  value = 3 * P * K / T: only the three RHS evaluations of the RK3
 step are counted as "evaluations"; the constraint pass is extra work inside the timed region.
 
@@ -40,8 +40,10 @@ METRIC = "gh_rhs_grid_point_evals_per_s"
 UNIT = "points/s"
 
 # algorithmic traffic per grid point and launch, DESIGN.md §5
-BYTES_RHS_PT = (50 + 150 + 4 + 12 + 50) * 8      # k_rhs: 216 reads (+ table lookups, cached) + 50 writes = 2 128 B
-BYTES_RK_PT = {True: (3 + 1) * 50 * 8, False: (2 + 1) * 50 * 8}   # k_rk: u0?, u_s, k -> out
+BYTES_RHS_PT = (50 + 150 + 4 + 12 + 50) * 8      # k_rhs as gh_rhs: 216 reads (+ table lookups, cached) + 50 writes = 2 128 B
+# inside gh_rk_step the stage update (A7) is the epilogue of k_rhs: stage 1 moves the same 2 128 B (writes u1 instead of
+# d_t u), stages 2 and 3 also read u0: 2 528 B.  Average over the three launches of a step:
+BYTES_RHS_RK_PT = (BYTES_RHS_PT + 2 * (BYTES_RHS_PT + 50 * 8)) / 3.0
 FLOP_RHS_PT = 4391                                # SURVEY.md §8(a) A4+A5 instrumented count
 
 
@@ -54,10 +56,13 @@ def load_peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-# FP64 FMA-pipe peak for the derivative kernels: 148 SMs x 64 DFMA lanes x 2 flop x clock.  Quoted at
-# the max SM clock; the clock actually held is in the "clocks" key.
-def fp64_peak_tflops(sm_mhz: float = 1965.0) -> float:
-    return 148 * 64 * 2 * sm_mhz * 1e6 / 1e12
+# FP64 peak for the derivative kernels (bound "alu"): measured with paper_1804_09101_b200/tools/fp64_peak.cu on this
+# pool's B200 at 1965 MHz; DFMA and DMMA share one datapath (mixing them gains nothing), DESIGN.md §6.
+FP64_PEAK_MEASURED_TFLOPS = 37.1    # DMMA m8n8k4, register resident, profiles/r01_fp64_peak.md (DFMA: 33.9; nominal 37.2)
+
+
+def fp64_peak_tflops() -> float:
+    return FP64_PEAK_MEASURED_TFLOPS
 
 
 # ------------------------------------------------------------------------------------------------------------------
@@ -224,8 +229,7 @@ def kernel_work(descs):
             cheb_flop += 50.0 * p * sum(2 * n - 1 for n in d["n"])
     return {
         "P": P,
-        "k_rhs": {"bytes": float(BYTES_RHS_PT) * P, "flop": float(FLOP_RHS_PT) * P, "bound": "hbm"},
-        "k_rk": {"bytes": None, "flop": 200.0 * P, "bound": "hbm"},       # bytes depend on the stage, filled by the caller
+        "k_rhs": {"bytes": float(BYTES_RHS_RK_PT) * P, "flop": float(FLOP_RHS_PT + 200) * P, "bound": "hbm"},
         "k_con": {"bytes": (50 + 120 + 4) * 8.0 * P, "flop": 1200.0 * P, "bound": "hbm"},
         "k_cheb": {"bytes": 8.0 * (50 * Ps + 50 * Ps + 50 * Pb + 150 * Pb), "flop": cheb_flop, "bound": "alu"},
         "k_ang": {"bytes": 8.0 * (50 + 100) * Ps, "flop": ang_flop, "bound": "alu"},
@@ -248,6 +252,25 @@ def read_traffic(kernel: str, P: int):
                 except ValueError:
                     continue
     return None
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# multi-rank bookkeeping ("replicas only"): no data-path collective, only the timing reduction
+# ------------------------------------------------------------------------------------------------------------------
+def max_over_ranks(values, dist, device):
+    """MAX over ranks of each entry of `values` (device times); identity when dist is None."""
+    if dist is None:
+        return [float(v) for v in values]
+    import torch
+
+    t = torch.tensor([float(v) for v in values], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t]
+
+
+def whole_job_value(world: int, points_per_rank: int, steps: int, ms_max: float) -> float:
+    """Replicas: every rank evaluates 3 RHS per step on its own copy; the job's rate divides by the slowest rank's time."""
+    return world * 3.0 * points_per_rank * steps / (ms_max * 1e-3)
 
 
 # ------------------------------------------------------------------------------------------------------------------
@@ -352,11 +375,7 @@ def run_ours(args):
     if not bool(torch.isfinite(out_host).all()):
         raise SystemExit("bench.py: non-finite state after the e2e region")
 
-    tmax, e2emax = ms, e2e_s / e2e_steps
-    if dist is not None:
-        t = torch.tensor([ms, e2e_s / e2e_steps], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        tmax, e2emax = float(t[0]), float(t[1])
+    tmax, e2emax = max_over_ranks([ms, e2e_s / e2e_steps], dist, dev)
     if rank != 0:
         dom.close()
         if dist is not None:
@@ -370,11 +389,10 @@ def finish_ours(args, world, label, cfg, descs, reps, P, S, ms, e2e_step_s, e2e_
                 norms, base, dom, dist):
     hbm_peak, peak_src = load_peaks()
     steps = args.steps
-    value = world * 3.0 * P * steps / (ms * 1e-3)
+    value = whole_job_value(world, P, steps, ms)
     # per-kernel numbers from the CUDA events the library records around each launch on its own stream
-    work["k_rk"]["bytes"] = P * (BYTES_RK_PT[False] + 2 * BYTES_RK_PT[True]) / 3.0
     total_kernel_ms = sum(v[0] for v in prof.values()) or 1.0
-    calls_per_step = {"k_rhs": 3, "k_rk": 3, "k_con": 1, "k_cheb": 4, "k_ang": 4}   # library calls that run the kernel
+    calls_per_step = {"k_rhs": 3, "k_con": 1, "k_cheb": 4, "k_ang": 4}   # library calls that run the kernel
     kernels = {}
     for name, (kms, cnt) in prof.items():
         if cnt == 0:
@@ -400,7 +418,7 @@ def finish_ours(args, world, label, cfg, descs, reps, P, S, ms, e2e_step_s, e2e_
     else:
         roof = {"kernel": top, "bound": "alu", "achieved": kernels[top]["achieved_TFLOPs"], "peak": fp64_peak, "unit": "TFLOP/s",
                 "frac": kernels[top]["achieved_TFLOPs"] / fp64_peak,
-                "peak_source": "derived: 148 SM x 64 FP64 FMA lanes x 2 x 1.965 GHz (DESIGN.md §5)",
+                "peak_source": "measured: DMMA m8n8k4 register-resident microbenchmark on this pool's B200 (profiles/r01_fp64_peak.md)",
                 "algorithmic_flop_per_launch": work[top]["flop"], "traffic": read_traffic(top, P)}
     # the fused RHS kernel is the one north_star sets a target for: always report it too
     roof_rhs = None
