@@ -46,9 +46,10 @@ struct AngItem {
   int32_t plane0;
   int32_t nplanes;
   int32_t nb_alloc;              // planes the shared-memory layout is sized for (>= nplanes)
-  int32_t m_Fa, m_Fs, m_T;       // offsets (doubles) in the table memory, all in DMMA fragment order: Fa [k_step][n_tile][32],
-                                 // Fs [k_step][n_tile][32], stacked per-m matrices [Th_m ; m Pr_m] as [m][k_step][m_tile][32]
-  int16_t nch1, nch3;            // n-chunks per m-tile in S1 / S3 (host-chosen for the best balance over the warps)
+  int32_t m_Fa, m_Fs, m_T;       // offsets (doubles) in the table memory, all in DMMA fragment order [k_step][n_tile][32]:
+                                 // Fa = (even | odd) analysis, Fs = (even | odd) synthesis (see K_ang); stacked per-m
+                                 // matrices [Th_m ; m Pr_m] as [m][k_step][m_tile][32]
+  int8_t nch1e, nch1o, nch3, pad8_;   // n-chunks per m-tile in S1 (even, odd GEMM) / S3 (host-chosen for balance over the warps)
 };
 
 }  // namespace ghd

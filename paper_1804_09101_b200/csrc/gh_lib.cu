@@ -66,9 +66,9 @@ inline void sub_dims(const gh_subdomain_desc& d, int& n0, int& n1, int& n2) {
 
 // K_ang shared memory for nb planes of band limit L: X and Y ([nb][plane stride]) + F ([n_phi rounded to 8][pitch])
 // n-chunks per m-tile that minimise (rounds over the warps) x (DMMAs per unit + fixed cost); w = DMMAs per n-tile and k-step
-inline int ang_best_nch(int NT, int MT1, int NW, int w) {
+inline int ang_best_nch(int NT, int MT1, int NW, int w, int per_max) {
   int best = 0; double bc = 1e300;
-  for (int nch = (NT + ANG_NTC - 1) / ANG_NTC; nch <= NT; ++nch) {
+  for (int nch = (NT + per_max - 1) / per_max; nch <= NT; ++nch) {
     const int per = (NT + nch - 1) / nch;
     if ((NT + per - 1) / per != nch) continue;          // same chunking the kernel derives from nch
     const double cost = (double)((MT1 * nch + NW - 1) / NW) * (w * per + 0.6);
@@ -77,8 +77,8 @@ inline int ang_best_nch(int NT, int MT1, int NW, int w) {
   return best;
 }
 inline size_t ang_smem_bytes(int L, int nb) { return ang_smem_doubles(L, nb) * sizeof(double); }
-inline size_t shell_fa_doubles(int L) { return (size_t)((2 * L + 2 + 3) / 4) * ((2 * L + 1 + 7) / 8) * 32; }   // [k_step][n_tile][32]
-inline size_t shell_fs_doubles(int L) { return (size_t)((2 * L + 1 + 3) / 4) * ((2 * L + 2 + 7) / 8) * 32; }
+inline size_t shell_fa_doubles(int L) { return ang_fa_doubles(L); }   // (even | odd) analysis fragments
+inline size_t shell_fs_doubles(int L) { return ang_fs_doubles(L); }   // (even | odd) synthesis fragments
 inline size_t shell_t_doubles(int L) {    // [m][k_step][m_tile][32], stacked [Th_m ; m Pr_m], see AngItem
   const size_t nt = L + 1, mtn = (2 * nt + 7) / 8, ks = (nt + 3) / 4;
   return (size_t)(L + 1) * ks * mtn * 32;
@@ -361,20 +361,33 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
         // all three operands in DMMA fragment order, zero padded to whole tiles; lane = 4 g + t
         {
           const int np = 2 * L + 2, nq = 2 * L + 1, nt = L + 1;
-          // Fa as the B operand of S1: fragment (k_step, n_tile): element (k = 4 ks + t, n = 8 nt_ + g) = Fa[q = n][k]
-          const int ksp = (np + 3) / 4, ntq = (nq + 7) / 8;
+          // The real DFT is folded about phi = pi (K_ang S0): with h = L+1 = np/2,
+          //   even analysis  B[k = 0..h][m = 0..L]      = Fa[m][k]            (cos rows; the weight of k and np-k is the same)
+          //   odd  analysis  B[k' = k-1, k = 1..L][m' = m-1, m = 1..L] = Fa[L+m][k]   (sin rows)
+          // fragment (k_step, n_tile): element (K index 4 ks + t, N index 8 n + g)
+          const AngDims dm = ang_dims(L);
+          const int h = dm.h;
           std::vector<ghb::ld> FA(shell_fa_doubles(L), 0);
-          for (int ks = 0; ks < ksp; ++ks) for (int n = 0; n < ntq; ++n) for (int lane = 0; lane < 32; ++lane) {
-            const int k = ks * 4 + lane % 4, q = n * 8 + lane / 4;
-            if (k < np && q < nq) FA[((size_t)ks * ntq + n) * 32 + lane] = B.Fa[(size_t)q * np + k];
+          for (int ks = 0; ks < dm.KSe1; ++ks) for (int n = 0; n < dm.NTc; ++n) for (int lane = 0; lane < 32; ++lane) {
+            const int k = ks * 4 + lane % 4, m = n * 8 + lane / 4;
+            if (k <= h && m <= L) FA[((size_t)ks * dm.NTc + n) * 32 + lane] = B.Fa[(size_t)m * np + k];
+          }
+          const size_t fao = (size_t)dm.KSe1 * dm.NTc * 32;
+          for (int ks = 0; ks < dm.KSo1; ++ks) for (int n = 0; n < dm.NTs; ++n) for (int lane = 0; lane < 32; ++lane) {
+            const int k = ks * 4 + lane % 4 + 1, m = n * 8 + lane / 4 + 1;
+            if (k <= L && m <= L) FA[fao + ((size_t)ks * dm.NTs + n) * 32 + lane] = B.Fa[(size_t)(L + m) * np + k];
           }
           o.Fa = put(FA);
-          // Fs as the B operand of S3: element (k = q = 4 ks + t, n = phi index 8 nt_ + g) = Fs[phi][q]
-          const int ksq = (nq + 3) / 4, ntp = (np + 7) / 8;
+          //   even synthesis B[m = 0..L][k = 0..h] = Fs[k][m];   odd synthesis B[m' = m-1][k = 0..h] = Fs[k][L+m], zero at k = 0, h
           std::vector<ghb::ld> FS(shell_fs_doubles(L), 0);
-          for (int ks = 0; ks < ksq; ++ks) for (int n = 0; n < ntp; ++n) for (int lane = 0; lane < 32; ++lane) {
-            const int q = ks * 4 + lane % 4, k = n * 8 + lane / 4;
-            if (q < nq && k < np) FS[((size_t)ks * ntp + n) * 32 + lane] = B.Fs[(size_t)k * nq + q];
+          for (int ks = 0; ks < dm.KSe3; ++ks) for (int n = 0; n < dm.NT3; ++n) for (int lane = 0; lane < 32; ++lane) {
+            const int m = ks * 4 + lane % 4, k = n * 8 + lane / 4;
+            if (m <= L && k <= h) FS[((size_t)ks * dm.NT3 + n) * 32 + lane] = B.Fs[(size_t)k * nq + m];
+          }
+          const size_t fso = (size_t)dm.KSe3 * dm.NT3 * 32;
+          for (int ks = 0; ks < dm.KSo3; ++ks) for (int n = 0; n < dm.NT3; ++n) for (int lane = 0; lane < 32; ++lane) {
+            const int m = ks * 4 + lane % 4 + 1, k = n * 8 + lane / 4;
+            if (m <= L && k >= 1 && k < h) FS[fso + ((size_t)ks * dm.NT3 + n) * 32 + lane] = B.Fs[(size_t)k * nq + L + m];
           }
           o.Fs = put(FS);
           // stacked [Th_m ; m Pr_m] (2 nt x nt) as the A operand of S2: element (row = 8 mt + g, col = 4 ks + t)
@@ -415,8 +428,10 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
         it.m_Fa = o.Fa; it.m_Fs = o.Fs; it.m_T = o.T;
         {
           const int NW = (pl.ang_class[s] ? ANG_TPB1 : ANG_TPB0) / 32, MT1 = (it.nplanes * (L + 1) + 7) / 8;
-          it.nch1 = (int16_t)ang_best_nch((2 * L + 1 + 7) / 8, MT1, NW, 1);
-          it.nch3 = (int16_t)ang_best_nch((2 * L + 2 + 7) / 8, MT1, NW, 2);
+          const AngDims dm = ang_dims(L);
+          it.nch1e = (int8_t)ang_best_nch(dm.NTc, MT1, NW, 1, ANG_NTC);
+          it.nch1o = (int8_t)ang_best_nch(dm.NTs, MT1, NW, 1, ANG_NTC);
+          it.nch3 = (int8_t)ang_best_nch(dm.NT3, MT1, NW, 4, ANG_NTC3);
         }
         (pl.ang_class[s] ? ang1 : ang).push_back(it);
       }

@@ -119,32 +119,51 @@ k_cheb(const ChebItem* __restrict__ items, const double* __restrict__ tables, co
 
 // ---------------------------------------------------------------------------------------------------------
 // K_ang.  grid = (n_items, ncomp).  One CTA: `nb` (theta,phi) planes of one component of one shell, kept in shared
-// memory through three GEMM stages on the FP64 tensor cores (mma.sync.m8n8k4):
-//   S1  C[r][q]        = sum_k  U[r][k] Fa[q][k]             rows r = (plane b, theta j); real DFT, Nyquist dropped
-//   S2  [A ; B'](m)    = [Th_m ; m Pr_m] C_m                  per m, columns (t = cos/sin, plane b); A in place over C,
-//                                                             B' into the cos<->sin partner slot with sign: d/dphi
-//   S3  d_theta u[r][k] = sum_q A[r][q] Fs[k][q],   d_phi u[r][k] = sum_q B'[r][q] Fs[k][q]
+// memory through three GEMM stages on the FP64 tensor cores (mma.sync.m8n8k4).  With h = L+1 = n_phi/2:
+//   S0  fold    E_k = U_k + U_{n_phi-k}, O_k = U_k - U_{n_phi-k} (k = 1..L), E_0 = U_0, E_h = U_h: cos(m phi) is even and
+//               sin(m phi) odd about phi = pi, so the real DFT splits into two half-length ones (half the flop of S1, S3)
+//   S1  Cc[r][m] = sum_{k=0..h} E[r][k] Fa_c[m][k]  (m = 0..L),   Cs[r][m] = sum_{k=1..L} O[r][k] Fa_s[m][k]  (m = 1..L)
+//   S2  [A ; B'](m) = [Th_m ; m Pr_m] C_m   per m, columns (t = cos/sin, plane b); A in place over C, B' into the
+//               cos<->sin partner slot with sign (d/dphi in coefficient space)
+//   S3  e[r][k] = sum_m Ac[r][m] Fs_c[k][m],  o[r][k] = sum_m As[r][m] Fs_s[k][m]  (k = 0..h), same for B';
+//               d u[r][k] = e + o,  d u[r][n_phi-k] = e - o, stored straight from the accumulators
 // Every matrix operand is stored in DMMA fragment order, zero padded to whole tiles ([k_step][tile][32 lanes]: one
 // conflict-free LDS.64 / coalesced 256-byte LDG per fragment, tile offsets are immediates), so the inner loops carry
-// no bounds predicate: about 2-3 issued instructions per DMMA.  Fa / Fs fragments live in shared memory; the per-m
-// stacked matrices [Th_m ; m Pr_m] stream from L2 one k-step ahead.  Planes: X (U, later B') and Y (C, later A), row
-// (b, j) at b*ps + j*pitch doubles; pitch = 4 mod 8 and ps = 1 mod 16 keep the data-fragment loads conflict-free.
-// Rows beyond the tile range read a zeroed row.  Outputs go straight from the S3 accumulators to global memory.
+// no bounds predicate.  Fa / Fs fragments live in shared memory; the per-m stacked matrices [Th_m ; m Pr_m] stream
+// from L2 two k-steps ahead.  Planes: X (folded U, later B') and Y (C, later A), row (b, j) at b*ps + j*pitch
+// doubles; coefficient rows hold cos m at column m and sin m at column kc + m - 1 (kc = 8 ceil(h/8)); folded rows
+// hold E at 0..h and O at ke.. (ke = 4 ceil((h+1)/4)).  pitch = 4 mod 8 and ps = 1 mod 16 keep the data-fragment
+// loads conflict-free.  Rows beyond the tile range read a zeroed row.
 // ---------------------------------------------------------------------------------------------------------
-__host__ __device__ inline int ang_pitch(int L) {   // row pitch (doubles): >= 8*ceil(n_q/8) and 4*ceil(n_phi/4), = 4 mod 8
-  const int a = (2 * L + 1 + 7) / 8 * 8, b = (2 * L + 2 + 3) / 4 * 4;
+struct AngDims {
+  int h, KSe1, NTc, KSo1, NTs, kc, ke, KSe3, KSo3, NT3;
+};
+__host__ __device__ inline AngDims ang_dims(int L) {
+  AngDims d;
+  d.h = L + 1;
+  d.KSe1 = (d.h + 1 + 3) / 4; d.NTc = (d.h + 7) / 8;      // S1 even: K = h+1 (k = 0..h),  N = h   (m = 0..L)
+  d.KSo1 = (L + 3) / 4;       d.NTs = (L + 7) / 8;        // S1 odd:  K = L   (k = 1..L),  N = L   (m = 1..L)
+  d.kc = 8 * d.NTc; d.ke = 4 * d.KSe1;
+  d.KSe3 = (d.h + 3) / 4; d.KSo3 = (L + 3) / 4;           // S3: K = h (m = 0..L) / L (m = 1..L)
+  d.NT3 = (d.h + 1 + 7) / 8;                              //     N = h+1 (k = 0..h) for both
+  return d;
+}
+__host__ __device__ inline int ang_pitch(int L) {   // row pitch (doubles), = 4 mod 8
+  const AngDims d = ang_dims(L);
+  const int a = d.kc + 8 * d.NTs, b = d.ke + 4 * d.KSo1;
   int p = a > b ? a : b;
   return (p % 8 == 0) ? p + 4 : p;
 }
 __host__ __device__ inline int ang_plane_stride(int L) {   // plane stride (doubles): rows padded to 4, = 1 mod 16
   return ((L + 1 + 3) / 4 * 4 * ang_pitch(L) + 15) / 16 * 16 + 1;
 }
-// shared memory (doubles) of K_ang for nb planes: X, Y, one zero row, F fragments, row-offset table (ints)
+__host__ __device__ inline size_t ang_fa_doubles(int L) { const AngDims d = ang_dims(L); return (size_t)(d.KSe1 * d.NTc + d.KSo1 * d.NTs) * 32; }
+__host__ __device__ inline size_t ang_fs_doubles(int L) { const AngDims d = ang_dims(L); return (size_t)(d.KSe3 + d.KSo3) * d.NT3 * 32; }
 __host__ __device__ inline size_t ang_f_doubles(int L) {
-  const size_t np = 2 * L + 2, nq = 2 * L + 1;
-  const size_t fa = ((np + 3) / 4) * ((nq + 7) / 8) * 32, fs = ((nq + 3) / 4) * ((np + 7) / 8) * 32;
+  const size_t fa = ang_fa_doubles(L), fs = ang_fs_doubles(L);
   return fa > fs ? fa : fs;
 }
+// shared memory (doubles) of K_ang for nb planes: X, Y, one zero row, F fragments, row-offset table (ints)
 __host__ __device__ inline size_t ang_smem_doubles(int L, int nb) {
   const size_t rows = (size_t)nb * (L + 1);
   return 2 * (size_t)nb * ang_plane_stride(L) + ang_pitch(L) + 16 + ang_f_doubles(L) + ((rows + 8) * sizeof(int) + 7) / 8;
@@ -185,34 +204,62 @@ __device__ __forceinline__ void ang_s1_unit(const double* __restrict__ ap, const
   }
 }
 
-// S3 unit: one m-tile x NTC n-tiles, both parts (theta from Y, phi from X) sharing the Fs fragments
+// S3 unit: one m-tile x NTC n-tiles (columns k = 0..h), both parts (theta from Y, phi from X), even and odd GEMMs;
+// a0p / a1p: this lane's rows (+ tl) of Y / X at the cos region; the sin region starts kc doubles further.
 template <int NTC>
-__device__ __forceinline__ void ang_s3_unit(const double* __restrict__ a0p, const double* __restrict__ a1p,
-                                            const double* __restrict__ bp, int KS, int NT, double* __restrict__ g0,
-                                            double* __restrict__ g1, int c0, int np, bool rok) {
-  double acc0[NTC][2], acc1[NTC][2];
+__device__ __forceinline__ void ang_s3_unit(const double* __restrict__ a0p, const double* __restrict__ a1p, int kc,
+                                            const double* __restrict__ bpe, const double* __restrict__ bpo, int KSe,
+                                            int KSo, int NT, double* __restrict__ g0, double* __restrict__ g1, int c0,
+                                            int h, int np, bool rok) {
+  double e0[NTC][2], e1[NTC][2], o0[NTC][2], o1[NTC][2];
 #pragma unroll
-  for (int n = 0; n < NTC; ++n) acc0[n][0] = acc0[n][1] = acc1[n][0] = acc1[n][1] = 0.0;
+  for (int n = 0; n < NTC; ++n) {
+    e0[n][0] = e0[n][1] = e1[n][0] = e1[n][1] = 0.0;
+    o0[n][0] = o0[n][1] = o1[n][0] = o1[n][1] = 0.0;
+  }
   const int bstep = NT * 32;
+  {
+    const double* p0 = a0p; const double* p1 = a1p;
 #pragma unroll 2
-  for (int ks = 0; ks < KS; ++ks) {
-    const double a0 = a0p[0], a1 = a1p[0];
+    for (int ks = 0; ks < KSe; ++ks) {
+      const double a0 = p0[0], a1 = p1[0];
 #pragma unroll
-    for (int n = 0; n < NTC; ++n) {
-      const double b = bp[n * 32];
-      dmma884(acc0[n][0], acc0[n][1], a0, b);
-      dmma884(acc1[n][0], acc1[n][1], a1, b);
+      for (int n = 0; n < NTC; ++n) {
+        const double b = bpe[n * 32];
+        dmma884(e0[n][0], e0[n][1], a0, b);
+        dmma884(e1[n][0], e1[n][1], a1, b);
+      }
+      p0 += 4; p1 += 4; bpe += bstep;
     }
-    a0p += 4; a1p += 4; bp += bstep;
+  }
+  {
+    const double* p0 = a0p + kc; const double* p1 = a1p + kc;
+#pragma unroll 2
+    for (int ks = 0; ks < KSo; ++ks) {
+      const double a0 = p0[0], a1 = p1[0];
+#pragma unroll
+      for (int n = 0; n < NTC; ++n) {
+        const double b = bpo[n * 32];
+        dmma884(o0[n][0], o0[n][1], a0, b);
+        dmma884(o1[n][0], o1[n][1], a1, b);
+      }
+      p0 += 4; p1 += 4; bpo += bstep;
+    }
   }
   if (rok) {
 #pragma unroll
     for (int n = 0; n < NTC; ++n) {
-      const int c = c0 + n * 8;
-      if (c < np) {
-        *reinterpret_cast<double2*>(g0 + c) = make_double2(acc0[n][0], acc0[n][1]);
-        *reinterpret_cast<double2*>(g1 + c) = make_double2(acc1[n][0], acc1[n][1]);
+      const int k = c0 + n * 8;             // even; this lane holds columns k and k + 1
+      if (k + 1 <= h) {
+        *reinterpret_cast<double2*>(g0 + k) = make_double2(e0[n][0] + o0[n][0], e0[n][1] + o0[n][1]);
+        *reinterpret_cast<double2*>(g1 + k) = make_double2(e1[n][0] + o1[n][0], e1[n][1] + o1[n][1]);
+      } else if (k <= h) {
+        g0[k] = e0[n][0] + o0[n][0];
+        g1[k] = e1[n][0] + o1[n][0];
       }
+      // mirror columns n_phi - k (k = 1..L)
+      if (k >= 1 && k < h) { g0[np - k] = e0[n][0] - o0[n][0]; g1[np - k] = e1[n][0] - o1[n][0]; }
+      if (k + 1 < h) { g0[np - k - 1] = e0[n][1] - o0[n][1]; g1[np - k - 1] = e1[n][1] - o1[n][1]; }
     }
   }
 }
@@ -221,30 +268,46 @@ __device__ __forceinline__ void ang_s3_unit(const double* __restrict__ a0p, cons
 template <int MT2>
 __device__ __forceinline__ void ang_s2_unit(const double* __restrict__ tp /* T_m fragments + lane */, int KS2,
                                             double* __restrict__ X, double* __restrict__ Y, int m, int ntile, int nb,
-                                            int L, int pitch, int ps, int g, int tl) {
+                                            int L, int kc, int pitch, int ps, int g, int tl) {
   const int nt = L + 1, ncols = (m == 0) ? nb : 2 * nb;
+  const int slot_c = m, slot_s = kc + m - 1;      // coefficient columns of cos m / sin m
   // B fragment column of this lane
   const int cb = ntile * 8 + g;
   const bool bok = cb < ncols;
   const int tb = (bok && cb >= nb) ? 1 : 0, bb = bok ? cb - tb * nb : 0;
-  const double* __restrict__ yp = Y + bb * ps + (tb ? L + m : m) + tl * pitch;
+  const double* __restrict__ yp = Y + bb * ps + (tb ? slot_s : slot_c) + tl * pitch;
   double acc[MT2][2];
 #pragma unroll
   for (int mt = 0; mt < MT2; ++mt) acc[mt][0] = acc[mt][1] = 0.0;
-  double an[MT2];
+  // A fragments one k-step ahead, two when the m-tile count leaves registers for it (L2 latency)
+  constexpr bool DEEP = MT2 <= 6;
+  double a1[MT2], a2[DEEP ? MT2 : 1];
 #pragma unroll
-  for (int mt = 0; mt < MT2; ++mt) an[mt] = __ldg(tp + mt * 32);
+  for (int mt = 0; mt < MT2; ++mt) a1[mt] = __ldg(tp + mt * 32);
+  tp += MT2 * 32;
+  if (DEEP) {
+#pragma unroll
+    for (int mt = 0; mt < MT2; ++mt) a2[DEEP ? mt : 0] = (KS2 > 1) ? __ldg(tp + mt * 32) : 0.0;
+    tp += MT2 * 32;
+  }
   const int ystep = 4 * pitch;
 #pragma unroll 1
   for (int ks = 0; ks < KS2; ++ks) {
     double a[MT2];
 #pragma unroll
-    for (int mt = 0; mt < MT2; ++mt) a[mt] = an[mt];
-    tp += MT2 * 32;
-    if (ks + 1 < KS2) {
+    for (int mt = 0; mt < MT2; ++mt) a[mt] = a1[mt];
+    if (DEEP) {
 #pragma unroll
-      for (int mt = 0; mt < MT2; ++mt) an[mt] = __ldg(tp + mt * 32);
+      for (int mt = 0; mt < MT2; ++mt) a1[mt] = a2[DEEP ? mt : 0];
+      if (ks + 2 < KS2) {
+#pragma unroll
+        for (int mt = 0; mt < MT2; ++mt) a2[DEEP ? mt : 0] = __ldg(tp + mt * 32);
+      }
+    } else if (ks + 1 < KS2) {
+#pragma unroll
+      for (int mt = 0; mt < MT2; ++mt) a1[mt] = __ldg(tp + mt * 32);
     }
+    tp += MT2 * 32;
     const double yv = yp[0];
     const double b = bok ? yv : 0.0;
     yp += ystep;
@@ -252,31 +315,27 @@ __device__ __forceinline__ void ang_s2_unit(const double* __restrict__ tp /* T_m
     for (int mt = 0; mt < MT2; ++mt) dmma884(acc[mt][0], acc[mt][1], a[mt], b);
   }
   __syncwarp();   // every lane has read its C_m entries before any lane overwrites them
-  // C fragment: stacked row 8 mt + g, columns 8 ntile + 2 tl + e
-  int coff[2]; int ctt[2]; bool cok[2];
+  // C fragment: stacked row 8 mt + g, columns 8 ntile + 2 tl + e.  Destination per column e: A -> Y at the same slot;
+  // B' -> X at the partner slot with sign (cos input -> sin slot, negated; sin input -> cos slot); m = 0 -> 0
+  double* ydst[2]; double* xdst[2]; double sgn[2]; bool cok[2];
 #pragma unroll
   for (int e = 0; e < 2; ++e) {
     const int c = ntile * 8 + 2 * tl + e;
     cok[e] = c < ncols;
-    ctt[e] = (cok[e] && c >= nb) ? 1 : 0;
-    coff[e] = (cok[e] ? c - ctt[e] * nb : 0) * ps;
+    const int t = (cok[e] && c >= nb) ? 1 : 0, bq = cok[e] ? c - t * nb : 0;
+    ydst[e] = Y + bq * ps + (t ? slot_s : slot_c);
+    xdst[e] = X + bq * ps + ((t || m == 0) ? slot_c : slot_s);
+    sgn[e] = (m == 0) ? 0.0 : (t ? 1.0 : -1.0);
   }
 #pragma unroll
   for (int mt = 0; mt < MT2; ++mt) {
     const int rr = mt * 8 + g;
-    if (rr < 2 * nt) {
-      const bool phi = rr >= nt;
-      const int jo = (phi ? rr - nt : rr) * pitch;
+    if (rr < nt) {
 #pragma unroll
-      for (int e = 0; e < 2; ++e)
-        if (cok[e]) {
-          const double v = acc[mt][e];
-          const int row = coff[e] + jo;
-          if (!phi) Y[row + (ctt[e] ? L + m : m)] = v;            // A: same coefficient slot
-          else if (m == 0) X[row] = 0.0;                           // d/dphi of the m = 0 mode
-          else if (ctt[e] == 0) X[row + L + m] = -v;               // sin slot <- -m (Pr C_cos)
-          else X[row + m] = v;                                     // cos slot <- +m (Pr C_sin)
-        }
+      for (int e = 0; e < 2; ++e) if (cok[e]) ydst[e][rr * pitch] = acc[mt][e];
+    } else if (rr < 2 * nt) {
+#pragma unroll
+      for (int e = 0; e < 2; ++e) if (cok[e]) xdst[e][(rr - nt) * pitch] = sgn[e] * acc[mt][e];
     }
   }
 }
@@ -289,11 +348,18 @@ __device__ __forceinline__ void ang_s2_unit(const double* __restrict__ tp /* T_m
     case 4: CALL(4); break;                            \
     default: CALL(5); break;                           \
   }
+#define GH_NTC3_SWITCH(nn, CALL)                      \
+  switch (nn) {                                        \
+    case 1: CALL(1); break;                            \
+    case 2: CALL(2); break;                            \
+    default: CALL(3); break;                           \
+  }
 
-constexpr int ANG_NTC = 5;   // most n-tiles per warp unit in S1 / S3
+constexpr int ANG_NTC = 5;    // most n-tiles per warp unit in S1
+constexpr int ANG_NTC3 = 3;   // most n-tiles per warp unit in S3 (four accumulator sets)
 
 template <int TPB>
-__global__ void __launch_bounds__(TPB)
+__global__ void __launch_bounds__(TPB, TPB <= 256 ? 2 : 1)
 k_ang(const AngItem* __restrict__ items, const double* __restrict__ tables, const double* __restrict__ in,
       double* __restrict__ out, int64_t S, int ncomp) {
   extern __shared__ __align__(16) double sm[];
@@ -301,10 +367,11 @@ k_ang(const AngItem* __restrict__ items, const double* __restrict__ tables, cons
   const AngItem it = items[blockIdx.x];
   const int comp = blockIdx.y, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int g = lane >> 2, tl = lane & 3;
-  const int L = it.L, nt = L + 1, np = 2 * L + 2, nq = 2 * L + 1, plane = nt * np;
+  const int L = it.L, nt = L + 1, np = 2 * L + 2, plane = nt * np;
+  const AngDims D = ang_dims(L);
+  const int h = D.h, kc = D.kc, ke = D.ke;
   const int nb = it.nplanes, R = nb * nt;
   const int pitch = ang_pitch(L), ps = ang_plane_stride(L);
-  const int KSp = (np + 3) >> 2, KSq = (nq + 3) >> 2, NTq = (nq + 7) >> 3, NTp = (np + 7) >> 3;
   const int64_t goff = it.off + (int64_t)it.plane0 * plane;
   const double* __restrict__ src = in + (int64_t)comp * S + goff;
   double* __restrict__ dth = out + ((int64_t)1 * ncomp + comp) * S + goff;
@@ -313,19 +380,20 @@ k_ang(const AngItem* __restrict__ items, const double* __restrict__ tables, cons
   double* X = sm;                               // [nb][ps]
   double* Y = X + (size_t)it.nb_alloc * ps;     // [nb][ps]
   double* Z = Y + (size_t)it.nb_alloc * ps;     // zero row [pitch + 16]
-  double* F = Z + pitch + 16;                   // Fa fragments, later Fs fragments
+  double* F = Z + pitch + 16;                   // Fa fragments (even | odd), later Fs fragments (even | odd)
   int* rowoff = reinterpret_cast<int*>(F + ang_f_doubles(L));   // [R rounded up to 8]: offset of row r in X / Y; pad rows -> Z
-  const int zoff = (int)(Z - X);                // offset of the zero row relative to X (also used relative to Y: see below)
+  const int zoff = (int)(Z - X);
 
-  // ---- stage 0: U -> X and Fa fragments -> F by cp.async; zero the K-padding; row-offset table ----
+  // ---- stage 0: raw U -> Y and Fa fragments -> F by cp.async (all loads in flight at once); tables; padding ----
   {
-    for (int e = tid; e < R * np; e += TPB) {
-      const int r = e / np, k = e - r * np;
+    for (int r = warp; r < R; r += NW) {
       const int b = r / nt, j = r - b * nt;
-      cp_async8(X + (size_t)b * ps + j * pitch + k, src + e);
+      const double* __restrict__ urow = src + (size_t)r * np;
+      double* yrow = Y + (size_t)b * ps + j * pitch;
+      for (int c = lane; c < np; c += 32) cp_async8(yrow + c, urow + c);
     }
     const double* __restrict__ Fa = tables + it.m_Fa;
-    const int nfa = KSp * NTq * 32;
+    const int nfa = (int)ang_fa_doubles(L);
     for (int e = tid * 2; e < nfa; e += TPB * 2) cp_async16(F + e, Fa + e);
     cp_async_commit();
     const int R8 = (R + 7) & ~7;
@@ -334,13 +402,7 @@ k_ang(const AngItem* __restrict__ items, const double* __restrict__ tables, cons
       rowoff[r] = (r < R) ? b * ps + j * pitch : zoff;
     }
     for (int e = tid; e < pitch + 16; e += TPB) Z[e] = 0.0;
-    // U columns [np, pitch) of every row (K padding of S1, finite values for S3), rows [nt, 4*ceil(nt/4)) of Y (K padding of S2)
-    const int padc = pitch - np;
-    for (int e = tid; e < R * padc; e += TPB) {
-      const int r = e / padc, k = np + (e - r * padc);
-      const int b = r / nt, j = r - b * nt;
-      X[(size_t)b * ps + j * pitch + k] = 0.0;
-    }
+    // rows [nt, 4*ceil(nt/4)) of Y (K padding of S2)
     const int ntp = (nt + 3) & ~3, padr = (ntp - nt) * pitch;
     for (int e = tid; e < nb * padr; e += TPB) {
       const int b = e / padr;
@@ -349,23 +411,57 @@ k_ang(const AngItem* __restrict__ items, const double* __restrict__ tables, cons
     cp_async_wait<0>();
   }
   __syncthreads();
+  // ---- S0: fold Y (raw) -> X: columns 0..h E, [h+1, ke) zero, ke..ke+L-1 O_1..O_L, rest zero (K padding of S1; finite for S3) ----
+  {
+    const int yx = (int)(Y - X);
+    for (int r = warp; r < R; r += NW) {
+      double* xrow = X + rowoff[r];
+      const double* yrow = xrow + yx;
+      for (int c = lane; c < pitch; c += 32) {
+        double v = 0.0;
+        if (c <= h) {
+          v = yrow[c];
+          if (c >= 1 && c < h) v += yrow[np - c];
+        } else if (c >= ke && c < ke + L) {
+          const int k = c - ke + 1;
+          v = yrow[k] - yrow[np - k];
+        }
+        xrow[c] = v;
+      }
+    }
+  }
+  __syncthreads();
 
   const int MT1 = (R + 7) >> 3;
-  // ---- S1: C = U Fa^T ----
+  // ---- S1: Cc = E Fa_c^T (columns 0..), Cs = O Fa_s^T (columns kc..) ----
   {
-    const int nch = it.nch1, per = (NTq + nch - 1) / nch;
-    for (int u = warp; u < MT1 * nch; u += NW) {
-      const int mt = u / nch, ch = u - mt * nch;
-      const int n0 = ch * per, nn = min(per, NTq - n0);
+    const int nche = it.nch1e, pere = (D.NTc + nche - 1) / nche;
+    const int ncho = it.nch1o, pero = (D.NTs + ncho - 1) / ncho;
+    const int upm = nche + ncho;                       // units per m-tile
+    const double* __restrict__ Fo = F + D.KSe1 * D.NTc * 32;
+    for (int u = warp; u < MT1 * upm; u += NW) {
+      const int mt = u / upm, ch = u - mt * upm;
       const int r = mt * 8 + g;
       const int ro = rowoff[r];
-      const double* ap = X + ro + tl;
-      const double* bp = F + n0 * 32 + lane;
-      double* yrow = Y + ro;
-      const int c0 = n0 * 8 + 2 * tl;
-#define GH_CALL(K) ang_s1_unit<K>(ap, bp, KSp, NTq, yrow, c0, pitch, r < R)
-      GH_NTC_SWITCH(nn, GH_CALL)
+      if (ch < nche) {
+        const int n0 = ch * pere, nn = min(pere, D.NTc - n0);
+        const double* ap = X + ro + tl;
+        const double* bp = F + n0 * 32 + lane;
+        double* yrow = Y + ro;
+        const int c0 = n0 * 8 + 2 * tl;
+#define GH_CALL(K) ang_s1_unit<K>(ap, bp, D.KSe1, D.NTc, yrow, c0, pitch, r < R)
+        GH_NTC_SWITCH(nn, GH_CALL)
 #undef GH_CALL
+      } else {
+        const int n0 = (ch - nche) * pero, nn = min(pero, D.NTs - n0);
+        const double* ap = X + ro + ke + tl;
+        const double* bp = Fo + n0 * 32 + lane;
+        double* yrow = Y + ro + kc;
+        const int c0 = n0 * 8 + 2 * tl;
+#define GH_CALL(K) ang_s1_unit<K>(ap, bp, D.KSo1, D.NTs, yrow, c0, pitch - kc, r < R)
+        GH_NTC_SWITCH(nn, GH_CALL)
+#undef GH_CALL
+      }
     }
   }
   __syncthreads();
@@ -373,7 +469,7 @@ k_ang(const AngItem* __restrict__ items, const double* __restrict__ tables, cons
   // ---- Fs fragments -> F (free once S1 is done; S2 does not touch it) ----
   {
     const double* __restrict__ Fs = tables + it.m_Fs;
-    const int nfs = KSq * NTp * 32;
+    const int nfs = (int)ang_fs_doubles(L);
     for (int e = tid * 2; e < nfs; e += TPB * 2) cp_async16(F + e, Fs + e);
     cp_async_commit();
   }
@@ -386,43 +482,48 @@ k_ang(const AngItem* __restrict__ items, const double* __restrict__ tables, cons
       const int m = u / NTn, ntile = u - m * NTn;
       if (m == 0 && ntile * 8 >= nb) continue;
       const double* tp = T + (size_t)m * KS2 * MT2 * 32;
+#define GH_S2(K) ang_s2_unit<K>(tp, KS2, X, Y, m, ntile, nb, L, kc, pitch, ps, g, tl)
       switch (MT2) {
-        case 1: ang_s2_unit<1>(tp, KS2, X, Y, m, ntile, nb, L, pitch, ps, g, tl); break;
-        case 2: ang_s2_unit<2>(tp, KS2, X, Y, m, ntile, nb, L, pitch, ps, g, tl); break;
-        case 3: ang_s2_unit<3>(tp, KS2, X, Y, m, ntile, nb, L, pitch, ps, g, tl); break;
-        case 4: ang_s2_unit<4>(tp, KS2, X, Y, m, ntile, nb, L, pitch, ps, g, tl); break;
-        case 5: ang_s2_unit<5>(tp, KS2, X, Y, m, ntile, nb, L, pitch, ps, g, tl); break;
-        case 6: ang_s2_unit<6>(tp, KS2, X, Y, m, ntile, nb, L, pitch, ps, g, tl); break;
-        case 7: ang_s2_unit<7>(tp, KS2, X, Y, m, ntile, nb, L, pitch, ps, g, tl); break;
-        case 8: ang_s2_unit<8>(tp, KS2, X, Y, m, ntile, nb, L, pitch, ps, g, tl); break;
-        case 9: ang_s2_unit<9>(tp, KS2, X, Y, m, ntile, nb, L, pitch, ps, g, tl); break;
-        case 10: ang_s2_unit<10>(tp, KS2, X, Y, m, ntile, nb, L, pitch, ps, g, tl); break;
-        case 11: ang_s2_unit<11>(tp, KS2, X, Y, m, ntile, nb, L, pitch, ps, g, tl); break;
-        default: ang_s2_unit<12>(tp, KS2, X, Y, m, ntile, nb, L, pitch, ps, g, tl); break;
+        case 1: GH_S2(1); break;
+        case 2: GH_S2(2); break;
+        case 3: GH_S2(3); break;
+        case 4: GH_S2(4); break;
+        case 5: GH_S2(5); break;
+        case 6: GH_S2(6); break;
+        case 7: GH_S2(7); break;
+        case 8: GH_S2(8); break;
+        case 9: GH_S2(9); break;
+        case 10: GH_S2(10); break;
+        case 11: GH_S2(11); break;
+        default: GH_S2(12); break;
       }
+#undef GH_S2
     }
   }
   cp_async_wait<0>();
   __syncthreads();
 
-  // ---- S3: [d_theta u ; d_phi u] = [A ; B'] Fs^T, stored straight from the accumulator fragments ----
+  // ---- S3: even / odd syntheses of A (Y) and B' (X), unfolded in the epilogue ----
   {
-    const int nch = it.nch3, per = (NTp + nch - 1) / nch;
+    const int nch = it.nch3, per = (D.NT3 + nch - 1) / nch;
     const int yx = (int)(Y - X);
+    const double* __restrict__ Fo = F + D.KSe3 * D.NT3 * 32;
     for (int u = warp; u < MT1 * nch; u += NW) {
       const int mt = u / nch, ch = u - mt * nch;
-      const int n0 = ch * per, nn = min(per, NTp - n0);
+      const int n0 = ch * per, nn = min(per, D.NT3 - n0);
       const int r = mt * 8 + g;
       const bool rok = r < R;
       const int ro = rowoff[r];
       const double* a1p = X + ro + tl;                             // B'
       const double* a0p = rok ? a1p + yx : a1p;                     // A (pad rows: the zero row for both)
-      const double* bp = F + n0 * 32 + lane;
+      const int kcr = rok ? kc : 0;                                 // the zero row is only pitch + 16 long
+      const double* bpe = F + n0 * 32 + lane;
+      const double* bpo = Fo + n0 * 32 + lane;
       const int c0 = n0 * 8 + 2 * tl;
       double* g0 = dth + (size_t)r * np;
       double* g1 = dph + (size_t)r * np;
-#define GH_CALL(K) ang_s3_unit<K>(a0p, a1p, bp, KSq, NTp, g0, g1, c0, np, rok)
-      GH_NTC_SWITCH(nn, GH_CALL)
+#define GH_CALL(K) ang_s3_unit<K>(a0p, a1p, kcr, bpe, bpo, D.KSe3, D.KSo3, D.NT3, g0, g1, c0, h, np, rok)
+      GH_NTC3_SWITCH(nn, GH_CALL)
 #undef GH_CALL
     }
   }
