@@ -75,19 +75,31 @@ __device__ __forceinline__ bool geometry(const double (&psi)[10], Geom& G) {
   return ok;
 }
 
+// Phi_iab accessors: registers (K_con) or this thread's column of a shared-memory array [30][TILE_PTS] (K_rhs, where
+// Phi in registers is what forces spills: the compiler fetches each value where it is used instead).
+struct PhiReg {
+  const double (&v)[3][10];
+  __device__ __forceinline__ double operator()(int i, int s) const { return v[i][s]; }
+};
+struct PhiSm {
+  const double* p;   // + tid
+  __device__ __forceinline__ double operator()(int i, int s) const { return p[(i * 10 + s) * TILE_PTS]; }
+};
+
 // Christoffel symbols of the first kind from the first-order variables, as 4 symmetric matrices
 // Gam[a][SI(b,c)] = 1/2 (D_b psi_ac + D_c psi_ab - D_a psi_bc),  D_0 = -N Pi + N^i Phi_i,  D_i = Phi_i.
-__device__ __forceinline__ void christoffel(const Geom& G, const double (&Pi)[10], const double (&Phi)[3][10],
+template <class PI, class PH>
+__device__ __forceinline__ void christoffel(const Geom& G, const PI& Pi, const PH& Phi,
                                             double (&Gam)[4][10]) {
   double D0[10];
 #pragma unroll
   for (int s = 0; s < 10; ++s) {
     double v = -G.N * Pi[s];
 #pragma unroll
-    for (int i = 0; i < 3; ++i) v = fma(G.sh[i], Phi[i][s], v);
+    for (int i = 0; i < 3; ++i) v = fma(G.sh[i], Phi(i, s), v);
     D0[s] = v;
   }
-#define GH_D(c, s) ((c) == 0 ? D0[s] : Phi[(c) - 1][s])
+#define GH_D(c, s) ((c) == 0 ? D0[s] : Phi((c) - 1, s))
 #pragma unroll
   for (int a = 0; a < 4; ++a)
 #pragma unroll
@@ -95,6 +107,23 @@ __device__ __forceinline__ void christoffel(const Geom& G, const double (&Pi)[10
 #pragma unroll
       for (int c = b; c < 4; ++c)
         Gam[a][SI(b, c)] = 0.5 * (GH_D(b, SI(a, c)) + GH_D(c, SI(a, b)) - GH_D(a, SI(b, c)));
+#undef GH_D
+}
+
+// One Christoffel matrix Gam_a[SI(b,c)] on the fly from D_0 (registers) and Phi.  K_rhs never holds all four: the 40
+// values are what pushes the kernel over 255 registers; recomputing a matrix costs 30 flop.  The empty asm makes each
+// recomputed value opaque, so that the compiler cannot merge the copies back into one long-lived array.
+template <int a, class PH>
+__device__ __forceinline__ void gam_row(const double (&D0)[10], const PH& Phi, double (&Ga)[10]) {
+#define GH_D(c, s) ((c) == 0 ? D0[s] : Phi((c) - 1, s))
+#pragma unroll
+  for (int b = 0; b < 4; ++b)
+#pragma unroll
+    for (int c = b; c < 4; ++c) {
+      double v = 0.5 * (GH_D(b, SI(a, c)) + GH_D(c, SI(a, b)) - GH_D(a, SI(b, c)));
+      asm("" : "+d"(v));
+      Ga[SI(b, c)] = v;
+    }
 #undef GH_D
 }
 
@@ -119,10 +148,52 @@ struct Alg {
   double w[3][3];  // w[i][j] = t^c Phi_i(j+1)c
 };
 
-__device__ __forceinline__ void algebraic(const Geom& G, const double (&Pi)[10], const double (&Phi)[3][10],
+template <int a, class PH>
+__device__ __forceinline__ void alg_gamma(const Geom& G, const double (&D0)[10], const PH& Phi, const double (&H)[4],
+                                          const double (&Hup)[4], Alg& A) {
+  double Ga[10];
+  gam_row<a>(D0, Phi, Ga);
+  A.C[a] = H[a] + symdot(G.pinv, Ga);
+#pragma unroll
+  for (int s = 0; s < 10; ++s) A.S[s] = fma(Hup[a], Ga[s], A.S[s]);      // H^d Gam_dab
+  double Y[4][4];  // Y[d][e] = psi^{dc} Gam_a[c][e]
+#pragma unroll
+  for (int d = 0; d < 4; ++d)
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      double v = 0.0;
+#pragma unroll
+      for (int c = 0; c < 4; ++c) v = fma(G.pinv[SI(d, c)], Ga[SI(c, e)], v);
+      Y[d][e] = v;
+    }
+  double R[10];    // R_a = psi^-1 Gam_a psi^-1
+#pragma unroll
+  for (int d = 0; d < 4; ++d)
+#pragma unroll
+    for (int f = d; f < 4; ++f) {
+      double v = 0.0;
+#pragma unroll
+      for (int e = 0; e < 4; ++e) v = fma(Y[d][e], G.pinv[SI(e, f)], v);
+      R[SI(d, f)] = v;
+    }
+  // T_ab = psi^{cd} psi^{ef} Gam_ace Gam_bdf = R_a : Gam_b
+  A.S[SI(a, a)] -= symdot(R, Ga);
+  if (a < 1) { double Gb[10]; gam_row<1>(D0, Phi, Gb); A.S[SI(a, 1)] -= symdot(R, Gb); }
+  if (a < 2) { double Gb[10]; gam_row<2>(D0, Phi, Gb); A.S[SI(a, 2)] -= symdot(R, Gb); }
+  if (a < 3) { double Gb[10]; gam_row<3>(D0, Phi, Gb); A.S[SI(a, 3)] -= symdot(R, Gb); }
+}
+
+template <class PI, class PH>
+__device__ __forceinline__ void algebraic(const Geom& G, const PI& Pi, const PH& Phi,
                                           const double (&H)[4], Alg& A) {
-  double Gam[4][10];
-  christoffel(G, Pi, Phi, Gam);
+  double D0[10];   // D_0 psi_ab = -N Pi_ab + N^i Phi_iab
+#pragma unroll
+  for (int s = 0; s < 10; ++s) {
+    double v = -G.N * Pi[s];
+#pragma unroll
+    for (int i = 0; i < 3; ++i) v = fma(G.sh[i], Phi(i, s), v);
+    D0[s] = v;
+  }
   double Hup[4];
 #pragma unroll
   for (int d = 0; d < 4; ++d) {
@@ -132,44 +203,15 @@ __device__ __forceinline__ void algebraic(const Geom& G, const double (&Pi)[10],
     Hup[d] = v;
   }
 #pragma unroll
-  for (int a = 0; a < 4; ++a) A.C[a] = H[a] + symdot(G.pinv, Gam[a]);
+  for (int s = 0; s < 10; ++s) A.S[s] = 0.0;
+  // per a: Gam_a -> C_a, H^a Gam_a, R_a = psi^-1 Gam_a psi^-1; then - T_ab = - R_a : Gam_b for b >= a
+  alg_gamma<0>(G, D0, Phi, H, Hup, A);
+  alg_gamma<1>(G, D0, Phi, H, Hup, A);
+  alg_gamma<2>(G, D0, Phi, H, Hup, A);
+  alg_gamma<3>(G, D0, Phi, H, Hup, A);
   A.tC = 0.0;
 #pragma unroll
   for (int a = 0; a < 4; ++a) A.tC = fma(G.tu[a], A.C[a], A.tC);
-  // H^d Gam_dab
-#pragma unroll
-  for (int s = 0; s < 10; ++s) {
-    double v = 0.0;
-#pragma unroll
-    for (int d = 0; d < 4; ++d) v = fma(Hup[d], Gam[d][s], v);
-    A.S[s] = v;
-  }
-  // - T_ab,  T_ab = psi^{cd} psi^{ef} Gam_ace Gam_bdf = R_a^{df} Gam_bdf,  R_a = psi^-1 Gam_a psi^-1
-#pragma unroll
-  for (int a = 0; a < 4; ++a) {
-    double Y[4][4];  // Y[d][e] = psi^{dc} Gam_a[c][e]
-#pragma unroll
-    for (int d = 0; d < 4; ++d)
-#pragma unroll
-      for (int e = 0; e < 4; ++e) {
-        double v = 0.0;
-#pragma unroll
-        for (int c = 0; c < 4; ++c) v = fma(G.pinv[SI(d, c)], Gam[a][SI(c, e)], v);
-        Y[d][e] = v;
-      }
-    double R[10];
-#pragma unroll
-    for (int d = 0; d < 4; ++d)
-#pragma unroll
-      for (int f = d; f < 4; ++f) {
-        double v = 0.0;
-#pragma unroll
-        for (int e = 0; e < 4; ++e) v = fma(Y[d][e], G.pinv[SI(e, f)], v);
-        R[SI(d, f)] = v;
-      }
-#pragma unroll
-    for (int b = a; b < 4; ++b) A.S[SI(a, b)] -= symdot(R, Gam[b]);
-  }
   // - Pi_ac psi^{cd} Pi_db
   {
     double Q[4][4];  // Q[c][b] = psi^{cd} Pi_db
@@ -202,7 +244,7 @@ __device__ __forceinline__ void algebraic(const Geom& G, const double (&Pi)[10],
       for (int b = 0; b < 4; ++b) {
         double v = 0.0;
 #pragma unroll
-        for (int d = 0; d < 4; ++d) v = fma(G.pinv[SI(c, d)], Phi[i][SI(d, b)], v);
+        for (int d = 0; d < 4; ++d) v = fma(G.pinv[SI(c, d)], Phi(i, SI(d, b)), v);
         Z[c][b] = v;
       }
 #pragma unroll
@@ -212,7 +254,7 @@ __device__ __forceinline__ void algebraic(const Geom& G, const double (&Pi)[10],
       for (int c = 0; c < 4; ++c) {
         double v = 0.0;
 #pragma unroll
-        for (int j = 0; j < 3; ++j) v = fma(G.gi[S3(i, j)], Phi[j][SI(a, c)], v);
+        for (int j = 0; j < 3; ++j) v = fma(G.gi[S3(i, j)], Phi(j, SI(a, c)), v);
         up[c] = v;
       }
 #pragma unroll
@@ -239,13 +281,13 @@ __device__ __forceinline__ void algebraic(const Geom& G, const double (&Pi)[10],
 #pragma unroll
     for (int c = 0; c < 4; ++c)
 #pragma unroll
-      for (int d = 0; d < 4; ++d) u = fma(G.tu[c] * G.tu[d], Phi[i][SI(c, d)], u);
+      for (int d = 0; d < 4; ++d) u = fma(G.tu[c] * G.tu[d], Phi(i, SI(c, d)), u);
     A.s[i] = u;
 #pragma unroll
     for (int j = 0; j < 3; ++j) {
       double x = 0.0;
 #pragma unroll
-      for (int c = 0; c < 4; ++c) x = fma(G.tu[c], Phi[i][SI(j + 1, c)], x);
+      for (int c = 0; c < 4; ++c) x = fma(G.tu[c], Phi(i, SI(j + 1, c)), x);
       A.w[i][j] = x;
     }
   }
@@ -281,8 +323,8 @@ __device__ __forceinline__ void rhs_store(double* out, const RkArgs& rk, int64_t
 // the loads of pairs s .. s+RHS_RING-1 are in flight while the algebra of stage 2 and the assembly of earlier pairs
 // run, which is what an HBM-bound kernel with 255 registers per thread (8 warps per SM) cannot get from the warp
 // scheduler alone.
-constexpr int RHS_RING = 4, RHS_RING_ROWS = 22;   // 15 derivatives + 2 gauge-source gradients + 5 u0 values (RK = 2)
-constexpr size_t RHS_SMEM_BYTES = (size_t)RHS_RING * RHS_RING_ROWS * TILE_PTS * sizeof(double);
+constexpr int RHS_RING = 3, RHS_RING_ROWS = 22, RHS_PHI_ROWS = 30;   // 15 derivatives + 2 gauge-source gradients + 5 u0 values (RK = 2)
+constexpr size_t RHS_SMEM_BYTES = (size_t)(RHS_PHI_ROWS + RHS_RING * RHS_RING_ROWS) * TILE_PTS * sizeof(double);
 
 template <int PAIR, int RK>
 __device__ __forceinline__ void rhs_prefetch(double* __restrict__ slot /* + tid */, const double* __restrict__ du,
@@ -309,7 +351,8 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
                                           const double* u, const double* __restrict__ du,
                                           const double* __restrict__ Hs, const double* __restrict__ dHs,
                                           double* k, const RkArgs& rk, int64_t S, int* __restrict__ flag,
-                                          double* __restrict__ ring /* + tid */) {
+                                          double* __restrict__ phis /* + tid */) {
+  double* __restrict__ ring = phis + RHS_PHI_ROWS * TILE_PTS;
   const int64_t p = sd.off + local;
   // face mask (A6)
   bool frozen;
@@ -321,27 +364,28 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
                (i2 == 0 && sd.face[4] == 1) || (i2 == sd.n2 - 1 && sd.face[5] == 1);
   }
   constexpr int SLOT = RHS_RING_ROWS * TILE_PTS;
+  // Phi_iab of this point -> shared memory (first cp.async group), then the first RHS_RING pairs of stage 3
+#pragma unroll
+  for (int c = 0; c < RHS_PHI_ROWS; ++c) cp_async8(phis + c * TILE_PTS, u + (int64_t)(50 - RHS_PHI_ROWS + c) * S + p);
+  cp_async_commit();
   if (!frozen) {
     rhs_prefetch<0, RK>(ring + 0 * SLOT, du, dHs, rk.u0, S, p);
     rhs_prefetch<1, RK>(ring + 1 * SLOT, du, dHs, rk.u0, S, p);
     rhs_prefetch<2, RK>(ring + 2 * SLOT, du, dHs, rk.u0, S, p);
-    rhs_prefetch<3, RK>(ring + 3 * SLOT, du, dHs, rk.u0, S, p);
   }
-  double psi[10], Pi[10], Phi[3][10], H[4];
-#pragma unroll
-  for (int s = 0; s < 10; ++s) psi[s] = u[(int64_t)s * S + p];
+  const PhiSm Phi{phis};
+  double psi[10], H[4], Pi[10];
 #pragma unroll
   for (int s = 0; s < 10; ++s) Pi[s] = u[(int64_t)(10 + s) * S + p];
 #pragma unroll
-  for (int i = 0; i < 3; ++i)
-#pragma unroll
-    for (int s = 0; s < 10; ++s) Phi[i][s] = u[(int64_t)(20 + 10 * i + s) * S + p];
+  for (int s = 0; s < 10; ++s) psi[s] = u[(int64_t)s * S + p];
 #pragma unroll
   for (int a = 0; a < 4; ++a) H[a] = Hs[(int64_t)a * S + p];
 
   Geom G;
   const bool ok = geometry(psi, G);
   if (!ok) atomicOr(flag, 1);
+  if (frozen) cp_async_wait<0>(); else cp_async_wait<RHS_RING>();   // the Phi group has landed
   if (!ok || frozen) {
     cp_async_wait<0>();   // nothing of this thread may still be landing in shared memory when the CTA retires
 #pragma unroll
@@ -351,7 +395,7 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
       rhs_store<RK>(k, rk, (int64_t)(10 + s) * S + p, 0.0, Pi[s], RK == 2 ? rk.u0[(int64_t)(10 + s) * S + p] : 0.0);
 #pragma unroll
       for (int i = 0; i < 3; ++i)
-        rhs_store<RK>(k, rk, (int64_t)(20 + 10 * i + s) * S + p, 0.0, Phi[i][s], RK == 2 ? rk.u0[(int64_t)(20 + 10 * i + s) * S + p] : 0.0);
+        rhs_store<RK>(k, rk, (int64_t)(20 + 10 * i + s) * S + p, 0.0, Phi(i, s), RK == 2 ? rk.u0[(int64_t)(20 + 10 * i + s) * S + p] : 0.0);
     }
     return;
   }
@@ -369,7 +413,6 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
       const int s = SI(a, b);
       // groups committed so far: min(10, s + RHS_RING); group s must have landed
       if (s + RHS_RING <= 10) cp_async_wait<RHS_RING - 1>();
-      else if (s == 7) cp_async_wait<2>();
       else if (s == 8) cp_async_wait<1>();
       else cp_async_wait<0>();
       const double* __restrict__ slot = ring + (s % RHS_RING) * SLOT;
@@ -391,7 +434,7 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
       for (int kk = 0; kk < 3; ++kk) {
         sdpsi = fma(G.sh[kk], d[0][kk], sdpsi);
         sdPi = fma(G.sh[kk], d[1][kk], sdPi);
-        sPhi = fma(G.sh[kk], Phi[kk][s], sPhi);
+        sPhi = fma(G.sh[kk], Phi(kk, s), sPhi);
       }
       rhs_store<RK>(k, rk, (int64_t)s * S + p, (1.0 + g1) * sdpsi - N * Pi[s] - g1 * sPhi, psi[s], RK == 2 ? slot[17 * TILE_PTS] : 0.0);
 
@@ -405,7 +448,7 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
       for (int j = 0; j < 3; ++j) {
         double v = 0.0;
 #pragma unroll
-        for (int kk = 0; kk < 3; ++kk) v = fma(G.gi[S3(j, kk)], Phi[kk][s], v);
+        for (int kk = 0; kk < 3; ++kk) v = fma(G.gi[S3(j, kk)], Phi(kk, s), v);
         up[j] = v;
       }
       // 1/2 (d_a H_b + d_b H_a), d_0 H = 0 ; dHs[(i*4+b)] = d_i H_b
@@ -429,15 +472,16 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
 #pragma unroll
         for (int j = 0; j < 3; ++j) wup = fma(A.w[i][j], up[j], wup);
         rhs_store<RK>(k, rk, (int64_t)(20 + 10 * i + s) * S + p,
-                      sdPhi - N * d[1][i] + N * g2 * (d[0][i] - Phi[i][s]) + 0.5 * N * A.s[i] * Pi[s] + N * wup, Phi[i][s], RK == 2 ? slot[(19 + i) * TILE_PTS] : 0.0);
+                      sdPhi - N * d[1][i] + N * g2 * (d[0][i] - Phi(i, s)) + 0.5 * N * A.s[i] * Pi[s] + N * wup, Phi(i, s), RK == 2 ? slot[(19 + i) * TILE_PTS] : 0.0);
       }
       // every value of the slot has been consumed: refill it with pair s + RHS_RING
-      if (s == 0) rhs_prefetch<4, RK>(ring + 0 * SLOT, du, dHs, rk.u0, S, p);
-      if (s == 1) rhs_prefetch<5, RK>(ring + 1 * SLOT, du, dHs, rk.u0, S, p);
-      if (s == 2) rhs_prefetch<6, RK>(ring + 2 * SLOT, du, dHs, rk.u0, S, p);
-      if (s == 3) rhs_prefetch<7, RK>(ring + 3 * SLOT, du, dHs, rk.u0, S, p);
-      if (s == 4) rhs_prefetch<8, RK>(ring + 0 * SLOT, du, dHs, rk.u0, S, p);
-      if (s == 5) rhs_prefetch<9, RK>(ring + 1 * SLOT, du, dHs, rk.u0, S, p);
+      if (s == 0) rhs_prefetch<3, RK>(ring + 0 * SLOT, du, dHs, rk.u0, S, p);
+      if (s == 1) rhs_prefetch<4, RK>(ring + 1 * SLOT, du, dHs, rk.u0, S, p);
+      if (s == 2) rhs_prefetch<5, RK>(ring + 2 * SLOT, du, dHs, rk.u0, S, p);
+      if (s == 3) rhs_prefetch<6, RK>(ring + 0 * SLOT, du, dHs, rk.u0, S, p);
+      if (s == 4) rhs_prefetch<7, RK>(ring + 1 * SLOT, du, dHs, rk.u0, S, p);
+      if (s == 5) rhs_prefetch<8, RK>(ring + 2 * SLOT, du, dHs, rk.u0, S, p);
+      if (s == 6) rhs_prefetch<9, RK>(ring + 0 * SLOT, du, dHs, rk.u0, S, p);
 
     }
 }
@@ -448,7 +492,7 @@ k_rhs(const SubDev* __restrict__ subs, const int32_t* __restrict__ tile_first, i
       const double* __restrict__ tables, const double* u, const double* __restrict__ du,
       const double* __restrict__ Hs, const double* __restrict__ dHs, double* k, RkArgs rk, int64_t S,
       int* __restrict__ flag) {
-  extern __shared__ __align__(16) double ring_s[];   // [RHS_RING][RHS_RING_ROWS][TILE_PTS]
+  extern __shared__ __align__(16) double ring_s[];   // Phi [30][TILE_PTS], then the ring [RHS_RING][RHS_RING_ROWS][TILE_PTS]
   __shared__ SubDev sd_s;
   __shared__ int tile0_s;
   if (threadIdx.x == 0) {
@@ -490,7 +534,7 @@ __device__ __forceinline__ void con_point(const SubDev& sd, const double* __rest
   if (!geometry(psi, G)) { atomicOr(flag, 1); return; }
   {
     double Gam[4][10];
-    christoffel(G, Pi, Phi, Gam);
+    christoffel(G, Pi, PhiReg{Phi}, Gam);
 #pragma unroll
     for (int a = 0; a < 4; ++a) {
       const double c = H[a] + symdot(G.pinv, Gam[a]);
