@@ -22,8 +22,14 @@ using namespace ghd;
 namespace {
 
 constexpr int CHEB_TPB = 128;                     // K_cheb: 4 warps
-constexpr int CHEB_COMP_WALK = 5;                 // components one K_cheb CTA walks over
-constexpr int CHEB_NTW0 = 4, CHEB_NTW1 = 2;       // n-tiles per warp: class 0 (N <= 32), class 1 (N <= 64)
+#ifndef GH_CHEB_WALK
+#define GH_CHEB_WALK 25
+#endif
+#ifndef GH_CHEB_NTW0
+#define GH_CHEB_NTW0 2
+#endif
+constexpr int CHEB_COMP_WALK = GH_CHEB_WALK;      // components one K_cheb CTA walks over
+constexpr int CHEB_NTW0 = GH_CHEB_NTW0, CHEB_NTW1 = 2;       // n-tiles per warp: class 0 (N <= 32), class 1 (N <= 64)
 constexpr int CHEB_CT0 = (CHEB_TPB / 32) * 8 * CHEB_NTW0, CHEB_CT1 = (CHEB_TPB / 32) * 8 * CHEB_NTW1;   // columns per CTA
 inline int cheb_class(int N) { return N <= 32 ? 0 : 1; }
 inline int cheb_ct(int N) { return cheb_class(N) ? CHEB_CT1 : CHEB_CT0; }
