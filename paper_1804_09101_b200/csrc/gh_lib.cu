@@ -376,7 +376,8 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
           std::vector<ghb::ld> FA(shell_fa_doubles(L), 0);
           for (int ks = 0; ks < dm.KSe1; ++ks) for (int n = 0; n < dm.NTc; ++n) for (int lane = 0; lane < 32; ++lane) {
             const int k = ks * 4 + lane % 4, m = n * 8 + lane / 4;
-            if (k <= h && m <= L) FA[((size_t)ks * dm.NTc + n) * 32 + lane] = B.Fa[(size_t)m * np + k];
+            // the kernel forms U_k + U_{np-k} for every k: k = h is its own mirror, so its weight is halved
+            if (k <= h && m <= L) FA[((size_t)ks * dm.NTc + n) * 32 + lane] = (k == h ? (ghb::ld)0.5 : (ghb::ld)1) * B.Fa[(size_t)m * np + k];
           }
           const size_t fao = (size_t)dm.KSe1 * dm.NTc * 32;
           for (int ks = 0; ks < dm.KSo1; ++ks) for (int n = 0; n < dm.NTs; ++n) for (int lane = 0; lane < 32; ++lane) {

@@ -120,8 +120,10 @@ k_cheb(const ChebItem* __restrict__ items, const double* __restrict__ tables, co
 // ---------------------------------------------------------------------------------------------------------
 // K_ang.  grid = (n_items, ncomp).  One CTA: `nb` (theta,phi) planes of one component of one shell, kept in shared
 // memory through three GEMM stages on the FP64 tensor cores (mma.sync.m8n8k4).  With h = L+1 = n_phi/2:
-//   S0  fold    E_k = U_k + U_{n_phi-k}, O_k = U_k - U_{n_phi-k} (k = 1..L), E_0 = U_0, E_h = U_h: cos(m phi) is even and
-//               sin(m phi) odd about phi = pi, so the real DFT splits into two half-length ones (half the flop of S1, S3)
+//   fold        E_k = U_k + U_{n_phi-k}, O_k = U_k - U_{n_phi-k} (k = 1..L), E_0 = U_0, E_h = U_h: cos(m phi) is even and
+//               sin(m phi) odd about phi = pi, so the real DFT splits into two half-length ones (half the flop of S1,
+//               S3).  The fold happens in the A-operand load of S1 (two LDS and one add per fragment; the raw row
+//               carries a zero at column n_phi and the k = h row of Fa_c is halved, so no lane needs a predicate)
 //   S1  Cc[r][m] = sum_{k=0..h} E[r][k] Fa_c[m][k]  (m = 0..L),   Cs[r][m] = sum_{k=1..L} O[r][k] Fa_s[m][k]  (m = 1..L)
 //   S2  [A ; B'](m) = [Th_m ; m Pr_m] C_m   per m, columns (t = cos/sin, plane b); A in place over C, B' into the
 //               cos<->sin partner slot with sign (d/dphi in coefficient space)
@@ -130,10 +132,10 @@ k_cheb(const ChebItem* __restrict__ items, const double* __restrict__ tables, co
 // Every matrix operand is stored in DMMA fragment order, zero padded to whole tiles ([k_step][tile][32 lanes]: one
 // conflict-free LDS.64 / coalesced 256-byte LDG per fragment, tile offsets are immediates), so the inner loops carry
 // no bounds predicate.  Fa / Fs fragments live in shared memory; the per-m stacked matrices [Th_m ; m Pr_m] stream
-// from L2 two k-steps ahead.  Planes: X (folded U, later B') and Y (C, later A), row (b, j) at b*ps + j*pitch
-// doubles; coefficient rows hold cos m at column m and sin m at column kc + m - 1 (kc = 8 ceil(h/8)); folded rows
-// hold E at 0..h and O at ke.. (ke = 4 ceil((h+1)/4)).  pitch = 4 mod 8 and ps = 1 mod 16 keep the data-fragment
-// loads conflict-free.  Rows beyond the tile range read a zeroed row.
+// from L2 two k-steps ahead.  Planes: X (raw U, later B') and Y (C, later A), row (b, j) at b*ps + j*pitch
+// doubles; coefficient rows hold cos m at column m and sin m at column kc + m - 1 (kc = 8 ceil(h/8)).
+// pitch = 4 mod 8 and ps = 1 mod 16 keep the data-fragment loads conflict-free.  Rows beyond the tile range read a
+// zeroed row.
 // ---------------------------------------------------------------------------------------------------------
 struct AngDims {
   int h, KSe1, NTc, KSo1, NTs, kc, ke, KSe3, KSo3, NT3;
@@ -150,8 +152,8 @@ __host__ __device__ inline AngDims ang_dims(int L) {
 }
 __host__ __device__ inline int ang_pitch(int L) {   // row pitch (doubles), = 4 mod 8
   const AngDims d = ang_dims(L);
-  const int a = d.kc + 8 * d.NTs, b = d.ke + 4 * d.KSo1;
-  int p = a > b ? a : b;
+  const int a = d.kc + 8 * d.NTs, b = 2 * L + 2 + 1;      // coefficient rows; raw rows need n_phi + 1 (a zero at column n_phi)
+  int p = ((a > b ? a : b) + 3) / 4 * 4;
   return (p % 8 == 0) ? p + 4 : p;
 }
 __host__ __device__ inline int ang_plane_stride(int L) {   // plane stride (doubles): rows padded to 4, = 1 mod 16
@@ -180,9 +182,11 @@ __device__ __forceinline__ void cp_async16(double* smem_dst, const double* gsrc)
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
-// S1 unit: one m-tile (8 rows) x NTC n-tiles.  ap: this lane's A row (+ tl); bp: F fragments of the first n-tile (+ lane)
+// S1 unit: one m-tile (8 rows) x NTC n-tiles.  The A operand is folded on the fly from the raw row: element k is
+// U[k] + sg U[n_phi - k]; ap / am: this lane's first element and its mirror; bp: F fragments of the first n-tile (+ lane)
 template <int NTC>
-__device__ __forceinline__ void ang_s1_unit(const double* __restrict__ ap, const double* __restrict__ bp, int KS, int NT,
+__device__ __forceinline__ void ang_s1_unit(const double* __restrict__ ap, const double* __restrict__ am, double sg,
+                                            const double* __restrict__ bp, int KS, int NT,
                                             double* __restrict__ yrow, int c0, int pitch, bool rok) {
   double acc[NTC][2];
 #pragma unroll
@@ -190,10 +194,10 @@ __device__ __forceinline__ void ang_s1_unit(const double* __restrict__ ap, const
   const int bstep = NT * 32;
 #pragma unroll 2
   for (int ks = 0; ks < KS; ++ks) {
-    const double a = ap[0];
+    const double a = fma(sg, am[0], ap[0]);
 #pragma unroll
     for (int n = 0; n < NTC; ++n) dmma884(acc[n][0], acc[n][1], a, bp[n * 32]);
-    ap += 4; bp += bstep;
+    ap += 4; am -= 4; bp += bstep;
   }
   if (rok) {
 #pragma unroll
@@ -369,7 +373,7 @@ k_ang(const AngItem* __restrict__ items, const double* __restrict__ tables, cons
   const int g = lane >> 2, tl = lane & 3;
   const int L = it.L, nt = L + 1, np = 2 * L + 2, plane = nt * np;
   const AngDims D = ang_dims(L);
-  const int h = D.h, kc = D.kc, ke = D.ke;
+  const int h = D.h, kc = D.kc;
   const int nb = it.nplanes, R = nb * nt;
   const int pitch = ang_pitch(L), ps = ang_plane_stride(L);
   const int64_t goff = it.off + (int64_t)it.plane0 * plane;
@@ -384,13 +388,15 @@ k_ang(const AngItem* __restrict__ items, const double* __restrict__ tables, cons
   int* rowoff = reinterpret_cast<int*>(F + ang_f_doubles(L));   // [R rounded up to 8]: offset of row r in X / Y; pad rows -> Z
   const int zoff = (int)(Z - X);
 
-  // ---- stage 0: raw U -> Y and Fa fragments -> F by cp.async (all loads in flight at once); tables; padding ----
+  // ---- stage 0: raw U -> X and Fa fragments -> F by cp.async (all loads in flight at once); tables; padding ----
   {
+    const int padc = pitch - np;
     for (int r = warp; r < R; r += NW) {
       const int b = r / nt, j = r - b * nt;
       const double* __restrict__ urow = src + (size_t)r * np;
-      double* yrow = Y + (size_t)b * ps + j * pitch;
-      for (int c = lane; c < np; c += 32) cp_async8(yrow + c, urow + c);
+      double* xrow = X + (size_t)b * ps + j * pitch;
+      for (int c = lane; c < np; c += 32) cp_async8(xrow + c, urow + c);
+      if (lane < padc) xrow[np + lane] = 0.0;      // column n_phi = 0 (mirror of k = 0); the rest finite for S3
     }
     const double* __restrict__ Fa = tables + it.m_Fa;
     const int nfa = (int)ang_fa_doubles(L);
@@ -411,26 +417,6 @@ k_ang(const AngItem* __restrict__ items, const double* __restrict__ tables, cons
     cp_async_wait<0>();
   }
   __syncthreads();
-  // ---- S0: fold Y (raw) -> X: columns 0..h E, [h+1, ke) zero, ke..ke+L-1 O_1..O_L, rest zero (K padding of S1; finite for S3) ----
-  {
-    const int yx = (int)(Y - X);
-    for (int r = warp; r < R; r += NW) {
-      double* xrow = X + rowoff[r];
-      const double* yrow = xrow + yx;
-      for (int c = lane; c < pitch; c += 32) {
-        double v = 0.0;
-        if (c <= h) {
-          v = yrow[c];
-          if (c >= 1 && c < h) v += yrow[np - c];
-        } else if (c >= ke && c < ke + L) {
-          const int k = c - ke + 1;
-          v = yrow[k] - yrow[np - k];
-        }
-        xrow[c] = v;
-      }
-    }
-  }
-  __syncthreads();
 
   const int MT1 = (R + 7) >> 3;
   // ---- S1: Cc = E Fa_c^T (columns 0..), Cs = O Fa_s^T (columns kc..) ----
@@ -445,20 +431,22 @@ k_ang(const AngItem* __restrict__ items, const double* __restrict__ tables, cons
       const int ro = rowoff[r];
       if (ch < nche) {
         const int n0 = ch * pere, nn = min(pere, D.NTc - n0);
-        const double* ap = X + ro + tl;
+        const double* ap = X + ro + tl;                  // k = 4 ks + tl, mirror n_phi - k
+        const double* am = X + ro + np - tl;
         const double* bp = F + n0 * 32 + lane;
         double* yrow = Y + ro;
         const int c0 = n0 * 8 + 2 * tl;
-#define GH_CALL(K) ang_s1_unit<K>(ap, bp, D.KSe1, D.NTc, yrow, c0, pitch, r < R)
+#define GH_CALL(K) ang_s1_unit<K>(ap, am, 1.0, bp, D.KSe1, D.NTc, yrow, c0, pitch, r < R)
         GH_NTC_SWITCH(nn, GH_CALL)
 #undef GH_CALL
       } else {
         const int n0 = (ch - nche) * pero, nn = min(pero, D.NTs - n0);
-        const double* ap = X + ro + ke + tl;
+        const double* ap = X + ro + 1 + tl;              // k = 4 ks + tl + 1, mirror n_phi - k
+        const double* am = X + ro + np - 1 - tl;
         const double* bp = Fo + n0 * 32 + lane;
         double* yrow = Y + ro + kc;
         const int c0 = n0 * 8 + 2 * tl;
-#define GH_CALL(K) ang_s1_unit<K>(ap, bp, D.KSo1, D.NTs, yrow, c0, pitch - kc, r < R)
+#define GH_CALL(K) ang_s1_unit<K>(ap, am, -1.0, bp, D.KSo1, D.NTs, yrow, c0, pitch - kc, r < R)
         GH_NTC_SWITCH(nn, GH_CALL)
 #undef GH_CALL
       }
