@@ -153,8 +153,14 @@ bool make_plan(const gh_subdomain_desc* descs, int32_t n_sub, Plan& pl, std::str
       if (!seenL.count(L)) { seenL[L] = 1; tab += shell_matrix_doubles(L); }
       // planes per CTA: the most (<= 8) that keep two CTAs on an SM if that is at least 4, else the most that fit
       int pb = 0, cls = 0;
-      for (int nb = ANG_NB_MAX; nb >= 4; --nb) if (ang_smem_bytes(L, nb) <= ANG_SMEM_2CTA) { pb = nb; break; }
-      if (!pb) { cls = 1; for (int nb = ANG_NB_MAX; nb >= 1; --nb) if (ang_smem_bytes(L, nb) <= SMEM_MAX) { pb = nb; break; } }
+#ifndef GH_ANG_MIN0
+#define GH_ANG_MIN0 4
+#endif
+#ifndef GH_ANG_CAP1
+#define GH_ANG_CAP1 8
+#endif
+      for (int nb = ANG_NB_MAX; nb >= GH_ANG_MIN0; --nb) if (ang_smem_bytes(L, nb) <= ANG_SMEM_2CTA) { pb = nb; break; }
+      if (!pb) { cls = 1; for (int nb = GH_ANG_CAP1; nb >= 1; --nb) if (ang_smem_bytes(L, nb) <= SMEM_MAX) { pb = nb; break; } }
       if (!pb) { err = "shell L too large for shared memory"; return false; }
       const int chunks = (n0 + pb - 1) / pb;
       pb = (n0 + chunks - 1) / chunks;            // near-equal chunks

@@ -133,7 +133,7 @@ k_cheb(const ChebItem* __restrict__ items, const double* __restrict__ tables, co
 // conflict-free LDS.64 / coalesced 256-byte LDG per fragment, tile offsets are immediates), so the inner loops carry
 // no bounds predicate.  Fa / Fs fragments live in shared memory; the per-m stacked matrices [Th_m ; m Pr_m] stream
 // from L2 two k-steps ahead.  Planes: X (raw U, later B') and Y (C, later A), row (b, j) at b*ps + j*pitch
-// doubles; coefficient rows hold cos m at column m and sin m at column kc + m - 1 (kc = 8 ceil(h/8)).
+// doubles; coefficient rows hold cos m at column m and sin m at column kc + m - 1 (kc = 4 ceil(h/4)).
 // pitch = 4 mod 8 and ps = 1 mod 16 keep the data-fragment loads conflict-free.  Rows beyond the tile range read a
 // zeroed row.
 // ---------------------------------------------------------------------------------------------------------
@@ -145,19 +145,19 @@ __host__ __device__ inline AngDims ang_dims(int L) {
   d.h = L + 1;
   d.KSe1 = (d.h + 1 + 3) / 4; d.NTc = (d.h + 7) / 8;      // S1 even: K = h+1 (k = 0..h),  N = h   (m = 0..L)
   d.KSo1 = (L + 3) / 4;       d.NTs = (L + 7) / 8;        // S1 odd:  K = L   (k = 1..L),  N = L   (m = 1..L)
-  d.kc = 8 * d.NTc; d.ke = 4 * d.KSe1;
   d.KSe3 = (d.h + 3) / 4; d.KSo3 = (L + 3) / 4;           // S3: K = h (m = 0..L) / L (m = 1..L)
+  d.kc = 4 * d.KSe3; d.ke = 0;                            // coefficient rows: cos m at m, sin m at kc + m - 1
   d.NT3 = (d.h + 1 + 7) / 8;                              //     N = h+1 (k = 0..h) for both
   return d;
 }
 __host__ __device__ inline int ang_pitch(int L) {   // row pitch (doubles), = 4 mod 8
   const AngDims d = ang_dims(L);
-  const int a = d.kc + 8 * d.NTs, b = 2 * L + 2 + 1;      // coefficient rows; raw rows need n_phi + 1 (a zero at column n_phi)
+  const int a = d.kc + 4 * d.KSo3, b = 2 * L + 2 + 1;     // coefficient rows; raw rows need n_phi + 1 (a zero at column n_phi)
   int p = ((a > b ? a : b) + 3) / 4 * 4;
   return (p % 8 == 0) ? p + 4 : p;
 }
-__host__ __device__ inline int ang_plane_stride(int L) {   // plane stride (doubles): rows padded to 4, = 1 mod 16
-  return ((L + 1 + 3) / 4 * 4 * ang_pitch(L) + 15) / 16 * 16 + 1;
+__host__ __device__ inline int ang_plane_stride(int L) {   // plane stride (doubles), = 1 mod 16
+  return ((L + 1) * ang_pitch(L) + 15) / 16 * 16 + 1;
 }
 __host__ __device__ inline size_t ang_fa_doubles(int L) { const AngDims d = ang_dims(L); return (size_t)(d.KSe1 * d.NTc + d.KSo1 * d.NTs) * 32; }
 __host__ __device__ inline size_t ang_fs_doubles(int L) { const AngDims d = ang_dims(L); return (size_t)(d.KSe3 + d.KSo3) * d.NT3 * 32; }
@@ -187,7 +187,7 @@ template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile(
 template <int NTC>
 __device__ __forceinline__ void ang_s1_unit(const double* __restrict__ ap, const double* __restrict__ am, double sg,
                                             const double* __restrict__ bp, int KS, int NT,
-                                            double* __restrict__ yrow, int c0, int pitch, bool rok) {
+                                            double* __restrict__ yrow, int c0, int climit, bool rok) {
   double acc[NTC][2];
 #pragma unroll
   for (int n = 0; n < NTC; ++n) acc[n][0] = acc[n][1] = 0.0;
@@ -203,7 +203,7 @@ __device__ __forceinline__ void ang_s1_unit(const double* __restrict__ ap, const
 #pragma unroll
     for (int n = 0; n < NTC; ++n) {
       const int c = c0 + n * 8;
-      if (c < pitch) { yrow[c] = acc[n][0]; yrow[c + 1] = acc[n][1]; }
+      if (c < climit) { yrow[c] = acc[n][0]; yrow[c + 1] = acc[n][1]; }     // climit: end of the cos / sin region (multiple of 4)
     }
   }
 }
@@ -312,8 +312,8 @@ __device__ __forceinline__ void ang_s2_unit(const double* __restrict__ tp /* T_m
       for (int mt = 0; mt < MT2; ++mt) a1[mt] = __ldg(tp + mt * 32);
     }
     tp += MT2 * 32;
-    const double yv = yp[0];
-    const double b = bok ? yv : 0.0;
+    const double yv = yp[0];                                  // rows j >= nt (K padding) read whatever follows: discarded
+    const double b = (bok && ks * 4 + tl < nt) ? yv : 0.0;
     yp += ystep;
 #pragma unroll
     for (int mt = 0; mt < MT2; ++mt) dmma884(acc[mt][0], acc[mt][1], a[mt], b);
@@ -408,12 +408,6 @@ k_ang(const AngItem* __restrict__ items, const double* __restrict__ tables, cons
       rowoff[r] = (r < R) ? b * ps + j * pitch : zoff;
     }
     for (int e = tid; e < pitch + 16; e += TPB) Z[e] = 0.0;
-    // rows [nt, 4*ceil(nt/4)) of Y (K padding of S2)
-    const int ntp = (nt + 3) & ~3, padr = (ntp - nt) * pitch;
-    for (int e = tid; e < nb * padr; e += TPB) {
-      const int b = e / padr;
-      Y[(size_t)b * ps + nt * pitch + (e - b * padr)] = 0.0;
-    }
     cp_async_wait<0>();
   }
   __syncthreads();
@@ -436,7 +430,7 @@ k_ang(const AngItem* __restrict__ items, const double* __restrict__ tables, cons
         const double* bp = F + n0 * 32 + lane;
         double* yrow = Y + ro;
         const int c0 = n0 * 8 + 2 * tl;
-#define GH_CALL(K) ang_s1_unit<K>(ap, am, 1.0, bp, D.KSe1, D.NTc, yrow, c0, pitch, r < R)
+#define GH_CALL(K) ang_s1_unit<K>(ap, am, 1.0, bp, D.KSe1, D.NTc, yrow, c0, kc, r < R)
         GH_NTC_SWITCH(nn, GH_CALL)
 #undef GH_CALL
       } else {
@@ -446,7 +440,7 @@ k_ang(const AngItem* __restrict__ items, const double* __restrict__ tables, cons
         const double* bp = Fo + n0 * 32 + lane;
         double* yrow = Y + ro + kc;
         const int c0 = n0 * 8 + 2 * tl;
-#define GH_CALL(K) ang_s1_unit<K>(ap, am, -1.0, bp, D.KSo1, D.NTs, yrow, c0, pitch - kc, r < R)
+#define GH_CALL(K) ang_s1_unit<K>(ap, am, -1.0, bp, D.KSo1, D.NTs, yrow, c0, 4 * D.KSo3, r < R)
         GH_NTC_SWITCH(nn, GH_CALL)
 #undef GH_CALL
       }
