@@ -85,9 +85,9 @@ inline int ang_best_nch(int NT, int MT1, int NW, int w, int per_max) {
 inline size_t ang_smem_bytes(int L, int nb) { return ang_smem_doubles(L, nb) * sizeof(double); }
 inline size_t shell_fa_doubles(int L) { return ang_fa_doubles(L); }   // (even | odd) analysis fragments
 inline size_t shell_fs_doubles(int L) { return ang_fs_doubles(L); }   // (even | odd) synthesis fragments
-inline size_t shell_t_doubles(int L) {    // [m][k_step][m_tile][32], stacked [Th_m ; m Pr_m], see AngItem
-  const size_t nt = L + 1, mtn = (2 * nt + 7) / 8, ks = (nt + 3) / 4;
-  return (size_t)(L + 1) * ks * mtn * 32;
+inline size_t shell_t_doubles(int L) {    // [m][k_step][even|odd][m_tile][32]: the equator-folded stacked matrices of K_ang S2
+  const size_t nt = L + 1, hh = (nt + 1) / 2, mth = (2 * hh + 7) / 8, ksh = (hh + 3) / 4;
+  return (size_t)(L + 1) * ksh * 2 * mth * 32;
 }
 inline size_t shell_matrix_doubles(int L) { return shell_fa_doubles(L) + shell_fs_doubles(L) + shell_t_doubles(L); }
 
@@ -403,18 +403,26 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
             if (m <= L && k >= 1 && k < h) FS[fso + ((size_t)ks * dm.NT3 + n) * 32 + lane] = B.Fs[(size_t)k * nq + L + m];
           }
           o.Fs = put(FS);
-          // stacked [Th_m ; m Pr_m] (2 nt x nt) as the A operand of S2: element (row = 8 mt + g, col = 4 ks + t)
-          const int mtn = (2 * nt + 7) / 8, ks2 = (nt + 3) / 4;
+          // S2 A operands, folded about the equator (jbar = nt-1-j; K_ang S2 forms p_j = C_j + C_jbar, q_j = C_j - C_jbar, j < hh):
+          //   ME (acts on p) = 1/2 (M[r][j] + M[r][jbar]),  MO (acts on q) = 1/2 (M[r][j] - M[r][jbar]),  r, j < hh,
+          //   M = Th_m for stacked rows [0, hh) and m Pr_m for rows [hh, 2 hh); the equator node (j = jbar, odd nt) has
+          //   p = 2 C_j, q = 0: its ME column is 1/2 M[r][j].   element (row = 8 mt + g, col = 4 ks + t)
+          const int hh = (nt + 1) / 2, mth = (2 * hh + 7) / 8, ksh = (hh + 3) / 4;
           std::vector<ghb::ld> T(shell_t_doubles(L), 0);
-          for (int m = 0; m <= L; ++m) for (int ks = 0; ks < ks2; ++ks) for (int mt = 0; mt < mtn; ++mt) for (int lane = 0; lane < 32; ++lane) {
-            const int row = mt * 8 + lane / 4, col = ks * 4 + lane % 4;
-            ghb::ld v = 0;
-            if (col < nt) {
-              if (row < nt) v = B.Th[((size_t)m * nt + row) * nt + col];
-              else if (row < 2 * nt) v = (ghb::ld)m * B.Pr[((size_t)m * nt + (row - nt)) * nt + col];
+          for (int m = 0; m <= L; ++m) for (int ks = 0; ks < ksh; ++ks) for (int w = 0; w < 2; ++w) for (int mt = 0; mt < mth; ++mt)
+            for (int lane = 0; lane < 32; ++lane) {
+              const int row = mt * 8 + lane / 4, j = ks * 4 + lane % 4;
+              ghb::ld v = 0;
+              if (j < hh && row < 2 * hh) {
+                const int r = row < hh ? row : row - hh, jb = nt - 1 - j;
+                const std::vector<ghb::ld>& M = row < hh ? B.Th : B.Pr;
+                const ghb::ld f = row < hh ? (ghb::ld)1 : (ghb::ld)m;
+                const ghb::ld a = M[((size_t)m * nt + r) * nt + j], c = M[((size_t)m * nt + r) * nt + jb];
+                if (jb == j) v = w == 0 ? f * a / 2 : (ghb::ld)0;
+                else v = f * (w == 0 ? a + c : a - c) / 2;
+              }
+              T[((((size_t)m * ksh + ks) * 2 + w) * mth + mt) * 32 + lane] = v;
             }
-            T[(((size_t)m * ks2 + ks) * mtn + mt) * 32 + lane] = v;
-          }
           o.T = put(T);
         }
         Lcache[L] = o;

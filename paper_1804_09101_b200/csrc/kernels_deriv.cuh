@@ -126,7 +126,7 @@ k_cheb(const ChebItem* __restrict__ items, const double* __restrict__ tables, co
 //               carries a zero at column n_phi and the k = h row of Fa_c is halved, so no lane needs a predicate)
 //   S1  Cc[r][m] = sum_{k=0..h} E[r][k] Fa_c[m][k]  (m = 0..L),   Cs[r][m] = sum_{k=1..L} O[r][k] Fa_s[m][k]  (m = 1..L)
 //   S2  [A ; B'](m) = [Th_m ; m Pr_m] C_m   per m, columns (t = cos/sin, plane b); A in place over C, B' into the
-//               cos<->sin partner slot with sign (d/dphi in coefficient space)
+//               cos<->sin partner slot with sign (d/dphi in coefficient space); folded about the equator (see S2 unit)
 //   S3  e[r][k] = sum_m Ac[r][m] Fs_c[k][m],  o[r][k] = sum_m As[r][m] Fs_s[k][m]  (k = 0..h), same for B';
 //               d u[r][k] = e + o,  d u[r][n_phi-k] = e - o, stored straight from the accumulators
 // Every matrix operand is stored in DMMA fragment order, zero padded to whole tiles ([k_step][tile][32 lanes]: one
@@ -138,7 +138,7 @@ k_cheb(const ChebItem* __restrict__ items, const double* __restrict__ tables, co
 // zeroed row.
 // ---------------------------------------------------------------------------------------------------------
 struct AngDims {
-  int h, KSe1, NTc, KSo1, NTs, kc, ke, KSe3, KSo3, NT3;
+  int h, KSe1, NTc, KSo1, NTs, kc, KSe3, KSo3, NT3;
 };
 __host__ __device__ inline AngDims ang_dims(int L) {
   AngDims d;
@@ -146,7 +146,7 @@ __host__ __device__ inline AngDims ang_dims(int L) {
   d.KSe1 = (d.h + 1 + 3) / 4; d.NTc = (d.h + 7) / 8;      // S1 even: K = h+1 (k = 0..h),  N = h   (m = 0..L)
   d.KSo1 = (L + 3) / 4;       d.NTs = (L + 7) / 8;        // S1 odd:  K = L   (k = 1..L),  N = L   (m = 1..L)
   d.KSe3 = (d.h + 3) / 4; d.KSo3 = (L + 3) / 4;           // S3: K = h (m = 0..L) / L (m = 1..L)
-  d.kc = 4 * d.KSe3; d.ke = 0;                            // coefficient rows: cos m at m, sin m at kc + m - 1
+  d.kc = 4 * d.KSe3;                                      // coefficient rows: cos m at m, sin m at kc + m - 1
   d.NT3 = (d.h + 1 + 7) / 8;                              //     N = h+1 (k = 0..h) for both
   return d;
 }
@@ -268,59 +268,53 @@ __device__ __forceinline__ void ang_s3_unit(const double* __restrict__ a0p, cons
   }
 }
 
-// S2 unit: mode m, n-tile `ntile` of its columns; MT2 m-tiles of the stacked matrix [Th_m ; m Pr_m]
-template <int MT2>
-__device__ __forceinline__ void ang_s2_unit(const double* __restrict__ tp /* T_m fragments + lane */, int KS2,
+// S2 unit: mode m, n-tile `ntile` of its columns.  The Gauss-Legendre nodes are symmetric about the equator
+// (theta_{nt-1-j} = pi - theta_j), the projector Pr_m commutes with that reflection and d/dtheta anticommutes, so with
+// p_j = C_j + C_jbar, q_j = C_j - C_jbar (j < hh = ceil(nt/2), jbar = nt-1-j) folded on the fly in the B-operand load,
+//   [alpha ; gamma] = ME_m p,  [beta ; delta] = MO_m q      (two stacked (2 hh x hh) matrices instead of one (2 nt x nt))
+//   A_j = alpha + beta, A_jbar = beta - alpha;   B_j = gamma + delta, B_jbar = gamma - delta:      half the flop of S2.
+// MTH m-tiles of each stacked matrix; fragments [ks][which][mt][32] stream from L2 one k-step ahead.
+template <int MTH>
+__device__ __forceinline__ void ang_s2_unit(const double* __restrict__ tp /* T_m fragments + lane */, int KSh,
                                             double* __restrict__ X, double* __restrict__ Y, int m, int ntile, int nb,
                                             int L, int kc, int pitch, int ps, int g, int tl) {
-  const int nt = L + 1, ncols = (m == 0) ? nb : 2 * nb;
+  const int nt = L + 1, hh = (nt + 1) >> 1, ncols = (m == 0) ? nb : 2 * nb;
   const int slot_c = m, slot_s = kc + m - 1;      // coefficient columns of cos m / sin m
   // B fragment column of this lane
   const int cb = ntile * 8 + g;
   const bool bok = cb < ncols;
   const int tb = (bok && cb >= nb) ? 1 : 0, bb = bok ? cb - tb * nb : 0;
-  const double* __restrict__ yp = Y + bb * ps + (tb ? slot_s : slot_c) + tl * pitch;
-  double acc[MT2][2];
+  const double* __restrict__ ycol = Y + bb * ps + (tb ? slot_s : slot_c);
+  double ap_[MTH][2], aq_[MTH][2];
 #pragma unroll
-  for (int mt = 0; mt < MT2; ++mt) acc[mt][0] = acc[mt][1] = 0.0;
-  // A fragments one k-step ahead, two when the m-tile count leaves registers for it (L2 latency)
-  constexpr bool DEEP = MT2 <= 6;
-  double a1[MT2], a2[DEEP ? MT2 : 1];
+  for (int mt = 0; mt < MTH; ++mt) ap_[mt][0] = ap_[mt][1] = aq_[mt][0] = aq_[mt][1] = 0.0;
+  double np_[MTH], nq_[MTH];      // next k-step's A fragments
 #pragma unroll
-  for (int mt = 0; mt < MT2; ++mt) a1[mt] = __ldg(tp + mt * 32);
-  tp += MT2 * 32;
-  if (DEEP) {
-#pragma unroll
-    for (int mt = 0; mt < MT2; ++mt) a2[DEEP ? mt : 0] = (KS2 > 1) ? __ldg(tp + mt * 32) : 0.0;
-    tp += MT2 * 32;
-  }
-  const int ystep = 4 * pitch;
+  for (int mt = 0; mt < MTH; ++mt) { np_[mt] = __ldg(tp + mt * 32); nq_[mt] = __ldg(tp + (MTH + mt) * 32); }
 #pragma unroll 1
-  for (int ks = 0; ks < KS2; ++ks) {
-    double a[MT2];
+  for (int ks = 0; ks < KSh; ++ks) {
+    double fp[MTH], fq[MTH];
 #pragma unroll
-    for (int mt = 0; mt < MT2; ++mt) a[mt] = a1[mt];
-    if (DEEP) {
+    for (int mt = 0; mt < MTH; ++mt) { fp[mt] = np_[mt]; fq[mt] = nq_[mt]; }
+    tp += 2 * MTH * 32;
+    if (ks + 1 < KSh) {
 #pragma unroll
-      for (int mt = 0; mt < MT2; ++mt) a1[mt] = a2[DEEP ? mt : 0];
-      if (ks + 2 < KS2) {
-#pragma unroll
-        for (int mt = 0; mt < MT2; ++mt) a2[DEEP ? mt : 0] = __ldg(tp + mt * 32);
-      }
-    } else if (ks + 1 < KS2) {
-#pragma unroll
-      for (int mt = 0; mt < MT2; ++mt) a1[mt] = __ldg(tp + mt * 32);
+      for (int mt = 0; mt < MTH; ++mt) { np_[mt] = __ldg(tp + mt * 32); nq_[mt] = __ldg(tp + (MTH + mt) * 32); }
     }
-    tp += MT2 * 32;
-    const double yv = yp[0];                                  // rows j >= nt (K padding) read whatever follows: discarded
-    const double b = (bok && ks * 4 + tl < nt) ? yv : 0.0;
-    yp += ystep;
+    const int j = ks * 4 + tl;
+    const bool jok = bok && j < hh;
+    const int jc = jok ? j : 0;
+    const double y0 = ycol[jc * pitch], y1 = ycol[(nt - 1 - jc) * pitch];
+    const double bp = jok ? y0 + y1 : 0.0, bq = jok ? y0 - y1 : 0.0;
 #pragma unroll
-    for (int mt = 0; mt < MT2; ++mt) dmma884(acc[mt][0], acc[mt][1], a[mt], b);
+    for (int mt = 0; mt < MTH; ++mt) {
+      dmma884(ap_[mt][0], ap_[mt][1], fp[mt], bp);
+      dmma884(aq_[mt][0], aq_[mt][1], fq[mt], bq);
+    }
   }
   __syncwarp();   // every lane has read its C_m entries before any lane overwrites them
-  // C fragment: stacked row 8 mt + g, columns 8 ntile + 2 tl + e.  Destination per column e: A -> Y at the same slot;
-  // B' -> X at the partner slot with sign (cos input -> sin slot, negated; sin input -> cos slot); m = 0 -> 0
+  // C fragments: stacked row 8 mt + g (rows [0, hh): theta part, [hh, 2 hh): phi part), columns 8 ntile + 2 tl + e.
+  // A -> Y at the same slot; B' -> X at the partner slot with sign (cos input -> sin slot, negated; sin -> cos); m = 0 -> 0
   double* ydst[2]; double* xdst[2]; double sgn[2]; bool cok[2];
 #pragma unroll
   for (int e = 0; e < 2; ++e) {
@@ -332,14 +326,24 @@ __device__ __forceinline__ void ang_s2_unit(const double* __restrict__ tp /* T_m
     sgn[e] = (m == 0) ? 0.0 : (t ? 1.0 : -1.0);
   }
 #pragma unroll
-  for (int mt = 0; mt < MT2; ++mt) {
+  for (int mt = 0; mt < MTH; ++mt) {
     const int rr = mt * 8 + g;
-    if (rr < nt) {
+    if (rr < hh) {
+      const int jb = nt - 1 - rr;
 #pragma unroll
-      for (int e = 0; e < 2; ++e) if (cok[e]) ydst[e][rr * pitch] = acc[mt][e];
-    } else if (rr < 2 * nt) {
+      for (int e = 0; e < 2; ++e)
+        if (cok[e]) {
+          ydst[e][rr * pitch] = ap_[mt][e] + aq_[mt][e];
+          if (jb != rr) ydst[e][jb * pitch] = aq_[mt][e] - ap_[mt][e];
+        }
+    } else if (rr < 2 * hh) {
+      const int j = rr - hh, jb = nt - 1 - j;
 #pragma unroll
-      for (int e = 0; e < 2; ++e) if (cok[e]) xdst[e][(rr - nt) * pitch] = sgn[e] * acc[mt][e];
+      for (int e = 0; e < 2; ++e)
+        if (cok[e]) {
+          xdst[e][j * pitch] = sgn[e] * (ap_[mt][e] + aq_[mt][e]);
+          if (jb != j) xdst[e][jb * pitch] = sgn[e] * (ap_[mt][e] - aq_[mt][e]);
+        }
     }
   }
 }
@@ -391,12 +395,14 @@ k_ang(const AngItem* __restrict__ items, const double* __restrict__ tables, cons
   // ---- stage 0: raw U -> X and Fa fragments -> F by cp.async (all loads in flight at once); tables; padding ----
   {
     const int padc = pitch - np;
+    int b = warp / nt, j = warp - b * nt;
     for (int r = warp; r < R; r += NW) {
-      const int b = r / nt, j = r - b * nt;
       const double* __restrict__ urow = src + (size_t)r * np;
       double* xrow = X + (size_t)b * ps + j * pitch;
       for (int c = lane; c < np; c += 32) cp_async8(xrow + c, urow + c);
       if (lane < padc) xrow[np + lane] = 0.0;      // column n_phi = 0 (mirror of k = 0); the rest finite for S3
+      j += NW;
+      while (j >= nt) { j -= nt; ++b; }
     }
     const double* __restrict__ Fa = tables + it.m_Fa;
     const int nfa = (int)ang_fa_doubles(L);
@@ -457,27 +463,21 @@ k_ang(const AngItem* __restrict__ items, const double* __restrict__ tables, cons
   }
   // ---- S2: per m and n-tile of its columns ----
   {
-    const int MT2 = (2 * nt + 7) >> 3, KS2 = (nt + 3) >> 2;
+    const int hh = (nt + 1) >> 1, MTH = (2 * hh + 7) >> 3, KSh = (hh + 3) >> 2;
     const int NTn = (2 * nb + 7) >> 3;
     const double* __restrict__ T = tables + it.m_T + lane;
     for (int u = warp; u < (L + 1) * NTn; u += NW) {
       const int m = u / NTn, ntile = u - m * NTn;
       if (m == 0 && ntile * 8 >= nb) continue;
-      const double* tp = T + (size_t)m * KS2 * MT2 * 32;
-#define GH_S2(K) ang_s2_unit<K>(tp, KS2, X, Y, m, ntile, nb, L, kc, pitch, ps, g, tl)
-      switch (MT2) {
+      const double* tp = T + (size_t)m * KSh * 2 * MTH * 32;
+#define GH_S2(K) ang_s2_unit<K>(tp, KSh, X, Y, m, ntile, nb, L, kc, pitch, ps, g, tl)
+      switch (MTH) {
         case 1: GH_S2(1); break;
         case 2: GH_S2(2); break;
         case 3: GH_S2(3); break;
         case 4: GH_S2(4); break;
         case 5: GH_S2(5); break;
-        case 6: GH_S2(6); break;
-        case 7: GH_S2(7); break;
-        case 8: GH_S2(8); break;
-        case 9: GH_S2(9); break;
-        case 10: GH_S2(10); break;
-        case 11: GH_S2(11); break;
-        default: GH_S2(12); break;
+        default: GH_S2(6); break;
       }
 #undef GH_S2
     }
