@@ -564,27 +564,31 @@ gh_status check_flag(gh_domain* d) {   // stream must be synchronised by the cal
 
 // A2 + A3: logical derivatives of `ncomp` components of `in` into out[3][ncomp][S]
 // (blocks: d/dx, d/dy, d/dz already Cartesian; shells: d/dr, d/dtheta, d/dphi).
-gh_status launch_derivs(gh_domain* d, const double* in, double* out, int ncomp) {
+gh_status launch_derivs(gh_domain* d, const double* in, double* out, int ncomp, int skip_lo = 0, int skip_n = 0) {
   const Plan& pl = d->pl;
-  // each K_cheb CTA walks over ncomp / cheb_gy components (amortises its launch and matrix load)
-  const int cheb_gy = (ncomp % CHEB_COMP_WALK == 0) ? ncomp / CHEB_COMP_WALK : ncomp;
+  const CompMap cm{ncomp, skip_lo, skip_n};        // `in` / `out` have ncomp components, of which skip_n are left out
+  const int nrun = ncomp - skip_n;
+  // each K_cheb CTA walks over nrun / cheb_gy components (amortises its launch and matrix load)
+  int walk = 1;
+  for (int w = CHEB_COMP_WALK; w >= 1; --w) if (nrun % w == 0) { walk = w; break; }
+  const int cheb_gy = nrun / walk;
   if (pl.n_cheb_class[0]) {
     ProfScope ps(d, GH_K_CHEB);
     k_cheb<CHEB_TPB, 4, 8, CHEB_NTW0><<<dim3(pl.n_cheb_class[0], cheb_gy), CHEB_TPB, pl.cheb_smem, d->stream>>>(
-        d->cheb, d->tables, in, out, pl.S, ncomp);
+        d->cheb, d->tables, in, out, pl.S, nrun, cm);
   }
   if (pl.n_cheb_class[1]) {
     ProfScope ps(d, GH_K_CHEB);
     k_cheb<CHEB_TPB, 8, 16, CHEB_NTW1><<<dim3(pl.n_cheb_class[1], cheb_gy), CHEB_TPB, pl.cheb_smem, d->stream>>>(
-        d->cheb + pl.n_cheb_class[0], d->tables, in, out, pl.S, ncomp);
+        d->cheb + pl.n_cheb_class[0], d->tables, in, out, pl.S, nrun, cm);
   }
   for (int cls = 0, first = 0; cls < 2; first += pl.n_ang_class[cls], ++cls) {
     if (!pl.n_ang_class[cls]) continue;
     ProfScope ps(d, GH_K_SHELL_ANG);
     if (cls == 0)
-      k_ang<ANG_TPB0><<<dim3(pl.n_ang_class[0], ncomp), ANG_TPB0, pl.ang_smem[0], d->stream>>>(d->ang + first, d->tables, in, out, pl.S, ncomp);
+      k_ang<ANG_TPB0><<<dim3(pl.n_ang_class[0], nrun), ANG_TPB0, pl.ang_smem[0], d->stream>>>(d->ang + first, d->tables, in, out, pl.S, cm);
     else
-      k_ang<ANG_TPB1><<<dim3(pl.n_ang_class[1], ncomp), ANG_TPB1, pl.ang_smem[1], d->stream>>>(d->ang + first, d->tables, in, out, pl.S, ncomp);
+      k_ang<ANG_TPB1><<<dim3(pl.n_ang_class[1], nrun), ANG_TPB1, pl.ang_smem[1], d->stream>>>(d->ang + first, d->tables, in, out, pl.S, cm);
   }
   GH_CUDA(d, cudaGetLastError());
   return GH_OK;
@@ -709,7 +713,7 @@ extern "C" gh_status gh_constraint_norms(gh_domain* d, double* out, double* per_
   if (!d || !out) return fail(d, GH_ERR_ARG, "NULL argument");
   if (!d->has_fields) return fail(d, GH_ERR_STATE, "gh_constraint_norms before gh_set_fields");
   const Plan& pl = d->pl;
-  gh_status st = launch_derivs(d, d->ua, d->du, NCOMP);
+  gh_status st = launch_derivs(d, d->ua, d->du, NCOMP, 10, 10);   // the constraints need no derivative of Pi (components 10..19)
   if (st != GH_OK) return st;
   {
     ProfScope ps(d, GH_K_CONSTRAINTS);

@@ -25,10 +25,17 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
       : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
 
+// The derivative kernels run over `ncomp` components of an array with `total` components, skipping `skip_n` of them from
+// `skip_lo` on (gh_constraint_norms needs no derivative of Pi): launch index c -> component c (< skip_lo) or c + skip_n.
+struct CompMap {
+  int total, skip_lo, skip_n;
+  __device__ __forceinline__ int map(int c) const { return c < skip_lo ? c : c + skip_n; }
+};
+
 template <int TPB, int MTM, int KSM, int NTW>
 __global__ void __launch_bounds__(TPB, (MTM * NTW >= 16) ? 3 : 5)
 k_cheb(const ChebItem* __restrict__ items, const double* __restrict__ tables, const double* __restrict__ in,
-       double* __restrict__ out, int64_t S, int ncomp) {
+       double* __restrict__ out, int64_t S, int ncomp, CompMap cm) {
   extern __shared__ __align__(16) double sm[];   // D in fragment order [mt][ks][32]
   const ChebItem it = items[blockIdx.x];
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -63,7 +70,8 @@ k_cheb(const ChebItem* __restrict__ items, const double* __restrict__ tables, co
 
   // the CTA walks over components blockIdx.y, blockIdx.y + gridDim.y, ... (one launch and one matrix load for all of them)
 #pragma unroll 1
-  for (int comp = blockIdx.y; comp < ncomp; comp += gridDim.y) {
+  for (int cw = blockIdx.y; cw < ncomp; cw += gridDim.y) {
+    const int comp = cm.map(cw);
     // B fragments of the whole warp tile.  (si is laundered so that the compiler recomputes the 2 x KS x NTW element
     // offsets per component instead of keeping them all live across the loop: that costs 40 registers and a CTA per SM)
     int si = si0;
@@ -96,7 +104,7 @@ k_cheb(const ChebItem* __restrict__ items, const double* __restrict__ tables, co
           }
       }
     // C fragments: row a = 8 mt + g, columns 8 n + 2 tl and + 1
-    double* __restrict__ dst = out + ((int64_t)it.axis * ncomp + comp) * S + it.base;
+    double* __restrict__ dst = out + ((int64_t)it.axis * cm.total + comp) * S + it.base;
 #pragma unroll
     for (int n = 0; n < NTW; ++n) {
       const int c = wc0 + n * 8 + 2 * tl;
@@ -369,11 +377,11 @@ constexpr int ANG_NTC3 = 3;   // most n-tiles per warp unit in S3 (four accumula
 template <int TPB>
 __global__ void __launch_bounds__(TPB, TPB <= 256 ? 2 : 1)
 k_ang(const AngItem* __restrict__ items, const double* __restrict__ tables, const double* __restrict__ in,
-      double* __restrict__ out, int64_t S, int ncomp) {
+      double* __restrict__ out, int64_t S, CompMap cm) {
   extern __shared__ __align__(16) double sm[];
   constexpr int NW = TPB / 32;
   const AngItem it = items[blockIdx.x];
-  const int comp = blockIdx.y, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int comp = cm.map(blockIdx.y), ncomp = cm.total, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int g = lane >> 2, tl = lane & 3;
   const int L = it.L, nt = L + 1, np = 2 * L + 2, plane = nt * np;
   const AngDims D = ang_dims(L);

@@ -388,14 +388,22 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
   if (frozen) cp_async_wait<0>(); else cp_async_wait<RHS_RING>();   // the Phi group has landed
   if (!ok || frozen) {
     cp_async_wait<0>();   // nothing of this thread may still be landing in shared memory when the CTA retires
+    // frozen points issued no prefetch: u0 comes straight from memory.  All 50 loads go out before the first store: u0 and
+    // out are not __restrict__ (they may be the same array), so a load placed after a store would have to wait for it
+    double z[5][10];
+    if (RK == 2) {
+#pragma unroll
+      for (int c5 = 0; c5 < 5; ++c5)
+#pragma unroll
+        for (int s = 0; s < 10; ++s) z[c5][s] = rk.u0[(int64_t)(10 * c5 + s) * S + p];
+    }
 #pragma unroll
     for (int s = 0; s < 10; ++s) {
-      // (frozen points issued no prefetch: u0 comes straight from memory; read before the store, same address when in place)
-      rhs_store<RK>(k, rk, (int64_t)s * S + p, 0.0, psi[s], RK == 2 ? rk.u0[(int64_t)s * S + p] : 0.0);
-      rhs_store<RK>(k, rk, (int64_t)(10 + s) * S + p, 0.0, Pi[s], RK == 2 ? rk.u0[(int64_t)(10 + s) * S + p] : 0.0);
+      rhs_store<RK>(k, rk, (int64_t)s * S + p, 0.0, psi[s], RK == 2 ? z[0][s] : 0.0);
+      rhs_store<RK>(k, rk, (int64_t)(10 + s) * S + p, 0.0, Pi[s], RK == 2 ? z[1][s] : 0.0);
 #pragma unroll
       for (int i = 0; i < 3; ++i)
-        rhs_store<RK>(k, rk, (int64_t)(20 + 10 * i + s) * S + p, 0.0, Phi(i, s), RK == 2 ? rk.u0[(int64_t)(20 + 10 * i + s) * S + p] : 0.0);
+        rhs_store<RK>(k, rk, (int64_t)(20 + 10 * i + s) * S + p, 0.0, Phi(i, s), RK == 2 ? z[2 + i][s] : 0.0);
     }
     return;
   }

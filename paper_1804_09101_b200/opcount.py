@@ -53,6 +53,24 @@ def shell_factored_flop(n_e: int, n_r: int, L: int) -> int:
     return n_e * pts * ((2 * n_r - 1) + 8 * (2 * L + 1))
 
 
+def shell_executed_dmma_flop(n_e: int, n_r: int, L: int, nb: int = 8) -> int:
+    """Flop the angular kernel K_ang actually issues on the FP64 tensor cores for one shell (512 per mma.m8n8k4), with
+    both symmetry folds (phi about pi in S1/S3, theta about the equator in S2) and every tile padded to 8 x 8 x 4; planes are
+    processed in groups of `nb`.  Lower than 8(2L+1) per point: the folds halve the three GEMM stages."""
+    h = nt = L + 1
+    hh = (nt + 1) // 2
+    groups, rem = divmod(n_r, nb)
+    total = 0
+    for planes in [nb] * groups + ([rem] if rem else []):
+        mt1 = -(-planes * nt // 8)
+        s1 = mt1 * (-(-(h + 1) // 4) * -(-h // 8) + -(-L // 4) * -(-L // 8))
+        s3 = mt1 * 2 * (-(-h // 4) + -(-L // 4)) * -(-(h + 1) // 8)
+        ntn = -(-2 * planes // 8)
+        s2 = (L + 1) * 2 * -(-2 * hh // 8) * -(-hh // 4) * ntn
+        total += s1 + s2 + s3
+    return n_e * total * 512
+
+
 def effective_rates(m_transactions: float, flop: float, seconds: float):
     """Eqs. 3-4: BW_eff = w M / T (GB/s), P_eff = F / T (GFLOP/s)."""
     return 8.0 * m_transactions / seconds / 1e9, flop / seconds / 1e9
