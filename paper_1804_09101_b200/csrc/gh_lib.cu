@@ -569,8 +569,10 @@ gh_status launch_derivs(gh_domain* d, const double* in, double* out, int ncomp, 
   const CompMap cm{ncomp, skip_lo, skip_n};        // `in` / `out` have ncomp components, of which skip_n are left out
   const int nrun = ncomp - skip_n;
   // each K_cheb CTA walks over nrun / cheb_gy components (amortises its launch and matrix load)
+  // ... but small domains need the CTAs more than the amortisation: keep at least ~4 CTAs per SM in the grid
   int walk = 1;
-  for (int w = CHEB_COMP_WALK; w >= 1; --w) if (nrun % w == 0) { walk = w; break; }
+  for (int w = CHEB_COMP_WALK; w >= 1; --w)
+    if (nrun % w == 0 && (w == 1 || (int64_t)pl.n_cheb_items * (nrun / w) >= 4 * 148)) { walk = w; break; }
   const int cheb_gy = nrun / walk;
   if (pl.n_cheb_class[0]) {
     ProfScope ps(d, GH_K_CHEB);
