@@ -32,7 +32,9 @@
  * Gauss-Legendre exactness, Y_lm orthonormality / Unsold / closed forms,
  * Cartesian polynomials on shells, Kerr-Schild lapse/shift closed forms,
  * stationarity of exact Kerr-Schild data with analytic derivatives, the harmonic
- * gauge wave, homogeneous damping-term cases, RK3 order.  PARITY UNPINNED (pure
+ * gauge wave, homogeneous damping-term cases, RK3 order; spectral filter (O9):
+ * single Chebyshev modes and single Y_lm scaled by sigma, sigma = 1 identity /
+ * projection, Heaviside idempotence, linearity.  PARITY UNPINNED (pure
  * conventions, fixed by DESIGN.md): the normalisation of the constraint norms
  * (unweighted RMS over points and components) and the default gamma's.
  */
@@ -295,6 +297,87 @@ void ora_shell_project(int L, const double* u, double* out) {
   shell_plane(t, a, b, NULL, 1);
   for (int i = 0; i < np; ++i) out[i] = (double)b[i];
   free(a); free(b); ylm_free(t);
+}
+
+/* ---------------------------------------------------------------------- */
+/* O9 — spectral filter (NEXT-1).  "Spectral filtering of 1D basis        */
+/* functions is similar to differentiation, the only difference being the */
+/* specific form of the transformation matrix"; on     */
+/* shells: PhysToSpec -> filter -> SpecToPhys, here    */
+/* the scalar-in-l part; "we do not include a filter along the r-axis"    */
+/* (PAPER.md:500).  The filter function sigma is an INPUT (tables).       */
+/* ---------------------------------------------------------------------- */
+/* one Chebyshev line in place: u~_k <- sigma[k] u~_k  (Eqs. 17, 16) */
+static void cheb_filter_line(int N, real* u, int64_t st, const double* sigma) {
+  real* ut = malloc(sizeof(real) * N);
+  for (int k = 0; k < N; ++k) {
+    real s = 0;
+    for (int j = 0; j < N; ++j) { real cj = (j == 0 || j == N - 1) ? 2 : 1; s += u[j * st] * cheb_T(N, k, j) / cj; }
+    real ck = (k == 0 || k == N - 1) ? 2 : 1;
+    ut[k] = (real)sigma[k] * 2 * s / ((real)(N - 1) * ck);
+  }
+  for (int j = 0; j < N; ++j) { real s = 0; for (int k = 0; k < N; ++k) s += ut[k] * cheb_T(N, k, j); u[j * st] = s; }
+  free(ut);
+}
+
+/* one (theta,phi) plane: a_lm <- sigma_l[l] a_lm, then synthesis (Eq. 23 with filtered coefficients) */
+static void shell_filter_plane(const ylm_table* t, const real* u, real* out, const double* sigma_l) {
+  int L = t->L, n = t->nth, nph = t->nph;
+  real* are = calloc((size_t)n * n, sizeof(real)); real* aim = calloc((size_t)n * n, sizeof(real));
+  real dphi = 2 * R_PI / (real)nph;
+  for (int l = 0; l <= L; ++l) for (int m = 0; m <= l; ++m) {
+    real sr = 0, si = 0; const real* pb = t->pb + (int64_t)(l * n + m) * n;
+    for (int j = 0; j < n; ++j) for (int k = 0; k < nph; ++k) {
+      real f = t->w[j] * dphi * pb[j] * u[j * nph + k];
+      sr += f * t->cs[m * nph + k]; si -= f * t->sn[m * nph + k];
+    }
+    are[l * n + m] = (real)sigma_l[l] * sr; aim[l * n + m] = (real)sigma_l[l] * si;
+  }
+  for (int j = 0; j < n; ++j) for (int k = 0; k < nph; ++k) {
+    real s0 = 0;
+    for (int l = 0; l <= L; ++l) for (int m = 0; m <= l; ++m) {
+      real fac = (m == 0) ? 1 : 2;
+      real re = are[l * n + m] * t->cs[m * nph + k] - aim[l * n + m] * t->sn[m * nph + k];
+      s0 += fac * t->pb[(int64_t)(l * n + m) * n + j] * re;
+    }
+    out[j * nph + k] = s0;
+  }
+  free(are); free(aim);
+}
+
+/* u[ncomp][P] in place.  blocks: sig0/sig1/sig2 = sigma_k along x/y/z ([N_x], [N_y], [N_z]);
+ * shells: sig0 = sigma_l ([L+1]), sig1/sig2 unused. */
+int ora_filter_subdomain(const ora_subdomain* sd, int ncomp, double* u, const double* sig0, const double* sig1, const double* sig2) {
+  int n0, n1, n2; dims(sd, &n0, &n1, &n2); int64_t P = (int64_t)n0 * n1 * n2;
+  if (sd->kind == 1) {
+    int nn[3] = {n0, n1, n2}; int64_t st[3] = {(int64_t)n1 * n2, n2, 1}; const double* sg[3] = {sig0, sig1, sig2};
+#pragma omp parallel for schedule(dynamic)
+    for (int c = 0; c < ncomp; ++c) {
+      real* w = malloc(sizeof(real) * P);
+      for (int64_t p = 0; p < P; ++p) w[p] = u[(int64_t)c * P + p];
+      for (int d = 0; d < 3; ++d) {
+        int e = (d + 1) % 3, f = (d + 2) % 3;
+        for (int a = 0; a < nn[e]; ++a) for (int b = 0; b < nn[f]; ++b) cheb_filter_line(nn[d], w + a * st[e] + b * st[f], st[d], sg[d]);
+      }
+      for (int64_t p = 0; p < P; ++p) u[(int64_t)c * P + p] = (double)w[p];
+      free(w);
+    }
+    return 0;
+  }
+  int L = sd->n[1]; ylm_table* t = ylm_build(L); int64_t np = (int64_t)n1 * n2;
+#pragma omp parallel for schedule(dynamic)
+  for (int c = 0; c < ncomp; ++c) {
+    real* a = malloc(sizeof(real) * np); real* b = malloc(sizeof(real) * np);
+    for (int i = 0; i < n0; ++i) {
+      double* uc = u + (int64_t)c * P + i * np;
+      for (int64_t q = 0; q < np; ++q) a[q] = uc[q];
+      shell_filter_plane(t, a, b, sig0);
+      for (int64_t q = 0; q < np; ++q) uc[q] = (double)b[q];
+    }
+    free(a); free(b);
+  }
+  ylm_free(t);
+  return 0;
 }
 
 /* ---------------------------------------------------------------------- */

@@ -100,6 +100,8 @@ class Oracle:
         L.ora_rk3_subdomain.restype = C.c_int
         L.ora_constraints_subdomain.argtypes = [C.POINTER(Subdomain), _dp, _dp, _dp, _dp, C.c_void_p]
         L.ora_constraints_subdomain.restype = C.c_int
+        L.ora_filter_subdomain.argtypes = [C.POINTER(Subdomain), C.c_int, _dp, _dp, _dp, _dp]
+        L.ora_filter_subdomain.restype = C.c_int
         self.threads = threads
         if threads is not None:
             try:
@@ -153,6 +155,17 @@ class Oracle:
         u = np.ascontiguousarray(u, dtype=np.float64)
         out = np.empty_like(u)
         self.lib.ora_shell_project(L, u, out)
+        return out
+
+    def spectral_filter(self, sd: dict, u: np.ndarray, sigmas) -> np.ndarray:
+        """O9: filtered copy of u[ncomp][P].  sigmas: blocks [sigma_x, sigma_y, sigma_z] (one value per Chebyshev mode);
+        shells [sigma_l] (l = 0..L; no radial filter)."""
+        s = make_subdomain(sd)
+        out = np.array(u, dtype=np.float64, order="C", copy=True)
+        sg = [np.ascontiguousarray(x, dtype=np.float64) for x in sigmas]
+        while len(sg) < 3:
+            sg.append(sg[0])
+        self.lib.ora_filter_subdomain(C.byref(s), out.shape[0], out, sg[0], sg[1], sg[2])
         return out
 
     def gradient(self, sd: dict, u: np.ndarray) -> np.ndarray:
