@@ -129,12 +129,44 @@ gh_status gh_rk_step(gh_domain* dom, double dt);
  * GH_ERR_SINGULAR if the device flag was raised. */
 gh_status gh_constraint_norms(gh_domain* dom, double* out, double* per_sub);
 
+/* ---- spectral filter (NEXT-1 of DESIGN.md; "Filter ~ 30 % of CPU runtime", 452-460, 500-516) ----------
+ * "Spectral filtering of 1D basis functions is similar to differentiation, the only difference being the specific
+ * form of the transformation matrix": on blocks the state is multiplied along every axis by the
+ * cached matrix F = SpecToPhys diag(sigma_k) PhysToSpec (Eqs. 16-17); on shells every (theta,phi) plane goes
+ * PhysToSpec -> sigma_l a_lm -> SpecToPhys (the scalar-in-l filter: the tensor-harmonic coupling
+ * matrix is not defined in the paper), with no filter along r ("we do not include a filter along the r-axis",
+ * PAPER.md:500).  The paper names its two filter functions "Heaviside" and "ExpCheb" without formulas; reading S20:
+ *   GH_FILTER_HEAVISIDE: sigma_k = 1 for k <= kmax - cut, else 0            (the top `cut` modes are removed)
+ *   GH_FILTER_EXP:       sigma_k = exp(-alpha (k / kmax)^(2 p))
+ * with k the Chebyshev mode number (kmax = N-1 on that axis) or the harmonic degree l (kmax = L). */
+typedef enum { GH_FILTER_NONE = 0, GH_FILTER_HEAVISIDE = 1, GH_FILTER_EXP = 2 } gh_filter_kind;
+typedef struct {
+  int32_t kind;   /* gh_filter_kind */
+  int32_t cut;    /* HEAVISIDE: number of top modes removed (>= 0) */
+  double alpha;   /* EXP */
+  int32_t p;      /* EXP: half order (>= 1) */
+  int32_t pad_;
+} gh_filter_desc;
+
+/* Choose the filters: `block_axes` for the three Chebyshev axes of every block, `shell_angular` for the l-filter of every
+ * shell (either may be NULL or kind NONE: that family is left untouched).  Builds the matrices on the host in long
+ * double and uploads them (synchronises).  descs: HOST. */
+gh_status gh_set_filter(gh_domain* dom, const gh_filter_desc* block_axes, const gh_filter_desc* shell_angular);
+
+/* state <- filtered state, in place, asynchronous on the domain's stream.  GH_ERR_STATE before gh_set_filter /
+ * gh_set_fields.  The derivative scratch is used as temporary storage. */
+gh_status gh_apply_filter(gh_domain* dom);
+
+/* The filter function itself, for tests: sigma[0..kmax].  HOST. */
+gh_status gh_filter_sigma(const gh_filter_desc* f, int32_t kmax, double* sigma);
+
 /* Per-kernel device time of the most recent gh_rhs / gh_rk_step / gh_constraint_norms, in
  * milliseconds, measured with CUDA events on the domain's stream when profiling is enabled with
  * gh_set_profiling(dom, 1) (off by default: event records cost launch latency).
  * ms: HOST [GH_NUM_KERNELS] accumulated since the last call to gh_profile_reset; counts likewise. */
-#define GH_NUM_KERNELS 8
-enum { GH_K_CHEB = 0, GH_K_SHELL_ANG = 1, GH_K_RHS = 2, GH_K_RK = 3, GH_K_CONSTRAINTS = 4, GH_K_REDUCE = 5, GH_K_JAC = 6, GH_K_OTHER = 7 };
+#define GH_NUM_KERNELS 10
+enum { GH_K_CHEB = 0, GH_K_SHELL_ANG = 1, GH_K_RHS = 2, GH_K_RK = 3, GH_K_CONSTRAINTS = 4, GH_K_REDUCE = 5, GH_K_JAC = 6, GH_K_OTHER = 7,
+       GH_K_FILTER_CHEB = 8, GH_K_FILTER_ANG = 9 };
 gh_status gh_set_profiling(gh_domain* dom, int enabled);
 gh_status gh_profile_read(gh_domain* dom, double* ms, int64_t* counts);
 gh_status gh_profile_reset(gh_domain* dom);

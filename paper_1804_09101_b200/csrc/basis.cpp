@@ -133,4 +133,43 @@ void shell_basis(int L, ShellBasis& B) {
   }
 }
 
+void cheb_filter_matrix(int N, const std::vector<ld>& sigma, std::vector<ld>& F) {
+  F.assign((size_t)N * N, 0);
+  const int n = N - 1;
+  // T_k(x_j) = (-1)^k cos(pi j k / n) for x_j = -cos(pi j / n); the argument is reduced in integers
+  auto T = [&](int k, int j) {
+    const long long r = ((long long)j * k) % (2LL * n);
+    const ld v = cosl(PI_L * r / (ld)n);
+    return (k & 1) ? -v : v;
+  };
+  for (int a = 0; a < N; ++a)
+    for (int j = 0; j < N; ++j) {
+      ld s = 0;
+      const ld cj = (j == 0 || j == n) ? 2 : 1;
+      for (int k = 0; k < N; ++k) {
+        const ld ck = (k == 0 || k == n) ? 2 : 1;
+        s += T(k, a) * sigma[k] * T(k, j) / ck;
+      }
+      F[(size_t)a * N + j] = 2 * s / ((ld)n * cj);
+    }
+}
+
+void shell_filter_composites(int L, const std::vector<ld>& sigma_l, std::vector<ld>& G) {
+  const int nt = L + 1;
+  std::vector<ld> ct, w, st(nt);
+  gauss_legendre(L, ct, w);
+  for (int j = 0; j < nt; ++j) st[j] = sqrtl((1 - ct[j]) * (1 + ct[j]));
+  G.assign((size_t)(L + 1) * nt * nt, 0);
+  std::vector<std::vector<ld>> P(nt);
+  for (int m = 0; m <= L; ++m) {
+    for (int j = 0; j < nt; ++j) pbar_column(L, m, ct[j], st[j], P[j]);
+    for (int jo = 0; jo < nt; ++jo)
+      for (int ji = 0; ji < nt; ++ji) {
+        ld sp = 0;
+        for (int l = m; l <= L; ++l) sp += sigma_l[l] * P[jo][l - m] * P[ji][l - m];
+        G[((size_t)m * nt + jo) * nt + ji] = 2 * PI_L * w[ji] * sp;
+      }
+  }
+}
+
 }  // namespace ghb

@@ -32,4 +32,11 @@ struct ShellBasis {
 };
 void shell_basis(int L, ShellBasis& B);
 
+// Spectral filter matrices (NEXT-1).
+// Chebyshev line filter F = SpecToPhys diag(sigma) PhysToSpec on N CGL nodes (row-major N x N), Eqs. 16-17:
+//   F[a][j] = sum_k T_k(x_a) sigma_k (2/(N-1)) (1/(c_k c_j)) T_k(x_j).
+void cheb_filter_matrix(int N, const std::vector<ld>& sigma, std::vector<ld>& F);
+// Per-m filtered projectors on the Gauss-Legendre colatitudes: G[m][j'][j] = 2 pi sum_{l=m}^{L} sigma_l Pbar_lm(j') w_j Pbar_lm(j).
+void shell_filter_composites(int L, const std::vector<ld>& sigma_l, std::vector<ld>& G);
+
 }  // namespace ghb

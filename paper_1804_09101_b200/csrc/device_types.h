@@ -49,6 +49,7 @@ struct AngItem {
   int32_t m_Fa, m_Fs, m_T;       // offsets (doubles) in the table memory, all in DMMA fragment order [k_step][n_tile][32]:
                                  // Fa = (even | odd) analysis, Fs = (even | odd) synthesis (see K_ang); stacked per-m
                                  // matrices [Th_m ; m Pr_m] as [m][k_step][m_tile][32]
+  int32_t m_G;                   // spectral filter: per-m folded filtered projectors [m][k_step][even|odd][m_tile][32] (gh_set_filter)
   int8_t nch1e, nch1o, nch3, pad8_;   // n-chunks per m-tile in S1 (even, odd GEMM) / S3 (host-chosen for balance over the warps)
 };
 

@@ -56,13 +56,15 @@ struct Plan {
   int64_t P = 0, S = 0;
   int n_tiles = 0;
   size_t table_doubles = 0;
+  size_t ftable_doubles = 0;             // spectral-filter matrices, directly behind the derivative tables
+  int n_fcheb[3][2] = {{0, 0}, {0, 0}, {0, 0}}, n_fcheb_items = 0;   // filter work items of the blocks per axis and class
   int n_cheb_items = 0, n_cheb_class[2] = {0, 0}, n_ang_items = 0;
   int n_ang_class[2] = {0, 0};           // K_ang items per shared-memory class (0: two CTAs per SM, 1: one)
   size_t cheb_smem = 0, ang_smem[2] = {0, 0};
   std::vector<int> ang_pb;               // planes per CTA for each subdomain (0 for blocks)
   std::vector<int> ang_class;            // shared-memory class of each shell
   // workspace offsets (bytes)
-  size_t o_ua, o_ub, o_k, o_du, o_H, o_dH, o_tables, o_subs, o_tiles, o_cheb, o_ang, o_part, o_persub, o_flag, total;
+  size_t o_ua, o_ub, o_k, o_du, o_H, o_dH, o_tables, o_subs, o_tiles, o_cheb, o_fcheb, o_ang, o_part, o_persub, o_flag, total;
 };
 
 inline void sub_dims(const gh_subdomain_desc& d, int& n0, int& n1, int& n2) {
@@ -90,6 +92,10 @@ inline size_t shell_t_doubles(int L) {    // [m][k_step][even|odd][m_tile][32]: 
   return (size_t)(L + 1) * ksh * 2 * mth * 32;
 }
 inline size_t shell_matrix_doubles(int L) { return shell_fa_doubles(L) + shell_fs_doubles(L) + shell_t_doubles(L); }
+inline size_t shell_g_doubles(int L) {    // [m][k_step][even|odd][m_tile][32]: equator-folded filtered projectors (hh rows)
+  const size_t nt = L + 1, hh = (nt + 1) / 2, mtf = (hh + 7) / 8, ksh = (hh + 3) / 4;
+  return (size_t)(L + 1) * ksh * 2 * mtf * 32;
+}
 
 bool validate(const gh_subdomain_desc* descs, int32_t n_sub, std::string& err) {
   char buf[256];
@@ -146,11 +152,12 @@ bool make_plan(const gh_subdomain_desc* descs, int32_t n_sub, Plan& pl, std::str
       const int items = (int)((cols + cheb_ct(N) - 1) / cheb_ct(N));
       pl.n_cheb_items += items; pl.n_cheb_class[cheb_class(N)] += items;
       pl.cheb_smem = std::max(pl.cheb_smem, cheb_frag_doubles(N) * sizeof(double));
+      if (d.kind == GH_BLOCK) { pl.ftable_doubles += cheb_frag_doubles(N); pl.n_fcheb[a][cheb_class(N)] += items; pl.n_fcheb_items += items; }
     }
     if (d.kind == GH_SHELL) {
       const int L = d.n[1];
       tab += (size_t)round_up(n0, 2) + 2 * (size_t)round_up(n1, 2) + 2 * (size_t)round_up(n2, 2);
-      if (!seenL.count(L)) { seenL[L] = 1; tab += shell_matrix_doubles(L); }
+      if (!seenL.count(L)) { seenL[L] = 1; tab += shell_matrix_doubles(L); pl.ftable_doubles += shell_g_doubles(L); }
       // planes per CTA: the most (<= 8) that keep two CTAs on an SM if that is at least 4, else the most that fit
       int pb = 0, cls = 0;
 #ifndef GH_ANG_MIN0
@@ -178,10 +185,11 @@ bool make_plan(const gh_subdomain_desc* descs, int32_t n_sub, Plan& pl, std::str
   const size_t comp = (size_t)pl.S * sizeof(double);
   pl.o_ua = c.take(NCOMP * comp); pl.o_ub = c.take(NCOMP * comp); pl.o_k = c.take(NCOMP * comp);
   pl.o_du = c.take(3 * NCOMP * comp); pl.o_H = c.take(4 * comp); pl.o_dH = c.take(12 * comp);
-  pl.o_tables = c.take(pl.table_doubles * sizeof(double));
+  pl.o_tables = c.take((pl.table_doubles + pl.ftable_doubles) * sizeof(double));
   pl.o_subs = c.take((size_t)n_sub * sizeof(SubDev));
   pl.o_tiles = c.take((size_t)(n_sub + 1) * sizeof(int32_t));
   pl.o_cheb = c.take((size_t)pl.n_cheb_items * sizeof(ChebItem));
+  pl.o_fcheb = c.take((size_t)std::max(1, pl.n_fcheb_items) * sizeof(ChebItem));
   pl.o_ang = c.take((size_t)std::max(1, pl.n_ang_items) * sizeof(AngItem));
   pl.o_part = c.take((size_t)pl.n_tiles * 6 * sizeof(double));
   pl.o_persub = c.take((size_t)n_sub * 6 * sizeof(double));
@@ -200,7 +208,12 @@ struct gh_domain {
   SubDev* subs = nullptr;
   int32_t* tiles = nullptr;
   ChebItem* cheb = nullptr;
+  ChebItem* fcheb = nullptr;             // filter items of the blocks, ordered [axis][class]
   AngItem* ang = nullptr;
+  struct FBlock { int N; double unused; size_t off; };     // one filter matrix slot per (block, axis): offset (doubles) from `tables`
+  std::vector<FBlock> f_blocks;
+  std::map<int, size_t> f_L;             // shell band limit L -> offset (doubles) of its filtered projectors from `tables`
+  bool filt_blocks = false, filt_shells = false;
   double *part = nullptr, *persub = nullptr;
   int* flag = nullptr;
   std::vector<SubDev> h_subs;
@@ -310,12 +323,14 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
   d->ua = (double*)(w + pl.o_ua); d->ub = (double*)(w + pl.o_ub); d->k = (double*)(w + pl.o_k);
   d->du = (double*)(w + pl.o_du); d->H = (double*)(w + pl.o_H); d->dH = (double*)(w + pl.o_dH);
   d->tables = (double*)(w + pl.o_tables); d->subs = (SubDev*)(w + pl.o_subs); d->tiles = (int32_t*)(w + pl.o_tiles);
-  d->cheb = (ChebItem*)(w + pl.o_cheb); d->ang = (AngItem*)(w + pl.o_ang);
+  d->cheb = (ChebItem*)(w + pl.o_cheb); d->ang = (AngItem*)(w + pl.o_ang); d->fcheb = (ChebItem*)(w + pl.o_fcheb);
   d->part = (double*)(w + pl.o_part); d->persub = (double*)(w + pl.o_persub); d->flag = (int*)(w + pl.o_flag);
 
   // ---- tables and work lists on the host ----
   std::vector<double> tab(pl.table_doubles, 0.0);
   std::vector<ChebItem> cheb, cheb1; cheb.reserve(pl.n_cheb_items);   // class 0 items, class 1 items (appended below)
+  std::vector<ChebItem> fch[3][2];       // spectral-filter items of the blocks per axis and class
+  size_t ftp = pl.table_doubles;         // running offset inside the filter-table region
   std::vector<AngItem> ang, ang1; ang.reserve(pl.n_ang_items);   // class 0 items, class 1 items (appended below)
   d->h_subs.resize(n_sub);
   size_t tp = 0;
@@ -361,7 +376,9 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
         else if (a == 1) { it.col_inner = (int)nn[2]; it.outer_stride = nn[1] * nn[2]; }
         else { it.col_inner = 1; it.outer_stride = nn[2]; }
         (cheb_class(N) ? cheb1 : cheb).push_back(it);
+        if (de.kind == GH_BLOCK) { ChebItem fi = it; fi.dmat = (int)ftp; fi.axis = 0; fch[a][cheb_class(N)].push_back(fi); }
       }
+      if (de.kind == GH_BLOCK) { d->f_blocks.push_back({N, 0.0, ftp}); ftp += cheb_frag_doubles(N); }
     }
     if (de.kind == GH_SHELL) {
       d->has_shell = true;
@@ -426,6 +443,7 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
           o.T = put(T);
         }
         Lcache[L] = o;
+        d->f_L[L] = ftp; ftp += shell_g_doubles(L);
       }
       const ShellOff& o = Lcache[L];
       // coordinate tables of this shell (for the Jacobian of Eq. 8)
@@ -446,7 +464,7 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
       for (int p0 = 0; p0 < n0; p0 += pb) {
         AngItem it; memset(&it, 0, sizeof it);
         it.off = sd.off; it.L = L; it.plane0 = p0; it.nplanes = std::min(pb, n0 - p0); it.nb_alloc = pb;
-        it.m_Fa = o.Fa; it.m_Fs = o.Fs; it.m_T = o.T;
+        it.m_Fa = o.Fa; it.m_Fs = o.Fs; it.m_T = o.T; it.m_G = (int)d->f_L[L];
         {
           const int NW = (pl.ang_class[s] ? ANG_TPB1 : ANG_TPB0) / 32, MT1 = (it.nplanes * (L + 1) + 7) / 8;
           const AngDims dm = ang_dims(L);
@@ -462,7 +480,10 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
   }
   ang.insert(ang.end(), ang1.begin(), ang1.end());
   cheb.insert(cheb.end(), cheb1.begin(), cheb1.end());
-  if (tp != pl.table_doubles || (int)cheb.size() != pl.n_cheb_items || (int)ang.size() != pl.n_ang_items) {
+  std::vector<ChebItem> fcheb;
+  for (int a = 0; a < 3; ++a) for (int c = 0; c < 2; ++c) fcheb.insert(fcheb.end(), fch[a][c].begin(), fch[a][c].end());
+  if (tp != pl.table_doubles || (int)cheb.size() != pl.n_cheb_items || (int)ang.size() != pl.n_ang_items ||
+      (int)fcheb.size() != pl.n_fcheb_items || ftp != pl.table_doubles + pl.ftable_doubles) {
     delete d; return fail(nullptr, GH_ERR_STATE, "internal: plan and build disagree");
   }
 
@@ -476,12 +497,15 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
   GH_CREATE_CUDA(cudaMemcpyAsync(d->tiles, pl.tile_first.data(), (size_t)(n_sub + 1) * sizeof(int32_t), cudaMemcpyHostToDevice, st));
   GH_CREATE_CUDA(cudaMemcpyAsync(d->cheb, cheb.data(), cheb.size() * sizeof(ChebItem), cudaMemcpyHostToDevice, st));
   if (!ang.empty()) GH_CREATE_CUDA(cudaMemcpyAsync(d->ang, ang.data(), ang.size() * sizeof(AngItem), cudaMemcpyHostToDevice, st));
+  if (!fcheb.empty()) GH_CREATE_CUDA(cudaMemcpyAsync(d->fcheb, fcheb.data(), fcheb.size() * sizeof(ChebItem), cudaMemcpyHostToDevice, st));
   GH_CREATE_CUDA(cudaStreamSynchronize(st));   // host staging vectors die at return
   GH_CREATE_CUDA(cudaFuncSetAttribute(k_rhs<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RHS_SMEM_BYTES));
   GH_CREATE_CUDA(cudaFuncSetAttribute(k_rhs<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RHS_SMEM_BYTES));
   GH_CREATE_CUDA(cudaFuncSetAttribute(k_rhs<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RHS_SMEM_BYTES));
-  if (pl.n_ang_class[0]) GH_CREATE_CUDA(cudaFuncSetAttribute(k_ang<ANG_TPB0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.ang_smem[0]));
-  if (pl.n_ang_class[1]) GH_CREATE_CUDA(cudaFuncSetAttribute(k_ang<ANG_TPB1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.ang_smem[1]));
+  if (pl.n_ang_class[0]) GH_CREATE_CUDA(cudaFuncSetAttribute(k_ang<ANG_TPB0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.ang_smem[0]));
+  if (pl.n_ang_class[1]) GH_CREATE_CUDA(cudaFuncSetAttribute(k_ang<ANG_TPB1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.ang_smem[1]));
+  if (pl.n_ang_class[0]) GH_CREATE_CUDA(cudaFuncSetAttribute(k_ang<ANG_TPB0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.ang_smem[0]));
+  if (pl.n_ang_class[1]) GH_CREATE_CUDA(cudaFuncSetAttribute(k_ang<ANG_TPB1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.ang_smem[1]));
 #undef GH_CREATE_CUDA
   *out = d;
   return GH_OK;
@@ -588,9 +612,9 @@ gh_status launch_derivs(gh_domain* d, const double* in, double* out, int ncomp, 
     if (!pl.n_ang_class[cls]) continue;
     ProfScope ps(d, GH_K_SHELL_ANG);
     if (cls == 0)
-      k_ang<ANG_TPB0><<<dim3(pl.n_ang_class[0], nrun), ANG_TPB0, pl.ang_smem[0], d->stream>>>(d->ang + first, d->tables, in, out, pl.S, cm);
+      k_ang<ANG_TPB0, false><<<dim3(pl.n_ang_class[0], nrun), ANG_TPB0, pl.ang_smem[0], d->stream>>>(d->ang + first, d->tables, in, out, pl.S, cm);
     else
-      k_ang<ANG_TPB1><<<dim3(pl.n_ang_class[1], nrun), ANG_TPB1, pl.ang_smem[1], d->stream>>>(d->ang + first, d->tables, in, out, pl.S, cm);
+      k_ang<ANG_TPB1, false><<<dim3(pl.n_ang_class[1], nrun), ANG_TPB1, pl.ang_smem[1], d->stream>>>(d->ang + first, d->tables, in, out, pl.S, cm);
   }
   GH_CUDA(d, cudaGetLastError());
   return GH_OK;
@@ -749,6 +773,129 @@ extern "C" gh_status gh_constraint_norms(gh_domain* d, double* out, double* per_
 }
 
 // ------------------------------------------------------------------------------------------------------
+// spectral filter (NEXT-1): the same kernels with filter matrices in place of differentiation matrices
+// ------------------------------------------------------------------------------------------------------
+namespace {
+bool filter_sigma(const gh_filter_desc* f, int kmax, std::vector<ghb::ld>& sg) {
+  sg.assign(kmax + 1, 1);
+  if (!f || f->kind == GH_FILTER_NONE) return true;
+  if (f->kind == GH_FILTER_HEAVISIDE) {
+    if (f->cut < 0) return false;
+    for (int k = 0; k <= kmax; ++k) sg[k] = (k <= kmax - f->cut) ? 1 : 0;
+    return true;
+  }
+  if (f->kind == GH_FILTER_EXP) {
+    if (f->p < 1 || !std::isfinite(f->alpha) || f->alpha < 0) return false;
+    for (int k = 0; k <= kmax; ++k) sg[k] = kmax > 0 ? expl(-(ghb::ld)f->alpha * powl((ghb::ld)k / (ghb::ld)kmax, 2 * f->p)) : (ghb::ld)1;
+    return true;
+  }
+  return false;
+}
+}  // namespace
+
+extern "C" gh_status gh_filter_sigma(const gh_filter_desc* f, int32_t kmax, double* sigma) {
+  std::vector<ghb::ld> sg;
+  if (!sigma || kmax < 0 || !filter_sigma(f, kmax, sg)) return GH_ERR_ARG;
+  for (int k = 0; k <= kmax; ++k) sigma[k] = (double)sg[k];
+  return GH_OK;
+}
+
+extern "C" gh_status gh_set_filter(gh_domain* d, const gh_filter_desc* fb, const gh_filter_desc* fs) {
+  if (!d) return GH_ERR_ARG;
+  const Plan& pl = d->pl;
+  std::vector<double> ft(pl.ftable_doubles, 0.0);
+  const size_t base = pl.table_doubles;
+  std::vector<ghb::ld> sg, M;
+  const bool on_b = fb && fb->kind != GH_FILTER_NONE && !d->f_blocks.empty();
+  const bool on_s = fs && fs->kind != GH_FILTER_NONE && !d->f_L.empty();
+  if (on_b) {
+    std::map<int, std::vector<ghb::ld>> cache;      // N -> filter matrix
+    for (const auto& b : d->f_blocks) {
+      const int N = b.N;
+      if (!cache.count(N)) {
+        if (!filter_sigma(fb, N - 1, sg)) return fail(d, GH_ERR_ARG, "bad block filter descriptor");
+        ghb::cheb_filter_matrix(N, sg, cache[N]);
+      }
+      const std::vector<ghb::ld>& F = cache[N];
+      const int mtn = (N + 7) / 8, ksn = (N + 3) / 4;
+      for (int mt = 0; mt < mtn; ++mt) for (int ks = 0; ks < ksn; ++ks) for (int lane = 0; lane < 32; ++lane) {
+        const int row = mt * 8 + lane / 4, col = ks * 4 + lane % 4;
+        ft[b.off - base + ((size_t)mt * ksn + ks) * 32 + lane] = (row < N && col < N) ? (double)F[(size_t)row * N + col] : 0.0;
+      }
+    }
+  }
+  if (on_s) {
+    for (const auto& kv : d->f_L) {
+      const int L = kv.first, nt = L + 1, hh = (nt + 1) / 2, mtf = (hh + 7) / 8, ksh = (hh + 3) / 4;
+      if (!filter_sigma(fs, L, sg)) return fail(d, GH_ERR_ARG, "bad shell filter descriptor");
+      ghb::shell_filter_composites(L, sg, M);
+      // folded about the equator exactly like the projector rows of K_ang S2: ME = (G[r][j] + G[r][jbar]) / 2, MO = (.. - ..) / 2
+      for (int m = 0; m <= L; ++m) for (int ks = 0; ks < ksh; ++ks) for (int w = 0; w < 2; ++w) for (int mt = 0; mt < mtf; ++mt)
+        for (int lane = 0; lane < 32; ++lane) {
+          const int r = mt * 8 + lane / 4, j = ks * 4 + lane % 4;
+          ghb::ld v = 0;
+          if (j < hh && r < hh) {
+            const int jb = nt - 1 - j;
+            const ghb::ld a = M[((size_t)m * nt + r) * nt + j], c = M[((size_t)m * nt + r) * nt + jb];
+            if (jb == j) v = w == 0 ? a / 2 : (ghb::ld)0;
+            else v = (w == 0 ? a + c : a - c) / 2;
+          }
+          ft[kv.second - base + ((((size_t)m * ksh + ks) * 2 + w) * mtf + mt) * 32 + lane] = (double)v;
+        }
+    }
+  }
+  if (pl.ftable_doubles) {
+    GH_CUDA(d, cudaMemcpyAsync(d->tables + base, ft.data(), ft.size() * sizeof(double), cudaMemcpyHostToDevice, d->stream));
+    GH_CUDA(d, cudaStreamSynchronize(d->stream));
+  }
+  d->filt_blocks = on_b; d->filt_shells = on_s;
+  return GH_OK;
+}
+
+extern "C" gh_status gh_apply_filter(gh_domain* d) {
+  if (!d) return GH_ERR_ARG;
+  if (!d->has_fields) return fail(d, GH_ERR_STATE, "gh_apply_filter before gh_set_fields");
+  const Plan& pl = d->pl;
+  const CompMap cm{NCOMP, 0, 0};
+  if (d->filt_blocks) {
+    // x: ua -> T1, y: T1 -> T2, z: T2 -> ua   (T1, T2: the first two slots of the derivative scratch; only block points move)
+    int walk = 1;
+    for (int w = CHEB_COMP_WALK; w >= 1; --w)
+      if (NCOMP % w == 0 && (w == 1 || (int64_t)pl.n_fcheb_items / 3 * (NCOMP / w) >= 4 * 148)) { walk = w; break; }
+    const int gy = NCOMP / walk;
+    const double* src[3] = {d->ua, d->du, d->du + (size_t)NCOMP * pl.S};
+    double* dst[3] = {d->du, d->du + (size_t)NCOMP * pl.S, d->ua};
+    int first = 0;
+    for (int a = 0; a < 3; ++a) {
+      if (pl.n_fcheb[a][0]) {
+        ProfScope ps(d, GH_K_FILTER_CHEB);
+        k_cheb<CHEB_TPB, 4, 8, CHEB_NTW0><<<dim3(pl.n_fcheb[a][0], gy), CHEB_TPB, pl.cheb_smem, d->stream>>>(
+            d->fcheb + first, d->tables, src[a], dst[a], pl.S, NCOMP, cm);
+      }
+      first += pl.n_fcheb[a][0];
+      if (pl.n_fcheb[a][1]) {
+        ProfScope ps(d, GH_K_FILTER_CHEB);
+        k_cheb<CHEB_TPB, 8, 16, CHEB_NTW1><<<dim3(pl.n_fcheb[a][1], gy), CHEB_TPB, pl.cheb_smem, d->stream>>>(
+            d->fcheb + first, d->tables, src[a], dst[a], pl.S, NCOMP, cm);
+      }
+      first += pl.n_fcheb[a][1];
+    }
+  }
+  if (d->filt_shells) {
+    for (int cls = 0, first = 0; cls < 2; first += pl.n_ang_class[cls], ++cls) {
+      if (!pl.n_ang_class[cls]) continue;
+      ProfScope ps(d, GH_K_FILTER_ANG);
+      if (cls == 0)
+        k_ang<ANG_TPB0, true><<<dim3(pl.n_ang_class[0], NCOMP), ANG_TPB0, pl.ang_smem[0], d->stream>>>(d->ang + first, d->tables, d->ua, d->ua, pl.S, cm);
+      else
+        k_ang<ANG_TPB1, true><<<dim3(pl.n_ang_class[1], NCOMP), ANG_TPB1, pl.ang_smem[1], d->stream>>>(d->ang + first, d->tables, d->ua, d->ua, pl.S, cm);
+    }
+  }
+  GH_CUDA(d, cudaGetLastError());
+  return GH_OK;
+}
+
+// ------------------------------------------------------------------------------------------------------
 // profiling / bookkeeping
 // ------------------------------------------------------------------------------------------------------
 extern "C" gh_status gh_set_profiling(gh_domain* d, int enabled) {
@@ -773,7 +920,7 @@ extern "C" gh_status gh_profile_reset(gh_domain* d) {
 }
 
 extern "C" const char* gh_kernel_name(int k) {
-  static const char* names[GH_NUM_KERNELS] = {"k_cheb", "k_ang", "k_rhs", "k_rk", "k_con", "k_con_reduce", "k_jac", "other"};
+  static const char* names[GH_NUM_KERNELS] = {"k_cheb", "k_ang", "k_rhs", "k_rk", "k_con", "k_con_reduce", "k_jac", "other", "k_cheb(filter)", "k_ang(filter)"};
   return (k >= 0 && k < GH_NUM_KERNELS) ? names[k] : "?";
 }
 

@@ -218,7 +218,8 @@ __device__ __forceinline__ void ang_s1_unit(const double* __restrict__ ap, const
 
 // S3 unit: one m-tile x NTC n-tiles (columns k = 0..h), both parts (theta from Y, phi from X), even and odd GEMMs;
 // a0p / a1p: this lane's rows (+ tl) of Y / X at the cos region; the sin region starts kc doubles further.
-template <int NTC>
+// PARTS = 1 (spectral filter): only the Y part, stored to g0.
+template <int NTC, int PARTS>
 __device__ __forceinline__ void ang_s3_unit(const double* __restrict__ a0p, const double* __restrict__ a1p, int kc,
                                             const double* __restrict__ bpe, const double* __restrict__ bpo, int KSe,
                                             int KSo, int NT, double* __restrict__ g0, double* __restrict__ g1, int c0,
@@ -234,12 +235,12 @@ __device__ __forceinline__ void ang_s3_unit(const double* __restrict__ a0p, cons
     const double* p0 = a0p; const double* p1 = a1p;
 #pragma unroll 2
     for (int ks = 0; ks < KSe; ++ks) {
-      const double a0 = p0[0], a1 = p1[0];
+      const double a0 = p0[0], a1 = PARTS == 2 ? p1[0] : 0.0;
 #pragma unroll
       for (int n = 0; n < NTC; ++n) {
         const double b = bpe[n * 32];
         dmma884(e0[n][0], e0[n][1], a0, b);
-        dmma884(e1[n][0], e1[n][1], a1, b);
+        if (PARTS == 2) dmma884(e1[n][0], e1[n][1], a1, b);
       }
       p0 += 4; p1 += 4; bpe += bstep;
     }
@@ -248,12 +249,12 @@ __device__ __forceinline__ void ang_s3_unit(const double* __restrict__ a0p, cons
     const double* p0 = a0p + kc; const double* p1 = a1p + kc;
 #pragma unroll 2
     for (int ks = 0; ks < KSo; ++ks) {
-      const double a0 = p0[0], a1 = p1[0];
+      const double a0 = p0[0], a1 = PARTS == 2 ? p1[0] : 0.0;
 #pragma unroll
       for (int n = 0; n < NTC; ++n) {
         const double b = bpo[n * 32];
         dmma884(o0[n][0], o0[n][1], a0, b);
-        dmma884(o1[n][0], o1[n][1], a1, b);
+        if (PARTS == 2) dmma884(o1[n][0], o1[n][1], a1, b);
       }
       p0 += 4; p1 += 4; bpo += bstep;
     }
@@ -264,14 +265,14 @@ __device__ __forceinline__ void ang_s3_unit(const double* __restrict__ a0p, cons
       const int k = c0 + n * 8;             // even; this lane holds columns k and k + 1
       if (k + 1 <= h) {
         *reinterpret_cast<double2*>(g0 + k) = make_double2(e0[n][0] + o0[n][0], e0[n][1] + o0[n][1]);
-        *reinterpret_cast<double2*>(g1 + k) = make_double2(e1[n][0] + o1[n][0], e1[n][1] + o1[n][1]);
+        if (PARTS == 2) *reinterpret_cast<double2*>(g1 + k) = make_double2(e1[n][0] + o1[n][0], e1[n][1] + o1[n][1]);
       } else if (k <= h) {
         g0[k] = e0[n][0] + o0[n][0];
-        g1[k] = e1[n][0] + o1[n][0];
+        if (PARTS == 2) g1[k] = e1[n][0] + o1[n][0];
       }
       // mirror columns n_phi - k (k = 1..L)
-      if (k >= 1 && k < h) { g0[np - k] = e0[n][0] - o0[n][0]; g1[np - k] = e1[n][0] - o1[n][0]; }
-      if (k + 1 < h) { g0[np - k - 1] = e0[n][1] - o0[n][1]; g1[np - k - 1] = e1[n][1] - o1[n][1]; }
+      if (k >= 1 && k < h) { g0[np - k] = e0[n][0] - o0[n][0]; if (PARTS == 2) g1[np - k] = e1[n][0] - o1[n][0]; }
+      if (k + 1 < h) { g0[np - k - 1] = e0[n][1] - o0[n][1]; if (PARTS == 2) g1[np - k - 1] = e1[n][1] - o1[n][1]; }
     }
   }
 }
@@ -282,7 +283,9 @@ __device__ __forceinline__ void ang_s3_unit(const double* __restrict__ a0p, cons
 //   [alpha ; gamma] = ME_m p,  [beta ; delta] = MO_m q      (two stacked (2 hh x hh) matrices instead of one (2 nt x nt))
 //   A_j = alpha + beta, A_jbar = beta - alpha;   B_j = gamma + delta, B_jbar = gamma - delta:      half the flop of S2.
 // MTH m-tiles of each stacked matrix; fragments [ks][which][mt][32] stream from L2 one k-step ahead.
-template <int MTH>
+// FILTER: the stacked matrix is only the filtered projector G_m (hh rows, commutes with the reflection like Pr_m): the
+// filtered coefficients gamma +- delta replace C in Y; X is not written.
+template <int MTH, bool FILTER>
 __device__ __forceinline__ void ang_s2_unit(const double* __restrict__ tp /* T_m fragments + lane */, int KSh,
                                             double* __restrict__ X, double* __restrict__ Y, int m, int ntile, int nb,
                                             int L, int kc, int pitch, int ps, int g, int tl) {
@@ -342,9 +345,9 @@ __device__ __forceinline__ void ang_s2_unit(const double* __restrict__ tp /* T_m
       for (int e = 0; e < 2; ++e)
         if (cok[e]) {
           ydst[e][rr * pitch] = ap_[mt][e] + aq_[mt][e];
-          if (jb != rr) ydst[e][jb * pitch] = aq_[mt][e] - ap_[mt][e];
+          if (jb != rr) ydst[e][jb * pitch] = FILTER ? ap_[mt][e] - aq_[mt][e] : aq_[mt][e] - ap_[mt][e];
         }
-    } else if (rr < 2 * hh) {
+    } else if (!FILTER && rr < 2 * hh) {
       const int j = rr - hh, jb = nt - 1 - j;
 #pragma unroll
       for (int e = 0; e < 2; ++e)
@@ -374,10 +377,10 @@ __device__ __forceinline__ void ang_s2_unit(const double* __restrict__ tp /* T_m
 constexpr int ANG_NTC = 5;    // most n-tiles per warp unit in S1
 constexpr int ANG_NTC3 = 3;   // most n-tiles per warp unit in S3 (four accumulator sets)
 
-template <int TPB>
+template <int TPB, bool FILTER>
 __global__ void __launch_bounds__(TPB, TPB <= 256 ? 2 : 1)
-k_ang(const AngItem* __restrict__ items, const double* __restrict__ tables, const double* __restrict__ in,
-      double* __restrict__ out, int64_t S, CompMap cm) {
+k_ang(const AngItem* __restrict__ items, const double* __restrict__ tables, const double* in,
+      double* out, int64_t S, CompMap cm) {
   extern __shared__ __align__(16) double sm[];
   constexpr int NW = TPB / 32;
   const AngItem it = items[blockIdx.x];
@@ -389,9 +392,11 @@ k_ang(const AngItem* __restrict__ items, const double* __restrict__ tables, cons
   const int nb = it.nplanes, R = nb * nt;
   const int pitch = ang_pitch(L), ps = ang_plane_stride(L);
   const int64_t goff = it.off + (int64_t)it.plane0 * plane;
-  const double* __restrict__ src = in + (int64_t)comp * S + goff;
-  double* __restrict__ dth = out + ((int64_t)1 * ncomp + comp) * S + goff;
-  double* __restrict__ dph = out + ((int64_t)2 * ncomp + comp) * S + goff;
+  const double* src = in + (int64_t)comp * S + goff;
+  // derivative slots 1 (theta) and 2 (phi) of `out`; FILTER: the filtered planes, over the input when out == in (every plane
+  // of this CTA is in shared memory before the first store)
+  double* dth = FILTER ? out + (int64_t)comp * S + goff : out + ((int64_t)1 * ncomp + comp) * S + goff;
+  double* dph = out + ((int64_t)2 * ncomp + comp) * S + goff;
 
   double* X = sm;                               // [nb][ps]
   double* Y = X + (size_t)it.nb_alloc * ps;     // [nb][ps]
@@ -471,14 +476,14 @@ k_ang(const AngItem* __restrict__ items, const double* __restrict__ tables, cons
   }
   // ---- S2: per m and n-tile of its columns ----
   {
-    const int hh = (nt + 1) >> 1, MTH = (2 * hh + 7) >> 3, KSh = (hh + 3) >> 2;
+    const int hh = (nt + 1) >> 1, MTH = ((FILTER ? hh : 2 * hh) + 7) >> 3, KSh = (hh + 3) >> 2;
     const int NTn = (2 * nb + 7) >> 3;
-    const double* __restrict__ T = tables + it.m_T + lane;
+    const double* __restrict__ T = tables + (FILTER ? it.m_G : it.m_T) + lane;
     for (int u = warp; u < (L + 1) * NTn; u += NW) {
       const int m = u / NTn, ntile = u - m * NTn;
       if (m == 0 && ntile * 8 >= nb) continue;
       const double* tp = T + (size_t)m * KSh * 2 * MTH * 32;
-#define GH_S2(K) ang_s2_unit<K>(tp, KSh, X, Y, m, ntile, nb, L, kc, pitch, ps, g, tl)
+#define GH_S2(K) ang_s2_unit<K, FILTER>(tp, KSh, X, Y, m, ntile, nb, L, kc, pitch, ps, g, tl)
       switch (MTH) {
         case 1: GH_S2(1); break;
         case 2: GH_S2(2); break;
@@ -512,7 +517,7 @@ k_ang(const AngItem* __restrict__ items, const double* __restrict__ tables, cons
       const int c0 = n0 * 8 + 2 * tl;
       double* g0 = dth + (size_t)r * np;
       double* g1 = dph + (size_t)r * np;
-#define GH_CALL(K) ang_s3_unit<K>(a0p, a1p, kcr, bpe, bpo, D.KSe3, D.KSo3, D.NT3, g0, g1, c0, h, np, rok)
+#define GH_CALL(K) ang_s3_unit<K, FILTER ? 1 : 2>(a0p, a1p, kcr, bpe, bpo, D.KSe3, D.KSo3, D.NT3, g0, g1, c0, h, np, rok)
       GH_NTC3_SWITCH(nn, GH_CALL)
 #undef GH_CALL
     }

@@ -19,7 +19,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libgh.so")
 
 GH_NCOMP = 50
-GH_NUM_KERNELS = 8
+GH_NUM_KERNELS = 10
+GH_FILTER_NONE, GH_FILTER_HEAVISIDE, GH_FILTER_EXP = range(3)
 GH_OK, GH_ERR_ARG, GH_ERR_WORKSPACE, GH_ERR_CUDA, GH_ERR_STATE, GH_ERR_SINGULAR = range(6)
 STATUS_NAMES = ["GH_OK", "GH_ERR_ARG", "GH_ERR_WORKSPACE", "GH_ERR_CUDA", "GH_ERR_STATE", "GH_ERR_SINGULAR"]
 
@@ -29,6 +30,7 @@ EXPORTS = [
     "gh_set_fields", "gh_get_fields", "gh_set_gauge_source", "gh_rhs", "gh_gradient", "gh_rk_step",
     "gh_constraint_norms", "gh_set_profiling", "gh_profile_read", "gh_profile_reset", "gh_kernel_name",
     "gh_launch_count", "gh_last_error", "gh_basis_cheb", "gh_basis_gauss_legendre", "gh_basis_shell",
+    "gh_set_filter", "gh_apply_filter", "gh_filter_sigma",
 ]
 
 
@@ -36,6 +38,23 @@ class GHError(RuntimeError):
     def __init__(self, status: int, message: str):
         super().__init__(f"{STATUS_NAMES[status] if 0 <= status < 6 else status}: {message}")
         self.status = status
+
+
+class gh_filter_desc(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("cut", C.c_int32), ("alpha", C.c_double), ("p", C.c_int32), ("pad_", C.c_int32)]
+
+
+def make_filter(f):
+    """None | {'kind': 'heaviside', 'cut': n} | {'kind': 'exp', 'alpha': a, 'p': p} -> gh_filter_desc or None."""
+    if f is None:
+        return None
+    d = gh_filter_desc()
+    kind = f.get("kind", "none")
+    d.kind = {"none": GH_FILTER_NONE, "heaviside": GH_FILTER_HEAVISIDE, "exp": GH_FILTER_EXP}[kind]
+    d.cut = int(f.get("cut", 0))
+    d.alpha = float(f.get("alpha", 0.0))
+    d.p = int(f.get("p", 1))
+    return d
 
 
 class gh_subdomain_desc(C.Structure):
@@ -90,6 +109,10 @@ def lib() -> C.CDLL:
     L.gh_basis_cheb.argtypes = [C.c_int32, dp, dp]
     L.gh_basis_gauss_legendre.argtypes = [C.c_int32, dp, dp]
     L.gh_basis_shell.argtypes = [C.c_int32, dp, dp, dp, dp]
+    fp = C.POINTER(gh_filter_desc)
+    L.gh_set_filter.argtypes = [vp, fp, fp]
+    L.gh_apply_filter.argtypes = [vp]
+    L.gh_filter_sigma.argtypes = [fp, C.c_int32, dp]
     _lib = L
     return L
 
@@ -209,6 +232,24 @@ def gh_constraint_norms(h, n_sub: int, per_sub: bool = False):
     return (out, ps) if per_sub else out
 
 
+def gh_set_filter(h, block_axes=None, shell_angular=None):
+    fb, fs = make_filter(block_axes), make_filter(shell_angular)
+    _check(lib().gh_set_filter(h, C.byref(fb) if fb is not None else None, C.byref(fs) if fs is not None else None), h)
+
+
+def gh_apply_filter(h):
+    _check(lib().gh_apply_filter(h), h)
+
+
+def gh_filter_sigma(f, kmax: int) -> np.ndarray:
+    d = make_filter(f)
+    out = np.empty(kmax + 1)
+    st = lib().gh_filter_sigma(C.byref(d), int(kmax), out.ctypes.data)
+    if st != GH_OK:
+        raise GHError(st, "gh_filter_sigma: bad descriptor")
+    return out
+
+
 def gh_basis_cheb(N: int):
     x, D = np.zeros(N), np.zeros((N, N))
     _check(lib().gh_basis_cheb(N, x.ctypes.data, D.ctypes.data), None)
@@ -313,6 +354,12 @@ class Domain:
 
     def constraint_norms(self, per_sub: bool = False):
         return gh_constraint_norms(self.h, self.n_sub, per_sub)
+
+    def set_filter(self, block_axes=None, shell_angular=None):
+        gh_set_filter(self.h, block_axes, shell_angular)
+
+    def apply_filter(self):
+        gh_apply_filter(self.h)
 
     def set_profiling(self, on: bool):
         _check(lib().gh_set_profiling(self.h, int(on)), self.h)

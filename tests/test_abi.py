@@ -123,3 +123,14 @@ def test_shell_matrices_realise_the_ylm_derivatives(L, oracle):
     assert np.allclose(Pr[0], np.eye(nt), atol=1e-13)      # m = 0: all l <= L resolved by L+1 nodes
     for m in range(L + 1):
         assert np.linalg.matrix_rank(Pr[m], tol=1e-9) == L + 1 - m
+
+
+def test_filter_sigma_reading_s20():
+    """gh_filter_sigma against the formulas stated in include/gh.h (reading S20), retyped here."""
+    s = gh.gh_filter_sigma({"kind": "heaviside", "cut": 3}, 9)
+    assert np.array_equal(s, (np.arange(10) <= 6).astype(float))
+    s = gh.gh_filter_sigma({"kind": "exp", "alpha": 36.0, "p": 4}, 12)
+    assert np.allclose(s, np.exp(-36.0 * (np.arange(13) / 12.0) ** 8), rtol=1e-13, atol=0)   # long double there, double here
+    assert np.array_equal(gh.gh_filter_sigma({"kind": "none"}, 5), np.ones(6))
+    with pytest.raises(gh.GHError):
+        gh.gh_filter_sigma({"kind": "exp", "alpha": 1.0, "p": 0}, 5)

@@ -185,3 +185,44 @@ def test_c3_evolution_parity_100_steps(oracle):
     """The full C3 run: 100 RK3 steps, every shell, compared after steps 1, 10 and 100."""
     worst = _c3_run(oracle, shells=list(range(8)), checkpoints=[1, 10, 100])
     print(f"C3 100 steps: worst |gpu - oracle| / ||X||inf = {worst:.3e}")
+
+
+# ---- NEXT-1: spectral filter ------------------------------------------------------------------------------------------
+FILTERS = [({"kind": "exp", "alpha": 36.0, "p": 6}, {"kind": "exp", "alpha": 36.0, "p": 6}),
+           ({"kind": "heaviside", "cut": 2}, {"kind": "heaviside", "cut": 2})]
+
+
+@pytest.mark.parametrize("fidx", [0, 1])
+def test_filter_parity(case, oracle, fidx):
+    """gh_apply_filter against the oracle's modal filter (O9) on the same state; the filter function is evaluated on each side
+    from the formulas of reading S20 (here in numpy, there in gh_filter_sigma)."""
+    name, cfg, descs, coords, us, Hs, dom = case
+    fb, fs = FILTERS[fidx]
+
+    def sigma(f, kmax):
+        k = np.arange(kmax + 1)
+        if f["kind"] == "heaviside":
+            return (k <= kmax - f["cut"]).astype(float)
+        return np.exp(-f["alpha"] * (k / kmax) ** (2 * f["p"]))
+
+    dom.set_fields(dom.pack(us), 0.0)
+    dom.set_filter(block_axes=fb, shell_angular=fs)
+    dom.apply_filter()
+    got = dom.unpack(dom.get_fields())
+    for s, d in enumerate(descs):
+        if d["kind"] == "shell":
+            ref = oracle.spectral_filter(d, us[s], [sigma(fs, d["n"][1])])
+        else:
+            ref = oracle.spectral_filter(d, us[s], [sigma(fb, n - 1) for n in d["n"]])
+        assert_parity(got[s], ref, tol=TOL, what=f"{name} sub {s} filter {fidx}")
+        assert np.max(np.abs(ref - us[s])) > 0          # the filter did something to the perturbed state
+    # switching a family off leaves it untouched, bit for bit
+    dom.set_fields(dom.pack(us), 0.0)
+    dom.set_filter(block_axes=None, shell_angular=fs)
+    dom.apply_filter()
+    got = dom.unpack(dom.get_fields())
+    for s, d in enumerate(descs):
+        if d["kind"] == "block":
+            assert np.array_equal(got[s], us[s])
+    dom.set_filter(None, None)
+    dom.set_fields(dom.pack(us), 0.0)
