@@ -378,6 +378,8 @@ def run_ours(args):
     if not bool(torch.isfinite(out_host).all()):
         raise SystemExit("bench.py: non-finite state after the e2e region")
 
+    filt = time_filter(dom, u_dev, descs) if rank == 0 else None
+
     tmax, e2emax = max_over_ranks([ms, e2e_s / e2e_steps], dist, dev)
     if rank != 0:
         dom.close()
@@ -385,11 +387,42 @@ def run_ours(args):
             dist.barrier(); dist.destroy_process_group()
         return
     return finish_ours(args, world, label, cfg, descs, reps, P, S, tmax, e2emax, e2e_steps, launches, prof, work, clocks,
-                       norms, base, dom, dist)
+                       norms, base, dom, dist, filt)
+
+
+def time_filter(dom, u_dev, descs, reps: int = 5):
+    """NEXT-1 (outside the timed step): gh_apply_filter with the exponential filter on every block axis and in l on every
+    shell; per-kernel device time from the library's CUDA events, mean of `reps` calls after 2 warm-ups."""
+    from paper_1804_09101_b200 import configs
+
+    f = {"kind": "exp", "alpha": 36.0, "p": 32}
+    dom.set_filter(block_axes=f, shell_angular=f)
+    dom.set_fields(u_dev, 0.0)
+    for _ in range(2):
+        dom.apply_filter()
+    dom.set_profiling(True)
+    dom.profile_reset()
+    for _ in range(reps):
+        dom.apply_filter()
+    prof = dom.profile_read()
+    dom.set_profiling(False)
+    dom.set_filter(None, None)
+    Ps = sum(configs.num_points(d) for d in descs if d["kind"] == "shell")
+    Pb = sum(configs.num_points(d) for d in descs if d["kind"] == "block")
+    ms_c = prof["k_cheb(filter)"][0] / reps
+    ms_a = prof["k_ang(filter)"][0] / reps
+    out = {"filter": "exp(-36 (k/kmax)^64) on the 3 Chebyshev axes of every block and in l on every shell", "ms_per_call": ms_c + ms_a}
+    if ms_c > 0:   # three passes, each reads and writes the 50 block components once
+        out["k_cheb(filter)"] = {"ms_per_call": ms_c, "achieved_GBps": 3 * 2 * 50 * 8.0 * Pb / (ms_c * 1e-3) / 1e9, "bound": "hbm"}
+    if ms_a > 0:   # analysis + filtered projector + one synthesis: about 5 (2L+1) flop per point and component unfolded
+        fl = sum(50.0 * configs.num_points(d) * 5 * (2 * d["n"][1] + 1) for d in descs if d["kind"] == "shell")
+        out["k_ang(filter)"] = {"ms_per_call": ms_a, "achieved_GBps": 2 * 50 * 8.0 * Ps / (ms_a * 1e-3) / 1e9,
+                                "achieved_TFLOPs": fl / (ms_a * 1e-3) / 1e12, "bound": "alu"}
+    return out
 
 
 def finish_ours(args, world, label, cfg, descs, reps, P, S, ms, e2e_step_s, e2e_steps, launches, prof, work, clocks,
-                norms, base, dom, dist):
+                norms, base, dom, dist, filt=None):
     hbm_peak, peak_src = load_peaks()
     steps = args.steps
     value = whole_job_value(world, P, steps, ms)
@@ -399,7 +432,7 @@ def finish_ours(args, world, label, cfg, descs, reps, P, S, ms, e2e_step_s, e2e_
     calls_per_step = {"k_rhs": 3, "k_con": 1, "k_cheb": 3.8, "k_ang": 3.8}   # library calls that run the kernel
     kernels = {}
     for name, (kms, cnt) in prof.items():
-        if cnt == 0:
+        if cnt == 0 or "filter" in name:
             continue
         e = {"launches_per_step": cnt / steps, "ms_per_launch": kms / cnt, "ms_per_step": kms / steps,
              "share_of_kernel_time": kms / total_kernel_ms}
@@ -461,6 +494,7 @@ def finish_ours(args, world, label, cfg, descs, reps, P, S, ms, e2e_step_s, e2e_
                 "path": "gh_set_fields(HOST pinned) + gh_rk_step + gh_constraint_norms + gh_get_fields(HOST pinned)"},
         "clocks": clocks,
         "constraint_norms_after": [[float(x) for x in r] for r in np.asarray(norms)],
+        "spectral_filter": filt,
     }
     print(json.dumps(out))
     sys.stdout.flush()
