@@ -285,8 +285,12 @@ __device__ __forceinline__ void ang_s3_unit(const double* __restrict__ a0p, cons
 // MTH m-tiles of each stacked matrix; fragments [ks][which][mt][32] stream from L2 one k-step ahead.
 // FILTER: the stacked matrix is only the filtered projector G_m (hh rows, commutes with the reflection like Pr_m): the
 // filtered coefficients gamma +- delta replace C in Y; X is not written.
+// np_ / nq_: the fragments of this unit's first k-step, already loaded; on return they hold those of the NEXT unit's first
+// k-step (tnext, or untouched if tnext == nullptr), fetched during this unit's last k-step so that the L2 latency hides
+// behind its DMMAs and epilogue: the units are only 3-5 k-steps long.
 template <int MTH, bool FILTER>
-__device__ __forceinline__ void ang_s2_unit(const double* __restrict__ tp /* T_m fragments + lane */, int KSh,
+__device__ __forceinline__ void ang_s2_unit(const double* __restrict__ tp /* T_m fragments + lane */,
+                                            const double* __restrict__ tnext, double (&np_)[MTH], double (&nq_)[MTH], int KSh,
                                             double* __restrict__ X, double* __restrict__ Y, int m, int ntile, int nb,
                                             int L, int kc, int pitch, int ps, int g, int tl) {
   const int nt = L + 1, hh = (nt + 1) >> 1, ncols = (m == 0) ? nb : 2 * nb;
@@ -299,18 +303,16 @@ __device__ __forceinline__ void ang_s2_unit(const double* __restrict__ tp /* T_m
   double ap_[MTH][2], aq_[MTH][2];
 #pragma unroll
   for (int mt = 0; mt < MTH; ++mt) ap_[mt][0] = ap_[mt][1] = aq_[mt][0] = aq_[mt][1] = 0.0;
-  double np_[MTH], nq_[MTH];      // next k-step's A fragments
-#pragma unroll
-  for (int mt = 0; mt < MTH; ++mt) { np_[mt] = __ldg(tp + mt * 32); nq_[mt] = __ldg(tp + (MTH + mt) * 32); }
 #pragma unroll 1
   for (int ks = 0; ks < KSh; ++ks) {
     double fp[MTH], fq[MTH];
 #pragma unroll
     for (int mt = 0; mt < MTH; ++mt) { fp[mt] = np_[mt]; fq[mt] = nq_[mt]; }
     tp += 2 * MTH * 32;
-    if (ks + 1 < KSh) {
+    const double* __restrict__ tn = (ks + 1 < KSh) ? tp : tnext;
+    if (tn) {
 #pragma unroll
-      for (int mt = 0; mt < MTH; ++mt) { np_[mt] = __ldg(tp + mt * 32); nq_[mt] = __ldg(tp + (MTH + mt) * 32); }
+      for (int mt = 0; mt < MTH; ++mt) { np_[mt] = __ldg(tn + mt * 32); nq_[mt] = __ldg(tn + (MTH + mt) * 32); }
     }
     const int j = ks * 4 + tl;
     const bool jok = bok && j < hh;
@@ -356,6 +358,33 @@ __device__ __forceinline__ void ang_s2_unit(const double* __restrict__ tp /* T_m
           if (jb != j) xdst[e][jb * pitch] = sgn[e] * (ap_[mt][e] - aq_[mt][e]);
         }
     }
+  }
+}
+
+// all S2 units of one warp: u = warp, warp + NW, ... over (m, n-tile)
+template <int MTH, bool FILTER>
+__device__ __forceinline__ void ang_s2_loop(const double* __restrict__ T /* + lane */, int KSh, double* __restrict__ X,
+                                            double* __restrict__ Y, int nb, int L, int kc, int pitch, int ps, int g, int tl,
+                                            int warp, int NW) {
+  const int NTn = (2 * nb + 7) >> 3, nunits = (L + 1) * NTn;
+  const size_t mstride = (size_t)KSh * 2 * MTH * 32;
+  auto skip = [&](int u) { return u < NTn && u * 8 >= nb; };       // m = 0 has only the nb cos columns
+  int u = warp;
+  while (u < nunits && skip(u)) u += NW;
+  if (u >= nunits) return;
+  double np_[MTH], nq_[MTH];
+  {
+    const double* __restrict__ tp = T + (size_t)(u / NTn) * mstride;
+#pragma unroll
+    for (int mt = 0; mt < MTH; ++mt) { np_[mt] = __ldg(tp + mt * 32); nq_[mt] = __ldg(tp + (MTH + mt) * 32); }
+  }
+  while (u < nunits) {
+    int un = u + NW;
+    while (un < nunits && skip(un)) un += NW;
+    const int m = u / NTn, ntile = u - m * NTn;
+    const double* tnext = un < nunits ? T + (size_t)(un / NTn) * mstride : nullptr;
+    ang_s2_unit<MTH, FILTER>(T + (size_t)m * mstride, tnext, np_, nq_, KSh, X, Y, m, ntile, nb, L, kc, pitch, ps, g, tl);
+    u = un;
   }
 }
 
@@ -477,23 +506,17 @@ k_ang(const AngItem* __restrict__ items, const double* __restrict__ tables, cons
   // ---- S2: per m and n-tile of its columns ----
   {
     const int hh = (nt + 1) >> 1, MTH = ((FILTER ? hh : 2 * hh) + 7) >> 3, KSh = (hh + 3) >> 2;
-    const int NTn = (2 * nb + 7) >> 3;
     const double* __restrict__ T = tables + (FILTER ? it.m_G : it.m_T) + lane;
-    for (int u = warp; u < (L + 1) * NTn; u += NW) {
-      const int m = u / NTn, ntile = u - m * NTn;
-      if (m == 0 && ntile * 8 >= nb) continue;
-      const double* tp = T + (size_t)m * KSh * 2 * MTH * 32;
-#define GH_S2(K) ang_s2_unit<K, FILTER>(tp, KSh, X, Y, m, ntile, nb, L, kc, pitch, ps, g, tl)
-      switch (MTH) {
-        case 1: GH_S2(1); break;
-        case 2: GH_S2(2); break;
-        case 3: GH_S2(3); break;
-        case 4: GH_S2(4); break;
-        case 5: GH_S2(5); break;
-        default: GH_S2(6); break;
-      }
-#undef GH_S2
+#define GH_S2(K) ang_s2_loop<K, FILTER>(T, KSh, X, Y, nb, L, kc, pitch, ps, g, tl, warp, NW)
+    switch (MTH) {
+      case 1: GH_S2(1); break;
+      case 2: GH_S2(2); break;
+      case 3: GH_S2(3); break;
+      case 4: GH_S2(4); break;
+      case 5: GH_S2(5); break;
+      default: GH_S2(6); break;
     }
+#undef GH_S2
   }
   cp_async_wait<0>();
   __syncthreads();
