@@ -618,6 +618,85 @@ static int frozen(const ora_subdomain* sd, int64_t p) {
          (j == n1 - 1 && sd->face[3] == 1) || (k == 0 && sd->face[4] == 1) || (k == n2 - 1 && sd->face[5] == 1);
 }
 
+/* ---------------------------------------------------------------------- */
+/* O10 — characteristic boundary condition, "freeze what comes in"        */
+/* (NEXT-2 (i); the paper's ApplyBCs module,  */
+/* which it left on the CPU).  The paper gives no formulas; these are the */
+/* characteristic fields of the first-order GH system of ref. [34]'s      */
+/* lineage (reading S21).  At a face point with outward unit    */
+/* normal n_i = s_i / sqrt(g^{jk} s_j s_k), n^i = g^{ij} n_j:             */
+/*   u0_ab   = psi_ab                              speed -(1+g1) n_k N^k  */
+/*   u1+-_ab = Pi_ab +- n^i Phi_iab - g2 psi_ab     speed -n_k N^k +- N    */
+/*   u2_iab  = (delta_i^k - n_i n^k) Phi_kab        speed -n_k N^k         */
+/* The time derivative of every field whose speed is negative (it enters  */
+/* the domain) is set to zero, the others keep the value the evolution    */
+/* equations give; then back:  dt psi = dt u0,                            */
+/*   dt Pi = (dt u1+ + dt u1-)/2 + g2 dt u0,                              */
+/*   dt Phi_i = (dt u1+ - dt u1-)/2 n_i + dt u2_i.                        */
+/* ---------------------------------------------------------------------- */
+static int char_bc_point(const real psi[4][4], const real gam[3], const real s[3], real dtpsi[4][4], real dtPi[4][4],
+                         real dtPhi[3][4][4]) {
+  geom G; if (geometry(psi, &G)) return 1;
+  real nn = 0; for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) nn += G.ginv[i][j] * s[i] * s[j];
+  nn = R_SQRT(nn);
+  real nd[3], nu[3], nN = 0;
+  for (int i = 0; i < 3; ++i) nd[i] = s[i] / nn;
+  for (int i = 0; i < 3; ++i) { nu[i] = 0; for (int j = 0; j < 3; ++j) nu[i] += G.ginv[i][j] * nd[j]; }
+  for (int k = 0; k < 3; ++k) nN += nd[k] * G.shift[k];
+  real v0 = -(1 + gam[1]) * nN, v1p = -nN + G.lapse, v1m = -nN - G.lapse, v2 = -nN;
+  for (int a = 0; a < 4; ++a) for (int b = 0; b < 4; ++b) {
+    real dpsi = dtpsi[a][b], dPi = dtPi[a][b], dPhi[3] = {dtPhi[0][a][b], dtPhi[1][a][b], dtPhi[2][a][b]};
+    real nPhi = 0; for (int i = 0; i < 3; ++i) nPhi += nu[i] * dPhi[i];
+    real u0 = dpsi, u1p = dPi + nPhi - gam[2] * dpsi, u1m = dPi - nPhi - gam[2] * dpsi, u2[3];
+    for (int i = 0; i < 3; ++i) u2[i] = dPhi[i] - nd[i] * nPhi;
+    if (v0 < 0) u0 = 0;
+    if (v1p < 0) u1p = 0;
+    if (v1m < 0) u1m = 0;
+    if (v2 < 0) { u2[0] = u2[1] = u2[2] = 0; }
+    dtpsi[a][b] = u0;
+    dtPi[a][b] = (u1p + u1m) / 2 + gam[2] * u0;
+    for (int i = 0; i < 3; ++i) dtPhi[i][a][b] = (u1p - u1m) / 2 * nd[i] + u2[i];
+  }
+  return 0;
+}
+
+/* for the pins: psi[16], gamma[3], s[3] (outward direction, any length); dtpsi[16], dtPi[16], dtPhi[48] in place;
+ * speeds[4] = v0, v1+, v1-, v2 (may be NULL). */
+int ora_char_bc_point(const double* psi, const double* gamma, const double* s, double* dtpsi, double* dtPi, double* dtPhi, double* speeds) {
+  real p[4][4], a[4][4], b[4][4], c[3][4][4], g3[3] = {gamma[0], gamma[1], gamma[2]}, s3[3] = {s[0], s[1], s[2]};
+  for (int x = 0; x < 4; ++x) for (int y = 0; y < 4; ++y) { p[x][y] = psi[4 * x + y]; a[x][y] = dtpsi[4 * x + y]; b[x][y] = dtPi[4 * x + y];
+    for (int i = 0; i < 3; ++i) c[i][x][y] = dtPhi[16 * i + 4 * x + y]; }
+  if (char_bc_point(p, g3, s3, a, b, c)) return 1;
+  for (int x = 0; x < 4; ++x) for (int y = 0; y < 4; ++y) { dtpsi[4 * x + y] = (double)a[x][y]; dtPi[4 * x + y] = (double)b[x][y];
+    for (int i = 0; i < 3; ++i) dtPhi[16 * i + 4 * x + y] = (double)c[i][x][y]; }
+  if (speeds) {
+    geom G; geometry(p, &G);
+    real nn = 0; for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) nn += G.ginv[i][j] * s3[i] * s3[j];
+    real nN = 0; for (int k = 0; k < 3; ++k) nN += s3[k] / R_SQRT(nn) * G.shift[k];
+    speeds[0] = (double)(-(1 + g3[1]) * nN); speeds[1] = (double)(-nN + G.lapse); speeds[2] = (double)(-nN - G.lapse); speeds[3] = (double)(-nN);
+  }
+  return 0;
+}
+
+/* outward directions s_i of the faces flagged CHARACTERISTIC (= 2) that contain point p, in face order; returns how many */
+static int char_faces(const ora_subdomain* sd, int64_t p, const real* xyz3 /* x,y,z of the point relative to the shell centre */, real s[6][3]) {
+  int n0, n1, n2; dims(sd, &n0, &n1, &n2);
+  int k = (int)(p % n2), j = (int)((p / n2) % n1), i = (int)(p / ((int64_t)n1 * n2));
+  int n = 0;
+  if (sd->kind == 0) {
+    real r = R_SQRT(xyz3[0] * xyz3[0] + xyz3[1] * xyz3[1] + xyz3[2] * xyz3[2]);
+    if (i == 0 && sd->face[0] == 2) { for (int q = 0; q < 3; ++q) s[n][q] = -xyz3[q] / r; ++n; }
+    if (i == n0 - 1 && sd->face[1] == 2) { for (int q = 0; q < 3; ++q) s[n][q] = xyz3[q] / r; ++n; }
+    return n;
+  }
+  int idx[3] = {i, j, k}, ext[3] = {n0, n1, n2};
+  for (int a = 0; a < 3; ++a) {
+    if (idx[a] == 0 && sd->face[2 * a] == 2) { s[n][0] = s[n][1] = s[n][2] = 0; s[n][a] = -1; ++n; }
+    if (idx[a] == ext[a] - 1 && sd->face[2 * a + 1] == 2) { s[n][0] = s[n][1] = s[n][2] = 0; s[n][a] = 1; ++n; }
+  }
+  return n;
+}
+
 /* real-typed core: u[50][P], H[4][P], gH[12][P] ([i][a]) -> dtu[50][P]. Returns #non-physical points. */
 static int rhs_real(const ora_subdomain* sd, const real* u, const real* H, const real* gH, real* dtu) {
   int64_t P = ora_num_points(sd);
@@ -625,19 +704,25 @@ static int rhs_real(const ora_subdomain* sd, const real* u, const real* H, const
   gradient_real(sd, 50, u, g);
   real gam[3] = {sd->gamma[0], sd->gamma[1], sd->gamma[2]};
   int bad = 0;
+  double* xyz = malloc(sizeof(double) * 3 * P); ora_coords(sd, xyz);
 #pragma omp parallel for schedule(static) reduction(+ : bad)
   for (int64_t p = 0; p < P; ++p) {
     point_in in; fill_point(&in, u, g, H, gH, P, p);
     real a[4][4], b[4][4], c[3][4][4];
     if (rhs_point(&in, gam, a, b, c)) { bad += 1; memset(a, 0, sizeof a); memset(b, 0, sizeof b); memset(c, 0, sizeof c); }
     int fz = frozen(sd, p);
+    if (!fz) {   /* O10: characteristic faces, in face order (a FROZEN face through the point wins) */
+      real rel[3] = {(real)xyz[p] - (real)sd->center[0], (real)xyz[P + p] - (real)sd->center[1], (real)xyz[2 * P + p] - (real)sd->center[2]};
+      real sdir[6][3]; int nf = char_faces(sd, p, rel, sdir);
+      for (int f = 0; f < nf; ++f) char_bc_point(in.psi, gam, sdir[f], a, b, c);
+    }
     for (int x = 0; x < 4; ++x) for (int y = x; y < 4; ++y) {
       int s = SYM[x][y];
       dtu[(int64_t)s * P + p] = fz ? 0 : a[x][y]; dtu[(int64_t)(10 + s) * P + p] = fz ? 0 : b[x][y];
       for (int i = 0; i < 3; ++i) dtu[(int64_t)(20 + 10 * i + s) * P + p] = fz ? 0 : c[i][x][y];
     }
   }
-  free(g);
+  free(g); free(xyz);
   return bad;
 }
 

@@ -100,6 +100,8 @@ class Oracle:
         L.ora_rk3_subdomain.restype = C.c_int
         L.ora_constraints_subdomain.argtypes = [C.POINTER(Subdomain), _dp, _dp, _dp, _dp, C.c_void_p]
         L.ora_constraints_subdomain.restype = C.c_int
+        L.ora_char_bc_point.argtypes = [_dp] * 7
+        L.ora_char_bc_point.restype = C.c_int
         L.ora_filter_subdomain.argtypes = [C.POINTER(Subdomain), C.c_int, _dp, _dp, _dp, _dp]
         L.ora_filter_subdomain.restype = C.c_int
         self.threads = threads
@@ -191,6 +193,15 @@ class Oracle:
         if bad:
             raise ValueError("non-physical metric")
         return o1, o2, o3
+
+    def char_bc_point(self, psi, gamma, s, dtpsi, dtPi, dtPhi):
+        """O10 at one point: freeze the incoming characteristic fields.  psi[4,4]; s[3] outward direction;
+        dtpsi[4,4], dtPi[4,4], dtPhi[3,4,4] -> (dtpsi', dtPi', dtPhi', speeds[v0, v1+, v1-, v2])."""
+        c = lambda a: np.array(a, dtype=np.float64, order="C", copy=True)
+        a, b, d3, sp = c(dtpsi), c(dtPi), c(dtPhi), np.empty(4)
+        if self.lib.ora_char_bc_point(c(psi), c(gamma), c(s), a, b, d3, sp):
+            raise ValueError("non-physical metric")
+        return a, b, d3, sp
 
     def constraints_point(self, psi, Pi, Phi, dpsi, dPhi, H):
         c = lambda a: np.ascontiguousarray(a, dtype=np.float64)
