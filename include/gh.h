@@ -55,7 +55,12 @@ typedef enum {
 } gh_status;
 
 typedef enum { GH_SHELL = 0, GH_BLOCK = 1 } gh_kind;
-typedef enum { GH_FACE_FREE = 0, GH_FACE_FROZEN = 1 } gh_face;
+/* FREE: no boundary treatment (e.g. an excision face inside the horizon).  FROZEN: d_t u = 0 on the face.
+ * CHARACTERISTIC (NEXT-2 (i); the paper's ApplyBCs module, which it left on the CPU): the time
+ * derivatives of the characteristic fields that ENTER through the face are set to zero, the others keep what the evolution
+ * equations give (reading S21 writes the fields and speeds out); fused into the RHS kernel.  At block edges the
+ * faces are applied in the order -x,+x,-y,+y,-z,+z; a FROZEN face through the same point wins. */
+typedef enum { GH_FACE_FREE = 0, GH_FACE_FROZEN = 1, GH_FACE_CHARACTERISTIC = 2 } gh_face;
 
 /* One spectral subdomain (PAPER.md:371 I1^3 blocks, PAPER.md:386 I1 x S2 shells). */
 typedef struct {

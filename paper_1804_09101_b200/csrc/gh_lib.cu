@@ -115,7 +115,7 @@ bool validate(const gh_subdomain_desc* descs, int32_t n_sub, std::string& err) {
       }
     } else { snprintf(buf, sizeof buf, "subdomain %d: unknown kind %d", s, d.kind); err = buf; return false; }
     for (int f = 0; f < 6; ++f)
-      if (d.face[f] != GH_FACE_FREE && d.face[f] != GH_FACE_FROZEN) { snprintf(buf, sizeof buf, "subdomain %d: bad face flag", s); err = buf; return false; }
+      if (d.face[f] != GH_FACE_FREE && d.face[f] != GH_FACE_FROZEN && d.face[f] != GH_FACE_CHARACTERISTIC) { snprintf(buf, sizeof buf, "subdomain %d: bad face flag", s); err = buf; return false; }
     for (int g = 0; g < 3; ++g)
       if (!std::isfinite(d.gamma[g])) { snprintf(buf, sizeof buf, "subdomain %d: non-finite gamma", s); err = buf; return false; }
   }
@@ -217,7 +217,7 @@ struct gh_domain {
   double *part = nullptr, *persub = nullptr;
   int* flag = nullptr;
   std::vector<SubDev> h_subs;
-  bool has_fields = false, has_shell = false, has_block = false;
+  bool has_fields = false, has_shell = false, has_block = false, has_char = false;
   double t = 0.0;
   int64_t launches = 0;
   std::string err;
@@ -343,7 +343,7 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
     memset(&sd, 0, sizeof sd);
     int n0, n1, n2; sub_dims(de, n0, n1, n2);
     sd.kind = de.kind; sd.n0 = n0; sd.n1 = n1; sd.n2 = n2; sd.off = pl.offsets[s]; sd.P = n0 * n1 * n2;
-    for (int f = 0; f < 6; ++f) sd.face[f] = de.face[f];
+    for (int f = 0; f < 6; ++f) { sd.face[f] = de.face[f]; if (f < (de.kind == GH_SHELL ? 2 : 6) && de.face[f] == GH_FACE_CHARACTERISTIC) d->has_char = true; }
     for (int g = 0; g < 3; ++g) sd.gamma[g] = de.gamma[g];
     const int naxes = de.kind == GH_SHELL ? 1 : 3;
     const int64_t nn[3] = {n0, n1, n2};
@@ -499,9 +499,12 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
   if (!ang.empty()) GH_CREATE_CUDA(cudaMemcpyAsync(d->ang, ang.data(), ang.size() * sizeof(AngItem), cudaMemcpyHostToDevice, st));
   if (!fcheb.empty()) GH_CREATE_CUDA(cudaMemcpyAsync(d->fcheb, fcheb.data(), fcheb.size() * sizeof(ChebItem), cudaMemcpyHostToDevice, st));
   GH_CREATE_CUDA(cudaStreamSynchronize(st));   // host staging vectors die at return
-  GH_CREATE_CUDA(cudaFuncSetAttribute(k_rhs<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RHS_SMEM_BYTES));
-  GH_CREATE_CUDA(cudaFuncSetAttribute(k_rhs<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RHS_SMEM_BYTES));
-  GH_CREATE_CUDA(cudaFuncSetAttribute(k_rhs<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RHS_SMEM_BYTES));
+  GH_CREATE_CUDA(cudaFuncSetAttribute(k_rhs<0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RHS_SMEM_BYTES));
+  GH_CREATE_CUDA(cudaFuncSetAttribute(k_rhs<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RHS_SMEM_BYTES));
+  GH_CREATE_CUDA(cudaFuncSetAttribute(k_rhs<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RHS_SMEM_BYTES));
+  GH_CREATE_CUDA(cudaFuncSetAttribute(k_rhs<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RHS_SMEM_BYTES));
+  GH_CREATE_CUDA(cudaFuncSetAttribute(k_rhs<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RHS_SMEM_BYTES));
+  GH_CREATE_CUDA(cudaFuncSetAttribute(k_rhs<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RHS_SMEM_BYTES));
   if (pl.n_ang_class[0]) GH_CREATE_CUDA(cudaFuncSetAttribute(k_ang<ANG_TPB0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.ang_smem[0]));
   if (pl.n_ang_class[1]) GH_CREATE_CUDA(cudaFuncSetAttribute(k_ang<ANG_TPB1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.ang_smem[1]));
   if (pl.n_ang_class[0]) GH_CREATE_CUDA(cudaFuncSetAttribute(k_ang<ANG_TPB0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.ang_smem[0]));
@@ -630,12 +633,10 @@ gh_status launch_rhs(gh_domain* d, const double* u, double* out, int rk_mode = 0
     ProfScope ps(d, GH_K_RHS);
     const RkArgs rk{u0, a, b, dt};
     const int grid = d->pl.n_tiles;
-    if (rk_mode == 0)
-      k_rhs<0><<<grid, TILE_PTS, RHS_SMEM_BYTES, d->stream>>>(d->subs, d->tiles, d->pl.n_sub, d->tables, u, d->du, d->H, d->dH, out, rk, d->pl.S, d->flag);
-    else if (rk_mode == 1)
-      k_rhs<1><<<grid, TILE_PTS, RHS_SMEM_BYTES, d->stream>>>(d->subs, d->tiles, d->pl.n_sub, d->tables, u, d->du, d->H, d->dH, out, rk, d->pl.S, d->flag);
-    else
-      k_rhs<2><<<grid, TILE_PTS, RHS_SMEM_BYTES, d->stream>>>(d->subs, d->tiles, d->pl.n_sub, d->tables, u, d->du, d->H, d->dH, out, rk, d->pl.S, d->flag);
+#define GH_RHS_LAUNCH(M, C) k_rhs<M, C><<<grid, TILE_PTS, RHS_SMEM_BYTES, d->stream>>>(d->subs, d->tiles, d->pl.n_sub, d->tables, u, d->du, d->H, d->dH, out, rk, d->pl.S, d->flag)
+    if (d->has_char) { if (rk_mode == 0) GH_RHS_LAUNCH(0, true); else if (rk_mode == 1) GH_RHS_LAUNCH(1, true); else GH_RHS_LAUNCH(2, true); }
+    else { if (rk_mode == 0) GH_RHS_LAUNCH(0, false); else if (rk_mode == 1) GH_RHS_LAUNCH(1, false); else GH_RHS_LAUNCH(2, false); }
+#undef GH_RHS_LAUNCH
   }
   GH_CUDA(d, cudaGetLastError());
   return GH_OK;

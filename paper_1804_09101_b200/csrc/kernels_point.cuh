@@ -309,6 +309,39 @@ __device__ __forceinline__ void algebraic(const Geom& G, const PI& Pi, const PH&
 // ---------------------------------------------------------------------------------------------------------
 struct RkArgs { const double* u0; double a, b, dt; };
 
+// Characteristic boundary condition (NEXT-2 (i), reading S21) for one symmetric pair (ab) at a face point with outward
+// direction s: with n_i = s_i / sqrt(g^{jk} s_j s_k), n^i = g^{ij} n_j,
+//   u0 = psi (speed -(1+g1) n.N),  u1+- = Pi +- n^i Phi_i - g2 psi (speed -n.N +- N),  u2_i = Phi_i - n_i n^k Phi_k (speed -n.N);
+// the time derivatives of the fields with negative speed (entering the domain) are set to zero, the rest kept.
+__device__ __forceinline__ void char_bc_pair(const Geom& G, double g1, double g2, double sx, double sy, double sz,
+                                             double& dpsi, double& dPi, double (&dPhi)[3]) {
+  const double sv[3] = {sx, sy, sz};
+  double gs[3], nn = 0.0;
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    double v = 0.0;
+#pragma unroll
+    for (int j = 0; j < 3; ++j) v = fma(G.gi[S3(i, j)], sv[j], v);
+    gs[i] = v;
+    nn = fma(v, sv[i], nn);
+  }
+  const double inv = 1.0 / sqrt(nn);
+  double nd[3], nu[3], nN = 0.0, nPhi = 0.0;
+#pragma unroll
+  for (int i = 0; i < 3; ++i) { nd[i] = sv[i] * inv; nu[i] = gs[i] * inv; nN = fma(nd[i], G.sh[i], nN); nPhi = fma(nu[i], dPhi[i], nPhi); }
+  double u0 = dpsi, u1p = dPi + nPhi - g2 * dpsi, u1m = dPi - nPhi - g2 * dpsi, u2[3];
+#pragma unroll
+  for (int i = 0; i < 3; ++i) u2[i] = dPhi[i] - nd[i] * nPhi;
+  if (-(1.0 + g1) * nN < 0.0) u0 = 0.0;
+  if (-nN + G.N < 0.0) u1p = 0.0;
+  if (-nN - G.N < 0.0) u1m = 0.0;
+  if (-nN < 0.0) { u2[0] = 0.0; u2[1] = 0.0; u2[2] = 0.0; }
+  dpsi = u0;
+  dPi = 0.5 * (u1p + u1m) + g2 * u0;
+#pragma unroll
+  for (int i = 0; i < 3; ++i) dPhi[i] = 0.5 * (u1p - u1m) * nd[i] + u2[i];
+}
+
 template <int RK>
 __device__ __forceinline__ void rhs_store(double* out, const RkArgs& rk, int64_t idx, double dtu, double us, double u0v) {
   if (RK == 0) { out[idx] = dtu; return; }
@@ -346,7 +379,7 @@ __device__ __forceinline__ void rhs_prefetch(double* __restrict__ slot /* + tid 
   cp_async_commit();
 }
 
-template <bool SHELL, int RK>
+template <bool SHELL, int RK, bool CBC>
 __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __restrict__ tables, int local,
                                           const double* u, const double* __restrict__ du,
                                           const double* __restrict__ Hs, const double* __restrict__ dHs,
@@ -356,12 +389,16 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
   const int64_t p = sd.off + local;
   // face mask (A6)
   bool frozen;
+  int cmask = 0;   // faces flagged CHARACTERISTIC (2) through this point, bit f = face f
   {
     const int i2 = local % sd.n2, t = local / sd.n2, i1 = t % sd.n1, i0 = t / sd.n1;
-    frozen = (i0 == 0 && sd.face[0] == 1) || (i0 == sd.n0 - 1 && sd.face[1] == 1);
-    if (!SHELL)
-      frozen = frozen || (i1 == 0 && sd.face[2] == 1) || (i1 == sd.n1 - 1 && sd.face[3] == 1) ||
-               (i2 == 0 && sd.face[4] == 1) || (i2 == sd.n2 - 1 && sd.face[5] == 1);
+    const bool on[6] = {i0 == 0, i0 == sd.n0 - 1, !SHELL && i1 == 0, !SHELL && i1 == sd.n1 - 1, !SHELL && i2 == 0, !SHELL && i2 == sd.n2 - 1};
+    frozen = false;
+#pragma unroll
+    for (int f = 0; f < (SHELL ? 2 : 6); ++f) {
+      frozen = frozen || (on[f] && sd.face[f] == 1);
+      if (CBC && on[f] && sd.face[f] == 2) cmask |= 1 << f;
+    }
   }
   constexpr int SLOT = RHS_RING_ROWS * TILE_PTS;
   // Phi_iab of this point -> shared memory (first cp.async group), then the first RHS_RING pairs of stage 3
@@ -444,7 +481,7 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
         sdPi = fma(G.sh[kk], d[1][kk], sdPi);
         sPhi = fma(G.sh[kk], Phi(kk, s), sPhi);
       }
-      rhs_store<RK>(k, rk, (int64_t)s * S + p, (1.0 + g1) * sdpsi - N * Pi[s] - g1 * sPhi, psi[s], RK == 2 ? slot[17 * TILE_PTS] : 0.0);
+      double o_psi = (1.0 + g1) * sdpsi - N * Pi[s] - g1 * sPhi;
 
       double gdPhi = 0.0;   // g^{ki} d_k Phi_iab
 #pragma unroll
@@ -471,7 +508,7 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
       const double tbCa = (b == 0 ? -N * A.C[a] : 0.0), taCb = (a == 0 ? -N * A.C[b] : 0.0);
       double r = sdPi - N * gdPhi + g1 * g2 * (sdpsi - sPhi) + 2.0 * N * (A.S[s] - symdH) - 0.5 * N * A.ttPi * Pi[s] -
                  N * pup + N * g0 * (tbCa + taCb - psi[s] * A.tC);
-      rhs_store<RK>(k, rk, (int64_t)(10 + s) * S + p, r, Pi[s], RK == 2 ? slot[18 * TILE_PTS] : 0.0);
+      double o_Phi[3];
 #pragma unroll
       for (int i = 0; i < 3; ++i) {
         double sdPhi = 0.0, wup = 0.0;
@@ -479,9 +516,22 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
         for (int kk = 0; kk < 3; ++kk) sdPhi = fma(G.sh[kk], d[2 + i][kk], sdPhi);
 #pragma unroll
         for (int j = 0; j < 3; ++j) wup = fma(A.w[i][j], up[j], wup);
-        rhs_store<RK>(k, rk, (int64_t)(20 + 10 * i + s) * S + p,
-                      sdPhi - N * d[1][i] + N * g2 * (d[0][i] - Phi(i, s)) + 0.5 * N * A.s[i] * Pi[s] + N * wup, Phi(i, s), RK == 2 ? slot[(19 + i) * TILE_PTS] : 0.0);
+        o_Phi[i] = sdPhi - N * d[1][i] + N * g2 * (d[0][i] - Phi(i, s)) + 0.5 * N * A.s[i] * Pi[s] + N * wup;
       }
+      if (CBC && cmask) {   // characteristic faces through this point, in face order (rare: face points only)
+#pragma unroll
+        for (int f = 0; f < (SHELL ? 2 : 6); ++f)
+          if (cmask & (1 << f)) {
+            const double sg = (f & 1) ? 1.0 : -1.0;
+            if (SHELL) char_bc_pair(G, g1, g2, sg * J.xr, sg * J.yr, sg * J.zr, o_psi, r, o_Phi);   // +- r^ = (st cp, st sp, ct)
+            else char_bc_pair(G, g1, g2, f / 2 == 0 ? sg : 0.0, f / 2 == 1 ? sg : 0.0, f / 2 == 2 ? sg : 0.0, o_psi, r, o_Phi);
+          }
+      }
+      rhs_store<RK>(k, rk, (int64_t)s * S + p, o_psi, psi[s], RK == 2 ? slot[17 * TILE_PTS] : 0.0);
+      rhs_store<RK>(k, rk, (int64_t)(10 + s) * S + p, r, Pi[s], RK == 2 ? slot[18 * TILE_PTS] : 0.0);
+#pragma unroll
+      for (int i = 0; i < 3; ++i)
+        rhs_store<RK>(k, rk, (int64_t)(20 + 10 * i + s) * S + p, o_Phi[i], Phi(i, s), RK == 2 ? slot[(19 + i) * TILE_PTS] : 0.0);
       // every value of the slot has been consumed: refill it with pair s + RHS_RING
       if (s == 0) rhs_prefetch<3, RK>(ring + 0 * SLOT, du, dHs, rk.u0, S, p);
       if (s == 1) rhs_prefetch<4, RK>(ring + 1 * SLOT, du, dHs, rk.u0, S, p);
@@ -494,7 +544,8 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
     }
 }
 
-template <int RK>
+// CBC: the domain has faces flagged CHARACTERISTIC (a second instantiation, so that domains without them do not pay for it)
+template <int RK, bool CBC>
 __global__ void __launch_bounds__(TILE_PTS, 2)
 k_rhs(const SubDev* __restrict__ subs, const int32_t* __restrict__ tile_first, int n_sub,
       const double* __restrict__ tables, const double* u, const double* __restrict__ du,
@@ -512,8 +563,8 @@ k_rhs(const SubDev* __restrict__ subs, const int32_t* __restrict__ tile_first, i
   const SubDev& sd = sd_s;
   const int local = (blockIdx.x - tile0_s) * TILE_PTS + threadIdx.x;
   if (local >= sd.P) return;
-  if (sd.kind == 0) rhs_point<true, RK>(sd, tables, local, u, du, Hs, dHs, k, rk, S, flag, ring_s + threadIdx.x);
-  else rhs_point<false, RK>(sd, tables, local, u, du, Hs, dHs, k, rk, S, flag, ring_s + threadIdx.x);
+  if (sd.kind == 0) rhs_point<true, RK, CBC>(sd, tables, local, u, du, Hs, dHs, k, rk, S, flag, ring_s + threadIdx.x);
+  else rhs_point<false, RK, CBC>(sd, tables, local, u, du, Hs, dHs, k, rk, S, flag, ring_s + threadIdx.x);
 }
 
 // ---------------------------------------------------------------------------------------------------------

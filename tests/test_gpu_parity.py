@@ -40,7 +40,16 @@ def _wide():
                       configs.block([2, 3, 64], (3.0, 3.0, -2.0), (4.0, 4.0, 2.0), gamma=[0.0, 0.0, 0.0])]}
 
 
-CASES = {"c1": configs.c1, "c2": configs.c2, "mixed": _mini_mixed, "wide": _wide}
+def _charbc():
+    """NEXT-2 (i): faces flagged CHARACTERISTIC (2): an excision shell whose inner face lies inside the horizon (nothing comes
+    in there), an outer shell, and a block with characteristic, frozen and free faces meeting at its edges and corners."""
+    return {"id": 9, "spin": 0.4, "amplitude": 1e-3,
+            "descs": [configs.shell(7, 6, 1.7, 3.0, face=(2, 2), gamma=[1.0, -1.0, 1.0]),
+                      configs.shell(6, 8, 3.0, 8.0, face=(2, 2), gamma=[2.0, -0.4, 1.5]),
+                      configs.block([7, 6, 8], (3.0, -1.0, -2.0), (5.0, 1.0, 0.5), face=(2, 2, 0, 2, 1, 2), gamma=[1.0, -0.7, 0.5])]}
+
+
+CASES = {"c1": configs.c1, "c2": configs.c2, "mixed": _mini_mixed, "wide": _wide, "charbc": _charbc}
 
 
 @pytest.fixture(scope="module", params=list(CASES))
