@@ -34,7 +34,9 @@
  * stationarity of exact Kerr-Schild data with analytic derivatives, the harmonic
  * gauge wave, homogeneous damping-term cases, RK3 order; spectral filter (O9):
  * single Chebyshev modes and single Y_lm scaled by sigma, sigma = 1 identity /
- * projection, Heaviside idempotence, linearity.  PARITY UNPINNED (pure
+ * projection, Heaviside idempotence, linearity; characteristic boundary condition
+ * (O10): eigenvectors of the RHS's principal part; Dormand-Prince step (O11): the
+ * order conditions of the tableau and 5th-order convergence on the gauge wave.  PARITY UNPINNED (pure
  * conventions, fixed by DESIGN.md): the normalisation of the constraint norms
  * (unweighted RMS over points and components) and the default gamma's.
  */
@@ -778,6 +780,53 @@ int ora_rk3_subdomain(const ora_subdomain* sd, double* u, const double* H, const
   }
   for (int64_t i = 0; i < n; ++i) u[i] = (double)u0[i];
   free(u0); free(us); free(k); free(Hr); free(gH);
+  return bad;
+}
+
+/* ---------------------------------------------------------------------- */
+/* O11 — Dormand-Prince 5(4) step (NEXT-3): the stepper the paper names    */
+/* ("high-order Dormand Prince").  Explicit 7-stage pair of   */
+/* Dormand & Prince (1980): 5th-order solution (its weights are row 7 of   */
+/* the matrix, so stage 7 is the RHS at the new state) and the embedded    */
+/* 4th-order weights bh; err = dt sum_j (b_j - bh_j) k_j.                  */
+/* ---------------------------------------------------------------------- */
+static const real DP_C[7] = {0, (real)1 / 5, (real)3 / 10, (real)4 / 5, (real)8 / 9, 1, 1};
+static const real DP_A[7][6] = {
+  {0, 0, 0, 0, 0, 0},
+  {(real)1 / 5, 0, 0, 0, 0, 0},
+  {(real)3 / 40, (real)9 / 40, 0, 0, 0, 0},
+  {(real)44 / 45, -(real)56 / 15, (real)32 / 9, 0, 0, 0},
+  {(real)19372 / 6561, -(real)25360 / 2187, (real)64448 / 6561, -(real)212 / 729, 0, 0},
+  {(real)9017 / 3168, -(real)355 / 33, (real)46732 / 5247, (real)49 / 176, -(real)5103 / 18656, 0},
+  {(real)35 / 384, 0, (real)500 / 1113, (real)125 / 192, -(real)2187 / 6784, (real)11 / 84}};
+static const real DP_BH[7] = {(real)5179 / 57600, 0, (real)7571 / 16695, (real)393 / 640, -(real)92097 / 339200, (real)187 / 2100, (real)1 / 40};
+
+/* c[7], a[7*6] (row-major, a[i][j], j < i), b[7] (5th order = row 7 of a, b[6] = 0), bh[7] (4th order) */
+void ora_dp5_tableau(double* c, double* a, double* b, double* bh) {
+  for (int i = 0; i < 7; ++i) { c[i] = (double)DP_C[i]; bh[i] = (double)DP_BH[i]; b[i] = i < 6 ? (double)DP_A[6][i] : 0.0;
+    for (int j = 0; j < 6; ++j) a[6 * i + j] = (double)DP_A[i][j]; }
+}
+
+/* one step of size dt: u[50][P] <- 5th-order solution, err[50][P] <- dt sum_j (b_j - bh_j) k_j.  Returns #non-physical points. */
+int ora_dp5_subdomain(const ora_subdomain* sd, double* u, const double* H, const double* dH, double dt, double* err) {
+  int64_t P = ora_num_points(sd), n = 50 * P;
+  real* u0 = malloc(sizeof(real) * n); real* us = malloc(sizeof(real) * n); real* k[7];
+  for (int q = 0; q < 7; ++q) k[q] = malloc(sizeof(real) * n);
+  real* Hr = malloc(sizeof(real) * 4 * P); real* gH = malloc(sizeof(real) * 12 * P);
+  for (int64_t i = 0; i < n; ++i) u0[i] = u[i];
+  for (int64_t i = 0; i < 4 * P; ++i) Hr[i] = H[i];
+  if (dH) for (int64_t i = 0; i < 12 * P; ++i) gH[i] = dH[i]; else gradient_real(sd, 4, Hr, gH);
+  real h = dt; int bad = 0;
+  for (int st = 0; st < 7; ++st) {
+    for (int64_t i = 0; i < n; ++i) { real a = 0; for (int j = 0; j < st; ++j) a += DP_A[st][j] * k[j][i]; us[i] = u0[i] + h * a; }
+    bad += rhs_real(sd, us, Hr, gH, k[st]);
+  }
+  /* us now holds the 5th-order solution (row 7 of the matrix are its weights) */
+  for (int64_t i = 0; i < n; ++i) {
+    real e = 0; for (int j = 0; j < 7; ++j) e += ((j < 6 ? DP_A[6][j] : 0) - DP_BH[j]) * k[j][i];
+    u[i] = (double)us[i]; err[i] = (double)(h * e);
+  }
+  free(u0); free(us); for (int q = 0; q < 7; ++q) free(k[q]); free(Hr); free(gH);
   return bad;
 }
 

@@ -100,6 +100,10 @@ class Oracle:
         L.ora_rk3_subdomain.restype = C.c_int
         L.ora_constraints_subdomain.argtypes = [C.POINTER(Subdomain), _dp, _dp, _dp, _dp, C.c_void_p]
         L.ora_constraints_subdomain.restype = C.c_int
+        L.ora_dp5_tableau.argtypes = [_dp] * 4
+        L.ora_dp5_tableau.restype = None
+        L.ora_dp5_subdomain.argtypes = [C.POINTER(Subdomain), _dp, _dp, C.c_void_p, C.c_double, _dp]
+        L.ora_dp5_subdomain.restype = C.c_int
         L.ora_char_bc_point.argtypes = [_dp] * 7
         L.ora_char_bc_point.restype = C.c_int
         L.ora_filter_subdomain.argtypes = [C.POINTER(Subdomain), C.c_int, _dp, _dp, _dp, _dp]
@@ -250,6 +254,23 @@ class Oracle:
         if bad:
             raise ValueError(f"{bad} non-physical points")
         return u
+
+    def dp5_tableau(self):
+        c, a, b, bh = np.empty(7), np.empty((7, 6)), np.empty(7), np.empty(7)
+        self.lib.ora_dp5_tableau(c, a, b, bh)
+        return c, a, b, bh
+
+    def dp5(self, sd: dict, u, H, dt: float, dH=None):
+        """O11: one Dormand-Prince 5(4) step -> (u_new[50,P], err[50,P])."""
+        s = make_subdomain(sd)
+        out = np.array(u, dtype=np.float64, order="C", copy=True)
+        err = np.empty_like(out)
+        Hc = np.ascontiguousarray(H, dtype=np.float64)
+        dHc = None if dH is None else np.ascontiguousarray(dH, dtype=np.float64)
+        bad = self.lib.ora_dp5_subdomain(C.byref(s), out, Hc, None if dHc is None else dHc.ctypes.data, float(dt), err)
+        if bad:
+            raise ValueError("non-physical metric")
+        return out, err
 
     def constraints(self, sd: dict, u, H, fields: bool = False):
         """-> (sums[3], maxs[3], Cfield[64,P] or None) for one subdomain."""
