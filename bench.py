@@ -379,6 +379,7 @@ def run_ours(args):
         raise SystemExit("bench.py: non-finite state after the e2e region")
 
     filt = time_filter(dom, u_dev, descs) if rank == 0 else None
+    dp5 = time_dp5(dom, u_dev, dt, P) if rank == 0 else None
 
     tmax, e2emax = max_over_ranks([ms, e2e_s / e2e_steps], dist, dev)
     if rank != 0:
@@ -387,7 +388,7 @@ def run_ours(args):
             dist.barrier(); dist.destroy_process_group()
         return
     return finish_ours(args, world, label, cfg, descs, reps, P, S, tmax, e2emax, e2e_steps, launches, prof, work, clocks,
-                       norms, base, dom, dist, filt)
+                       norms, base, dom, dist, filt, dp5)
 
 
 def time_filter(dom, u_dev, descs, reps: int = 5):
@@ -421,8 +422,28 @@ def time_filter(dom, u_dev, descs, reps: int = 5):
     return out
 
 
+def time_dp5(dom, u_dev, dt, P, reps: int = 3):
+    """NEXT-3 (outside the timed step): gh_dp5_step, 6 new RHS evaluations per step (the 7th stage is reused as the next
+    step's first).  Wall time around `reps` steps after one warm-up step (the call synchronises: it returns the error norms)."""
+    import torch
+
+    try:
+        dom.dp5_attach()
+    except Exception as e:          # not enough device memory for the 7 stage arrays
+        return {"unavailable": str(e)}
+    dom.set_fields(u_dev, 0.0)
+    dom.dp5_step(dt)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(reps):
+        rms, mx, acc = dom.dp5_step(dt)
+    torch.cuda.synchronize()
+    s_per = (time.perf_counter() - t0) / reps
+    return {"ms_per_step": s_per * 1e3, "rhs_evals_per_step": 6, "points_per_s": 6.0 * P / s_per, "err_rms": rms, "err_max": mx}
+
+
 def finish_ours(args, world, label, cfg, descs, reps, P, S, ms, e2e_step_s, e2e_steps, launches, prof, work, clocks,
-                norms, base, dom, dist, filt=None):
+                norms, base, dom, dist, filt=None, dp5=None):
     hbm_peak, peak_src = load_peaks()
     steps = args.steps
     value = whole_job_value(world, P, steps, ms)
@@ -432,7 +453,7 @@ def finish_ours(args, world, label, cfg, descs, reps, P, S, ms, e2e_step_s, e2e_
     calls_per_step = {"k_rhs": 3, "k_con": 1, "k_cheb": 3.8, "k_ang": 3.8}   # library calls that run the kernel
     kernels = {}
     for name, (kms, cnt) in prof.items():
-        if cnt == 0 or "filter" in name:
+        if cnt == 0 or "filter" in name or name.startswith("k_dp"):
             continue
         e = {"launches_per_step": cnt / steps, "ms_per_launch": kms / cnt, "ms_per_step": kms / steps,
              "share_of_kernel_time": kms / total_kernel_ms}
@@ -495,6 +516,7 @@ def finish_ours(args, world, label, cfg, descs, reps, P, S, ms, e2e_step_s, e2e_
         "clocks": clocks,
         "constraint_norms_after": [[float(x) for x in r] for r in np.asarray(norms)],
         "spectral_filter": filt,
+        "dormand_prince_5_4": dp5,
     }
     print(json.dumps(out))
     sys.stdout.flush()

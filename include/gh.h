@@ -165,13 +165,28 @@ gh_status gh_apply_filter(gh_domain* dom);
 /* The filter function itself, for tests: sigma[0..kmax].  HOST. */
 gh_status gh_filter_sigma(const gh_filter_desc* f, int32_t kmax, double* sigma);
 
+/* ---- Dormand-Prince 5(4) step (NEXT-3 of DESIGN.md; the stepper the paper names, "high-order Dormand Prince",
+ * PAPER.md:81) -----------------------------------------------------------------------------------------------------
+ * Seven-stage explicit pair of Dormand & Prince (1980): the 5th-order solution advances the state, the embedded 4th-order
+ * one gives err = dt sum_j (b_j - bh_j) k_j for step-size control.  The seven stage derivatives need 7 x [50][comp_stride]
+ * doubles of extra device memory, attached separately so that RK3 users do not pay for it. */
+size_t gh_dp5_workspace_bytes(const gh_domain* dom);
+/* dev_ws: DEVICE, 256-byte aligned, >= gh_dp5_workspace_bytes; owned by the caller, valid until destroy.  Zeroes it. */
+gh_status gh_dp5_attach(gh_domain* dom, void* dev_ws, size_t bytes);
+/* One step of size dt.  err: HOST [2] = {rms, max} of the error estimate over all 50 components and points (unweighted).
+ * tol > 0: the step is taken only if max <= tol, otherwise the state is left as it was (*accepted = 0) and the caller
+ * retries with a smaller dt; tol <= 0: always taken.  accepted may be NULL.  Synchronises (it returns host data).
+ * The last stage is the RHS at the new state and is reused as the first stage of the next step when nothing else touched
+ * the state in between. */
+gh_status gh_dp5_step(gh_domain* dom, double dt, double tol, double* err, int* accepted);
+
 /* Per-kernel device time of the most recent gh_rhs / gh_rk_step / gh_constraint_norms, in
  * milliseconds, measured with CUDA events on the domain's stream when profiling is enabled with
  * gh_set_profiling(dom, 1) (off by default: event records cost launch latency).
  * ms: HOST [GH_NUM_KERNELS] accumulated since the last call to gh_profile_reset; counts likewise. */
-#define GH_NUM_KERNELS 10
+#define GH_NUM_KERNELS 12
 enum { GH_K_CHEB = 0, GH_K_SHELL_ANG = 1, GH_K_RHS = 2, GH_K_RK = 3, GH_K_CONSTRAINTS = 4, GH_K_REDUCE = 5, GH_K_JAC = 6, GH_K_OTHER = 7,
-       GH_K_FILTER_CHEB = 8, GH_K_FILTER_ANG = 9 };
+       GH_K_FILTER_CHEB = 8, GH_K_FILTER_ANG = 9, GH_K_DP_STAGE = 10, GH_K_DP_ERR = 11 };
 gh_status gh_set_profiling(gh_domain* dom, int enabled);
 gh_status gh_profile_read(gh_domain* dom, double* ms, int64_t* counts);
 gh_status gh_profile_reset(gh_domain* dom);

@@ -214,6 +214,10 @@ struct gh_domain {
   std::vector<FBlock> f_blocks;
   std::map<int, size_t> f_L;             // shell band limit L -> offset (doubles) of its filtered projectors from `tables`
   bool filt_blocks = false, filt_shells = false;
+  // Dormand-Prince 5(4): seven stage derivatives in a separately attached workspace
+  double* dpk[7] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  double *dp_part = nullptr, *dp_out = nullptr;
+  bool dp_fsal = false;                  // dpk[0] already holds the RHS of the current state
   double *part = nullptr, *persub = nullptr;
   int* flag = nullptr;
   std::vector<SubDev> h_subs;
@@ -660,7 +664,7 @@ extern "C" gh_status gh_set_fields(gh_domain* d, const double* u, int on_device,
   const size_t bytes = (size_t)NCOMP * d->pl.S * sizeof(double);
   GH_CUDA(d, cudaMemcpyAsync(d->ua, u, bytes, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, d->stream));
   if (!on_device) GH_CUDA(d, cudaStreamSynchronize(d->stream));
-  d->t = t; d->has_fields = true;
+  d->t = t; d->has_fields = true; d->dp_fsal = false;
   return GH_OK;
 }
 
@@ -679,6 +683,7 @@ extern "C" gh_status gh_set_gauge_source(gh_domain* d, const double* H, const do
   if (!d || !H) return fail(d, GH_ERR_ARG, "NULL argument");
   const size_t comp = (size_t)d->pl.S * sizeof(double);
   const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+  d->dp_fsal = false;
   GH_CUDA(d, cudaMemcpyAsync(d->H, H, 4 * comp, kind, d->stream));
   if (dH) {
     GH_CUDA(d, cudaMemcpyAsync(d->dH, dH, 12 * comp, kind, d->stream));
@@ -732,7 +737,7 @@ extern "C" gh_status gh_rk_step(gh_domain* d, double dt) {
   if ((st = launch_rhs(d, d->ub, d->ub, 2, d->ua, 0.75, 0.25, dt)) != GH_OK) return st;
   // u_new = 1/3 u0 + 2/3 (u2 + dt k(u2))    (ub -> ua, over u0)
   if ((st = launch_rhs(d, d->ub, d->ua, 2, d->ua, 1.0 / 3.0, 2.0 / 3.0, dt)) != GH_OK) return st;
-  d->t += dt;
+  d->t += dt; d->dp_fsal = false;
   return GH_OK;
 }
 
@@ -856,6 +861,7 @@ extern "C" gh_status gh_set_filter(gh_domain* d, const gh_filter_desc* fb, const
 extern "C" gh_status gh_apply_filter(gh_domain* d) {
   if (!d) return GH_ERR_ARG;
   if (!d->has_fields) return fail(d, GH_ERR_STATE, "gh_apply_filter before gh_set_fields");
+  d->dp_fsal = false;
   const Plan& pl = d->pl;
   const CompMap cm{NCOMP, 0, 0};
   if (d->filt_blocks) {
@@ -897,6 +903,86 @@ extern "C" gh_status gh_apply_filter(gh_domain* d) {
 }
 
 // ------------------------------------------------------------------------------------------------------
+// Dormand-Prince 5(4) step (NEXT-3)
+// ------------------------------------------------------------------------------------------------------
+namespace {
+constexpr int DP_GRID = 148 * 8;     // streaming kernels: 8 CTAs of 256 threads per SM
+const double DP_A[7][6] = {
+    {0, 0, 0, 0, 0, 0},
+    {1.0 / 5, 0, 0, 0, 0, 0},
+    {3.0 / 40, 9.0 / 40, 0, 0, 0, 0},
+    {44.0 / 45, -56.0 / 15, 32.0 / 9, 0, 0, 0},
+    {19372.0 / 6561, -25360.0 / 2187, 64448.0 / 6561, -212.0 / 729, 0, 0},
+    {9017.0 / 3168, -355.0 / 33, 46732.0 / 5247, 49.0 / 176, -5103.0 / 18656, 0},
+    {35.0 / 384, 0, 500.0 / 1113, 125.0 / 192, -2187.0 / 6784, 11.0 / 84}};
+const double DP_BH[7] = {5179.0 / 57600, 0, 7571.0 / 16695, 393.0 / 640, -92097.0 / 339200, 187.0 / 2100, 1.0 / 40};
+inline size_t dp_bytes(const Plan& pl) {
+  return 7 * (size_t)round_up((int64_t)(NCOMP * pl.S * sizeof(double)), 256) + (size_t)round_up(2 * DP_GRID * sizeof(double), 256) + 256;
+}
+}  // namespace
+
+extern "C" size_t gh_dp5_workspace_bytes(const gh_domain* d) { return d ? dp_bytes(d->pl) : 0; }
+
+extern "C" gh_status gh_dp5_attach(gh_domain* d, void* ws, size_t bytes) {
+  if (!d) return GH_ERR_ARG;
+  if (!ws || ((uintptr_t)ws & 255) != 0) return fail(d, GH_ERR_WORKSPACE, "DP5 workspace is NULL or not 256-byte aligned");
+  if (bytes < dp_bytes(d->pl)) return fail(d, GH_ERR_WORKSPACE, "DP5 workspace too small: need " + std::to_string(dp_bytes(d->pl)) + " bytes");
+  char* w = (char*)ws;
+  const size_t one = (size_t)round_up((int64_t)(NCOMP * d->pl.S * sizeof(double)), 256);
+  for (int j = 0; j < 7; ++j) d->dpk[j] = (double*)(w + j * one);
+  d->dp_part = (double*)(w + 7 * one);
+  d->dp_out = (double*)(w + 7 * one + (size_t)round_up(2 * DP_GRID * sizeof(double), 256));
+  d->dp_fsal = false;
+  GH_CUDA(d, cudaMemsetAsync(ws, 0, dp_bytes(d->pl), d->stream));     // the padding between subdomains must be (and stays) zero
+  return GH_OK;
+}
+
+extern "C" gh_status gh_dp5_step(gh_domain* d, double dt, double tol, double* err, int* accepted) {
+  if (!d || !err) return fail(d, GH_ERR_ARG, "NULL argument");
+  if (!d->has_fields) return fail(d, GH_ERR_STATE, "gh_dp5_step before gh_set_fields");
+  if (!d->dpk[0]) return fail(d, GH_ERR_STATE, "gh_dp5_step before gh_dp5_attach");
+  if (!std::isfinite(dt)) return fail(d, GH_ERR_ARG, "dt is not finite");
+  const int64_t n2 = (int64_t)NCOMP * d->pl.S / 2;
+  const int grid = (int)std::min<int64_t>((n2 + 255) / 256, DP_GRID);
+  gh_status st;
+  // k1 = f(u): the last stage of the previous accepted step when the state has not been touched since
+  if (!d->dp_fsal && (st = launch_rhs(d, d->ua, d->dpk[0])) != GH_OK) return st;
+  for (int s = 1; s < 7; ++s) {      // ub = u + dt sum_j a_sj k_j;  k_{s+1} = f(ub);  after s = 6, ub is the 5th-order solution
+    DpArgs A; A.nk = s;
+    for (int j = 0; j < 7; ++j) { A.k[j] = (const double2*)d->dpk[j]; A.a[j] = j < s ? DP_A[s][j] : 0.0; }
+    {
+      ProfScope ps(d, GH_K_DP_STAGE);
+      k_dp_stage<<<grid, 256, 0, d->stream>>>((const double2*)d->ua, A, dt, (double2*)d->ub, n2);
+    }
+    if ((st = launch_rhs(d, d->ub, d->dpk[s])) != GH_OK) return st;
+  }
+  {
+    DpArgs A; A.nk = 7;
+    for (int j = 0; j < 7; ++j) { A.k[j] = (const double2*)d->dpk[j]; A.a[j] = (j < 6 ? DP_A[6][j] : 0.0) - DP_BH[j]; }
+    ProfScope ps(d, GH_K_DP_ERR);
+    k_dp_err<<<grid, 256, 0, d->stream>>>(A, dt, d->dp_part, n2);
+    k_dp_err_final<<<1, 32, 0, d->stream>>>(d->dp_part, grid, d->dp_out);
+  }
+  GH_CUDA(d, cudaGetLastError());
+  double h[2] = {0, 0};
+  GH_CUDA(d, cudaMemcpyAsync(h, d->dp_out, sizeof h, cudaMemcpyDeviceToHost, d->stream));
+  st = check_flag(d);   // synchronises
+  if (st != GH_OK) { d->dp_fsal = false; return st; }
+  err[0] = std::sqrt(h[0] / ((double)NCOMP * (double)d->pl.P));
+  err[1] = h[1];
+  const bool ok = !(tol > 0.0) || (err[1] <= tol);
+  if (accepted) *accepted = ok ? 1 : 0;
+  if (ok) {
+    std::swap(d->ua, d->ub);            // the new state; k7 = f(new state) becomes k1 of the next step
+    std::swap(d->dpk[0], d->dpk[6]);
+    d->t += dt; d->dp_fsal = true;
+  } else {
+    d->dp_fsal = true;                  // the state is unchanged and dpk[0] still is its RHS
+  }
+  return GH_OK;
+}
+
+// ------------------------------------------------------------------------------------------------------
 // profiling / bookkeeping
 // ------------------------------------------------------------------------------------------------------
 extern "C" gh_status gh_set_profiling(gh_domain* d, int enabled) {
@@ -921,7 +1007,7 @@ extern "C" gh_status gh_profile_reset(gh_domain* d) {
 }
 
 extern "C" const char* gh_kernel_name(int k) {
-  static const char* names[GH_NUM_KERNELS] = {"k_cheb", "k_ang", "k_rhs", "k_rk", "k_con", "k_con_reduce", "k_jac", "other", "k_cheb(filter)", "k_ang(filter)"};
+  static const char* names[GH_NUM_KERNELS] = {"k_cheb", "k_ang", "k_rhs", "k_rk", "k_con", "k_con_reduce", "k_jac", "other", "k_cheb(filter)", "k_ang(filter)", "k_dp_stage", "k_dp_err"};
   return (k >= 0 && k < GH_NUM_KERNELS) ? names[k] : "?";
 }
 

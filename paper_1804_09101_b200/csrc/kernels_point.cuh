@@ -568,6 +568,57 @@ k_rhs(const SubDev* __restrict__ subs, const int32_t* __restrict__ tile_first, i
 }
 
 // ---------------------------------------------------------------------------------------------------------
+// Dormand-Prince 5(4) (NEXT-3).  K_dp_stage: out = u + dt sum_{j<nk} a_j k_j over the whole store (padding is zero and
+// stays zero).  K_dp_err: e = dt sum_j d_j k_j -> per-block {sum e^2, max |e|}; K_dp_err_final folds the partials in
+// a fixed order.  All HBM-bound streaming kernels.
+// ---------------------------------------------------------------------------------------------------------
+struct DpArgs { const double2* k[7]; double a[7]; int nk; };
+
+__global__ void __launch_bounds__(256)
+k_dp_stage(const double2* __restrict__ u, DpArgs A, double dt, double2* __restrict__ out, int64_t n2) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n2; i += (int64_t)gridDim.x * blockDim.x) {
+    double sx = 0.0, sy = 0.0;
+#pragma unroll
+    for (int j = 0; j < 7; ++j)
+      if (j < A.nk) { const double2 v = A.k[j][i]; sx = fma(A.a[j], v.x, sx); sy = fma(A.a[j], v.y, sy); }
+    const double2 w = u[i];
+    out[i] = make_double2(fma(dt, sx, w.x), fma(dt, sy, w.y));
+  }
+}
+
+__global__ void __launch_bounds__(256)
+k_dp_err(DpArgs A, double dt, double* __restrict__ part, int64_t n2) {
+  __shared__ double red[8][2];
+  double ss = 0.0, mx = 0.0;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n2; i += (int64_t)gridDim.x * blockDim.x) {
+    double sx = 0.0, sy = 0.0;
+#pragma unroll
+    for (int j = 0; j < 7; ++j)
+      if (j < A.nk) { const double2 v = A.k[j][i]; sx = fma(A.a[j], v.x, sx); sy = fma(A.a[j], v.y, sy); }
+    sx *= dt; sy *= dt;
+    ss = fma(sx, sx, ss); ss = fma(sy, sy, ss);
+    mx = fmax(mx, fmax(fabs(sx), fabs(sy)));
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) { ss += __shfl_xor_sync(0xffffffffu, ss, o); mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o)); }
+  if ((threadIdx.x & 31) == 0) { red[threadIdx.x >> 5][0] = ss; red[threadIdx.x >> 5][1] = mx; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < 8; ++w) { ss += red[w][0]; mx = fmax(mx, red[w][1]); }
+    part[2 * blockIdx.x] = ss; part[2 * blockIdx.x + 1] = mx;
+  }
+}
+
+__global__ void __launch_bounds__(32)
+k_dp_err_final(const double* __restrict__ part, int nblocks, double* __restrict__ out) {
+  double ss = 0.0, mx = 0.0;
+  for (int b = threadIdx.x; b < nblocks; b += 32) { ss += part[2 * b]; mx = fmax(mx, part[2 * b + 1]); }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) { ss += __shfl_xor_sync(0xffffffffu, ss, o); mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o)); }
+  if (threadIdx.x == 0) { out[0] = ss; out[1] = mx; }
+}
+
+// ---------------------------------------------------------------------------------------------------------
 // K_con (A8): constraints at a point, then warp-shuffle + block reduction to per-tile partials
 // part[tile][6] = {sum C_a^2, sum C_iab^2, sum C_ijab^2, max|C_a|, max|C_iab|, max|C_ijab|};
 // K_con_reduce folds the tiles of each subdomain in a fixed order (deterministic).

@@ -19,7 +19,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libgh.so")
 
 GH_NCOMP = 50
-GH_NUM_KERNELS = 10
+GH_NUM_KERNELS = 12
 GH_FILTER_NONE, GH_FILTER_HEAVISIDE, GH_FILTER_EXP = range(3)
 GH_OK, GH_ERR_ARG, GH_ERR_WORKSPACE, GH_ERR_CUDA, GH_ERR_STATE, GH_ERR_SINGULAR = range(6)
 STATUS_NAMES = ["GH_OK", "GH_ERR_ARG", "GH_ERR_WORKSPACE", "GH_ERR_CUDA", "GH_ERR_STATE", "GH_ERR_SINGULAR"]
@@ -31,6 +31,7 @@ EXPORTS = [
     "gh_constraint_norms", "gh_set_profiling", "gh_profile_read", "gh_profile_reset", "gh_kernel_name",
     "gh_launch_count", "gh_last_error", "gh_basis_cheb", "gh_basis_gauss_legendre", "gh_basis_shell",
     "gh_set_filter", "gh_apply_filter", "gh_filter_sigma",
+    "gh_dp5_workspace_bytes", "gh_dp5_attach", "gh_dp5_step",
 ]
 
 
@@ -113,6 +114,10 @@ def lib() -> C.CDLL:
     L.gh_set_filter.argtypes = [vp, fp, fp]
     L.gh_apply_filter.argtypes = [vp]
     L.gh_filter_sigma.argtypes = [fp, C.c_int32, dp]
+    L.gh_dp5_workspace_bytes.restype = C.c_size_t
+    L.gh_dp5_workspace_bytes.argtypes = [vp]
+    L.gh_dp5_attach.argtypes = [vp, vp, C.c_size_t]
+    L.gh_dp5_step.argtypes = [vp, C.c_double, C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_int)]
     _lib = L
     return L
 
@@ -250,6 +255,22 @@ def gh_filter_sigma(f, kmax: int) -> np.ndarray:
     return out
 
 
+def gh_dp5_workspace_bytes(h) -> int:
+    return int(lib().gh_dp5_workspace_bytes(h))
+
+
+def gh_dp5_attach(h, workspace_ptr: int, nbytes: int):
+    _check(lib().gh_dp5_attach(h, C.c_void_p(workspace_ptr), nbytes), h)
+
+
+def gh_dp5_step(h, dt: float, tol: float = 0.0):
+    """-> (err_rms, err_max, accepted)"""
+    err = (C.c_double * 2)()
+    acc = C.c_int(0)
+    _check(lib().gh_dp5_step(h, float(dt), float(tol), err, C.byref(acc)), h)
+    return float(err[0]), float(err[1]), bool(acc.value)
+
+
 def gh_basis_cheb(N: int):
     x, D = np.zeros(N), np.zeros((N, N))
     _check(lib().gh_basis_cheb(N, x.ctypes.data, D.ctypes.data), None)
@@ -354,6 +375,17 @@ class Domain:
 
     def constraint_norms(self, per_sub: bool = False):
         return gh_constraint_norms(self.h, self.n_sub, per_sub)
+
+    def dp5_attach(self):
+        """Allocate (torch) and attach the workspace of the Dormand-Prince stepper."""
+        import torch
+
+        n = gh_dp5_workspace_bytes(self.h)
+        self._dp_ws = torch.empty(n + 256, dtype=torch.uint8, device=self.device)
+        gh_dp5_attach(self.h, (self._dp_ws.data_ptr() + 255) // 256 * 256, n)
+
+    def dp5_step(self, dt: float, tol: float = 0.0):
+        return gh_dp5_step(self.h, dt, tol)
 
     def set_filter(self, block_axes=None, shell_angular=None):
         gh_set_filter(self.h, block_axes, shell_angular)

@@ -21,7 +21,7 @@ def built():
 
 def test_exports_every_declared_symbol():
     hdr = open(os.path.join(ROOT, "include", "gh.h")).read()
-    declared = set(re.findall(r"\b(gh_[a-z_]+)\s*\(", hdr))
+    declared = set(re.findall(r"\b(gh_[a-z0-9_]+)\s*\(", hdr))
     assert declared == set(gh.EXPORTS)
     L = gh.lib()
     for name in declared:

@@ -235,3 +235,48 @@ def test_filter_parity(case, oracle, fidx):
             assert np.array_equal(got[s], us[s])
     dom.set_filter(None, None)
     dom.set_fields(dom.pack(us), 0.0)
+
+
+# ---- NEXT-3: Dormand-Prince 5(4) ----------------------------------------------------------------------------------------
+def test_dp5_step_parity(case, oracle):
+    """gh_dp5_step against the oracle's step (O11): new state to the S15 bar, the error estimate's rms / max to 1e-9 relative
+    plus the rounding floor; two consecutive steps (the second reuses the last stage as its first) against two oracle steps;
+    a rejected step leaves the state bit-identical."""
+    name, cfg, descs, coords, us, Hs, dom = case
+    if name == "wide":
+        pytest.skip("the long-double oracle needs ~14 RHS evaluations here; covered by the other cases")
+    dt = 0.25 * configs.min_spacing(descs)
+    dom.set_fields(dom.pack(us), 0.0)
+    dom.dp5_attach()
+    rms, mx, acc = dom.dp5_step(dt)
+    assert acc
+    new = dom.unpack(dom.get_fields())
+    refs, errs = zip(*[oracle.dp5(d, us[s], Hs[s], dt) for s, d in enumerate(descs)])
+    for s in range(len(descs)):
+        assert_parity(new[s], refs[s], tol=TOL, what=f"{name} sub {s} dp5")
+    ref_max = max(float(np.abs(e).max()) for e in errs)
+    ref_rms = np.sqrt(sum(float((e ** 2).sum()) for e in errs) / (50 * sum(e.shape[1] for e in errs)))
+    floor = 1e-11 * dt * max(float(np.abs(u).max()) for u in us)
+    assert abs(mx - ref_max) <= 1e-9 * ref_max + floor and abs(rms - ref_rms) <= 1e-9 * ref_rms + floor
+    assert mx > 0
+    # second step: first-same-as-last
+    dom.dp5_step(dt)
+    new2 = dom.unpack(dom.get_fields())
+    for s, d in enumerate(descs):
+        ref2, _ = oracle.dp5(d, refs[s], Hs[s], dt)
+        assert_parity(new2[s], ref2, tol=TOL, what=f"{name} sub {s} dp5 step 2")
+    # a step whose error estimate exceeds the tolerance is not taken
+    before = dom.get_fields().copy()
+    rms3, mx3, acc3 = dom.dp5_step(dt, tol=1e-30)
+    assert not acc3 and mx3 > 1e-30
+    assert np.array_equal(dom.get_fields(), before)
+    dom.set_fields(dom.pack(us), 0.0)
+
+
+def test_dp5_needs_its_workspace():
+    dom = gh.Domain(configs.c1()["descs"])
+    dom.set_fields(np.zeros((50, dom.S)), 0.0)
+    with pytest.raises(gh.GHError) as e:
+        dom.dp5_step(1e-3)
+    assert e.value.status == gh.GH_ERR_STATE
+    dom.close()
