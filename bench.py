@@ -378,8 +378,8 @@ def run_ours(args):
     if not bool(torch.isfinite(out_host).all()):
         raise SystemExit("bench.py: non-finite state after the e2e region")
 
-    filt = time_filter(dom, u_dev, descs) if rank == 0 else None
-    dp5 = time_dp5(dom, u_dev, dt, P) if rank == 0 else None
+    filt = time_filter(dom, u_dev, descs) if rank == 0 and not args.no_extras else None
+    dp5 = time_dp5(dom, u_dev, dt, P) if rank == 0 and not args.no_extras else None
 
     tmax, e2emax = max_over_ranks([ms, e2e_s / e2e_steps], dist, dev)
     if rank != 0:
@@ -559,9 +559,11 @@ def main():
     ap.add_argument("--workload", default="c4", choices=["c1", "c2", "c3", "c4"])
     ap.add_argument("--min-points", type=int, default=4_000_000, help="C4: replicate the base set until P >= this")
     ap.add_argument("--e2e-steps", type=int, default=5)
-    ap.add_argument("--cpu-points", type=int, default=250_000, help="points in the cpu_baseline sample (~10-30 s)")
+    ap.add_argument("--cpu-points", type=int, default=1_300_000,
+                    help="points in the cpu_baseline sample (default: the whole 64-subdomain base set, ~10 s on 16 cores)")
     ap.add_argument("--ref-points", type=int, default=60_000, help="points per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the spectral-filter and Dormand-Prince legs (run after the timed step)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
