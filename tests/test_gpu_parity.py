@@ -280,3 +280,22 @@ def test_dp5_needs_its_workspace():
         dom.dp5_step(1e-3)
     assert e.value.status == gh.GH_ERR_STATE
     dom.close()
+
+
+def test_gradient_parity_at_the_size_limits(oracle):
+    """GH_MAX_L = 47 (the last m-tile count of K_ang S2, one plane group of two planes) and GH_MAX_CHEB_N = 64 on the radial axis."""
+    descs = [configs.shell(2, 47, 3.0, 4.0), configs.shell(64, 3, 2.0, 9.0)]
+    cfg = {"id": 10, "spin": 0.2, "amplitude": 1e-3, "descs": descs}
+    descs, coords, us, Hs = build_case(cfg, oracle)
+    dom = _domain(descs, Hs, us)
+    g = dom.gradient()
+    for s, d in enumerate(descs):
+        ref = oracle.gradient(d, us[s])
+        got = g[:, :, dom.offsets[s]:dom.offsets[s] + dom.sizes[s]]
+        for k in range(3):
+            assert_parity(got[k], ref[k], state=us[s], tol=TOL, what=f"limits sub {s} d_{k}")
+    dom.close()
+    with pytest.raises(gh.GHError):
+        gh.Domain([configs.shell(4, 48, 3.0, 4.0)])
+    with pytest.raises(gh.GHError):
+        gh.Domain([configs.block([65, 4, 4], (0, 0, 0), (1, 1, 1))])
