@@ -15,6 +15,14 @@ def pytest_configure(config):
     config.addinivalue_line("markers", "slow: long-running oracle comparison")
 
 
+@pytest.fixture(scope="session", autouse=True)
+def _library_is_built():
+    """libgh.so is built in-tree (nvcc cross-compiles without a GPU); a no-op when it is newer than its sources."""
+    from paper_1804_09101_b200 import build
+
+    build.build()
+
+
 @pytest.fixture(scope="session")
 def oracle():
     from oracle.gh_oracle import Oracle
