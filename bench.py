@@ -180,12 +180,12 @@ def oracle_sample(base_cfg, budget_points: int = 60_000):
     return pick, pts
 
 
-def time_oracle(base_cfg, pick, steps: int, warmup: int):
+def time_oracle(base_cfg, pick, steps: int, warmup: int, threads=None):
     """One 'step' = one oracle RHS evaluation (Real=double build, OpenMP) of every picked subdomain."""
     from oracle.gh_oracle import Oracle
     from paper_1804_09101_b200 import inputs
 
-    ora = Oracle("double")
+    ora = Oracle("double", threads=threads)
     descs = [base_cfg["descs"][s] for s in pick]
     coords = [ora.coords(d) for d in descs]
     us, Hs = [], []
@@ -207,6 +207,8 @@ def time_oracle(base_cfg, pick, steps: int, warmup: int):
     omp = os.environ.get("OMP_NUM_THREADS")
     if omp:
         cores = min(cores, int(omp))
+    if threads is not None:
+        cores = min(cores, int(threads))
     return pts * steps / dt, dt / steps, cores, pts
 
 
@@ -494,6 +496,11 @@ def finish_ours(args, world, label, cfg, descs, reps, P, S, ms, e2e_step_s, e2e_
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": f"one oracle RHS evaluation (Real=double build, OpenMP) of subdomains {pick} of the workload's base set "
                          f"({pts} points, {s_per:.1f} s)"}
+        # the paper's own comparisons are against ONE CPU core: the same oracle on one thread, smaller sample
+        pick1, _ = oracle_sample(base, max(20_000, args.cpu_points // 20))
+        v1, s1, _, pts1 = time_oracle(base, pick1, 1, 0, threads=1)
+        cpu["single_core"] = {"value": v1, "unit": UNIT, "cores": 1,
+                              "sample": f"subdomains {pick1} ({pts1} points, {s1:.1f} s), one thread"}
 
     h2d = 50 * S * 8
     d2h = 50 * S * 8 + 6 * 8
