@@ -680,6 +680,41 @@ int ora_char_bc_point(const double* psi, const double* gamma, const double* s, d
   return 0;
 }
 
+/* ---------------------------------------------------------------------- */
+/* O12 — characteristic penalty exchange across an internal boundary       */
+/* (NEXT-2 (iii); "internal boundaries ... characteristic"). */
+/* Reading S22: with du = (own - neighbour) state at the coincident point, */
+/* projected on the characteristic fields along the own outward normal,    */
+/*   dt u^a  +=  - p |v_a| (u^a_own - u^a_nbr)    for every field with     */
+/* v_a < 0 (it enters), p = (N_r - 1)^2 / (r_out - r_in) of the own shell  */
+/* (the Chebyshev penalty bound N^2/2 of the reference interval times the  */
+/* map factor 2/Delta); outgoing fields are left alone; then the same back */
+/* map as O10.                                                             */
+/* ---------------------------------------------------------------------- */
+static int char_penalty_point(const real psi[4][4], const real gam[3], const real s[3], real pen, const real dpsi[4][4],
+                              const real dPi[4][4], const real dPhi[3][4][4], real dtpsi[4][4], real dtPi[4][4], real dtPhi[3][4][4]) {
+  geom G; if (geometry(psi, &G)) return 1;
+  real nn = 0; for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) nn += G.ginv[i][j] * s[i] * s[j];
+  nn = R_SQRT(nn);
+  real nd[3], nu[3], nN = 0;
+  for (int i = 0; i < 3; ++i) nd[i] = s[i] / nn;
+  for (int i = 0; i < 3; ++i) { nu[i] = 0; for (int j = 0; j < 3; ++j) nu[i] += G.ginv[i][j] * nd[j]; }
+  for (int k = 0; k < 3; ++k) nN += nd[k] * G.shift[k];
+  real v0 = -(1 + gam[1]) * nN, v1p = -nN + G.lapse, v1m = -nN - G.lapse, v2 = -nN;
+  for (int a = 0; a < 4; ++a) for (int b = 0; b < 4; ++b) {
+    real e3[3] = {dPhi[0][a][b], dPhi[1][a][b], dPhi[2][a][b]};
+    real nPhi = 0; for (int i = 0; i < 3; ++i) nPhi += nu[i] * e3[i];
+    real u0 = dpsi[a][b], u1p = dPi[a][b] + nPhi - gam[2] * dpsi[a][b], u1m = dPi[a][b] - nPhi - gam[2] * dpsi[a][b], u2[3];
+    for (int i = 0; i < 3; ++i) u2[i] = e3[i] - nd[i] * nPhi;
+    real c0 = v0 < 0 ? pen * v0 * u0 : 0, c1p = v1p < 0 ? pen * v1p * u1p : 0, c1m = v1m < 0 ? pen * v1m * u1m : 0;   /* v < 0: -p|v| = p v */
+    real c2[3]; for (int i = 0; i < 3; ++i) c2[i] = v2 < 0 ? pen * v2 * u2[i] : 0;
+    dtpsi[a][b] += c0;
+    dtPi[a][b] += (c1p + c1m) / 2 + gam[2] * c0;
+    for (int i = 0; i < 3; ++i) dtPhi[i][a][b] += (c1p - c1m) / 2 * nd[i] + c2[i];
+  }
+  return 0;
+}
+
 /* outward directions s_i of the faces flagged CHARACTERISTIC (= 2) that contain point p, in face order; returns how many */
 static int char_faces(const ora_subdomain* sd, int64_t p, const real* xyz3 /* x,y,z of the point relative to the shell centre */, real s[6][3]) {
   int n0, n1, n2; dims(sd, &n0, &n1, &n2);
@@ -700,6 +735,9 @@ static int char_faces(const ora_subdomain* sd, int64_t p, const real* xyz3 /* x,
 }
 
 /* real-typed core: u[50][P], H[4][P], gH[12][P] ([i][a]) -> dtu[50][P]. Returns #non-physical points. */
+static const double* g_nbr_in = NULL;    /* neighbour state on the inner / outer face of a shell, [50][n_theta n_phi], set by */
+static const double* g_nbr_out = NULL;   /* ora_rhs_subdomain_ifc around its call (faces flagged INTERFACE = 3) */
+
 static int rhs_real(const ora_subdomain* sd, const real* u, const real* H, const real* gH, real* dtu) {
   int64_t P = ora_num_points(sd);
   real* g = malloc(sizeof(real) * 150 * P);
@@ -717,6 +755,24 @@ static int rhs_real(const ora_subdomain* sd, const real* u, const real* H, const
       real rel[3] = {(real)xyz[p] - (real)sd->center[0], (real)xyz[P + p] - (real)sd->center[1], (real)xyz[2 * P + p] - (real)sd->center[2]};
       real sdir[6][3]; int nf = char_faces(sd, p, rel, sdir);
       for (int f = 0; f < nf; ++f) char_bc_point(in.psi, gam, sdir[f], a, b, c);
+      if (sd->kind == 0) {   /* O12: interface faces of shells */
+        int n0, n1, n2; dims(sd, &n0, &n1, &n2); int64_t pl = (int64_t)n1 * n2, q = p % pl; int i0 = (int)(p / pl);
+        real rr = R_SQRT(rel[0] * rel[0] + rel[1] * rel[1] + rel[2] * rel[2]);
+        real pen = (real)(n0 - 1) * (real)(n0 - 1) / ((real)sd->hi[0] - (real)sd->lo[0]);
+        for (int f = 0; f < 2; ++f) {
+          const double* nb = f == 0 ? g_nbr_in : g_nbr_out;
+          if (!(sd->face[f] == 3 && nb && i0 == (f == 0 ? 0 : n0 - 1))) continue;
+          real sg = f == 0 ? -1 : 1, sv[3] = {sg * rel[0] / rr, sg * rel[1] / rr, sg * rel[2] / rr};
+          real dps[4][4], dPi_[4][4], dPh[3][4][4];
+          for (int x = 0; x < 4; ++x) for (int y = 0; y < 4; ++y) {
+            int sxy = SYM[x][y];
+            dps[x][y] = in.psi[x][y] - (real)nb[(int64_t)sxy * pl + q];
+            dPi_[x][y] = in.Pi[x][y] - (real)nb[(int64_t)(10 + sxy) * pl + q];
+            for (int i = 0; i < 3; ++i) dPh[i][x][y] = in.Phi[i][x][y] - (real)nb[(int64_t)(20 + 10 * i + sxy) * pl + q];
+          }
+          char_penalty_point(in.psi, gam, sv, pen, dps, dPi_, dPh, a, b, c);
+        }
+      }
     }
     for (int x = 0; x < 4; ++x) for (int y = x; y < 4; ++y) {
       int s = SYM[x][y];
@@ -757,6 +813,16 @@ int ora_rhs_subdomain(const ora_subdomain* sd, const double* u, const double* H,
   int bad = rhs_real(sd, ur, Hr, gH, out);
   for (int64_t i = 0; i < 50 * P; ++i) dtu[i] = (double)out[i];
   free(ur); free(Hr); free(gH); free(out);
+  return bad;
+}
+
+/* RHS of one shell coupled to its neighbours (O12): nbr_in / nbr_out = the neighbour's state on the coincident face,
+ * [50][n_theta n_phi], or NULL.  Not re-entrant (the face planes are passed through file-scope pointers). */
+int ora_rhs_subdomain_ifc(const ora_subdomain* sd, const double* u, const double* H, const double* dH, const double* nbr_in,
+                          const double* nbr_out, double* dtu) {
+  g_nbr_in = nbr_in; g_nbr_out = nbr_out;
+  int bad = ora_rhs_subdomain(sd, u, H, dH, dtu);
+  g_nbr_in = NULL; g_nbr_out = NULL;
   return bad;
 }
 

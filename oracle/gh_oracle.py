@@ -100,6 +100,8 @@ class Oracle:
         L.ora_rk3_subdomain.restype = C.c_int
         L.ora_constraints_subdomain.argtypes = [C.POINTER(Subdomain), _dp, _dp, _dp, _dp, C.c_void_p]
         L.ora_constraints_subdomain.restype = C.c_int
+        L.ora_rhs_subdomain_ifc.argtypes = [C.POINTER(Subdomain), _dp, _dp, C.c_void_p, C.c_void_p, C.c_void_p, _dp]
+        L.ora_rhs_subdomain_ifc.restype = C.c_int
         L.ora_dp5_tableau.argtypes = [_dp] * 4
         L.ora_dp5_tableau.restype = None
         L.ora_dp5_subdomain.argtypes = [C.POINTER(Subdomain), _dp, _dp, C.c_void_p, C.c_double, _dp]
@@ -254,6 +256,19 @@ class Oracle:
         if bad:
             raise ValueError(f"{bad} non-physical points")
         return u
+
+    def rhs_ifc(self, sd: dict, u, H, nbr_in=None, nbr_out=None) -> np.ndarray:
+        """O12: RHS of one shell whose INTERFACE faces (flag 3) see the neighbour's face state nbr_*[50, n_theta*n_phi]."""
+        s = make_subdomain(sd)
+        u = np.ascontiguousarray(u, dtype=np.float64)
+        H = np.ascontiguousarray(H, dtype=np.float64)
+        keep = [None if a is None else np.ascontiguousarray(a, dtype=np.float64) for a in (nbr_in, nbr_out)]
+        ptr = [None if a is None else a.ctypes.data for a in keep]
+        out = np.empty_like(u)
+        bad = self.lib.ora_rhs_subdomain_ifc(C.byref(s), u, H, None, ptr[0], ptr[1], out)
+        if bad:
+            raise ValueError(f"{bad} non-physical points")
+        return out
 
     def dp5_tableau(self):
         c, a, b, bh = np.empty(7), np.empty((7, 6)), np.empty(7), np.empty(7)
