@@ -59,8 +59,14 @@ typedef enum { GH_SHELL = 0, GH_BLOCK = 1 } gh_kind;
  * CHARACTERISTIC (NEXT-2 (i); the paper's ApplyBCs module, which it left on the CPU): the time
  * derivatives of the characteristic fields that ENTER through the face are set to zero, the others keep what the evolution
  * equations give (reading S21 writes the fields and speeds out); fused into the RHS kernel.  At block edges the
- * faces are applied in the order -x,+x,-y,+y,-z,+z; a FROZEN face through the same point wins. */
-typedef enum { GH_FACE_FREE = 0, GH_FACE_FROZEN = 1, GH_FACE_CHARACTERISTIC = 2 } gh_face;
+ * faces are applied in the order -x,+x,-y,+y,-z,+z; a FROZEN face through the same point wins.
+ * INTERFACE (NEXT-2 (iii), shells only): the outer face of shell s and the inner face of shell s+1 (the next descriptor) are
+ * one internal boundary: both must carry this flag, and the two shells must share centre, band limit L and the radius
+ * (their face grids then coincide point by point).  Every characteristic field that enters a shell through the face is
+ * relaxed towards the neighbour's value:  d_t u^a += -p |v_a| (u^a_own - u^a_neighbour),  p = (N_r - 1)^2 / (r_out - r_in)
+ * of the own shell (reading S22); outgoing fields are untouched.  Fused into the RHS kernel, which reads the
+ * neighbour's face state straight from the field store. */
+typedef enum { GH_FACE_FREE = 0, GH_FACE_FROZEN = 1, GH_FACE_CHARACTERISTIC = 2, GH_FACE_INTERFACE = 3 } gh_face;
 
 /* One spectral subdomain (PAPER.md:371 I1^3 blocks, PAPER.md:386 I1 x S2 shells). */
 typedef struct {

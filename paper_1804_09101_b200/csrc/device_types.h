@@ -20,6 +20,10 @@ struct SubDev {
   int32_t t_ct, t_st;      // cos/sin(theta_j)     [n1]
   int32_t t_cp, t_sp;      // cos/sin(phi_k)       [n2]
   int32_t pad_;
+  // shells with INTERFACE faces: start (inside a component) of the neighbour's coincident (theta,phi) plane for the inner /
+  // outer face (-1: none) and the penalty factor (N_r - 1)^2 / (r_out - r_in)
+  int64_t nbr[2];
+  double pen;
 };
 
 // One tile of Chebyshev lines: out[a, col] = sum_i D[a][i] in[i, col] for `ncols` columns (A2, Eq. 22).

@@ -114,8 +114,23 @@ bool validate(const gh_subdomain_desc* descs, int32_t n_sub, std::string& err) {
         if (!(d.hi[a] > d.lo[a])) { snprintf(buf, sizeof buf, "subdomain %d: block needs lo < hi on every axis", s); err = buf; return false; }
       }
     } else { snprintf(buf, sizeof buf, "subdomain %d: unknown kind %d", s, d.kind); err = buf; return false; }
-    for (int f = 0; f < 6; ++f)
-      if (d.face[f] != GH_FACE_FREE && d.face[f] != GH_FACE_FROZEN && d.face[f] != GH_FACE_CHARACTERISTIC) { snprintf(buf, sizeof buf, "subdomain %d: bad face flag", s); err = buf; return false; }
+    for (int f = 0; f < 6; ++f) {
+      if (d.face[f] == GH_FACE_INTERFACE && f < 2 && d.kind == GH_SHELL) {
+        // the partner: the previous (inner face) / next (outer face) descriptor, a shell with the same centre and L whose
+        // facing face carries the flag too and sits at the same radius
+        const int o = f == 0 ? s - 1 : s + 1;
+        bool ok = o >= 0 && o < n_sub && descs[o].kind == GH_SHELL && descs[o].n[1] == d.n[1] && descs[o].face[1 - f] == GH_FACE_INTERFACE;
+        if (ok) {
+          const double ra = f == 0 ? d.lo[0] : d.hi[0], rb = f == 0 ? descs[o].hi[0] : descs[o].lo[0];
+          ok = std::fabs(ra - rb) <= 1e-12 * std::fabs(ra);
+          for (int c = 0; c < 3; ++c) ok = ok && descs[o].center[c] == d.center[c];
+        }
+        if (!ok) { snprintf(buf, sizeof buf, "subdomain %d: INTERFACE face %d has no matching neighbour shell", s, f); err = buf; return false; }
+        continue;
+      }
+      if (d.face[f] == GH_FACE_INTERFACE && f < (d.kind == GH_SHELL ? 2 : 6)) { snprintf(buf, sizeof buf, "subdomain %d: interfaces between blocks are not built", s); err = buf; return false; }
+      if (d.face[f] != GH_FACE_FREE && d.face[f] != GH_FACE_FROZEN && d.face[f] != GH_FACE_CHARACTERISTIC && d.face[f] != GH_FACE_INTERFACE) { snprintf(buf, sizeof buf, "subdomain %d: bad face flag", s); err = buf; return false; }
+    }
     for (int g = 0; g < 3; ++g)
       if (!std::isfinite(d.gamma[g])) { snprintf(buf, sizeof buf, "subdomain %d: non-finite gamma", s); err = buf; return false; }
   }
@@ -221,7 +236,7 @@ struct gh_domain {
   double *part = nullptr, *persub = nullptr;
   int* flag = nullptr;
   std::vector<SubDev> h_subs;
-  bool has_fields = false, has_shell = false, has_block = false, has_char = false;
+  bool has_fields = false, has_shell = false, has_block = false, has_char = false, has_ifc = false;
   double t = 0.0;
   int64_t launches = 0;
   std::string err;
@@ -348,6 +363,13 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
     int n0, n1, n2; sub_dims(de, n0, n1, n2);
     sd.kind = de.kind; sd.n0 = n0; sd.n1 = n1; sd.n2 = n2; sd.off = pl.offsets[s]; sd.P = n0 * n1 * n2;
     for (int f = 0; f < 6; ++f) { sd.face[f] = de.face[f]; if (f < (de.kind == GH_SHELL ? 2 : 6) && de.face[f] == GH_FACE_CHARACTERISTIC) d->has_char = true; }
+    sd.nbr[0] = sd.nbr[1] = -1; sd.pen = 0.0;
+    if (de.kind == GH_SHELL) {
+      sd.pen = (double)(n0 - 1) * (double)(n0 - 1) / (de.hi[0] - de.lo[0]);
+      const int64_t plane = (int64_t)n1 * n2;
+      if (de.face[0] == GH_FACE_INTERFACE) { sd.nbr[0] = pl.offsets[s - 1] + (int64_t)(descs[s - 1].n[0] - 1) * plane; d->has_char = d->has_ifc = true; }
+      if (de.face[1] == GH_FACE_INTERFACE) { sd.nbr[1] = pl.offsets[s + 1]; d->has_char = d->has_ifc = true; }
+    }
     for (int g = 0; g < 3; ++g) sd.gamma[g] = de.gamma[g];
     const int naxes = de.kind == GH_SHELL ? 1 : 3;
     const int64_t nn[3] = {n0, n1, n2};
@@ -730,6 +752,14 @@ extern "C" gh_status gh_rk_step(gh_domain* d, double dt) {
   if (!d->has_fields) return fail(d, GH_ERR_STATE, "gh_rk_step before gh_set_fields");
   if (!std::isfinite(dt)) return fail(d, GH_ERR_ARG, "dt is not finite");
   gh_status st;
+  if (d->has_ifc) {
+    // INTERFACE faces read the neighbour's face state from the stage input, so no stage may run in place: ua -> ub -> k -> ua
+    if ((st = launch_rhs(d, d->ua, d->ub, 1, nullptr, 0.0, 1.0, dt)) != GH_OK) return st;
+    if ((st = launch_rhs(d, d->ub, d->k, 2, d->ua, 0.75, 0.25, dt)) != GH_OK) return st;
+    if ((st = launch_rhs(d, d->k, d->ua, 2, d->ua, 1.0 / 3.0, 2.0 / 3.0, dt)) != GH_OK) return st;
+    d->t += dt; d->dp_fsal = false;
+    return GH_OK;
+  }
   // the stage update (A7) is the epilogue of the fused RHS kernel: d_t u never goes to memory
   // u1 = u0 + dt k(u0)                      (ua -> ub)
   if ((st = launch_rhs(d, d->ua, d->ub, 1, nullptr, 0.0, 1.0, dt)) != GH_OK) return st;

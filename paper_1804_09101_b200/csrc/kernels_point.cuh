@@ -342,6 +342,38 @@ __device__ __forceinline__ void char_bc_pair(const Geom& G, double g1, double g2
   for (int i = 0; i < 3; ++i) dPhi[i] = 0.5 * (u1p - u1m) * nd[i] + u2[i];
 }
 
+// Characteristic penalty exchange (NEXT-2 (iii), reading S22) for one symmetric pair at an INTERFACE point: e* = own minus
+// neighbour state; every field entering along the outward direction s gets  d_t u^a += p v_a (u^a_own - u^a_nbr)  (v_a < 0).
+__device__ __forceinline__ void char_penalty_pair(const Geom& G, double g1, double g2, double sx, double sy, double sz, double pen,
+                                                  double epsi, double ePi, const double (&ePhi)[3],
+                                                  double& dpsi, double& dPi, double (&dPhi)[3]) {
+  const double sv[3] = {sx, sy, sz};
+  double gs[3], nn = 0.0;
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    double v = 0.0;
+#pragma unroll
+    for (int j = 0; j < 3; ++j) v = fma(G.gi[S3(i, j)], sv[j], v);
+    gs[i] = v;
+    nn = fma(v, sv[i], nn);
+  }
+  const double inv = 1.0 / sqrt(nn);
+  double nd[3], nu[3], nN = 0.0, nPhi = 0.0;
+#pragma unroll
+  for (int i = 0; i < 3; ++i) { nd[i] = sv[i] * inv; nu[i] = gs[i] * inv; nN = fma(nd[i], G.sh[i], nN); nPhi = fma(nu[i], ePhi[i], nPhi); }
+  const double v0 = -(1.0 + g1) * nN, v1p = -nN + G.N, v1m = -nN - G.N, v2 = -nN;
+  const double c0 = v0 < 0.0 ? pen * v0 * epsi : 0.0;
+  const double c1p = v1p < 0.0 ? pen * v1p * (ePi + nPhi - g2 * epsi) : 0.0;
+  const double c1m = v1m < 0.0 ? pen * v1m * (ePi - nPhi - g2 * epsi) : 0.0;
+  dpsi += c0;
+  dPi += 0.5 * (c1p + c1m) + g2 * c0;
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    const double c2 = v2 < 0.0 ? pen * v2 * (ePhi[i] - nd[i] * nPhi) : 0.0;
+    dPhi[i] += 0.5 * (c1p - c1m) * nd[i] + c2;
+  }
+}
+
 template <int RK>
 __device__ __forceinline__ void rhs_store(double* out, const RkArgs& rk, int64_t idx, double dtu, double us, double u0v) {
   if (RK == 0) { out[idx] = dtu; return; }
@@ -398,6 +430,7 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
     for (int f = 0; f < (SHELL ? 2 : 6); ++f) {
       frozen = frozen || (on[f] && sd.face[f] == 1);
       if (CBC && on[f] && sd.face[f] == 2) cmask |= 1 << f;
+      if (CBC && SHELL && f < 2 && on[f] && sd.face[f] == 3) cmask |= 64 << f;      // INTERFACE faces: bits 6, 7
     }
   }
   constexpr int SLOT = RHS_RING_ROWS * TILE_PTS;
@@ -518,7 +551,20 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
         for (int j = 0; j < 3; ++j) wup = fma(A.w[i][j], up[j], wup);
         o_Phi[i] = sdPhi - N * d[1][i] + N * g2 * (d[0][i] - Phi(i, s)) + 0.5 * N * A.s[i] * Pi[s] + N * wup;
       }
-      if (CBC && cmask) {   // characteristic faces through this point, in face order (rare: face points only)
+      if (CBC && SHELL && (cmask & 192)) {   // INTERFACE faces: the neighbour's state at the coincident point, straight from u
+        const int q = local % (sd.n1 * sd.n2);
+#pragma unroll
+        for (int f = 0; f < 2; ++f)
+          if (cmask & (64 << f)) {
+            const int64_t t = sd.nbr[f] + q;
+            const double sg = f ? 1.0 : -1.0;
+            const double ePhi[3] = {Phi(0, s) - u[(int64_t)(20 + s) * S + t], Phi(1, s) - u[(int64_t)(30 + s) * S + t],
+                                    Phi(2, s) - u[(int64_t)(40 + s) * S + t]};
+            char_penalty_pair(G, g1, g2, sg * J.xr, sg * J.yr, sg * J.zr, sd.pen, psi[s] - u[(int64_t)s * S + t],
+                              Pi[s] - u[(int64_t)(10 + s) * S + t], ePhi, o_psi, r, o_Phi);
+          }
+      }
+      if (CBC && (cmask & 63)) {   // characteristic faces through this point, in face order (rare: face points only)
 #pragma unroll
         for (int f = 0; f < (SHELL ? 2 : 6); ++f)
           if (cmask & (1 << f)) {

@@ -339,3 +339,61 @@ def test_c4_full_size_sampled_parity(oracle):
         o1 = dom.offsets[s + (len(descs) // nbase - 1) * nbase]
         assert np.array_equal(k[:, o0:o0 + n], k[:, o1:o1 + n]) and np.array_equal(new[:, o0:o0 + n], new[:, o1:o1 + n])
     dom.close()
+
+
+# ---- NEXT-2 (iii): characteristic penalty exchange across shell interfaces ------------------------------------------------
+def _interface_case():
+    return {"id": 11, "spin": 0.5, "amplitude": 1e-3,
+            "descs": [configs.shell(6, 5, 2.0, 3.0, face=(0, 3), gamma=[1.0, -1.0, 1.0]),
+                      configs.shell(7, 5, 3.0, 5.0, face=(3, 3), gamma=[1.5, -0.6, 2.0]),
+                      configs.shell(5, 5, 5.0, 9.0, face=(3, 2), gamma=[1.0, -0.3, 0.5]),
+                      configs.block([5, 4, 6], (10.0, -1.0, -1.0), (12.0, 1.0, 1.0))]}
+
+
+def _oracle_rhs_coupled(oracle, descs, us, Hs):
+    """every subdomain's RHS with the neighbours' face planes sliced out of their states (shells 0-1-2 are chained)"""
+    out = []
+    for s, d in enumerate(descs):
+        if d["kind"] != "shell":
+            out.append(oracle.rhs(d, us[s], Hs[s]))
+            continue
+        pl = (d["n"][1] + 1) * (2 * d["n"][1] + 2)
+        nin = us[s - 1][:, -pl:] if d["face"][0] == 3 else None
+        nout = us[s + 1][:, :pl] if d["face"][1] == 3 else None
+        out.append(oracle.rhs_ifc(d, us[s], Hs[s], nbr_in=nin, nbr_out=nout))
+    return out
+
+
+def test_interface_exchange_parity(oracle):
+    cfg = _interface_case()
+    descs, coords, us, Hs = build_case(cfg, oracle)
+    dom = _domain(descs, Hs, us)
+    k = dom.unpack(dom.rhs())
+    ref = _oracle_rhs_coupled(oracle, descs, us, Hs)
+    for s in range(len(descs)):
+        assert_parity(k[s], ref[s], state=us[s], tol=TOL, what=f"interface sub {s} rhs")
+    # the exchange really acts: against uncoupled (FREE) faces the interface planes differ
+    free = [dict(d, face=[0 if f == 3 else f for f in d["face"]]) for d in descs]
+    assert np.max(np.abs(ref[1] - oracle.rhs(free[1], us[1], Hs[1]))) > 1e-6
+    # one SSP-RK3 step: the Shu-Osher combination of three coupled evaluations (composition pinned in test_oracle_rk3.py)
+    dt = 0.25 * configs.min_spacing(descs)
+    k1 = ref
+    u1 = [u + dt * a for u, a in zip(us, k1)]
+    k2 = _oracle_rhs_coupled(oracle, descs, u1, Hs)
+    u2 = [0.75 * u + 0.25 * (v + dt * a) for u, v, a in zip(us, u1, k2)]
+    k3 = _oracle_rhs_coupled(oracle, descs, u2, Hs)
+    un = [u / 3 + (2.0 / 3.0) * (v + dt * a) for u, v, a in zip(us, u2, k3)]
+    dom.set_fields(dom.pack(us), 0.0)
+    dom.rk_step(dt)
+    new = dom.unpack(dom.get_fields())
+    for s in range(len(descs)):
+        assert_parity(new[s], un[s], tol=TOL, what=f"interface sub {s} rk3")
+    dom.close()
+    # pairing rules are enforced
+    bad = [configs.shell(6, 5, 2.0, 3.0, face=(0, 3)), configs.shell(7, 6, 3.0, 5.0, face=(3, 0))]       # different L
+    with pytest.raises(gh.GHError):
+        gh.Domain(bad)
+    with pytest.raises(gh.GHError):
+        gh.Domain([configs.shell(6, 5, 2.0, 3.0, face=(0, 3)), configs.shell(7, 5, 3.5, 5.0, face=(3, 0))])   # radii do not meet
+    with pytest.raises(gh.GHError):
+        gh.Domain([configs.block(5, (0, 0, 0), (1, 1, 1), face=(3, 0, 0, 0, 0, 0))])
