@@ -1,5 +1,6 @@
 """Long evolution of the C3 domain (8 concentric shells around a Kerr-Schild hole, a = 0.7, 1e-5 perturbation) with the
-four combinations of boundary treatment (FROZEN / CHARACTERISTIC faces, readings S11, S21) and angular spectral
+combinations of boundary treatment (FROZEN / CHARACTERISTIC faces on decoupled shells, or shells coupled through INTERFACE
+faces, readings S11, S21, S22) and angular spectral
 filter (off / exponential in l, reading S20).  The paper's test problem "remains stable for at least several thousand
 timesteps" with its filter and boundary modules on; this shows which of the library's pieces that takes.
 
@@ -20,7 +21,10 @@ def run(face_flag: int, use_filter: bool, nsteps: int, checkpoints):
     cfg = configs.c3()
     descs = [dict(d) for d in cfg["descs"]]
     for s, d in enumerate(descs):
-        d["face"] = [0 if s == 0 else face_flag, face_flag, 0, 0, 0, 0]      # innermost inner face stays FREE (excision)
+        if face_flag == 3:     # shells coupled through INTERFACE faces, CHARACTERISTIC outermost face
+            d["face"] = [0 if s == 0 else 3, 3 if s + 1 < len(descs) else 2, 0, 0, 0, 0]
+        else:
+            d["face"] = [0 if s == 0 else face_flag, face_flag, 0, 0, 0, 0]  # innermost inner face stays FREE (excision)
     dom = gh.Domain(descs)
     coords = dom.coords()
     us, Hs = inputs.initial_data(descs, coords, cfg["spin"], cfg["amplitude"], cfg["id"])
@@ -51,7 +55,7 @@ def main():
     ap.add_argument("--steps", type=int, default=2000)
     args = ap.parse_args()
     cps = sorted({0, 100, args.steps // 4, args.steps // 2, args.steps})
-    for flag, name in ((1, "FROZEN"), (2, "CHARACTERISTIC")):
+    for flag, name in ((1, "FROZEN"), (2, "CHARACTERISTIC"), (3, "INTERFACE between shells, CHARACTERISTIC outside")):
         for filt in (False, True):
             rows = run(flag, filt, args.steps, cps)
             print(f"faces {name}, l-filter {'on' if filt else 'off'}:")
