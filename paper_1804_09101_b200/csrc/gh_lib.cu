@@ -84,6 +84,24 @@ inline int ang_best_nch(int NT, int MT1, int NW, int w, int per_max) {
   }
   return best;
 }
+// Modelled duration of one K_ang CTA (units: one DMMA slot of a warp) for `np_` planes of band limit L on NW warps: per stage
+// the number of rounds the warps need times the DMMAs of one unit, plus a fixed part for staging and barriers.  Used only
+// to choose the planes per CTA and the CTA class of a shell; the S1 / S3 chunkings are the ones the kernel will use.
+constexpr double ANG_FIX = 40.0;     // fixed part of a CTA (staging, barriers), in DMMA slots; 10-300 measured, flat optimum near 40
+constexpr double ANG_C0W = 2.0;      // class 0 runs two CTAs per SM
+inline double ang_cta_cost(int L, int np_, int NW) {
+  const AngDims D = ang_dims(L);
+  const int nt = L + 1, MT1 = (np_ * nt + 7) / 8;
+  const int nche = ang_best_nch(D.NTc, MT1, NW, 1, ANG_NTC), ncho = ang_best_nch(D.NTs, MT1, NW, 1, ANG_NTC);
+  const int nch3 = ang_best_nch(D.NT3, MT1, NW, 4, ANG_NTC3);
+  const int pere = (D.NTc + nche - 1) / nche, pero = (D.NTs + ncho - 1) / ncho, per3 = (D.NT3 + nch3 - 1) / nch3;
+  const double c1 = (double)((MT1 * (nche + ncho) + NW - 1) / NW) * std::max(D.KSe1 * pere, D.KSo1 * pero);
+  const int hh = (nt + 1) / 2, MTH = (2 * hh + 7) / 8, KSh = (hh + 3) / 4, NTn = (2 * np_ + 7) / 8;
+  const int units2 = (L + 1) * NTn - ((NTn == 2 && np_ <= 8) ? 1 : 0);
+  const double c2 = (double)((units2 + NW - 1) / NW) * (KSh * 2 * MTH);
+  const double c3 = (double)((MT1 * nch3 + NW - 1) / NW) * ((D.KSe3 + D.KSo3) * per3 * 2);
+  return c1 + c2 + c3 + ANG_FIX;
+}
 inline size_t ang_smem_bytes(int L, int nb) { return ang_smem_doubles(L, nb) * sizeof(double); }
 inline size_t shell_fa_doubles(int L) { return ang_fa_doubles(L); }   // (even | odd) analysis fragments
 inline size_t shell_fs_doubles(int L) { return ang_fs_doubles(L); }   // (even | odd) synthesis fragments
@@ -173,19 +191,24 @@ bool make_plan(const gh_subdomain_desc* descs, int32_t n_sub, Plan& pl, std::str
       const int L = d.n[1];
       tab += (size_t)round_up(n0, 2) + 2 * (size_t)round_up(n1, 2) + 2 * (size_t)round_up(n2, 2);
       if (!seenL.count(L)) { seenL[L] = 1; tab += shell_matrix_doubles(L); pl.ftable_doubles += shell_g_doubles(L); }
-      // planes per CTA: the most (<= 8) that keep two CTAs on an SM if that is at least 4, else the most that fit
+      // planes per CTA and CTA class (0: 256 threads, two CTAs per SM; 1: 512 threads, one CTA per SM): of all that fit in
+      // shared memory, the pair with the smallest modelled time for the whole shell (sum over its CTAs / CTAs per SM).
+      // Against "the most planes that fit" this is worth 3 % of K_ang on C4 (tile quantisation over the warps).
       int pb = 0, cls = 0;
-#ifndef GH_ANG_MIN0
-#define GH_ANG_MIN0 4
-#endif
-#ifndef GH_ANG_CAP1
-#define GH_ANG_CAP1 8
-#endif
-      for (int nb = ANG_NB_MAX; nb >= GH_ANG_MIN0; --nb) if (ang_smem_bytes(L, nb) <= ANG_SMEM_2CTA) { pb = nb; break; }
-      if (!pb) { cls = 1; for (int nb = GH_ANG_CAP1; nb >= 1; --nb) if (ang_smem_bytes(L, nb) <= SMEM_MAX) { pb = nb; break; } }
+      {
+        double best = 1e300;
+        for (int c = 0; c < 2; ++c)
+          for (int nb = 1; nb <= ANG_NB_MAX; ++nb) {
+            if (ang_smem_bytes(L, nb) > (c == 0 ? ANG_SMEM_2CTA : SMEM_MAX)) continue;
+            const int NW = (c == 0 ? ANG_TPB0 : ANG_TPB1) / 32;
+            double t = 0;
+            for (int p0 = 0; p0 < n0; p0 += nb) t += ang_cta_cost(L, std::min(nb, n0 - p0), NW);
+            t /= (c == 0 ? ANG_C0W : 1.0);
+            if (t < best) { best = t; pb = nb; cls = c; }
+          }
+      }
       if (!pb) { err = "shell L too large for shared memory"; return false; }
       const int chunks = (n0 + pb - 1) / pb;
-      pb = (n0 + chunks - 1) / chunks;            // near-equal chunks
       pl.ang_pb[s] = pb; pl.ang_class[s] = cls;
       pl.n_ang_items += chunks; pl.n_ang_class[cls] += chunks;
       pl.ang_smem[cls] = std::max(pl.ang_smem[cls], ang_smem_bytes(L, pb));
