@@ -40,7 +40,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     tmp = LIB + f".tmp{os.getpid()}"
-    extra = os.environ.get("GH_NVCC_EXTRA", "").split()      # tuning experiments only (e.g. -DGH_GAM_FLY=0)
+    extra = os.environ.get("GH_NVCC_EXTRA", "").split()      # extra nvcc flags, for experiments
     cmd = [nvcc, *NVCC_FLAGS, *extra, *(["-Xptxas", "-v"] if verbose else []), *[os.path.join(CSRC, s) for s in SOURCES], "-o", tmp]
     res = subprocess.run(cmd, capture_output=True, text=True)
     if res.returncode != 0:

@@ -22,14 +22,10 @@ using namespace ghd;
 namespace {
 
 constexpr int CHEB_TPB = 128;                     // K_cheb: 4 warps
-#ifndef GH_CHEB_WALK
-#define GH_CHEB_WALK 25
-#endif
-#ifndef GH_CHEB_NTW0
-#define GH_CHEB_NTW0 2
-#endif
-constexpr int CHEB_COMP_WALK = GH_CHEB_WALK;      // components one K_cheb CTA walks over
-constexpr int CHEB_NTW0 = GH_CHEB_NTW0, CHEB_NTW1 = 2;       // n-tiles per warp: class 0 (N <= 32), class 1 (N <= 64)
+// measured on C4 (ms per call): 4 n-tiles per warp and 5 components per CTA 1.50; 2 and 5: 1.33; 2 and 10: 1.28; 2 and 25: 1.25;
+// 2 and 50: 1.28; 1 n-tile per warp: 1.41-1.47
+constexpr int CHEB_COMP_WALK = 25;                // components one K_cheb CTA walks over
+constexpr int CHEB_NTW0 = 2, CHEB_NTW1 = 2;       // n-tiles per warp: class 0 (N <= 32), class 1 (N <= 64)
 constexpr int CHEB_CT0 = (CHEB_TPB / 32) * 8 * CHEB_NTW0, CHEB_CT1 = (CHEB_TPB / 32) * 8 * CHEB_NTW1;   // columns per CTA
 inline int cheb_class(int N) { return N <= 32 ? 0 : 1; }
 inline int cheb_ct(int N) { return cheb_class(N) ? CHEB_CT1 : CHEB_CT0; }
@@ -178,8 +174,6 @@ bool make_plan(const gh_subdomain_desc* descs, int32_t n_sub, Plan& pl, std::str
     const int naxes = d.kind == GH_SHELL ? 1 : 3;
     for (int a = 0; a < naxes; ++a) {
       const int N = d.n[a];
-      const int nn[3] = {n0, n1, n2};
-      (void)nn;
       tab += cheb_frag_doubles(N);
       const int64_t cols = Ps / N;
       const int items = (int)((cols + cheb_ct(N) - 1) / cheb_ct(N));
