@@ -36,9 +36,12 @@
  * single Chebyshev modes and single Y_lm scaled by sigma, sigma = 1 identity /
  * projection, Heaviside idempotence, linearity; characteristic boundary condition
  * (O10): eigenvectors of the RHS's principal part; Dormand-Prince step (O11): the
- * order conditions of the tableau and 5th-order convergence on the gauge wave.  PARITY UNPINNED (pure
- * conventions, fixed by DESIGN.md): the normalisation of the constraint norms
- * (unweighted RMS over points and components) and the default gamma's.
+ * order conditions of the tableau and 5th-order convergence on the gauge wave;
+ * interface exchange (O12): projection of what it adds onto the characteristic fields.
+ * PARITY UNPINNED (pure conventions, fixed by DESIGN.md): the normalisation of the
+ * constraint norms (unweighted RMS over points and components), the default gamma's,
+ * and the VALUE of the interface penalty factor p = (N_r-1)^2/(r_out-r_in) of O12 (its
+ * structure - which fields, which sign, proportional to |v| - is pinned).
  */
 #include <math.h>
 #include <stdint.h>
