@@ -1,7 +1,7 @@
 """Size sweep of gh_rhs (BASELINE.json configs[4]): single shells with N_r = L+1 = n, single cubes
 N^3, and the paper's "SingleBH" / "BBH" shell prescriptions, Kerr-Schild a = 0.5 + seeded 1e-4 perturbation.
 
-    python -m paper_1804_09101_b200.sweep [--reps 20] [--markdown]
+    python -m paper_1804_09101_b200.sweep [--reps 20] [--markdown] [--fill 2000000]
 
 Per member: points, gh_rhs time (median of `reps` after 5 warm-ups, CUDA events on the library's stream via its
 profiling interface), grid-point evaluations/s, derivative-kernel FP64 rate (algorithmic flop of DESIGN.md §6 over
@@ -31,17 +31,19 @@ def members():
     return out
 
 
-def run_member(label, cfg, reps, device="cuda:0"):
+def run_member(label, cfg, reps, device="cuda:0", fill_points=0):
     import torch
 
-    from . import gh, inputs, opcount
+    from . import configs, gh, inputs, opcount
 
-    descs = cfg["descs"]
+    base = cfg["descs"]
+    copies = max(1, -(-fill_points // configs.num_points(base[0]))) if fill_points else 1
+    descs = [dict(base[0]) for _ in range(copies)]          # independent replicas of the member (throughput regime)
     dom = gh.Domain(descs, device=device)
-    coords = dom.coords()
-    us, Hs = inputs.initial_data(descs, coords, cfg["spin"], cfg["amplitude"], cfg["id"])
-    dom.set_gauge_source(dom.pack(Hs))
-    dom.set_fields(dom.pack(us), 0.0)
+    coords = dom.coords()[:1]
+    us, Hs = inputs.initial_data(base, coords, cfg["spin"], cfg["amplitude"], cfg["id"])
+    dom.set_gauge_source(dom.pack([Hs[0]] * copies))
+    dom.set_fields(dom.pack([us[0]] * copies), 0.0)
     out = dom.empty(50)
     for _ in range(5):
         dom.rhs(out)
@@ -60,14 +62,14 @@ def run_member(label, cfg, reps, device="cuda:0"):
     d = descs[0]
     if d["kind"] == "shell":
         n_r, L = d["n"][0], d["n"][1]
-        flop = opcount.shell_factored_flop(50, n_r, L)
-        flop_paper = opcount.shell_deriv_dense(50, n_r, L + 1, 2 * L + 2)[1]
+        flop = copies * opcount.shell_factored_flop(50, n_r, L)
+        flop_paper = copies * opcount.shell_deriv_dense(50, n_r, L + 1, 2 * L + 2)[1]
     else:
-        flop = opcount.block_deriv(50, *d["n"])[1]
+        flop = copies * opcount.block_deriv(50, *d["n"])[1]
         flop_paper = flop
     ms, ms_d, ms_r = float(np.median(tot)), float(np.median(der)), float(np.median(rhs))
     dom.close()
-    return {"member": label, "points": P, "gh_rhs_ms": ms, "points_per_s": P / (ms * 1e-3),
+    return {"member": label + (f" x{copies}" if copies > 1 else ""), "points": P, "gh_rhs_ms": ms, "points_per_s": P / (ms * 1e-3),
             "deriv_ms": ms_d, "deriv_TFLOPs": flop / (ms_d * 1e-3) / 1e12,
             "deriv_TFLOPs_paper_convention": flop_paper / (ms_d * 1e-3) / 1e12,
             "k_rhs_ms": ms_r, "k_rhs_GBps": 2128.0 * P / (ms_r * 1e-3) / 1e9}
@@ -77,11 +79,13 @@ def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--reps", type=int, default=20)
     ap.add_argument("--markdown", action="store_true")
+    ap.add_argument("--fill", type=int, default=0,
+                    help="replicate each member until it has at least this many points (throughput regime; 0: single subdomain, latency regime)")
     args = ap.parse_args()
     from . import build
 
     build.build()
-    rows = [run_member(lbl, cfg, args.reps) for lbl, cfg in members()]
+    rows = [run_member(lbl, cfg, args.reps, fill_points=args.fill) for lbl, cfg in members()]
     if args.markdown:
         print("| member | points | gh_rhs ms | points/s | deriv ms | deriv TFLOP/s (executed map) | deriv TFLOP/s (paper's dense count) | k_rhs ms | k_rhs GB/s |")
         print("|---|---|---|---|---|---|---|---|---|")
