@@ -32,7 +32,9 @@ inline int cheb_ct(int N) { return cheb_class(N) ? CHEB_CT1 : CHEB_CT0; }
 inline size_t cheb_frag_doubles(int N) { return (size_t)((N + 7) / 8) * ((N + 3) / 4) * 32; }   // D in fragment order
 constexpr int ANG_TPB0 = 256, ANG_TPB1 = 512;    // K_ang threads: class 0 (two CTAs per SM), class 1 (one CTA per SM)
 constexpr size_t ANG_SMEM_2CTA = 113 * 1024;     // K_ang shared memory that still lets two CTAs share an SM
-constexpr int ANG_NB_MAX = 8;                    // planes per K_ang CTA (S2 holds 2*nb <= 16 columns per m)
+constexpr int ANG_NB_MAX = 8;                    // planes per K_ang CTA offered to the plan (S2 then has <= 2 column tiles per m)
+constexpr int ANG_NB_MAX_SMALL_L = 24;           // ... for L < 12, where a plane is a few tiles only (SingleBH k = 0: 5.96 -> 4.91 ms
+                                                 // per 2e6 points; for L >= 12 more than 8 planes measured slightly slower on C4)
 constexpr size_t SMEM_MAX = 227 * 1024;
 
 thread_local std::string g_create_error;
@@ -192,7 +194,7 @@ bool make_plan(const gh_subdomain_desc* descs, int32_t n_sub, Plan& pl, std::str
       {
         double best = 1e300;
         for (int c = 0; c < 2; ++c)
-          for (int nb = 1; nb <= ANG_NB_MAX; ++nb) {
+          for (int nb = 1; nb <= (L < 12 ? ANG_NB_MAX_SMALL_L : ANG_NB_MAX); ++nb) {
             if (ang_smem_bytes(L, nb) > (c == 0 ? ANG_SMEM_2CTA : SMEM_MAX)) continue;
             const int NW = (c == 0 ? ANG_TPB0 : ANG_TPB1) / 32;
             double t = 0;
