@@ -20,6 +20,8 @@ def members():
     from . import configs
 
     out = []
+    # the paper's whole-code test problem: 2 shells of (10, 19, 38) points; only its first shell is replicated by --fill
+    out.append(("paper test problem, 2 shells (10,19,38)", configs.paper_two_shells()))
     for n in (8, 16, 24, 32, 40, 48):
         out.append((f"shell n={n} (N_r={n}, L={n - 1})", configs.c5_shell(n)))
     for N in (10, 16, 20, 32, 40, 64):
@@ -38,12 +40,14 @@ def run_member(label, cfg, reps, device="cuda:0", fill_points=0):
 
     base = cfg["descs"]
     copies = max(1, -(-fill_points // configs.num_points(base[0]))) if fill_points else 1
-    descs = [dict(base[0]) for _ in range(copies)]          # independent replicas of the member (throughput regime)
+    if copies > 1:
+        base = base[:1]
+    descs = [dict(d) for _ in range(copies) for d in base]   # independent replicas of the member (throughput regime)
     dom = gh.Domain(descs, device=device)
-    coords = dom.coords()[:1]
+    coords = dom.coords()[:len(base)]
     us, Hs = inputs.initial_data(base, coords, cfg["spin"], cfg["amplitude"], cfg["id"])
-    dom.set_gauge_source(dom.pack([Hs[0]] * copies))
-    dom.set_fields(dom.pack([us[0]] * copies), 0.0)
+    dom.set_gauge_source(dom.pack(list(Hs) * copies))
+    dom.set_fields(dom.pack(list(us) * copies), 0.0)
     out = dom.empty(50)
     for _ in range(5):
         dom.rhs(out)
@@ -59,14 +63,15 @@ def run_member(label, cfg, reps, device="cuda:0", fill_points=0):
     dom.set_profiling(False)
     torch.cuda.synchronize()
     P = dom.P
-    d = descs[0]
-    if d["kind"] == "shell":
-        n_r, L = d["n"][0], d["n"][1]
-        flop = copies * opcount.shell_factored_flop(50, n_r, L)
-        flop_paper = copies * opcount.shell_deriv_dense(50, n_r, L + 1, 2 * L + 2)[1]
-    else:
-        flop = copies * opcount.block_deriv(50, *d["n"])[1]
-        flop_paper = flop
+    flop = flop_paper = 0
+    for d in descs:
+        if d["kind"] == "shell":
+            n_r, L = d["n"][0], d["n"][1]
+            flop += opcount.shell_factored_flop(50, n_r, L)
+            flop_paper += opcount.shell_deriv_dense(50, n_r, L + 1, 2 * L + 2)[1]
+        else:
+            flop += opcount.block_deriv(50, *d["n"])[1]
+            flop_paper += opcount.block_deriv(50, *d["n"])[1]
     ms, ms_d, ms_r = float(np.median(tot)), float(np.median(der)), float(np.median(rhs))
     dom.close()
     return {"member": label + (f" x{copies}" if copies > 1 else ""), "points": P, "gh_rhs_ms": ms, "points_per_s": P / (ms * 1e-3),
