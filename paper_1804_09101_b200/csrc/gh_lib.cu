@@ -25,10 +25,11 @@ constexpr int CHEB_TPB = 128;                     // K_cheb: 4 warps
 // measured on C4 (ms per call): 4 n-tiles per warp and 5 components per CTA 1.50; 2 and 5: 1.33; 2 and 10: 1.28; 2 and 25: 1.25;
 // 2 and 50: 1.28; 1 n-tile per warp: 1.41-1.47
 constexpr int CHEB_COMP_WALK = 25;                // components one K_cheb CTA walks over
-constexpr int CHEB_NTW0 = 2, CHEB_NTW1 = 2;       // n-tiles per warp: class 0 (N <= 32), class 1 (N <= 64)
-constexpr int CHEB_CT0 = (CHEB_TPB / 32) * 8 * CHEB_NTW0, CHEB_CT1 = (CHEB_TPB / 32) * 8 * CHEB_NTW1;   // columns per CTA
-inline int cheb_class(int N) { return N <= 32 ? 0 : 1; }
-inline int cheb_ct(int N) { return cheb_class(N) ? CHEB_CT1 : CHEB_CT0; }
+constexpr int CHEB_NTW = 2;                       // n-tiles per warp
+constexpr int CHEB_CT = (CHEB_TPB / 32) * 8 * CHEB_NTW;   // columns per CTA
+constexpr int CHEB_NCLASS = 3;                    // register-tile classes: N <= 32 (5 CTAs per SM), N <= 48 (4), N <= 64 (3)
+inline int cheb_class(int N) { return N <= 32 ? 0 : N <= 48 ? 1 : 2; }
+inline int cheb_ct(int) { return CHEB_CT; }
 inline size_t cheb_frag_doubles(int N) { return (size_t)((N + 7) / 8) * ((N + 3) / 4) * 32; }   // D in fragment order
 constexpr int ANG_TPB0 = 256, ANG_TPB1 = 512;    // K_ang threads: class 0 (two CTAs per SM), class 1 (one CTA per SM)
 constexpr size_t ANG_SMEM_2CTA = 113 * 1024;     // K_ang shared memory that still lets two CTAs share an SM
@@ -55,8 +56,8 @@ struct Plan {
   int n_tiles = 0;
   size_t table_doubles = 0;
   size_t ftable_doubles = 0;             // spectral-filter matrices, directly behind the derivative tables
-  int n_fcheb[3][2] = {{0, 0}, {0, 0}, {0, 0}}, n_fcheb_items = 0;   // filter work items of the blocks per axis and class
-  int n_cheb_items = 0, n_cheb_class[2] = {0, 0}, n_ang_items = 0;
+  int n_fcheb[3][CHEB_NCLASS] = {}, n_fcheb_items = 0;   // filter work items of the blocks per axis and class
+  int n_cheb_items = 0, n_cheb_class[CHEB_NCLASS] = {}, n_ang_items = 0;
   int n_ang_class[2] = {0, 0};           // K_ang items per shared-memory class (0: two CTAs per SM, 1: one)
   size_t cheb_smem = 0, ang_smem[2] = {0, 0};
   std::vector<int> ang_pb;               // planes per CTA for each subdomain (0 for blocks)
@@ -366,8 +367,8 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
 
   // ---- tables and work lists on the host ----
   std::vector<double> tab(pl.table_doubles, 0.0);
-  std::vector<ChebItem> cheb, cheb1; cheb.reserve(pl.n_cheb_items);   // class 0 items, class 1 items (appended below)
-  std::vector<ChebItem> fch[3][2];       // spectral-filter items of the blocks per axis and class
+  std::vector<ChebItem> cheb, chebc[CHEB_NCLASS];   // items per class (concatenated below)
+  std::vector<ChebItem> fch[3][CHEB_NCLASS];       // spectral-filter items of the blocks per axis and class
   size_t ftp = pl.table_doubles;         // running offset inside the filter-table region
   std::vector<AngItem> ang, ang1; ang.reserve(pl.n_ang_items);   // class 0 items, class 1 items (appended below)
   d->h_subs.resize(n_sub);
@@ -420,7 +421,7 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
         if (a == 0) { it.col_inner = (int)(nn[1] * nn[2]); it.outer_stride = 0; }
         else if (a == 1) { it.col_inner = (int)nn[2]; it.outer_stride = nn[1] * nn[2]; }
         else { it.col_inner = 1; it.outer_stride = nn[2]; }
-        (cheb_class(N) ? cheb1 : cheb).push_back(it);
+        chebc[cheb_class(N)].push_back(it);
         if (de.kind == GH_BLOCK) { ChebItem fi = it; fi.dmat = (int)ftp; fi.axis = 0; fch[a][cheb_class(N)].push_back(fi); }
       }
       if (de.kind == GH_BLOCK) { d->f_blocks.push_back({N, 0.0, ftp}); ftp += cheb_frag_doubles(N); }
@@ -524,9 +525,9 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
     }
   }
   ang.insert(ang.end(), ang1.begin(), ang1.end());
-  cheb.insert(cheb.end(), cheb1.begin(), cheb1.end());
+  for (int c = 0; c < CHEB_NCLASS; ++c) cheb.insert(cheb.end(), chebc[c].begin(), chebc[c].end());
   std::vector<ChebItem> fcheb;
-  for (int a = 0; a < 3; ++a) for (int c = 0; c < 2; ++c) fcheb.insert(fcheb.end(), fch[a][c].begin(), fch[a][c].end());
+  for (int a = 0; a < 3; ++a) for (int c = 0; c < CHEB_NCLASS; ++c) fcheb.insert(fcheb.end(), fch[a][c].begin(), fch[a][c].end());
   if (tp != pl.table_doubles || (int)cheb.size() != pl.n_cheb_items || (int)ang.size() != pl.n_ang_items ||
       (int)fcheb.size() != pl.n_fcheb_items || ftp != pl.table_doubles + pl.ftable_doubles) {
     delete d; return fail(nullptr, GH_ERR_STATE, "internal: plan and build disagree");
@@ -636,6 +637,18 @@ gh_status check_flag(gh_domain* d) {   // stream must be synchronised by the cal
 
 // A2 + A3: logical derivatives of `ncomp` components of `in` into out[3][ncomp][S]
 // (blocks: d/dx, d/dy, d/dz already Cartesian; shells: d/dr, d/dtheta, d/dphi).
+// one K_cheb launch over the n items of register-tile class c (N <= 32: 4 x 8 tiles of D; N <= 48: 6 x 12; N <= 64: 8 x 16)
+void launch_cheb_class(gh_domain* d, int prof_cls, int c, const ChebItem* items, int n, int gy, const double* in, double* out,
+                       int nrun, const CompMap& cm) {
+  if (!n) return;
+  const Plan& pl = d->pl;
+  ProfScope ps(d, prof_cls);
+  const dim3 grid(n, gy);
+  if (c == 0) k_cheb<CHEB_TPB, 4, 8, CHEB_NTW><<<grid, CHEB_TPB, pl.cheb_smem, d->stream>>>(items, d->tables, in, out, pl.S, nrun, cm);
+  else if (c == 1) k_cheb<CHEB_TPB, 6, 12, CHEB_NTW><<<grid, CHEB_TPB, pl.cheb_smem, d->stream>>>(items, d->tables, in, out, pl.S, nrun, cm);
+  else k_cheb<CHEB_TPB, 8, 16, CHEB_NTW><<<grid, CHEB_TPB, pl.cheb_smem, d->stream>>>(items, d->tables, in, out, pl.S, nrun, cm);
+}
+
 gh_status launch_derivs(gh_domain* d, const double* in, double* out, int ncomp, int skip_lo = 0, int skip_n = 0) {
   const Plan& pl = d->pl;
   const CompMap cm{ncomp, skip_lo, skip_n};        // `in` / `out` have ncomp components, of which skip_n are left out
@@ -646,16 +659,8 @@ gh_status launch_derivs(gh_domain* d, const double* in, double* out, int ncomp, 
   for (int w = CHEB_COMP_WALK; w >= 1; --w)
     if (nrun % w == 0 && (w == 1 || (int64_t)pl.n_cheb_items * (nrun / w) >= 4 * 148)) { walk = w; break; }
   const int cheb_gy = nrun / walk;
-  if (pl.n_cheb_class[0]) {
-    ProfScope ps(d, GH_K_CHEB);
-    k_cheb<CHEB_TPB, 4, 8, CHEB_NTW0><<<dim3(pl.n_cheb_class[0], cheb_gy), CHEB_TPB, pl.cheb_smem, d->stream>>>(
-        d->cheb, d->tables, in, out, pl.S, nrun, cm);
-  }
-  if (pl.n_cheb_class[1]) {
-    ProfScope ps(d, GH_K_CHEB);
-    k_cheb<CHEB_TPB, 8, 16, CHEB_NTW1><<<dim3(pl.n_cheb_class[1], cheb_gy), CHEB_TPB, pl.cheb_smem, d->stream>>>(
-        d->cheb + pl.n_cheb_class[0], d->tables, in, out, pl.S, nrun, cm);
-  }
+  for (int c = 0, first = 0; c < CHEB_NCLASS; first += pl.n_cheb_class[c], ++c)
+    launch_cheb_class(d, GH_K_CHEB, c, d->cheb + first, pl.n_cheb_class[c], cheb_gy, in, out, nrun, cm);
   for (int cls = 0, first = 0; cls < 2; first += pl.n_ang_class[cls], ++cls) {
     if (!pl.n_ang_class[cls]) continue;
     ProfScope ps(d, GH_K_SHELL_ANG);
@@ -923,18 +928,8 @@ extern "C" gh_status gh_apply_filter(gh_domain* d) {
     double* dst[3] = {d->du, d->du + (size_t)NCOMP * pl.S, d->ua};
     int first = 0;
     for (int a = 0; a < 3; ++a) {
-      if (pl.n_fcheb[a][0]) {
-        ProfScope ps(d, GH_K_FILTER_CHEB);
-        k_cheb<CHEB_TPB, 4, 8, CHEB_NTW0><<<dim3(pl.n_fcheb[a][0], gy), CHEB_TPB, pl.cheb_smem, d->stream>>>(
-            d->fcheb + first, d->tables, src[a], dst[a], pl.S, NCOMP, cm);
-      }
-      first += pl.n_fcheb[a][0];
-      if (pl.n_fcheb[a][1]) {
-        ProfScope ps(d, GH_K_FILTER_CHEB);
-        k_cheb<CHEB_TPB, 8, 16, CHEB_NTW1><<<dim3(pl.n_fcheb[a][1], gy), CHEB_TPB, pl.cheb_smem, d->stream>>>(
-            d->fcheb + first, d->tables, src[a], dst[a], pl.S, NCOMP, cm);
-      }
-      first += pl.n_fcheb[a][1];
+      for (int c = 0; c < CHEB_NCLASS; first += pl.n_fcheb[a][c], ++c)
+        launch_cheb_class(d, GH_K_FILTER_CHEB, c, d->fcheb + first, pl.n_fcheb[a][c], gy, src[a], dst[a], NCOMP, cm);
     }
   }
   if (d->filt_shells) {

@@ -31,13 +31,16 @@ def _mini_mixed():
 
 def _wide():
     """sizes that reach the other kernel classes: L = 31 and 23 (L = 7 mod 8: the raw-row pitch is set by n_phi + 1; L = 31
-    uses the 512-thread K_ang class), Chebyshev axes with N > 32 (second K_cheb instantiation), odd and tiny extents."""
+    uses the 512-thread K_ang class), Chebyshev axes in all three K_cheb classes and on both sides of their limits (32 | 33,
+    48 | 49, 64), odd and tiny extents."""
     return {"id": 8, "spin": 0.6, "amplitude": 1e-4,
             "descs": [configs.shell(5, 31, 2.5, 3.5, face=(1, 0)),
                       configs.shell(6, 23, 3.5, 6.0, face=(0, 0), gamma=[2.0, -0.5, 1.5]),
                       configs.block([33, 7, 9], (3.0, -1.0, -2.0), (6.0, 1.5, 1.0), face=(0, 1, 0, 0, 1, 0)),
                       configs.block([5, 40, 6], (-1.0, 3.0, -1.0), (1.0, 7.0, 1.0)),
-                      configs.block([2, 3, 64], (3.0, 3.0, -2.0), (4.0, 4.0, 2.0), gamma=[0.0, 0.0, 0.0])]}
+                      configs.block([2, 3, 64], (3.0, 3.0, -2.0), (4.0, 4.0, 2.0), gamma=[0.0, 0.0, 0.0]),
+                      configs.block([48, 2, 49], (5.0, 3.0, -2.0), (7.0, 4.0, 2.0), face=(1, 1, 0, 0, 0, 1)),
+                      configs.block([3, 32, 2], (-3.0, 3.0, -2.0), (-2.0, 6.0, -1.0))]}
 
 
 def _charbc():
