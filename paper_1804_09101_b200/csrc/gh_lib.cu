@@ -27,8 +27,8 @@ constexpr int CHEB_TPB = 128;                     // K_cheb: 4 warps
 constexpr int CHEB_COMP_WALK = 25;                // components one K_cheb CTA walks over
 constexpr int CHEB_NTW = 2;                       // n-tiles per warp
 constexpr int CHEB_CT = (CHEB_TPB / 32) * 8 * CHEB_NTW;   // columns per CTA
-constexpr int CHEB_NCLASS = 3;                    // register-tile classes: N <= 32 (5 CTAs per SM), N <= 48 (4), N <= 64 (3)
-inline int cheb_class(int N) { return N <= 32 ? 0 : N <= 48 ? 1 : 2; }
+constexpr int CHEB_NCLASS = 4;                    // register-tile classes: N <= 24 (7 CTAs per SM), N <= 32 (5), N <= 48 (4), N <= 64 (3)
+inline int cheb_class(int N) { return N <= 24 ? 0 : N <= 32 ? 1 : N <= 48 ? 2 : 3; }
 inline int cheb_ct(int) { return CHEB_CT; }
 inline size_t cheb_frag_doubles(int N) { return (size_t)((N + 7) / 8) * ((N + 3) / 4) * 32; }   // D in fragment order
 constexpr int ANG_TPB0 = 256, ANG_TPB1 = 512;    // K_ang threads: class 0 (two CTAs per SM), class 1 (one CTA per SM)
@@ -644,8 +644,9 @@ void launch_cheb_class(gh_domain* d, int prof_cls, int c, const ChebItem* items,
   const Plan& pl = d->pl;
   ProfScope ps(d, prof_cls);
   const dim3 grid(n, gy);
-  if (c == 0) k_cheb<CHEB_TPB, 4, 8, CHEB_NTW><<<grid, CHEB_TPB, pl.cheb_smem, d->stream>>>(items, d->tables, in, out, pl.S, nrun, cm);
-  else if (c == 1) k_cheb<CHEB_TPB, 6, 12, CHEB_NTW><<<grid, CHEB_TPB, pl.cheb_smem, d->stream>>>(items, d->tables, in, out, pl.S, nrun, cm);
+  if (c == 0) k_cheb<CHEB_TPB, 3, 6, CHEB_NTW><<<grid, CHEB_TPB, pl.cheb_smem, d->stream>>>(items, d->tables, in, out, pl.S, nrun, cm);
+  else if (c == 1) k_cheb<CHEB_TPB, 4, 8, CHEB_NTW><<<grid, CHEB_TPB, pl.cheb_smem, d->stream>>>(items, d->tables, in, out, pl.S, nrun, cm);
+  else if (c == 2) k_cheb<CHEB_TPB, 6, 12, CHEB_NTW><<<grid, CHEB_TPB, pl.cheb_smem, d->stream>>>(items, d->tables, in, out, pl.S, nrun, cm);
   else k_cheb<CHEB_TPB, 8, 16, CHEB_NTW><<<grid, CHEB_TPB, pl.cheb_smem, d->stream>>>(items, d->tables, in, out, pl.S, nrun, cm);
 }
 

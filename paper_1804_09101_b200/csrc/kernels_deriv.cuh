@@ -33,7 +33,7 @@ struct CompMap {
 };
 
 template <int TPB, int MTM, int KSM, int NTW>
-__global__ void __launch_bounds__(TPB, (MTM * NTW >= 16) ? 3 : (MTM * NTW >= 12) ? 4 : 5)
+__global__ void __launch_bounds__(TPB, (MTM * NTW >= 16) ? 3 : (MTM * NTW >= 12) ? 4 : (MTM * NTW >= 8) ? 5 : 7)
 k_cheb(const ChebItem* __restrict__ items, const double* __restrict__ tables, const double* __restrict__ in,
        double* __restrict__ out, int64_t S, int ncomp, CompMap cm) {
   extern __shared__ __align__(16) double sm[];   // D in fragment order [mt][ks][32]
