@@ -637,7 +637,7 @@ gh_status check_flag(gh_domain* d) {   // stream must be synchronised by the cal
 
 // A2 + A3: logical derivatives of `ncomp` components of `in` into out[3][ncomp][S]
 // (blocks: d/dx, d/dy, d/dz already Cartesian; shells: d/dr, d/dtheta, d/dphi).
-// one K_cheb launch over the n items of register-tile class c (N <= 32: 4 x 8 tiles of D; N <= 48: 6 x 12; N <= 64: 8 x 16)
+// one K_cheb launch over the n items of register-tile class c (N <= 24: 3 x 6 tiles of D; N <= 32: 4 x 8; N <= 48: 6 x 12; N <= 64: 8 x 16)
 void launch_cheb_class(gh_domain* d, int prof_cls, int c, const ChebItem* items, int n, int gy, const double* in, double* out,
                        int nrun, const CompMap& cm) {
   if (!n) return;
