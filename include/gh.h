@@ -181,7 +181,8 @@ size_t gh_dp5_workspace_bytes(const gh_domain* dom);
 gh_status gh_dp5_attach(gh_domain* dom, void* dev_ws, size_t bytes);
 /* One step of size dt.  err: HOST [2] = {rms, max} of the error estimate over all 50 components and points (unweighted).
  * tol > 0: the step is taken only if max <= tol, otherwise the state is left as it was (*accepted = 0) and the caller
- * retries with a smaller dt; tol <= 0: always taken.  accepted may be NULL.  Synchronises (it returns host data).
+ * retries with a smaller dt; tol <= 0: always taken - except that a non-finite error estimate (NaN / Inf anywhere in the
+ * stage derivatives) is never accepted.  accepted may be NULL.  Synchronises (it returns host data).
  * The last stage is the RHS at the new state and is reused as the first stage of the next step when nothing else touched
  * the state in between. */
 gh_status gh_dp5_step(gh_domain* dom, double dt, double tol, double* err, int* accepted);
@@ -197,6 +198,15 @@ gh_status gh_set_profiling(gh_domain* dom, int enabled);
 gh_status gh_profile_read(gh_domain* dom, double* ms, int64_t* counts);
 gh_status gh_profile_reset(gh_domain* dom);
 const char* gh_kernel_name(int k);
+
+/* Execution options (all default 0; they change HOW the path runs, never what it computes - results are bit-identical).
+ *   GH_OPT_RK_OUT_OF_PLACE  1: every stage of gh_rk_step writes to a buffer it does not read (ua -> ub -> k -> ua) instead of
+ *                           updating in place.  The in-place stages are by design (the fused RHS kernel holds every field of a
+ *                           point in registers / shared memory before its first store); this switch exists so that a test can
+ *                           demand bit-equality of the two (compute-sanitizer is not available on the GPU pool). */
+#define GH_NUM_OPTIONS 8
+enum { GH_OPT_RK_OUT_OF_PLACE = 0 };
+gh_status gh_set_option(gh_domain* dom, int option, int value);
 
 /* Number of kernel launches issued by the library on this domain since creation. */
 int64_t gh_launch_count(const gh_domain* dom);

@@ -257,6 +257,8 @@ struct gh_domain {
   int* flag = nullptr;
   std::vector<SubDev> h_subs;
   bool has_fields = false, has_shell = false, has_block = false, has_char = false, has_ifc = false;
+  int device = 0, n_sm = 148;            // the device the workspace lives on (current at create) and its SM count
+  int opt[GH_NUM_OPTIONS] = {0};         // gh_set_option
   double t = 0.0;
   int64_t launches = 0;
   std::string err;
@@ -270,6 +272,15 @@ struct gh_domain {
 };
 
 namespace {
+
+// Every entry point that touches the device runs with the domain's device current and restores the caller's on return.
+struct DeviceGuard {
+  int prev = -1; bool sw = false;
+  explicit DeviceGuard(const gh_domain* d) {
+    if (d && cudaGetDevice(&prev) == cudaSuccess && prev != d->device) sw = cudaSetDevice(d->device) == cudaSuccess;
+  }
+  ~DeviceGuard() { if (sw) cudaSetDevice(prev); }
+};
 
 gh_status fail(gh_domain* d, gh_status st, const std::string& msg) {
   if (d) d->err = msg; else g_create_error = msg;
@@ -358,6 +369,14 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
 
   gh_domain* d = new gh_domain();
   d->pl = pl; d->ws = (char*)dev_workspace; d->stream = (cudaStream_t)cuda_stream;
+  {
+    cudaPointerAttributes pa;      // the workspace decides the device (falls back to the current one)
+    if (cudaPointerGetAttributes(&pa, dev_workspace) == cudaSuccess && pa.type == cudaMemoryTypeDevice) d->device = pa.device;
+    else { cudaGetLastError(); cudaGetDevice(&d->device); }
+    int nsm = 0;
+    if (cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, d->device) == cudaSuccess && nsm > 0) d->n_sm = nsm;
+  }
+  DeviceGuard guard_(d);
   char* w = d->ws;
   d->ua = (double*)(w + pl.o_ua); d->ub = (double*)(w + pl.o_ub); d->k = (double*)(w + pl.o_k);
   d->du = (double*)(w + pl.o_du); d->H = (double*)(w + pl.o_H); d->dH = (double*)(w + pl.o_dH);
@@ -551,16 +570,19 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
   GH_CREATE_CUDA(cudaFuncSetAttribute(k_rhs<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RHS_SMEM_BYTES));
   GH_CREATE_CUDA(cudaFuncSetAttribute(k_rhs<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RHS_SMEM_BYTES));
   GH_CREATE_CUDA(cudaFuncSetAttribute(k_rhs<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RHS_SMEM_BYTES));
-  if (pl.n_ang_class[0]) GH_CREATE_CUDA(cudaFuncSetAttribute(k_ang<ANG_TPB0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.ang_smem[0]));
-  if (pl.n_ang_class[1]) GH_CREATE_CUDA(cudaFuncSetAttribute(k_ang<ANG_TPB1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.ang_smem[1]));
-  if (pl.n_ang_class[0]) GH_CREATE_CUDA(cudaFuncSetAttribute(k_ang<ANG_TPB0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.ang_smem[0]));
-  if (pl.n_ang_class[1]) GH_CREATE_CUDA(cudaFuncSetAttribute(k_ang<ANG_TPB1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.ang_smem[1]));
+  // the attribute belongs to the FUNCTION, not to this domain: always the class ceiling, so that a later, smaller domain can
+  // never lower it under a live domain's launch size
+  GH_CREATE_CUDA(cudaFuncSetAttribute(k_ang<ANG_TPB0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ANG_SMEM_2CTA));
+  GH_CREATE_CUDA(cudaFuncSetAttribute(k_ang<ANG_TPB1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
+  GH_CREATE_CUDA(cudaFuncSetAttribute(k_ang<ANG_TPB0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ANG_SMEM_2CTA));
+  GH_CREATE_CUDA(cudaFuncSetAttribute(k_ang<ANG_TPB1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
 #undef GH_CREATE_CUDA
   *out = d;
   return GH_OK;
 }
 
 extern "C" void gh_domain_destroy(gh_domain* d) {
+  DeviceGuard guard_(d);
   if (!d) return;
   for (auto& p : d->pending) { cudaEventDestroy(p.a); cudaEventDestroy(p.b); }
   for (auto e : d->pool) cudaEventDestroy(e);
@@ -576,6 +598,7 @@ extern "C" gh_status gh_domain_layout(const gh_domain* d, int64_t* n_points, int
 }
 
 extern "C" gh_status gh_domain_coords(const gh_domain* cd, double* xyz, int on_device) {
+  DeviceGuard guard_(cd);
   gh_domain* d = const_cast<gh_domain*>(cd);
   if (!d || !xyz) return fail(d, GH_ERR_ARG, "NULL argument");
   const int64_t S = d->pl.S;
@@ -658,7 +681,7 @@ gh_status launch_derivs(gh_domain* d, const double* in, double* out, int ncomp, 
   // ... but small domains need the CTAs more than the amortisation: keep at least ~4 CTAs per SM in the grid
   int walk = 1;
   for (int w = CHEB_COMP_WALK; w >= 1; --w)
-    if (nrun % w == 0 && (w == 1 || (int64_t)pl.n_cheb_items * (nrun / w) >= 4 * 148)) { walk = w; break; }
+    if (nrun % w == 0 && (w == 1 || (int64_t)pl.n_cheb_items * (nrun / w) >= 4 * d->n_sm)) { walk = w; break; }
   const int cheb_gy = nrun / walk;
   for (int c = 0, first = 0; c < CHEB_NCLASS; first += pl.n_cheb_class[c], ++c)
     launch_cheb_class(d, GH_K_CHEB, c, d->cheb + first, pl.n_cheb_class[c], cheb_gy, in, out, nrun, cm);
@@ -707,6 +730,7 @@ gh_status launch_jac(gh_domain* d, double* g, int ncomp) {
 // state in / out
 // ------------------------------------------------------------------------------------------------------
 extern "C" gh_status gh_set_fields(gh_domain* d, const double* u, int on_device, double t) {
+  DeviceGuard guard_(d);
   if (!d || !u) return fail(d, GH_ERR_ARG, "NULL argument");
   const size_t bytes = (size_t)NCOMP * d->pl.S * sizeof(double);
   GH_CUDA(d, cudaMemcpyAsync(d->ua, u, bytes, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, d->stream));
@@ -716,6 +740,7 @@ extern "C" gh_status gh_set_fields(gh_domain* d, const double* u, int on_device,
 }
 
 extern "C" gh_status gh_get_fields(const gh_domain* cd, double* u, int on_device, double* t) {
+  DeviceGuard guard_(cd);
   gh_domain* d = const_cast<gh_domain*>(cd);
   if (!d || !u) return fail(d, GH_ERR_ARG, "NULL argument");
   if (!d->has_fields) return fail(d, GH_ERR_STATE, "gh_get_fields before gh_set_fields");
@@ -727,6 +752,7 @@ extern "C" gh_status gh_get_fields(const gh_domain* cd, double* u, int on_device
 }
 
 extern "C" gh_status gh_set_gauge_source(gh_domain* d, const double* H, const double* dH, int on_device) {
+  DeviceGuard guard_(d);
   if (!d || !H) return fail(d, GH_ERR_ARG, "NULL argument");
   const size_t comp = (size_t)d->pl.S * sizeof(double);
   const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
@@ -748,6 +774,7 @@ extern "C" gh_status gh_set_gauge_source(gh_domain* d, const double* H, const do
 // compute entry points
 // ------------------------------------------------------------------------------------------------------
 extern "C" gh_status gh_rhs(gh_domain* d, double* dtu, int on_device) {
+  DeviceGuard guard_(d);
   if (!d || !dtu) return fail(d, GH_ERR_ARG, "NULL argument");
   if (!d->has_fields) return fail(d, GH_ERR_STATE, "gh_rhs before gh_set_fields");
   if (on_device) return launch_rhs(d, d->ua, dtu);
@@ -758,8 +785,10 @@ extern "C" gh_status gh_rhs(gh_domain* d, double* dtu, int on_device) {
 }
 
 extern "C" gh_status gh_gradient(gh_domain* d, double* du, int on_device) {
+  DeviceGuard guard_(d);
   if (!d || !du) return fail(d, GH_ERR_ARG, "NULL argument");
   if (!d->has_fields) return fail(d, GH_ERR_STATE, "gh_gradient before gh_set_fields");
+  if (on_device && ((uintptr_t)du & 15) != 0) return fail(d, GH_ERR_ARG, "gh_gradient: a DEVICE du must be 16-byte aligned (the derivative kernels store double2)");
   double* tgt = on_device ? du : d->du;
   gh_status st = launch_derivs(d, d->ua, tgt, NCOMP);
   if (st != GH_OK) return st;
@@ -773,11 +802,12 @@ extern "C" gh_status gh_gradient(gh_domain* d, double* du, int on_device) {
 }
 
 extern "C" gh_status gh_rk_step(gh_domain* d, double dt) {
+  DeviceGuard guard_(d);
   if (!d) return GH_ERR_ARG;
   if (!d->has_fields) return fail(d, GH_ERR_STATE, "gh_rk_step before gh_set_fields");
   if (!std::isfinite(dt)) return fail(d, GH_ERR_ARG, "dt is not finite");
   gh_status st;
-  if (d->has_ifc) {
+  if (d->has_ifc || d->opt[GH_OPT_RK_OUT_OF_PLACE]) {
     // INTERFACE faces read the neighbour's face state from the stage input, so no stage may run in place: ua -> ub -> k -> ua
     if ((st = launch_rhs(d, d->ua, d->ub, 1, nullptr, 0.0, 1.0, dt)) != GH_OK) return st;
     if ((st = launch_rhs(d, d->ub, d->k, 2, d->ua, 0.75, 0.25, dt)) != GH_OK) return st;
@@ -797,6 +827,7 @@ extern "C" gh_status gh_rk_step(gh_domain* d, double dt) {
 }
 
 extern "C" gh_status gh_constraint_norms(gh_domain* d, double* out, double* per_sub) {
+  DeviceGuard guard_(d);
   if (!d || !out) return fail(d, GH_ERR_ARG, "NULL argument");
   if (!d->has_fields) return fail(d, GH_ERR_STATE, "gh_constraint_norms before gh_set_fields");
   const Plan& pl = d->pl;
@@ -822,7 +853,7 @@ extern "C" gh_status gh_constraint_norms(gh_domain* d, double* out, double* per_
     const double Ps = (double)n0 * n1 * n2;
     for (int q = 0; q < 3; ++q) {
       sum[q] += h[(size_t)s * 6 + q];
-      mx[q] = std::max(mx[q], h[(size_t)s * 6 + 3 + q]);
+      { const double v = h[(size_t)s * 6 + 3 + q]; if (v != v || v > mx[q]) mx[q] = v; }     // NaN propagates
       if (per_sub) {
         per_sub[(size_t)s * 6 + 2 * q] = std::sqrt(h[(size_t)s * 6 + q] / (Ps * ncomp[q]));
         per_sub[(size_t)s * 6 + 2 * q + 1] = h[(size_t)s * 6 + 3 + q];
@@ -862,6 +893,7 @@ extern "C" gh_status gh_filter_sigma(const gh_filter_desc* f, int32_t kmax, doub
 }
 
 extern "C" gh_status gh_set_filter(gh_domain* d, const gh_filter_desc* fb, const gh_filter_desc* fs) {
+  DeviceGuard guard_(d);
   if (!d) return GH_ERR_ARG;
   const Plan& pl = d->pl;
   std::vector<double> ft(pl.ftable_doubles, 0.0);
@@ -914,6 +946,7 @@ extern "C" gh_status gh_set_filter(gh_domain* d, const gh_filter_desc* fb, const
 }
 
 extern "C" gh_status gh_apply_filter(gh_domain* d) {
+  DeviceGuard guard_(d);
   if (!d) return GH_ERR_ARG;
   if (!d->has_fields) return fail(d, GH_ERR_STATE, "gh_apply_filter before gh_set_fields");
   d->dp_fsal = false;
@@ -923,7 +956,7 @@ extern "C" gh_status gh_apply_filter(gh_domain* d) {
     // x: ua -> T1, y: T1 -> T2, z: T2 -> ua   (T1, T2: the first two slots of the derivative scratch; only block points move)
     int walk = 1;
     for (int w = CHEB_COMP_WALK; w >= 1; --w)
-      if (NCOMP % w == 0 && (w == 1 || (int64_t)pl.n_fcheb_items / 3 * (NCOMP / w) >= 4 * 148)) { walk = w; break; }
+      if (NCOMP % w == 0 && (w == 1 || (int64_t)pl.n_fcheb_items / 3 * (NCOMP / w) >= 4 * d->n_sm)) { walk = w; break; }
     const int gy = NCOMP / walk;
     const double* src[3] = {d->ua, d->du, d->du + (size_t)NCOMP * pl.S};
     double* dst[3] = {d->du, d->du + (size_t)NCOMP * pl.S, d->ua};
@@ -951,7 +984,7 @@ extern "C" gh_status gh_apply_filter(gh_domain* d) {
 // Dormand-Prince 5(4) step (NEXT-3)
 // ------------------------------------------------------------------------------------------------------
 namespace {
-constexpr int DP_GRID = 148 * 8;     // streaming kernels: 8 CTAs of 256 threads per SM
+constexpr int DP_GRID = 256 * 8;     // upper bound of the streaming-kernel grid (partials buffer); launches use 8 CTAs of 256 threads per SM
 const double DP_A[7][6] = {
     {0, 0, 0, 0, 0, 0},
     {1.0 / 5, 0, 0, 0, 0, 0},
@@ -969,6 +1002,7 @@ inline size_t dp_bytes(const Plan& pl) {
 extern "C" size_t gh_dp5_workspace_bytes(const gh_domain* d) { return d ? dp_bytes(d->pl) : 0; }
 
 extern "C" gh_status gh_dp5_attach(gh_domain* d, void* ws, size_t bytes) {
+  DeviceGuard guard_(d);
   if (!d) return GH_ERR_ARG;
   if (!ws || ((uintptr_t)ws & 255) != 0) return fail(d, GH_ERR_WORKSPACE, "DP5 workspace is NULL or not 256-byte aligned");
   if (bytes < dp_bytes(d->pl)) return fail(d, GH_ERR_WORKSPACE, "DP5 workspace too small: need " + std::to_string(dp_bytes(d->pl)) + " bytes");
@@ -983,12 +1017,13 @@ extern "C" gh_status gh_dp5_attach(gh_domain* d, void* ws, size_t bytes) {
 }
 
 extern "C" gh_status gh_dp5_step(gh_domain* d, double dt, double tol, double* err, int* accepted) {
+  DeviceGuard guard_(d);
   if (!d || !err) return fail(d, GH_ERR_ARG, "NULL argument");
   if (!d->has_fields) return fail(d, GH_ERR_STATE, "gh_dp5_step before gh_set_fields");
   if (!d->dpk[0]) return fail(d, GH_ERR_STATE, "gh_dp5_step before gh_dp5_attach");
   if (!std::isfinite(dt)) return fail(d, GH_ERR_ARG, "dt is not finite");
   const int64_t n2 = (int64_t)NCOMP * d->pl.S / 2;
-  const int grid = (int)std::min<int64_t>((n2 + 255) / 256, DP_GRID);
+  const int grid = (int)std::min<int64_t>((n2 + 255) / 256, std::min(DP_GRID, d->n_sm * 8));
   gh_status st;
   // k1 = f(u): the last stage of the previous accepted step when the state has not been touched since
   if (!d->dp_fsal && (st = launch_rhs(d, d->ua, d->dpk[0])) != GH_OK) return st;
@@ -1015,7 +1050,8 @@ extern "C" gh_status gh_dp5_step(gh_domain* d, double dt, double tol, double* er
   if (st != GH_OK) { d->dp_fsal = false; return st; }
   err[0] = std::sqrt(h[0] / ((double)NCOMP * (double)d->pl.P));
   err[1] = h[1];
-  const bool ok = !(tol > 0.0) || (err[1] <= tol);
+  // a non-finite estimate (NaN in Pi or Phi with psi still physical is not caught by the singular flag) never passes
+  const bool ok = std::isfinite(err[0]) && std::isfinite(err[1]) && (!(tol > 0.0) || (err[1] <= tol));
   if (accepted) *accepted = ok ? 1 : 0;
   if (ok) {
     std::swap(d->ua, d->ub);            // the new state; k7 = f(new state) becomes k1 of the next step
@@ -1031,6 +1067,7 @@ extern "C" gh_status gh_dp5_step(gh_domain* d, double dt, double tol, double* er
 // profiling / bookkeeping
 // ------------------------------------------------------------------------------------------------------
 extern "C" gh_status gh_set_profiling(gh_domain* d, int enabled) {
+  DeviceGuard guard_(d);
   if (!d) return GH_ERR_ARG;
   drain_profile(d);
   d->prof = enabled != 0;
@@ -1038,6 +1075,7 @@ extern "C" gh_status gh_set_profiling(gh_domain* d, int enabled) {
 }
 
 extern "C" gh_status gh_profile_read(gh_domain* d, double* ms, int64_t* counts) {
+  DeviceGuard guard_(d);
   if (!d) return GH_ERR_ARG;
   drain_profile(d);
   for (int k = 0; k < GH_NUM_KERNELS; ++k) { if (ms) ms[k] = d->prof_ms[k]; if (counts) counts[k] = d->prof_n[k]; }
@@ -1045,6 +1083,7 @@ extern "C" gh_status gh_profile_read(gh_domain* d, double* ms, int64_t* counts) 
 }
 
 extern "C" gh_status gh_profile_reset(gh_domain* d) {
+  DeviceGuard guard_(d);
   if (!d) return GH_ERR_ARG;
   drain_profile(d);
   for (int k = 0; k < GH_NUM_KERNELS; ++k) { d->prof_ms[k] = 0; d->prof_n[k] = 0; }
@@ -1054,6 +1093,13 @@ extern "C" gh_status gh_profile_reset(gh_domain* d) {
 extern "C" const char* gh_kernel_name(int k) {
   static const char* names[GH_NUM_KERNELS] = {"k_cheb", "k_ang", "k_rhs", "k_rk", "k_con", "k_con_reduce", "k_jac", "other", "k_cheb(filter)", "k_ang(filter)", "k_dp_stage", "k_dp_err"};
   return (k >= 0 && k < GH_NUM_KERNELS) ? names[k] : "?";
+}
+
+extern "C" gh_status gh_set_option(gh_domain* d, int option, int value) {
+  if (!d) return GH_ERR_ARG;
+  if (option < 0 || option >= GH_NUM_OPTIONS) return fail(d, GH_ERR_ARG, "gh_set_option: unknown option");
+  d->opt[option] = value;
+  return GH_OK;
 }
 
 extern "C" int64_t gh_launch_count(const gh_domain* d) { return d ? d->launches : 0; }

@@ -27,6 +27,9 @@ __host__ __device__ constexpr int S3(int i, int j) {
   return i <= j ? (i * 3 - (i * (i - 1)) / 2 + j - i) : (j * 3 - (j * (j - 1)) / 2 + i - j);
 }
 
+// max that PROPAGATES NaN (fmax drops a NaN operand: a NaN constraint or error estimate would report a finite maximum)
+__device__ __forceinline__ double nanmax(double a, double b) { return (a != a || b != b) ? (a + b) : fmax(a, b); }
+
 struct Geom {
   double gi[6];     // g^{ij}
   double sh[3];     // N^i
@@ -643,14 +646,14 @@ k_dp_err(DpArgs A, double dt, double* __restrict__ part, int64_t n2) {
       if (j < A.nk) { const double2 v = A.k[j][i]; sx = fma(A.a[j], v.x, sx); sy = fma(A.a[j], v.y, sy); }
     sx *= dt; sy *= dt;
     ss = fma(sx, sx, ss); ss = fma(sy, sy, ss);
-    mx = fmax(mx, fmax(fabs(sx), fabs(sy)));
+    mx = nanmax(mx, nanmax(fabs(sx), fabs(sy)));
   }
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) { ss += __shfl_xor_sync(0xffffffffu, ss, o); mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o)); }
+  for (int o = 16; o > 0; o >>= 1) { ss += __shfl_xor_sync(0xffffffffu, ss, o); mx = nanmax(mx, __shfl_xor_sync(0xffffffffu, mx, o)); }
   if ((threadIdx.x & 31) == 0) { red[threadIdx.x >> 5][0] = ss; red[threadIdx.x >> 5][1] = mx; }
   __syncthreads();
   if (threadIdx.x == 0) {
-    for (int w = 1; w < 8; ++w) { ss += red[w][0]; mx = fmax(mx, red[w][1]); }
+    for (int w = 1; w < 8; ++w) { ss += red[w][0]; mx = nanmax(mx, red[w][1]); }
     part[2 * blockIdx.x] = ss; part[2 * blockIdx.x + 1] = mx;
   }
 }
@@ -658,9 +661,9 @@ k_dp_err(DpArgs A, double dt, double* __restrict__ part, int64_t n2) {
 __global__ void __launch_bounds__(32)
 k_dp_err_final(const double* __restrict__ part, int nblocks, double* __restrict__ out) {
   double ss = 0.0, mx = 0.0;
-  for (int b = threadIdx.x; b < nblocks; b += 32) { ss += part[2 * b]; mx = fmax(mx, part[2 * b + 1]); }
+  for (int b = threadIdx.x; b < nblocks; b += 32) { ss += part[2 * b]; mx = nanmax(mx, part[2 * b + 1]); }
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) { ss += __shfl_xor_sync(0xffffffffu, ss, o); mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o)); }
+  for (int o = 16; o > 0; o >>= 1) { ss += __shfl_xor_sync(0xffffffffu, ss, o); mx = nanmax(mx, __shfl_xor_sync(0xffffffffu, mx, o)); }
   if (threadIdx.x == 0) { out[0] = ss; out[1] = mx; }
 }
 
@@ -695,7 +698,7 @@ __device__ __forceinline__ void con_point(const SubDev& sd, const double* __rest
     for (int a = 0; a < 4; ++a) {
       const double c = H[a] + symdot(G.pinv, Gam[a]);
       acc[0] = fma(c, c, acc[0]);
-      acc[3] = fmax(acc[3], fabs(c));
+      acc[3] = nanmax(acc[3], fabs(c));
     }
   }
   ShellJac J;
@@ -721,12 +724,12 @@ __device__ __forceinline__ void con_point(const SubDev& sd, const double* __rest
     for (int i = 0; i < 3; ++i) {
       const double c = d[0][i] - u[(int64_t)(20 + 10 * i + s) * S + p];
       acc[1] = fma(c, c, acc[1]);
-      acc[4] = fmax(acc[4], fabs(c));
+      acc[4] = nanmax(acc[4], fabs(c));
     }
     // C_ijab = d_i Phi_jab - d_j Phi_iab for (i,j) = (0,1), (0,2), (1,2)
     const double c01 = d[2][0] - d[1][1], c02 = d[3][0] - d[1][2], c12 = d[3][1] - d[2][2];
     acc[2] = fma(c01, c01, acc[2]); acc[2] = fma(c02, c02, acc[2]); acc[2] = fma(c12, c12, acc[2]);
-    acc[5] = fmax(acc[5], fmax(fabs(c01), fmax(fabs(c02), fabs(c12))));
+    acc[5] = nanmax(acc[5], nanmax(fabs(c01), nanmax(fabs(c02), fabs(c12))));
   }
 }
 
@@ -755,7 +758,7 @@ k_con(const SubDev* __restrict__ subs, const int32_t* __restrict__ tile_first, i
 #pragma unroll
     for (int q = 0; q < 3; ++q) acc[q] += __shfl_xor_sync(0xffffffffu, acc[q], o);
 #pragma unroll
-    for (int q = 3; q < 6; ++q) acc[q] = fmax(acc[q], __shfl_xor_sync(0xffffffffu, acc[q], o));
+    for (int q = 3; q < 6; ++q) acc[q] = nanmax(acc[q], __shfl_xor_sync(0xffffffffu, acc[q], o));
   }
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   if (lane == 0)
@@ -765,7 +768,7 @@ k_con(const SubDev* __restrict__ subs, const int32_t* __restrict__ tile_first, i
   if (threadIdx.x < 6) {
     const int q = threadIdx.x;
     double v = red[0][q];
-    for (int w = 1; w < TILE_PTS / 32; ++w) v = (q < 3) ? v + red[w][q] : fmax(v, red[w][q]);
+    for (int w = 1; w < TILE_PTS / 32; ++w) v = (q < 3) ? v + red[w][q] : nanmax(v, red[w][q]);
     part[(int64_t)blockIdx.x * 6 + q] = v;
   }
 }
@@ -780,14 +783,14 @@ k_con_reduce(const int32_t* __restrict__ tile_first, const double* __restrict__ 
 #pragma unroll
     for (int q = 0; q < 3; ++q) acc[q] += part[(int64_t)t * 6 + q];
 #pragma unroll
-    for (int q = 3; q < 6; ++q) acc[q] = fmax(acc[q], part[(int64_t)t * 6 + q]);
+    for (int q = 3; q < 6; ++q) acc[q] = nanmax(acc[q], part[(int64_t)t * 6 + q]);
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
 #pragma unroll
     for (int q = 0; q < 3; ++q) acc[q] += __shfl_xor_sync(0xffffffffu, acc[q], o);
 #pragma unroll
-    for (int q = 3; q < 6; ++q) acc[q] = fmax(acc[q], __shfl_xor_sync(0xffffffffu, acc[q], o));
+    for (int q = 3; q < 6; ++q) acc[q] = nanmax(acc[q], __shfl_xor_sync(0xffffffffu, acc[q], o));
   }
   if (lane == 0)
 #pragma unroll

@@ -21,6 +21,7 @@ LIB_PATH = os.path.join(_HERE, "libgh.so")
 GH_NCOMP = 50
 GH_NUM_KERNELS = 12
 GH_FILTER_NONE, GH_FILTER_HEAVISIDE, GH_FILTER_EXP = range(3)
+GH_OPT_RK_OUT_OF_PLACE = 0
 GH_OK, GH_ERR_ARG, GH_ERR_WORKSPACE, GH_ERR_CUDA, GH_ERR_STATE, GH_ERR_SINGULAR = range(6)
 STATUS_NAMES = ["GH_OK", "GH_ERR_ARG", "GH_ERR_WORKSPACE", "GH_ERR_CUDA", "GH_ERR_STATE", "GH_ERR_SINGULAR"]
 
@@ -31,7 +32,7 @@ EXPORTS = [
     "gh_constraint_norms", "gh_set_profiling", "gh_profile_read", "gh_profile_reset", "gh_kernel_name",
     "gh_launch_count", "gh_last_error", "gh_basis_cheb", "gh_basis_gauss_legendre", "gh_basis_shell",
     "gh_set_filter", "gh_apply_filter", "gh_filter_sigma",
-    "gh_dp5_workspace_bytes", "gh_dp5_attach", "gh_dp5_step",
+    "gh_dp5_workspace_bytes", "gh_dp5_attach", "gh_dp5_step", "gh_set_option",
 ]
 
 
@@ -118,6 +119,7 @@ def lib() -> C.CDLL:
     L.gh_dp5_workspace_bytes.argtypes = [vp]
     L.gh_dp5_attach.argtypes = [vp, vp, C.c_size_t]
     L.gh_dp5_step.argtypes = [vp, C.c_double, C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_int)]
+    L.gh_set_option.argtypes = [vp, ip, ip]
     _lib = L
     return L
 
@@ -392,6 +394,9 @@ class Domain:
 
     def apply_filter(self):
         gh_apply_filter(self.h)
+
+    def set_option(self, option: int, value: int):
+        _check(lib().gh_set_option(self.h, int(option), int(value)), self.h)
 
     def set_profiling(self, on: bool):
         _check(lib().gh_set_profiling(self.h, int(on)), self.h)

@@ -186,14 +186,16 @@ def _c3_run(oracle, shells, checkpoints):
     return worst
 
 
-def test_c3_evolution_parity_10_steps(oracle):
-    """BASELINE.json configs[2], first 10 of its 100 steps; compared after steps 1 and 10 on the excision shell (FREE inner
-    face) and the outermost shell."""
-    _c3_run(oracle, shells=[0, 7], checkpoints=[1, 10])
+def test_c3_evolution_parity_100_steps(oracle):
+    """BASELINE.json configs[2] as stated: 100 RK3 steps of the 8-shell domain at dt = 0.25 min spacing; the GPU steps all 8
+    shells, the oracle follows the excision shell (FREE inner face) and the outermost shell (the shells are decoupled, reading
+    S11); compared after steps 1, 10 and 100 so that a drift shows before it fails."""
+    worst = _c3_run(oracle, shells=[0, 7], checkpoints=[1, 10, 100])
+    print(f"C3 100 steps, shells 0 and 7: worst |gpu - oracle| / ||X||inf = {worst:.3e}")
 
 
 @pytest.mark.skipif(not os.environ.get("GH_LONG_TESTS"), reason="about 35 minutes of oracle time: set GH_LONG_TESTS=1")
-def test_c3_evolution_parity_100_steps(oracle):
+def test_c3_evolution_parity_100_steps_all_shells(oracle):
     """The full C3 run: 100 RK3 steps, every shell, compared after steps 1, 10 and 100."""
     worst = _c3_run(oracle, shells=list(range(8)), checkpoints=[1, 10, 100])
     print(f"C3 100 steps: worst |gpu - oracle| / ||X||inf = {worst:.3e}")
@@ -246,8 +248,13 @@ def test_dp5_step_parity(case, oracle):
     plus the rounding floor; two consecutive steps (the second reuses the last stage as its first) against two oracle steps;
     a rejected step leaves the state bit-identical."""
     name, cfg, descs, coords, us, Hs, dom = case
+    own = None
     if name == "wide":
-        pytest.skip("the long-double oracle needs ~14 RHS evaluations here; covered by the other cases")
+        # the long-double oracle needs ~14 RHS evaluations per subdomain: on this case a 2-subdomain subset (the 512-thread
+        # K_ang class shell and the block that straddles the K_cheb class limit 32 | 33) in a domain of its own
+        keep = [0, 2]
+        descs, us, Hs = [descs[s] for s in keep], [us[s] for s in keep], [Hs[s] for s in keep]
+        dom = own = _domain(descs, Hs, us)
     dt = 0.25 * configs.min_spacing(descs)
     dom.set_fields(dom.pack(us), 0.0)
     dom.dp5_attach()
@@ -274,6 +281,8 @@ def test_dp5_step_parity(case, oracle):
     assert not acc3 and mx3 > 1e-30
     assert np.array_equal(dom.get_fields(), before)
     dom.set_fields(dom.pack(us), 0.0)
+    if own is not None:
+        own.close()
 
 
 def test_dp5_needs_its_workspace():
@@ -283,6 +292,18 @@ def test_dp5_needs_its_workspace():
         dom.dp5_step(1e-3)
     assert e.value.status == gh.GH_ERR_STATE
     dom.close()
+
+
+def _rhs_and_step_parity(oracle, dom, descs, us, Hs, what):
+    """gh_rhs and one gh_rk_step of the whole domain against the oracle, subdomain by subdomain"""
+    k = dom.unpack(dom.rhs())
+    dt = 0.25 * configs.min_spacing(descs)
+    dom.rk_step(dt)
+    new = dom.unpack(dom.get_fields())
+    for s, d in enumerate(descs):
+        assert_parity(k[s], oracle.rhs(d, us[s], Hs[s]), state=us[s], tol=TOL, what=f"{what} sub {s} rhs")
+        assert_parity(new[s], oracle.rk3(d, us[s], Hs[s], dt, 1), tol=TOL, what=f"{what} sub {s} rk3")
+    dom.set_fields(dom.pack(us), 0.0)
 
 
 def test_gradient_parity_at_the_size_limits(oracle):
@@ -297,6 +318,7 @@ def test_gradient_parity_at_the_size_limits(oracle):
         got = g[:, :, dom.offsets[s]:dom.offsets[s] + dom.sizes[s]]
         for k in range(3):
             assert_parity(got[k], ref[k], state=us[s], tol=TOL, what=f"limits sub {s} d_{k}")
+    _rhs_and_step_parity(oracle, dom, descs, us, Hs, "limits")
     dom.close()
     with pytest.raises(gh.GHError):
         gh.Domain([configs.shell(4, 48, 3.0, 4.0)])
@@ -431,3 +453,72 @@ def test_random_domains_parity(oracle):
             assert_parity(k[s], oracle.rhs(d, us[s], Hs[s]), state=us[s], tol=TOL, what=what + " rhs")
             assert_parity(new[s], oracle.rk3(d, us[s], Hs[s], dt, 1), tol=TOL, what=what + " rk3")
         dom.close()
+
+
+# ---- robustness of the boundary ----------------------------------------------------------------------------------
+def test_small_domain_created_while_a_large_one_is_alive(oracle):
+    """The dynamic-shared-memory attribute of K_ang belongs to the function, not to a domain: creating a C1 domain while an
+    L = 31 domain (512-thread class, ~200 KB of shared memory) is alive must not break the large one's next launch."""
+    big_cfg = {"id": 12, "spin": 0.3, "amplitude": 1e-3, "descs": [configs.shell(4, 31, 2.5, 3.5), configs.shell(4, 20, 3.5, 5.0)]}
+    descs, coords, us, Hs = build_case(big_cfg, oracle)
+    big = _domain(descs, Hs, us)
+    before = big.rhs()
+    small = gh.Domain(configs.c1()["descs"])
+    small.set_fields(np.zeros((50, small.S)), 0.0)
+    after = big.rhs()
+    assert np.array_equal(before, after)
+    g = big.gradient()
+    ref = oracle.gradient(descs[0], us[0])
+    for k in range(3):
+        assert_parity(g[k][:, big.offsets[0]:big.offsets[0] + big.sizes[0]], ref[k], state=us[0], tol=TOL, what=f"two domains d_{k}")
+    small.close(); big.close()
+
+
+def test_rk_stages_in_place_equal_out_of_place():
+    """K_rhs updates the RK stage buffers in place (u / u0 / out alias by design): the same step with every stage written to a
+    buffer it does not read (GH_OPT_RK_OUT_OF_PLACE) must give the same bits (compute-sanitizer is unavailable on the pool)."""
+    from oracle.gh_oracle import Oracle      # only for the grid coordinates of the seeded inputs
+    ora = Oracle("long double")
+    for cfg in (_mini_mixed(), _charbc(), configs.c3()):
+        descs, coords, us, Hs = build_case(cfg, ora)
+        dom = _domain(descs, Hs, us)
+        dt = 0.25 * configs.min_spacing(descs)
+        res = []
+        for oop in (0, 1, 0):
+            dom.set_option(gh.GH_OPT_RK_OUT_OF_PLACE, oop)
+            dom.set_fields(dom.pack(us), 0.0)
+            for _ in range(3):
+                dom.rk_step(dt)
+            res.append(dom.get_fields().copy())
+        assert np.array_equal(res[0], res[1]) and np.array_equal(res[0], res[2])
+        assert np.max(np.abs(res[0] - dom.pack(us))) > 0
+        dom.close()
+
+
+def test_misaligned_device_gradient_pointer_is_rejected():
+    import torch
+    dom = gh.Domain(configs.c1()["descs"])
+    dom.set_fields(np.zeros((50, dom.S)), 0.0)
+    buf = torch.empty(3 * 50 * dom.S + 1, dtype=torch.float64, device="cuda")
+    with pytest.raises(gh.GHError) as e:
+        gh.gh_gradient(dom.h, buf[1:])
+    assert e.value.status == gh.GH_ERR_ARG
+    gh.gh_gradient(dom.h, buf[:-1])
+    dom.close()
+
+
+def test_nan_reaches_the_reported_maxima(oracle):
+    """A NaN in Pi leaves psi physical (the singular flag stays down) but makes C_a NaN there: the reported max must be NaN, not the
+    finite maximum of the other points (fmax drops NaN operands), and a Dormand-Prince step with a NaN estimate is not accepted."""
+    cfg = _mini_mixed()
+    descs, coords, us, Hs = build_case(cfg, oracle)
+    dom = _domain(descs, Hs, us)
+    bad = [u.copy() for u in us]
+    bad[1][13, 77] = np.nan
+    dom.set_fields(dom.pack(bad), 0.0)
+    out, per = dom.constraint_norms(per_sub=True)
+    assert np.isnan(out[0, 1]) and np.isnan(out[0, 0]) and np.isnan(per[1, 0, 1]) and np.isfinite(per[0]).all()
+    dom.dp5_attach()
+    rms, mx, acc = dom.dp5_step(1e-3)
+    assert not acc and (np.isnan(mx) or np.isnan(rms))
+    dom.close()

@@ -220,3 +220,94 @@ def test_constraint_linearity_and_frozen_faces(oracle):
     norms = oracle.constraint_norms([sd], [u0 + du], [H])
     assert np.allclose(norms[:, 0], np.sqrt(sums / (xyz.shape[1] * np.array([4, 30, 30]))))
     assert np.allclose(norms[1], [np.sqrt((C1[4:34] ** 2).mean()), np.abs(C1[4:34]).max()])
+
+
+def _poly_phi(sd, xyz, seed, deg=3):
+    """Seeded polynomial dPhi_iab (degree <= deg per axis in the block's reference coordinates) and its ANALYTIC Cartesian
+    gradient, both from the monomial coefficients in numpy (nothing of the oracle): -> Phi[30, P], grad[3, 30, P]."""
+    rng = np.random.default_rng(seed)
+    lo, hi = np.array(sd["lo"]), np.array(sd["hi"])
+    X = (2 * xyz - (lo + hi)[:, None]) / (hi - lo)[:, None]          # reference cube coordinates
+    c = rng.uniform(-1, 1, (30, deg + 1, deg + 1, deg + 1))
+    pw = [np.stack([X[a] ** p for p in range(deg + 1)]) for a in range(3)]                                   # X^p
+    dpw = [np.stack([p * X[a] ** max(p - 1, 0) for p in range(deg + 1)]) * (2 / (hi[a] - lo[a])) for a in range(3)]  # d/dx_a X^p
+    Phi = np.einsum("cpqr,pn,qn,rn->cn", c, pw[0], pw[1], pw[2])
+    grad = np.stack([np.einsum("cpqr,pn,qn,rn->cn", c, *(dpw[b] if b == a else pw[b] for b in range(3))) for a in range(3)])
+    return Phi, grad
+
+
+def test_c_ijab_on_non_vanishing_data(oracle):
+    """O8, the C_ijab part: C_ijab = d_i Phi_jab - d_j Phi_iab must equal the ANALYTIC curl
+    of a seeded polynomial Phi on a block, component by component for the pairs (x,y), (x,z), (y,z) in that order; a wrong
+    pair table, a dropped pair or a repeated index fails (the three curls differ).  Both as absolute values (Minkowski psi,
+    Phi = polynomial) and by linearity on top of exact Kerr-Schild data; sums[2] / maxs[2] against their numpy restatement."""
+    sd = configs.block([6, 5, 7], (3.0, -1.0, -1.5), (5.0, 1.0, 1.0))
+    xyz = oracle.coords(sd)
+    P = xyz.shape[1]
+    dPhi, g = _poly_phi(sd, xyz, 314)
+    # analytic curl rows in the oracle's documented order: 34 + 10 q + s, q = 0, 1, 2 for (i,j) = (0,1), (0,2), (1,2)
+    curl = np.concatenate([g[i][10 * j:10 * j + 10] - g[j][10 * i:10 * i + 10] for i, j in ((0, 1), (0, 2), (1, 2))])
+    assert min(np.abs(curl[10 * q:10 * q + 10] - curl[10 * r:10 * r + 10]).max() for q, r in ((0, 1), (0, 2), (1, 2))) > 0.1
+    # (a) Minkowski metric, Pi = 0, Phi = the polynomial, H = 0
+    psi = np.broadcast_to(np.diag([-1.0, 1.0, 1.0, 1.0])[..., None], (4, 4, P))
+    u = inputs.pack_fields(psi, np.zeros((4, 4, P)), np.zeros((3, 4, 4, P)))
+    u[20:50] = dPhi
+    sums, maxs, C = oracle.constraints(sd, u, np.zeros((4, P)), fields=True)
+    scale = np.abs(curl).max()
+    assert np.abs(C[34:64] - curl).max() < 1e-13 * scale
+    assert np.abs(C[4:34] + dPhi).max() < 1e-15            # C_iab = d_i psi - Phi_i with constant psi
+    assert abs(sums[2] - (C[34:64] ** 2).sum()) <= 1e-14 * sums[2] and maxs[2] == np.abs(C[34:64]).max()
+    assert abs(sums[1] - (C[4:34] ** 2).sum()) <= 1e-14 * sums[1] and maxs[1] == np.abs(C[4:34]).max()
+    # (b) on top of exact Kerr-Schild data, by linearity (the unperturbed C_ijab is the truncation error of d_i Phi_j)
+    u0 = inputs.pack_fields(*inputs.kerr_schild(xyz, 1.0, 0.4))
+    H = inputs.kerr_schild_gauge_source(xyz, 1.0, 0.4)
+    u1 = u0.copy()
+    u1[20:50] += 1e-2 * dPhi
+    _, _, C0 = oracle.constraints(sd, u0, H, fields=True)
+    s1, m1, C1 = oracle.constraints(sd, u1, H, fields=True)
+    assert np.abs((C1 - C0)[34:64] - 1e-2 * curl).max() < 1e-13 * 1e-2 * scale
+    assert abs(s1[2] - (C1[34:64] ** 2).sum()) <= 1e-14 * s1[2] and m1[2] == np.abs(C1[34:64]).max()
+    # the point-level function: antisymmetric in (i,j), zero diagonal, upper pairs = the analytic curl at a point
+    p = 17
+    full = lambda a: np.array([[a[inputs.SYM_PAIRS.index((min(x, y), max(x, y)))] for y in range(4)] for x in range(4)])
+    dPhi_p = np.array([[full(g[k][10 * i:10 * i + 10, p]) for i in range(3)] for k in range(3)])      # [k][i][a][b] = d_k Phi_iab
+    _, _, Cij = oracle.constraints_point(np.diag([-1.0, 1.0, 1.0, 1.0]), np.zeros((4, 4)), np.zeros((3, 4, 4)), np.zeros((3, 4, 4)),
+                                         dPhi_p, np.zeros(4))
+    assert np.abs(Cij + Cij.swapaxes(0, 1)).max() == 0 and np.abs(Cij[[0, 1, 2], [0, 1, 2]]).max() == 0
+    for q, (i, j) in enumerate(((0, 1), (0, 2), (1, 2))):
+        assert np.abs(Cij[i, j] - full(curl[10 * q:10 * q + 10, p])).max() < 1e-15 * scale
+
+
+def test_stated_conventions(oracle):
+    """The three conventions DESIGN.md fixes and calls 'parity unpinned' (S16 unweighted RMS normalisation, S2 default gamma's,
+    S22 the VALUE of the interface penalty): no mathematics decides them, so these asserts only keep the oracle, the configs and
+    the documents saying the same thing."""
+    assert configs.GAMMA_DEFAULT == [1.0, -1.0, 1.0]                                                   # S2
+    sd = configs.block([4, 3, 5], (3.0, -1.0, -1.0), (5.0, 1.0, 1.0))
+    xyz = oracle.coords(sd)
+    P = xyz.shape[1]
+    u = inputs.pack_fields(np.broadcast_to(np.diag([-1.0, 1.0, 1.0, 1.0])[..., None], (4, 4, P)), np.zeros((4, 4, P)), np.zeros((3, 4, 4, P)))
+    u[20:50] = 0.5                                                                                    # C_iab = -0.5 everywhere
+    norms = oracle.constraint_norms([sd, sd], [u, u], [np.zeros((4, P))] * 2)
+    assert abs(norms[1, 0] - 0.5) < 1e-15 and norms[1, 1] == 0.5                                       # S16: unweighted RMS over points x 30
+    # S22: p = (N_r - 1)^2 / (r_out - r_in): a unit jump in psi_tt across an outer interface face of flat space with shift
+    # pointing inwards (v0 = -(1+g1) n.N < 0 only if n.N > 0: use gamma1 = 0 and an outward shift) changes d_t psi_tt by p v0
+    sh = configs.shell(5, 2, 2.0, 4.0, face=(0, 3), gamma=[0.0, 0.0, 0.0])
+    xs = oracle.coords(sh)
+    Ps = xs.shape[1]
+    psi = np.broadcast_to(np.diag([-1.0, 1.0, 1.0, 1.0])[..., None], (4, 4, Ps)).copy()
+    r = np.sqrt((xs ** 2).sum(0))
+    beta = 0.3
+    for i in range(3):
+        psi[0, i + 1] = psi[i + 1, 0] = beta * xs[i] / r                                               # N^i = beta r^: n.N = beta > 0
+    psi[0, 0] = -1.0 + beta ** 2
+    us = inputs.pack_fields(psi, np.zeros((4, 4, Ps)), np.zeros((3, 4, 4, Ps)))
+    pl = 3 * 6
+    nbr = us[:, :pl].copy()
+    nbr[:] = us[:, -pl:]
+    k0 = oracle.rhs_ifc(sh, us, np.zeros((4, Ps)), nbr_out=nbr)
+    nbr[0] -= 1.0                                                                                     # own - neighbour = +1 in psi_tt
+    k1 = oracle.rhs_ifc(sh, us, np.zeros((4, Ps)), nbr_out=nbr)
+    pen = (5 - 1) ** 2 / (4.0 - 2.0)
+    assert np.abs((k1 - k0)[0, -pl:] - pen * (-(1 + 0.0) * beta)).max() < 1e-13
+    assert np.abs((k1 - k0)[:, :-pl]).max() == 0
