@@ -37,7 +37,10 @@
  * projection, Heaviside idempotence, linearity; characteristic boundary condition
  * (O10): eigenvectors of the RHS's principal part; Dormand-Prince step (O11): the
  * order conditions of the tableau and 5th-order convergence on the gauge wave;
- * interface exchange (O12): projection of what it adds onto the characteristic fields.
+ * interface exchange (O12): projection of what it adds onto the characteristic fields;
+ * constraints (O8): C_ijab of a polynomial Phi equals its analytic curl; SpatialCoordJac
+ * (O13): the tensor law with diag(1, J) by einsum, composition, Kerr-Schild axisymmetry, the
+ * paper's printed operation counts.
  * PARITY UNPINNED (pure conventions, fixed by DESIGN.md): the normalisation of the
  * constraint norms (unweighted RMS over points and components), the default gamma's,
  * and the VALUE of the interface penalty factor p = (N_r-1)^2/(r_out-r_in) of O12 (its
@@ -924,5 +927,141 @@ int ora_constraints_subdomain(const ora_subdomain* sd, const double* u, const do
   }
   for (int q = 0; q < 3; ++q) { sums[q] = (double)S[q]; maxs[q] = (double)M[q]; }
   free(ur); free(Hr); free(gH); free(g);
+  return bad;
+}
+
+/* ---------------------------------------------------------------------- */
+/* O13 — SpatialCoordJac (NEXT-4; §3.3, Eqs. 9-11): "makes */
+/* a coordinate change of a tensor's spatial indices only, by contracting   */
+/* every possible combination of said spatial indices with the Jacobian.    */
+/* First, one contraction per rank is performed over the purely spatial     */
+/* indices.  Next, each index is respectively set to its timelike component */
+/* and one contraction per remaining index is performed.  Subsequently, two */
+/* indices are made timelike, ... The purely timelike component encounters  */
+/* a null-op."  Rank 2:  T_ij = J_i^k J_j^l T_kl, T_0j = J_j^l T_0l,        */
+/* T_i0 = J_i^k T_k0.  Written for any rank r <= 3 on FULL 4^r arrays with  */
+/* no symmetry use, in exactly that order: for every set Z of indices made  */
+/* timelike (|Z| = 0, 1, ..., r) the other r - |Z| indices are contracted   */
+/* with J one after the other.  *flops counts 2d - 1 = 5 per element each   */
+/* contraction produces (Eq. 13: 15 for rank 1, 120 for rank 2).            */
+/* ---------------------------------------------------------------------- */
+static void scj_full(int r, const real J[3][3], const real* Tin, real* Tout, double* flops) {
+  int n = 1; for (int q = 0; q < r; ++q) n *= 4;
+  double fl = 0;
+  for (int Z = 0; Z < (1 << r); ++Z) {            /* bit q of Z set: index q is timelike */
+    int pos[3], ns = 0;                          /* positions of the spatial indices */
+    for (int q = 0; q < r; ++q) if (!((Z >> q) & 1)) pos[ns++] = q;
+    int m = 1; for (int q = 0; q < ns; ++q) m *= 3;
+    real W[27], V[27];
+    /* gather the sub-tensor: spatial indices run over 1..3, the indices in Z are 0 */
+    for (int e = 0; e < m; ++e) {
+      int idx[3] = {0, 0, 0}, t = e;
+      for (int q = ns - 1; q >= 0; --q) { idx[pos[q]] = 1 + t % 3; t /= 3; }
+      int flat = 0; for (int q = 0; q < r; ++q) flat = flat * 4 + idx[q];
+      W[e] = Tin[flat];
+    }
+    /* one contraction per remaining index: W'[.. i ..] = sum_k J[i][k] W[.. k ..] */
+    for (int c = 0; c < ns; ++c) {
+      int stride = 1; for (int q = c + 1; q < ns; ++q) stride *= 3;
+      for (int e = 0; e < m; ++e) {
+        int i = (e / stride) % 3, base = e - i * stride;
+        real s = 0; for (int k = 0; k < 3; ++k) s += J[i][k] * W[base + k * stride];
+        V[e] = s; fl += 5;
+      }
+      for (int e = 0; e < m; ++e) W[e] = V[e];
+    }
+    for (int e = 0; e < m; ++e) {
+      int idx[3] = {0, 0, 0}, t = e;
+      for (int q = ns - 1; q >= 0; --q) { idx[pos[q]] = 1 + t % 3; t /= 3; }
+      int flat = 0; for (int q = 0; q < r; ++q) flat = flat * 4 + idx[q];
+      Tout[flat] = W[e];
+    }
+  }
+  (void)n;
+  if (flops) *flops = fl;
+}
+
+/* structure: 0 = T_a (rank 1), 1 = T_aa (rank 2, symmetric), 2 = T_ab (rank 2), 3 = T_abb (rank 3, T_abc = T_acb)
+ * (the four the paper's port handles). */
+static int scj_rank(int structure) { return structure == 0 ? 1 : structure == 3 ? 3 : 2; }
+
+/* one point, full arrays (4, 16, 16, 64 doubles), J[9] row-major J[3 i + k] = J_i^k; returns the flop count of the
+ * symmetry-free evaluation */
+double ora_scj_point(int structure, const double* J, const double* Tin, double* Tout) {
+  int r = scj_rank(structure), n = 1; for (int q = 0; q < r; ++q) n *= 4;
+  real Jr[3][3], a[64], b[64]; double fl = 0;
+  for (int i = 0; i < 3; ++i) for (int k = 0; k < 3; ++k) Jr[i][k] = J[3 * i + k];
+  for (int e = 0; e < n; ++e) a[e] = Tin[e];
+  scj_full(r, Jr, a, b, &fl);
+  for (int e = 0; e < n; ++e) Tout[e] = (double)b[e];
+  return fl;
+}
+
+/* Eq. 12: F / N_x = (2d-1) sum_j W(r,j) S(r,j) (r-j), by brute-force enumeration: the arrangements of j
+ * timelike indices and the spatial components that remain are counted ONCE per class under the tensor's symmetry. */
+double ora_scj_eq12(int structure) {
+  int r = scj_rank(structure);
+  int sym0 = structure == 1 ? 0 : structure == 3 ? 1 : -1;   /* the symmetric pair is (sym0, sym0 + 1) */
+  double F = 0;
+  for (int Z = 0; Z < (1 << r) - 1; ++Z) {
+    if (sym0 >= 0 && ((Z >> sym0) & 1) == 0 && ((Z >> (sym0 + 1)) & 1) == 1) continue;   /* T_..0b.. and T_..b0.. are one arrangement */
+    int ns = 0; for (int q = 0; q < r; ++q) if (!((Z >> q) & 1)) ++ns;
+    int m = 1; for (int q = 0; q < ns; ++q) m *= 3;
+    int S = 0;
+    int pairfree = sym0 >= 0 && !((Z >> sym0) & 1) && !((Z >> (sym0 + 1)) & 1);        /* both indices of the pair still spatial */
+    for (int e = 0; e < m; ++e) {
+      int idx[3] = {0, 0, 0}, pos[3], np_ = 0, t = e;
+      for (int q = 0; q < r; ++q) if (!((Z >> q) & 1)) pos[np_++] = q;
+      for (int q = ns - 1; q >= 0; --q) { idx[pos[q]] = t % 3; t /= 3; }
+      if (pairfree && idx[sym0] > idx[sym0 + 1]) continue;                                 /* count (k,l) and (l,k) once */
+      ++S;
+    }
+    F += 5.0 * S * ns;
+  }
+  return F;
+}
+
+/* packed storage of the four structures: T_a [4]; T_aa [10] (the order of SYM); T_ab [16] (4 a + b); T_abb [40] (10 a + SYM[b][c]) */
+static int scj_ne(int structure) { return structure == 0 ? 4 : structure == 1 ? 10 : structure == 2 ? 16 : 40; }
+
+/* whole arrays: J[9][P], T[N_e][P] -> out[N_e][P] (may alias T).  The packed symmetric storage is expanded to FULL arrays,
+ * transformed without symmetry use, and the upper triangle is stored back. */
+int ora_scj_subdomain(int structure, int64_t P, const double* J, const double* T, double* out) {
+  int r = scj_rank(structure), ne = scj_ne(structure), n = 1; for (int q = 0; q < r; ++q) n *= 4;
+#pragma omp parallel for schedule(static)
+  for (int64_t p = 0; p < P; ++p) {
+    real Jr[3][3], a[64], b[64];
+    for (int i = 0; i < 3; ++i) for (int k = 0; k < 3; ++k) Jr[i][k] = J[(int64_t)(3 * i + k) * P + p];
+    for (int e = 0; e < n; ++e) {
+      int c;
+      if (structure == 0 || structure == 2) c = e;
+      else if (structure == 1) c = SYM[e / 4][e % 4];
+      else c = 10 * (e / 16) + SYM[(e / 4) % 4][e % 4];
+      a[e] = T[(int64_t)c * P + p];
+    }
+    scj_full(r, Jr, a, b, NULL);
+    for (int e = 0; e < n; ++e) {
+      int c, keep = 1;
+      if (structure == 0 || structure == 2) c = e;
+      else if (structure == 1) { c = SYM[e / 4][e % 4]; keep = (e / 4) <= (e % 4); }
+      else { c = 10 * (e / 16) + SYM[(e / 4) % 4][e % 4]; keep = ((e / 4) % 4) <= (e % 4); }
+      if (keep) out[(int64_t)c * P + p] = (double)b[e];
+    }
+  }
+  (void)ne;
+  return 0;
+}
+
+/* the evolved state u[50][P]: psi_ab and Pi_ab as T_aa, Phi_iab as the spatial-first-index part of a T_abb whose timelike
+ * first index is absent (Phi has no 0ab components: the Jacobian never mixes them in, Eqs. 9-11) */
+int ora_scj_state(int64_t P, const double* J, const double* u, double* out) {
+  double* T = calloc((size_t)40 * P, sizeof(double)); double* R = malloc(sizeof(double) * 40 * P);
+  ora_scj_subdomain(1, P, J, u, out);
+  ora_scj_subdomain(1, P, J, u + 10 * P, out + 10 * P);
+  memcpy(T + 10 * P, u + 20 * P, sizeof(double) * 30 * P);
+  ora_scj_subdomain(3, P, J, T, R);
+  memcpy(out + 20 * P, R + 10 * P, sizeof(double) * 30 * P);
+  int bad = 0; for (int64_t i = 0; i < 10 * P; ++i) if (R[i] != 0) bad = 1;   /* the absent 0ab rows stay zero */
+  free(T); free(R);
   return bad;
 }

@@ -110,6 +110,14 @@ class Oracle:
         L.ora_char_bc_point.restype = C.c_int
         L.ora_filter_subdomain.argtypes = [C.POINTER(Subdomain), C.c_int, _dp, _dp, _dp, _dp]
         L.ora_filter_subdomain.restype = C.c_int
+        L.ora_scj_point.argtypes = [C.c_int, _dp, _dp, _dp]
+        L.ora_scj_point.restype = C.c_double
+        L.ora_scj_eq12.argtypes = [C.c_int]
+        L.ora_scj_eq12.restype = C.c_double
+        L.ora_scj_subdomain.argtypes = [C.c_int, C.c_int64, _dp, _dp, _dp]
+        L.ora_scj_subdomain.restype = C.c_int
+        L.ora_scj_state.argtypes = [C.c_int64, _dp, _dp, _dp]
+        L.ora_scj_state.restype = C.c_int
         self.threads = threads
         if threads is not None:
             try:
@@ -286,6 +294,35 @@ class Oracle:
         if bad:
             raise ValueError("non-physical metric")
         return out, err
+
+    # ---- O13: SpatialCoordJac (NEXT-4) -----------------------------------
+    SCJ = {"a": 0, "aa": 1, "ab": 2, "abb": 3}
+
+    def scj_point(self, structure: str, J, T):
+        """One point, FULL arrays (shape (4,), (4,4), (4,4), (4,4,4)); J[3,3] = J_i^k -> (T', flop count of the evaluation)."""
+        T = np.ascontiguousarray(T, dtype=np.float64)
+        out = np.empty_like(T)
+        fl = self.lib.ora_scj_point(self.SCJ[structure], np.ascontiguousarray(J, dtype=np.float64), T, out)
+        return out, float(fl)
+
+    def scj_eq12(self, structure: str) -> float:
+        return float(self.lib.ora_scj_eq12(self.SCJ[structure]))
+
+    def scj(self, structure: str, J, T) -> np.ndarray:
+        """Packed arrays: J[9,P], T[N_e,P] (N_e = 4, 10, 16, 40) -> T'[N_e,P]."""
+        J = np.ascontiguousarray(J, dtype=np.float64)
+        T = np.ascontiguousarray(T, dtype=np.float64)
+        out = np.empty_like(T)
+        self.lib.ora_scj_subdomain(self.SCJ[structure], T.shape[1], J, T, out)
+        return out
+
+    def scj_state(self, J, u) -> np.ndarray:
+        J = np.ascontiguousarray(J, dtype=np.float64)
+        u = np.ascontiguousarray(u, dtype=np.float64)
+        out = np.empty_like(u)
+        if self.lib.ora_scj_state(u.shape[1], J, u, out):
+            raise ValueError("SpatialCoordJac mixed a timelike first index into Phi")
+        return out
 
     def constraints(self, sd: dict, u, H, fields: bool = False):
         """-> (sums[3], maxs[3], Cfield[64,P] or None) for one subdomain."""
