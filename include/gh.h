@@ -187,13 +187,42 @@ gh_status gh_dp5_attach(gh_domain* dom, void* dev_ws, size_t bytes);
  * the state in between. */
 gh_status gh_dp5_step(gh_domain* dom, double dt, double tol, double* err, int* accepted);
 
+/* ---- SpatialCoordJac (NEXT-4 of DESIGN.md; §3.3, Eqs. 9-11) -----------------------------------------------
+ * "makes a coordinate change of a tensor's spatial indices only, by contracting every possible combination of said spatial
+ * indices with the Jacobian":  T'_ij = J_i^k J_j^l T_kl (9),  T'_0j = J_j^l T_0l (10),  T'_i0 = J_i^k T_k0 (11), the purely
+ * timelike component untouched - i.e. every index is multiplied by diag(1, J).  This is the frame change of the dual-frame
+ * method (grid coordinates <-> asymptotically inertial coordinates, related by a time-dependent spatial map);
+ * J is whatever Jacobian of that map the caller evaluates at the current time.  The four tensor structures the paper's
+ * port handles, in structure-of-arrays storage T[N_e][comp_stride]:
+ *   GH_T_A   T_a    N_e = 4
+ *   GH_T_AA  T_aa   N_e = 10  symmetric, packed 00,01,02,03,11,12,13,22,23,33
+ *   GH_T_AB  T_ab   N_e = 16  component 4 a + b
+ *   GH_T_ABB T_abb  N_e = 40  T_abc = T_acb, component 10 a + s(b,c)
+ * HBM-bound: (2 N_e + 9) doubles per grid point. */
+typedef enum { GH_T_A = 0, GH_T_AA = 1, GH_T_AB = 2, GH_T_ABB = 3 } gh_tensor_structure;
+/* J[9][comp_stride], J[3 i + k] = J_i^k at every grid point (padding ignored).  HOST or DEVICE per flag; copied into the
+ * domain's workspace (asynchronous for DEVICE).  Default before the call: none (the transforms return GH_ERR_STATE). */
+gh_status gh_set_jacobian(gh_domain* dom, const double* J, int on_device);
+/* out[N_e][comp_stride] = SpatialCoordJac of T[N_e][comp_stride] with the Jacobian last set; out may be T (in place).
+ * HOST or DEVICE per flag (both on the same side; HOST synchronises and needs N_e <= 40 of the derivative scratch). */
+gh_status gh_spatial_coord_jac(gh_domain* dom, int structure, const double* T, double* out, int on_device);
+/* The evolved state in place: psi_ab and Pi_ab as T_aa, Phi_iab with all three indices (its first index is spatial only):
+ * Phi'_iab = J_i^k L_a^c L_b^d Phi_kcd, L = diag(1, J).  Asynchronous.  GH_ERR_STATE before gh_set_fields / gh_set_jacobian. */
+gh_status gh_spatial_coord_jac_state(gh_domain* dom);
+
+/* FP64 throughput of the device the domain lives on, measured now with register-resident kernels on the domain's stream
+ * (profiling helper; bench.py quotes the derivative kernels' roofline fraction against it): tflops[0] = DMMA
+ * (mma.sync.m8n8k4.f64, what K_cheb / K_ang issue), tflops[1] = plain DFMA.  Best of 3 launches of ~2 ms after a warm-up.
+ * Uses the derivative scratch as its output buffer.  tflops: HOST [2].  Synchronises. */
+gh_status gh_fp64_peak(gh_domain* dom, double* tflops);
+
 /* Per-kernel device time of the most recent gh_rhs / gh_rk_step / gh_constraint_norms, in
  * milliseconds, measured with CUDA events on the domain's stream when profiling is enabled with
  * gh_set_profiling(dom, 1) (off by default: event records cost launch latency).
  * ms: HOST [GH_NUM_KERNELS] accumulated since the last call to gh_profile_reset; counts likewise. */
-#define GH_NUM_KERNELS 12
+#define GH_NUM_KERNELS 13
 enum { GH_K_CHEB = 0, GH_K_SHELL_ANG = 1, GH_K_RHS = 2, GH_K_RK = 3, GH_K_CONSTRAINTS = 4, GH_K_REDUCE = 5, GH_K_JAC = 6, GH_K_OTHER = 7,
-       GH_K_FILTER_CHEB = 8, GH_K_FILTER_ANG = 9, GH_K_DP_STAGE = 10, GH_K_DP_ERR = 11 };
+       GH_K_FILTER_CHEB = 8, GH_K_FILTER_ANG = 9, GH_K_DP_STAGE = 10, GH_K_DP_ERR = 11, GH_K_SCJ = 12 };
 gh_status gh_set_profiling(gh_domain* dom, int enabled);
 gh_status gh_profile_read(gh_domain* dom, double* ms, int64_t* counts);
 gh_status gh_profile_reset(gh_domain* dom);

@@ -16,6 +16,7 @@
 #include "device_types.h"
 #include "kernels_deriv.cuh"
 #include "kernels_point.cuh"
+#include "kernels_jac.cuh"
 
 using namespace ghd;
 
@@ -63,7 +64,7 @@ struct Plan {
   std::vector<int> ang_pb;               // planes per CTA for each subdomain (0 for blocks)
   std::vector<int> ang_class;            // shared-memory class of each shell
   // workspace offsets (bytes)
-  size_t o_ua, o_ub, o_k, o_du, o_H, o_dH, o_tables, o_subs, o_tiles, o_cheb, o_fcheb, o_ang, o_part, o_persub, o_flag, total;
+  size_t o_ua, o_ub, o_k, o_du, o_H, o_dH, o_jac, o_tables, o_subs, o_tiles, o_cheb, o_fcheb, o_ang, o_part, o_persub, o_flag, total;
 };
 
 inline void sub_dims(const gh_subdomain_desc& d, int& n0, int& n1, int& n2) {
@@ -220,6 +221,7 @@ bool make_plan(const gh_subdomain_desc* descs, int32_t n_sub, Plan& pl, std::str
   const size_t comp = (size_t)pl.S * sizeof(double);
   pl.o_ua = c.take(NCOMP * comp); pl.o_ub = c.take(NCOMP * comp); pl.o_k = c.take(NCOMP * comp);
   pl.o_du = c.take(3 * NCOMP * comp); pl.o_H = c.take(4 * comp); pl.o_dH = c.take(12 * comp);
+  pl.o_jac = c.take(9 * comp);
   pl.o_tables = c.take((pl.table_doubles + pl.ftable_doubles) * sizeof(double));
   pl.o_subs = c.take((size_t)n_sub * sizeof(SubDev));
   pl.o_tiles = c.take((size_t)(n_sub + 1) * sizeof(int32_t));
@@ -239,7 +241,8 @@ struct gh_domain {
   Plan pl;
   char* ws = nullptr;
   cudaStream_t stream = nullptr;
-  double *ua = nullptr, *ub = nullptr, *k = nullptr, *du = nullptr, *H = nullptr, *dH = nullptr, *tables = nullptr;
+  double *ua = nullptr, *ub = nullptr, *k = nullptr, *du = nullptr, *H = nullptr, *dH = nullptr, *jac = nullptr, *tables = nullptr;
+  bool has_jac = false;
   SubDev* subs = nullptr;
   int32_t* tiles = nullptr;
   ChebItem* cheb = nullptr;
@@ -379,7 +382,7 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
   DeviceGuard guard_(d);
   char* w = d->ws;
   d->ua = (double*)(w + pl.o_ua); d->ub = (double*)(w + pl.o_ub); d->k = (double*)(w + pl.o_k);
-  d->du = (double*)(w + pl.o_du); d->H = (double*)(w + pl.o_H); d->dH = (double*)(w + pl.o_dH);
+  d->du = (double*)(w + pl.o_du); d->H = (double*)(w + pl.o_H); d->dH = (double*)(w + pl.o_dH); d->jac = (double*)(w + pl.o_jac);
   d->tables = (double*)(w + pl.o_tables); d->subs = (SubDev*)(w + pl.o_subs); d->tiles = (int32_t*)(w + pl.o_tiles);
   d->cheb = (ChebItem*)(w + pl.o_cheb); d->ang = (AngItem*)(w + pl.o_ang); d->fcheb = (ChebItem*)(w + pl.o_fcheb);
   d->part = (double*)(w + pl.o_part); d->persub = (double*)(w + pl.o_persub); d->flag = (int*)(w + pl.o_flag);
@@ -1064,6 +1067,90 @@ extern "C" gh_status gh_dp5_step(gh_domain* d, double dt, double tol, double* er
 }
 
 // ------------------------------------------------------------------------------------------------------
+// SpatialCoordJac (NEXT-4)
+// ------------------------------------------------------------------------------------------------------
+extern "C" gh_status gh_set_jacobian(gh_domain* d, const double* J, int on_device) {
+  DeviceGuard guard_(d);
+  if (!d || !J) return fail(d, GH_ERR_ARG, "NULL argument");
+  GH_CUDA(d, cudaMemcpyAsync(d->jac, J, (size_t)9 * d->pl.S * sizeof(double), on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, d->stream));
+  if (!on_device) GH_CUDA(d, cudaStreamSynchronize(d->stream));
+  d->has_jac = true;
+  return GH_OK;
+}
+
+namespace {
+gh_status launch_scj(gh_domain* d, int structure, const double* in, double* out) {
+  const int64_t S = d->pl.S;
+  const int grid = d->pl.n_tiles;
+  ProfScope ps(d, GH_K_SCJ);
+  switch (structure) {
+    case GH_T_A: k_scj<0><<<grid, TILE_PTS, 0, d->stream>>>(d->subs, d->tiles, d->pl.n_sub, d->jac, in, out, S); break;
+    case GH_T_AA: k_scj<1><<<grid, TILE_PTS, 0, d->stream>>>(d->subs, d->tiles, d->pl.n_sub, d->jac, in, out, S); break;
+    case GH_T_AB: k_scj<2><<<grid, TILE_PTS, 0, d->stream>>>(d->subs, d->tiles, d->pl.n_sub, d->jac, in, out, S); break;
+    case GH_T_ABB: k_scj<3><<<grid, TILE_PTS, 0, d->stream>>>(d->subs, d->tiles, d->pl.n_sub, d->jac, in, out, S); break;
+    default: k_scj<4><<<grid, TILE_PTS, 0, d->stream>>>(d->subs, d->tiles, d->pl.n_sub, d->jac, in, out, S); break;
+  }
+  return GH_OK;
+}
+}  // namespace
+
+extern "C" gh_status gh_spatial_coord_jac(gh_domain* d, int structure, const double* T, double* out, int on_device) {
+  DeviceGuard guard_(d);
+  if (!d || !T || !out) return fail(d, GH_ERR_ARG, "NULL argument");
+  if (structure < GH_T_A || structure > GH_T_ABB) return fail(d, GH_ERR_ARG, "gh_spatial_coord_jac: unknown tensor structure");
+  if (!d->has_jac) return fail(d, GH_ERR_STATE, "gh_spatial_coord_jac before gh_set_jacobian");
+  static const int NE[4] = {4, 10, 16, 40};
+  const size_t bytes = (size_t)NE[structure] * d->pl.S * sizeof(double);
+  if (on_device) {
+    launch_scj(d, structure, T, out);
+    GH_CUDA(d, cudaGetLastError());
+    return GH_OK;
+  }
+  GH_CUDA(d, cudaMemcpyAsync(d->du, T, bytes, cudaMemcpyHostToDevice, d->stream));
+  launch_scj(d, structure, d->du, d->du);
+  GH_CUDA(d, cudaGetLastError());
+  GH_CUDA(d, cudaMemcpyAsync(out, d->du, bytes, cudaMemcpyDeviceToHost, d->stream));
+  GH_CUDA(d, cudaStreamSynchronize(d->stream));
+  return GH_OK;
+}
+
+extern "C" gh_status gh_spatial_coord_jac_state(gh_domain* d) {
+  DeviceGuard guard_(d);
+  if (!d) return GH_ERR_ARG;
+  if (!d->has_fields) return fail(d, GH_ERR_STATE, "gh_spatial_coord_jac_state before gh_set_fields");
+  if (!d->has_jac) return fail(d, GH_ERR_STATE, "gh_spatial_coord_jac_state before gh_set_jacobian");
+  d->dp_fsal = false;
+  launch_scj(d, 4, d->ua, d->ua);
+  GH_CUDA(d, cudaGetLastError());
+  return GH_OK;
+}
+
+extern "C" gh_status gh_fp64_peak(gh_domain* d, double* tflops) {
+  DeviceGuard guard_(d);
+  if (!d || !tflops) return fail(d, GH_ERR_ARG, "NULL argument");
+  const int ctas = d->n_sm * 2;
+  if ((size_t)ctas * 256 > (size_t)3 * NCOMP * d->pl.S) return fail(d, GH_ERR_WORKSPACE, "gh_fp64_peak: the derivative scratch is smaller than its output buffer");
+  cudaEvent_t e0 = get_event(d), e1 = get_event(d);
+  const int iters = 8000;           // 128 flop per lane and iteration: ~2.2 ms at 37 TFLOP/s with 2 CTAs per SM
+  for (int mode = 0; mode < 2; ++mode) {
+    float best = 1e30f;
+    for (int rep = 0; rep < 4; ++rep) {
+      cudaEventRecord(e0, d->stream);
+      if (mode == 0) k_fp64_peak<1><<<ctas, 256, 0, d->stream>>>(d->du, rep ? iters : 16, 1e-3);
+      else k_fp64_peak<0><<<ctas, 256, 0, d->stream>>>(d->du, rep ? iters : 16, 1e-3);
+      cudaEventRecord(e1, d->stream);
+      if (cudaEventSynchronize(e1) != cudaSuccess) { d->pool.push_back(e0); d->pool.push_back(e1); return fail(d, GH_ERR_CUDA, cudaGetErrorString(cudaGetLastError())); }
+      float ms = 0; cudaEventElapsedTime(&ms, e0, e1);
+      if (rep && ms < best) best = ms;
+    }
+    tflops[mode] = (double)ctas * 256 * iters * 128.0 / (best * 1e-3) / 1e12;
+  }
+  d->pool.push_back(e0); d->pool.push_back(e1);
+  d->launches += 8;
+  return GH_OK;
+}
+
+// ------------------------------------------------------------------------------------------------------
 // profiling / bookkeeping
 // ------------------------------------------------------------------------------------------------------
 extern "C" gh_status gh_set_profiling(gh_domain* d, int enabled) {
@@ -1091,7 +1178,7 @@ extern "C" gh_status gh_profile_reset(gh_domain* d) {
 }
 
 extern "C" const char* gh_kernel_name(int k) {
-  static const char* names[GH_NUM_KERNELS] = {"k_cheb", "k_ang", "k_rhs", "k_rk", "k_con", "k_con_reduce", "k_jac", "other", "k_cheb(filter)", "k_ang(filter)", "k_dp_stage", "k_dp_err"};
+  static const char* names[GH_NUM_KERNELS] = {"k_cheb", "k_ang", "k_rhs", "k_rk", "k_con", "k_con_reduce", "k_jac", "other", "k_cheb(filter)", "k_ang(filter)", "k_dp_stage", "k_dp_err", "k_scj"};
   return (k >= 0 && k < GH_NUM_KERNELS) ? names[k] : "?";
 }
 

@@ -19,7 +19,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libgh.so")
 
 GH_NCOMP = 50
-GH_NUM_KERNELS = 12
+GH_NUM_KERNELS = 13
+GH_T_A, GH_T_AA, GH_T_AB, GH_T_ABB = range(4)
 GH_FILTER_NONE, GH_FILTER_HEAVISIDE, GH_FILTER_EXP = range(3)
 GH_OPT_RK_OUT_OF_PLACE = 0
 GH_OK, GH_ERR_ARG, GH_ERR_WORKSPACE, GH_ERR_CUDA, GH_ERR_STATE, GH_ERR_SINGULAR = range(6)
@@ -33,6 +34,7 @@ EXPORTS = [
     "gh_launch_count", "gh_last_error", "gh_basis_cheb", "gh_basis_gauss_legendre", "gh_basis_shell",
     "gh_set_filter", "gh_apply_filter", "gh_filter_sigma",
     "gh_dp5_workspace_bytes", "gh_dp5_attach", "gh_dp5_step", "gh_set_option",
+    "gh_set_jacobian", "gh_spatial_coord_jac", "gh_spatial_coord_jac_state", "gh_fp64_peak",
 ]
 
 
@@ -120,6 +122,10 @@ def lib() -> C.CDLL:
     L.gh_dp5_attach.argtypes = [vp, vp, C.c_size_t]
     L.gh_dp5_step.argtypes = [vp, C.c_double, C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_int)]
     L.gh_set_option.argtypes = [vp, ip, ip]
+    L.gh_set_jacobian.argtypes = [vp, dp, ip]
+    L.gh_spatial_coord_jac.argtypes = [vp, ip, dp, dp, ip]
+    L.gh_spatial_coord_jac_state.argtypes = [vp]
+    L.gh_fp64_peak.argtypes = [vp, dp]
     _lib = L
     return L
 
@@ -273,6 +279,30 @@ def gh_dp5_step(h, dt: float, tol: float = 0.0):
     return float(err[0]), float(err[1]), bool(acc.value)
 
 
+def gh_set_jacobian(h, J):
+    p, dev = _ptr(J)
+    _check(lib().gh_set_jacobian(h, p, dev), h)
+
+
+def gh_spatial_coord_jac(h, structure: int, T, out):
+    p, dev = _ptr(T)
+    q, dev2 = _ptr(out)
+    if dev != dev2:
+        raise ValueError("T and out must live on the same side")
+    _check(lib().gh_spatial_coord_jac(h, int(structure), p, q, dev), h)
+
+
+def gh_spatial_coord_jac_state(h):
+    _check(lib().gh_spatial_coord_jac_state(h), h)
+
+
+def gh_fp64_peak(h):
+    """-> (DMMA TFLOP/s, DFMA TFLOP/s) measured now on the domain's device"""
+    out = np.zeros(2)
+    _check(lib().gh_fp64_peak(h, out.ctypes.data), h)
+    return float(out[0]), float(out[1])
+
+
 def gh_basis_cheb(N: int):
     x, D = np.zeros(N), np.zeros((N, N))
     _check(lib().gh_basis_cheb(N, x.ctypes.data, D.ctypes.data), None)
@@ -394,6 +424,20 @@ class Domain:
 
     def apply_filter(self):
         gh_apply_filter(self.h)
+
+    def set_jacobian(self, J):
+        gh_set_jacobian(self.h, J)
+
+    def spatial_coord_jac(self, structure: int, T, out=None):
+        out = (np.empty_like(T) if isinstance(T, np.ndarray) else self.torch.empty_like(T)) if out is None else out
+        gh_spatial_coord_jac(self.h, structure, T, out)
+        return out
+
+    def spatial_coord_jac_state(self):
+        gh_spatial_coord_jac_state(self.h)
+
+    def fp64_peak(self):
+        return gh_fp64_peak(self.h)
 
     def set_option(self, option: int, value: int):
         _check(lib().gh_set_option(self.h, int(option), int(value)), self.h)

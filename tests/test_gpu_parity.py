@@ -518,7 +518,12 @@ def test_nan_reaches_the_reported_maxima(oracle):
     dom.set_fields(dom.pack(bad), 0.0)
     out, per = dom.constraint_norms(per_sub=True)
     assert np.isnan(out[0, 1]) and np.isnan(out[0, 0]) and np.isnan(per[1, 0, 1]) and np.isfinite(per[0]).all()
+    # a Dormand-Prince step from that state is never accepted: either the NaN has spread into psi by a later stage (singular
+    # flag) or the estimate itself is NaN
     dom.dp5_attach()
-    rms, mx, acc = dom.dp5_step(1e-3)
-    assert not acc and (np.isnan(mx) or np.isnan(rms))
+    try:
+        rms, mx, acc = dom.dp5_step(1e-3)
+        assert not acc and (np.isnan(mx) or np.isnan(rms))
+    except gh.GHError as e:
+        assert e.status == gh.GH_ERR_SINGULAR
     dom.close()
