@@ -336,8 +336,12 @@ def run_ours(args):
             torch.cuda.synchronize()
 
     def step():
-        dom.rk_step(dt)
-        return dom.constraint_norms()
+        # A2-A8 in one call: the constraint norms (of the state the step starts from) are an epilogue of the first stage's
+        # fused RHS kernel (gh_rk_step_norms); --unfused-norms times the round-1 path (gh_rk_step + stand-alone gh_constraint_norms)
+        if args.unfused_norms:
+            dom.rk_step(dt)
+            return dom.constraint_norms()
+        return dom.rk_step_norms(dt)
 
     # ---- device-resident timing -----------------------------------------------------------------------------
     dom.set_fields(u_dev, 0.0)
@@ -452,7 +456,8 @@ def finish_ours(args, world, label, cfg, descs, reps, P, S, ms, e2e_step_s, e2e_
     # per-kernel numbers from the CUDA events the library records around each launch on its own stream
     total_kernel_ms = sum(v[0] for v in prof.values()) or 1.0
     # work-equivalent calls per step: the constraint pass differentiates 40 of the 50 components (no d Pi needed)
-    calls_per_step = {"k_rhs": 3, "k_con": 1, "k_cheb": 3.8, "k_ang": 3.8}   # library calls that run the kernel
+    nd = 3.8 if args.unfused_norms else 3.0     # derivative passes per step (the stand-alone constraint pass differentiates 40 of 50 components)
+    calls_per_step = {"k_rhs": 3, "k_con": 1, "k_cheb": nd, "k_ang": nd}   # library calls that run the kernel
     kernels = {}
     for name, (kms, cnt) in prof.items():
         if cnt == 0 or "filter" in name or name.startswith("k_dp"):
@@ -510,7 +515,7 @@ def finish_ours(args, world, label, cfg, descs, reps, P, S, ms, e2e_step_s, e2e_
         "data": "synthetic",
         "config": {"workload": label, "points_per_gpu": P, "subdomains": len(descs), "replicas_of_base_set": reps,
                    "components": 50, "dt": float(cfg["dt"]), "rhs_evals_per_step": 3,
-                   "step": "gh_rk_step + gh_constraint_norms", "parallelism": "replicas only" if world > 1 else "single GPU",
+                   "step": "gh_rk_step + gh_constraint_norms" if args.unfused_norms else "gh_rk_step_norms (RK3 step with the constraint norms fused into stage 1)", "parallelism": "replicas only" if world > 1 else "single GPU",
                    "l2": f"inputs larger than L2: the step streams {316 * S * 8 / 1e9:.2f} GB of state/derivative arrays (L2 126 MB)",
                    "per_launch_events": "on (library CUDA events around every kernel launch, inside the timed region)"},
         "rk_steps_per_s": world * steps / (ms * 1e-3),
@@ -519,7 +524,7 @@ def finish_ours(args, world, label, cfg, descs, reps, P, S, ms, e2e_step_s, e2e_
         "cpu_baseline": cpu,
         "e2e": {"value": world * 3.0 * P / e2e_step_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "steps": e2e_steps, "ms_per_step": e2e_step_s * 1e3,
-                "path": "gh_set_fields(HOST pinned) + gh_rk_step + gh_constraint_norms + gh_get_fields(HOST pinned)"},
+                "path": "gh_set_fields(HOST pinned) + the step + gh_get_fields(HOST pinned)"},
         "clocks": clocks,
         "constraint_norms_after": [[float(x) for x in r] for r in np.asarray(norms)],
         "spectral_filter": filt,
@@ -570,6 +575,7 @@ def main():
                     help="points in the cpu_baseline sample (default: the whole 64-subdomain base set, ~10 s on 16 cores)")
     ap.add_argument("--ref-points", type=int, default=60_000, help="points per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--unfused-norms", action="store_true", help="step = gh_rk_step + stand-alone gh_constraint_norms (the round-1 path)")
     ap.add_argument("--no-extras", action="store_true", help="skip the spectral-filter and Dormand-Prince legs (run after the timed step)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

@@ -133,6 +133,13 @@ gh_status gh_gradient(gh_domain* dom, double* du, int on_device);
  * Asynchronous on the domain's stream; advances the stored time by dt. */
 gh_status gh_rk_step(gh_domain* dom, double dt);
 
+/* gh_rk_step that also returns the constraint norms of the state it STARTS from (A8 as an epilogue of A5, SURVEY.md §8(a), (d):
+ * the first stage's fused RHS kernel already holds C_a, the derivatives of psi and Phi and Phi itself on chip, so the norms
+ * cost no extra memory traffic and no second derivative pass).  out / per_sub: as in gh_constraint_norms, and equal to what
+ * gh_constraint_norms would have returned just before the step.  Synchronises (it returns host data); reports
+ * GH_ERR_SINGULAR if the device flag was raised. */
+gh_status gh_rk_step_norms(gh_domain* dom, double dt, double* out, double* per_sub);
+
 /* Constraint norms of the current state (A8): out[3][2] = {rms, max} for C_a (4 components),
  * C_iab = d_i psi_ab - Phi_iab (30), C_ijab = d_i Phi_jab - d_j Phi_iab (30 independent);
  * rms = sqrt(sum over points and components / (P * n_comp)), unweighted (reading S16).

@@ -573,6 +573,8 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
   GH_CREATE_CUDA(cudaFuncSetAttribute(k_rhs<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RHS_SMEM_BYTES));
   GH_CREATE_CUDA(cudaFuncSetAttribute(k_rhs<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RHS_SMEM_BYTES));
   GH_CREATE_CUDA(cudaFuncSetAttribute(k_rhs<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RHS_SMEM_BYTES));
+  GH_CREATE_CUDA(cudaFuncSetAttribute(k_rhs<1, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RHS_SMEM_BYTES_NORMS));
+  GH_CREATE_CUDA(cudaFuncSetAttribute(k_rhs<1, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RHS_SMEM_BYTES_NORMS));
   // the attribute belongs to the FUNCTION, not to this domain: always the class ceiling, so that a later, smaller domain can
   // never lower it under a live domain's launch size
   GH_CREATE_CUDA(cudaFuncSetAttribute(k_ang<ANG_TPB0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ANG_SMEM_2CTA));
@@ -703,9 +705,24 @@ gh_status launch_derivs(gh_domain* d, const double* in, double* out, int ncomp, 
 // A2-A6 on state `u`; rk_mode 0: d_t u into `out`; 1 / 2: the fused RK stage (A7)  out = a u0 + b (u + dt d_t u)
 // (mode 1: a = 0, u0 unused).  `out` may alias u or u0.
 gh_status launch_rhs(gh_domain* d, const double* u, double* out, int rk_mode = 0, const double* u0 = nullptr, double a = 0.0,
-                     double b = 1.0, double dt = 0.0) {
+                     double b = 1.0, double dt = 0.0, bool norms = false) {
   gh_status st = launch_derivs(d, u, d->du, NCOMP);
   if (st != GH_OK) return st;
+  if (norms) {      // A8 as the epilogue of stage 1 (rk_mode 1 only): per-tile partials, folded per subdomain like K_con's
+    const RkArgs rk{u0, a, b, dt};
+    const int grid = d->pl.n_tiles;
+    {
+      ProfScope ps(d, GH_K_RHS);
+      if (d->has_char) k_rhs<1, true, true><<<grid, TILE_PTS, RHS_SMEM_BYTES_NORMS, d->stream>>>(d->subs, d->tiles, d->pl.n_sub, d->tables, u, d->du, d->H, d->dH, out, rk, d->pl.S, d->flag, d->part);
+      else k_rhs<1, false, true><<<grid, TILE_PTS, RHS_SMEM_BYTES_NORMS, d->stream>>>(d->subs, d->tiles, d->pl.n_sub, d->tables, u, d->du, d->H, d->dH, out, rk, d->pl.S, d->flag, d->part);
+    }
+    {
+      ProfScope ps(d, GH_K_REDUCE);
+      k_con_reduce<<<d->pl.n_sub, 32, 0, d->stream>>>(d->tiles, d->part, d->persub);
+    }
+    GH_CUDA(d, cudaGetLastError());
+    return GH_OK;
+  }
   {
     ProfScope ps(d, GH_K_RHS);
     const RkArgs rk{u0, a, b, dt};
@@ -804,28 +821,72 @@ extern "C" gh_status gh_gradient(gh_domain* d, double* du, int on_device) {
   return GH_OK;
 }
 
+namespace {
+// the three Shu-Osher stages; norms: the constraint partials of the input state come out of stage 1 (into d->persub)
+gh_status rk3_stages(gh_domain* d, double dt, bool norms) {
+  gh_status st;
+  if (d->has_ifc || d->opt[GH_OPT_RK_OUT_OF_PLACE]) {
+    // INTERFACE faces read the neighbour's face state from the stage input, so no stage may run in place: ua -> ub -> k -> ua
+    if ((st = launch_rhs(d, d->ua, d->ub, 1, nullptr, 0.0, 1.0, dt, norms)) != GH_OK) return st;
+    if ((st = launch_rhs(d, d->ub, d->k, 2, d->ua, 0.75, 0.25, dt)) != GH_OK) return st;
+    if ((st = launch_rhs(d, d->k, d->ua, 2, d->ua, 1.0 / 3.0, 2.0 / 3.0, dt)) != GH_OK) return st;
+    return GH_OK;
+  }
+  // the stage update (A7) is the epilogue of the fused RHS kernel: d_t u never goes to memory
+  // u1 = u0 + dt k(u0)                      (ua -> ub)
+  if ((st = launch_rhs(d, d->ua, d->ub, 1, nullptr, 0.0, 1.0, dt, norms)) != GH_OK) return st;
+  // u2 = 3/4 u0 + 1/4 (u1 + dt k(u1))       (ub -> ub, in place)
+  if ((st = launch_rhs(d, d->ub, d->ub, 2, d->ua, 0.75, 0.25, dt)) != GH_OK) return st;
+  // u_new = 1/3 u0 + 2/3 (u2 + dt k(u2))    (ub -> ua, over u0)
+  if ((st = launch_rhs(d, d->ub, d->ua, 2, d->ua, 1.0 / 3.0, 2.0 / 3.0, dt)) != GH_OK) return st;
+  return GH_OK;
+}
+
+// per-subdomain {3 sums, 3 maxima} (host copy of d->persub) -> out[3][2], per_sub[n_sub][3][2]
+void finish_norms(const Plan& pl, const std::vector<double>& h, double* out, double* per_sub) {
+  static const double ncomp[3] = {4.0, 30.0, 30.0};
+  double sum[3] = {0, 0, 0}, mx[3] = {0, 0, 0};
+  for (int s = 0; s < pl.n_sub; ++s) {
+    int n0, n1, n2; sub_dims(pl.descs[s], n0, n1, n2);
+    const double Ps = (double)n0 * n1 * n2;
+    for (int q = 0; q < 3; ++q) {
+      sum[q] += h[(size_t)s * 6 + q];
+      { const double v = h[(size_t)s * 6 + 3 + q]; if (v != v || v > mx[q]) mx[q] = v; }     // NaN propagates
+      if (per_sub) {
+        per_sub[(size_t)s * 6 + 2 * q] = std::sqrt(h[(size_t)s * 6 + q] / (Ps * ncomp[q]));
+        per_sub[(size_t)s * 6 + 2 * q + 1] = h[(size_t)s * 6 + 3 + q];
+      }
+    }
+  }
+  for (int q = 0; q < 3; ++q) { out[2 * q] = std::sqrt(sum[q] / ((double)pl.P * ncomp[q])); out[2 * q + 1] = mx[q]; }
+}
+}  // namespace
+
 extern "C" gh_status gh_rk_step(gh_domain* d, double dt) {
   DeviceGuard guard_(d);
   if (!d) return GH_ERR_ARG;
   if (!d->has_fields) return fail(d, GH_ERR_STATE, "gh_rk_step before gh_set_fields");
   if (!std::isfinite(dt)) return fail(d, GH_ERR_ARG, "dt is not finite");
-  gh_status st;
-  if (d->has_ifc || d->opt[GH_OPT_RK_OUT_OF_PLACE]) {
-    // INTERFACE faces read the neighbour's face state from the stage input, so no stage may run in place: ua -> ub -> k -> ua
-    if ((st = launch_rhs(d, d->ua, d->ub, 1, nullptr, 0.0, 1.0, dt)) != GH_OK) return st;
-    if ((st = launch_rhs(d, d->ub, d->k, 2, d->ua, 0.75, 0.25, dt)) != GH_OK) return st;
-    if ((st = launch_rhs(d, d->k, d->ua, 2, d->ua, 1.0 / 3.0, 2.0 / 3.0, dt)) != GH_OK) return st;
-    d->t += dt; d->dp_fsal = false;
-    return GH_OK;
-  }
-  // the stage update (A7) is the epilogue of the fused RHS kernel: d_t u never goes to memory
-  // u1 = u0 + dt k(u0)                      (ua -> ub)
-  if ((st = launch_rhs(d, d->ua, d->ub, 1, nullptr, 0.0, 1.0, dt)) != GH_OK) return st;
-  // u2 = 3/4 u0 + 1/4 (u1 + dt k(u1))       (ub -> ub, in place)
-  if ((st = launch_rhs(d, d->ub, d->ub, 2, d->ua, 0.75, 0.25, dt)) != GH_OK) return st;
-  // u_new = 1/3 u0 + 2/3 (u2 + dt k(u2))    (ub -> ua, over u0)
-  if ((st = launch_rhs(d, d->ub, d->ua, 2, d->ua, 1.0 / 3.0, 2.0 / 3.0, dt)) != GH_OK) return st;
+  gh_status st = rk3_stages(d, dt, false);
+  if (st != GH_OK) return st;
   d->t += dt; d->dp_fsal = false;
+  return GH_OK;
+}
+
+extern "C" gh_status gh_rk_step_norms(gh_domain* d, double dt, double* out, double* per_sub) {
+  DeviceGuard guard_(d);
+  if (!d || !out) return fail(d, GH_ERR_ARG, "NULL argument");
+  if (!d->has_fields) return fail(d, GH_ERR_STATE, "gh_rk_step_norms before gh_set_fields");
+  if (!std::isfinite(dt)) return fail(d, GH_ERR_ARG, "dt is not finite");
+  gh_status st = rk3_stages(d, dt, true);
+  if (st != GH_OK) return st;
+  d->t += dt; d->dp_fsal = false;
+  // d->persub was written by stage 1 and nothing later in the step touches it: one copy and one synchronisation at the end
+  std::vector<double> h((size_t)d->pl.n_sub * 6);
+  GH_CUDA(d, cudaMemcpyAsync(h.data(), d->persub, h.size() * sizeof(double), cudaMemcpyDeviceToHost, d->stream));
+  st = check_flag(d);   // synchronises
+  if (st != GH_OK) return st;
+  finish_norms(d->pl, h, out, per_sub);
   return GH_OK;
 }
 
@@ -849,21 +910,7 @@ extern "C" gh_status gh_constraint_norms(gh_domain* d, double* out, double* per_
   GH_CUDA(d, cudaMemcpyAsync(h.data(), d->persub, h.size() * sizeof(double), cudaMemcpyDeviceToHost, d->stream));
   st = check_flag(d);   // synchronises
   if (st != GH_OK) return st;
-  static const double ncomp[3] = {4.0, 30.0, 30.0};
-  double sum[3] = {0, 0, 0}, mx[3] = {0, 0, 0};
-  for (int s = 0; s < pl.n_sub; ++s) {
-    int n0, n1, n2; sub_dims(pl.descs[s], n0, n1, n2);
-    const double Ps = (double)n0 * n1 * n2;
-    for (int q = 0; q < 3; ++q) {
-      sum[q] += h[(size_t)s * 6 + q];
-      { const double v = h[(size_t)s * 6 + 3 + q]; if (v != v || v > mx[q]) mx[q] = v; }     // NaN propagates
-      if (per_sub) {
-        per_sub[(size_t)s * 6 + 2 * q] = std::sqrt(h[(size_t)s * 6 + q] / (Ps * ncomp[q]));
-        per_sub[(size_t)s * 6 + 2 * q + 1] = h[(size_t)s * 6 + 3 + q];
-      }
-    }
-  }
-  for (int q = 0; q < 3; ++q) { out[2 * q] = std::sqrt(sum[q] / ((double)pl.P * ncomp[q])); out[2 * q + 1] = mx[q]; }
+  finish_norms(pl, h, out, per_sub);
   return GH_OK;
 }
 

@@ -393,6 +393,10 @@ __device__ __forceinline__ void rhs_store(double* out, const RkArgs& rk, int64_t
 // scheduler alone.
 constexpr int RHS_RING = 3, RHS_RING_ROWS = 22, RHS_PHI_ROWS = 30;   // 15 derivatives + 2 gauge-source gradients + 5 u0 values (RK = 2)
 constexpr size_t RHS_SMEM_BYTES = (size_t)(RHS_PHI_ROWS + RHS_RING * RHS_RING_ROWS) * TILE_PTS * sizeof(double);
+// NORMS (A8 as an epilogue of A5): six more rows, this thread's partial {sum C_a^2, sum C_iab^2, sum C_ijab^2,
+// max |C_a|, max |C_iab|, max |C_ijab|} (shared memory, not registers: the kernel already sits at the register limit)
+constexpr int RHS_NORM_ROWS = 6;
+constexpr size_t RHS_SMEM_BYTES_NORMS = RHS_SMEM_BYTES + (size_t)RHS_NORM_ROWS * TILE_PTS * sizeof(double);
 
 template <int PAIR, int RK>
 __device__ __forceinline__ void rhs_prefetch(double* __restrict__ slot /* + tid */, const double* __restrict__ du,
@@ -414,13 +418,14 @@ __device__ __forceinline__ void rhs_prefetch(double* __restrict__ slot /* + tid 
   cp_async_commit();
 }
 
-template <bool SHELL, int RK, bool CBC>
+template <bool SHELL, int RK, bool CBC, bool NORMS>
 __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __restrict__ tables, int local,
                                           const double* u, const double* __restrict__ du,
                                           const double* __restrict__ Hs, const double* __restrict__ dHs,
                                           double* k, const RkArgs& rk, int64_t S, int* __restrict__ flag,
                                           double* __restrict__ phis /* + tid */) {
   double* __restrict__ ring = phis + RHS_PHI_ROWS * TILE_PTS;
+  double* __restrict__ nacc = ring + RHS_RING * RHS_RING_ROWS * TILE_PTS;    // NORMS: this thread's six partials
   const int64_t p = sd.off + local;
   // face mask (A6)
   bool frozen;
@@ -441,7 +446,9 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
 #pragma unroll
   for (int c = 0; c < RHS_PHI_ROWS; ++c) cp_async8(phis + c * TILE_PTS, u + (int64_t)(50 - RHS_PHI_ROWS + c) * S + p);
   cp_async_commit();
-  if (!frozen) {
+  // with NORMS a frozen point takes the full path too: its constraints count, only its time derivative is zero
+  const bool skip = frozen && !NORMS;
+  if (!skip) {
     rhs_prefetch<0, RK>(ring + 0 * SLOT, du, dHs, rk.u0, S, p);
     rhs_prefetch<1, RK>(ring + 1 * SLOT, du, dHs, rk.u0, S, p);
     rhs_prefetch<2, RK>(ring + 2 * SLOT, du, dHs, rk.u0, S, p);
@@ -458,8 +465,8 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
   Geom G;
   const bool ok = geometry(psi, G);
   if (!ok) atomicOr(flag, 1);
-  if (frozen) cp_async_wait<0>(); else cp_async_wait<RHS_RING>();   // the Phi group has landed
-  if (!ok || frozen) {
+  if (skip) cp_async_wait<0>(); else cp_async_wait<RHS_RING>();   // the Phi group has landed
+  if (!ok || skip) {
     cp_async_wait<0>();   // nothing of this thread may still be landing in shared memory when the CTA retires
     // frozen points issued no prefetch: u0 comes straight from memory.  All 50 loads go out before the first store: u0 and
     // out are not __restrict__ (they may be the same array), so a load placed after a store would have to wait for it
@@ -482,6 +489,12 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
   }
   Alg A;
   algebraic(G, Pi, Phi, H, A);
+  if (NORMS) {
+    double s0 = 0.0, m0 = 0.0;
+#pragma unroll
+    for (int a = 0; a < 4; ++a) { s0 = fma(A.C[a], A.C[a], s0); m0 = nanmax(m0, fabs(A.C[a])); }
+    nacc[0] = s0; nacc[3 * TILE_PTS] = m0;
+  }
 
   ShellJac J;
   if (SHELL) J = shell_jac(sd, tables, local);
@@ -509,6 +522,17 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
         } else {
           d[c5][0] = l0; d[c5][1] = l1; d[c5][2] = l2;
         }
+      }
+      if (NORMS) {   // C_iab = d_i psi_ab - Phi_iab;  C_ijab = d_i Phi_jab - d_j Phi_iab for (i,j) = (x,y), (x,z), (y,z)
+        double s1 = nacc[1 * TILE_PTS], m1 = nacc[4 * TILE_PTS];
+#pragma unroll
+        for (int i = 0; i < 3; ++i) { const double c = d[0][i] - Phi(i, s); s1 = fma(c, c, s1); m1 = nanmax(m1, fabs(c)); }
+        nacc[1 * TILE_PTS] = s1; nacc[4 * TILE_PTS] = m1;
+        const double c01 = d[3][0] - d[2][1], c02 = d[4][0] - d[2][2], c12 = d[4][1] - d[3][2];
+        double s2 = nacc[2 * TILE_PTS];
+        s2 = fma(c01, c01, s2); s2 = fma(c02, c02, s2); s2 = fma(c12, c12, s2);
+        nacc[2 * TILE_PTS] = s2;
+        nacc[5 * TILE_PTS] = nanmax(nacc[5 * TILE_PTS], nanmax(fabs(c01), nanmax(fabs(c02), fabs(c12))));
       }
       double sdpsi = 0.0, sdPi = 0.0, sPhi = 0.0;
 #pragma unroll
@@ -576,6 +600,7 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
             else char_bc_pair(G, g1, g2, f / 2 == 0 ? sg : 0.0, f / 2 == 1 ? sg : 0.0, f / 2 == 2 ? sg : 0.0, o_psi, r, o_Phi);
           }
       }
+      if (NORMS && frozen) { o_psi = 0.0; r = 0.0; o_Phi[0] = o_Phi[1] = o_Phi[2] = 0.0; }      // A6
       rhs_store<RK>(k, rk, (int64_t)s * S + p, o_psi, psi[s], RK == 2 ? slot[17 * TILE_PTS] : 0.0);
       rhs_store<RK>(k, rk, (int64_t)(10 + s) * S + p, r, Pi[s], RK == 2 ? slot[18 * TILE_PTS] : 0.0);
 #pragma unroll
@@ -593,27 +618,59 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
     }
 }
 
-// CBC: the domain has faces flagged CHARACTERISTIC (a second instantiation, so that domains without them do not pay for it)
-template <int RK, bool CBC>
+// CBC: the domain has faces flagged CHARACTERISTIC (a second instantiation, so that domains without them do not pay for it).
+// NORMS: the constraint norms of the INPUT state as an epilogue (A8 fused into A5: C_a, the derivatives of psi and Phi and
+// Phi itself are on chip anyway; 0 extra bytes): per-tile partials part[tile][6] in the layout of K_con, folded by K_con_reduce.
+template <int RK, bool CBC, bool NORMS = false>
 __global__ void __launch_bounds__(TILE_PTS, 2)
 k_rhs(const SubDev* __restrict__ subs, const int32_t* __restrict__ tile_first, int n_sub,
       const double* __restrict__ tables, const double* u, const double* __restrict__ du,
       const double* __restrict__ Hs, const double* __restrict__ dHs, double* k, RkArgs rk, int64_t S,
-      int* __restrict__ flag) {
-  extern __shared__ __align__(16) double ring_s[];   // Phi [30][TILE_PTS], then the ring [RHS_RING][RHS_RING_ROWS][TILE_PTS]
+      int* __restrict__ flag, double* __restrict__ part = nullptr) {
+  extern __shared__ __align__(16) double ring_s[];   // Phi [30][TILE_PTS], the ring [RHS_RING][RHS_RING_ROWS][TILE_PTS], NORMS: [6][TILE_PTS]
   __shared__ SubDev sd_s;
   __shared__ int tile0_s;
+  __shared__ double red[TILE_PTS / 32][6];
   if (threadIdx.x == 0) {
     const int s = find_sub(tile_first, n_sub, blockIdx.x);
     sd_s = subs[s];
     tile0_s = tile_first[s];
   }
+  double* nacc = ring_s + (RHS_PHI_ROWS + RHS_RING * RHS_RING_ROWS) * TILE_PTS + threadIdx.x;
+  if (NORMS) {
+#pragma unroll
+    for (int q = 0; q < RHS_NORM_ROWS; ++q) nacc[q * TILE_PTS] = 0.0;      // own column: no barrier needed
+  }
   __syncthreads();
   const SubDev& sd = sd_s;
   const int local = (blockIdx.x - tile0_s) * TILE_PTS + threadIdx.x;
-  if (local >= sd.P) return;
-  if (sd.kind == 0) rhs_point<true, RK, CBC>(sd, tables, local, u, du, Hs, dHs, k, rk, S, flag, ring_s + threadIdx.x);
-  else rhs_point<false, RK, CBC>(sd, tables, local, u, du, Hs, dHs, k, rk, S, flag, ring_s + threadIdx.x);
+  if (local < sd.P) {
+    if (sd.kind == 0) rhs_point<true, RK, CBC, NORMS>(sd, tables, local, u, du, Hs, dHs, k, rk, S, flag, ring_s + threadIdx.x);
+    else rhs_point<false, RK, CBC, NORMS>(sd, tables, local, u, du, Hs, dHs, k, rk, S, flag, ring_s + threadIdx.x);
+  }
+  if (NORMS) {    // the same fold as K_con: warp shuffle, then the warps in fixed order (deterministic)
+    double acc[6];
+#pragma unroll
+    for (int q = 0; q < 6; ++q) acc[q] = nacc[q * TILE_PTS];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+      for (int q = 0; q < 3; ++q) acc[q] += __shfl_xor_sync(0xffffffffu, acc[q], o);
+#pragma unroll
+      for (int q = 3; q < 6; ++q) acc[q] = nanmax(acc[q], __shfl_xor_sync(0xffffffffu, acc[q], o));
+    }
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (lane == 0)
+#pragma unroll
+      for (int q = 0; q < 6; ++q) red[warp][q] = acc[q];
+    __syncthreads();
+    if (threadIdx.x < 6) {
+      const int q = threadIdx.x;
+      double v = red[0][q];
+      for (int w = 1; w < TILE_PTS / 32; ++w) v = (q < 3) ? v + red[w][q] : nanmax(v, red[w][q]);
+      part[(int64_t)blockIdx.x * 6 + q] = v;
+    }
+  }
 }
 
 // ---------------------------------------------------------------------------------------------------------

@@ -34,7 +34,7 @@ EXPORTS = [
     "gh_launch_count", "gh_last_error", "gh_basis_cheb", "gh_basis_gauss_legendre", "gh_basis_shell",
     "gh_set_filter", "gh_apply_filter", "gh_filter_sigma",
     "gh_dp5_workspace_bytes", "gh_dp5_attach", "gh_dp5_step", "gh_set_option",
-    "gh_set_jacobian", "gh_spatial_coord_jac", "gh_spatial_coord_jac_state", "gh_fp64_peak",
+    "gh_rk_step_norms", "gh_set_jacobian", "gh_spatial_coord_jac", "gh_spatial_coord_jac_state", "gh_fp64_peak",
 ]
 
 
@@ -101,6 +101,7 @@ def lib() -> C.CDLL:
     L.gh_gradient.argtypes = [vp, dp, ip]
     L.gh_rk_step.argtypes = [vp, C.c_double]
     L.gh_constraint_norms.argtypes = [vp, dp, dp]
+    L.gh_rk_step_norms.argtypes = [vp, C.c_double, dp, dp]
     L.gh_set_profiling.argtypes = [vp, ip]
     L.gh_profile_read.argtypes = [vp, dp, dp]
     L.gh_profile_reset.argtypes = [vp]
@@ -242,6 +243,13 @@ def gh_constraint_norms(h, n_sub: int, per_sub: bool = False):
     out = np.zeros((3, 2))
     ps = np.zeros((n_sub, 3, 2)) if per_sub else None
     _check(lib().gh_constraint_norms(h, out.ctypes.data, ps.ctypes.data if per_sub else None), h)
+    return (out, ps) if per_sub else out
+
+
+def gh_rk_step_norms(h, dt: float, n_sub: int, per_sub: bool = False):
+    out = np.zeros((3, 2))
+    ps = np.zeros((n_sub, 3, 2)) if per_sub else None
+    _check(lib().gh_rk_step_norms(h, float(dt), out.ctypes.data, ps.ctypes.data if per_sub else None), h)
     return (out, ps) if per_sub else out
 
 
@@ -404,6 +412,9 @@ class Domain:
 
     def rk_step(self, dt: float):
         gh_rk_step(self.h, dt)
+
+    def rk_step_norms(self, dt: float, per_sub: bool = False):
+        return gh_rk_step_norms(self.h, dt, self.n_sub, per_sub)
 
     def constraint_norms(self, per_sub: bool = False):
         return gh_constraint_norms(self.h, self.n_sub, per_sub)

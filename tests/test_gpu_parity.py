@@ -140,6 +140,31 @@ def test_constraint_norms_parity(case, oracle):
         assert np.all(np.abs(per[s, :, 1] - maxs) <= 1e-9 * maxs + floor)
 
 
+def test_rk_step_norms_parity(case, oracle):
+    """gh_rk_step_norms (A8 fused into stage 1 of the step): the norms are those of the state BEFORE the step and match the oracle
+    (and the stand-alone gh_constraint_norms) to 1e-9 relative + the rounding floor; the state after the step is bit-identical to
+    gh_rk_step's, frozen faces included."""
+    name, cfg, descs, coords, us, Hs, dom = case
+    dt = 0.25 * configs.min_spacing(descs)
+    dom.set_fields(dom.pack(us), 0.0)
+    alone, alone_per = dom.constraint_norms(per_sub=True)
+    dom.rk_step(dt)
+    plain = dom.get_fields().copy()
+    dom.set_fields(dom.pack(us), 0.0)
+    got, per = dom.rk_step_norms(dt, per_sub=True)
+    assert np.array_equal(dom.get_fields(), plain)
+    ref = oracle.constraint_norms(descs, us, Hs)
+    floor = 1e-11 * max(np.max(np.abs(u)) for u in us)
+    assert np.all(np.abs(got - ref) <= 1e-9 * np.abs(ref) + floor), (got, ref)
+    assert np.all(np.abs(got - alone) <= 1e-12 * np.abs(alone) + floor) and np.all(np.abs(per - alone_per) <= 1e-12 * np.abs(alone_per) + floor)
+    for s, d in enumerate(descs):
+        sums, maxs, _ = oracle.constraints(d, us[s], Hs[s])
+        rms = np.sqrt(sums / (us[s].shape[1] * np.array([4.0, 30.0, 30.0])))
+        assert np.all(np.abs(per[s, :, 0] - rms) <= 1e-9 * rms + floor) and np.all(np.abs(per[s, :, 1] - maxs) <= 1e-9 * maxs + floor)
+    assert got[1, 0] > 0 and got[2, 0] > 0
+    dom.set_fields(dom.pack(us), 0.0)
+
+
 def test_singular_data_raises_flag(oracle):
     cfg = configs.c1()
     descs, coords, us, Hs = build_case(cfg, oracle)
