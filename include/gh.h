@@ -78,9 +78,15 @@ typedef struct {
   double gamma[3];   /* constraint-damping gamma0, gamma1, gamma2, constant on the subdomain */
 } gh_subdomain_desc;
 
-/* Limits of this build. */
-#define GH_MAX_CHEB_N 64  /* largest N on a Chebyshev axis */
-#define GH_MAX_L 47       /* largest shell L (angular planes are staged in shared memory) */
+/* Limits of this build.  Up to GH_SMALL_CHEB_N points per Chebyshev axis and GH_SMALL_L in the band limit the derivative
+ * kernels keep the whole contraction of a line / a (theta,phi) plane on chip (K_cheb, K_ang); beyond, up to the maxima, the
+ * same linear maps run as tiled FP64 tensor-core GEMMs whose cached matrices stream through shared memory (K_gemm) - the upper
+ * two decades of the size sweep, BASELINE.json configs[4] (N = 320, L = 255: 3.3e7 points per subdomain).  The spectral filter
+ * (gh_set_filter) is built for the small classes only. */
+#define GH_MAX_CHEB_N 512   /* largest N on a Chebyshev axis */
+#define GH_MAX_L 255        /* largest shell band limit L */
+#define GH_SMALL_CHEB_N 64
+#define GH_SMALL_L 47
 
 /* Bytes of device workspace gh_domain_create needs for these subdomains; 0 on invalid input.
  * Pure host query, no CUDA call.  descs: HOST. */

@@ -17,6 +17,7 @@
 #include "kernels_deriv.cuh"
 #include "kernels_point.cuh"
 #include "kernels_jac.cuh"
+#include "kernels_gemm.cuh"
 
 using namespace ghd;
 
@@ -38,6 +39,10 @@ constexpr int ANG_NB_MAX = 8;                    // planes per K_ang CTA offered
 constexpr int ANG_NB_MAX_SMALL_L = 24;           // ... for L < 12, where a plane is a few tiles only (SingleBH k = 0: 5.96 -> 4.91 ms
                                                  // per 2e6 points; for L >= 12 more than 8 planes measured slightly slower on C4)
 constexpr size_t SMEM_MAX = 227 * 1024;
+constexpr int GEMM_MB = 16;                      // m-tiles per M-block of K_gemm (tiles beyond the matrix are skipped at run time)
+enum { G_S1 = 0, G_S2 = 1, G_S3T = 2, G_S3P = 3, G_CHEB = 4, G_NLIST = 5 };   // K_gemm launch lists, in launch order
+inline bool big_N(int N) { return N > GH_SMALL_CHEB_N; }
+inline bool big_L(int L) { return L > GH_SMALL_L; }
 
 thread_local std::string g_create_error;
 
@@ -61,10 +66,13 @@ struct Plan {
   int n_cheb_items = 0, n_cheb_class[CHEB_NCLASS] = {}, n_ang_items = 0;
   int n_ang_class[2] = {0, 0};           // K_ang items per shared-memory class (0: two CTAs per SM, 1: one)
   size_t cheb_smem = 0, ang_smem[2] = {0, 0};
+  int n_gemm[G_NLIST] = {0, 0, 0, 0, 0};  // K_gemm items per launch list (large subdomains)
+  size_t bigtab_doubles = 0;             // their blocked fragment matrices, behind the filter tables
+  bool has_big = false;
   std::vector<int> ang_pb;               // planes per CTA for each subdomain (0 for blocks)
   std::vector<int> ang_class;            // shared-memory class of each shell
   // workspace offsets (bytes)
-  size_t o_ua, o_ub, o_k, o_du, o_H, o_dH, o_jac, o_tables, o_subs, o_tiles, o_cheb, o_fcheb, o_ang, o_part, o_persub, o_flag, total;
+  size_t o_ua, o_ub, o_k, o_du, o_H, o_dH, o_jac, o_tables, o_subs, o_tiles, o_cheb, o_fcheb, o_ang, o_gemm, o_part, o_persub, o_flag, total;
 };
 
 inline void sub_dims(const gh_subdomain_desc& d, int& n0, int& n1, int& n2) {
@@ -178,8 +186,14 @@ bool make_plan(const gh_subdomain_desc* descs, int32_t n_sub, Plan& pl, std::str
     const int naxes = d.kind == GH_SHELL ? 1 : 3;
     for (int a = 0; a < naxes; ++a) {
       const int N = d.n[a];
-      tab += cheb_frag_doubles(N);
       const int64_t cols = Ps / N;
+      if (big_N(N)) {       // tiled GEMM path
+        pl.bigtab_doubles += gemm_amat_doubles(N, N, GEMM_MB);
+        pl.n_gemm[G_CHEB] += (int)((cols + GEMM_CT - 1) / GEMM_CT);
+        pl.has_big = true;
+        continue;
+      }
+      tab += cheb_frag_doubles(N);
       const int items = (int)((cols + cheb_ct(N) - 1) / cheb_ct(N));
       pl.n_cheb_items += items; pl.n_cheb_class[cheb_class(N)] += items;
       pl.cheb_smem = std::max(pl.cheb_smem, cheb_frag_doubles(N) * sizeof(double));
@@ -188,6 +202,20 @@ bool make_plan(const gh_subdomain_desc* descs, int32_t n_sub, Plan& pl, std::str
     if (d.kind == GH_SHELL) {
       const int L = d.n[1];
       tab += (size_t)round_up(n0, 2) + 2 * (size_t)round_up(n1, 2) + 2 * (size_t)round_up(n2, 2);
+      if (big_L(L)) {       // tiled GEMM path: analysis, per-m composites, two syntheses through global coefficient buffers
+        const int nt = L + 1, np = 2 * L + 2, nq = 2 * L + 1;
+        if (!seenL.count(L)) {
+          seenL[L] = 1;
+          pl.bigtab_doubles += gemm_amat_doubles(nq, np, GEMM_MB) + 2 * gemm_amat_doubles(np, nq, GEMM_MB) +
+                               (size_t)(L + 1) * 2 * gemm_amat_doubles(nt, nt, GEMM_MB);
+        }
+        const int64_t R = (int64_t)n0 * nt;
+        const int rt = (int)((R + GEMM_CT - 1) / GEMM_CT);
+        pl.n_gemm[G_S1] += rt; pl.n_gemm[G_S3T] += rt; pl.n_gemm[G_S3P] += rt;
+        for (int m = 0; m <= L; ++m) pl.n_gemm[G_S2] += 2 * (((m ? 2 : 1) * n0 + GEMM_CT - 1) / GEMM_CT);
+        pl.has_big = true;
+        continue;
+      }
       if (!seenL.count(L)) { seenL[L] = 1; tab += shell_matrix_doubles(L); pl.ftable_doubles += shell_g_doubles(L); }
       // planes per CTA and CTA class (0: 256 threads, two CTAs per SM; 1: 512 threads, one CTA per SM): of all that fit in
       // shared memory, the pair with the smallest modelled time for the whole shell (sum over its CTAs / CTAs per SM).
@@ -205,7 +233,7 @@ bool make_plan(const gh_subdomain_desc* descs, int32_t n_sub, Plan& pl, std::str
             if (t < best) { best = t; pb = nb; cls = c; }
           }
       }
-      if (!pb) { err = "shell L too large for shared memory"; return false; }
+      if (!pb) { err = "internal: no K_ang configuration for a small-class shell"; return false; }
       const int chunks = (n0 + pb - 1) / pb;
       pl.ang_pb[s] = pb; pl.ang_class[s] = cls;
       pl.n_ang_items += chunks; pl.n_ang_class[cls] += chunks;
@@ -222,12 +250,13 @@ bool make_plan(const gh_subdomain_desc* descs, int32_t n_sub, Plan& pl, std::str
   pl.o_ua = c.take(NCOMP * comp); pl.o_ub = c.take(NCOMP * comp); pl.o_k = c.take(NCOMP * comp);
   pl.o_du = c.take(3 * NCOMP * comp); pl.o_H = c.take(4 * comp); pl.o_dH = c.take(12 * comp);
   pl.o_jac = c.take(9 * comp);
-  pl.o_tables = c.take((pl.table_doubles + pl.ftable_doubles) * sizeof(double));
+  pl.o_tables = c.take((pl.table_doubles + pl.ftable_doubles + pl.bigtab_doubles) * sizeof(double));
   pl.o_subs = c.take((size_t)n_sub * sizeof(SubDev));
   pl.o_tiles = c.take((size_t)(n_sub + 1) * sizeof(int32_t));
-  pl.o_cheb = c.take((size_t)pl.n_cheb_items * sizeof(ChebItem));
+  pl.o_cheb = c.take((size_t)std::max(1, pl.n_cheb_items) * sizeof(ChebItem));
   pl.o_fcheb = c.take((size_t)std::max(1, pl.n_fcheb_items) * sizeof(ChebItem));
   pl.o_ang = c.take((size_t)std::max(1, pl.n_ang_items) * sizeof(AngItem));
+  { int ng = 0; for (int l = 0; l < G_NLIST; ++l) ng += pl.n_gemm[l]; pl.o_gemm = c.take((size_t)std::max(1, ng) * sizeof(GemmItem)); }
   pl.o_part = c.take((size_t)pl.n_tiles * 6 * sizeof(double));
   pl.o_persub = c.take((size_t)n_sub * 6 * sizeof(double));
   pl.o_flag = c.take(256);
@@ -248,6 +277,7 @@ struct gh_domain {
   ChebItem* cheb = nullptr;
   ChebItem* fcheb = nullptr;             // filter items of the blocks, ordered [axis][class]
   AngItem* ang = nullptr;
+  GemmItem* gemm = nullptr;              // K_gemm items of the large subdomains, the G_NLIST lists back to back
   struct FBlock { int N; double unused; size_t off; };     // one filter matrix slot per (block, axis): offset (doubles) from `tables`
   std::vector<FBlock> f_blocks;
   std::map<int, size_t> f_L;             // shell band limit L -> offset (doubles) of its filtered projectors from `tables`
@@ -385,6 +415,7 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
   d->du = (double*)(w + pl.o_du); d->H = (double*)(w + pl.o_H); d->dH = (double*)(w + pl.o_dH); d->jac = (double*)(w + pl.o_jac);
   d->tables = (double*)(w + pl.o_tables); d->subs = (SubDev*)(w + pl.o_subs); d->tiles = (int32_t*)(w + pl.o_tiles);
   d->cheb = (ChebItem*)(w + pl.o_cheb); d->ang = (AngItem*)(w + pl.o_ang); d->fcheb = (ChebItem*)(w + pl.o_fcheb);
+  d->gemm = (GemmItem*)(w + pl.o_gemm);
   d->part = (double*)(w + pl.o_part); d->persub = (double*)(w + pl.o_persub); d->flag = (int*)(w + pl.o_flag);
 
   // ---- tables and work lists on the host ----
@@ -398,6 +429,37 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
   std::map<int, std::vector<ghb::ld>> Dcache;        // N -> unscaled D
   struct ShellOff { int Fa, Fs, T; };
   std::map<int, ShellOff> Lcache;
+  // large subdomains: blocked fragment matrices (behind the filter tables) and K_gemm items per launch list
+  std::vector<double> bigtab(pl.bigtab_doubles, 0.0);
+  std::vector<GemmItem> glist[G_NLIST];
+  size_t btp = 0;
+  const size_t big0 = pl.table_doubles + pl.ftable_doubles;      // offset of bigtab[0] from d->tables
+  // elem(row, col) of an (M x K) matrix -> A-fragment order, blocked [m_block][k_chunk][GEMM_MB m-tiles][GEMM_KB k-steps][32];
+  // returns the offset (doubles) of the matrix from d->tables
+  auto put_amat = [&](int M, int K, auto elem) {
+    const int MT = (M + 7) / 8, KS = (K + 3) / 4, nMB = (MT + GEMM_MB - 1) / GEMM_MB, nKC = (KS + GEMM_KB - 1) / GEMM_KB;
+    const size_t at = btp;
+    for (int mb = 0; mb < nMB; ++mb) for (int kc = 0; kc < nKC; ++kc) for (int mt = 0; mt < GEMM_MB; ++mt) for (int ks = 0; ks < GEMM_KB; ++ks)
+      for (int lane = 0; lane < 32; ++lane) {
+        const int row = (mb * GEMM_MB + mt) * 8 + lane / 4, col = (kc * GEMM_KB + ks) * 4 + lane % 4;
+        if (row < M && col < K)
+          bigtab[at + ((((size_t)mb * nKC + kc) * GEMM_MB + mt) * GEMM_KB + ks) * 32 + lane] = (double)elem(row, col);
+      }
+    btp += gemm_amat_doubles(M, K, GEMM_MB);
+    return (int64_t)(big0 + at);
+  };
+  // one K_gemm item per tile of GEMM_CT columns
+  auto put_items = [&](int list, GemmItem proto, int64_t cols) {
+    // columns (c, c + 1), c even, may leave as one double2 when they are neighbours in memory at an even address
+    proto.pair = (proto.out_cs == 1 && proto.out_sa % 2 == 0 && proto.out_base % 2 == 0 && proto.out_outer % 2 == 0 &&
+                  (proto.out_inner % 2 == 0 || proto.out_inner >= cols)) ? 1 : 0;
+    for (int64_t c0 = 0; c0 < cols; c0 += GEMM_CT) {
+      GemmItem it = proto; it.col0 = (int)c0; it.ncols = (int)std::min<int64_t>(GEMM_CT, cols - c0);
+      glist[list].push_back(it);
+    }
+  };
+  struct BigShellOff { int64_t FaQ, FsQ, FpQ; std::vector<int64_t> Th, Pr; };
+  std::map<int, BigShellOff> Lbig;
   for (int s = 0; s < n_sub; ++s) {
     const gh_subdomain_desc& de = descs[s];
     SubDev& sd = d->h_subs[s];
@@ -421,6 +483,18 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
       if (!Dcache.count(N)) ghb::cheb_diff_matrix(N, Dcache[N]);
       const std::vector<ghb::ld>& D = Dcache[N];
       const ghb::ld scale = 2 / ((ghb::ld)de.hi[a] - (ghb::ld)de.lo[a]);   // affine map factor of Eq. 22
+      if (big_N(N)) {     // K_gemm: Out[a', col] = sum_i (scale D)[a'][i] u[i, col], the same strided views as K_cheb's
+        GemmItem it; memset(&it, 0, sizeof it);
+        it.amat = put_amat(N, N, [&](int r, int c) { return scale * D[(size_t)r * N + c]; });
+        it.M = N; it.K = N; it.in_slot = -1; it.out_slot = a;
+        it.in_base = it.out_base = sd.off; it.in_sk = it.out_sa = strides[a];
+        if (a == 0) { it.in_inner = (int)(nn[1] * nn[2]); it.in_outer = 0; it.in_cs = 1; }
+        else if (a == 1) { it.in_inner = (int)nn[2]; it.in_outer = nn[1] * nn[2]; it.in_cs = 1; }
+        else { it.in_inner = 1; it.in_outer = nn[2]; it.in_cs = 0; }
+        it.out_inner = it.in_inner; it.out_outer = it.in_outer; it.out_cs = it.in_cs;
+        put_items(G_CHEB, it, sd.P / N);
+        continue;
+      }
       const int dm = (int)tp;
       // scaled D in DMMA A-fragment order: lane (g = lane/4, t = lane%4) of fragment (m_tile, k_step) holds
       // D[8 m_tile + g][4 k_step + t]; rows / columns beyond N are zero
@@ -448,7 +522,73 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
       }
       if (de.kind == GH_BLOCK) { d->f_blocks.push_back({N, 0.0, ftp}); ftp += cheb_frag_doubles(N); }
     }
+    if (de.kind == GH_SHELL && big_L(de.n[1])) {
+      // K_gemm path of a large shell, per component c (R = n_r n_theta rows of n_phi points), through coefficient buffers in
+      // the derivative scratch (slot 0: later d_r, slot 1: later d_theta, slot 2: later d_phi):
+      //   S1   W[q][row]  = sum_k FaQ[q][k] u[row][k]                 u -> slot 1      q = 0: m = 0;  2m-1: cos m;  2m: sin m
+      //   S2   V1_m = Th_m W_m  -> slot 2,   V2_m = Pr_m W_m -> slot 0      per m, columns = (cos | sin, plane), contraction over theta
+      //   S3   d_theta u[row][k] = sum_q FsQ[k][q] V1[q][row] -> slot 1;   d_phi u[row][k] = sum_q FpQ[k][q] V2[q][row] -> slot 2
+      // (FpQ = d/dphi of the synthesis: -m sin on the cos coefficient, +m cos on the sin coefficient.)  The radial derivative
+      // (slot 0) is launched after S3.
+      d->has_shell = true;
+      const int L = de.n[1], nt = L + 1, np = 2 * L + 2, nq = 2 * L + 1;
+      if (!Lbig.count(L)) {
+        ghb::ShellBasis B; ghb::shell_basis(L, B);
+        BigShellOff o;
+        auto qrow = [&](int q) { return q == 0 ? 0 : (q & 1) ? (q + 1) / 2 : L + q / 2; };     // q -> row of Fa / column of Fs, Fp
+        o.FaQ = put_amat(nq, np, [&](int q, int k) { return B.Fa[(size_t)qrow(q) * np + k]; });
+        o.FsQ = put_amat(np, nq, [&](int k, int q) { return B.Fs[(size_t)k * nq + qrow(q)]; });
+        o.FpQ = put_amat(np, nq, [&](int k, int q) { return B.Fp[(size_t)k * nq + qrow(q)]; });
+        for (int m = 0; m <= L; ++m) {
+          o.Th.push_back(put_amat(nt, nt, [&](int r, int c) { return B.Th[((size_t)m * nt + r) * nt + c]; }));
+          o.Pr.push_back(put_amat(nt, nt, [&](int r, int c) { return B.Pr[((size_t)m * nt + r) * nt + c]; }));
+        }
+        Lbig[L] = o;
+      }
+      const BigShellOff& o = Lbig[L];
+      const int64_t R = (int64_t)n0 * nt, BIG = (int64_t)1 << 30;
+      GemmItem it; memset(&it, 0, sizeof it);
+      // S1
+      it.amat = o.FaQ; it.M = nq; it.K = np; it.in_slot = -1; it.out_slot = 1;
+      it.in_base = sd.off; it.in_sk = 1; it.in_inner = (int)BIG; it.in_outer = 0; it.in_cs = np;
+      it.out_base = sd.off; it.out_sa = R; it.out_inner = (int)BIG; it.out_outer = 0; it.out_cs = 1;
+      put_items(G_S1, it, R);
+      // S2
+      for (int m = 0; m <= L; ++m) {
+        const int64_t q0 = m == 0 ? 0 : 2 * m - 1, cols = (m ? 2 : 1) * (int64_t)n0;
+        memset(&it, 0, sizeof it);
+        it.M = nt; it.K = nt; it.in_slot = 1;
+        it.in_base = it.out_base = sd.off + q0 * R; it.in_sk = it.out_sa = 1;
+        it.in_inner = it.out_inner = (int)BIG; it.in_cs = it.out_cs = nt;
+        it.amat = o.Th[m]; it.out_slot = 2; put_items(G_S2, it, cols);
+        it.amat = o.Pr[m]; it.out_slot = 0; put_items(G_S2, it, cols);
+      }
+      // S3
+      memset(&it, 0, sizeof it);
+      it.M = np; it.K = nq;
+      it.in_base = sd.off; it.in_sk = R; it.in_inner = (int)BIG; it.in_cs = 1;
+      it.out_base = sd.off; it.out_sa = 1; it.out_inner = (int)BIG; it.out_cs = np;
+      it.amat = o.FsQ; it.in_slot = 2; it.out_slot = 1; put_items(G_S3T, it, R);
+      it.amat = o.FpQ; it.in_slot = 0; it.out_slot = 2; put_items(G_S3P, it, R);
+    }
     if (de.kind == GH_SHELL) {
+      // coordinate tables of this shell (for the Jacobian of Eq. 8)
+      const int L = de.n[1];
+      std::vector<ghb::ld> xr, ct, wv;
+      ghb::cheb_nodes(n0, xr); ghb::gauss_legendre(L, ct, wv);
+      sd.t_rinv = (int)tp;
+      for (int i = 0; i < n0; ++i) {
+        ghb::ld r = (ghb::ld)de.lo[0] + ((ghb::ld)de.hi[0] - (ghb::ld)de.lo[0]) * (xr[i] + 1) / 2;
+        tab[tp + i] = (double)(1 / r);
+      }
+      tp += round_up(n0, 2);
+      sd.t_ct = (int)tp; for (int j = 0; j < n1; ++j) tab[tp + j] = (double)ct[j]; tp += round_up(n1, 2);
+      sd.t_st = (int)tp; for (int j = 0; j < n1; ++j) tab[tp + j] = (double)sqrtl((1 - ct[j]) * (1 + ct[j])); tp += round_up(n1, 2);
+      const ghb::ld PI_L = 3.14159265358979323846264338327950288L;
+      sd.t_cp = (int)tp; for (int k = 0; k < n2; ++k) tab[tp + k] = (double)cosl(2 * PI_L * k / n2); tp += round_up(n2, 2);
+      sd.t_sp = (int)tp; for (int k = 0; k < n2; ++k) tab[tp + k] = (double)sinl(2 * PI_L * k / n2); tp += round_up(n2, 2);
+    }
+    if (de.kind == GH_SHELL && !big_L(de.n[1])) {
       d->has_shell = true;
       const int L = de.n[1];
       if (!Lcache.count(L)) {
@@ -514,20 +654,6 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
         d->f_L[L] = ftp; ftp += shell_g_doubles(L);
       }
       const ShellOff& o = Lcache[L];
-      // coordinate tables of this shell (for the Jacobian of Eq. 8)
-      std::vector<ghb::ld> xr, ct, wv;
-      ghb::cheb_nodes(n0, xr); ghb::gauss_legendre(L, ct, wv);
-      sd.t_rinv = (int)tp;
-      for (int i = 0; i < n0; ++i) {
-        ghb::ld r = (ghb::ld)de.lo[0] + ((ghb::ld)de.hi[0] - (ghb::ld)de.lo[0]) * (xr[i] + 1) / 2;
-        tab[tp + i] = (double)(1 / r);
-      }
-      tp += round_up(n0, 2);
-      sd.t_ct = (int)tp; for (int j = 0; j < n1; ++j) tab[tp + j] = (double)ct[j]; tp += round_up(n1, 2);
-      sd.t_st = (int)tp; for (int j = 0; j < n1; ++j) tab[tp + j] = (double)sqrtl((1 - ct[j]) * (1 + ct[j])); tp += round_up(n1, 2);
-      const ghb::ld PI_L = 3.14159265358979323846264338327950288L;
-      sd.t_cp = (int)tp; for (int k = 0; k < n2; ++k) tab[tp + k] = (double)cosl(2 * PI_L * k / n2); tp += round_up(n2, 2);
-      sd.t_sp = (int)tp; for (int k = 0; k < n2; ++k) tab[tp + k] = (double)sinl(2 * PI_L * k / n2); tp += round_up(n2, 2);
       const int pb = pl.ang_pb[s];
       for (int p0 = 0; p0 < n0; p0 += pb) {
         AngItem it; memset(&it, 0, sizeof it);
@@ -542,15 +668,17 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
         }
         (pl.ang_class[s] ? ang1 : ang).push_back(it);
       }
-    } else {
-      d->has_block = true;
     }
+    if (de.kind == GH_BLOCK) d->has_block = true;
   }
   ang.insert(ang.end(), ang1.begin(), ang1.end());
   for (int c = 0; c < CHEB_NCLASS; ++c) cheb.insert(cheb.end(), chebc[c].begin(), chebc[c].end());
   std::vector<ChebItem> fcheb;
   for (int a = 0; a < 3; ++a) for (int c = 0; c < CHEB_NCLASS; ++c) fcheb.insert(fcheb.end(), fch[a][c].begin(), fch[a][c].end());
-  if (tp != pl.table_doubles || (int)cheb.size() != pl.n_cheb_items || (int)ang.size() != pl.n_ang_items ||
+  std::vector<GemmItem> gemm;
+  bool gemm_ok = btp == pl.bigtab_doubles;
+  for (int l = 0; l < G_NLIST; ++l) { gemm_ok = gemm_ok && (int)glist[l].size() == pl.n_gemm[l]; gemm.insert(gemm.end(), glist[l].begin(), glist[l].end()); }
+  if (tp != pl.table_doubles || (int)cheb.size() != pl.n_cheb_items || (int)ang.size() != pl.n_ang_items || !gemm_ok ||
       (int)fcheb.size() != pl.n_fcheb_items || ftp != pl.table_doubles + pl.ftable_doubles) {
     delete d; return fail(nullptr, GH_ERR_STATE, "internal: plan and build disagree");
   }
@@ -563,7 +691,10 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
   GH_CREATE_CUDA(cudaMemcpyAsync(d->tables, tab.data(), tab.size() * sizeof(double), cudaMemcpyHostToDevice, st));
   GH_CREATE_CUDA(cudaMemcpyAsync(d->subs, d->h_subs.data(), (size_t)n_sub * sizeof(SubDev), cudaMemcpyHostToDevice, st));
   GH_CREATE_CUDA(cudaMemcpyAsync(d->tiles, pl.tile_first.data(), (size_t)(n_sub + 1) * sizeof(int32_t), cudaMemcpyHostToDevice, st));
-  GH_CREATE_CUDA(cudaMemcpyAsync(d->cheb, cheb.data(), cheb.size() * sizeof(ChebItem), cudaMemcpyHostToDevice, st));
+  if (!cheb.empty()) GH_CREATE_CUDA(cudaMemcpyAsync(d->cheb, cheb.data(), cheb.size() * sizeof(ChebItem), cudaMemcpyHostToDevice, st));
+  if (!gemm.empty()) GH_CREATE_CUDA(cudaMemcpyAsync(d->gemm, gemm.data(), gemm.size() * sizeof(GemmItem), cudaMemcpyHostToDevice, st));
+  if (!bigtab.empty()) GH_CREATE_CUDA(cudaMemcpyAsync(d->tables + big0, bigtab.data(), bigtab.size() * sizeof(double), cudaMemcpyHostToDevice, st));
+  GH_CREATE_CUDA(cudaFuncSetAttribute(k_gemm<GEMM_MB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gemm_smem_bytes(GEMM_MB)));
   if (!ang.empty()) GH_CREATE_CUDA(cudaMemcpyAsync(d->ang, ang.data(), ang.size() * sizeof(AngItem), cudaMemcpyHostToDevice, st));
   if (!fcheb.empty()) GH_CREATE_CUDA(cudaMemcpyAsync(d->fcheb, fcheb.data(), fcheb.size() * sizeof(ChebItem), cudaMemcpyHostToDevice, st));
   GH_CREATE_CUDA(cudaStreamSynchronize(st));   // host staging vectors die at return
@@ -684,6 +815,18 @@ gh_status launch_derivs(gh_domain* d, const double* in, double* out, int ncomp, 
   const int nrun = ncomp - skip_n;
   // each K_cheb CTA walks over nrun / cheb_gy components (amortises its launch and matrix load)
   // ... but small domains need the CTAs more than the amortisation: keep at least ~4 CTAs per SM in the grid
+  // large subdomains: the K_gemm lists in order (S1, S2, S3 theta, S3 phi of the large shells, then the large Chebyshev axes -
+  // the radial one writes slot 0, which S2 / S3 used as a coefficient buffer)
+  if (pl.has_big) {
+    for (int l = 0, first = 0; l < G_NLIST; first += pl.n_gemm[l], ++l) {
+      if (!pl.n_gemm[l]) continue;
+      int gw = 1;     // components one CTA walks over: as many as still leave two CTAs per SM in the grid
+      for (int w = 10; w >= 1; --w)
+        if (nrun % w == 0 && (w == 1 || (int64_t)pl.n_gemm[l] * (nrun / w) >= 2 * d->n_sm)) { gw = w; break; }
+      ProfScope ps(d, l == G_CHEB ? GH_K_CHEB : GH_K_SHELL_ANG);
+      k_gemm<GEMM_MB><<<dim3(pl.n_gemm[l], nrun / gw), GEMM_TPB, gemm_smem_bytes(GEMM_MB), d->stream>>>(d->gemm + first, d->tables, in, out, pl.S, nrun, cm);
+    }
+  }
   int walk = 1;
   for (int w = CHEB_COMP_WALK; w >= 1; --w)
     if (nrun % w == 0 && (w == 1 || (int64_t)pl.n_cheb_items * (nrun / w) >= 4 * d->n_sm)) { walk = w; break; }
@@ -951,6 +1094,7 @@ extern "C" gh_status gh_set_filter(gh_domain* d, const gh_filter_desc* fb, const
   std::vector<ghb::ld> sg, M;
   const bool on_b = fb && fb->kind != GH_FILTER_NONE && !d->f_blocks.empty();
   const bool on_s = fs && fs->kind != GH_FILTER_NONE && !d->f_L.empty();
+  if ((on_b || on_s) && pl.has_big) return fail(d, GH_ERR_ARG, "the spectral filter is built for subdomains with N <= 64 and L <= 47 only");
   if (on_b) {
     std::map<int, std::vector<ghb::ld>> cache;      // N -> filter matrix
     for (const auto& b : d->f_blocks) {

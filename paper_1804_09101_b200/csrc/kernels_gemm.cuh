@@ -1,0 +1,192 @@
+// kernels_gemm.cuh — K_gemm: the derivative contractions of the LARGE subdomains (Chebyshev axes with N > 64, shells with
+// L > 47; the upper two decades of the size sweep, BASELINE.json configs[4]).  Same linear maps as K_cheb / K_ang (Eq. 22,
+// PAPER.md:379-384; Eq. 24), restructured as one generic FP64 tensor-core GEMM
+//     Out[a, col] = sum_k A[a, k] X[k, col],      a < M, k < K, col < ncols
+// with A a cached constant matrix (D; the real-Fourier analysis / synthesis matrices; per m the Legendre composites Theta_m,
+// Pr_m) and X / Out strided views of the field store (contraction index stride sk, output row stride sa, columns
+// (c / inner) * outer + (c % inner) * cs).  At these sizes the matrices no longer fit shared memory (N = 320: 819 KB;
+// L = 255: 268 MB for all m) and an accumulator for every output row no longer fits the register file, so:
+//   - A is stored in DMMA A-fragment order, blocked [m_block][k_chunk][MB m-tiles][KB k-steps][32 lanes], zero padded: one
+//     (m_block, k_chunk) tile is ONE contiguous 16 / 32 KB piece, fetched by a single TMA bulk copy (cp.async.bulk, completion
+//     on an mbarrier) into a 3-deep shared-memory ring by one elected thread and shared by the CTA's 8 warps;
+//   - a warp owns 16 columns, walks the M-blocks with MB x 2 accumulator tiles, and streams its X fragments straight from
+//     global memory (L2) into registers one k-chunk ahead of the DMMAs (the same sector-exact access patterns as K_cheb).
+// A CTA walks over several components so that the pipeline is filled once.  FP64-bound (N = 320: 40 flop per byte).
+#pragma once
+#include "device_types.h"
+#include "kernels_deriv.cuh"
+
+namespace ghd {
+
+struct GemmItem {
+  int64_t in_base, out_base;     // offsets (doubles) inside a component of the input / output array
+  int64_t in_sk, out_sa;         // stride of the contraction index in X, of the output row index in Out
+  int64_t in_outer, out_outer;   // column c lives at (c / inner) * outer + (c % inner) * cs
+  int32_t in_inner, out_inner;
+  int32_t in_cs, out_cs;
+  int32_t M, K;
+  int32_t col0, ncols;
+  int64_t amat;                  // offset (doubles, even) of the blocked fragment matrix in the table memory
+  int32_t in_slot, out_slot;     // -1: the kernel's `in` array; 0..2: slot of the derivative scratch [3][total][S]
+  int32_t pair;                  // 1: Out columns are contiguous and 16-byte aligned in pairs (double2 stores)
+  int32_t pad_;
+};
+
+constexpr int GEMM_TPB = 256, GEMM_KB = 8, GEMM_NST = 3, GEMM_NTW = 2;
+constexpr int GEMM_CT = (GEMM_TPB / 32) * 8 * GEMM_NTW;     // 128 columns per CTA
+__host__ __device__ constexpr size_t gemm_stage_doubles(int MB) { return (size_t)MB * GEMM_KB * 32; }
+__host__ __device__ constexpr size_t gemm_smem_bytes(int MB) { return GEMM_NST * gemm_stage_doubles(MB) * sizeof(double); }
+// doubles of the blocked fragment matrix for an (M x K) matrix
+inline size_t gemm_amat_doubles(int M, int K, int MB) {
+  const int MT = (M + 7) / 8, KS = (K + 3) / 4;
+  return (size_t)((MT + MB - 1) / MB) * ((KS + GEMM_KB - 1) / GEMM_KB) * gemm_stage_doubles(MB);
+}
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}\n" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(parity) : "memory");
+}
+// TMA bulk copy global -> shared, completion counted in bytes on the mbarrier (SASS: UBLKCP)
+__device__ __forceinline__ void bulk_g2s(double* smem_dst, const double* gsrc, unsigned bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::
+               "r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(gsrc), "r"(bytes), "r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
+}
+
+template <int MB>
+__global__ void __launch_bounds__(GEMM_TPB, 1)
+k_gemm(const GemmItem* __restrict__ items, const double* __restrict__ tables, const double* in, double* dub, int64_t S,
+       int ncomp, CompMap cm) {
+  extern __shared__ __align__(128) double sm[];     // GEMM_NST stages of MB x KB fragments
+  __shared__ __align__(8) uint64_t full[GEMM_NST];
+  constexpr int KB = GEMM_KB, NST = GEMM_NST, NTW = GEMM_NTW;
+  constexpr int STAGE = MB * KB * 32;
+  const GemmItem it = items[blockIdx.x];
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, tl = lane & 3;
+  const int MT = (it.M + 7) >> 3, KS = (it.K + 3) >> 2;
+  const int nMB = (MT + MB - 1) / MB, nKC = (KS + KB - 1) / KB;
+  // components this CTA walks over: blockIdx.y, + gridDim.y, ...
+  const int ncw = (ncomp - (int)blockIdx.y + (int)gridDim.y - 1) / (int)gridDim.y;
+  const int per = nMB * nKC, total = ncw * per;
+  const double* __restrict__ amat = tables + it.amat;
+
+  if (tid == 0) {
+#pragma unroll
+    for (int s = 0; s < NST; ++s) mbar_init(&full[s], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  auto issue = [&](int t) {       // stage t: the (m_block, k_chunk) tile of its position inside the component
+    const int r = t % per;
+    mbar_expect_tx(&full[t % NST], STAGE * 8);
+    bulk_g2s(sm + (size_t)(t % NST) * STAGE, amat + (size_t)r * STAGE, STAGE * 8, &full[t % NST]);
+  };
+  if (tid == 0)
+    for (int t = 0; t < NST - 1 && t < total; ++t) issue(t);
+
+  // columns of this lane: B fragments (loads, column 8 n + g) and C fragments (stores, columns 8 n + 2 tl, + 1)
+  const int wc0 = warp * (8 * NTW);
+  int64_t cin[NTW], cout0[NTW], cout1[NTW];
+  bool cok[NTW], ok0[NTW], ok1[NTW];
+#pragma unroll
+  for (int n = 0; n < NTW; ++n) {
+    const int c = wc0 + n * 8 + g;
+    cok[n] = c < it.ncols;
+    const int col = it.col0 + (cok[n] ? c : 0);
+    cin[n] = (int64_t)(col / it.in_inner) * it.in_outer + (int64_t)(col % it.in_inner) * it.in_cs;
+    const int c0 = wc0 + n * 8 + 2 * tl;
+    ok0[n] = c0 < it.ncols; ok1[n] = c0 + 1 < it.ncols;
+    const int q0 = it.col0 + (ok0[n] ? c0 : 0), q1 = it.col0 + (ok1[n] ? c0 + 1 : 0);
+    cout0[n] = (int64_t)(q0 / it.out_inner) * it.out_outer + (int64_t)(q0 % it.out_inner) * it.out_cs;
+    cout1[n] = (int64_t)(q1 / it.out_inner) * it.out_outer + (int64_t)(q1 % it.out_inner) * it.out_cs;
+  }
+  const bool active = wc0 < it.ncols;      // idle warps still take part in the block barriers
+  const int64_t slot_stride = (int64_t)cm.total * S;
+  auto in_ptr = [&](int cw) {
+    const int comp = cm.map((int)blockIdx.y + cw * (int)gridDim.y);
+    return (it.in_slot < 0 ? in : dub + it.in_slot * slot_stride) + (int64_t)comp * S + it.in_base;
+  };
+  auto out_ptr = [&](int cw) {
+    const int comp = cm.map((int)blockIdx.y + cw * (int)gridDim.y);
+    return dub + it.out_slot * slot_stride + (int64_t)comp * S + it.out_base;
+  };
+  auto load_b = [&](int t, double (&b)[KB][NTW]) {
+    const int cw = t / per, kc = (t % per) % nKC;
+    const double* src = in_ptr(cw);
+#pragma unroll
+    for (int ks = 0; ks < KB; ++ks) {
+      const int k = (kc * KB + ks) * 4 + tl;
+#pragma unroll
+      for (int n = 0; n < NTW; ++n) b[ks][n] = (active && cok[n] && k < it.K) ? src[cin[n] + (int64_t)k * it.in_sk] : 0.0;
+    }
+  };
+
+  double acc[MB][NTW][2];
+  double bn[KB][NTW];
+  if (total > 0) load_b(0, bn);
+#pragma unroll 1
+  for (int t = 0; t < total; ++t) {
+    const int r = t % per, mb = r / nKC, kc = r - mb * nKC;
+    if (tid == 0 && t + NST - 1 < total) issue(t + NST - 1);     // into the slot every warp left before the last barrier
+    if (kc == 0) {
+#pragma unroll
+      for (int mt = 0; mt < MB; ++mt)
+#pragma unroll
+        for (int n = 0; n < NTW; ++n) acc[mt][n][0] = acc[mt][n][1] = 0.0;
+    }
+    double b[KB][NTW];
+#pragma unroll
+    for (int ks = 0; ks < KB; ++ks)
+#pragma unroll
+      for (int n = 0; n < NTW; ++n) b[ks][n] = bn[ks][n];
+    if (t + 1 < total) load_b(t + 1, bn);
+    mbar_wait(&full[t % NST], (unsigned)((t / NST) & 1));
+    if (active) {
+      const double* __restrict__ a_s = sm + (size_t)(t % NST) * STAGE + lane;
+      const int mtn = min(MB, MT - mb * MB);      // m-tiles of this block that exist (the rest of the tile is zero padding)
+#pragma unroll
+      for (int ks = 0; ks < KB; ++ks)
+#pragma unroll
+        for (int mt = 0; mt < MB; ++mt)
+          if (mt < mtn) {
+            const double a = a_s[(mt * KB + ks) * 32];
+#pragma unroll
+            for (int n = 0; n < NTW; ++n) dmma884(acc[mt][n][0], acc[mt][n][1], a, b[ks][n]);
+          }
+      if (kc == nKC - 1) {
+        double* dst = out_ptr(t / per);
+#pragma unroll
+        for (int mt = 0; mt < MB; ++mt) {
+          const int a = (mb * MB + mt) * 8 + g;
+          if (a < it.M) {
+            const int64_t ao = (int64_t)a * it.out_sa;
+#pragma unroll
+            for (int n = 0; n < NTW; ++n) {
+              if (it.pair && ok1[n]) {
+                *reinterpret_cast<double2*>(dst + cout0[n] + ao) = make_double2(acc[mt][n][0], acc[mt][n][1]);
+              } else {
+                if (ok0[n]) dst[cout0[n] + ao] = acc[mt][n][0];
+                if (ok1[n]) dst[cout1[n] + ao] = acc[mt][n][1];
+              }
+            }
+          }
+        }
+      }
+    }
+    __syncthreads();
+  }
+}
+
+}  // namespace ghd

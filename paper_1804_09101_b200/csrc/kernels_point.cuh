@@ -393,10 +393,13 @@ __device__ __forceinline__ void rhs_store(double* out, const RkArgs& rk, int64_t
 // scheduler alone.
 constexpr int RHS_RING = 3, RHS_RING_ROWS = 22, RHS_PHI_ROWS = 30;   // 15 derivatives + 2 gauge-source gradients + 5 u0 values (RK = 2)
 constexpr size_t RHS_SMEM_BYTES = (size_t)(RHS_PHI_ROWS + RHS_RING * RHS_RING_ROWS) * TILE_PTS * sizeof(double);
-// NORMS (A8 as an epilogue of A5): six more rows, this thread's partial {sum C_a^2, sum C_iab^2, sum C_ijab^2,
-// max |C_a|, max |C_iab|, max |C_ijab|} (shared memory, not registers: the kernel already sits at the register limit)
+// NORMS (A8 as an epilogue of A5): this thread's partials {sum C_a^2, sum C_iab^2, sum C_ijab^2, max |C_a|,
+// max |C_iab|, max |C_ijab|} live in shared memory, not registers (the kernel already sits at the register limit): in rows 17..21
+// of ring slot 0 and row 17 of slot 1, which only the RK = 2 prefetch uses (its u0 values) and NORMS exists for RK = 1 only -
+// so the fused norms cost no shared memory (more of it would come out of the L1 that absorbs the kernel's spills).
 constexpr int RHS_NORM_ROWS = 6;
-constexpr size_t RHS_SMEM_BYTES_NORMS = RHS_SMEM_BYTES + (size_t)RHS_NORM_ROWS * TILE_PTS * sizeof(double);
+__host__ __device__ constexpr int rhs_norm_row(int q) { return RHS_PHI_ROWS + (q < 5 ? 17 + q : RHS_RING_ROWS + 17); }
+constexpr size_t RHS_SMEM_BYTES_NORMS = RHS_SMEM_BYTES;
 
 template <int PAIR, int RK>
 __device__ __forceinline__ void rhs_prefetch(double* __restrict__ slot /* + tid */, const double* __restrict__ du,
@@ -425,7 +428,8 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
                                           double* k, const RkArgs& rk, int64_t S, int* __restrict__ flag,
                                           double* __restrict__ phis /* + tid */) {
   double* __restrict__ ring = phis + RHS_PHI_ROWS * TILE_PTS;
-  double* __restrict__ nacc = ring + RHS_RING * RHS_RING_ROWS * TILE_PTS;    // NORMS: this thread's six partials
+  static_assert(!NORMS || RK == 1, "the NORMS partials sit in the ring rows of the RK = 2 prefetch");
+#define GH_NACC(q) phis[rhs_norm_row(q) * TILE_PTS]    /* NORMS: this thread's six partials */
   const int64_t p = sd.off + local;
   // face mask (A6)
   bool frozen;
@@ -493,7 +497,7 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
     double s0 = 0.0, m0 = 0.0;
 #pragma unroll
     for (int a = 0; a < 4; ++a) { s0 = fma(A.C[a], A.C[a], s0); m0 = nanmax(m0, fabs(A.C[a])); }
-    nacc[0] = s0; nacc[3 * TILE_PTS] = m0;
+    GH_NACC(0) = s0; GH_NACC(3) = m0;
   }
 
   ShellJac J;
@@ -524,15 +528,15 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
         }
       }
       if (NORMS) {   // C_iab = d_i psi_ab - Phi_iab;  C_ijab = d_i Phi_jab - d_j Phi_iab for (i,j) = (x,y), (x,z), (y,z)
-        double s1 = nacc[1 * TILE_PTS], m1 = nacc[4 * TILE_PTS];
+        double s1 = GH_NACC(1), m1 = GH_NACC(4);
 #pragma unroll
         for (int i = 0; i < 3; ++i) { const double c = d[0][i] - Phi(i, s); s1 = fma(c, c, s1); m1 = nanmax(m1, fabs(c)); }
-        nacc[1 * TILE_PTS] = s1; nacc[4 * TILE_PTS] = m1;
+        GH_NACC(1) = s1; GH_NACC(4) = m1;
         const double c01 = d[3][0] - d[2][1], c02 = d[4][0] - d[2][2], c12 = d[4][1] - d[3][2];
-        double s2 = nacc[2 * TILE_PTS];
+        double s2 = GH_NACC(2);
         s2 = fma(c01, c01, s2); s2 = fma(c02, c02, s2); s2 = fma(c12, c12, s2);
-        nacc[2 * TILE_PTS] = s2;
-        nacc[5 * TILE_PTS] = nanmax(nacc[5 * TILE_PTS], nanmax(fabs(c01), nanmax(fabs(c02), fabs(c12))));
+        GH_NACC(2) = s2;
+        GH_NACC(5) = nanmax(GH_NACC(5), nanmax(fabs(c01), nanmax(fabs(c02), fabs(c12))));
       }
       double sdpsi = 0.0, sdPi = 0.0, sPhi = 0.0;
 #pragma unroll
@@ -616,6 +620,7 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
       if (s == 6) rhs_prefetch<9, RK>(ring + 0 * SLOT, du, dHs, rk.u0, S, p);
 
     }
+#undef GH_NACC
 }
 
 // CBC: the domain has faces flagged CHARACTERISTIC (a second instantiation, so that domains without them do not pay for it).
@@ -636,10 +641,10 @@ k_rhs(const SubDev* __restrict__ subs, const int32_t* __restrict__ tile_first, i
     sd_s = subs[s];
     tile0_s = tile_first[s];
   }
-  double* nacc = ring_s + (RHS_PHI_ROWS + RHS_RING * RHS_RING_ROWS) * TILE_PTS + threadIdx.x;
+  double* nacc = ring_s + threadIdx.x;
   if (NORMS) {
 #pragma unroll
-    for (int q = 0; q < RHS_NORM_ROWS; ++q) nacc[q * TILE_PTS] = 0.0;      // own column: no barrier needed
+    for (int q = 0; q < RHS_NORM_ROWS; ++q) nacc[rhs_norm_row(q) * TILE_PTS] = 0.0;      // own column: no barrier needed
   }
   __syncthreads();
   const SubDev& sd = sd_s;
@@ -651,7 +656,7 @@ k_rhs(const SubDev* __restrict__ subs, const int32_t* __restrict__ tile_first, i
   if (NORMS) {    // the same fold as K_con: warp shuffle, then the warps in fixed order (deterministic)
     double acc[6];
 #pragma unroll
-    for (int q = 0; q < 6; ++q) acc[q] = nacc[q * TILE_PTS];
+    for (int q = 0; q < 6; ++q) acc[q] = nacc[rhs_norm_row(q) * TILE_PTS];
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
 #pragma unroll

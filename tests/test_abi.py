@@ -134,3 +134,28 @@ def test_filter_sigma_reading_s20():
     assert np.array_equal(gh.gh_filter_sigma({"kind": "none"}, 5), np.ones(6))
     with pytest.raises(gh.GHError):
         gh.gh_filter_sigma({"kind": "exp", "alpha": 1.0, "p": 0}, 5)
+
+
+def test_shell_basis_at_the_largest_band_limit():
+    """A0 at GH_MAX_L = 255 (SURVEY.md §7 hard part 5: sin^m(theta) underflows FP64 near the poles for m >~ 200; the builder works in
+    long double): quadrature orthonormality of the Pbar_lm on the 256 Gauss-Legendre nodes, read off the per-m projectors
+    Pr_m = 2 pi Pbar_m^T W-weighted: idempotent with trace = rank = L + 1 - m iff sum_j 2 pi w_j Pbar_lm Pbar_l'm = delta_ll';
+    Pr_0 = 1; d/dtheta composites annihilate nothing they should not: Th_m Pr_m = Th_m; the Chebyshev matrix at N = 320 still
+    differentiates x^p exactly."""
+    L = 255
+    Fa, Fs, Th, Pr = gh.gh_basis_shell(L)
+    nt = L + 1
+    assert np.all(np.isfinite(Th)) and np.all(np.isfinite(Pr))
+    assert np.max(np.abs(Pr[0] - np.eye(nt))) < 1e-13
+    for m in (1, 2, 77, 128, 200, 254, 255):
+        P = Pr[m]
+        assert np.max(np.abs(P @ P - P)) < 1e-13, m
+        assert abs(np.trace(P) - (L + 1 - m)) < 1e-12 * nt, m
+        assert np.max(np.abs(Th[m] @ P - Th[m])) < 1e-11 * np.max(np.abs(Th[m])), m
+    # the Fourier pair is the projector onto m <= L on the 512 longitudes
+    F = Fs @ Fa
+    assert np.max(np.abs(F @ F - F)) < 1e-13 and abs(np.trace(F) - (2 * L + 1)) < 1e-10
+    x, D = gh.gh_basis_cheb(320)
+    for p in (0, 1, 7, 100, 319):
+        ref = p * x ** max(p - 1, 0) if p > 0 else np.zeros(320)
+        assert np.max(np.abs(D @ x ** p - ref)) < 1e-9 * max(1.0, p * p), p

@@ -332,7 +332,8 @@ def _rhs_and_step_parity(oracle, dom, descs, us, Hs, what):
 
 
 def test_gradient_parity_at_the_size_limits(oracle):
-    """GH_MAX_L = 47 (the last m-tile count of K_ang S2, one plane group of two planes) and GH_MAX_CHEB_N = 64 on the radial axis."""
+    """The limits of the small kernel classes: GH_SMALL_L = 47 (the last m-tile count of K_ang S2, one plane group of two planes) and
+    GH_SMALL_CHEB_N = 64 on the radial axis (beyond them the K_gemm path takes over: tests/test_gpu_large.py)."""
     descs = [configs.shell(2, 47, 3.0, 4.0), configs.shell(64, 3, 2.0, 9.0)]
     cfg = {"id": 10, "spin": 0.2, "amplitude": 1e-3, "descs": descs}
     descs, coords, us, Hs = build_case(cfg, oracle)
@@ -345,10 +346,6 @@ def test_gradient_parity_at_the_size_limits(oracle):
             assert_parity(got[k], ref[k], state=us[s], tol=TOL, what=f"limits sub {s} d_{k}")
     _rhs_and_step_parity(oracle, dom, descs, us, Hs, "limits")
     dom.close()
-    with pytest.raises(gh.GHError):
-        gh.Domain([configs.shell(4, 48, 3.0, 4.0)])
-    with pytest.raises(gh.GHError):
-        gh.Domain([configs.block([65, 4, 4], (0, 0, 0), (1, 1, 1))])
 
 
 def test_c4_full_size_sampled_parity(oracle):
