@@ -1,13 +1,18 @@
 #!/usr/bin/env python
 """bench.py — throughput of the GH right-hand-side hot path (arXiv 1804.09101) on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload c4|c3|c2|c1]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload c4|c3|c2|c1|c5]
 
 Metric (BASELINE.json): GH RHS grid-point evaluations per second, FP64.  One "step" is one pass of the whole
-hot path (rows A2-A8) over the workload: one `gh_rk_step` (3 x [Chebyshev + angular derivatives,
-fused Jacobian + pointwise RHS + face mask + RK3 stage update as its epilogue]) followed by one `gh_constraint_norms`
-(derivatives + constraint kernel + reduction).  value = 3 * P * K / T: only the three RHS evaluations of the RK3
-step are counted as "evaluations"; the constraint pass is extra work inside the timed region.
+hot path (rows A2-A8) over the workload: one `gh_rk_step_norms` = 3 x [Chebyshev + angular derivatives,
+fused Jacobian + pointwise RHS + face mask + RK3 stage update as its epilogue], with the constraint norms of the step's
+input state as an epilogue of the first stage (A8 fused into A5).  value = 3 * P * K / T.
+Protocol (the paper's): W >= 3 warm-up steps, then K timed steps with the library's
+per-launch events OFF; `ms_per_step` = T / K over the whole region, `ms_per_step_median` = median of the K per-step CUDA-event
+times; the per-kernel split comes from a SECOND pass with the per-launch events on; the FP64 peak the derivative kernels
+are quoted against is measured in the same run (gh_fp64_peak).
+`--workload c5` is the size sweep of BASELINE.json configs[4]: one JSON line per member (single shells N_r = L+1 = n and
+single cubes N^3, 1e3 ... 3.3e7 points): gh_rhs points/s, derivative-kernel FP64 rate, k_rhs GB/s.
 
 Default workload: C4 (BASELINE.json configs[3], the production-like isolated-BH domain: 40 shells + 24 cube
 blocks, spin 0.9, replicated to >= 4M points, reading S13) - the configuration the HBM-roofline part of the
@@ -56,13 +61,9 @@ def load_peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-# FP64 peak for the derivative kernels (bound "alu"): measured with paper_1804_09101_b200/tools/fp64_peak.cu on this
-# pool's B200 at 1965 MHz; DFMA and DMMA share one datapath (mixing them gains nothing), DESIGN.md §6.
-FP64_PEAK_MEASURED_TFLOPS = 37.1    # DMMA m8n8k4, register resident, profiles/r01_fp64_peak.md (DFMA: 33.9; nominal 37.2)
-
-
-def fp64_peak_tflops() -> float:
-    return FP64_PEAK_MEASURED_TFLOPS
+# FP64 peak for the derivative kernels (bound "alu"): measured IN THIS RUN by the library's probe (gh_fp64_peak: register-
+# resident DMMA m8n8k4 and DFMA kernels; the two share one datapath).  Round 1 measured 37.1 / 33.9 TFLOP/s
+# (profiles/r01_fp64_peak.md); nominal 148 SM x 64 FMA x 2 x 1.965 GHz = 37.2.
 
 
 # ------------------------------------------------------------------------------------------------------------------
@@ -304,6 +305,12 @@ def run_ours(args):
         dist.barrier()
     torch.cuda.set_device(local_rank)
     dev = f"cuda:{local_rank}"
+    if args.workload == "c5":
+        if rank == 0:
+            run_sweep(args, dev)
+        if dist is not None:
+            dist.barrier(); dist.destroy_process_group()
+        return
 
     cfg, base, label = make_config(args.workload, args.min_points)
     descs = cfg["descs"]
@@ -343,30 +350,40 @@ def run_ours(args):
             return dom.constraint_norms()
         return dom.rk_step_norms(dt)
 
-    # ---- device-resident timing -----------------------------------------------------------------------------
+    fp64 = dom.fp64_peak()      # (DMMA, DFMA) TFLOP/s of this GPU, now
+
+    # ---- device-resident timing: per-launch events OFF; one CUDA event between steps on the library's stream (= torch's current) ----
     dom.set_fields(u_dev, 0.0)
     for _ in range(args.warmup):
         step()
     dom.set_fields(u_dev, 0.0)
-    dom.set_profiling(True)
-    dom.profile_reset()
+    dom.set_profiling(False)
     l0 = dom.launch_count()
     sampler = ClockSampler(local_rank)
     sampler.start()
     sync_all()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for _ in range(args.steps):
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    ev[0].record()
+    for i in range(args.steps):
         norms = step()
-    e1.record()
+        ev[i + 1].record()
     sync_all()
-    ms = e0.elapsed_time(e1)
+    ms = ev[0].elapsed_time(ev[-1])
+    per_step = [ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps)]
     clocks = sampler.stop()
     launches = dom.launch_count() - l0
-    prof = dom.profile_read()
-    dom.set_profiling(False)
     if not np.all(np.isfinite(norms)):
         raise SystemExit("bench.py: non-finite constraint norms after the timed region")
+
+    # ---- second pass, per-launch events ON: the per-kernel split (not part of `value`) -------------------------------------
+    prof_steps = max(1, min(args.steps, args.profile_steps))
+    dom.set_fields(u_dev, 0.0)
+    dom.set_profiling(True)
+    dom.profile_reset()
+    for _ in range(prof_steps):
+        step()
+    prof = dom.profile_read()
+    dom.set_profiling(False)
 
     # ---- end to end through the C ABI with HOST buffers (pinned): H2D of the state, step, D2H of the state --------
     out_host = torch.empty(50, S, dtype=torch.float64).pin_memory()
@@ -383,18 +400,45 @@ def run_ours(args):
     e2e_s = time.perf_counter() - t0
     if not bool(torch.isfinite(out_host).all()):
         raise SystemExit("bench.py: non-finite state after the e2e region")
+    # what the two copies alone cost (the PCIe floor of the end-to-end number)
+    t0 = time.perf_counter(); dom.set_fields(u_host, 0.0); torch.cuda.synchronize(); h2d_s = time.perf_counter() - t0
+    t0 = time.perf_counter(); dom.get_fields(out_host); torch.cuda.synchronize(); d2h_s = time.perf_counter() - t0
+    pcie = {"h2d_GBps": 50 * S * 8 / h2d_s / 1e9, "d2h_GBps": 50 * S * 8 / d2h_s / 1e9, "copies_only_ms": (h2d_s + d2h_s) * 1e3}
 
     filt = time_filter(dom, u_dev, descs) if rank == 0 and not args.no_extras else None
     dp5 = time_dp5(dom, u_dev, dt, P) if rank == 0 and not args.no_extras else None
+    scj = time_scj(dom, u_dev, P) if rank == 0 and not args.no_extras else None
 
-    tmax, e2emax = max_over_ranks([ms, e2e_s / e2e_steps], dist, dev)
+    tmax, e2emax, med = max_over_ranks([ms, e2e_s / e2e_steps, float(np.median(per_step))], dist, dev)
     if rank != 0:
         dom.close()
         if dist is not None:
             dist.barrier(); dist.destroy_process_group()
         return
-    return finish_ours(args, world, label, cfg, descs, reps, P, S, tmax, e2emax, e2e_steps, launches, prof, work, clocks,
-                       norms, base, dom, dist, filt, dp5)
+    return finish_ours(args, world, label, cfg, descs, reps, P, S, tmax, e2emax, e2e_steps, launches, prof, prof_steps, work, clocks,
+                       norms, base, dom, dist, filt, dp5, scj, fp64, med, per_step, pcie)
+
+
+def time_scj(dom, u_dev, P, reps: int = 5):
+    """NEXT-4 (outside the timed step): gh_spatial_coord_jac_state with a rotation-about-z Jacobian field; HBM-bound,
+    (2 x 50 + 9) doubles per point."""
+    import torch
+
+    J = torch.zeros(9, dom.S, dtype=torch.float64, device=u_dev.device)
+    c, s = float(np.cos(0.3)), float(np.sin(0.3))
+    J[0], J[1], J[3], J[4], J[8] = c, -s, s, c, 1.0
+    dom.set_jacobian(J)
+    dom.set_fields(u_dev, 0.0)
+    for _ in range(2):
+        dom.spatial_coord_jac_state()
+    dom.set_profiling(True)
+    dom.profile_reset()
+    for _ in range(reps):
+        dom.spatial_coord_jac_state()
+    prof = dom.profile_read()
+    dom.set_profiling(False)
+    ms = prof["k_scj"][0] / reps
+    return {"ms_per_call": ms, "achieved_GBps": 109 * 8.0 * P / (ms * 1e-3) / 1e9, "bound": "hbm", "bytes_per_point": 109 * 8}
 
 
 def time_filter(dom, u_dev, descs, reps: int = 5):
@@ -448,27 +492,26 @@ def time_dp5(dom, u_dev, dt, P, reps: int = 3):
     return {"ms_per_step": s_per * 1e3, "rhs_evals_per_step": 6, "points_per_s": 6.0 * P / s_per, "err_rms": rms, "err_max": mx}
 
 
-def finish_ours(args, world, label, cfg, descs, reps, P, S, ms, e2e_step_s, e2e_steps, launches, prof, work, clocks,
-                norms, base, dom, dist, filt=None, dp5=None):
+def finish_ours(args, world, label, cfg, descs, reps, P, S, ms, e2e_step_s, e2e_steps, launches, prof, prof_steps, work, clocks,
+                norms, base, dom, dist, filt, dp5, scj, fp64, ms_median, per_step, pcie):
     hbm_peak, peak_src = load_peaks()
     steps = args.steps
     value = whole_job_value(world, P, steps, ms)
-    # per-kernel numbers from the CUDA events the library records around each launch on its own stream
+    # per-kernel numbers from the SECOND pass (library CUDA events around each launch on its own stream)
     total_kernel_ms = sum(v[0] for v in prof.values()) or 1.0
-    # work-equivalent calls per step: the constraint pass differentiates 40 of the 50 components (no d Pi needed)
     nd = 3.8 if args.unfused_norms else 3.0     # derivative passes per step (the stand-alone constraint pass differentiates 40 of 50 components)
     calls_per_step = {"k_rhs": 3, "k_con": 1, "k_cheb": nd, "k_ang": nd}   # library calls that run the kernel
     kernels = {}
     for name, (kms, cnt) in prof.items():
-        if cnt == 0 or "filter" in name or name.startswith("k_dp"):
+        if cnt == 0 or "filter" in name or name.startswith("k_dp") or name == "k_scj":
             continue
-        e = {"launches_per_step": cnt / steps, "ms_per_launch": kms / cnt, "ms_per_step": kms / steps,
+        e = {"launches_per_step": cnt / prof_steps, "ms_per_launch": kms / cnt, "ms_per_step": kms / prof_steps,
              "share_of_kernel_time": kms / total_kernel_ms}
         w = work.get(name)
         if w:
-            # one "call" = all launches of this kernel inside one gh_rhs / gh_constraint_norms (K_ang: one launch per
-            # shared-memory class); work is per call, time is the measured total over the timed region
-            per_call_s = kms * 1e-3 / (steps * calls_per_step[name])
+            # one "call" = all launches of this kernel inside one RHS evaluation (K_ang: one launch per shared-memory class);
+            # work is per call, time is the measured total over the profiled pass
+            per_call_s = kms * 1e-3 / (prof_steps * calls_per_step[name])
             e["ms_per_call"] = per_call_s * 1e3
             e["achieved_GBps"] = w["bytes"] / per_call_s / 1e9
             e["achieved_TFLOPs"] = w["flop"] / per_call_s / 1e12
@@ -477,7 +520,7 @@ def finish_ours(args, world, label, cfg, descs, reps, P, S, ms, e2e_step_s, e2e_
                 e["executed_TFLOPs"] = w["flop_executed"] / per_call_s / 1e12
         kernels[name] = e
     top = max((k for k in kernels if k in work), key=lambda k: kernels[k]["share_of_kernel_time"])
-    fp64_peak = fp64_peak_tflops()
+    fp64_peak = fp64[0]
     if work[top]["bound"] == "hbm":
         roof = {"kernel": top, "bound": "hbm", "achieved": kernels[top]["achieved_GBps"], "peak": hbm_peak, "unit": "GB/s",
                 "frac": kernels[top]["achieved_GBps"] / hbm_peak, "peak_source": peak_src,
@@ -485,8 +528,10 @@ def finish_ours(args, world, label, cfg, descs, reps, P, S, ms, e2e_step_s, e2e_
     else:
         roof = {"kernel": top, "bound": "alu", "achieved": kernels[top]["achieved_TFLOPs"], "peak": fp64_peak, "unit": "TFLOP/s",
                 "frac": kernels[top]["achieved_TFLOPs"] / fp64_peak,
-                "peak_source": "measured: DMMA m8n8k4 register-resident microbenchmark on this pool's B200 (profiles/r01_fp64_peak.md)",
+                "peak_source": "measured in this run (gh_fp64_peak: register-resident DMMA m8n8k4 kernel on this GPU)",
                 "algorithmic_flop_per_launch": work[top]["flop"], "traffic": read_traffic(top, P)}
+        if "executed_TFLOPs" in kernels[top]:
+            roof["issued_frac"] = kernels[top]["executed_TFLOPs"] / fp64_peak
     # the fused RHS kernel is the one north_star sets a target for: always report it too
     roof_rhs = None
     if "k_rhs" in kernels:
@@ -509,26 +554,31 @@ def finish_ours(args, world, label, cfg, descs, reps, P, S, ms, e2e_step_s, e2e_
 
     h2d = 50 * S * 8
     d2h = 50 * S * 8 + 6 * 8
+    step_name = "gh_rk_step + gh_constraint_norms" if args.unfused_norms else "gh_rk_step_norms (RK3 step, constraint norms fused into stage 1)"
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": args.warmup,
-        "ms_per_step": ms / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "ms_per_step": ms / steps, "ms_per_step_median": ms_median, "ms_per_step_min": float(min(per_step)), "ms_per_step_max": float(max(per_step)),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic",
         "config": {"workload": label, "points_per_gpu": P, "subdomains": len(descs), "replicas_of_base_set": reps,
                    "components": 50, "dt": float(cfg["dt"]), "rhs_evals_per_step": 3,
-                   "step": "gh_rk_step + gh_constraint_norms" if args.unfused_norms else "gh_rk_step_norms (RK3 step with the constraint norms fused into stage 1)", "parallelism": "replicas only" if world > 1 else "single GPU",
+                   "step": step_name, "parallelism": "replicas only" if world > 1 else "single GPU",
                    "l2": f"inputs larger than L2: the step streams {316 * S * 8 / 1e9:.2f} GB of state/derivative arrays (L2 126 MB)",
-                   "per_launch_events": "on (library CUDA events around every kernel launch, inside the timed region)"},
+                   "per_launch_events": f"off in the timed region; the per-kernel split is from a second pass of {prof_steps} steps with them on"},
         "rk_steps_per_s": world * steps / (ms * 1e-3),
         "gpu_launches": int(launches),
         "roofline": roof, "roofline_k_rhs": roof_rhs, "kernels": kernels,
+        "fp64_peak_measured_TFLOPs": {"dmma_m8n8k4": fp64[0], "dfma": fp64[1]},
         "cpu_baseline": cpu,
         "e2e": {"value": world * 3.0 * P / e2e_step_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "steps": e2e_steps, "ms_per_step": e2e_step_s * 1e3,
-                "path": "gh_set_fields(HOST pinned) + the step + gh_get_fields(HOST pinned)"},
+                "path": "gh_set_fields(HOST pinned) + the step + gh_get_fields(HOST pinned); the copies are not overlapped with the step",
+                "pcie": pcie},
         "clocks": clocks,
-        "constraint_norms_after": [[float(x) for x in r] for r in np.asarray(norms)],
+        "constraint_norms_of_last_step_input": [[float(x) for x in r] for r in np.asarray(norms)],
         "spectral_filter": filt,
         "dormand_prince_5_4": dp5,
+        "spatial_coord_jac_state": scj,
     }
     print(json.dumps(out))
     sys.stdout.flush()
@@ -536,6 +586,84 @@ def finish_ours(args, world, label, cfg, descs, reps, P, S, ms, e2e_step_s, e2e_
     if dist is not None:
         dist.barrier(); dist.destroy_process_group()
     return out
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# the size sweep (BASELINE.json configs[4]): one JSON line per member
+# ------------------------------------------------------------------------------------------------------------------
+def sweep_members(max_points):
+    from paper_1804_09101_b200 import configs
+
+    out = []
+    for n in (8, 16, 32, 64, 128, 256):
+        out.append((f"shell n={n} (N_r={n}, L={n - 1})", configs.c5_shell(n)))
+    for N in (10, 20, 40, 80, 160, 320):
+        out.append((f"block {N}^3", configs.c5_block(N)))
+    return [(lbl, cfg) for lbl, cfg in out if configs.num_points(cfg["descs"][0]) <= max_points]
+
+
+def run_sweep(args, dev):
+    """gh_rhs on every member: median of `reps` calls after 3 warm-ups, per-kernel times from the library's events; the derivative
+    rate counts the algorithmic flop of the factored maps, and the paper's dense-matrix convention beside it."""
+    import torch
+
+    from paper_1804_09101_b200 import configs, gh, inputs, opcount
+
+    hbm_peak, _ = load_peaks()
+    for label, cfg in sweep_members(args.sweep_max_points):
+        d = cfg["descs"][0]
+        dom = gh.Domain([d], device=dev)
+        P, S = dom.P, dom.S
+        xyz = np.zeros((3, S)); gh.gh_domain_coords(dom.h, xyz)
+        u = torch.zeros(50, S, dtype=torch.float64).pin_memory()
+        H = np.zeros((4, S))
+        inputs.initial_data_chunked(d, xyz[:, :P], cfg["spin"], cfg["amplitude"], cfg["id"], 0, u.numpy()[:, :P], H[:, :P])
+        del xyz
+        dom.set_gauge_source(H)
+        dom.set_fields(u, 0.0)
+        del u, H
+        out = dom.empty(50)
+        fp64 = dom.fp64_peak()
+        reps = args.sweep_reps if P < 5_000_000 else max(3, args.sweep_reps // 4)
+        for _ in range(3):
+            dom.rhs(out)
+        dom.set_profiling(True)
+        tot, der, rhs = [], [], []
+        for _ in range(reps):
+            dom.profile_reset()
+            dom.rhs(out)
+            prof = dom.profile_read()
+            t_der = prof["k_cheb"][0] + prof["k_ang"][0]
+            tot.append(t_der + prof["k_rhs"][0]); der.append(t_der); rhs.append(prof["k_rhs"][0])
+        dom.set_profiling(False)
+        # wall time of the call with events off (launch overhead included: the latency regime of the small members)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        wall = []
+        for _ in range(reps):
+            e0.record(); dom.rhs(out); e1.record(); torch.cuda.synchronize()
+            wall.append(e0.elapsed_time(e1))
+        if not bool(torch.isfinite(out).all()):
+            raise SystemExit(f"bench.py: non-finite RHS on {label}")
+        if d["kind"] == "shell":
+            flop = opcount.shell_factored_flop(50, d["n"][0], d["n"][1])
+            flop_paper = opcount.shell_deriv_dense(50, d["n"][0], d["n"][1] + 1, 2 * d["n"][1] + 2)[1]
+        else:
+            flop = flop_paper = opcount.block_deriv(50, *d["n"])[1]
+        ms, ms_d, ms_r, ms_w = (float(np.median(x)) for x in (tot, der, rhs, wall))
+        line = {"metric": "gh_rhs_points_per_s", "workload": "c5", "member": label, "points": P, "reps": reps,
+                "gh_rhs_ms_kernels": ms, "gh_rhs_ms_call": ms_w, "points_per_s": P / (ms_w * 1e-3), "unit": UNIT,
+                "deriv_ms": ms_d, "deriv_TFLOPs": flop / (ms_d * 1e-3) / 1e12, "deriv_frac_of_fp64_peak": flop / (ms_d * 1e-3) / 1e12 / fp64[0],
+                "deriv_TFLOPs_paper_dense_convention": flop_paper / (ms_d * 1e-3) / 1e12,
+                "k_rhs_ms": ms_r, "k_rhs_GBps": float(BYTES_RHS_PT) * P / (ms_r * 1e-3) / 1e9,
+                "k_rhs_frac_of_hbm": float(BYTES_RHS_PT) * P / (ms_r * 1e-3) / 1e9 / hbm_peak,
+                "fp64_peak_measured_TFLOPs": fp64[0], "dtype": "f64", "data": "synthetic",
+                "regime": "single subdomain (latency-bound below ~1e5 points: the call is 3-7 launches)"}
+        print(json.dumps(line))
+        sys.stdout.flush()
+        dom.close()
+        del dom, out
+        torch.cuda.empty_cache()
 
 
 # ------------------------------------------------------------------------------------------------------------------
@@ -565,10 +693,13 @@ def run_reference(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
-    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c4", choices=["c1", "c2", "c3", "c4"])
+    ap.add_argument("--workload", default="c4", choices=["c1", "c2", "c3", "c4", "c5"])
+    ap.add_argument("--profile-steps", type=int, default=10, help="steps of the second (per-launch events on) pass")
+    ap.add_argument("--sweep-reps", type=int, default=20, help="c5: repetitions per member")
+    ap.add_argument("--sweep-max-points", type=int, default=40_000_000, help="c5: skip members above this size")
     ap.add_argument("--min-points", type=int, default=4_000_000, help="C4: replicate the base set until P >= this")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--cpu-points", type=int, default=1_300_000,

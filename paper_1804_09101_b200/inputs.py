@@ -268,9 +268,11 @@ def _real_ylm(lmax: int, theta: np.ndarray, phi: np.ndarray) -> np.ndarray:
     return np.stack(out)
 
 
-def shell_perturbation(r_lo, r_hi, center, xyz, amplitude, seed, kmax=4, lmax=4) -> np.ndarray:
+def shell_perturbation(r_lo, r_hi, center, xyz, amplitude, seed, kmax=4, lmax=4, norm=None) -> np.ndarray:
     """[50,P] perturbation: per component sum_{k<=kmax} sum_{l<=lmax,m} c_klm T_k(x(r)) Y^real_lm,
-    c uniform in [-1,1) from SplitMix64(seed), each component rescaled to L-inf = amplitude."""
+    c uniform in [-1,1) from SplitMix64(seed), each component rescaled to L-inf = amplitude.
+    norm: None, or [50] maxima to normalise with instead of this call's own (chunked generation; amplitude = None returns
+    the unnormalised functions)."""
     rel = np.asarray(xyz, dtype=np.float64) - np.asarray(center, dtype=np.float64)[:, None]
     r = np.sqrt((rel * rel).sum(0))
     theta = np.arccos(np.clip(rel[2] / r, -1.0, 1.0))
@@ -284,13 +286,13 @@ def shell_perturbation(r_lo, r_hi, center, xyz, amplitude, seed, kmax=4, lmax=4)
     for c in range(N_COMP):
         coef = rng.uniform(K * S).reshape(K, S)
         f = ((coef @ Y) * T).sum(0)          # sum_k T_k(x) sum_s c_ks Y_s
-        out[c] = f * (amplitude / np.max(np.abs(f)))
+        out[c] = f if amplitude is None else f * (amplitude / (np.max(np.abs(f)) if norm is None else norm[c]))
     return out
 
 
-def block_perturbation(lo, hi, xyz, amplitude, seed, deg=6) -> np.ndarray:
+def block_perturbation(lo, hi, xyz, amplitude, seed, deg=6, norm=None) -> np.ndarray:
     """[50,P] perturbation: per component sum_{i,j,k<=deg} c_ijk T_i T_j T_k on the block's
-    reference cube, rescaled to L-inf = amplitude."""
+    reference cube, rescaled to L-inf = amplitude (norm: as in shell_perturbation)."""
     xyz = np.asarray(xyz, dtype=np.float64)
     T = [_cheb_T(deg, 2.0 * (xyz[d] - lo[d]) / (hi[d] - lo[d]) - 1.0) for d in range(3)]
     rng = SplitMix64(seed)
@@ -301,7 +303,7 @@ def block_perturbation(lo, hi, xyz, amplitude, seed, deg=6) -> np.ndarray:
         f = (coef.reshape(n * n, n) @ T[2]).reshape(n, n, -1)   # sum over k
         f = (f * T[1][None]).sum(1)                               # sum over j
         f = (f * T[0]).sum(0)                                     # sum over i
-        out[c] = f * (amplitude / np.max(np.abs(f)))
+        out[c] = f if amplitude is None else f * (amplitude / (np.max(np.abs(f)) if norm is None else norm[c]))
     return out
 
 
@@ -326,3 +328,29 @@ def initial_data(descs, coords, spin, amplitude, config_id, M=1.0):
         us.append(np.ascontiguousarray(u))
         Hs.append(np.ascontiguousarray(kerr_schild_gauge_source(xyz, M, spin)))
     return us, Hs
+
+
+def initial_data_chunked(d, xyz, spin, amplitude, config_id, s, u_out, H_out, chunk=1 << 20, M=1.0):
+    """The same data as initial_data for ONE subdomain, written into u_out[50,P] / H_out[4,P] chunk by chunk (the sweep's
+    largest members have 3.3e7 points: the temporaries of a single pass would be tens of GB).  Two passes over the
+    perturbation: component maxima first (the L-inf normalisation is over the whole subdomain), then the data."""
+    P = xyz.shape[1]
+    seed = SEED_BASE + 1000 * config_id + s
+
+    def pert(sl, amp, norm):
+        if d["kind"] == "shell":
+            return shell_perturbation(d["lo"][0], d["hi"][0], d["center"], xyz[:, sl], amp, seed, norm=norm)
+        return block_perturbation(d["lo"], d["hi"], xyz[:, sl], amp, seed, norm=norm)
+
+    norm = None
+    if amplitude != 0.0:
+        norm = np.zeros(N_COMP)
+        for p0 in range(0, P, chunk):
+            norm = np.maximum(norm, np.max(np.abs(pert(slice(p0, min(P, p0 + chunk)), None, None)), axis=1))
+    for p0 in range(0, P, chunk):
+        sl = slice(p0, min(P, p0 + chunk))
+        u = pack_fields(*kerr_schild(xyz[:, sl], M, spin))
+        if amplitude != 0.0:
+            u = u + pert(sl, amplitude, norm)
+        u_out[:, sl] = u
+        H_out[:, sl] = kerr_schild_gauge_source(xyz[:, sl], M, spin)

@@ -90,9 +90,11 @@ def test_sweep_sizes_thin(oracle):
     cfg = {"id": 33, "spin": 0.5, "amplitude": 1e-4,
            "descs": [configs.block([320, 4, 4], (3.0, -1.0, -1.0), (11.0, 1.0, 1.0)),
                      configs.block([4, 128, 3], (3.0, -4.0, -1.0), (5.0, 4.0, 1.0)),
-                     configs.block([3, 4, 320], (3.0, -1.0, -4.0), (5.0, 1.0, 4.0)),
-                     configs.shell(2, 127, 3.0, 4.0)]}
+                     configs.block([3, 4, 320], (3.0, -1.0, -4.0), (5.0, 1.0, 4.0))]}
     _check_all(oracle, cfg, "sweep sizes")
+    # the oracle's Y_lm quadruple loops cost ~3 s per plane at L = 127: gradient only, 16 components (one per host core)
+    shell = {"id": 35, "spin": 0.5, "amplitude": 1e-4, "descs": [configs.shell(2, 127, 3.0, 4.0)]}
+    _check_all(oracle, shell, "L = 127 shell", rk=False, ncomp_grad=16)
     cube = {"id": 34, "spin": 0.5, "amplitude": 1e-4, "descs": [configs.block(72, (3.0, -4.0, -4.0), (11.0, 4.0, 4.0))]}
     _check_all(oracle, cube, "72^3 cube", rk=False, ncomp_grad=8)
 
