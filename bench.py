@@ -317,6 +317,8 @@ def run_ours(args):
     nbase = len(base["descs"])
     reps = len(descs) // nbase
     dom = gh.Domain(descs, device=dev)
+    if args.no_graph:
+        dom.set_option(gh.GH_OPT_NO_GRAPH, 1)
     P, S = dom.P, dom.S
 
     # inputs: analytic data evaluated on the library's own grid (gh_domain_coords) for the base subdomain set,
@@ -363,10 +365,10 @@ def run_ours(args):
     sampler.start()
     sync_all()
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
-    ev[0].record()
+    ev[0].record(dom.stream)          # the library's stream (the domain's own), which is where its kernels run
     for i in range(args.steps):
         norms = step()
-        ev[i + 1].record()
+        ev[i + 1].record(dom.stream)
     sync_all()
     ms = ev[0].elapsed_time(ev[-1])
     per_step = [ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps)]
@@ -564,7 +566,8 @@ def finish_ours(args, world, label, cfg, descs, reps, P, S, ms, e2e_step_s, e2e_
                    "components": 50, "dt": float(cfg["dt"]), "rhs_evals_per_step": 3,
                    "step": step_name, "parallelism": "replicas only" if world > 1 else "single GPU",
                    "l2": f"inputs larger than L2: the step streams {316 * S * 8 / 1e9:.2f} GB of state/derivative arrays (L2 126 MB)",
-                   "per_launch_events": f"off in the timed region; the per-kernel split is from a second pass of {prof_steps} steps with them on"},
+                   "per_launch_events": f"off in the timed region; the per-kernel split is from a second pass of {prof_steps} steps with them on",
+                   "cuda_graph": "off (--no-graph)" if args.no_graph else "each step replays one captured CUDA graph (gpu_launches counts its kernel nodes)"},
         "rk_steps_per_s": world * steps / (ms * 1e-3),
         "gpu_launches": int(launches),
         "roofline": roof, "roofline_k_rhs": roof_rhs, "kernels": kernels,
@@ -641,7 +644,7 @@ def run_sweep(args, dev):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         wall = []
         for _ in range(reps):
-            e0.record(); dom.rhs(out); e1.record(); torch.cuda.synchronize()
+            e0.record(dom.stream); dom.rhs(out); e1.record(dom.stream); torch.cuda.synchronize()
             wall.append(e0.elapsed_time(e1))
         if not bool(torch.isfinite(out).all()):
             raise SystemExit(f"bench.py: non-finite RHS on {label}")
@@ -706,6 +709,7 @@ def main():
                     help="points in the cpu_baseline sample (default: the whole 64-subdomain base set, ~10 s on 16 cores)")
     ap.add_argument("--ref-points", type=int, default=60_000, help="points per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-graph", action="store_true", help="enqueue the step's kernels one by one instead of replaying the captured CUDA graph")
     ap.add_argument("--unfused-norms", action="store_true", help="step = gh_rk_step + stand-alone gh_constraint_norms (the round-1 path)")
     ap.add_argument("--no-extras", action="store_true", help="skip the spectral-filter and Dormand-Prince legs (run after the timed step)")
     args = ap.parse_args()

@@ -245,9 +245,15 @@ const char* gh_kernel_name(int k);
  *   GH_OPT_RK_OUT_OF_PLACE  1: every stage of gh_rk_step writes to a buffer it does not read (ua -> ub -> k -> ua) instead of
  *                           updating in place.  The in-place stages are by design (the fused RHS kernel holds every field of a
  *                           point in registers / shared memory before its first store); this switch exists so that a test can
- *                           demand bit-equality of the two (compute-sanitizer is not available on the GPU pool). */
+ *                           demand bit-equality of the two (compute-sanitizer is not available on the GPU pool).
+ *   GH_OPT_NO_GRAPH         1: gh_rk_step / gh_rk_step_norms / gh_rhs(DEVICE) enqueue their kernels one by one.  Default 0: the
+ *                           whole call (the three stages of a step: up to ~20 launches) is captured once into a CUDA graph
+ *                           and replayed as ONE launch - the paper's central lesson is launch overhead (~20 us per kernel,
+ *                           PAPER.md:241, 472), and configs C1-C3 are launch-bound.  The graph is re-captured when dt, the
+ *                           buffers or an option change; it needs a real stream (not the legacy default stream 0, which
+ *                           cannot be captured: then, and while profiling is on, the kernels are enqueued one by one). */
 #define GH_NUM_OPTIONS 8
-enum { GH_OPT_RK_OUT_OF_PLACE = 0 };
+enum { GH_OPT_RK_OUT_OF_PLACE = 0, GH_OPT_NO_GRAPH = 1 };
 gh_status gh_set_option(gh_domain* dom, int option, int value);
 
 /* Number of kernel launches issued by the library on this domain since creation. */

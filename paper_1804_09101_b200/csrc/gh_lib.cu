@@ -292,6 +292,10 @@ struct gh_domain {
   bool has_fields = false, has_shell = false, has_block = false, has_char = false, has_ifc = false;
   int device = 0, n_sm = 148;            // the device the workspace lives on (current at create) and its SM count
   int opt[GH_NUM_OPTIONS] = {0};         // gh_set_option
+  // CUDA graphs of the step (kind 0: gh_rk_step, 1: gh_rk_step_norms) and of gh_rhs to a DEVICE pointer (kind 2), each valid
+  // for the key it was captured with
+  struct StepGraph { cudaGraphExec_t exec = nullptr; double dt = 0; const void *ua = nullptr, *ub = nullptr, *out = nullptr; int oop = 0; int64_t nlaunch = 0; };
+  StepGraph graphs[3];
   double t = 0.0;
   int64_t launches = 0;
   std::string err;
@@ -437,13 +441,13 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
   // elem(row, col) of an (M x K) matrix -> A-fragment order, blocked [m_block][k_chunk][GEMM_MB m-tiles][GEMM_KB k-steps][32];
   // returns the offset (doubles) of the matrix from d->tables
   auto put_amat = [&](int M, int K, auto elem) {
-    const int MT = (M + 7) / 8, KS = (K + 3) / 4, nMB = (MT + GEMM_MB - 1) / GEMM_MB, nKC = (KS + GEMM_KB - 1) / GEMM_KB;
+    const int MT = (M + 7) / 8, KS = (K + 3) / 4, mbs = gemm_mbs(M, GEMM_MB), nMB = (MT + mbs - 1) / mbs, nKC = (KS + GEMM_KB - 1) / GEMM_KB;
     const size_t at = btp;
-    for (int mb = 0; mb < nMB; ++mb) for (int kc = 0; kc < nKC; ++kc) for (int mt = 0; mt < GEMM_MB; ++mt) for (int ks = 0; ks < GEMM_KB; ++ks)
+    for (int mb = 0; mb < nMB; ++mb) for (int kc = 0; kc < nKC; ++kc) for (int mt = 0; mt < mbs; ++mt) for (int ks = 0; ks < GEMM_KB; ++ks)
       for (int lane = 0; lane < 32; ++lane) {
-        const int row = (mb * GEMM_MB + mt) * 8 + lane / 4, col = (kc * GEMM_KB + ks) * 4 + lane % 4;
+        const int row = (mb * mbs + mt) * 8 + lane / 4, col = (kc * GEMM_KB + ks) * 4 + lane % 4;
         if (row < M && col < K)
-          bigtab[at + ((((size_t)mb * nKC + kc) * GEMM_MB + mt) * GEMM_KB + ks) * 32 + lane] = (double)elem(row, col);
+          bigtab[at + ((((size_t)mb * nKC + kc) * mbs + mt) * GEMM_KB + ks) * 32 + lane] = (double)elem(row, col);
       }
     btp += gemm_amat_doubles(M, K, GEMM_MB);
     return (int64_t)(big0 + at);
@@ -453,6 +457,7 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
     // columns (c, c + 1), c even, may leave as one double2 when they are neighbours in memory at an even address
     proto.pair = (proto.out_cs == 1 && proto.out_sa % 2 == 0 && proto.out_base % 2 == 0 && proto.out_outer % 2 == 0 &&
                   (proto.out_inner % 2 == 0 || proto.out_inner >= cols)) ? 1 : 0;
+    proto.mbs = gemm_mbs(proto.M, GEMM_MB);
     for (int64_t c0 = 0; c0 < cols; c0 += GEMM_CT) {
       GemmItem it = proto; it.col0 = (int)c0; it.ncols = (int)std::min<int64_t>(GEMM_CT, cols - c0);
       glist[list].push_back(it);
@@ -720,6 +725,7 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
 extern "C" void gh_domain_destroy(gh_domain* d) {
   DeviceGuard guard_(d);
   if (!d) return;
+  for (auto& g : d->graphs) if (g.exec) cudaGraphExecDestroy(g.exec);
   for (auto& p : d->pending) { cudaEventDestroy(p.a); cudaEventDestroy(p.b); }
   for (auto e : d->pool) cudaEventDestroy(e);
   delete d;
@@ -889,6 +895,35 @@ gh_status launch_jac(gh_domain* d, double* g, int ncomp) {
 
 }  // namespace
 
+namespace {
+// Run `body` (kernel launches only) through the CUDA graph slot `kind`: captured on first use and whenever its key changes,
+// then replayed as one launch.  Falls back to plain enqueueing on the legacy default stream, while profiling, or when switched off.
+template <class F>
+gh_status run_graphed(gh_domain* d, int kind, double dt, const void* out, F body) {
+  if (d->opt[GH_OPT_NO_GRAPH] || d->prof || d->stream == nullptr) return body();
+  gh_domain::StepGraph& g = d->graphs[kind];
+  const int oop = d->opt[GH_OPT_RK_OUT_OF_PLACE];
+  if (!g.exec || g.dt != dt || g.ua != d->ua || g.ub != d->ub || g.out != out || g.oop != oop) {
+    if (g.exec) { cudaGraphExecDestroy(g.exec); g.exec = nullptr; }
+    const int64_t l0 = d->launches;
+    GH_CUDA(d, cudaStreamBeginCapture(d->stream, cudaStreamCaptureModeThreadLocal));
+    const gh_status st = body();
+    cudaGraph_t graph = nullptr;
+    const cudaError_t e = cudaStreamEndCapture(d->stream, &graph);
+    g.nlaunch = d->launches - l0; d->launches = l0;
+    if (st != GH_OK) { if (graph) cudaGraphDestroy(graph); return st; }
+    if (e != cudaSuccess) return fail(d, GH_ERR_CUDA, std::string("cudaStreamEndCapture: ") + cudaGetErrorString(e));
+    const cudaError_t ei = cudaGraphInstantiate(&g.exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (ei != cudaSuccess) { g.exec = nullptr; return fail(d, GH_ERR_CUDA, std::string("cudaGraphInstantiate: ") + cudaGetErrorString(ei)); }
+    g.dt = dt; g.ua = d->ua; g.ub = d->ub; g.out = out; g.oop = oop;
+  }
+  GH_CUDA(d, cudaGraphLaunch(g.exec, d->stream));
+  d->launches += g.nlaunch;
+  return GH_OK;
+}
+}  // namespace
+
 // ------------------------------------------------------------------------------------------------------
 // state in / out
 // ------------------------------------------------------------------------------------------------------
@@ -940,7 +975,7 @@ extern "C" gh_status gh_rhs(gh_domain* d, double* dtu, int on_device) {
   DeviceGuard guard_(d);
   if (!d || !dtu) return fail(d, GH_ERR_ARG, "NULL argument");
   if (!d->has_fields) return fail(d, GH_ERR_STATE, "gh_rhs before gh_set_fields");
-  if (on_device) return launch_rhs(d, d->ua, dtu);
+  if (on_device) return run_graphed(d, 2, 0.0, dtu, [&] { return launch_rhs(d, d->ua, dtu); });
   gh_status st = launch_rhs(d, d->ua, d->k);
   if (st != GH_OK) return st;
   GH_CUDA(d, cudaMemcpyAsync(dtu, d->k, (size_t)NCOMP * d->pl.S * sizeof(double), cudaMemcpyDeviceToHost, d->stream));
@@ -1010,7 +1045,7 @@ extern "C" gh_status gh_rk_step(gh_domain* d, double dt) {
   if (!d) return GH_ERR_ARG;
   if (!d->has_fields) return fail(d, GH_ERR_STATE, "gh_rk_step before gh_set_fields");
   if (!std::isfinite(dt)) return fail(d, GH_ERR_ARG, "dt is not finite");
-  gh_status st = rk3_stages(d, dt, false);
+  gh_status st = run_graphed(d, 0, dt, nullptr, [&] { return rk3_stages(d, dt, false); });
   if (st != GH_OK) return st;
   d->t += dt; d->dp_fsal = false;
   return GH_OK;
@@ -1021,7 +1056,7 @@ extern "C" gh_status gh_rk_step_norms(gh_domain* d, double dt, double* out, doub
   if (!d || !out) return fail(d, GH_ERR_ARG, "NULL argument");
   if (!d->has_fields) return fail(d, GH_ERR_STATE, "gh_rk_step_norms before gh_set_fields");
   if (!std::isfinite(dt)) return fail(d, GH_ERR_ARG, "dt is not finite");
-  gh_status st = rk3_stages(d, dt, true);
+  gh_status st = run_graphed(d, 1, dt, nullptr, [&] { return rk3_stages(d, dt, true); });
   if (st != GH_OK) return st;
   d->t += dt; d->dp_fsal = false;
   // d->persub was written by stage 1 and nothing later in the step touches it: one copy and one synchronisation at the end

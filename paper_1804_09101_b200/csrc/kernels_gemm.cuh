@@ -6,7 +6,7 @@
 // Pr_m) and X / Out strided views of the field store (contraction index stride sk, output row stride sa, columns
 // (c / inner) * outer + (c % inner) * cs).  At these sizes the matrices no longer fit shared memory (N = 320: 819 KB;
 // L = 255: 268 MB for all m) and an accumulator for every output row no longer fits the register file, so:
-//   - A is stored in DMMA A-fragment order, blocked [m_block][k_chunk][MB m-tiles][KB k-steps][32 lanes], zero padded: one
+//   - A is stored in DMMA A-fragment order, blocked [m_block][k_chunk][mbs <= MB m-tiles][KB k-steps][32 lanes], zero padded: one
 //     (m_block, k_chunk) tile is ONE contiguous 16 / 32 KB piece, fetched by a single TMA bulk copy (cp.async.bulk, completion
 //     on an mbarrier) into a 3-deep shared-memory ring by one elected thread and shared by the CTA's 8 warps;
 //   - a warp owns 16 columns, walks the M-blocks with MB x 2 accumulator tiles, and streams its X fragments straight from
@@ -29,17 +29,19 @@ struct GemmItem {
   int64_t amat;                  // offset (doubles, even) of the blocked fragment matrix in the table memory
   int32_t in_slot, out_slot;     // -1: the kernel's `in` array; 0..2: slot of the derivative scratch [3][total][S]
   int32_t pair;                  // 1: Out columns are contiguous and 16-byte aligned in pairs (double2 stores)
-  int32_t pad_;
+  int32_t mbs;                   // m-tiles per M-block (<= MB): the m-tiles are spread evenly over the fewest blocks
 };
 
 constexpr int GEMM_TPB = 256, GEMM_KB = 8, GEMM_NST = 3, GEMM_NTW = 2;
 constexpr int GEMM_CT = (GEMM_TPB / 32) * 8 * GEMM_NTW;     // 128 columns per CTA
 __host__ __device__ constexpr size_t gemm_stage_doubles(int MB) { return (size_t)MB * GEMM_KB * 32; }
 __host__ __device__ constexpr size_t gemm_smem_bytes(int MB) { return GEMM_NST * gemm_stage_doubles(MB) * sizeof(double); }
+// m-tiles per M-block for an M-row matrix: the fewest blocks of at most MB m-tiles, evenly filled (20 m-tiles: 10 + 10, not 16 + 4)
+inline int gemm_mbs(int M, int MB) { const int MT = (M + 7) / 8, nMB = (MT + MB - 1) / MB; return (MT + nMB - 1) / nMB; }
 // doubles of the blocked fragment matrix for an (M x K) matrix
 inline size_t gemm_amat_doubles(int M, int K, int MB) {
-  const int MT = (M + 7) / 8, KS = (K + 3) / 4;
-  return (size_t)((MT + MB - 1) / MB) * ((KS + GEMM_KB - 1) / GEMM_KB) * gemm_stage_doubles(MB);
+  const int MT = (M + 7) / 8, KS = (K + 3) / 4, mbs = gemm_mbs(M, MB);
+  return (size_t)((MT + mbs - 1) / mbs) * ((KS + GEMM_KB - 1) / GEMM_KB) * gemm_stage_doubles(mbs);
 }
 
 __device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
@@ -69,14 +71,15 @@ template <int MB>
 __global__ void __launch_bounds__(GEMM_TPB, 1)
 k_gemm(const GemmItem* __restrict__ items, const double* __restrict__ tables, const double* in, double* dub, int64_t S,
        int ncomp, CompMap cm) {
-  extern __shared__ __align__(128) double sm[];     // GEMM_NST stages of MB x KB fragments
+  extern __shared__ __align__(16) double sm[];      // GEMM_NST stages of MB x KB fragments (bulk copies need 16-byte alignment)
   __shared__ __align__(8) uint64_t full[GEMM_NST];
   constexpr int KB = GEMM_KB, NST = GEMM_NST, NTW = GEMM_NTW;
-  constexpr int STAGE = MB * KB * 32;
+  constexpr int STAGE_MAX = MB * KB * 32;
   const GemmItem it = items[blockIdx.x];
+  const int mbs = it.mbs, STAGE = mbs * KB * 32;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, tl = lane & 3;
   const int MT = (it.M + 7) >> 3, KS = (it.K + 3) >> 2;
-  const int nMB = (MT + MB - 1) / MB, nKC = (KS + KB - 1) / KB;
+  const int nMB = (MT + mbs - 1) / mbs, nKC = (KS + KB - 1) / KB;
   // components this CTA walks over: blockIdx.y, + gridDim.y, ...
   const int ncw = (ncomp - (int)blockIdx.y + (int)gridDim.y - 1) / (int)gridDim.y;
   const int per = nMB * nKC, total = ncw * per;
@@ -91,7 +94,7 @@ k_gemm(const GemmItem* __restrict__ items, const double* __restrict__ tables, co
   auto issue = [&](int t) {       // stage t: the (m_block, k_chunk) tile of its position inside the component
     const int r = t % per;
     mbar_expect_tx(&full[t % NST], STAGE * 8);
-    bulk_g2s(sm + (size_t)(t % NST) * STAGE, amat + (size_t)r * STAGE, STAGE * 8, &full[t % NST]);
+    bulk_g2s(sm + (size_t)(t % NST) * STAGE_MAX, amat + (size_t)r * STAGE, STAGE * 8, &full[t % NST]);
   };
   if (tid == 0)
     for (int t = 0; t < NST - 1 && t < total; ++t) issue(t);
@@ -154,8 +157,8 @@ k_gemm(const GemmItem* __restrict__ items, const double* __restrict__ tables, co
     if (t + 1 < total) load_b(t + 1, bn);
     mbar_wait(&full[t % NST], (unsigned)((t / NST) & 1));
     if (active) {
-      const double* __restrict__ a_s = sm + (size_t)(t % NST) * STAGE + lane;
-      const int mtn = min(MB, MT - mb * MB);      // m-tiles of this block that exist (the rest of the tile is zero padding)
+      const double* __restrict__ a_s = sm + (size_t)(t % NST) * STAGE_MAX + lane;
+      const int mtn = min(mbs, MT - mb * mbs);    // m-tiles of this block that exist
 #pragma unroll
       for (int ks = 0; ks < KB; ++ks)
 #pragma unroll
@@ -169,8 +172,8 @@ k_gemm(const GemmItem* __restrict__ items, const double* __restrict__ tables, co
         double* dst = out_ptr(t / per);
 #pragma unroll
         for (int mt = 0; mt < MB; ++mt) {
-          const int a = (mb * MB + mt) * 8 + g;
-          if (a < it.M) {
+          const int a = (mb * mbs + mt) * 8 + g;
+          if (mt < mtn && a < it.M) {
             const int64_t ao = (int64_t)a * it.out_sa;
 #pragma unroll
             for (int n = 0; n < NTW; ++n) {

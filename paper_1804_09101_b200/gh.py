@@ -22,7 +22,7 @@ GH_NCOMP = 50
 GH_NUM_KERNELS = 13
 GH_T_A, GH_T_AA, GH_T_AB, GH_T_ABB = range(4)
 GH_FILTER_NONE, GH_FILTER_HEAVISIDE, GH_FILTER_EXP = range(3)
-GH_OPT_RK_OUT_OF_PLACE = 0
+GH_OPT_RK_OUT_OF_PLACE, GH_OPT_NO_GRAPH = 0, 1
 GH_OK, GH_ERR_ARG, GH_ERR_WORKSPACE, GH_ERR_CUDA, GH_ERR_STATE, GH_ERR_SINGULAR = range(6)
 STATUS_NAMES = ["GH_OK", "GH_ERR_ARG", "GH_ERR_WORKSPACE", "GH_ERR_CUDA", "GH_ERR_STATE", "GH_ERR_SINGULAR"]
 
@@ -332,8 +332,29 @@ def gh_basis_shell(L: int):
 
 
 # ---- convenience wrapper -------------------------------------------------------------------------
+def _ordered(fn):
+    """Stream plumbing of a Domain method: the library works on the domain's own stream, torch on its current one; make each see
+    what the other enqueued before (two event waits, no host synchronisation)."""
+    import functools
+
+    @functools.wraps(fn)
+    def wrapper(self, *a, **kw):
+        cur = self.torch.cuda.current_stream(self.device)
+        if cur != self.stream:
+            self.stream.wait_stream(cur)
+        try:
+            return fn(self, *a, **kw)
+        finally:
+            if cur != self.stream:
+                cur.wait_stream(self.stream)
+    return wrapper
+
+
 class Domain:
-    """Owns the device workspace (a torch uint8 tensor) and the gh_domain handle."""
+    """Owns the device workspace (a torch uint8 tensor), the CUDA stream the library works on and the gh_domain handle.
+
+    stream: a torch.cuda.Stream, or None for a stream of the domain's own (not torch's default stream: the legacy default stream
+    cannot be captured into a CUDA graph, and the library replays each step as one graph launch)."""
 
     def __init__(self, descs, device: str = "cuda:0", stream=None):
         import torch
@@ -347,7 +368,8 @@ class Domain:
         base = self.workspace.data_ptr()
         aligned = (base + 255) // 256 * 256
         with torch.cuda.device(self.device):
-            self.stream = stream if stream is not None else torch.cuda.current_stream()
+            self.stream = stream if stream is not None else torch.cuda.Stream(device=self.device)
+            self.stream.wait_stream(torch.cuda.current_stream(self.device))
             self.h = gh_domain_create(self.descs, aligned, nbytes, self.stream.cuda_stream)
         self.P, self.S, self.offsets = gh_domain_layout(self.h, self.n_sub)
         self.sizes = [self._npts(d) for d in self.descs]
@@ -360,6 +382,7 @@ class Domain:
 
     def close(self):
         if getattr(self, "h", None) is not None:
+            self.stream.synchronize()
             gh_domain_destroy(self.h)
             self.h = None
 
@@ -389,36 +412,45 @@ class Domain:
     def empty(self, *lead):
         return self.torch.empty(*lead, self.S, dtype=self.torch.float64, device=self.device)
 
+    @_ordered
     def set_fields(self, u, t: float = 0.0):
         gh_set_fields(self.h, u, t)
 
+    @_ordered
     def get_fields(self, out=None):
         out = np.zeros((GH_NCOMP, self.S)) if out is None else out
         gh_get_fields(self.h, out)
         return out
 
+    @_ordered
     def set_gauge_source(self, H, dH=None):
         gh_set_gauge_source(self.h, H, dH)
 
+    @_ordered
     def rhs(self, out=None):
         out = np.zeros((GH_NCOMP, self.S)) if out is None else out
         gh_rhs(self.h, out)
         return out
 
+    @_ordered
     def gradient(self, out=None):
         out = np.zeros((3, GH_NCOMP, self.S)) if out is None else out
         gh_gradient(self.h, out)
         return out
 
+    @_ordered
     def rk_step(self, dt: float):
         gh_rk_step(self.h, dt)
 
+    @_ordered
     def rk_step_norms(self, dt: float, per_sub: bool = False):
         return gh_rk_step_norms(self.h, dt, self.n_sub, per_sub)
 
+    @_ordered
     def constraint_norms(self, per_sub: bool = False):
         return gh_constraint_norms(self.h, self.n_sub, per_sub)
 
+    @_ordered
     def dp5_attach(self):
         """Allocate (torch) and attach the workspace of the Dormand-Prince stepper."""
         import torch
@@ -427,26 +459,33 @@ class Domain:
         self._dp_ws = torch.empty(n + 256, dtype=torch.uint8, device=self.device)
         gh_dp5_attach(self.h, (self._dp_ws.data_ptr() + 255) // 256 * 256, n)
 
+    @_ordered
     def dp5_step(self, dt: float, tol: float = 0.0):
         return gh_dp5_step(self.h, dt, tol)
 
+    @_ordered
     def set_filter(self, block_axes=None, shell_angular=None):
         gh_set_filter(self.h, block_axes, shell_angular)
 
+    @_ordered
     def apply_filter(self):
         gh_apply_filter(self.h)
 
+    @_ordered
     def set_jacobian(self, J):
         gh_set_jacobian(self.h, J)
 
+    @_ordered
     def spatial_coord_jac(self, structure: int, T, out=None):
         out = (np.empty_like(T) if isinstance(T, np.ndarray) else self.torch.empty_like(T)) if out is None else out
         gh_spatial_coord_jac(self.h, structure, T, out)
         return out
 
+    @_ordered
     def spatial_coord_jac_state(self):
         gh_spatial_coord_jac_state(self.h)
 
+    @_ordered
     def fp64_peak(self):
         return gh_fp64_peak(self.h)
 

@@ -110,3 +110,125 @@ def test_limits_and_rejections():
         dom.set_filter(block_axes={"kind": "exp", "alpha": 36.0, "p": 6})
     assert e.value.status == gh.GH_ERR_ARG
     dom.close()
+
+
+# ---- the sweep's large members at FULL size, on sampled outputs the oracle computes one by one --------------------------------
+def _full(t10):
+    """packed symmetric [10, ...] -> full [4, 4, ...]"""
+    return np.array([[t10[inputs.SYM_PAIRS.index((min(a, b), max(a, b)))] for b in range(4)] for a in range(4)])
+
+
+def _sampled_member(oracle, cfg, n_pts=48, comps=(0, 5, 13, 24, 37, 49)):
+    """One sweep member at full size in the launch configuration bench.py --workload c5 times.  (1) The spectral Cartesian gradient
+    against the oracle on sampled planes (shell: the Y_lm double sums of whole (theta,phi) planes, O2) and sampled lines (the modal
+    Chebyshev derivative, O1), assembled with Eq. 8 at the sampled points.  (2) gh_rhs at sampled points against the oracle's
+    pointwise RHS (O5) fed with the state and the library's own gradient there (the pointwise algebra at full size; the
+    gradient itself is what (1) checks).  The gauge source's gradient is supplied to both sides (complex-step analytic)."""
+    import torch
+    from concurrent.futures import ThreadPoolExecutor
+
+    d = cfg["descs"][0]
+    dom = gh.Domain([d])
+    P, S = dom.P, dom.S
+    xyz = np.zeros((3, S)); gh.gh_domain_coords(dom.h, xyz)
+    u = np.zeros((50, S)); H = np.zeros((4, S)); dH = np.zeros((12, S))
+    inputs.initial_data_chunked(d, xyz[:, :P], cfg["spin"], cfg["amplitude"], cfg["id"], 0, u[:, :P], H[:, :P])
+    hstep = 1e-30
+    for p0 in range(0, P, 1 << 20):                     # d_i H_a analytically (complex step), chunked
+        sl = slice(p0, min(P, p0 + (1 << 20)))
+        for i in range(3):
+            z = xyz[:, sl].astype(complex); z[i] += 1j * hstep
+            dH[4 * i:4 * i + 4, sl] = np.imag(inputs.kerr_schild_gauge_source(z, 1.0, cfg["spin"])) / hstep
+    dom.set_gauge_source(H, dH)
+    dom.set_fields(u, 0.0)
+    g = dom.empty(3, 50)
+    dom.gradient(g)
+    k = dom.empty(50)
+    dom.rhs(k)
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(99)
+    n0, n1, n2 = (d["n"][0], d["n"][1] + 1, 2 * d["n"][1] + 2) if d["kind"] == "shell" else d["n"]
+    scale_u = float(np.abs(u).max())
+    worst = 0.0
+    if d["kind"] == "shell":
+        L = d["n"][1]
+        th, _ = oracle.gl_nodes(L)
+        lo, hi = d["lo"][0], d["hi"][0]
+        xr = oracle.cheb_nodes(n0)
+        planes = [0, n0 // 2]
+        jk = [(int(j), int(kk)) for j, kk in zip(rng.integers(0, n1, n_pts), rng.integers(0, n2, n_pts))]
+        with ThreadPoolExecutor(8) as ex:                # the oracle's plane transform releases the GIL (ctypes)
+            ang = list(ex.map(lambda a: oracle.shell_angular(L, u[a[1], :P].reshape(n0, n1, n2)[a[0]]), [(i, c) for i in planes for c in comps]))
+        it = iter(ang)
+        for i in planes:
+            r = lo + (hi - lo) * (xr[i] + 1) / 2
+            for c in comps:
+                dth, dph = next(it)
+                uc = u[c, :P].reshape(n0, n1, n2)
+                gg = g[:, c, :P].reshape(3, n0, n1, n2)[:, i].cpu().numpy()
+                for j, kk in jk:
+                    dr = oracle.cheb_derivative_line(np.ascontiguousarray(uc[:, j, kk]))[i] * 2 / (hi - lo)
+                    st, ct, ph = np.sin(th[j]), np.cos(th[j]), 2 * np.pi * kk / n2
+                    cp, sp = np.cos(ph), np.sin(ph)
+                    ref = np.array([st * cp * dr + ct * cp / r * dth[j, kk] - sp / (r * st) * dph[j, kk],
+                                    st * sp * dr + ct * sp / r * dth[j, kk] + cp / (r * st) * dph[j, kk],
+                                    ct * dr - st / r * dth[j, kk]])
+                    err = np.abs(gg[:, j, kk] - ref).max()
+                    sc = max(scale_u, np.abs(ref).max())
+                    worst = max(worst, err / sc)
+                    assert err <= TOL * sc, f"{d['n']} plane {i} comp {c} point ({j},{kk}): {err:.3e} > {TOL:g} * {sc:.3e}"
+    else:
+        strides = (n1 * n2, n2, 1)
+        for axis in range(3):
+            for _ in range(n_pts // 3):
+                idx = [int(rng.integers(0, n)) for n in (n0, n1, n2)]
+                idx[axis] = 0
+                base = idx[0] * strides[0] + idx[1] * strides[1] + idx[2] * strides[2]
+                line = base + np.arange(d["n"][axis]) * strides[axis]
+                for c in comps:
+                    ref = oracle.cheb_derivative_line(np.ascontiguousarray(u[c, line])) * 2 / (d["hi"][axis] - d["lo"][axis])
+                    got = g[axis, c, torch.from_numpy(line).cuda()].cpu().numpy()
+                    err = np.abs(got - ref).max()
+                    sc = max(scale_u, np.abs(ref).max())
+                    worst = max(worst, err / sc)
+                    assert err <= TOL * sc, f"{d['n']} axis {axis} comp {c}: {err:.3e} > {TOL:g} * {sc:.3e}"
+    # (2) pointwise RHS at sampled points
+    pts = rng.integers(0, P, 64)
+    gs = g[:, :, torch.from_numpy(pts).cuda()].cpu().numpy()        # [3, 50, n]
+    ks = k[:, torch.from_numpy(pts).cuda()].cpu().numpy()
+    frozen = np.zeros(len(pts), bool)
+    i0 = pts // (n1 * n2)
+    if d["kind"] == "shell":
+        frozen = ((i0 == 0) & (d["face"][0] == 1)) | ((i0 == n0 - 1) & (d["face"][1] == 1))
+    for q, p in enumerate(pts):
+        psi, Pi = _full(u[0:10, p]), _full(u[10:20, p])
+        Phi = np.array([_full(u[20 + 10 * i:30 + 10 * i, p]) for i in range(3)])
+        dpsi = np.array([_full(gs[kk, 0:10, q]) for kk in range(3)])
+        dPi = np.array([_full(gs[kk, 10:20, q]) for kk in range(3)])
+        dPhi = np.array([[_full(gs[kk, 20 + 10 * i:30 + 10 * i, q]) for i in range(3)] for kk in range(3)])
+        o = oracle.rhs_point(psi, Pi, Phi, dpsi, dPi, dPhi, H[:, p], dH[:, p].reshape(3, 4), d["gamma"])
+        ref = inputs.pack_fields(o[0][..., None], o[1][..., None], o[2][..., None])[:, 0]
+        if frozen[q]:
+            ref = np.zeros(50)
+        err = np.abs(ks[:, q] - ref).max()
+        sc = max(scale_u, np.abs(ref).max())
+        assert err <= TOL * sc, f"{d['n']} rhs at point {p}: {err:.3e} > {TOL:g} * {sc:.3e}"
+    dom.close()
+    return worst
+
+
+def test_c5_members_full_size_sampled(oracle):
+    """c5_shell(128) (4.2 M points, L = 127) and c5_block(160) (4.1 M points): the two members in the middle of the sweep's large range."""
+    for cfg in (configs.c5_shell(128), configs.c5_block(160)):
+        _sampled_member(oracle, cfg)
+
+
+import os
+
+
+@pytest.mark.skipif(not os.environ.get("GH_LONG_TESTS"), reason="the 3.3e7-point members: ~15 minutes of input generation and oracle planes; set GH_LONG_TESTS=1")
+def test_c5_top_members_full_size_sampled(oracle):
+    """The top of BASELINE.json configs[4]: c5_shell(256) (L = 255, 3.36e7 points) and c5_block(320) (3.28e7 points)."""
+    for cfg in (configs.c5_shell(256), configs.c5_block(320)):
+        w = _sampled_member(oracle, cfg, n_pts=24, comps=(0, 13, 37))
+        print(f"{cfg['descs'][0]['n']}: worst gradient gap / scale = {w:.3e}")
