@@ -15,6 +15,7 @@
 #include "basis.h"
 #include "device_types.h"
 #include "kernels_deriv.cuh"
+#include "kernels_ang.cuh"
 #include "kernels_point.cuh"
 #include "kernels_jac.cuh"
 #include "kernels_gemm.cuh"
@@ -34,7 +35,7 @@ inline int cheb_class(int N) { return N <= 24 ? 0 : N <= 32 ? 1 : N <= 48 ? 2 : 
 inline int cheb_ct(int) { return CHEB_CT; }
 inline size_t cheb_frag_doubles(int N) { return (size_t)((N + 7) / 8) * ((N + 3) / 4) * 32; }   // D in fragment order
 constexpr int ANG_TPB0 = 256, ANG_TPB1 = 512;    // K_ang threads: class 0 (two CTAs per SM), class 1 (one CTA per SM)
-constexpr size_t ANG_SMEM_2CTA = 113 * 1024;     // K_ang shared memory that still lets two CTAs share an SM
+constexpr size_t ANG_SMEM_2CTA = (GH_ANG_CTAS == 2 ? 113 : GH_ANG_CTAS == 3 ? 74 : 55) * 1024;     // K_ang shared memory that still lets GH_ANG_CTAS CTAs share an SM
 constexpr int ANG_NB_MAX = 8;                    // planes per K_ang CTA offered to the plan (S2 then has <= 2 column tiles per m)
 constexpr int ANG_NB_MAX_SMALL_L = 24;           // ... for L < 12, where a plane is a few tiles only (SingleBH k = 0: 5.96 -> 4.91 ms
                                                  // per 2e6 points; for L >= 12 more than 8 planes measured slightly slower on C4)
@@ -80,47 +81,43 @@ inline void sub_dims(const gh_subdomain_desc& d, int& n0, int& n1, int& n2) {
   else { n0 = d.n[0]; n1 = d.n[1]; n2 = d.n[2]; }
 }
 
-// K_ang shared memory for nb planes of band limit L: X and Y ([nb][plane stride]) + F ([n_phi rounded to 8][pitch])
-// n-chunks per m-tile that minimise (rounds over the warps) x (DMMAs per unit + fixed cost); w = DMMAs per n-tile and k-step
-inline int ang_best_nch(int NT, int MT1, int NW, int w, int per_max) {
+// n-chunks per m-tile of K_ang S3 that minimise (rounds over the warps) x (DMMAs per unit + fixed cost); at most 3 n-tiles per unit
+inline int ang_best_nch3(int NT3, int MT1, int NW) {
   int best = 0; double bc = 1e300;
-  for (int nch = (NT + per_max - 1) / per_max; nch <= NT; ++nch) {
-    const int per = (NT + nch - 1) / nch;
-    if ((NT + per - 1) / per != nch) continue;          // same chunking the kernel derives from nch
-    const double cost = (double)((MT1 * nch + NW - 1) / NW) * (w * per + 0.6);
+  for (int nch = (NT3 + 2) / 3; nch <= NT3; ++nch) {
+    const int per = (NT3 + nch - 1) / nch;
+    if ((NT3 + per - 1) / per != nch) continue;          // same chunking the kernel derives from nch
+    const double cost = (double)((MT1 * nch + NW - 1) / NW) * (4 * per + 0.6);
     if (cost < bc) { bc = cost; best = nch; }
   }
   return best;
 }
 // Modelled duration of one K_ang CTA (units: one DMMA slot of a warp) for `np_` planes of band limit L on NW warps: per stage
-// the number of rounds the warps need times the DMMAs of one unit, plus a fixed part for staging and barriers.  Used only
-// to choose the planes per CTA and the CTA class of a shell; the S1 / S3 chunkings are the ones the kernel will use.
+// the number of rounds the warps need times the DMMAs of one unit (the k-steps and tiles the kernel really runs), plus a fixed
+// part for staging and barriers.  Used only to choose the planes per CTA and the CTA class of a shell.
 constexpr double ANG_FIX = 40.0;     // fixed part of a CTA (staging, barriers), in DMMA slots; 10-300 measured, flat optimum near 40
-constexpr double ANG_C0W = 2.0;      // class 0 runs two CTAs per SM
+constexpr double ANG_C0W = (double)GH_ANG_CTAS;      // class 0 runs GH_ANG_CTAS CTAs per SM
 inline double ang_cta_cost(int L, int np_, int NW) {
-  const AngDims D = ang_dims(L);
-  const int nt = L + 1, MT1 = (np_ * nt + 7) / 8;
-  const int nche = ang_best_nch(D.NTc, MT1, NW, 1, ANG_NTC), ncho = ang_best_nch(D.NTs, MT1, NW, 1, ANG_NTC);
-  const int nch3 = ang_best_nch(D.NT3, MT1, NW, 4, ANG_NTC3);
-  const int pere = (D.NTc + nche - 1) / nche, pero = (D.NTs + ncho - 1) / ncho, per3 = (D.NT3 + nch3 - 1) / nch3;
-  const double c1 = (double)((MT1 * (nche + ncho) + NW - 1) / NW) * std::max(D.KSe1 * pere, D.KSo1 * pero);
-  const int hh = (nt + 1) / 2, MTH = (2 * hh + 7) / 8, KSh = (hh + 3) / 4, NTn = (2 * np_ + 7) / 8;
-  const int units2 = (L + 1) * NTn - ((NTn == 2 && np_ <= 8) ? 1 : 0);
-  const double c2 = (double)((units2 + NW - 1) / NW) * (KSh * 2 * MTH);
-  const double c3 = (double)((MT1 * nch3 + NW - 1) / NW) * ((D.KSe3 + D.KSo3) * per3 * 2);
+  const int NT = ang_nt_class(L), nt = L + 1, h = nt, MT1 = (np_ * nt + 7) / 8;
+  const int KSe1 = (h + 1 + 3) / 4, KSo1 = (L + 3) / 4, KSe3 = (h + 3) / 4, KSo3 = (L + 3) / 4, nt3 = (h + 1 + 7) / 8;
+  // S1: units (m-tile, parity) alternate over the warps: NW / 2 warps per parity
+  const double c1 = (double)((MT1 + NW / 2 - 1) / (NW / 2)) * std::max(KSe1, KSo1) * NT;
+  const int hh = (nt + 1) / 2, MTn = (2 * hh + 7) / 8, KSh = (hh + 3) / 4, ntn = (2 * np_ + 7) / 8, NTN = c_ntn(NT);
+  const int nchunk = (ntn + NTN - 1) / NTN;
+  const double c2 = (double)(((L + 1) * nchunk + NW - 1) / NW) * (KSh * 2 * MTn * std::min(NTN, ntn));
+  const int nch3 = ang_best_nch3(nt3, MT1, NW), per3 = (nt3 + nch3 - 1) / nch3;
+  const double c3 = (double)((MT1 * nch3 + NW - 1) / NW) * ((KSe3 + KSo3) * per3 * 2);
   return c1 + c2 + c3 + ANG_FIX;
 }
 inline size_t ang_smem_bytes(int L, int nb) { return ang_smem_doubles(L, nb) * sizeof(double); }
 inline size_t shell_fa_doubles(int L) { return ang_fa_doubles(L); }   // (even | odd) analysis fragments
 inline size_t shell_fs_doubles(int L) { return ang_fs_doubles(L); }   // (even | odd) synthesis fragments
-inline size_t shell_t_doubles(int L) {    // [m][k_step][even|odd][m_tile][32]: the equator-folded stacked matrices of K_ang S2
-  const size_t nt = L + 1, hh = (nt + 1) / 2, mth = (2 * hh + 7) / 8, ksh = (hh + 3) / 4;
-  return (size_t)(L + 1) * ksh * 2 * mth * 32;
+inline size_t shell_t_doubles(int L) {    // [m][k_step < NT][even|odd][m_tile < NT][32]: the equator-folded stacked matrices of K_ang S2
+  return (size_t)(L + 1) * c_tm(ang_nt_class(L));
 }
 inline size_t shell_matrix_doubles(int L) { return shell_fa_doubles(L) + shell_fs_doubles(L) + shell_t_doubles(L); }
-inline size_t shell_g_doubles(int L) {    // [m][k_step][even|odd][m_tile][32]: equator-folded filtered projectors (hh rows)
-  const size_t nt = L + 1, hh = (nt + 1) / 2, mtf = (hh + 7) / 8, ksh = (hh + 3) / 4;
-  return (size_t)(L + 1) * ksh * 2 * mtf * 32;
+inline size_t shell_g_doubles(int L) {    // [m][k_step < NT][even|odd][m_tile < ceil(NT/2)][32]: equator-folded filtered projectors (hh rows)
+  return (size_t)(L + 1) * c_gm(ang_nt_class(L));
 }
 
 bool validate(const gh_subdomain_desc* descs, int32_t n_sub, std::string& err) {
@@ -607,39 +604,40 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
           //   even analysis  B[k = 0..h][m = 0..L]      = Fa[m][k]            (cos rows; the weight of k and np-k is the same)
           //   odd  analysis  B[k' = k-1, k = 1..L][m' = m-1, m = 1..L] = Fa[L+m][k]   (sin rows)
           // fragment (k_step, n_tile): element (K index 4 ks + t, N index 8 n + g)
-          const AngDims dm = ang_dims(L);
-          const int h = dm.h;
+          // all dimensions are those of the shell's class NT = ceil(h / 8) (compile-time constants of K_ang), zero padded
+          const int NT = ang_nt_class(L), h = nt;
           std::vector<ghb::ld> FA(shell_fa_doubles(L), 0);
-          for (int ks = 0; ks < dm.KSe1; ++ks) for (int n = 0; n < dm.NTc; ++n) for (int lane = 0; lane < 32; ++lane) {
+          for (int ks = 0; ks < c_kse1(NT); ++ks) for (int n = 0; n < NT; ++n) for (int lane = 0; lane < 32; ++lane) {
             const int k = ks * 4 + lane % 4, m = n * 8 + lane / 4;
             // the kernel forms U_k + U_{np-k} for every k: k = h is its own mirror, so its weight is halved
-            if (k <= h && m <= L) FA[((size_t)ks * dm.NTc + n) * 32 + lane] = (k == h ? (ghb::ld)0.5 : (ghb::ld)1) * B.Fa[(size_t)m * np + k];
+            if (k <= h && m <= L) FA[((size_t)ks * NT + n) * 32 + lane] = (k == h ? (ghb::ld)0.5 : (ghb::ld)1) * B.Fa[(size_t)m * np + k];
           }
-          const size_t fao = (size_t)dm.KSe1 * dm.NTc * 32;
-          for (int ks = 0; ks < dm.KSo1; ++ks) for (int n = 0; n < dm.NTs; ++n) for (int lane = 0; lane < 32; ++lane) {
+          const size_t fao = (size_t)c_fa_e(NT);
+          for (int ks = 0; ks < c_kso1(NT); ++ks) for (int n = 0; n < NT; ++n) for (int lane = 0; lane < 32; ++lane) {
             const int k = ks * 4 + lane % 4 + 1, m = n * 8 + lane / 4 + 1;
-            if (k <= L && m <= L) FA[fao + ((size_t)ks * dm.NTs + n) * 32 + lane] = B.Fa[(size_t)(L + m) * np + k];
+            if (k <= L && m <= L) FA[fao + ((size_t)ks * NT + n) * 32 + lane] = B.Fa[(size_t)(L + m) * np + k];
           }
           o.Fa = put(FA);
           //   even synthesis B[m = 0..L][k = 0..h] = Fs[k][m];   odd synthesis B[m' = m-1][k = 0..h] = Fs[k][L+m], zero at k = 0, h
           std::vector<ghb::ld> FS(shell_fs_doubles(L), 0);
-          for (int ks = 0; ks < dm.KSe3; ++ks) for (int n = 0; n < dm.NT3; ++n) for (int lane = 0; lane < 32; ++lane) {
+          const int NT3 = c_nt3(NT);
+          for (int ks = 0; ks < c_ks3(NT); ++ks) for (int n = 0; n < NT3; ++n) for (int lane = 0; lane < 32; ++lane) {
             const int m = ks * 4 + lane % 4, k = n * 8 + lane / 4;
-            if (m <= L && k <= h) FS[((size_t)ks * dm.NT3 + n) * 32 + lane] = B.Fs[(size_t)k * nq + m];
+            if (m <= L && k <= h) FS[((size_t)ks * NT3 + n) * 32 + lane] = B.Fs[(size_t)k * nq + m];
           }
-          const size_t fso = (size_t)dm.KSe3 * dm.NT3 * 32;
-          for (int ks = 0; ks < dm.KSo3; ++ks) for (int n = 0; n < dm.NT3; ++n) for (int lane = 0; lane < 32; ++lane) {
+          const size_t fso = (size_t)c_fs_e(NT);
+          for (int ks = 0; ks < c_ks3(NT); ++ks) for (int n = 0; n < NT3; ++n) for (int lane = 0; lane < 32; ++lane) {
             const int m = ks * 4 + lane % 4 + 1, k = n * 8 + lane / 4;
-            if (m <= L && k >= 1 && k < h) FS[fso + ((size_t)ks * dm.NT3 + n) * 32 + lane] = B.Fs[(size_t)k * nq + L + m];
+            if (m <= L && k >= 1 && k < h) FS[fso + ((size_t)ks * NT3 + n) * 32 + lane] = B.Fs[(size_t)k * nq + L + m];
           }
           o.Fs = put(FS);
           // S2 A operands, folded about the equator (jbar = nt-1-j; K_ang S2 forms p_j = C_j + C_jbar, q_j = C_j - C_jbar, j < hh):
           //   ME (acts on p) = 1/2 (M[r][j] + M[r][jbar]),  MO (acts on q) = 1/2 (M[r][j] - M[r][jbar]),  r, j < hh,
           //   M = Th_m for stacked rows [0, hh) and m Pr_m for rows [hh, 2 hh); the equator node (j = jbar, odd nt) has
           //   p = 2 C_j, q = 0: its ME column is 1/2 M[r][j].   element (row = 8 mt + g, col = 4 ks + t)
-          const int hh = (nt + 1) / 2, mth = (2 * hh + 7) / 8, ksh = (hh + 3) / 4;
+          const int hh = (nt + 1) / 2;
           std::vector<ghb::ld> T(shell_t_doubles(L), 0);
-          for (int m = 0; m <= L; ++m) for (int ks = 0; ks < ksh; ++ks) for (int w = 0; w < 2; ++w) for (int mt = 0; mt < mth; ++mt)
+          for (int m = 0; m <= L; ++m) for (int ks = 0; ks < NT; ++ks) for (int w = 0; w < 2; ++w) for (int mt = 0; mt < NT; ++mt)
             for (int lane = 0; lane < 32; ++lane) {
               const int row = mt * 8 + lane / 4, j = ks * 4 + lane % 4;
               ghb::ld v = 0;
@@ -651,7 +649,7 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
                 if (jb == j) v = w == 0 ? f * a / 2 : (ghb::ld)0;
                 else v = f * (w == 0 ? a + c : a - c) / 2;
               }
-              T[((((size_t)m * ksh + ks) * 2 + w) * mth + mt) * 32 + lane] = v;
+              T[((((size_t)m * NT + ks) * 2 + w) * NT + mt) * 32 + lane] = v;
             }
           o.T = put(T);
         }
@@ -666,10 +664,7 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
         it.m_Fa = o.Fa; it.m_Fs = o.Fs; it.m_T = o.T; it.m_G = (int)d->f_L[L];
         {
           const int NW = (pl.ang_class[s] ? ANG_TPB1 : ANG_TPB0) / 32, MT1 = (it.nplanes * (L + 1) + 7) / 8;
-          const AngDims dm = ang_dims(L);
-          it.nch1e = (int8_t)ang_best_nch(dm.NTc, MT1, NW, 1, ANG_NTC);
-          it.nch1o = (int8_t)ang_best_nch(dm.NTs, MT1, NW, 1, ANG_NTC);
-          it.nch3 = (int8_t)ang_best_nch(dm.NT3, MT1, NW, 4, ANG_NTC3);
+          it.nch3 = (int8_t)ang_best_nch3((L + 1 + 1 + 7) / 8, MT1, NW);
         }
         (pl.ang_class[s] ? ang1 : ang).push_back(it);
       }
@@ -1148,11 +1143,12 @@ extern "C" gh_status gh_set_filter(gh_domain* d, const gh_filter_desc* fb, const
   }
   if (on_s) {
     for (const auto& kv : d->f_L) {
-      const int L = kv.first, nt = L + 1, hh = (nt + 1) / 2, mtf = (hh + 7) / 8, ksh = (hh + 3) / 4;
+      const int L = kv.first, nt = L + 1, hh = (nt + 1) / 2, NT = ang_nt_class(L), mtf = c_mtf(NT);
       if (!filter_sigma(fs, L, sg)) return fail(d, GH_ERR_ARG, "bad shell filter descriptor");
       ghb::shell_filter_composites(L, sg, M);
-      // folded about the equator exactly like the projector rows of K_ang S2: ME = (G[r][j] + G[r][jbar]) / 2, MO = (.. - ..) / 2
-      for (int m = 0; m <= L; ++m) for (int ks = 0; ks < ksh; ++ks) for (int w = 0; w < 2; ++w) for (int mt = 0; mt < mtf; ++mt)
+      // folded about the equator exactly like the projector rows of K_ang S2: ME = (G[r][j] + G[r][jbar]) / 2, MO = (.. - ..) / 2;
+      // laid out for the shell's class: [m][ks < NT][p | q][mt < ceil(NT/2)][32], zero padded
+      for (int m = 0; m <= L; ++m) for (int ks = 0; ks < NT; ++ks) for (int w = 0; w < 2; ++w) for (int mt = 0; mt < mtf; ++mt)
         for (int lane = 0; lane < 32; ++lane) {
           const int r = mt * 8 + lane / 4, j = ks * 4 + lane % 4;
           ghb::ld v = 0;
@@ -1162,7 +1158,7 @@ extern "C" gh_status gh_set_filter(gh_domain* d, const gh_filter_desc* fb, const
             if (jb == j) v = w == 0 ? a / 2 : (ghb::ld)0;
             else v = (w == 0 ? a + c : a - c) / 2;
           }
-          ft[kv.second - base + ((((size_t)m * ksh + ks) * 2 + w) * mtf + mt) * 32 + lane] = (double)v;
+          ft[kv.second - base + ((((size_t)m * NT + ks) * 2 + w) * mtf + mt) * 32 + lane] = (double)v;
         }
     }
   }

@@ -549,3 +549,26 @@ def test_nan_reaches_the_reported_maxima(oracle):
     except gh.GHError as e:
         assert e.status == gh.GH_ERR_SINGULAR
     dom.close()
+
+
+def test_repeated_calls_are_bit_identical(oracle):
+    """Shared memory left behind by other kernels must never reach a result (K_ang reads whole k-steps of its coefficient rows,
+    padding columns included): gh_rhs of the same state, called again and again with the filter (other kernels, other shared-memory
+    contents) and other domains in between, gives the same bits every time."""
+    cfg = _wide()
+    descs, coords, us, Hs = build_case(cfg, oracle)
+    dom = _domain(descs, Hs, us)
+    other = gh.Domain(configs.c3()["descs"])
+    rng = np.random.default_rng(3)
+    other.set_fields(rng.standard_normal((50, other.S)) * 1e300, 0.0)      # huge values through the same kernels on the same SMs
+    first = dom.rhs()
+    junk = other.empty(3, 50)
+    for i in range(12):
+        other.gradient(junk)
+        if i % 3 == 0:
+            dom.set_filter(block_axes={"kind": "exp", "alpha": 36.0, "p": 6}, shell_angular={"kind": "exp", "alpha": 36.0, "p": 6})
+            dom.apply_filter()
+            dom.set_filter(None, None)
+            dom.set_fields(dom.pack(us), 0.0)
+        assert np.array_equal(dom.rhs(), first), i
+    other.close(); dom.close()
