@@ -594,7 +594,7 @@ def finish_ours(args, world, label, cfg, descs, reps, P, S, ms, e2e_step_s, e2e_
 # ------------------------------------------------------------------------------------------------------------------
 # the size sweep (BASELINE.json configs[4]): one JSON line per member
 # ------------------------------------------------------------------------------------------------------------------
-def sweep_members(max_points):
+def sweep_members(max_points, paper_members=False):
     from paper_1804_09101_b200 import configs
 
     out = []
@@ -602,6 +602,12 @@ def sweep_members(max_points):
         out.append((f"shell n={n} (N_r={n}, L={n - 1})", configs.c5_shell(n)))
     for N in (10, 20, 40, 80, 160, 320):
         out.append((f"block {N}^3", configs.c5_block(N)))
+    if paper_members:      # the paper's own grid prescriptions for this sweep and its whole-code test shell
+        out.append(("paper test shell (10,19,38)", {**configs.paper_two_shells(), "descs": configs.paper_two_shells()["descs"][:1]}))
+        for k in range(0, 11):
+            out.append((f"SingleBH k={k}", configs.single_bh(k)))
+        for k in range(1, 17):
+            out.append((f"BBH k={k}", configs.bbh(k)))
     return [(lbl, cfg) for lbl, cfg in out if configs.num_points(cfg["descs"][0]) <= max_points]
 
 
@@ -613,7 +619,7 @@ def run_sweep(args, dev):
     from paper_1804_09101_b200 import configs, gh, inputs, opcount
 
     hbm_peak, _ = load_peaks()
-    for label, cfg in sweep_members(args.sweep_max_points):
+    for label, cfg in sweep_members(args.sweep_max_points, args.sweep_paper_members):
         d = cfg["descs"][0]
         dom = gh.Domain([d], device=dev)
         P, S = dom.P, dom.S
@@ -703,6 +709,7 @@ def main():
     ap.add_argument("--profile-steps", type=int, default=10, help="steps of the second (per-launch events on) pass")
     ap.add_argument("--sweep-reps", type=int, default=20, help="c5: repetitions per member")
     ap.add_argument("--sweep-max-points", type=int, default=40_000_000, help="c5: skip members above this size")
+    ap.add_argument("--sweep-paper-members", action="store_true", help="c5: also the paper's SingleBH / BBH shell prescriptions (PAPER.md:436)")
     ap.add_argument("--min-points", type=int, default=4_000_000, help="C4: replicate the base set until P >= this")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--cpu-points", type=int, default=1_300_000,
