@@ -1065,3 +1065,48 @@ int ora_scj_state(int64_t P, const double* J, const double* u, double* out) {
   free(T); free(R);
   return bad;
 }
+
+/* ---------------------------------------------------------------------- */
+/* O12b — spectral interpolation of a face state between shells of         */
+/* different band limit (NEXT-2 (iii) across non-matching grids; "at       */
+/* 'internal' boundaries between neighboring domains, the characteristic   */
+/* variables are computed and used as boundary conditions on the           */
+/* neighboring subdomain"; interpolation "via a direct       */
+/* summation of the spectral series").  One (theta,phi) plane */
+/* on the Gauss-Legendre x uniform grid of band limit Ls:                  */
+/*   a_lm = sum_{j,k} w_j (2 pi/N_phi) conj(Y_lm(theta_j,phi_k)) u_jk,     */
+/*   0 <= l <= Ls (Eq. 23's analysis), then the series is summed at the    */
+/* nodes (theta'_j', phi'_k') of the grid of band limit Ld:                */
+/*   out_j'k' = sum_l [a_l0 Y_l0 + 2 Re sum_{m>0} a_lm Y_lm](theta',phi'). */
+/* Explicit sums; Ls = Ld reduces to the projection of O2.                 */
+/* ---------------------------------------------------------------------- */
+void ora_shell_interp(int Ls, int Ld, const double* u, double* out) {
+  ylm_table* t = ylm_build(Ls);
+  int n = t->nth, nph = t->nph, nd = Ld + 1, npd = 2 * (Ld + 1);
+  real* are = calloc((size_t)n * n, sizeof(real)); real* aim = calloc((size_t)n * n, sizeof(real));
+  real dphi = 2 * R_PI / (real)nph;
+  for (int l = 0; l <= Ls; ++l) for (int m = 0; m <= l; ++m) {
+    real sr = 0, si = 0; const real* pb = t->pb + (int64_t)(l * n + m) * n;
+    for (int j = 0; j < n; ++j) for (int k = 0; k < nph; ++k) {
+      real f = t->w[j] * dphi * pb[j] * (real)u[j * nph + k];
+      sr += f * t->cs[m * nph + k]; si -= f * t->sn[m * nph + k];
+    }
+    are[l * n + m] = sr; aim[l * n + m] = si;
+  }
+  real* ctd = malloc(sizeof(real) * nd); real* wd = malloc(sizeof(real) * nd); gl_nodes(Ld, ctd, wd);
+  real* pb = malloc(sizeof(real) * n * n); real* dpb = malloc(sizeof(real) * n * n);
+  for (int j = 0; j < nd; ++j) {
+    pbar_all(Ls, ctd[j], pb, dpb);      /* Pbar_lm at the destination colatitude, l <= Ls */
+    for (int k = 0; k < npd; ++k) {
+      real s = 0;
+      for (int l = 0; l <= Ls; ++l) for (int m = 0; m <= l; ++m) {
+        int64_t q = ((int64_t)m * k) % npd; real ang = 2 * R_PI * (real)q / (real)npd;
+        real c = R_COS(ang), sn = R_SIN(ang);
+        real re = are[l * n + m] * c - aim[l * n + m] * sn;
+        s += ((m == 0) ? 1 : 2) * pb[l * n + m] * re;
+      }
+      out[j * npd + k] = (double)s;
+    }
+  }
+  free(are); free(aim); free(ctd); free(wd); free(pb); free(dpb); ylm_free(t);
+}

@@ -110,6 +110,7 @@ class Oracle:
         L.ora_char_bc_point.restype = C.c_int
         L.ora_filter_subdomain.argtypes = [C.POINTER(Subdomain), C.c_int, _dp, _dp, _dp, _dp]
         L.ora_filter_subdomain.restype = C.c_int
+        L.ora_shell_interp.argtypes = [C.c_int, C.c_int, _dp, _dp]
         L.ora_scj_point.argtypes = [C.c_int, _dp, _dp, _dp]
         L.ora_scj_point.restype = C.c_double
         L.ora_scj_eq12.argtypes = [C.c_int]
@@ -172,6 +173,17 @@ class Oracle:
         out = np.empty_like(u)
         self.lib.ora_shell_project(L, u, out)
         return out
+
+    def shell_interp(self, Ls: int, Ld: int, u: np.ndarray) -> np.ndarray:
+        """O12b: planes u[..., Ls+1, 2Ls+2] on the grid of band limit Ls -> the same series summed at the nodes of band limit Ld."""
+        u = np.ascontiguousarray(u, dtype=np.float64)
+        lead = u.shape[:-2]
+        assert u.shape[-2:] == (Ls + 1, 2 * Ls + 2)
+        flat = u.reshape(-1, Ls + 1, 2 * Ls + 2)
+        out = np.empty((flat.shape[0], Ld + 1, 2 * Ld + 2))
+        for i in range(flat.shape[0]):
+            self.lib.ora_shell_interp(Ls, Ld, np.ascontiguousarray(flat[i]), out[i])
+        return out.reshape(*lead, Ld + 1, 2 * Ld + 2)
 
     def spectral_filter(self, sd: dict, u: np.ndarray, sigmas) -> np.ndarray:
         """O9: filtered copy of u[ncomp][P].  sigmas: blocks [sigma_x, sigma_y, sigma_z] (one value per Chebyshev mode);

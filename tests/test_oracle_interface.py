@@ -88,3 +88,50 @@ def test_analytic_data_is_continuous_across_the_interface(oracle):
     free = dict(a, face=[0, 0, 0, 0, 0, 0])
     d = oracle.rhs_ifc(a, ua, Ha, nbr_out=ub[:, :pl]) - oracle.rhs(free, ua, Ha)
     assert np.max(np.abs(d)) < 1e-12
+
+
+# ---- O12b: spectral interpolation of a face plane between grids of different band limit ------------------------------------------
+def _nodes(oracle, L):
+    th, _ = oracle.gl_nodes(L)
+    ph = 2 * np.pi * np.arange(2 * L + 2) / (2 * L + 2)
+    return np.meshgrid(th, ph, indexing="ij")
+
+
+def test_interp_band_limited_fields_cross_unchanged(oracle):
+    """A field band-limited to l <= min(Ls, Ld) is the same function on both grids: closed-form real harmonics up to l = 3 (and
+    a seeded combination of them) sampled on the source grid come out as the same closed forms sampled on the destination
+    grid, coarser or finer; Ls = Ld is the projection of O2."""
+    def harmonics(th, ph):
+        x, y, z = np.sin(th) * np.cos(ph), np.sin(th) * np.sin(ph), np.cos(th)
+        return [np.ones_like(x), x, y, z, x * y, y * z, 3 * z * z - 1, x * z, x * x - y * y, x * y * z, z * (5 * z * z - 3), x * (x * x - 3 * y * y)]
+    rng = np.random.default_rng(2)
+    coef = rng.standard_normal(12)
+    for Ls, Ld in ((5, 8), (8, 5), (4, 3), (3, 7), (6, 6)):
+        ths, phs = _nodes(oracle, Ls)
+        thd, phd = _nodes(oracle, Ld)
+        hs, hd = harmonics(ths, phs), harmonics(thd, phd)
+        for a, b in zip(hs, hd):
+            assert np.abs(oracle.shell_interp(Ls, Ld, a) - b).max() < 1e-14 * max(1.0, np.abs(b).max())
+        fs = sum(c * a for c, a in zip(coef, hs)); fd = sum(c * b for c, b in zip(coef, hd))
+        assert np.abs(oracle.shell_interp(Ls, Ld, fs) - fd).max() < 2e-14 * np.abs(fd).max()
+    u = rng.standard_normal((7, 14))
+    assert np.abs(oracle.shell_interp(6, 6, u) - oracle.shell_project(6, u)).max() < 1e-14      # same grid: the projection
+
+
+def test_interp_is_linear_and_drops_nothing_it_can_represent(oracle):
+    """Linearity; coarse -> fine -> coarse is the projection on the coarse grid (the fine grid holds every coarse mode); a mode
+    l = Ls (the highest the source resolves) arrives on a finer grid with its norm, and fine -> coarse of a mode above the
+    coarse band limit is NOT zero at the nodes (the series is summed, not truncated: aliased point values)."""
+    rng = np.random.default_rng(4)
+    u, v = rng.standard_normal((5, 10)), rng.standard_normal((5, 10))
+    a = oracle.shell_interp(4, 7, 2.0 * u - 3.0 * v)
+    assert np.abs(a - (2.0 * oracle.shell_interp(4, 7, u) - 3.0 * oracle.shell_interp(4, 7, v))).max() < 1e-13
+    back = oracle.shell_interp(7, 4, oracle.shell_interp(4, 7, u))
+    assert np.abs(back - oracle.shell_project(4, u)).max() < 1e-13
+    th7, ph7 = _nodes(oracle, 7)
+    z = np.cos(th7)
+    p6 = (231 * z ** 6 - 315 * z ** 4 + 105 * z ** 2 - 5) / 16          # Legendre P_6: l = 6 > 4
+    down = oracle.shell_interp(7, 4, p6)
+    th4, _ = _nodes(oracle, 4)
+    z4 = np.cos(th4)
+    assert np.abs(down - (231 * z4 ** 6 - 315 * z4 ** 4 + 105 * z4 ** 2 - 5) / 16).max() < 1e-13
