@@ -61,8 +61,10 @@ typedef enum { GH_SHELL = 0, GH_BLOCK = 1 } gh_kind;
  * equations give (reading S21 writes the fields and speeds out); fused into the RHS kernel.  At block edges the
  * faces are applied in the order -x,+x,-y,+y,-z,+z; a FROZEN face through the same point wins.
  * INTERFACE (NEXT-2 (iii), shells only): the outer face of shell s and the inner face of shell s+1 (the next descriptor) are
- * one internal boundary: both must carry this flag, and the two shells must share centre, band limit L and the radius
- * (their face grids then coincide point by point).  Every characteristic field that enters a shell through the face is
+ * one internal boundary: both must carry this flag, and the two shells must share centre and the radius.  With the same band
+ * limit L their face grids coincide point by point; with different L (both <= 47) the neighbour's face state is first
+ * interpolated to the own grid by summing its spherical-harmonic series at the own nodes (K_face_interp: analysis on the
+ * neighbour's grid, all its modes l <= L_nbr kept; "interpolation ... via a direct summation of the spectral series").  Every characteristic field that enters a shell through the face is
  * relaxed towards the neighbour's value:  d_t u^a += -p |v_a| (u^a_own - u^a_neighbour),  p = (N_r - 1)^2 / (r_out - r_in)
  * of the own shell (reading S22); outgoing fields are untouched.  Fused into the RHS kernel, which reads the
  * neighbour's face state straight from the field store. */

@@ -172,4 +172,24 @@ void shell_filter_composites(int L, const std::vector<ld>& sigma_l, std::vector<
   }
 }
 
+void shell_interp_composites(int Ls, int Ld, std::vector<ld>& G) {
+  const int ns = Ls + 1, nd = Ld + 1;
+  std::vector<ld> cs, ws, cd, wd, ss(ns), sd(nd);
+  gauss_legendre(Ls, cs, ws); gauss_legendre(Ld, cd, wd);
+  for (int j = 0; j < ns; ++j) ss[j] = sqrtl((1 - cs[j]) * (1 + cs[j]));
+  for (int j = 0; j < nd; ++j) sd[j] = sqrtl((1 - cd[j]) * (1 + cd[j]));
+  G.assign((size_t)(Ls + 1) * nd * ns, 0);
+  std::vector<std::vector<ld>> Ps(ns), Pd(nd);
+  for (int m = 0; m <= Ls; ++m) {
+    for (int j = 0; j < ns; ++j) pbar_column(Ls, m, cs[j], ss[j], Ps[j]);
+    for (int j = 0; j < nd; ++j) pbar_column(Ls, m, cd[j], sd[j], Pd[j]);
+    for (int jo = 0; jo < nd; ++jo)
+      for (int ji = 0; ji < ns; ++ji) {
+        ld sp = 0;
+        for (int l = m; l <= Ls; ++l) sp += Pd[jo][l - m] * Ps[ji][l - m];
+        G[((size_t)m * nd + jo) * ns + ji] = 2 * PI_L * ws[ji] * sp;
+      }
+  }
+}
+
 }  // namespace ghb

@@ -39,4 +39,9 @@ void cheb_filter_matrix(int N, const std::vector<ld>& sigma, std::vector<ld>& F)
 // Per-m filtered projectors on the Gauss-Legendre colatitudes: G[m][j'][j] = 2 pi sum_{l=m}^{L} sigma_l Pbar_lm(j') w_j Pbar_lm(j).
 void shell_filter_composites(int L, const std::vector<ld>& sigma_l, std::vector<ld>& G);
 
+// Face interpolation between shells of different band limit (NEXT-2 (iii) across non-matching grids): per m = 0..Ls the
+// rectangular composite  G[m][j'][j] = 2 pi sum_{l=m}^{Ls} Pbar_lm(theta'_j') w_j Pbar_lm(theta_j)   (j' on the Gauss-Legendre grid
+// of band limit Ld, j on that of Ls): analysis on the source colatitudes, the series summed at the destination ones.
+void shell_interp_composites(int Ls, int Ld, std::vector<ld>& G);
+
 }  // namespace ghb

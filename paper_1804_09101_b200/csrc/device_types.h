@@ -24,6 +24,17 @@ struct SubDev {
   // outer face (-1: none) and the penalty factor (N_r - 1)^2 / (r_out - r_in)
   int64_t nbr[2];
   double pen;
+  // ... when the neighbour has a different band limit its face state is interpolated to this shell's grid first (K_face_interp):
+  // start (inside a component) of that copy in the interface buffer, -1: the grids coincide and nbr[] is used
+  int64_t nbi[2];
+};
+
+// One face plane to interpolate (NEXT-2 (iii) between shells of different L): the neighbour's (theta,phi) plane at src_off of
+// every component of the state -> dst_off of every component of the interface buffer, on this shell's grid.
+struct IfcItem {
+  int64_t src_off, dst_off;
+  int32_t Ls, Ld;
+  int64_t m_FaT, m_GT, m_FxT;   // offsets (doubles) in the table memory: FaT[k][q] (n_phi_s x n_q_s), GT[m][j][j'] (per m: n_theta_s x n_theta_d), FxT[q][k'] (n_q_s x n_phi_d)
 };
 
 // One tile of Chebyshev lines: out[a, col] = sum_i D[a][i] in[i, col] for `ncols` columns (A2, Eq. 22).

@@ -70,10 +70,13 @@ struct Plan {
   int n_gemm[G_NLIST] = {0, 0, 0, 0, 0};  // K_gemm items per launch list (large subdomains)
   size_t bigtab_doubles = 0;             // their blocked fragment matrices, behind the filter tables
   bool has_big = false;
+  int n_ifc_items = 0;                   // interface faces whose neighbour has a different band limit (K_face_interp)
+  int64_t Sf = 0;                        // component stride (doubles) of the interface buffer
+  size_t ifc_smem = 0, ifctab_doubles = 0;
   std::vector<int> ang_pb;               // planes per CTA for each subdomain (0 for blocks)
   std::vector<int> ang_class;            // shared-memory class of each shell
   // workspace offsets (bytes)
-  size_t o_ua, o_ub, o_k, o_du, o_H, o_dH, o_jac, o_tables, o_subs, o_tiles, o_cheb, o_fcheb, o_ang, o_gemm, o_part, o_persub, o_flag, total;
+  size_t o_ua, o_ub, o_k, o_du, o_H, o_dH, o_jac, o_tables, o_subs, o_tiles, o_cheb, o_fcheb, o_ang, o_gemm, o_ifc, o_ifci, o_part, o_persub, o_flag, total;
 };
 
 inline void sub_dims(const gh_subdomain_desc& d, int& n0, int& n1, int& n2) {
@@ -139,10 +142,10 @@ bool validate(const gh_subdomain_desc* descs, int32_t n_sub, std::string& err) {
     } else { snprintf(buf, sizeof buf, "subdomain %d: unknown kind %d", s, d.kind); err = buf; return false; }
     for (int f = 0; f < 6; ++f) {
       if (d.face[f] == GH_FACE_INTERFACE && f < 2 && d.kind == GH_SHELL) {
-        // the partner: the previous (inner face) / next (outer face) descriptor, a shell with the same centre and L whose
-        // facing face carries the flag too and sits at the same radius
+        // the partner: the previous (inner face) / next (outer face) descriptor, a shell with the same centre whose facing face
+        // carries the flag too and sits at the same radius (a different band limit L: its face state is interpolated)
         const int o = f == 0 ? s - 1 : s + 1;
-        bool ok = o >= 0 && o < n_sub && descs[o].kind == GH_SHELL && descs[o].n[1] == d.n[1] && descs[o].face[1 - f] == GH_FACE_INTERFACE;
+        bool ok = o >= 0 && o < n_sub && descs[o].kind == GH_SHELL && descs[o].face[1 - f] == GH_FACE_INTERFACE;
         if (ok) {
           const double ra = f == 0 ? d.lo[0] : d.hi[0], rb = f == 0 ? descs[o].hi[0] : descs[o].lo[0];
           ok = std::fabs(ra - rb) <= 1e-12 * std::fabs(ra);
@@ -170,6 +173,7 @@ bool make_plan(const gh_subdomain_desc* descs, int32_t n_sub, Plan& pl, std::str
   pl.ang_pb.assign(n_sub, 0);
   pl.ang_class.assign(n_sub, 0);
   std::map<int, int> seenL;
+  std::map<std::pair<int, int>, int> seenIfc;
   size_t tab = 0;
   int64_t off = 0, tiles = 0;
   for (int s = 0; s < n_sub; ++s) {
@@ -197,6 +201,16 @@ bool make_plan(const gh_subdomain_desc* descs, int32_t n_sub, Plan& pl, std::str
       if (d.kind == GH_BLOCK) { pl.ftable_doubles += cheb_frag_doubles(N); pl.n_fcheb[a][cheb_class(N)] += items; pl.n_fcheb_items += items; }
     }
     if (d.kind == GH_SHELL) {
+      for (int f = 0; f < 2; ++f) {
+        const int o = f == 0 ? s - 1 : s + 1;
+        if (d.face[f] != GH_FACE_INTERFACE || descs[o].n[1] == d.n[1]) continue;
+        const int Ls = descs[o].n[1], Ld = d.n[1];
+        if (Ls > GH_SMALL_L || Ld > GH_SMALL_L) { err = "interfaces between shells of different L are built for L <= 47"; return false; }
+        pl.n_ifc_items += 1; pl.Sf += round_up((int64_t)n1 * n2, 16);
+        const size_t nts = Ls + 1, nps = 2 * Ls + 2, nqs = 2 * Ls + 1, ntd = Ld + 1, npd = 2 * Ld + 2;
+        if (!seenIfc.count({Ls, Ld})) { seenIfc[{Ls, Ld}] = 1; pl.ifctab_doubles += nps * nqs + (size_t)(Ls + 1) * nts * ntd + nqs * npd; }
+        pl.ifc_smem = std::max(pl.ifc_smem, (nts * nps + nts * nqs + ntd * nqs) * sizeof(double));
+      }
       const int L = d.n[1];
       tab += (size_t)round_up(n0, 2) + 2 * (size_t)round_up(n1, 2) + 2 * (size_t)round_up(n2, 2);
       if (big_L(L)) {       // tiled GEMM path: analysis, per-m composites, two syntheses through global coefficient buffers
@@ -247,7 +261,9 @@ bool make_plan(const gh_subdomain_desc* descs, int32_t n_sub, Plan& pl, std::str
   pl.o_ua = c.take(NCOMP * comp); pl.o_ub = c.take(NCOMP * comp); pl.o_k = c.take(NCOMP * comp);
   pl.o_du = c.take(3 * NCOMP * comp); pl.o_H = c.take(4 * comp); pl.o_dH = c.take(12 * comp);
   pl.o_jac = c.take(9 * comp);
-  pl.o_tables = c.take((pl.table_doubles + pl.ftable_doubles + pl.bigtab_doubles) * sizeof(double));
+  pl.o_tables = c.take((pl.table_doubles + pl.ftable_doubles + pl.bigtab_doubles + pl.ifctab_doubles) * sizeof(double));
+  pl.o_ifc = c.take((size_t)std::max<int64_t>(1, NCOMP * pl.Sf) * sizeof(double));
+  pl.o_ifci = c.take((size_t)std::max(1, pl.n_ifc_items) * sizeof(IfcItem));
   pl.o_subs = c.take((size_t)n_sub * sizeof(SubDev));
   pl.o_tiles = c.take((size_t)(n_sub + 1) * sizeof(int32_t));
   pl.o_cheb = c.take((size_t)std::max(1, pl.n_cheb_items) * sizeof(ChebItem));
@@ -275,6 +291,8 @@ struct gh_domain {
   ChebItem* fcheb = nullptr;             // filter items of the blocks, ordered [axis][class]
   AngItem* ang = nullptr;
   GemmItem* gemm = nullptr;              // K_gemm items of the large subdomains, the G_NLIST lists back to back
+  IfcItem* ifci = nullptr;               // faces to interpolate (interfaces between shells of different L)
+  double* ifc = nullptr;                 // [50][Sf]: the neighbours' face states on the own grids
   struct FBlock { int N; double unused; size_t off; };     // one filter matrix slot per (block, axis): offset (doubles) from `tables`
   std::vector<FBlock> f_blocks;
   std::map<int, size_t> f_L;             // shell band limit L -> offset (doubles) of its filtered projectors from `tables`
@@ -416,7 +434,7 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
   d->du = (double*)(w + pl.o_du); d->H = (double*)(w + pl.o_H); d->dH = (double*)(w + pl.o_dH); d->jac = (double*)(w + pl.o_jac);
   d->tables = (double*)(w + pl.o_tables); d->subs = (SubDev*)(w + pl.o_subs); d->tiles = (int32_t*)(w + pl.o_tiles);
   d->cheb = (ChebItem*)(w + pl.o_cheb); d->ang = (AngItem*)(w + pl.o_ang); d->fcheb = (ChebItem*)(w + pl.o_fcheb);
-  d->gemm = (GemmItem*)(w + pl.o_gemm);
+  d->gemm = (GemmItem*)(w + pl.o_gemm); d->ifc = (double*)(w + pl.o_ifc); d->ifci = (IfcItem*)(w + pl.o_ifci);
   d->part = (double*)(w + pl.o_part); d->persub = (double*)(w + pl.o_persub); d->flag = (int*)(w + pl.o_flag);
 
   // ---- tables and work lists on the host ----
@@ -462,6 +480,13 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
   };
   struct BigShellOff { int64_t FaQ, FsQ, FpQ; std::vector<int64_t> Th, Pr; };
   std::map<int, BigShellOff> Lbig;
+  // interfaces between shells of different band limit: interpolation tables behind the large-class tables, items, buffer offsets
+  struct IfcOff { int64_t FaT, GT, FxT; };
+  std::map<std::pair<int, int>, IfcOff> IfcCache;
+  std::vector<double> ifctab(pl.ifctab_doubles, 0.0);
+  std::vector<IfcItem> ifci;
+  size_t itp = 0; int64_t ifc_next = 0;
+  const size_t ifc0 = pl.table_doubles + pl.ftable_doubles + pl.bigtab_doubles;
   for (int s = 0; s < n_sub; ++s) {
     const gh_subdomain_desc& de = descs[s];
     SubDev& sd = d->h_subs[s];
@@ -469,12 +494,46 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
     int n0, n1, n2; sub_dims(de, n0, n1, n2);
     sd.kind = de.kind; sd.n0 = n0; sd.n1 = n1; sd.n2 = n2; sd.off = pl.offsets[s]; sd.P = n0 * n1 * n2;
     for (int f = 0; f < 6; ++f) { sd.face[f] = de.face[f]; if (f < (de.kind == GH_SHELL ? 2 : 6) && de.face[f] == GH_FACE_CHARACTERISTIC) d->has_char = true; }
-    sd.nbr[0] = sd.nbr[1] = -1; sd.pen = 0.0;
+    sd.nbr[0] = sd.nbr[1] = -1; sd.nbi[0] = sd.nbi[1] = -1; sd.pen = 0.0;
     if (de.kind == GH_SHELL) {
       sd.pen = (double)(n0 - 1) * (double)(n0 - 1) / (de.hi[0] - de.lo[0]);
-      const int64_t plane = (int64_t)n1 * n2;
-      if (de.face[0] == GH_FACE_INTERFACE) { sd.nbr[0] = pl.offsets[s - 1] + (int64_t)(descs[s - 1].n[0] - 1) * plane; d->has_char = d->has_ifc = true; }
-      if (de.face[1] == GH_FACE_INTERFACE) { sd.nbr[1] = pl.offsets[s + 1]; d->has_char = d->has_ifc = true; }
+      for (int f = 0; f < 2; ++f) {
+        if (de.face[f] != GH_FACE_INTERFACE) continue;
+        d->has_char = d->has_ifc = true;
+        const int o = f == 0 ? s - 1 : s + 1;
+        const int Ls = descs[o].n[1], Ld = de.n[1];
+        const int64_t nplane = (int64_t)(Ls + 1) * (2 * Ls + 2);
+        // the neighbour's face plane: its outermost one for my inner face, its innermost one for my outer face
+        const int64_t src = f == 0 ? pl.offsets[o] + (int64_t)(descs[o].n[0] - 1) * nplane : pl.offsets[o];
+        if (Ls == Ld) { sd.nbr[f] = src; continue; }
+        if (!IfcCache.count({Ls, Ld})) {
+          // FaT[k][q] analysis on the source longitudes, GT[m][j][j'] per-m Legendre interpolation, FxT[q][k'] the series at the destination longitudes
+          ghb::ShellBasis B; ghb::shell_basis(Ls, B);
+          std::vector<ghb::ld> G; ghb::shell_interp_composites(Ls, Ld, G);
+          const int nts = Ls + 1, nps = 2 * Ls + 2, nqs = 2 * Ls + 1, ntd = Ld + 1, npd = 2 * Ld + 2;
+          IfcOff io; io.FaT = (int64_t)(ifc0 + itp);
+          for (int k = 0; k < nps; ++k) for (int q = 0; q < nqs; ++q) ifctab[itp + (size_t)k * nqs + q] = (double)B.Fa[(size_t)q * nps + k];
+          itp += (size_t)nps * nqs;
+          io.GT = (int64_t)(ifc0 + itp);
+          for (int m = 0; m <= Ls; ++m) for (int j = 0; j < nts; ++j) for (int jd = 0; jd < ntd; ++jd)
+            ifctab[itp + ((size_t)m * nts + j) * ntd + jd] = (double)G[((size_t)m * ntd + jd) * nts + j];
+          itp += (size_t)(Ls + 1) * nts * ntd;
+          io.FxT = (int64_t)(ifc0 + itp);
+          const ghb::ld PI_L = 3.14159265358979323846264338327950288L;
+          for (int q = 0; q < nqs; ++q) for (int k = 0; k < npd; ++k) {
+            const int m = q <= Ls ? q : q - Ls;
+            const ghb::ld ang = 2 * PI_L * (ghb::ld)(((long long)m * k) % npd) / npd;
+            ifctab[itp + (size_t)q * npd + k] = (double)(q == 0 ? (ghb::ld)1 : q <= Ls ? cosl(ang) : sinl(ang));
+          }
+          itp += (size_t)nqs * npd;
+          IfcCache[{Ls, Ld}] = io;
+        }
+        const IfcOff& io = IfcCache[{Ls, Ld}];
+        IfcItem it; memset(&it, 0, sizeof it);
+        it.src_off = src; it.dst_off = ifc_next; it.Ls = Ls; it.Ld = Ld; it.m_FaT = io.FaT; it.m_GT = io.GT; it.m_FxT = io.FxT;
+        sd.nbi[f] = ifc_next; ifc_next += round_up((int64_t)n1 * n2, 16);
+        ifci.push_back(it);
+      }
     }
     for (int g = 0; g < 3; ++g) sd.gamma[g] = de.gamma[g];
     const int naxes = de.kind == GH_SHELL ? 1 : 3;
@@ -678,6 +737,7 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
   std::vector<GemmItem> gemm;
   bool gemm_ok = btp == pl.bigtab_doubles;
   for (int l = 0; l < G_NLIST; ++l) { gemm_ok = gemm_ok && (int)glist[l].size() == pl.n_gemm[l]; gemm.insert(gemm.end(), glist[l].begin(), glist[l].end()); }
+  gemm_ok = gemm_ok && itp == pl.ifctab_doubles && (int)ifci.size() == pl.n_ifc_items && ifc_next == pl.Sf;
   if (tp != pl.table_doubles || (int)cheb.size() != pl.n_cheb_items || (int)ang.size() != pl.n_ang_items || !gemm_ok ||
       (int)fcheb.size() != pl.n_fcheb_items || ftp != pl.table_doubles + pl.ftable_doubles) {
     delete d; return fail(nullptr, GH_ERR_STATE, "internal: plan and build disagree");
@@ -694,6 +754,11 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
   if (!cheb.empty()) GH_CREATE_CUDA(cudaMemcpyAsync(d->cheb, cheb.data(), cheb.size() * sizeof(ChebItem), cudaMemcpyHostToDevice, st));
   if (!gemm.empty()) GH_CREATE_CUDA(cudaMemcpyAsync(d->gemm, gemm.data(), gemm.size() * sizeof(GemmItem), cudaMemcpyHostToDevice, st));
   if (!bigtab.empty()) GH_CREATE_CUDA(cudaMemcpyAsync(d->tables + big0, bigtab.data(), bigtab.size() * sizeof(double), cudaMemcpyHostToDevice, st));
+  if (!ifctab.empty()) GH_CREATE_CUDA(cudaMemcpyAsync(d->tables + ifc0, ifctab.data(), ifctab.size() * sizeof(double), cudaMemcpyHostToDevice, st));
+  if (!ifci.empty()) {
+    GH_CREATE_CUDA(cudaMemcpyAsync(d->ifci, ifci.data(), ifci.size() * sizeof(IfcItem), cudaMemcpyHostToDevice, st));
+    GH_CREATE_CUDA(cudaFuncSetAttribute(k_face_interp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
+  }
   GH_CREATE_CUDA(cudaFuncSetAttribute(k_gemm<GEMM_MB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gemm_smem_bytes(GEMM_MB)));
   if (!ang.empty()) GH_CREATE_CUDA(cudaMemcpyAsync(d->ang, ang.data(), ang.size() * sizeof(AngItem), cudaMemcpyHostToDevice, st));
   if (!fcheb.empty()) GH_CREATE_CUDA(cudaMemcpyAsync(d->fcheb, fcheb.data(), fcheb.size() * sizeof(ChebItem), cudaMemcpyHostToDevice, st));
@@ -852,12 +917,16 @@ gh_status launch_rhs(gh_domain* d, const double* u, double* out, int rk_mode = 0
                      double b = 1.0, double dt = 0.0, bool norms = false) {
   gh_status st = launch_derivs(d, u, d->du, NCOMP);
   if (st != GH_OK) return st;
+  if (d->pl.n_ifc_items) {      // the neighbours' face states of this stage's input, on the grids of the shells that read them
+    ProfScope ps(d, GH_K_OTHER);
+    k_face_interp<<<dim3(d->pl.n_ifc_items, NCOMP), 256, d->pl.ifc_smem, d->stream>>>(d->ifci, d->tables, u, d->ifc, d->pl.S, d->pl.Sf);
+  }
   if (norms) {      // A8 as the epilogue of stage 1 (rk_mode 1 only): per-tile partials, folded per subdomain like K_con's
     const RkArgs rk{u0, a, b, dt};
     const int grid = d->pl.n_tiles;
     {
       ProfScope ps(d, GH_K_RHS);
-      if (d->has_char) k_rhs<1, true, true><<<grid, TILE_PTS, RHS_SMEM_BYTES_NORMS, d->stream>>>(d->subs, d->tiles, d->pl.n_sub, d->tables, u, d->du, d->H, d->dH, out, rk, d->pl.S, d->flag, d->part);
+      if (d->has_char) k_rhs<1, true, true><<<grid, TILE_PTS, RHS_SMEM_BYTES_NORMS, d->stream>>>(d->subs, d->tiles, d->pl.n_sub, d->tables, u, d->du, d->H, d->dH, out, rk, d->pl.S, d->flag, d->part, d->ifc, d->pl.Sf);
       else k_rhs<1, false, true><<<grid, TILE_PTS, RHS_SMEM_BYTES_NORMS, d->stream>>>(d->subs, d->tiles, d->pl.n_sub, d->tables, u, d->du, d->H, d->dH, out, rk, d->pl.S, d->flag, d->part);
     }
     {
@@ -871,7 +940,7 @@ gh_status launch_rhs(gh_domain* d, const double* u, double* out, int rk_mode = 0
     ProfScope ps(d, GH_K_RHS);
     const RkArgs rk{u0, a, b, dt};
     const int grid = d->pl.n_tiles;
-#define GH_RHS_LAUNCH(M, C) k_rhs<M, C><<<grid, TILE_PTS, RHS_SMEM_BYTES, d->stream>>>(d->subs, d->tiles, d->pl.n_sub, d->tables, u, d->du, d->H, d->dH, out, rk, d->pl.S, d->flag)
+#define GH_RHS_LAUNCH(M, C) k_rhs<M, C><<<grid, TILE_PTS, RHS_SMEM_BYTES, d->stream>>>(d->subs, d->tiles, d->pl.n_sub, d->tables, u, d->du, d->H, d->dH, out, rk, d->pl.S, d->flag, nullptr, d->ifc, d->pl.Sf)
     if (d->has_char) { if (rk_mode == 0) GH_RHS_LAUNCH(0, true); else if (rk_mode == 1) GH_RHS_LAUNCH(1, true); else GH_RHS_LAUNCH(2, true); }
     else { if (rk_mode == 0) GH_RHS_LAUNCH(0, false); else if (rk_mode == 1) GH_RHS_LAUNCH(1, false); else GH_RHS_LAUNCH(2, false); }
 #undef GH_RHS_LAUNCH

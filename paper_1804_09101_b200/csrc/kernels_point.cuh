@@ -312,6 +312,58 @@ __device__ __forceinline__ void algebraic(const Geom& G, const PI& Pi, const PH&
 // ---------------------------------------------------------------------------------------------------------
 struct RkArgs { const double* u0; double a, b, dt; };
 
+// ---------------------------------------------------------------------------------------------------------
+// K_face_interp (NEXT-2 (iii) between shells of different band limit; "at 'internal' boundaries between neighboring domains, the
+// characteristic variables are computed and used as boundary conditions on the neighboring subdomain"; interpolation
+// "via a direct summation of the spectral series"): the neighbour's face state, given on its own Gauss-Legendre x
+// uniform grid of band limit Ls, is analysed there and the series is summed at the nodes of this shell's grid (band limit Ld):
+//   C[j][q]  = sum_k  u[j][k] Fa_s[q][k]          real DFT on the source longitudes (q = 0: m = 0; 1..Ls: cos m; Ls+1..2Ls: sin m)
+//   D[j'][q] = sum_j  G_m(q)[j'][j] C[j][q]       per m: 2 pi sum_l Pbar_lm(theta'_j') w_j Pbar_lm(theta_j)
+//   out[j'][k'] = sum_q D[j'][q] Fx[k'][q]        the Fourier series at the destination longitudes (all m <= Ls, not truncated)
+// grid = (faces, components); a face is a few thousand points: plain DFMA, operands staged in shared memory, the matrices stored
+// transposed so that consecutive threads read consecutive addresses.
+// ---------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_face_interp(const IfcItem* __restrict__ items, const double* __restrict__ tables, const double* __restrict__ u,
+              double* __restrict__ ifc, int64_t S, int64_t Sf) {
+  extern __shared__ __align__(16) double fsm[];
+  const IfcItem it = items[blockIdx.x];
+  const int c = blockIdx.y, tid = threadIdx.x;
+  const int nts = it.Ls + 1, nps = 2 * it.Ls + 2, nqs = 2 * it.Ls + 1, ntd = it.Ld + 1, npd = 2 * it.Ld + 2;
+  double* U = fsm;                       // [nts][nps]
+  double* Cq = U + nts * nps;            // [nts][nqs]
+  double* Dq = Cq + nts * nqs;           // [ntd][nqs]
+  const double* __restrict__ src = u + (int64_t)c * S + it.src_off;
+  for (int e = tid; e < nts * nps; e += 256) U[e] = src[e];
+  __syncthreads();
+  const double* __restrict__ FaT = tables + it.m_FaT;
+  for (int e = tid; e < nts * nqs; e += 256) {
+    const int j = e / nqs, q = e - j * nqs;
+    double s = 0.0;
+    for (int k = 0; k < nps; ++k) s = fma(U[j * nps + k], __ldg(FaT + (int64_t)k * nqs + q), s);
+    Cq[e] = s;
+  }
+  __syncthreads();
+  const double* __restrict__ GT = tables + it.m_GT;
+  for (int e = tid; e < ntd * nqs; e += 256) {
+    const int q = e / ntd, jd = e - q * ntd;
+    const int m = q <= it.Ls ? q : q - it.Ls;
+    const double* __restrict__ g = GT + (int64_t)m * nts * ntd + jd;
+    double s = 0.0;
+    for (int j = 0; j < nts; ++j) s = fma(__ldg(g + (int64_t)j * ntd), Cq[j * nqs + q], s);
+    Dq[jd * nqs + q] = s;
+  }
+  __syncthreads();
+  const double* __restrict__ FxT = tables + it.m_FxT;
+  double* __restrict__ dst = ifc + (int64_t)c * Sf + it.dst_off;
+  for (int e = tid; e < ntd * npd; e += 256) {
+    const int jd = e / npd, k = e - jd * npd;
+    double s = 0.0;
+    for (int q = 0; q < nqs; ++q) s = fma(Dq[jd * nqs + q], __ldg(FxT + (int64_t)q * npd + k), s);
+    dst[e] = s;
+  }
+}
+
 // Characteristic boundary condition (NEXT-2 (i), reading S21) for one symmetric pair (ab) at a face point with outward
 // direction s: with n_i = s_i / sqrt(g^{jk} s_j s_k), n^i = g^{ij} n_j,
 //   u0 = psi (speed -(1+g1) n.N),  u1+- = Pi +- n^i Phi_i - g2 psi (speed -n.N +- N),  u2_i = Phi_i - n_i n^k Phi_k (speed -n.N);
@@ -426,7 +478,8 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
                                           const double* u, const double* __restrict__ du,
                                           const double* __restrict__ Hs, const double* __restrict__ dHs,
                                           double* k, const RkArgs& rk, int64_t S, int* __restrict__ flag,
-                                          double* __restrict__ phis /* + tid */) {
+                                          double* __restrict__ phis /* + tid */, const double* __restrict__ ifc = nullptr,
+                                          int64_t Sf = 0) {
   double* __restrict__ ring = phis + RHS_PHI_ROWS * TILE_PTS;
   static_assert(!NORMS || RK == 1, "the NORMS partials sit in the ring rows of the RK = 2 prefetch");
 #define GH_NACC(q) phis[rhs_norm_row(q) * TILE_PTS]    /* NORMS: this thread's six partials */
@@ -587,12 +640,16 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
 #pragma unroll
         for (int f = 0; f < 2; ++f)
           if (cmask & (64 << f)) {
-            const int64_t t = sd.nbr[f] + q;
+            // the neighbour's state at this point of the face: straight from the store where the grids coincide, else from
+            // the interpolated copy K_face_interp made of it on this shell's grid
+            const bool ip = sd.nbi[f] >= 0;
+            const double* nb = ip ? ifc + sd.nbi[f] + q : u + sd.nbr[f] + q;
+            const int64_t ns = ip ? Sf : S;
             const double sg = f ? 1.0 : -1.0;
-            const double ePhi[3] = {Phi(0, s) - u[(int64_t)(20 + s) * S + t], Phi(1, s) - u[(int64_t)(30 + s) * S + t],
-                                    Phi(2, s) - u[(int64_t)(40 + s) * S + t]};
-            char_penalty_pair(G, g1, g2, sg * J.xr, sg * J.yr, sg * J.zr, sd.pen, psi[s] - u[(int64_t)s * S + t],
-                              Pi[s] - u[(int64_t)(10 + s) * S + t], ePhi, o_psi, r, o_Phi);
+            const double ePhi[3] = {Phi(0, s) - nb[(int64_t)(20 + s) * ns], Phi(1, s) - nb[(int64_t)(30 + s) * ns],
+                                    Phi(2, s) - nb[(int64_t)(40 + s) * ns]};
+            char_penalty_pair(G, g1, g2, sg * J.xr, sg * J.yr, sg * J.zr, sd.pen, psi[s] - nb[(int64_t)s * ns],
+                              Pi[s] - nb[(int64_t)(10 + s) * ns], ePhi, o_psi, r, o_Phi);
           }
       }
       if (CBC && (cmask & 63)) {   // characteristic faces through this point, in face order (rare: face points only)
@@ -631,7 +688,7 @@ __global__ void __launch_bounds__(TILE_PTS, 2)
 k_rhs(const SubDev* __restrict__ subs, const int32_t* __restrict__ tile_first, int n_sub,
       const double* __restrict__ tables, const double* u, const double* __restrict__ du,
       const double* __restrict__ Hs, const double* __restrict__ dHs, double* k, RkArgs rk, int64_t S,
-      int* __restrict__ flag, double* __restrict__ part = nullptr) {
+      int* __restrict__ flag, double* __restrict__ part = nullptr, const double* __restrict__ ifc = nullptr, int64_t Sf = 0) {
   extern __shared__ __align__(16) double ring_s[];   // Phi [30][TILE_PTS], the ring [RHS_RING][RHS_RING_ROWS][TILE_PTS], NORMS: [6][TILE_PTS]
   __shared__ SubDev sd_s;
   __shared__ int tile0_s;
@@ -650,7 +707,7 @@ k_rhs(const SubDev* __restrict__ subs, const int32_t* __restrict__ tile_first, i
   const SubDev& sd = sd_s;
   const int local = (blockIdx.x - tile0_s) * TILE_PTS + threadIdx.x;
   if (local < sd.P) {
-    if (sd.kind == 0) rhs_point<true, RK, CBC, NORMS>(sd, tables, local, u, du, Hs, dHs, k, rk, S, flag, ring_s + threadIdx.x);
+    if (sd.kind == 0) rhs_point<true, RK, CBC, NORMS>(sd, tables, local, u, du, Hs, dHs, k, rk, S, flag, ring_s + threadIdx.x, ifc, Sf);
     else rhs_point<false, RK, CBC, NORMS>(sd, tables, local, u, du, Hs, dHs, k, rk, S, flag, ring_s + threadIdx.x);
   }
   if (NORMS) {    // the same fold as K_con: warp shuffle, then the warps in fixed order (deterministic)
