@@ -584,6 +584,57 @@ int ora_rhs_point(const double* psi, const double* Pi, const double* Phi, const 
   return 0;
 }
 
+/* ---------------------------------------------------------------------- */
+/* O14 — dual-frame right-hand side (NEXT-4; "data is represented at        */
+/* collocation points at fixed grid-coordinates ... The evolution equations, */
+/* however, are formulated in asymptotic inertial coordinates.  The two      */
+/* coordinate systems share the same time-coordinate, and their spatial      */
+/* coordinates are related by a time-dependent coordinate transformation",   */
+/* PAPER.md:87).  With grid coordinates xbar, inertial x = x(xbar, t),       */
+/*   Jm_i^k = d xbar^k / d x^i   and   v^i = (d x^i / d t) at fixed xbar:    */
+/*   d_i u = Jm_i^k dbar_k u          (DiffJac, Eq. 8)     */
+/*   d_t u |_xbar = F[u, d_i u] + v^i d_i u                                   */
+/* where F is the single-frame right-hand side O5 and the tensor components  */
+/* stay inertial-frame Cartesian.                                            */
+/* ---------------------------------------------------------------------- */
+static void map_derivs(point_in* in, const real J[3][3]) {
+  for (int a = 0; a < 4; ++a) for (int b = 0; b < 4; ++b) {
+    real o[3], n[3];
+    for (int k = 0; k < 3; ++k) o[k] = in->dpsi[k][a][b];
+    for (int i = 0; i < 3; ++i) { n[i] = 0; for (int k = 0; k < 3; ++k) n[i] += J[i][k] * o[k]; }
+    for (int i = 0; i < 3; ++i) in->dpsi[i][a][b] = n[i];
+    for (int k = 0; k < 3; ++k) o[k] = in->dPi[k][a][b];
+    for (int i = 0; i < 3; ++i) { n[i] = 0; for (int k = 0; k < 3; ++k) n[i] += J[i][k] * o[k]; }
+    for (int i = 0; i < 3; ++i) in->dPi[i][a][b] = n[i];
+    for (int j = 0; j < 3; ++j) {
+      for (int k = 0; k < 3; ++k) o[k] = in->dPhi[k][j][a][b];
+      for (int i = 0; i < 3; ++i) { n[i] = 0; for (int k = 0; k < 3; ++k) n[i] += J[i][k] * o[k]; }
+      for (int i = 0; i < 3; ++i) in->dPhi[i][j][a][b] = n[i];
+    }
+  }
+}
+static void map_advect(const point_in* in, const real v[3], real a[4][4], real b[4][4], real c[3][4][4]) {
+  for (int x = 0; x < 4; ++x) for (int y = 0; y < 4; ++y) for (int i = 0; i < 3; ++i) {
+    a[x][y] += v[i] * in->dpsi[i][x][y]; b[x][y] += v[i] * in->dPi[i][x][y];
+    for (int j = 0; j < 3; ++j) c[j][x][y] += v[i] * in->dPhi[i][j][x][y];
+  }
+}
+
+/* one point: the derivative inputs are GRID-frame (dbar_k); Jm[9] row-major Jm[3 i + k], v[3]; dH is inertial-frame */
+int ora_rhs_point_map(const double* psi, const double* Pi, const double* Phi, const double* dpsi, const double* dPi,
+                      const double* dPhi, const double* H, const double* dH, const double* gamma, const double* Jm, const double* v,
+                      double* dtpsi, double* dtPi, double* dtPhi) {
+  point_in in; load_point(&in, psi, Pi, Phi, dpsi, dPi, dPhi, H, dH);
+  real g[3] = {gamma[0], gamma[1], gamma[2]}, a[4][4], b[4][4], c[3][4][4], J[3][3], vv[3] = {v[0], v[1], v[2]};
+  for (int i = 0; i < 3; ++i) for (int k = 0; k < 3; ++k) J[i][k] = Jm[3 * i + k];
+  map_derivs(&in, J);
+  if (rhs_point(&in, g, a, b, c)) return 1;
+  map_advect(&in, vv, a, b, c);
+  for (int x = 0; x < 4; ++x) for (int y = 0; y < 4; ++y) { dtpsi[x * 4 + y] = (double)a[x][y]; dtPi[x * 4 + y] = (double)b[x][y];
+    for (int i = 0; i < 3; ++i) dtPhi[(i * 4 + x) * 4 + y] = (double)c[i][x][y]; }
+  return 0;
+}
+
 int ora_constraints_point(const double* psi, const double* Pi, const double* Phi, const double* dpsi, const double* dPhi,
                           const double* H, double* Ca, double* Ciab, double* Cijab) {
   static const double z48[48] = {0}, z12[12] = {0};
@@ -743,6 +794,8 @@ static int char_faces(const ora_subdomain* sd, int64_t p, const real* xyz3 /* x,
 /* real-typed core: u[50][P], H[4][P], gH[12][P] ([i][a]) -> dtu[50][P]. Returns #non-physical points. */
 static const double* g_nbr_in = NULL;    /* neighbour state on the inner / outer face of a shell, [50][n_theta n_phi], set by */
 static const double* g_nbr_out = NULL;   /* ora_rhs_subdomain_ifc around its call (faces flagged INTERFACE = 3) */
+static const double* g_map_J = NULL;     /* O14: frame map Jm[9][P] and grid velocity v[3][P], set by ora_rhs_subdomain_map / */
+static const double* g_map_v = NULL;     /* ora_rk3_subdomain_map around their calls */
 
 static int rhs_real(const ora_subdomain* sd, const real* u, const real* H, const real* gH, real* dtu) {
   int64_t P = ora_num_points(sd);
@@ -755,6 +808,10 @@ static int rhs_real(const ora_subdomain* sd, const real* u, const real* H, const
   for (int64_t p = 0; p < P; ++p) {
     point_in in; fill_point(&in, u, g, H, gH, P, p);
     real a[4][4], b[4][4], c[3][4][4];
+    if (g_map_J) {   /* O14: grid-frame derivatives -> inertial frame */
+      real J[3][3]; for (int i = 0; i < 3; ++i) for (int k = 0; k < 3; ++k) J[i][k] = g_map_J[(int64_t)(3 * i + k) * P + p];
+      map_derivs(&in, J);
+    }
     if (rhs_point(&in, gam, a, b, c)) { bad += 1; memset(a, 0, sizeof a); memset(b, 0, sizeof b); memset(c, 0, sizeof c); }
     int fz = frozen(sd, p);
     if (!fz) {   /* O10: characteristic faces, in face order (a FROZEN face through the point wins) */
@@ -779,6 +836,10 @@ static int rhs_real(const ora_subdomain* sd, const real* u, const real* H, const
           char_penalty_point(in.psi, gam, sv, pen, dps, dPi_, dPh, a, b, c);
         }
       }
+    }
+    if (g_map_v && !fz) {   /* O14: the time derivative at the fixed grid point (boundary treatments acted on the inertial-frame part) */
+      real vv[3] = {g_map_v[p], g_map_v[P + p], g_map_v[2 * P + p]};
+      map_advect(&in, vv, a, b, c);
     }
     for (int x = 0; x < 4; ++x) for (int y = x; y < 4; ++y) {
       int s = SYM[x][y];
@@ -1109,4 +1170,15 @@ void ora_shell_interp(int Ls, int Ld, const double* u, double* out) {
     }
   }
   free(are); free(aim); free(ctd); free(wd); free(pb); free(dpb); ylm_free(t);
+}
+
+/* O14 on one subdomain: Jm[9][P], v[3][P] (held fixed), dH[12][P] the inertial-frame gradient of H (required: the library's own
+ * derivative of H would be a grid-frame one).  nsteps = 0: the right-hand side into out[50][P]; nsteps > 0: that many SSP-RK3 steps of
+ * u in place with the map frozen (out unused).  Not re-entrant. */
+int ora_rhs_subdomain_map(const ora_subdomain* sd, double* u, const double* H, const double* dH, const double* Jm, const double* v,
+                          double dt, int nsteps, double* out) {
+  g_map_J = Jm; g_map_v = v;
+  int bad = nsteps > 0 ? ora_rk3_subdomain(sd, u, H, dH, dt, nsteps) : ora_rhs_subdomain(sd, u, H, dH, out);
+  g_map_J = NULL; g_map_v = NULL;
+  return bad;
 }

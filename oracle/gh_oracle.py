@@ -110,6 +110,10 @@ class Oracle:
         L.ora_char_bc_point.restype = C.c_int
         L.ora_filter_subdomain.argtypes = [C.POINTER(Subdomain), C.c_int, _dp, _dp, _dp, _dp]
         L.ora_filter_subdomain.restype = C.c_int
+        L.ora_rhs_point_map.argtypes = [_dp] * 14
+        L.ora_rhs_point_map.restype = C.c_int
+        L.ora_rhs_subdomain_map.argtypes = [C.POINTER(Subdomain), _dp, _dp, _dp, _dp, _dp, C.c_double, C.c_int, _dp]
+        L.ora_rhs_subdomain_map.restype = C.c_int
         L.ora_shell_interp.argtypes = [C.c_int, C.c_int, _dp, _dp]
         L.ora_scj_point.argtypes = [C.c_int, _dp, _dp, _dp]
         L.ora_scj_point.restype = C.c_double
@@ -219,6 +223,26 @@ class Oracle:
         if bad:
             raise ValueError("non-physical metric")
         return o1, o2, o3
+
+    def rhs_point_map(self, psi, Pi, Phi, dpsi, dPi, dPhi, H, dH, gamma, Jm, v):
+        """O14 at a point: derivative inputs in the GRID frame, Jm[3,3] = d xbar^k / d x^i, v[3] the grid velocity; dH inertial."""
+        c = lambda a: np.ascontiguousarray(a, dtype=np.float64)
+        o1, o2, o3 = np.empty((4, 4)), np.empty((4, 4)), np.empty((3, 4, 4))
+        bad = self.lib.ora_rhs_point_map(c(psi), c(Pi), c(Phi), c(dpsi), c(dPi), c(dPhi), c(H), c(dH), c(gamma), c(Jm), c(v), o1, o2, o3)
+        if bad:
+            raise ValueError("non-physical metric")
+        return o1, o2, o3
+
+    def rhs_map(self, sd: dict, u, H, dH, Jm, v, dt: float = 0.0, nsteps: int = 0) -> np.ndarray:
+        """O14 on a subdomain: nsteps = 0 -> the dual-frame RHS; nsteps > 0 -> the state after that many RK3 steps (map frozen)."""
+        s = make_subdomain(sd)
+        uu = np.array(u, dtype=np.float64, order="C", copy=True)
+        out = np.empty_like(uu)
+        c = lambda a: np.ascontiguousarray(a, dtype=np.float64)
+        bad = self.lib.ora_rhs_subdomain_map(C.byref(s), uu, c(H), c(dH), c(Jm), c(v), float(dt), int(nsteps), out)
+        if bad:
+            raise ValueError(f"{bad} non-physical points")
+        return uu if nsteps > 0 else out
 
     def char_bc_point(self, psi, gamma, s, dtpsi, dtPi, dtPhi):
         """O10 at one point: freeze the incoming characteristic fields.  psi[4,4]; s[3] outward direction;
