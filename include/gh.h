@@ -225,6 +225,21 @@ gh_status gh_spatial_coord_jac(gh_domain* dom, int structure, const double* T, d
  * Phi'_iab = J_i^k L_a^c L_b^d Phi_kcd, L = diag(1, J).  Asynchronous.  GH_ERR_STATE before gh_set_fields / gh_set_jacobian. */
 gh_status gh_spatial_coord_jac_state(gh_domain* dom);
 
+/* ---- dual frame (NEXT-4) -------------------------------------------------------------------------------------------
+ * "data is represented at collocation points at fixed grid-coordinates ...  The evolution equations, however, are formulated in
+ * asymptotic inertial coordinates.  The two coordinate systems share the same time-coordinate, and their spatial coordinates are
+ * related by a time-dependent coordinate transformation."  The caller evaluates the map x = x(xbar, t) at the current time and
+ * hands over its kinematics at the grid points:
+ *   Jm[9][comp_stride], Jm[3 i + k] = d xbar^k / d x^i      (d/dx^i = Jm_i^k d/dxbar^k: DiffJac, Eq. 8)
+ *   v[3][comp_stride],  v^i = d x^i / d t at fixed xbar       (the velocity of the grid points in the inertial frame)
+ * From then on gh_rhs, gh_rk_step(_norms), gh_dp5_step and gh_constraint_norms use inertial-frame derivatives d_i u = Jm_i^k dbar_k u
+ * and the time derivative AT THE FIXED GRID POINTS:  d_t u |_xbar = F[u, d_i u] + v^i d_i u  (F: the single-frame right-hand side;
+ * tensor components stay inertial-frame Cartesian).  Boundary treatments act on F; FROZEN faces hold their grid-frame value
+ * (no advection there).  The map is held fixed until the next call (within one step it is frozen: re-set it as time advances).
+ * The gauge source's gradient dH must then be given explicitly, in the inertial frame.  gh_gradient stays a grid-frame gradient.
+ * Jm = v = NULL: back to the single frame.  HOST or DEVICE per flag.  Cost: two more HBM passes per RHS evaluation, only while set. */
+gh_status gh_set_frame_map(gh_domain* dom, const double* Jm, const double* v, int on_device);
+
 /* FP64 throughput of the device the domain lives on, measured now with register-resident kernels on the domain's stream
  * (profiling helper; bench.py quotes the derivative kernels' roofline fraction against it): tflops[0] = DMMA
  * (mma.sync.m8n8k4.f64, what K_cheb / K_ang issue), tflops[1] = plain DFMA.  Best of 3 launches of ~2 ms after a warm-up.

@@ -76,7 +76,7 @@ struct Plan {
   std::vector<int> ang_pb;               // planes per CTA for each subdomain (0 for blocks)
   std::vector<int> ang_class;            // shared-memory class of each shell
   // workspace offsets (bytes)
-  size_t o_ua, o_ub, o_k, o_du, o_H, o_dH, o_jac, o_tables, o_subs, o_tiles, o_cheb, o_fcheb, o_ang, o_gemm, o_ifc, o_ifci, o_part, o_persub, o_flag, total;
+  size_t o_ua, o_ub, o_k, o_du, o_H, o_dH, o_jac, o_mapJ, o_mapv, o_tables, o_subs, o_tiles, o_cheb, o_fcheb, o_ang, o_gemm, o_ifc, o_ifci, o_part, o_persub, o_flag, total;
 };
 
 inline void sub_dims(const gh_subdomain_desc& d, int& n0, int& n1, int& n2) {
@@ -260,7 +260,7 @@ bool make_plan(const gh_subdomain_desc* descs, int32_t n_sub, Plan& pl, std::str
   const size_t comp = (size_t)pl.S * sizeof(double);
   pl.o_ua = c.take(NCOMP * comp); pl.o_ub = c.take(NCOMP * comp); pl.o_k = c.take(NCOMP * comp);
   pl.o_du = c.take(3 * NCOMP * comp); pl.o_H = c.take(4 * comp); pl.o_dH = c.take(12 * comp);
-  pl.o_jac = c.take(9 * comp);
+  pl.o_jac = c.take(9 * comp); pl.o_mapJ = c.take(9 * comp); pl.o_mapv = c.take(3 * comp);
   pl.o_tables = c.take((pl.table_doubles + pl.ftable_doubles + pl.bigtab_doubles + pl.ifctab_doubles) * sizeof(double));
   pl.o_ifc = c.take((size_t)std::max<int64_t>(1, NCOMP * pl.Sf) * sizeof(double));
   pl.o_ifci = c.take((size_t)std::max(1, pl.n_ifc_items) * sizeof(IfcItem));
@@ -285,6 +285,8 @@ struct gh_domain {
   cudaStream_t stream = nullptr;
   double *ua = nullptr, *ub = nullptr, *k = nullptr, *du = nullptr, *H = nullptr, *dH = nullptr, *jac = nullptr, *tables = nullptr;
   bool has_jac = false;
+  double *mapJ = nullptr, *mapv = nullptr;   // dual frame (gh_set_frame_map)
+  bool has_map = false;
   SubDev* subs = nullptr;
   int32_t* tiles = nullptr;
   ChebItem* cheb = nullptr;
@@ -309,7 +311,7 @@ struct gh_domain {
   int opt[GH_NUM_OPTIONS] = {0};         // gh_set_option
   // CUDA graphs of the step (kind 0: gh_rk_step, 1: gh_rk_step_norms) and of gh_rhs to a DEVICE pointer (kind 2), each valid
   // for the key it was captured with
-  struct StepGraph { cudaGraphExec_t exec = nullptr; double dt = 0; const void *ua = nullptr, *ub = nullptr, *out = nullptr; int oop = 0; int64_t nlaunch = 0; };
+  struct StepGraph { cudaGraphExec_t exec = nullptr; double dt = 0; const void *ua = nullptr, *ub = nullptr, *out = nullptr; int oop = 0, map = 0; int64_t nlaunch = 0; };
   StepGraph graphs[3];
   double t = 0.0;
   int64_t launches = 0;
@@ -432,6 +434,7 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
   char* w = d->ws;
   d->ua = (double*)(w + pl.o_ua); d->ub = (double*)(w + pl.o_ub); d->k = (double*)(w + pl.o_k);
   d->du = (double*)(w + pl.o_du); d->H = (double*)(w + pl.o_H); d->dH = (double*)(w + pl.o_dH); d->jac = (double*)(w + pl.o_jac);
+  d->mapJ = (double*)(w + pl.o_mapJ); d->mapv = (double*)(w + pl.o_mapv);
   d->tables = (double*)(w + pl.o_tables); d->subs = (SubDev*)(w + pl.o_subs); d->tiles = (int32_t*)(w + pl.o_tiles);
   d->cheb = (ChebItem*)(w + pl.o_cheb); d->ang = (AngItem*)(w + pl.o_ang); d->fcheb = (ChebItem*)(w + pl.o_fcheb);
   d->gemm = (GemmItem*)(w + pl.o_gemm); d->ifc = (double*)(w + pl.o_ifc); d->ifci = (IfcItem*)(w + pl.o_ifci);
@@ -917,6 +920,16 @@ gh_status launch_rhs(gh_domain* d, const double* u, double* out, int rk_mode = 0
                      double b = 1.0, double dt = 0.0, bool norms = false) {
   gh_status st = launch_derivs(d, u, d->du, NCOMP);
   if (st != GH_OK) return st;
+  if (d->has_map) {             // dual frame: the derivative scratch becomes inertial-frame (K_rhs applies the spherical Jacobian itself)
+    ProfScope ps(d, GH_K_OTHER);
+    k_map_pre<<<d->pl.n_tiles, TILE_PTS, 0, d->stream>>>(d->subs, d->tiles, d->pl.n_sub, d->tables, d->mapJ, d->du, d->pl.S, NCOMP);
+  }
+  // ... and after the fused kernel: + coef v^i d_i u, the time derivative at the fixed grid points
+  auto map_post = [&]() {
+    if (!d->has_map) return;
+    ProfScope ps(d, GH_K_OTHER);
+    k_map_post<<<d->pl.n_tiles, TILE_PTS, 0, d->stream>>>(d->subs, d->tiles, d->pl.n_sub, d->tables, d->mapv, d->du, out, d->pl.S, rk_mode == 0 ? 1.0 : b * dt);
+  };
   if (d->pl.n_ifc_items) {      // the neighbours' face states of this stage's input, on the grids of the shells that read them
     ProfScope ps(d, GH_K_OTHER);
     k_face_interp<<<dim3(d->pl.n_ifc_items, NCOMP), 256, d->pl.ifc_smem, d->stream>>>(d->ifci, d->tables, u, d->ifc, d->pl.S, d->pl.Sf);
@@ -933,6 +946,7 @@ gh_status launch_rhs(gh_domain* d, const double* u, double* out, int rk_mode = 0
       ProfScope ps(d, GH_K_REDUCE);
       k_con_reduce<<<d->pl.n_sub, 32, 0, d->stream>>>(d->tiles, d->part, d->persub);
     }
+    map_post();
     GH_CUDA(d, cudaGetLastError());
     return GH_OK;
   }
@@ -945,6 +959,7 @@ gh_status launch_rhs(gh_domain* d, const double* u, double* out, int rk_mode = 0
     else { if (rk_mode == 0) GH_RHS_LAUNCH(0, false); else if (rk_mode == 1) GH_RHS_LAUNCH(1, false); else GH_RHS_LAUNCH(2, false); }
 #undef GH_RHS_LAUNCH
   }
+  map_post();
   GH_CUDA(d, cudaGetLastError());
   return GH_OK;
 }
@@ -967,7 +982,7 @@ gh_status run_graphed(gh_domain* d, int kind, double dt, const void* out, F body
   if (d->opt[GH_OPT_NO_GRAPH] || d->prof || d->stream == nullptr) return body();
   gh_domain::StepGraph& g = d->graphs[kind];
   const int oop = d->opt[GH_OPT_RK_OUT_OF_PLACE];
-  if (!g.exec || g.dt != dt || g.ua != d->ua || g.ub != d->ub || g.out != out || g.oop != oop) {
+  if (!g.exec || g.dt != dt || g.ua != d->ua || g.ub != d->ub || g.out != out || g.oop != oop || g.map != (int)d->has_map) {
     if (g.exec) { cudaGraphExecDestroy(g.exec); g.exec = nullptr; }
     const int64_t l0 = d->launches;
     GH_CUDA(d, cudaStreamBeginCapture(d->stream, cudaStreamCaptureModeThreadLocal));
@@ -980,7 +995,7 @@ gh_status run_graphed(gh_domain* d, int kind, double dt, const void* out, F body
     const cudaError_t ei = cudaGraphInstantiate(&g.exec, graph, 0);
     cudaGraphDestroy(graph);
     if (ei != cudaSuccess) { g.exec = nullptr; return fail(d, GH_ERR_CUDA, std::string("cudaGraphInstantiate: ") + cudaGetErrorString(ei)); }
-    g.dt = dt; g.ua = d->ua; g.ub = d->ub; g.out = out; g.oop = oop;
+    g.dt = dt; g.ua = d->ua; g.ub = d->ub; g.out = out; g.oop = oop; g.map = (int)d->has_map;
   }
   GH_CUDA(d, cudaGraphLaunch(g.exec, d->stream));
   d->launches += g.nlaunch;
@@ -1139,6 +1154,10 @@ extern "C" gh_status gh_constraint_norms(gh_domain* d, double* out, double* per_
   const Plan& pl = d->pl;
   gh_status st = launch_derivs(d, d->ua, d->du, NCOMP, 10, 10);   // the constraints need no derivative of Pi (components 10..19)
   if (st != GH_OK) return st;
+  if (d->has_map) {             // dual frame: C_iab and C_ijab are built from inertial-frame derivatives
+    ProfScope ps(d, GH_K_OTHER);
+    k_map_pre<<<pl.n_tiles, TILE_PTS, 0, d->stream>>>(d->subs, d->tiles, pl.n_sub, d->tables, d->mapJ, d->du, pl.S, NCOMP);
+  }
   {
     ProfScope ps(d, GH_K_CONSTRAINTS);
     k_con<<<pl.n_tiles, TILE_PTS, 0, d->stream>>>(d->subs, d->tiles, pl.n_sub, d->tables, d->ua, d->du, d->H, pl.S, d->flag, d->part);
@@ -1413,6 +1432,21 @@ extern "C" gh_status gh_spatial_coord_jac_state(gh_domain* d) {
   d->dp_fsal = false;
   launch_scj(d, 4, d->ua, d->ua);
   GH_CUDA(d, cudaGetLastError());
+  return GH_OK;
+}
+
+extern "C" gh_status gh_set_frame_map(gh_domain* d, const double* Jm, const double* v, int on_device) {
+  DeviceGuard guard_(d);
+  if (!d) return GH_ERR_ARG;
+  if ((Jm == nullptr) != (v == nullptr)) return fail(d, GH_ERR_ARG, "gh_set_frame_map: give both Jm and v, or neither");
+  d->dp_fsal = false;
+  if (!Jm) { d->has_map = false; return GH_OK; }
+  const size_t comp = (size_t)d->pl.S * sizeof(double);
+  const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+  GH_CUDA(d, cudaMemcpyAsync(d->mapJ, Jm, 9 * comp, kind, d->stream));
+  GH_CUDA(d, cudaMemcpyAsync(d->mapv, v, 3 * comp, kind, d->stream));
+  if (!on_device) GH_CUDA(d, cudaStreamSynchronize(d->stream));
+  d->has_map = true;
   return GH_OK;
 }
 

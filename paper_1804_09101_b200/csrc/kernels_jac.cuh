@@ -122,6 +122,82 @@ k_scj(const SubDev* __restrict__ subs, const int32_t* __restrict__ tile_first, i
 }
 
 // ---------------------------------------------------------------------------------------------------------
+// Dual frame (NEXT-4; fields at fixed grid coordinates xbar, equations in inertial coordinates x(xbar, t) with the
+// same time coordinate).  With Jm_i^k = d xbar^k / d x^i and the grid velocity v^i = d x^i / d t at fixed xbar:
+//   d_i u = Jm_i^k dbar_k u   (DiffJac, Eq. 8),     d_t u |_xbar = F[u, d_i u] + v^i d_i u.
+// Two passes around the unchanged fused RHS kernel, launched only while a map is set (the single-frame hot path pays nothing):
+// K_map_pre rewrites the logical derivative scratch so that K_rhs / K_con, which apply the shell's spherical Jacobian A themselves,
+// see inertial-frame derivatives: blocks du <- Jm du; shells du <- (A^-1 Jm A) du.  K_map_post adds coef * v^i d_i u to the output
+// (coef = 1 for d_t u, b dt inside an RK stage, whose update is linear in d_t u) except on FROZEN faces, which hold their grid-frame
+// value.  Both HBM-bound: 2 x 150 and 150 + 2 x 50 doubles per point.
+// ---------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ bool point_frozen(const SubDev& sd, int local) {
+  const int i2 = local % sd.n2, t = local / sd.n2, i1 = t % sd.n1, i0 = t / sd.n1;
+  bool fz = (i0 == 0 && sd.face[0] == 1) || (i0 == sd.n0 - 1 && sd.face[1] == 1);
+  if (sd.kind != 0)
+    fz = fz || (i1 == 0 && sd.face[2] == 1) || (i1 == sd.n1 - 1 && sd.face[3] == 1) || (i2 == 0 && sd.face[4] == 1) || (i2 == sd.n2 - 1 && sd.face[5] == 1);
+  return fz;
+}
+
+__global__ void __launch_bounds__(TILE_PTS)
+k_map_pre(const SubDev* __restrict__ subs, const int32_t* __restrict__ tile_first, int n_sub, const double* __restrict__ tables,
+          const double* __restrict__ mapJ, double* __restrict__ du, int64_t S, int ncomp) {
+  const int sub = find_sub(tile_first, n_sub, blockIdx.x);
+  const SubDev sd = subs[sub];
+  const int local = (blockIdx.x - __ldg(tile_first + sub)) * TILE_PTS + threadIdx.x;
+  if (local >= sd.P) return;
+  const int64_t p = sd.off + local;
+  double M[9];
+  scj_load_j(mapJ, S, p, M);
+  if (sd.kind == 0) {      // M <- A^-1 Jm A with A the logical -> Cartesian Jacobian of Eq. 8
+    const ShellJac J = shell_jac(sd, tables, local);
+    const double A[9] = {J.xr, J.xt, J.xp, J.yr, J.yt, J.yp, J.zr, J.zt, 0.0};
+    // A^-1 from the closed form: d_r = r^ . grad, d_theta = r theta^ . grad, d_phi = r sin(theta) phi^ . grad
+    const double st = sqrt(J.xr * J.xr + J.yr * J.yr), ct = J.zr, r = -st / J.zt;
+    const double cp = J.xr / st, sp = J.yr / st;
+    const double Ai[9] = {st * cp, st * sp, ct, r * ct * cp, r * ct * sp, -r * st, -r * st * sp, r * st * cp, 0.0};
+    double T[9];
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+      for (int k = 0; k < 3; ++k) T[3 * i + k] = M[3 * i] * A[k] + M[3 * i + 1] * A[3 + k] + M[3 * i + 2] * A[6 + k];
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+      for (int k = 0; k < 3; ++k) M[3 * i + k] = Ai[3 * i] * T[k] + Ai[3 * i + 1] * T[3 + k] + Ai[3 * i + 2] * T[6 + k];
+  }
+  const int64_t DS = (int64_t)ncomp * S;
+  for (int c = 0; c < ncomp; ++c) {
+    double* q = du + (int64_t)c * S + p;
+    const double d0 = q[0], d1 = q[DS], d2 = q[2 * DS];
+    q[0] = M[0] * d0 + M[1] * d1 + M[2] * d2;
+    q[DS] = M[3] * d0 + M[4] * d1 + M[5] * d2;
+    q[2 * DS] = M[6] * d0 + M[7] * d1 + M[8] * d2;
+  }
+}
+
+__global__ void __launch_bounds__(TILE_PTS)
+k_map_post(const SubDev* __restrict__ subs, const int32_t* __restrict__ tile_first, int n_sub, const double* __restrict__ tables,
+           const double* __restrict__ mapv, const double* __restrict__ du, double* __restrict__ out, int64_t S, double coef) {
+  const int sub = find_sub(tile_first, n_sub, blockIdx.x);
+  const SubDev sd = subs[sub];
+  const int local = (blockIdx.x - __ldg(tile_first + sub)) * TILE_PTS + threadIdx.x;
+  if (local >= sd.P || point_frozen(sd, local)) return;
+  const int64_t p = sd.off + local;
+  double w0 = coef * __ldg(mapv + p), w1 = coef * __ldg(mapv + S + p), w2 = coef * __ldg(mapv + 2 * S + p);
+  if (sd.kind == 0) {      // v . (A d_logical): fold A into the weights
+    const ShellJac J = shell_jac(sd, tables, local);
+    const double a0 = w0 * J.xr + w1 * J.yr + w2 * J.zr, a1 = w0 * J.xt + w1 * J.yt + w2 * J.zt, a2 = w0 * J.xp + w1 * J.yp;
+    w0 = a0; w1 = a1; w2 = a2;
+  }
+  const int64_t DS = (int64_t)NCOMP * S;
+  for (int c = 0; c < NCOMP; ++c) {
+    const double* q = du + (int64_t)c * S + p;
+    out[(int64_t)c * S + p] += w0 * q[0] + w1 * q[DS] + w2 * q[2 * DS];
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------
 // FP64 peak probe (profiling helper, gh_fp64_peak): register-resident kernels, MODE 0 = DFMA chains (64 independent
 // accumulators per lane group), MODE 1 = DMMA mma.sync.m8n8k4 (8 independent accumulator pairs per warp).  128 flop per lane
 // and iteration in both modes.  The derivative kernels report their roofline fraction against what this measures in the

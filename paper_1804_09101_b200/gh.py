@@ -34,7 +34,7 @@ EXPORTS = [
     "gh_launch_count", "gh_last_error", "gh_basis_cheb", "gh_basis_gauss_legendre", "gh_basis_shell",
     "gh_set_filter", "gh_apply_filter", "gh_filter_sigma",
     "gh_dp5_workspace_bytes", "gh_dp5_attach", "gh_dp5_step", "gh_set_option",
-    "gh_rk_step_norms", "gh_set_jacobian", "gh_spatial_coord_jac", "gh_spatial_coord_jac_state", "gh_fp64_peak",
+    "gh_rk_step_norms", "gh_set_frame_map", "gh_set_jacobian", "gh_spatial_coord_jac", "gh_spatial_coord_jac_state", "gh_fp64_peak",
 ]
 
 
@@ -123,6 +123,7 @@ def lib() -> C.CDLL:
     L.gh_dp5_attach.argtypes = [vp, vp, C.c_size_t]
     L.gh_dp5_step.argtypes = [vp, C.c_double, C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_int)]
     L.gh_set_option.argtypes = [vp, ip, ip]
+    L.gh_set_frame_map.argtypes = [vp, dp, dp, ip]
     L.gh_set_jacobian.argtypes = [vp, dp, ip]
     L.gh_spatial_coord_jac.argtypes = [vp, ip, dp, dp, ip]
     L.gh_spatial_coord_jac_state.argtypes = [vp]
@@ -285,6 +286,14 @@ def gh_dp5_step(h, dt: float, tol: float = 0.0):
     acc = C.c_int(0)
     _check(lib().gh_dp5_step(h, float(dt), float(tol), err, C.byref(acc)), h)
     return float(err[0]), float(err[1]), bool(acc.value)
+
+
+def gh_set_frame_map(h, Jm=None, v=None):
+    p, dev = _ptr(Jm)
+    q, dev2 = _ptr(v)
+    if Jm is not None and v is not None and dev != dev2:
+        raise ValueError("Jm and v must live on the same side")
+    _check(lib().gh_set_frame_map(h, p, q, dev), h)
 
 
 def gh_set_jacobian(h, J):
@@ -470,6 +479,10 @@ class Domain:
     @_ordered
     def apply_filter(self):
         gh_apply_filter(self.h)
+
+    @_ordered
+    def set_frame_map(self, Jm=None, v=None):
+        gh_set_frame_map(self.h, Jm, v)
 
     @_ordered
     def set_jacobian(self, J):
