@@ -33,6 +33,70 @@ struct CompMap {
   __device__ __forceinline__ int map(int c) const { return c < skip_lo ? c : c + skip_n; }
 };
 
+// The component walk of one warp with EXACT compile-time tile counts MT = ceil(N/8), KS = ceil(N/4) (KS = 2 MT - 1 or 2 MT): guards
+// inside unrolled loops (`if (ks < KS)`) compile to predicated DMMAs, which still take their issue and pipe slots when switched
+// off - for N = 16 in the N <= 24 class that was 10 of 18 DMMAs per k-sweep (ncu / cuobjdump, profiles/r02_ncu_k_ang.md §2 a).
+template <int MT, int KS, int NTW>
+__device__ __forceinline__ void cheb_body(const ChebItem& it, const double* __restrict__ sm, const double* __restrict__ in,
+                                          double* __restrict__ out, int64_t S, int ncomp, const CompMap& cm, int si0,
+                                          const int (&caddr)[NTW], const bool (&cok)[NTW], const int (&c0a)[NTW],
+                                          const int (&c1a)[NTW], bool pair, int wc0, int lane) {
+  const int g = lane >> 2, tl = lane & 3, N = it.N, ncols = it.ncols;
+  // the CTA walks over components blockIdx.y, blockIdx.y + gridDim.y, ... (one launch and one matrix load for all of them)
+#pragma unroll 1
+  for (int cw = blockIdx.y; cw < ncomp; cw += gridDim.y) {
+    const int comp = cm.map(cw);
+    // B fragments of the whole warp tile.  (si is laundered so that the compiler recomputes the 2 x KS x NTW element
+    // offsets per component instead of keeping them all live across the loop: that costs 40 registers and a CTA per SM)
+    int si = si0;
+    asm volatile("" : "+r"(si));
+    double b[KS][NTW];
+    {
+      const double* __restrict__ src = in + (int64_t)comp * S + it.base;
+#pragma unroll
+      for (int ks = 0; ks < KS; ++ks) {
+        const int i = ks * 4 + tl;
+#pragma unroll
+        for (int n = 0; n < NTW; ++n) b[ks][n] = (cok[n] && i < N) ? src[caddr[n] + i * si] : 0.0;
+      }
+    }
+    double acc[MT][NTW][2];
+#pragma unroll
+    for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+      for (int n = 0; n < NTW; ++n) acc[mt][n][0] = acc[mt][n][1] = 0.0;
+#pragma unroll
+    for (int ks = 0; ks < KS; ++ks)
+#pragma unroll
+      for (int mt = 0; mt < MT; ++mt) {
+        const double a = sm[(mt * KS + ks) * 32 + lane];
+#pragma unroll
+        for (int n = 0; n < NTW; ++n) dmma884(acc[mt][n][0], acc[mt][n][1], a, b[ks][n]);
+      }
+    // C fragments: row a = 8 mt + g, columns 8 n + 2 tl and + 1
+    double* __restrict__ dst = out + ((int64_t)it.axis * cm.total + comp) * S + it.base;
+#pragma unroll
+    for (int n = 0; n < NTW; ++n) {
+      const int c = wc0 + n * 8 + 2 * tl;
+      const bool ok0 = c < ncols, ok1 = c + 1 < ncols;
+#pragma unroll
+      for (int mt = 0; mt < MT; ++mt) {
+        const int a = mt * 8 + g;
+        if (a < N) {
+          if (pair && ok1) {
+            *reinterpret_cast<double2*>(dst + c0a[n] + a * si) = make_double2(acc[mt][n][0], acc[mt][n][1]);
+          } else {
+            if (ok0) dst[c0a[n] + a * si] = acc[mt][n][0];
+            if (ok1) dst[c1a[n] + a * si] = acc[mt][n][1];
+          }
+        }
+      }
+    }
+  }
+}
+
+// MTM / KSM: the largest tile counts of the launch's register class (they size the registers: launch bounds); the body runs with the
+// item's exact counts.
 template <int TPB, int MTM, int KSM, int NTW>
 __global__ void __launch_bounds__(TPB, (MTM * NTW >= 16) ? 3 : (MTM * NTW >= 12) ? 4 : (MTM * NTW >= 8) ? 5 : 7)
 k_cheb(const ChebItem* __restrict__ items, const double* __restrict__ tables, const double* __restrict__ in,
@@ -68,62 +132,16 @@ k_cheb(const ChebItem* __restrict__ items, const double* __restrict__ tables, co
 
   __syncthreads();
   if (wc0 >= ncols) return;
-
-  // the CTA walks over components blockIdx.y, blockIdx.y + gridDim.y, ... (one launch and one matrix load for all of them)
-#pragma unroll 1
-  for (int cw = blockIdx.y; cw < ncomp; cw += gridDim.y) {
-    const int comp = cm.map(cw);
-    // B fragments of the whole warp tile.  (si is laundered so that the compiler recomputes the 2 x KS x NTW element
-    // offsets per component instead of keeping them all live across the loop: that costs 40 registers and a CTA per SM)
-    int si = si0;
-    asm volatile("" : "+r"(si));
-    double b[KSM][NTW];
-    {
-      const double* __restrict__ src = in + (int64_t)comp * S + it.base;
-#pragma unroll
-      for (int ks = 0; ks < KSM; ++ks)
-        if (ks < KS) {
-          const int i = ks * 4 + tl;
-#pragma unroll
-          for (int n = 0; n < NTW; ++n) b[ks][n] = (cok[n] && i < N) ? src[caddr[n] + i * si] : 0.0;
-        }
-    }
-    double acc[MTM][NTW][2];
-#pragma unroll
-    for (int mt = 0; mt < MTM; ++mt)
-#pragma unroll
-      for (int n = 0; n < NTW; ++n) acc[mt][n][0] = acc[mt][n][1] = 0.0;
-#pragma unroll
-    for (int ks = 0; ks < KSM; ++ks)
-      if (ks < KS) {
-#pragma unroll
-        for (int mt = 0; mt < MTM; ++mt)
-          if (mt < MTn) {
-            const double a = sm[(mt * KS + ks) * 32 + lane];
-#pragma unroll
-            for (int n = 0; n < NTW; ++n) dmma884(acc[mt][n][0], acc[mt][n][1], a, b[ks][n]);
-          }
-      }
-    // C fragments: row a = 8 mt + g, columns 8 n + 2 tl and + 1
-    double* __restrict__ dst = out + ((int64_t)it.axis * cm.total + comp) * S + it.base;
-#pragma unroll
-    for (int n = 0; n < NTW; ++n) {
-      const int c = wc0 + n * 8 + 2 * tl;
-      const bool ok0 = c < ncols, ok1 = c + 1 < ncols;
-#pragma unroll
-      for (int mt = 0; mt < MTM; ++mt) {
-        const int a = mt * 8 + g;
-        if (mt < MTn && a < N) {
-          if (pair && ok1) {
-            *reinterpret_cast<double2*>(dst + c0a[n] + a * si) = make_double2(acc[mt][n][0], acc[mt][n][1]);
-          } else {
-            if (ok0) dst[c0a[n] + a * si] = acc[mt][n][0];
-            if (ok1) dst[c1a[n] + a * si] = acc[mt][n][1];
-          }
-        }
-      }
-    }
-  }
+  // exact tile counts of this item: KS = KSM - d, MT = ceil(KS / 2), for the (at most six) counts of the class
+#define GH_CHEB_BODY(K) cheb_body<((K) + 1) / 2, (K), NTW>(it, sm, in, out, S, ncomp, cm, si0, caddr, cok, c0a, c1a, pair, wc0, lane)
+  constexpr int KLO = KSM == 6 ? 1 : KSM == 8 ? 7 : KSM == 12 ? 9 : 13;     // smallest KS of the class (N <= 24 | 32 | 48 | 64)
+  if (KS == KSM) GH_CHEB_BODY(KSM);
+  else if (KSM - 1 >= KLO && KS == KSM - 1) GH_CHEB_BODY(KSM - 1 >= 1 ? KSM - 1 : 1);
+  else if (KSM - 2 >= KLO && KS == KSM - 2) GH_CHEB_BODY(KSM - 2 >= 1 ? KSM - 2 : 1);
+  else if (KSM - 3 >= KLO && KS == KSM - 3) GH_CHEB_BODY(KSM - 3 >= 1 ? KSM - 3 : 1);
+  else if (KSM - 4 >= KLO && KS == KSM - 4) GH_CHEB_BODY(KSM - 4 >= 1 ? KSM - 4 : 1);
+  else GH_CHEB_BODY(KSM - 5 >= 1 ? KSM - 5 : 1);
+#undef GH_CHEB_BODY
 }
 
 __device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc) {
