@@ -84,7 +84,7 @@ typedef struct {
  * kernels keep the whole contraction of a line / a (theta,phi) plane on chip (K_cheb, K_ang); beyond, up to the maxima, the
  * same linear maps run as tiled FP64 tensor-core GEMMs whose cached matrices stream through shared memory (K_gemm) - the upper
  * two decades of the size sweep, BASELINE.json configs[4] (N = 320, L = 255: 3.3e7 points per subdomain).  The spectral filter
- * (gh_set_filter) is built for the small classes only. */
+ * (gh_set_filter) covers both classes the same way (filter matrices in place of differentiation matrices). */
 #define GH_MAX_CHEB_N 512   /* largest N on a Chebyshev axis */
 #define GH_MAX_L 255        /* largest shell band limit L */
 #define GH_SMALL_CHEB_N 64

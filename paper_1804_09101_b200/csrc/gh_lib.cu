@@ -41,7 +41,8 @@ constexpr int ANG_NB_MAX_SMALL_L = 24;           // ... for L < 12, where a plan
                                                  // per 2e6 points; for L >= 12 more than 8 planes measured slightly slower on C4)
 constexpr size_t SMEM_MAX = 227 * 1024;
 constexpr int GEMM_MB = 16;                      // m-tiles per M-block of K_gemm (tiles beyond the matrix are skipped at run time)
-enum { G_S1 = 0, G_S2 = 1, G_S3T = 2, G_S3P = 3, G_CHEB = 4, G_NLIST = 5 };   // K_gemm launch lists, in launch order
+enum { G_S1 = 0, G_S2 = 1, G_S3T = 2, G_S3P = 3, G_CHEB = 4, G_NDERIV = 5,      // K_gemm launch lists of the derivatives, in launch order
+       G_FX = 5, G_FY = 6, G_FZ = 7, G_FS2 = 8, G_FS3 = 9, G_NLIST = 10 };        // ... and of the spectral filter (block axes; shell composites and synthesis)
 inline bool big_N(int N) { return N > GH_SMALL_CHEB_N; }
 inline bool big_L(int L) { return L > GH_SMALL_L; }
 
@@ -67,7 +68,8 @@ struct Plan {
   int n_cheb_items = 0, n_cheb_class[CHEB_NCLASS] = {}, n_ang_items = 0;
   int n_ang_class[2] = {0, 0};           // K_ang items per shared-memory class (0: two CTAs per SM, 1: one)
   size_t cheb_smem = 0, ang_smem[2] = {0, 0};
-  int n_gemm[G_NLIST] = {0, 0, 0, 0, 0};  // K_gemm items per launch list (large subdomains)
+  int n_gemm[G_NLIST] = {0};             // K_gemm items per launch list (large subdomains)
+  size_t fbigtab_doubles = 0;            // filter matrices of the large classes, behind the interface tables (written by gh_set_filter)
   size_t bigtab_doubles = 0;             // their blocked fragment matrices, behind the filter tables
   bool has_big = false;
   int n_ifc_items = 0;                   // interface faces whose neighbour has a different band limit (K_face_interp)
@@ -121,6 +123,19 @@ inline size_t shell_t_doubles(int L) {    // [m][k_step < NT][even|odd][m_tile <
 inline size_t shell_matrix_doubles(int L) { return shell_fa_doubles(L) + shell_fs_doubles(L) + shell_t_doubles(L); }
 inline size_t shell_g_doubles(int L) {    // [m][k_step < NT][even|odd][m_tile < ceil(NT/2)][32]: equator-folded filtered projectors (hh rows)
   return (size_t)(L + 1) * c_gm(ang_nt_class(L));
+}
+
+// elem(row, col) of an (M x K) matrix -> K_gemm's A-fragment order, blocked [m_block][k_chunk][mbs m-tiles][GEMM_KB k-steps][32]
+// (zero padded), into dst[0 .. gemm_amat_doubles(M, K, GEMM_MB))
+template <class F>
+void fill_amat(double* dst, int M, int K, F elem) {
+  const int MT = (M + 7) / 8, KS = (K + 3) / 4, mbs = gemm_mbs(M, GEMM_MB), nMB = (MT + mbs - 1) / mbs, nKC = (KS + GEMM_KB - 1) / GEMM_KB;
+  std::fill(dst, dst + gemm_amat_doubles(M, K, GEMM_MB), 0.0);
+  for (int mb = 0; mb < nMB; ++mb) for (int kc = 0; kc < nKC; ++kc) for (int mt = 0; mt < mbs; ++mt) for (int ks = 0; ks < GEMM_KB; ++ks)
+    for (int lane = 0; lane < 32; ++lane) {
+      const int row = (mb * mbs + mt) * 8 + lane / 4, col = (kc * GEMM_KB + ks) * 4 + lane % 4;
+      if (row < M && col < K) dst[((((size_t)mb * nKC + kc) * mbs + mt) * GEMM_KB + ks) * 32 + lane] = (double)elem(row, col);
+    }
 }
 
 bool validate(const gh_subdomain_desc* descs, int32_t n_sub, std::string& err) {
@@ -191,6 +206,7 @@ bool make_plan(const gh_subdomain_desc* descs, int32_t n_sub, Plan& pl, std::str
       if (big_N(N)) {       // tiled GEMM path
         pl.bigtab_doubles += gemm_amat_doubles(N, N, GEMM_MB);
         pl.n_gemm[G_CHEB] += (int)((cols + GEMM_CT - 1) / GEMM_CT);
+        if (d.kind == GH_BLOCK) { pl.fbigtab_doubles += gemm_amat_doubles(N, N, GEMM_MB); pl.n_gemm[G_FX + a] += (int)((cols + GEMM_CT - 1) / GEMM_CT); }
         pl.has_big = true;
         continue;
       }
@@ -219,11 +235,15 @@ bool make_plan(const gh_subdomain_desc* descs, int32_t n_sub, Plan& pl, std::str
           seenL[L] = 1;
           pl.bigtab_doubles += gemm_amat_doubles(nq, np, GEMM_MB) + 2 * gemm_amat_doubles(np, nq, GEMM_MB) +
                                (size_t)(L + 1) * 2 * gemm_amat_doubles(nt, nt, GEMM_MB);
+          pl.fbigtab_doubles += (size_t)(L + 1) * gemm_amat_doubles(nt, nt, GEMM_MB);
         }
         const int64_t R = (int64_t)n0 * nt;
         const int rt = (int)((R + GEMM_CT - 1) / GEMM_CT);
-        pl.n_gemm[G_S1] += rt; pl.n_gemm[G_S3T] += rt; pl.n_gemm[G_S3P] += rt;
-        for (int m = 0; m <= L; ++m) pl.n_gemm[G_S2] += 2 * (((m ? 2 : 1) * n0 + GEMM_CT - 1) / GEMM_CT);
+        pl.n_gemm[G_S1] += rt; pl.n_gemm[G_S3T] += rt; pl.n_gemm[G_S3P] += rt; pl.n_gemm[G_FS3] += rt;
+        for (int m = 0; m <= L; ++m) {
+          const int ct = ((m ? 2 : 1) * n0 + GEMM_CT - 1) / GEMM_CT;
+          pl.n_gemm[G_S2] += 2 * ct; pl.n_gemm[G_FS2] += ct;
+        }
         pl.has_big = true;
         continue;
       }
@@ -261,7 +281,7 @@ bool make_plan(const gh_subdomain_desc* descs, int32_t n_sub, Plan& pl, std::str
   pl.o_ua = c.take(NCOMP * comp); pl.o_ub = c.take(NCOMP * comp); pl.o_k = c.take(NCOMP * comp);
   pl.o_du = c.take(3 * NCOMP * comp); pl.o_H = c.take(4 * comp); pl.o_dH = c.take(12 * comp);
   pl.o_jac = c.take(9 * comp); pl.o_mapJ = c.take(9 * comp); pl.o_mapv = c.take(3 * comp);
-  pl.o_tables = c.take((pl.table_doubles + pl.ftable_doubles + pl.bigtab_doubles + pl.ifctab_doubles) * sizeof(double));
+  pl.o_tables = c.take((pl.table_doubles + pl.ftable_doubles + pl.bigtab_doubles + pl.ifctab_doubles + pl.fbigtab_doubles) * sizeof(double));
   pl.o_ifc = c.take((size_t)std::max<int64_t>(1, NCOMP * pl.Sf) * sizeof(double));
   pl.o_ifci = c.take((size_t)std::max(1, pl.n_ifc_items) * sizeof(IfcItem));
   pl.o_subs = c.take((size_t)n_sub * sizeof(SubDev));
@@ -298,6 +318,9 @@ struct gh_domain {
   struct FBlock { int N; double unused; size_t off; };     // one filter matrix slot per (block, axis): offset (doubles) from `tables`
   std::vector<FBlock> f_blocks;
   std::map<int, size_t> f_L;             // shell band limit L -> offset (doubles) of its filtered projectors from `tables`
+  struct FBig { int N; size_t off; };     // large classes: one K_gemm filter matrix slot per (block, large axis) ...
+  std::vector<FBig> f_big_blocks;
+  std::map<int, std::vector<size_t>> f_big_L;   // ... and per large L the slots of its per-m filtered projectors
   bool filt_blocks = false, filt_shells = false;
   // Dormand-Prince 5(4): seven stage derivatives in a separately attached workspace
   double* dpk[7] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
@@ -459,17 +482,14 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
   // elem(row, col) of an (M x K) matrix -> A-fragment order, blocked [m_block][k_chunk][GEMM_MB m-tiles][GEMM_KB k-steps][32];
   // returns the offset (doubles) of the matrix from d->tables
   auto put_amat = [&](int M, int K, auto elem) {
-    const int MT = (M + 7) / 8, KS = (K + 3) / 4, mbs = gemm_mbs(M, GEMM_MB), nMB = (MT + mbs - 1) / mbs, nKC = (KS + GEMM_KB - 1) / GEMM_KB;
     const size_t at = btp;
-    for (int mb = 0; mb < nMB; ++mb) for (int kc = 0; kc < nKC; ++kc) for (int mt = 0; mt < mbs; ++mt) for (int ks = 0; ks < GEMM_KB; ++ks)
-      for (int lane = 0; lane < 32; ++lane) {
-        const int row = (mb * mbs + mt) * 8 + lane / 4, col = (kc * GEMM_KB + ks) * 4 + lane % 4;
-        if (row < M && col < K)
-          bigtab[at + ((((size_t)mb * nKC + kc) * mbs + mt) * GEMM_KB + ks) * 32 + lane] = (double)elem(row, col);
-      }
+    fill_amat(bigtab.data() + at, M, K, elem);
     btp += gemm_amat_doubles(M, K, GEMM_MB);
     return (int64_t)(big0 + at);
   };
+  // filter matrices of the large classes: slots behind the interface tables, filled by gh_set_filter
+  const size_t fbig0 = pl.table_doubles + pl.ftable_doubles + pl.bigtab_doubles + pl.ifctab_doubles;
+  size_t fbp = 0;
   // one K_gemm item per tile of GEMM_CT columns
   auto put_items = [&](int list, GemmItem proto, int64_t cols) {
     // columns (c, c + 1), c even, may leave as one double2 when they are neighbours in memory at an even address
@@ -557,6 +577,13 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
         else { it.in_inner = 1; it.in_outer = nn[2]; it.in_cs = 0; }
         it.out_inner = it.in_inner; it.out_outer = it.in_outer; it.out_cs = it.in_cs;
         put_items(G_CHEB, it, sd.P / N);
+        if (de.kind == GH_BLOCK) {      // the same strided view with the filter matrix: x: u -> T1 (slot 0), y: T1 -> T2 (slot 1), z: T2 -> u
+          GemmItem fi = it;
+          fi.amat = (int64_t)(fbig0 + fbp);
+          fi.in_slot = a == 0 ? -1 : a - 1; fi.out_slot = a == 2 ? -1 : a;
+          d->f_big_blocks.push_back({N, fbig0 + fbp}); fbp += gemm_amat_doubles(N, N, GEMM_MB);
+          put_items(G_FX + a, fi, sd.P / N);
+        }
         continue;
       }
       const int dm = (int)tp;
@@ -634,6 +661,21 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
       it.out_base = sd.off; it.out_sa = 1; it.out_inner = (int)BIG; it.out_cs = np;
       it.amat = o.FsQ; it.in_slot = 2; it.out_slot = 1; put_items(G_S3T, it, R);
       it.amat = o.FpQ; it.in_slot = 0; it.out_slot = 2; put_items(G_S3P, it, R);
+      // spectral filter of a large shell: S1 as above (u -> W in slot 1), per m the filtered projector G_m W -> slot 2, synthesis -> u
+      it.amat = o.FsQ; it.in_slot = 2; it.out_slot = -1; put_items(G_FS3, it, R);
+      if (!d->f_big_L.count(L)) {
+        std::vector<size_t> offs;
+        for (int m = 0; m <= L; ++m) { offs.push_back(fbig0 + fbp); fbp += gemm_amat_doubles(nt, nt, GEMM_MB); }
+        d->f_big_L[L] = offs;
+      }
+      for (int m = 0; m <= L; ++m) {
+        const int64_t q0 = m == 0 ? 0 : 2 * m - 1, cols = (m ? 2 : 1) * (int64_t)n0;
+        memset(&it, 0, sizeof it);
+        it.M = nt; it.K = nt; it.in_slot = 1; it.out_slot = 2;
+        it.in_base = it.out_base = sd.off + q0 * R; it.in_sk = it.out_sa = 1;
+        it.in_inner = it.out_inner = (int)BIG; it.in_cs = it.out_cs = nt;
+        it.amat = (int64_t)d->f_big_L[L][m]; put_items(G_FS2, it, cols);
+      }
     }
     if (de.kind == GH_SHELL) {
       // coordinate tables of this shell (for the Jacobian of Eq. 8)
@@ -740,7 +782,7 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
   std::vector<GemmItem> gemm;
   bool gemm_ok = btp == pl.bigtab_doubles;
   for (int l = 0; l < G_NLIST; ++l) { gemm_ok = gemm_ok && (int)glist[l].size() == pl.n_gemm[l]; gemm.insert(gemm.end(), glist[l].begin(), glist[l].end()); }
-  gemm_ok = gemm_ok && itp == pl.ifctab_doubles && (int)ifci.size() == pl.n_ifc_items && ifc_next == pl.Sf;
+  gemm_ok = gemm_ok && fbp == pl.fbigtab_doubles && itp == pl.ifctab_doubles && (int)ifci.size() == pl.n_ifc_items && ifc_next == pl.Sf;
   if (tp != pl.table_doubles || (int)cheb.size() != pl.n_cheb_items || (int)ang.size() != pl.n_ang_items || !gemm_ok ||
       (int)fcheb.size() != pl.n_fcheb_items || ftp != pl.table_doubles + pl.ftable_doubles) {
     delete d; return fail(nullptr, GH_ERR_STATE, "internal: plan and build disagree");
@@ -878,6 +920,19 @@ void launch_cheb_class(gh_domain* d, int prof_cls, int c, const ChebItem* items,
   else k_cheb<CHEB_TPB, 8, 16, CHEB_NTW><<<grid, CHEB_TPB, pl.cheb_smem, d->stream>>>(items, d->tables, in, out, pl.S, nrun, cm);
 }
 
+// one K_gemm launch over launch list l (the items of the lists lie one after another in d->gemm)
+void launch_gemm_list(gh_domain* d, int prof_cls, int l, const double* in, double* out, int nrun, const CompMap& cm) {
+  const Plan& pl = d->pl;
+  if (!pl.n_gemm[l]) return;
+  int first = 0;
+  for (int k = 0; k < l; ++k) first += pl.n_gemm[k];
+  int gw = 1;     // components one CTA walks over: as many as still leave two CTAs per SM in the grid
+  for (int w = 10; w >= 1; --w)
+    if (nrun % w == 0 && (w == 1 || (int64_t)pl.n_gemm[l] * (nrun / w) >= 2 * d->n_sm)) { gw = w; break; }
+  ProfScope ps(d, prof_cls);
+  k_gemm<GEMM_MB><<<dim3(pl.n_gemm[l], nrun / gw), GEMM_TPB, gemm_smem_bytes(GEMM_MB), d->stream>>>(d->gemm + first, d->tables, in, out, pl.S, nrun, cm);
+}
+
 gh_status launch_derivs(gh_domain* d, const double* in, double* out, int ncomp, int skip_lo = 0, int skip_n = 0) {
   const Plan& pl = d->pl;
   const CompMap cm{ncomp, skip_lo, skip_n};        // `in` / `out` have ncomp components, of which skip_n are left out
@@ -886,16 +941,8 @@ gh_status launch_derivs(gh_domain* d, const double* in, double* out, int ncomp, 
   // ... but small domains need the CTAs more than the amortisation: keep at least ~4 CTAs per SM in the grid
   // large subdomains: the K_gemm lists in order (S1, S2, S3 theta, S3 phi of the large shells, then the large Chebyshev axes -
   // the radial one writes slot 0, which S2 / S3 used as a coefficient buffer)
-  if (pl.has_big) {
-    for (int l = 0, first = 0; l < G_NLIST; first += pl.n_gemm[l], ++l) {
-      if (!pl.n_gemm[l]) continue;
-      int gw = 1;     // components one CTA walks over: as many as still leave two CTAs per SM in the grid
-      for (int w = 10; w >= 1; --w)
-        if (nrun % w == 0 && (w == 1 || (int64_t)pl.n_gemm[l] * (nrun / w) >= 2 * d->n_sm)) { gw = w; break; }
-      ProfScope ps(d, l == G_CHEB ? GH_K_CHEB : GH_K_SHELL_ANG);
-      k_gemm<GEMM_MB><<<dim3(pl.n_gemm[l], nrun / gw), GEMM_TPB, gemm_smem_bytes(GEMM_MB), d->stream>>>(d->gemm + first, d->tables, in, out, pl.S, nrun, cm);
-    }
-  }
+  if (pl.has_big)
+    for (int l = 0; l < G_NDERIV; ++l) launch_gemm_list(d, l == G_CHEB ? GH_K_CHEB : GH_K_SHELL_ANG, l, in, out, nrun, cm);
   int walk = 1;
   for (int w = CHEB_COMP_WALK; w >= 1; --w)
     if (nrun % w == 0 && (w == 1 || (int64_t)pl.n_cheb_items * (nrun / w) >= 4 * d->n_sm)) { walk = w; break; }
@@ -1210,9 +1257,32 @@ extern "C" gh_status gh_set_filter(gh_domain* d, const gh_filter_desc* fb, const
   std::vector<double> ft(pl.ftable_doubles, 0.0);
   const size_t base = pl.table_doubles;
   std::vector<ghb::ld> sg, M;
-  const bool on_b = fb && fb->kind != GH_FILTER_NONE && !d->f_blocks.empty();
-  const bool on_s = fs && fs->kind != GH_FILTER_NONE && !d->f_L.empty();
-  if ((on_b || on_s) && pl.has_big) return fail(d, GH_ERR_ARG, "the spectral filter is built for subdomains with N <= 64 and L <= 47 only");
+  const bool on_b = fb && fb->kind != GH_FILTER_NONE && !(d->f_blocks.empty() && d->f_big_blocks.empty());
+  const bool on_s = fs && fs->kind != GH_FILTER_NONE && !(d->f_L.empty() && d->f_big_L.empty());
+  // large classes: the same matrices, unfolded, in K_gemm's blocked fragment order
+  std::vector<double> fbig(pl.fbigtab_doubles, 0.0);
+  const size_t fbig0 = pl.table_doubles + pl.ftable_doubles + pl.bigtab_doubles + pl.ifctab_doubles;
+  if (on_b) {
+    std::map<int, std::vector<ghb::ld>> cache;
+    for (const auto& b : d->f_big_blocks) {
+      const int N = b.N;
+      if (!cache.count(N)) {
+        if (!filter_sigma(fb, N - 1, sg)) return fail(d, GH_ERR_ARG, "bad block filter descriptor");
+        ghb::cheb_filter_matrix(N, sg, cache[N]);
+      }
+      const std::vector<ghb::ld>& F = cache[N];
+      fill_amat(fbig.data() + (b.off - fbig0), N, N, [&](int r, int c) { return F[(size_t)r * N + c]; });
+    }
+  }
+  if (on_s) {
+    for (const auto& kv : d->f_big_L) {
+      const int L = kv.first, nt = L + 1;
+      if (!filter_sigma(fs, L, sg)) return fail(d, GH_ERR_ARG, "bad shell filter descriptor");
+      ghb::shell_filter_composites(L, sg, M);
+      for (int m = 0; m <= L; ++m)
+        fill_amat(fbig.data() + (kv.second[m] - fbig0), nt, nt, [&](int r, int c) { return M[((size_t)m * nt + r) * nt + c]; });
+    }
+  }
   if (on_b) {
     std::map<int, std::vector<ghb::ld>> cache;      // N -> filter matrix
     for (const auto& b : d->f_blocks) {
@@ -1250,10 +1320,9 @@ extern "C" gh_status gh_set_filter(gh_domain* d, const gh_filter_desc* fb, const
         }
     }
   }
-  if (pl.ftable_doubles) {
-    GH_CUDA(d, cudaMemcpyAsync(d->tables + base, ft.data(), ft.size() * sizeof(double), cudaMemcpyHostToDevice, d->stream));
-    GH_CUDA(d, cudaStreamSynchronize(d->stream));
-  }
+  if (pl.ftable_doubles) GH_CUDA(d, cudaMemcpyAsync(d->tables + base, ft.data(), ft.size() * sizeof(double), cudaMemcpyHostToDevice, d->stream));
+  if (pl.fbigtab_doubles) GH_CUDA(d, cudaMemcpyAsync(d->tables + fbig0, fbig.data(), fbig.size() * sizeof(double), cudaMemcpyHostToDevice, d->stream));
+  GH_CUDA(d, cudaStreamSynchronize(d->stream));      // the host staging vectors die at return
   d->filt_blocks = on_b; d->filt_shells = on_s;
   return GH_OK;
 }
@@ -1277,9 +1346,14 @@ extern "C" gh_status gh_apply_filter(gh_domain* d) {
     for (int a = 0; a < 3; ++a) {
       for (int c = 0; c < CHEB_NCLASS; first += pl.n_fcheb[a][c], ++c)
         launch_cheb_class(d, GH_K_FILTER_CHEB, c, d->fcheb + first, pl.n_fcheb[a][c], gy, src[a], dst[a], NCOMP, cm);
+      launch_gemm_list(d, GH_K_FILTER_CHEB, G_FX + a, d->ua, d->du, NCOMP, cm);     // large axes: the items name the same slots
     }
   }
   if (d->filt_shells) {
+    // large shells: analysis (the derivative path's S1 list), per m the filtered projector, synthesis back into the state
+    launch_gemm_list(d, GH_K_FILTER_ANG, G_S1, d->ua, d->du, NCOMP, cm);
+    launch_gemm_list(d, GH_K_FILTER_ANG, G_FS2, d->ua, d->du, NCOMP, cm);
+    launch_gemm_list(d, GH_K_FILTER_ANG, G_FS3, d->ua, d->du, NCOMP, cm);
     for (int cls = 0, first = 0; cls < 2; first += pl.n_ang_class[cls], ++cls) {
       if (!pl.n_ang_class[cls]) continue;
       ProfScope ps(d, GH_K_FILTER_ANG);

@@ -29,7 +29,7 @@ struct GemmItem {
   int32_t M, K;
   int32_t col0, ncols;
   int64_t amat;                  // offset (doubles, even) of the blocked fragment matrix in the table memory
-  int32_t in_slot, out_slot;     // -1: the kernel's `in` array; 0..2: slot of the derivative scratch [3][total][S]
+  int32_t in_slot, out_slot;     // -1: the kernel's `in` array (as output: the spectral filter writes the state back); 0..2: slot of the derivative scratch [3][total][S]
   int32_t pair;                  // 1: Out columns are contiguous and 16-byte aligned in pairs (double2 stores)
   int32_t mbs;                   // m-tiles per M-block (<= MB): the m-tiles are spread evenly over the fewest blocks
 };
@@ -125,7 +125,7 @@ k_gemm(const GemmItem* __restrict__ items, const double* __restrict__ tables, co
   };
   auto out_ptr = [&](int cw) {
     const int comp = cm.map((int)blockIdx.y + cw * (int)gridDim.y);
-    return dub + it.out_slot * slot_stride + (int64_t)comp * S + it.out_base;
+    return (it.out_slot < 0 ? const_cast<double*>(in) : dub + it.out_slot * slot_stride) + (int64_t)comp * S + it.out_base;
   };
   auto load_b = [&](int t, double (&b)[KB][NTW]) {
     const int cw = t / per, kc = (t % per) % nKC;
