@@ -70,11 +70,11 @@ typedef long double real;
 #endif
 
 typedef struct {
-  int32_t kind;      /* 0 = shell (I1 x S2), 1 = block (I1^3) */
-  int32_t n[3];      /* shell: {N_r, L, unused}; block: {N_x, N_y, N_z} */
-  double lo[3], hi[3]; /* shell: lo[0]=r_in, hi[0]=r_out; block: corners */
-  double center[3];  /* shell centre */
-  int32_t face[6];   /* 1 = FROZEN. shell: [0]=inner,[1]=outer; block: -x,+x,-y,+y,-z,+z */
+  int32_t kind;      /* 0 = shell (I1 x S2), 1 = block (I1^3), 2 = cylindrical shell (O15: I1 x I1 x S1, axis along z) */
+  int32_t n[3];      /* shell: {N_r, L, unused}; block: {N_x, N_y, N_z}; cylinder: {N_rho, N_z, N_phi} */
+  double lo[3], hi[3]; /* shell: lo[0]=r_in, hi[0]=r_out; block: corners; cylinder: [0] = rho_in / rho_out, [1] = z range (rel. to centre) */
+  double center[3];  /* shell centre; cylinder: a point of the axis */
+  int32_t face[6];   /* 1 = FROZEN. shell: [0]=inner,[1]=outer; block: -x,+x,-y,+y,-z,+z; cylinder: rho_in, rho_out, z_lo, z_hi */
   double gamma[3];   /* constraint damping gamma0, gamma1, gamma2 */
 } ora_subdomain;
 
@@ -145,6 +145,20 @@ void ora_coords(const ora_subdomain* sd, double* xyz) {
       xyz[2 * P + p] = (double)((real)sd->center[2] + r * ct[j]);
     }
     free(xr); free(ct); free(w);
+  } else if (sd->kind == 2) {
+    /* O15: rho on Chebyshev-Gauss-Lobatto nodes of [rho_in, rho_out], z likewise, phi_k = 2 pi k / N_phi; phi fastest */
+    real* xr = malloc(sizeof(real) * n0); cgl_nodes(n0, xr);
+    real* xz = malloc(sizeof(real) * n1); cgl_nodes(n1, xz);
+    for (int i = 0; i < n0; ++i) for (int j = 0; j < n1; ++j) for (int k = 0; k < n2; ++k) {
+      real rho = (real)sd->lo[0] + ((real)sd->hi[0] - (real)sd->lo[0]) * (xr[i] + 1) / 2;
+      real z = (real)sd->lo[1] + ((real)sd->hi[1] - (real)sd->lo[1]) * (xz[j] + 1) / 2;
+      real ph = 2 * R_PI * (real)k / (real)n2;
+      int64_t p = ((int64_t)i * n1 + j) * n2 + k;
+      xyz[p] = (double)((real)sd->center[0] + rho * R_COS(ph));
+      xyz[P + p] = (double)((real)sd->center[1] + rho * R_SIN(ph));
+      xyz[2 * P + p] = (double)((real)sd->center[2] + z);
+    }
+    free(xr); free(xz);
   } else {
     real* x[3]; int nn[3] = {n0, n1, n2};
     for (int d = 0; d < 3; ++d) { x[d] = malloc(sizeof(real) * nn[d]); cgl_nodes(nn[d], x[d]); }
@@ -190,6 +204,56 @@ void ora_cheb_derivative_line(int N, const double* u, double* du) {
   real* a = malloc(sizeof(real) * N); real* b = malloc(sizeof(real) * N);
   for (int j = 0; j < N; ++j) a[j] = u[j];
   cheb_line(N, a, 1, b, 1);
+  for (int j = 0; j < N; ++j) du[j] = (double)b[j];
+  free(a); free(b);
+}
+
+/* ---------------------------------------------------------------------- */
+/* O15 — Fourier derivative / filter of one periodic line (the S1 factor  */
+/* of the cylindrical shells the paper names for binary runs,             */
+/* PAPER.md:79, 564; it gives no formulas: DESIGN.md reading S25).  The   */
+/* same three steps as Eqs. 14-18 with the basis e^{i m phi}:             */
+/*  (a) PhysToSpec  a_m = (1/N) sum_k u_k cos(m phi_k),                   */
+/*                  b_m = (1/N) sum_k u_k sin(m phi_k),  phi_k = 2 pi k/N */
+/*  (b) modal step: derivative (a_m, b_m) -> (m b_m, -m a_m); filter      */
+/*      (a_m, b_m) -> sigma_m (a_m, b_m)                                  */
+/*  (c) SpecToPhys  u_k = a_0 + 2 sum_{0<m<N/2} (a_m cos + b_m sin)       */
+/*                        [+ a_{N/2} cos(N phi_k / 2) for even N]         */
+/* The derivative of the Nyquist mode of an even N vanishes at the nodes  */
+/* (d/dphi cos(N phi/2) = -(N/2) sin(N phi_k/2) = 0) and is dropped.      */
+/* ---------------------------------------------------------------------- */
+static real four_c(int N, int m, int k) { int64_t q = ((int64_t)m * k) % N; return R_COS(2 * R_PI * (real)q / (real)N); }
+static real four_s(int N, int m, int k) { int64_t q = ((int64_t)m * k) % N; return R_SIN(2 * R_PI * (real)q / (real)N); }
+
+/* mode 0: derivative d/dphi; mode 1: filter with sigma[0 .. N/2].  u, out have strides st, dst; out may alias u. */
+static void fourier_line(int N, const real* u, int64_t st, real* out, int64_t dst, int mode, const double* sigma) {
+  int M = N / 2;
+  real* a = malloc(sizeof(real) * (M + 1)); real* b = malloc(sizeof(real) * (M + 1)); real* o = malloc(sizeof(real) * N);
+  for (int m = 0; m <= M; ++m) {
+    real sa = 0, sb = 0;
+    for (int k = 0; k < N; ++k) { sa += u[k * st] * four_c(N, m, k); sb += u[k * st] * four_s(N, m, k); }
+    a[m] = sa / (real)N; b[m] = sb / (real)N;
+  }
+  for (int m = 0; m <= M; ++m) {
+    if (mode == 0) { real am = a[m]; a[m] = (real)m * b[m]; b[m] = -(real)m * am; if (2 * m == N) a[m] = b[m] = 0; }
+    else { a[m] *= (real)sigma[m]; b[m] *= (real)sigma[m]; }
+  }
+  for (int k = 0; k < N; ++k) {
+    real s0 = a[0];
+    for (int m = 1; m <= M; ++m) {
+      if (2 * m == N) s0 += a[m] * four_c(N, m, k);
+      else s0 += 2 * (a[m] * four_c(N, m, k) + b[m] * four_s(N, m, k));
+    }
+    o[k] = s0;
+  }
+  for (int k = 0; k < N; ++k) out[k * dst] = o[k];
+  free(a); free(b); free(o);
+}
+
+void ora_fourier_derivative_line(int N, const double* u, double* du) {
+  real* a = malloc(sizeof(real) * N); real* b = malloc(sizeof(real) * N);
+  for (int j = 0; j < N; ++j) a[j] = u[j];
+  fourier_line(N, a, 1, b, 1, 0, NULL);
   for (int j = 0; j < N; ++j) du[j] = (double)b[j];
   free(a); free(b);
 }
@@ -354,7 +418,8 @@ static void shell_filter_plane(const ylm_table* t, const real* u, real* out, con
 }
 
 /* u[ncomp][P] in place.  blocks: sig0/sig1/sig2 = sigma_k along x/y/z ([N_x], [N_y], [N_z]);
- * shells: sig0 = sigma_l ([L+1]), sig1/sig2 unused. */
+ * shells: sig0 = sigma_l ([L+1]), sig1/sig2 unused; cylinders: sig0 / sig1 = sigma_k along rho / z ([N_rho], [N_z]),
+ * sig2 = sigma_m of the Fourier modes ([N_phi/2 + 1]). */
 int ora_filter_subdomain(const ora_subdomain* sd, int ncomp, double* u, const double* sig0, const double* sig1, const double* sig2) {
   int n0, n1, n2; dims(sd, &n0, &n1, &n2); int64_t P = (int64_t)n0 * n1 * n2;
   if (sd->kind == 1) {
@@ -367,6 +432,19 @@ int ora_filter_subdomain(const ora_subdomain* sd, int ncomp, double* u, const do
         int e = (d + 1) % 3, f = (d + 2) % 3;
         for (int a = 0; a < nn[e]; ++a) for (int b = 0; b < nn[f]; ++b) cheb_filter_line(nn[d], w + a * st[e] + b * st[f], st[d], sg[d]);
       }
+      for (int64_t p = 0; p < P; ++p) u[(int64_t)c * P + p] = (double)w[p];
+      free(w);
+    }
+    return 0;
+  }
+  if (sd->kind == 2) {
+#pragma omp parallel for schedule(dynamic)
+    for (int c = 0; c < ncomp; ++c) {
+      real* w = malloc(sizeof(real) * P);
+      for (int64_t p = 0; p < P; ++p) w[p] = u[(int64_t)c * P + p];
+      for (int j = 0; j < n1; ++j) for (int k = 0; k < n2; ++k) cheb_filter_line(n0, w + (int64_t)j * n2 + k, (int64_t)n1 * n2, sig0);
+      for (int i = 0; i < n0; ++i) for (int k = 0; k < n2; ++k) cheb_filter_line(n1, w + (int64_t)i * n1 * n2 + k, n2, sig1);
+      for (int i = 0; i < n0; ++i) for (int j = 0; j < n1; ++j) { real* l = w + ((int64_t)i * n1 + j) * n2; fourier_line(n2, l, 1, l, 1, 1, sig2); }
       for (int64_t p = 0; p < P; ++p) u[(int64_t)c * P + p] = (double)w[p];
       free(w);
     }
@@ -408,6 +486,35 @@ static void gradient_real(const ora_subdomain* sd, int ncomp, const real* u, rea
         for (int i = 0; i < nn[d]; ++i) out[i * st[d]] *= sc;
       }
     }
+    return;
+  }
+  if (sd->kind == 2) {
+    /* cylindrical shells (O15): O1 in rho and in z, the Fourier derivative in phi, then Eq. 8 with the cylindrical Jacobian
+     *   d_x = cos(phi) d_rho - (sin(phi)/rho) d_phi,  d_y = sin(phi) d_rho + (cos(phi)/rho) d_phi,  d_z = d_z */
+    real* xr = malloc(sizeof(real) * n0); cgl_nodes(n0, xr);
+    real scr = 2 / ((real)sd->hi[0] - (real)sd->lo[0]), scz = 2 / ((real)sd->hi[1] - (real)sd->lo[1]);
+    int64_t pl = (int64_t)n1 * n2;
+#pragma omp parallel for schedule(dynamic)
+    for (int c = 0; c < ncomp; ++c) {
+      const real* uc = u + (int64_t)c * P;
+      real* dr = malloc(sizeof(real) * P); real* dz = malloc(sizeof(real) * P); real* dph = malloc(sizeof(real) * P);
+      for (int64_t q = 0; q < pl; ++q) cheb_line(n0, uc + q, pl, dr + q, pl);
+      for (int i = 0; i < n0; ++i) for (int k = 0; k < n2; ++k) cheb_line(n1, uc + i * pl + k, n2, dz + i * pl + k, n2);
+      for (int i = 0; i < n0; ++i) for (int j = 0; j < n1; ++j) fourier_line(n2, uc + i * pl + (int64_t)j * n2, 1, dph + i * pl + (int64_t)j * n2, 1, 0, NULL);
+      for (int i = 0; i < n0; ++i) {
+        real rho = (real)sd->lo[0] + ((real)sd->hi[0] - (real)sd->lo[0]) * (xr[i] + 1) / 2;
+        for (int j = 0; j < n1; ++j) for (int k = 0; k < n2; ++k) {
+          real ph = 2 * R_PI * (real)k / (real)n2, cp = R_COS(ph), sp = R_SIN(ph);
+          int64_t p = i * pl + (int64_t)j * n2 + k;
+          real a = scr * dr[p], b = scz * dz[p], e = dph[p];
+          g[((int64_t)0 * ncomp + c) * P + p] = cp * a - (sp / rho) * e;
+          g[((int64_t)1 * ncomp + c) * P + p] = sp * a + (cp / rho) * e;
+          g[((int64_t)2 * ncomp + c) * P + p] = b;
+        }
+      }
+      free(dr); free(dz); free(dph);
+    }
+    free(xr);
     return;
   }
   /* shells: O1 in r, O2 in (theta,phi), then Eq. 8 with the spherical Jacobian */
@@ -673,6 +780,8 @@ static int frozen(const ora_subdomain* sd, int64_t p) {
   int n0, n1, n2; dims(sd, &n0, &n1, &n2);
   int k = (int)(p % n2), j = (int)((p / n2) % n1), i = (int)(p / ((int64_t)n1 * n2));
   if (sd->kind == 0) return (i == 0 && sd->face[0] == 1) || (i == n0 - 1 && sd->face[1] == 1);
+  if (sd->kind == 2)   /* the phi direction is periodic: four faces */
+    return (i == 0 && sd->face[0] == 1) || (i == n0 - 1 && sd->face[1] == 1) || (j == 0 && sd->face[2] == 1) || (j == n1 - 1 && sd->face[3] == 1);
   return (i == 0 && sd->face[0] == 1) || (i == n0 - 1 && sd->face[1] == 1) || (j == 0 && sd->face[2] == 1) ||
          (j == n1 - 1 && sd->face[3] == 1) || (k == 0 && sd->face[4] == 1) || (k == n2 - 1 && sd->face[5] == 1);
 }
@@ -781,6 +890,14 @@ static int char_faces(const ora_subdomain* sd, int64_t p, const real* xyz3 /* x,
     real r = R_SQRT(xyz3[0] * xyz3[0] + xyz3[1] * xyz3[1] + xyz3[2] * xyz3[2]);
     if (i == 0 && sd->face[0] == 2) { for (int q = 0; q < 3; ++q) s[n][q] = -xyz3[q] / r; ++n; }
     if (i == n0 - 1 && sd->face[1] == 2) { for (int q = 0; q < 3; ++q) s[n][q] = xyz3[q] / r; ++n; }
+    return n;
+  }
+  if (sd->kind == 2) {   /* rho faces: -+ rho^ = -+ (cos phi, sin phi, 0); z faces: -+ z^ */
+    real rho = R_SQRT(xyz3[0] * xyz3[0] + xyz3[1] * xyz3[1]);
+    if (i == 0 && sd->face[0] == 2) { s[n][0] = -xyz3[0] / rho; s[n][1] = -xyz3[1] / rho; s[n][2] = 0; ++n; }
+    if (i == n0 - 1 && sd->face[1] == 2) { s[n][0] = xyz3[0] / rho; s[n][1] = xyz3[1] / rho; s[n][2] = 0; ++n; }
+    if (j == 0 && sd->face[2] == 2) { s[n][0] = s[n][1] = 0; s[n][2] = -1; ++n; }
+    if (j == n1 - 1 && sd->face[3] == 2) { s[n][0] = s[n][1] = 0; s[n][2] = 1; ++n; }
     return n;
   }
   int idx[3] = {i, j, k}, ext[3] = {n0, n1, n2};

@@ -47,9 +47,9 @@ class Subdomain(C.Structure):
 
 
 def make_subdomain(d: dict) -> Subdomain:
-    """d: {'kind': 'shell'|'block', 'n': [..], 'lo': [..], 'hi': [..], 'center': [..], 'face': [..], 'gamma': [..]}"""
+    """d: {'kind': 'shell'|'block'|'cylinder', 'n': [..], 'lo': [..], 'hi': [..], 'center': [..], 'face': [..], 'gamma': [..]}"""
     s = Subdomain()
-    s.kind = 0 if d["kind"] == "shell" else 1
+    s.kind = {"shell": 0, "block": 1, "cylinder": 2}[d["kind"]]
     n = list(d["n"]) + [0] * (3 - len(d["n"]))
     lo = list(d["lo"]) + [0.0] * (3 - len(d["lo"]))
     hi = list(d["hi"]) + [0.0] * (3 - len(d["hi"]))
@@ -82,6 +82,7 @@ class Oracle:
         L.ora_gl_nodes.argtypes = [C.c_int, _dp, _dp]
         L.ora_coords.argtypes = [C.POINTER(Subdomain), _dp]
         L.ora_cheb_derivative_line.argtypes = [C.c_int, _dp, _dp]
+        L.ora_fourier_derivative_line.argtypes = [C.c_int, _dp, _dp]
         L.ora_pbar.argtypes = [C.c_int, C.c_double, _dp, _dp]
         L.ora_shell_angular.argtypes = [C.c_int, _dp, _dp, _dp]
         L.ora_shell_project.argtypes = [C.c_int, _dp, _dp]
@@ -157,6 +158,13 @@ class Oracle:
         u = np.ascontiguousarray(u, dtype=np.float64)
         du = np.empty_like(u)
         self.lib.ora_cheb_derivative_line(u.shape[0], u, du)
+        return du
+
+    def fourier_derivative_line(self, u: np.ndarray) -> np.ndarray:
+        """O15: d/dphi of one periodic line sampled at phi_k = 2 pi k / N."""
+        u = np.ascontiguousarray(u, dtype=np.float64)
+        du = np.empty_like(u)
+        self.lib.ora_fourier_derivative_line(u.shape[0], u, du)
         return du
 
     def pbar(self, L: int, theta: float):

@@ -32,6 +32,20 @@ def block(n, lo, hi, face=(0,) * 6, gamma=None):
             "center": [0.0, 0.0, 0.0], "face": list(face), "gamma": list(gamma or GAMMA_DEFAULT)}
 
 
+def cylinder(n, rho_in, rho_out, z_lo, z_hi, face=(0, 0, 0, 0), gamma=None, center=(0.0, 0.0, 0.0)):
+    """Cylindrical shell (reading S25), axis along z through `center`: n = (N_rho, N_z, N_phi); z range relative to
+    the centre; faces rho_in, rho_out, z_lo, z_hi."""
+    return {"kind": "cylinder", "n": [int(v) for v in n], "lo": [float(rho_in), float(z_lo), 0.0],
+            "hi": [float(rho_out), float(z_hi), 0.0], "center": [float(c) for c in center],
+            "face": list(face) + [0] * (6 - len(face)), "gamma": list(gamma or GAMMA_DEFAULT)}
+
+
+def cylinder_box(d):
+    """Cartesian bounding box (lo, hi) of a cylindrical shell."""
+    c, ro = d["center"], d["hi"][0]
+    return [c[0] - ro, c[1] - ro, c[2] + d["lo"][1]], [c[0] + ro, c[1] + ro, c[2] + d["hi"][1]]
+
+
 def num_points(d) -> int:
     if d["kind"] == "shell":
         return d["n"][0] * (d["n"][1] + 1) * (2 * d["n"][1] + 2)
@@ -51,6 +65,10 @@ def min_spacing(descs) -> float:
             th0 = math.pi * 0.75 / (L + 1.5)
             best = min(best, r_in * math.sin(th0) * 2.0 * math.sin(math.pi / (2 * L + 2)))
             best = min(best, r_in * math.pi / (L + 1.5))
+        elif d["kind"] == "cylinder":
+            for a in range(2):
+                best = min(best, 0.5 * (d["hi"][a] - d["lo"][a]) * (1.0 - math.cos(math.pi / (d["n"][a] - 1))))
+            best = min(best, 2.0 * d["lo"][0] * math.sin(math.pi / d["n"][2]))
         else:
             for a in range(3):
                 best = min(best, 0.5 * (d["hi"][a] - d["lo"][a]) * (1.0 - math.cos(math.pi / (d["n"][a] - 1))))

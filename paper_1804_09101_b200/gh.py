@@ -19,6 +19,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libgh.so")
 
 GH_NCOMP = 50
+GH_SHELL, GH_BLOCK, GH_CYLINDER = range(3)
 GH_NUM_KERNELS = 13
 GH_T_A, GH_T_AA, GH_T_AB, GH_T_ABB = range(4)
 GH_FILTER_NONE, GH_FILTER_HEAVISIDE, GH_FILTER_EXP = range(3)
@@ -137,7 +138,7 @@ def make_descs(descs):
     arr = (gh_subdomain_desc * len(descs))()
     for s, d in enumerate(descs):
         e = arr[s]
-        e.kind = 0 if d["kind"] == "shell" else 1
+        e.kind = {"shell": GH_SHELL, "block": GH_BLOCK, "cylinder": GH_CYLINDER}[d["kind"]]
         n = list(d["n"]) + [0] * (3 - len(d["n"]))
         lo = list(d["lo"]) + [0.0] * (3 - len(d["lo"]))
         hi = list(d["hi"]) + [0.0] * (3 - len(d["hi"]))

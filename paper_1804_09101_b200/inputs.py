@@ -310,7 +310,7 @@ def block_perturbation(lo, hi, xyz, amplitude, seed, deg=6, norm=None) -> np.nda
 def initial_data(descs, coords, spin, amplitude, config_id, M=1.0):
     """Fields u[50,P_total] and gauge source H[4,P_total] for a list of subdomains.
 
-    ``descs``: list of dicts with keys kind ('shell'|'block'), lo, hi, center;
+    ``descs``: list of dicts with keys kind ('shell'|'block'|'cylinder'), lo, hi, center;
     ``coords``: list of xyz[3,P_s] arrays (from the oracle's grid or from
     ``gh_domain_coords`` — the generator never builds collocation grids itself).
     Returns lists (u_s, H_s), one entry per subdomain.
@@ -323,6 +323,10 @@ def initial_data(descs, coords, spin, amplitude, config_id, M=1.0):
         if amplitude != 0.0:
             if d["kind"] == "shell":
                 u = u + shell_perturbation(d["lo"][0], d["hi"][0], d["center"], xyz, amplitude, seed)
+            elif d["kind"] == "cylinder":     # the block family on the cylinder's Cartesian bounding box
+                c, ro = d["center"], d["hi"][0]
+                u = u + block_perturbation([c[0] - ro, c[1] - ro, c[2] + d["lo"][1]], [c[0] + ro, c[1] + ro, c[2] + d["hi"][1]],
+                                           xyz, amplitude, seed)
             else:
                 u = u + block_perturbation(d["lo"], d["hi"], xyz, amplitude, seed)
         us.append(np.ascontiguousarray(u))
