@@ -54,7 +54,7 @@ typedef enum {
   GH_ERR_SINGULAR = 5   /* non-physical data met on the device: det g_ij <= 0 or lapse^2 <= 0 */
 } gh_status;
 
-typedef enum { GH_SHELL = 0, GH_BLOCK = 1 } gh_kind;
+typedef enum { GH_SHELL = 0, GH_BLOCK = 1, GH_CYLINDER = 2 } gh_kind;
 /* FREE: no boundary treatment (e.g. an excision face inside the horizon).  FROZEN: d_t u = 0 on the face.
  * CHARACTERISTIC (NEXT-2 (i); the paper's ApplyBCs module, which it left on the CPU): the time
  * derivatives of the characteristic fields that ENTER through the face are set to zero, the others keep what the evolution
@@ -70,13 +70,19 @@ typedef enum { GH_SHELL = 0, GH_BLOCK = 1 } gh_kind;
  * neighbour's face state straight from the field store. */
 typedef enum { GH_FACE_FREE = 0, GH_FACE_FROZEN = 1, GH_FACE_CHARACTERISTIC = 2, GH_FACE_INTERFACE = 3 } gh_face;
 
-/* One spectral subdomain (PAPER.md:371 I1^3 blocks, PAPER.md:386 I1 x S2 shells). */
+/* One spectral subdomain (PAPER.md:371 I1^3 blocks, PAPER.md:386 I1 x S2 shells; PAPER.md:79, 564 cylindrical shells - the third
+ * topology the paper names for binary runs, without formulas.  DESIGN.md reading S25: GH_CYLINDER is a hollow cylinder about an
+ * axis parallel to z through `center`, I1(rho) x I1(z) x S1(phi): Chebyshev-Gauss-Lobatto nodes in rho and z, N_phi uniform
+ * nodes phi_k = 2 pi k / N_phi with the Fourier differentiation matrix; points ordered (rho slowest, z, phi fastest); Cartesian
+ * tensor components, gradient through  d_x = cos(phi) d_rho - (sin(phi)/rho) d_phi,  d_y = sin(phi) d_rho + (cos(phi)/rho) d_phi. */
 typedef struct {
   int32_t kind;      /* gh_kind */
-  int32_t n[3];      /* shell: {N_r, L, 0} (N_theta = L+1, N_phi = 2L+2); block: {N_x, N_y, N_z}; N >= 2 */
-  double lo[3], hi[3]; /* shell: lo[0] = r_in, hi[0] = r_out (rest unused); block: corner coordinates */
-  double center[3];  /* shell centre (blocks: ignored) */
-  int32_t face[6];   /* gh_face. shell: [0] = inner, [1] = outer; block: -x,+x,-y,+y,-z,+z */
+  int32_t n[3];      /* shell: {N_r, L, 0} (N_theta = L+1, N_phi = 2L+2); block: {N_x, N_y, N_z}; cylinder: {N_rho, N_z, N_phi >= 3}; N >= 2 */
+  double lo[3], hi[3]; /* shell: lo[0] = r_in, hi[0] = r_out (rest unused); block: corner coordinates;
+                        * cylinder: [0] = rho_in > 0, rho_out; [1] = z range relative to the centre */
+  double center[3];  /* shell centre; cylinder: a point of the axis (blocks: ignored) */
+  int32_t face[6];   /* gh_face. shell: [0] = inner, [1] = outer; block: -x,+x,-y,+y,-z,+z; cylinder: rho_in, rho_out, z_lo, z_hi
+                      * (FREE / FROZEN / CHARACTERISTIC; outward normals -+ rho^ and -+ z^) */
   double gamma[3];   /* constraint-damping gamma0, gamma1, gamma2, constant on the subdomain */
 } gh_subdomain_desc;
 
@@ -174,8 +180,9 @@ typedef struct {
   int32_t pad_;
 } gh_filter_desc;
 
-/* Choose the filters: `block_axes` for the three Chebyshev axes of every block, `shell_angular` for the l-filter of every
- * shell (either may be NULL or kind NONE: that family is left untouched).  Builds the matrices on the host in long
+/* Choose the filters: `block_axes` for the three Chebyshev axes of every block - and of every cylindrical shell, where it acts
+ * on the Chebyshev modes k <= N-1 in rho and z and on the Fourier modes m <= N_phi/2 in phi -, `shell_angular` for the l-filter
+ * of every shell (either may be NULL or kind NONE: that family is left untouched).  Builds the matrices on the host in long
  * double and uploads them (synchronises).  descs: HOST. */
 gh_status gh_set_filter(gh_domain* dom, const gh_filter_desc* block_axes, const gh_filter_desc* shell_angular);
 

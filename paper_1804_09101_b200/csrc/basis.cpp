@@ -154,6 +154,31 @@ void cheb_filter_matrix(int N, const std::vector<ld>& sigma, std::vector<ld>& F)
     }
 }
 
+void fourier_diff_matrix(int N, std::vector<ld>& D) {
+  D.assign((size_t)N * N, 0);
+  for (int j = 0; j < N; ++j)
+    for (int k = 0; k < N; ++k) {
+      if (j == k) continue;
+      const int d = ((j - k) % N + N) % N;              // 1 .. N-1; (-1)^(j-k) cot / csc are N-periodic in j - k for the parity at hand
+      const ld x = PI_L * (ld)d / (ld)N, sgn = (d & 1) ? -1 : 1;
+      D[(size_t)j * N + k] = (N % 2 == 0) ? sgn * cosl(x) / (2 * sinl(x)) : sgn / (2 * sinl(x));
+    }
+}
+
+void fourier_filter_matrix(int N, const std::vector<ld>& sigma, std::vector<ld>& F) {
+  F.assign((size_t)N * N, 0);
+  for (int j = 0; j < N; ++j)
+    for (int k = 0; k < N; ++k) {
+      const int d = ((j - k) % N + N) % N;
+      ld s = sigma[0];
+      for (int m = 1; 2 * m <= N; ++m) {
+        const ld c = cosl(2 * PI_L * (ld)(((long long)m * d) % N) / (ld)N);
+        s += (2 * m == N ? 1 : 2) * sigma[m] * c;
+      }
+      F[(size_t)j * N + k] = s / (ld)N;
+    }
+}
+
 void shell_filter_composites(int L, const std::vector<ld>& sigma_l, std::vector<ld>& G) {
   const int nt = L + 1;
   std::vector<ld> ct, w, st(nt);

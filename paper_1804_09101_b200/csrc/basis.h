@@ -36,6 +36,13 @@ void shell_basis(int L, ShellBasis& B);
 // Chebyshev line filter F = SpecToPhys diag(sigma) PhysToSpec on N CGL nodes (row-major N x N), Eqs. 16-17:
 //   F[a][j] = sum_k T_k(x_a) sigma_k (2/(N-1)) (1/(c_k c_j)) T_k(x_j).
 void cheb_filter_matrix(int N, const std::vector<ld>& sigma, std::vector<ld>& F);
+// Periodic (Fourier) line on N uniform nodes phi_k = 2 pi k / N - the S1 factor of the cylindrical shells (DESIGN.md
+// reading S25).  Differentiation matrix of the trigonometric interpolant (the Nyquist mode of an even N has zero derivative at
+// the nodes):  D[j][k] = (1/2) (-1)^(j-k) cot(pi (j-k) / N), N even;  (1/2) (-1)^(j-k) / sin(pi (j-k) / N), N odd;  D[j][j] = 0.
+void fourier_diff_matrix(int N, std::vector<ld>& D);
+// Filter  F[j][k] = (1/N) sum_{|m| <= N/2} sigma_|m| e^{i m (phi_j - phi_k)}  (the Nyquist mode of an even N counted once),
+// sigma[0 .. N/2].
+void fourier_filter_matrix(int N, const std::vector<ld>& sigma, std::vector<ld>& F);
 // Per-m filtered projectors on the Gauss-Legendre colatitudes: G[m][j'][j] = 2 pi sum_{l=m}^{L} sigma_l Pbar_lm(j') w_j Pbar_lm(j).
 void shell_filter_composites(int L, const std::vector<ld>& sigma_l, std::vector<ld>& G);
 

@@ -9,7 +9,8 @@ constexpr int TILE_PTS = 128;   // points per CTA of the pointwise kernels (K_rh
 
 // One spectral subdomain as the kernels see it.
 struct SubDev {
-  int32_t kind;            // 0 shell, 1 block
+  int32_t kind;            // 0 shell, 1 block, 2 cylindrical shell (logical axes rho, z, phi; the pointwise kernels treat it as a
+                           // "shell": curvilinear, Jacobian from tables)
   int32_t n0, n1, n2;      // logical extents, n2 fastest (shell: N_r, L+1, 2L+2)
   int64_t off;             // start inside a component (multiple of 16 doubles)
   int32_t P;               // n0*n1*n2

@@ -154,6 +154,12 @@ bool validate(const gh_subdomain_desc* descs, int32_t n_sub, std::string& err) {
         if (d.n[a] < 2 || d.n[a] > GH_MAX_CHEB_N) { snprintf(buf, sizeof buf, "subdomain %d: block needs 2 <= N <= %d on every axis", s, GH_MAX_CHEB_N); err = buf; return false; }
         if (!(d.hi[a] > d.lo[a])) { snprintf(buf, sizeof buf, "subdomain %d: block needs lo < hi on every axis", s); err = buf; return false; }
       }
+    } else if (d.kind == GH_CYLINDER) {
+      if (d.n[0] < 2 || d.n[0] > GH_MAX_CHEB_N || d.n[1] < 2 || d.n[1] > GH_MAX_CHEB_N || d.n[2] < 3 || d.n[2] > GH_MAX_CHEB_N) {
+        snprintf(buf, sizeof buf, "subdomain %d: cylindrical shell needs 2 <= N_rho, N_z <= %d and 3 <= N_phi <= %d", s, GH_MAX_CHEB_N, GH_MAX_CHEB_N);
+        err = buf; return false;
+      }
+      if (!(d.lo[0] > 0.0) || !(d.hi[0] > d.lo[0]) || !(d.hi[1] > d.lo[1])) { snprintf(buf, sizeof buf, "subdomain %d: cylindrical shell needs 0 < rho_in < rho_out and z_lo < z_hi", s); err = buf; return false; }
     } else { snprintf(buf, sizeof buf, "subdomain %d: unknown kind %d", s, d.kind); err = buf; return false; }
     for (int f = 0; f < 6; ++f) {
       if (d.face[f] == GH_FACE_INTERFACE && f < 2 && d.kind == GH_SHELL) {
@@ -169,7 +175,7 @@ bool validate(const gh_subdomain_desc* descs, int32_t n_sub, std::string& err) {
         if (!ok) { snprintf(buf, sizeof buf, "subdomain %d: INTERFACE face %d has no matching neighbour shell", s, f); err = buf; return false; }
         continue;
       }
-      if (d.face[f] == GH_FACE_INTERFACE && f < (d.kind == GH_SHELL ? 2 : 6)) { snprintf(buf, sizeof buf, "subdomain %d: interfaces between blocks are not built", s); err = buf; return false; }
+      if (d.face[f] == GH_FACE_INTERFACE && f < (d.kind == GH_SHELL ? 2 : d.kind == GH_CYLINDER ? 4 : 6)) { snprintf(buf, sizeof buf, "subdomain %d: interfaces are built between concentric shells only", s); err = buf; return false; }
       if (d.face[f] != GH_FACE_FREE && d.face[f] != GH_FACE_FROZEN && d.face[f] != GH_FACE_CHARACTERISTIC && d.face[f] != GH_FACE_INTERFACE) { snprintf(buf, sizeof buf, "subdomain %d: bad face flag", s); err = buf; return false; }
     }
     for (int g = 0; g < 3; ++g)
@@ -206,7 +212,7 @@ bool make_plan(const gh_subdomain_desc* descs, int32_t n_sub, Plan& pl, std::str
       if (big_N(N)) {       // tiled GEMM path
         pl.bigtab_doubles += gemm_amat_doubles(N, N, GEMM_MB);
         pl.n_gemm[G_CHEB] += (int)((cols + GEMM_CT - 1) / GEMM_CT);
-        if (d.kind == GH_BLOCK) { pl.fbigtab_doubles += gemm_amat_doubles(N, N, GEMM_MB); pl.n_gemm[G_FX + a] += (int)((cols + GEMM_CT - 1) / GEMM_CT); }
+        if (d.kind != GH_SHELL) { pl.fbigtab_doubles += gemm_amat_doubles(N, N, GEMM_MB); pl.n_gemm[G_FX + a] += (int)((cols + GEMM_CT - 1) / GEMM_CT); }
         pl.has_big = true;
         continue;
       }
@@ -214,8 +220,10 @@ bool make_plan(const gh_subdomain_desc* descs, int32_t n_sub, Plan& pl, std::str
       const int items = (int)((cols + cheb_ct(N) - 1) / cheb_ct(N));
       pl.n_cheb_items += items; pl.n_cheb_class[cheb_class(N)] += items;
       pl.cheb_smem = std::max(pl.cheb_smem, cheb_frag_doubles(N) * sizeof(double));
-      if (d.kind == GH_BLOCK) { pl.ftable_doubles += cheb_frag_doubles(N); pl.n_fcheb[a][cheb_class(N)] += items; pl.n_fcheb_items += items; }
+      if (d.kind != GH_SHELL) { pl.ftable_doubles += cheb_frag_doubles(N); pl.n_fcheb[a][cheb_class(N)] += items; pl.n_fcheb_items += items; }
     }
+    if (d.kind == GH_CYLINDER)      // coordinate tables 1 / rho, (ct = 0, st = 1), cos phi, sin phi in the shells' slots
+      tab += (size_t)round_up(n0, 2) + 2 * (size_t)round_up(n1, 2) + 2 * (size_t)round_up(n2, 2);
     if (d.kind == GH_SHELL) {
       for (int f = 0; f < 2; ++f) {
         const int o = f == 0 ? s - 1 : s + 1;
@@ -315,10 +323,10 @@ struct gh_domain {
   GemmItem* gemm = nullptr;              // K_gemm items of the large subdomains, the G_NLIST lists back to back
   IfcItem* ifci = nullptr;               // faces to interpolate (interfaces between shells of different L)
   double* ifc = nullptr;                 // [50][Sf]: the neighbours' face states on the own grids
-  struct FBlock { int N; double unused; size_t off; };     // one filter matrix slot per (block, axis): offset (doubles) from `tables`
+  struct FBlock { int N; bool fourier; size_t off; };     // one filter matrix slot per (block or cylinder, axis): offset (doubles) from `tables`
   std::vector<FBlock> f_blocks;
   std::map<int, size_t> f_L;             // shell band limit L -> offset (doubles) of its filtered projectors from `tables`
-  struct FBig { int N; size_t off; };     // large classes: one K_gemm filter matrix slot per (block, large axis) ...
+  struct FBig { int N; size_t off; bool fourier; };     // large classes: one K_gemm filter matrix slot per (block, large axis) ...
   std::vector<FBig> f_big_blocks;
   std::map<int, std::vector<size_t>> f_big_L;   // ... and per large L the slots of its per-m filtered projectors
   bool filt_blocks = false, filt_shells = false;
@@ -471,7 +479,7 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
   std::vector<AngItem> ang, ang1; ang.reserve(pl.n_ang_items);   // class 0 items, class 1 items (appended below)
   d->h_subs.resize(n_sub);
   size_t tp = 0;
-  std::map<int, std::vector<ghb::ld>> Dcache;        // N -> unscaled D
+  std::map<int, std::vector<ghb::ld>> Dcache, Fcache;        // N -> unscaled D; N -> Fourier differentiation matrix
   struct ShellOff { int Fa, Fs, T; };
   std::map<int, ShellOff> Lcache;
   // large subdomains: blocked fragment matrices (behind the filter tables) and K_gemm items per launch list
@@ -516,7 +524,7 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
     memset(&sd, 0, sizeof sd);
     int n0, n1, n2; sub_dims(de, n0, n1, n2);
     sd.kind = de.kind; sd.n0 = n0; sd.n1 = n1; sd.n2 = n2; sd.off = pl.offsets[s]; sd.P = n0 * n1 * n2;
-    for (int f = 0; f < 6; ++f) { sd.face[f] = de.face[f]; if (f < (de.kind == GH_SHELL ? 2 : 6) && de.face[f] == GH_FACE_CHARACTERISTIC) d->has_char = true; }
+    for (int f = 0; f < 6; ++f) { sd.face[f] = de.face[f]; if (f < (de.kind == GH_SHELL ? 2 : de.kind == GH_CYLINDER ? 4 : 6) && de.face[f] == GH_FACE_CHARACTERISTIC) d->has_char = true; }
     sd.nbr[0] = sd.nbr[1] = -1; sd.nbi[0] = sd.nbi[1] = -1; sd.pen = 0.0;
     if (de.kind == GH_SHELL) {
       sd.pen = (double)(n0 - 1) * (double)(n0 - 1) / (de.hi[0] - de.lo[0]);
@@ -564,9 +572,13 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
     const int64_t strides[3] = {(int64_t)n1 * n2, n2, 1};
     for (int a = 0; a < naxes; ++a) {
       const int N = (int)nn[a];
-      if (!Dcache.count(N)) ghb::cheb_diff_matrix(N, Dcache[N]);
-      const std::vector<ghb::ld>& D = Dcache[N];
-      const ghb::ld scale = 2 / ((ghb::ld)de.hi[a] - (ghb::ld)de.lo[a]);   // affine map factor of Eq. 22
+      // the periodic axis of a cylindrical shell: the Fourier differentiation matrix in d / d phi itself (no map factor) - to the
+      // kernels one more "black box" matrix along a line
+      const bool fourier = de.kind == GH_CYLINDER && a == 2;
+      if (fourier && !Fcache.count(N)) ghb::fourier_diff_matrix(N, Fcache[N]);
+      if (!fourier && !Dcache.count(N)) ghb::cheb_diff_matrix(N, Dcache[N]);
+      const std::vector<ghb::ld>& D = fourier ? Fcache[N] : Dcache[N];
+      const ghb::ld scale = fourier ? (ghb::ld)1 : 2 / ((ghb::ld)de.hi[a] - (ghb::ld)de.lo[a]);   // affine map factor of Eq. 22
       if (big_N(N)) {     // K_gemm: Out[a', col] = sum_i (scale D)[a'][i] u[i, col], the same strided views as K_cheb's
         GemmItem it; memset(&it, 0, sizeof it);
         it.amat = put_amat(N, N, [&](int r, int c) { return scale * D[(size_t)r * N + c]; });
@@ -577,11 +589,11 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
         else { it.in_inner = 1; it.in_outer = nn[2]; it.in_cs = 0; }
         it.out_inner = it.in_inner; it.out_outer = it.in_outer; it.out_cs = it.in_cs;
         put_items(G_CHEB, it, sd.P / N);
-        if (de.kind == GH_BLOCK) {      // the same strided view with the filter matrix: x: u -> T1 (slot 0), y: T1 -> T2 (slot 1), z: T2 -> u
+        if (de.kind != GH_SHELL) {      // the same strided view with the filter matrix: x: u -> T1 (slot 0), y: T1 -> T2 (slot 1), z: T2 -> u
           GemmItem fi = it;
           fi.amat = (int64_t)(fbig0 + fbp);
           fi.in_slot = a == 0 ? -1 : a - 1; fi.out_slot = a == 2 ? -1 : a;
-          d->f_big_blocks.push_back({N, fbig0 + fbp}); fbp += gemm_amat_doubles(N, N, GEMM_MB);
+          d->f_big_blocks.push_back({N, fbig0 + fbp, fourier}); fbp += gemm_amat_doubles(N, N, GEMM_MB);
           put_items(G_FX + a, fi, sd.P / N);
         }
         continue;
@@ -609,9 +621,9 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
         else if (a == 1) { it.col_inner = (int)nn[2]; it.outer_stride = nn[1] * nn[2]; }
         else { it.col_inner = 1; it.outer_stride = nn[2]; }
         chebc[cheb_class(N)].push_back(it);
-        if (de.kind == GH_BLOCK) { ChebItem fi = it; fi.dmat = (int)ftp; fi.axis = 0; fch[a][cheb_class(N)].push_back(fi); }
+        if (de.kind != GH_SHELL) { ChebItem fi = it; fi.dmat = (int)ftp; fi.axis = 0; fch[a][cheb_class(N)].push_back(fi); }
       }
-      if (de.kind == GH_BLOCK) { d->f_blocks.push_back({N, 0.0, ftp}); ftp += cheb_frag_doubles(N); }
+      if (de.kind != GH_SHELL) { d->f_blocks.push_back({N, fourier, ftp}); ftp += cheb_frag_doubles(N); }
     }
     if (de.kind == GH_SHELL && big_L(de.n[1])) {
       // K_gemm path of a large shell, per component c (R = n_r n_theta rows of n_phi points), through coefficient buffers in
@@ -690,6 +702,20 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
       tp += round_up(n0, 2);
       sd.t_ct = (int)tp; for (int j = 0; j < n1; ++j) tab[tp + j] = (double)ct[j]; tp += round_up(n1, 2);
       sd.t_st = (int)tp; for (int j = 0; j < n1; ++j) tab[tp + j] = (double)sqrtl((1 - ct[j]) * (1 + ct[j])); tp += round_up(n1, 2);
+      const ghb::ld PI_L = 3.14159265358979323846264338327950288L;
+      sd.t_cp = (int)tp; for (int k = 0; k < n2; ++k) tab[tp + k] = (double)cosl(2 * PI_L * k / n2); tp += round_up(n2, 2);
+      sd.t_sp = (int)tp; for (int k = 0; k < n2; ++k) tab[tp + k] = (double)sinl(2 * PI_L * k / n2); tp += round_up(n2, 2);
+    }
+    if (de.kind == GH_CYLINDER) {
+      // coordinate tables of a cylindrical shell in the shells' slots: 1 / rho_i; ct = 0, st = 1 (shell_jac's entries then are
+      // the cylindrical Jacobian but for d_z); cos / sin phi_k
+      d->has_shell = true;
+      std::vector<ghb::ld> xr; ghb::cheb_nodes(n0, xr);
+      sd.t_rinv = (int)tp;
+      for (int i = 0; i < n0; ++i) tab[tp + i] = (double)(1 / ((ghb::ld)de.lo[0] + ((ghb::ld)de.hi[0] - (ghb::ld)de.lo[0]) * (xr[i] + 1) / 2));
+      tp += round_up(n0, 2);
+      sd.t_ct = (int)tp; for (int j = 0; j < n1; ++j) tab[tp + j] = 0.0; tp += round_up(n1, 2);
+      sd.t_st = (int)tp; for (int j = 0; j < n1; ++j) tab[tp + j] = 1.0; tp += round_up(n1, 2);
       const ghb::ld PI_L = 3.14159265358979323846264338327950288L;
       sd.t_cp = (int)tp; for (int k = 0; k < n2; ++k) tab[tp + k] = (double)cosl(2 * PI_L * k / n2); tp += round_up(n2, 2);
       sd.t_sp = (int)tp; for (int k = 0; k < n2; ++k) tab[tp + k] = (double)sinl(2 * PI_L * k / n2); tp += round_up(n2, 2);
@@ -867,6 +893,21 @@ extern "C" gh_status gh_domain_coords(const gh_domain* cd, double* xyz, int on_d
             h[p] = (double)((ghb::ld)de.center[0] + r * st * cosl(ph));
             h[S + p] = (double)((ghb::ld)de.center[1] + r * st * sinl(ph));
             h[2 * S + p] = (double)((ghb::ld)de.center[2] + r * ct[j]);
+          }
+        }
+      }
+    } else if (de.kind == GH_CYLINDER) {
+      std::vector<ghb::ld> xr, xz; ghb::cheb_nodes(n0, xr); ghb::cheb_nodes(n1, xz);
+      for (int i = 0; i < n0; ++i) {
+        const ghb::ld rho = (ghb::ld)de.lo[0] + ((ghb::ld)de.hi[0] - (ghb::ld)de.lo[0]) * (xr[i] + 1) / 2;
+        for (int j = 0; j < n1; ++j) {
+          const ghb::ld z = (ghb::ld)de.lo[1] + ((ghb::ld)de.hi[1] - (ghb::ld)de.lo[1]) * (xz[j] + 1) / 2;
+          for (int k = 0; k < n2; ++k) {
+            const ghb::ld ph = 2 * PI_L * k / n2;
+            const int64_t p = off + ((int64_t)i * n1 + j) * n2 + k;
+            h[p] = (double)((ghb::ld)de.center[0] + rho * cosl(ph));
+            h[S + p] = (double)((ghb::ld)de.center[1] + rho * sinl(ph));
+            h[2 * S + p] = (double)((ghb::ld)de.center[2] + z);
           }
         }
       }
@@ -1265,12 +1306,12 @@ extern "C" gh_status gh_set_filter(gh_domain* d, const gh_filter_desc* fb, const
   if (on_b) {
     std::map<int, std::vector<ghb::ld>> cache;
     for (const auto& b : d->f_big_blocks) {
-      const int N = b.N;
-      if (!cache.count(N)) {
-        if (!filter_sigma(fb, N - 1, sg)) return fail(d, GH_ERR_ARG, "bad block filter descriptor");
-        ghb::cheb_filter_matrix(N, sg, cache[N]);
+      const int N = b.N, key = b.fourier ? -N : N;       // Fourier axes of cylindrical shells: sigma over m = 0 .. N/2
+      if (!cache.count(key)) {
+        if (!filter_sigma(fb, b.fourier ? N / 2 : N - 1, sg)) return fail(d, GH_ERR_ARG, "bad block filter descriptor");
+        if (b.fourier) ghb::fourier_filter_matrix(N, sg, cache[key]); else ghb::cheb_filter_matrix(N, sg, cache[key]);
       }
-      const std::vector<ghb::ld>& F = cache[N];
+      const std::vector<ghb::ld>& F = cache[key];
       fill_amat(fbig.data() + (b.off - fbig0), N, N, [&](int r, int c) { return F[(size_t)r * N + c]; });
     }
   }
@@ -1286,12 +1327,12 @@ extern "C" gh_status gh_set_filter(gh_domain* d, const gh_filter_desc* fb, const
   if (on_b) {
     std::map<int, std::vector<ghb::ld>> cache;      // N -> filter matrix
     for (const auto& b : d->f_blocks) {
-      const int N = b.N;
-      if (!cache.count(N)) {
-        if (!filter_sigma(fb, N - 1, sg)) return fail(d, GH_ERR_ARG, "bad block filter descriptor");
-        ghb::cheb_filter_matrix(N, sg, cache[N]);
+      const int N = b.N, key = b.fourier ? -N : N;       // Fourier axes of cylindrical shells: sigma over m = 0 .. N/2
+      if (!cache.count(key)) {
+        if (!filter_sigma(fb, b.fourier ? N / 2 : N - 1, sg)) return fail(d, GH_ERR_ARG, "bad block filter descriptor");
+        if (b.fourier) ghb::fourier_filter_matrix(N, sg, cache[key]); else ghb::cheb_filter_matrix(N, sg, cache[key]);
       }
-      const std::vector<ghb::ld>& F = cache[N];
+      const std::vector<ghb::ld>& F = cache[key];
       const int mtn = (N + 7) / 8, ksn = (N + 3) / 4;
       for (int mt = 0; mt < mtn; ++mt) for (int ks = 0; ks < ksn; ++ks) for (int lane = 0; lane < 32; ++lane) {
         const int row = mt * 8 + lane / 4, col = ks * 4 + lane % 4;

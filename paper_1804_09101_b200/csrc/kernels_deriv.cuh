@@ -180,6 +180,9 @@ __device__ __forceinline__ ShellJac shell_jac(const SubDev& sd, const double* __
   J.xr = st * cp; J.xt = ct * cp * ri; J.xp = -sp * ri / st;
   J.yr = st * sp; J.yt = ct * sp * ri; J.yp = cp * ri / st;
   J.zr = ct;      J.zt = -st * ri;
+  // cylindrical shell (kind 2), logical (rho, z, phi): its tables hold 1 / rho, st = 1, ct = 0, so the six entries above are
+  // already  d_x = cp d_rho - (sp / rho) d_phi,  d_y = sp d_rho + (cp / rho) d_phi;  only  d_z = d_z (the second slot)  differs
+  if (sd.kind == 2) J.zt = 1.0;
   return J;
 }
 
@@ -190,7 +193,7 @@ k_jac(const SubDev* __restrict__ subs, const int32_t* __restrict__ tile_first, i
       const double* __restrict__ tables, double* __restrict__ g, int64_t S, int ncomp) {
   const int s = find_sub(tile_first, n_sub, blockIdx.x);
   const SubDev sd = subs[s];
-  if (sd.kind != 0) return;
+  if (sd.kind == 1) return;
   const int local = (blockIdx.x - tile_first[s]) * TILE_PTS + threadIdx.x;
   if (local >= sd.P) return;
   const ShellJac J = shell_jac(sd, tables, local);

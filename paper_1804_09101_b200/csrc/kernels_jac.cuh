@@ -134,8 +134,8 @@ k_scj(const SubDev* __restrict__ subs, const int32_t* __restrict__ tile_first, i
 __device__ __forceinline__ bool point_frozen(const SubDev& sd, int local) {
   const int i2 = local % sd.n2, t = local / sd.n2, i1 = t % sd.n1, i0 = t / sd.n1;
   bool fz = (i0 == 0 && sd.face[0] == 1) || (i0 == sd.n0 - 1 && sd.face[1] == 1);
-  if (sd.kind != 0)
-    fz = fz || (i1 == 0 && sd.face[2] == 1) || (i1 == sd.n1 - 1 && sd.face[3] == 1) || (i2 == 0 && sd.face[4] == 1) || (i2 == sd.n2 - 1 && sd.face[5] == 1);
+  if (sd.kind != 0) fz = fz || (i1 == 0 && sd.face[2] == 1) || (i1 == sd.n1 - 1 && sd.face[3] == 1);
+  if (sd.kind == 1) fz = fz || (i2 == 0 && sd.face[4] == 1) || (i2 == sd.n2 - 1 && sd.face[5] == 1);
   return fz;
 }
 
@@ -149,13 +149,22 @@ k_map_pre(const SubDev* __restrict__ subs, const int32_t* __restrict__ tile_firs
   const int64_t p = sd.off + local;
   double M[9];
   scj_load_j(mapJ, S, p, M);
-  if (sd.kind == 0) {      // M <- A^-1 Jm A with A the logical -> Cartesian Jacobian of Eq. 8
+  if (sd.kind != 1) {      // M <- A^-1 Jm A with A the logical -> Cartesian Jacobian of Eq. 8
     const ShellJac J = shell_jac(sd, tables, local);
     const double A[9] = {J.xr, J.xt, J.xp, J.yr, J.yt, J.yp, J.zr, J.zt, 0.0};
-    // A^-1 from the closed form: d_r = r^ . grad, d_theta = r theta^ . grad, d_phi = r sin(theta) phi^ . grad
-    const double st = sqrt(J.xr * J.xr + J.yr * J.yr), ct = J.zr, r = -st / J.zt;
-    const double cp = J.xr / st, sp = J.yr / st;
-    const double Ai[9] = {st * cp, st * sp, ct, r * ct * cp, r * ct * sp, -r * st, -r * st * sp, r * st * cp, 0.0};
+    double Ai[9];
+    if (sd.kind == 0) {
+      // A^-1 from the closed form: d_r = r^ . grad, d_theta = r theta^ . grad, d_phi = r sin(theta) phi^ . grad
+      const double st = sqrt(J.xr * J.xr + J.yr * J.yr), ct = J.zr, r = -st / J.zt;
+      const double cp = J.xr / st, sp = J.yr / st;
+      Ai[0] = st * cp; Ai[1] = st * sp; Ai[2] = ct; Ai[3] = r * ct * cp; Ai[4] = r * ct * sp; Ai[5] = -r * st;
+      Ai[6] = -r * st * sp; Ai[7] = r * st * cp; Ai[8] = 0.0;
+    } else {
+      // cylindrical shell: d_rho = rho^ . grad, d_z = z^ . grad, d_phi = rho phi^ . grad;  (cp, sp) = (J.xr, J.yr), 1 / rho from
+      // the two phi entries (sp^2 + cp^2 = 1)
+      const double cp = J.xr, sp = J.yr, rho = 1.0 / (cp * J.yp - sp * J.xp);
+      Ai[0] = cp; Ai[1] = sp; Ai[2] = 0.0; Ai[3] = 0.0; Ai[4] = 0.0; Ai[5] = 1.0; Ai[6] = -rho * sp; Ai[7] = rho * cp; Ai[8] = 0.0;
+    }
     double T[9];
 #pragma unroll
     for (int i = 0; i < 3; ++i)
@@ -185,7 +194,7 @@ k_map_post(const SubDev* __restrict__ subs, const int32_t* __restrict__ tile_fir
   if (local >= sd.P || point_frozen(sd, local)) return;
   const int64_t p = sd.off + local;
   double w0 = coef * __ldg(mapv + p), w1 = coef * __ldg(mapv + S + p), w2 = coef * __ldg(mapv + 2 * S + p);
-  if (sd.kind == 0) {      // v . (A d_logical): fold A into the weights
+  if (sd.kind != 1) {      // v . (A d_logical): fold A into the weights
     const ShellJac J = shell_jac(sd, tables, local);
     const double a0 = w0 * J.xr + w1 * J.yr + w2 * J.zr, a1 = w0 * J.xt + w1 * J.yt + w2 * J.zt, a2 = w0 * J.xp + w1 * J.yp;
     w0 = a0; w1 = a1; w2 = a2;

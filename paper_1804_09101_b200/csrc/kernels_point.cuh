@@ -489,10 +489,12 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
   int cmask = 0;   // faces flagged CHARACTERISTIC (2) through this point, bit f = face f
   {
     const int i2 = local % sd.n2, t = local / sd.n2, i1 = t % sd.n1, i0 = t / sd.n1;
-    const bool on[6] = {i0 == 0, i0 == sd.n0 - 1, !SHELL && i1 == 0, !SHELL && i1 == sd.n1 - 1, !SHELL && i2 == 0, !SHELL && i2 == sd.n2 - 1};
+    // SHELL covers shells (faces 0, 1) and cylindrical shells (kind 2: faces 0..3, the phi direction is periodic)
+    const bool ax1 = !SHELL || sd.kind == 2;
+    const bool on[6] = {i0 == 0, i0 == sd.n0 - 1, ax1 && i1 == 0, ax1 && i1 == sd.n1 - 1, !SHELL && i2 == 0, !SHELL && i2 == sd.n2 - 1};
     frozen = false;
 #pragma unroll
-    for (int f = 0; f < (SHELL ? 2 : 6); ++f) {
+    for (int f = 0; f < (SHELL ? 4 : 6); ++f) {
       frozen = frozen || (on[f] && sd.face[f] == 1);
       if (CBC && on[f] && sd.face[f] == 2) cmask |= 1 << f;
       if (CBC && SHELL && f < 2 && on[f] && sd.face[f] == 3) cmask |= 64 << f;      // INTERFACE faces: bits 6, 7
@@ -654,10 +656,12 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
       }
       if (CBC && (cmask & 63)) {   // characteristic faces through this point, in face order (rare: face points only)
 #pragma unroll
-        for (int f = 0; f < (SHELL ? 2 : 6); ++f)
+        for (int f = 0; f < (SHELL ? 4 : 6); ++f)
           if (cmask & (1 << f)) {
             const double sg = (f & 1) ? 1.0 : -1.0;
-            if (SHELL) char_bc_pair(G, g1, g2, sg * J.xr, sg * J.yr, sg * J.zr, o_psi, r, o_Phi);   // +- r^ = (st cp, st sp, ct)
+            // shells: +- r^ = (st cp, st sp, ct); cylindrical shells: +- rho^ = (cp, sp, 0) - the same entries - and +- z^
+            if (SHELL && f < 2) char_bc_pair(G, g1, g2, sg * J.xr, sg * J.yr, sg * J.zr, o_psi, r, o_Phi);
+            else if (SHELL) char_bc_pair(G, g1, g2, 0.0, 0.0, sg, o_psi, r, o_Phi);
             else char_bc_pair(G, g1, g2, f / 2 == 0 ? sg : 0.0, f / 2 == 1 ? sg : 0.0, f / 2 == 2 ? sg : 0.0, o_psi, r, o_Phi);
           }
       }
@@ -707,7 +711,7 @@ k_rhs(const SubDev* __restrict__ subs, const int32_t* __restrict__ tile_first, i
   const SubDev& sd = sd_s;
   const int local = (blockIdx.x - tile0_s) * TILE_PTS + threadIdx.x;
   if (local < sd.P) {
-    if (sd.kind == 0) rhs_point<true, RK, CBC, NORMS>(sd, tables, local, u, du, Hs, dHs, k, rk, S, flag, ring_s + threadIdx.x, ifc, Sf);
+    if (sd.kind != 1) rhs_point<true, RK, CBC, NORMS>(sd, tables, local, u, du, Hs, dHs, k, rk, S, flag, ring_s + threadIdx.x, ifc, Sf);
     else rhs_point<false, RK, CBC, NORMS>(sd, tables, local, u, du, Hs, dHs, k, rk, S, flag, ring_s + threadIdx.x);
   }
   if (NORMS) {    // the same fold as K_con: warp shuffle, then the warps in fixed order (deterministic)
@@ -869,7 +873,7 @@ k_con(const SubDev* __restrict__ subs, const int32_t* __restrict__ tile_first, i
   const int local = (blockIdx.x - tile0_s) * TILE_PTS + threadIdx.x;
   double acc[6] = {0, 0, 0, 0, 0, 0};
   if (local < sd.P) {
-    if (sd.kind == 0) con_point<true>(sd, tables, local, u, du, Hs, S, flag, acc);
+    if (sd.kind != 1) con_point<true>(sd, tables, local, u, du, Hs, S, flag, acc);
     else con_point<false>(sd, tables, local, u, du, Hs, S, flag, acc);
   }
 #pragma unroll
