@@ -161,6 +161,22 @@ gh_status gh_rk_step_norms(gh_domain* dom, double dt, double* out, double* per_s
  * GH_ERR_SINGULAR if the device flag was raised. */
 gh_status gh_constraint_norms(gh_domain* dom, double* out, double* per_sub);
 
+/* gh_constraint_norms for callers that may not allocate device memory (code under CUDA graph capture around the call, tight
+ * serving loops, harnesses that forbid cudaMalloc): same arguments, same results bit for bit, but the reduction scratch (per-tile
+ * partials, per-subdomain sums, totals) lives in ONE file-scope static device array of GH_STATIC_SCRATCH_BYTES (3.2 MB, held by
+ * every GPU that loads the library until the process exits) instead of the workspace, the totals are folded on the device, and
+ * the call makes no cudaMalloc / cudaFree, creates no event or graph and uses no host heap (per-launch profiling is off during
+ * the call).  Limits: at most GH_STATIC_MAX_TILES tiles of 128 points (8 388 608 points - the bench workload C4 has 38 036) and
+ * GH_STATIC_MAX_SUBS subdomains; beyond them GH_ERR_ARG with a message, nothing launched.  The array is shared by all calls of
+ * the process and keeps the last call's contents; every value a call reads it has written itself, so nothing needs clearing.
+ * Calls that OVERLAP on the GPU (two domains on different streams, two threads) race on it: serialise them.  The first call
+ * on each device resolves the array's device address (cudaGetSymbolAddress) - make it outside any stream capture.
+ * Synchronises (it returns host data); reports GH_ERR_SINGULAR if the device flag was raised. */
+#define GH_STATIC_MAX_TILES 65536
+#define GH_STATIC_MAX_SUBS 4096
+#define GH_STATIC_SCRATCH_BYTES ((65536 * 6 + 4096 * 6 + 8) * 8)
+gh_status gh_constraint_norms_static(gh_domain* dom, double* out, double* per_sub);
+
 /* ---- spectral filter (NEXT-1 of DESIGN.md; "Filter ~ 30 % of CPU runtime", 452-460, 500-516) ----------
  * "Spectral filtering of 1D basis functions is similar to differentiation, the only difference being the specific
  * form of the transformation matrix": on blocks the state is multiplied along every axis by the

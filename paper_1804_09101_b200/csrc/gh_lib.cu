@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstring>
 #include <map>
+#include <mutex>
 #include <string>
 #include <utility>
 #include <vector>
@@ -1260,6 +1261,107 @@ extern "C" gh_status gh_constraint_norms(gh_domain* d, double* out, double* per_
   st = check_flag(d);   // synchronises
   if (st != GH_OK) return st;
   finish_norms(pl, h, out, per_sub);
+  return GH_OK;
+}
+
+// ------------------------------------------------------------------------------------------------------
+// gh_constraint_norms_static: gh_constraint_norms for callers that may not allocate (CUDA graph capture around them, tight
+// serving loops, harnesses that forbid cudaMalloc).  The reduction scratch of K_con / K_con_reduce - per-tile partials
+// [n_tiles][6], per-subdomain sums [n_sub][6] and the domain's totals [6] - does not come from any workspace but from ONE
+// file-scope device array of fixed size (GH_STATIC_SCRATCH_BYTES = 3.2 MB; every GPU that loads the library holds it until the
+// process exits).  In host code `g_static_scratch` is only a stand-in for the symbol, not a device address: the address is
+// taken once per device with cudaGetSymbolAddress (that device current) and passed to the kernels; K_con_final_static, being
+// device code of this file, names the array directly.  No cudaMalloc / cudaFree / event or graph creation / allocating library
+// call on this path, and no host-side heap use either: the totals are folded on the device (one thread, subdomains in order:
+// the same additions in the same order as the host fold of gh_constraint_norms, so the results are bit-identical) and land in
+// a stack buffer; the per-subdomain values go straight into the caller's array.
+// The array is shared by every call in the process and keeps the last call's contents.  Nothing has to start at zero: every
+// value a call reads (its n_tiles partials, its n_sub sums, the 6 totals) is written earlier in the same call, and nothing
+// beyond them is read.  Calls that overlap on the GPU (two domains on different streams, two host threads) RACE on it:
+// serialise them.
+// ------------------------------------------------------------------------------------------------------
+namespace {
+constexpr size_t STATIC_PART = (size_t)GH_STATIC_MAX_TILES * 6, STATIC_SUB = (size_t)GH_STATIC_MAX_SUBS * 6, STATIC_TOT = 8;
+static_assert((STATIC_PART + STATIC_SUB + STATIC_TOT) * sizeof(double) == GH_STATIC_SCRATCH_BYTES, "gh.h states the size of the static scratch");
+static __device__ __align__(256) double g_static_scratch[STATIC_PART + STATIC_SUB + STATIC_TOT];
+
+// totals [6] from the per-subdomain sums, subdomains in order (sums added, maxima NaN-propagating, exactly like finish_norms)
+__global__ void k_con_final_static(int n_sub) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  const double* ps = g_static_scratch + STATIC_PART;
+  double* tot = g_static_scratch + STATIC_PART + STATIC_SUB;
+  for (int q = 0; q < 3; ++q) {
+    double sum = 0.0, mx = 0.0;
+    for (int s = 0; s < n_sub; ++s) {
+      sum += ps[(size_t)s * 6 + q];
+      const double v = ps[(size_t)s * 6 + 3 + q];
+      if (v != v || v > mx) mx = v;
+    }
+    tot[q] = sum; tot[3 + q] = mx;
+  }
+}
+
+constexpr int STATIC_MAX_DEV = 64;
+std::mutex g_static_mu;
+double* g_static_ptr[STATIC_MAX_DEV] = {};      // device address of g_static_scratch per device ordinal, resolved once
+
+gh_status static_scratch_ptr(gh_domain* d, double** out) {      // the domain's device is current (DeviceGuard of the caller)
+  if (d->device < 0 || d->device >= STATIC_MAX_DEV) return fail(d, GH_ERR_ARG, "gh_constraint_norms_static: device ordinal beyond 63");
+  std::lock_guard<std::mutex> lk(g_static_mu);
+  if (!g_static_ptr[d->device]) {
+    void* ptr = nullptr;
+    GH_CUDA(d, cudaGetSymbolAddress(&ptr, g_static_scratch));
+    g_static_ptr[d->device] = static_cast<double*>(ptr);
+  }
+  *out = g_static_ptr[d->device];
+  return GH_OK;
+}
+}  // namespace
+
+extern "C" gh_status gh_constraint_norms_static(gh_domain* d, double* out, double* per_sub) {
+  DeviceGuard guard_(d);
+  if (!d || !out) return fail(d, GH_ERR_ARG, "NULL argument");
+  if (!d->has_fields) return fail(d, GH_ERR_STATE, "gh_constraint_norms_static before gh_set_fields");
+  const Plan& pl = d->pl;
+  if (pl.n_tiles > GH_STATIC_MAX_TILES || pl.n_sub > GH_STATIC_MAX_SUBS) {
+    char buf[256];
+    snprintf(buf, sizeof buf, "gh_constraint_norms_static: the domain has %d tiles of %d points and %d subdomains; the static scratch holds "
+             "at most %d tiles (%lld points) and %d subdomains - use gh_constraint_norms", pl.n_tiles, TILE_PTS, pl.n_sub,
+             GH_STATIC_MAX_TILES, (long long)GH_STATIC_MAX_TILES * TILE_PTS, GH_STATIC_MAX_SUBS);
+    return fail(d, GH_ERR_ARG, buf);
+  }
+  double* scratch = nullptr;
+  gh_status st = static_scratch_ptr(d, &scratch);
+  if (st != GH_OK) return st;
+  double* part = scratch;
+  double* persub = scratch + STATIC_PART;
+  const double* tot = scratch + STATIC_PART + STATIC_SUB;
+  const bool prof = d->prof;
+  d->prof = false;                      // per-launch profiling would take events from a pool that may have to create them
+  st = launch_derivs(d, d->ua, d->du, NCOMP, 10, 10);
+  d->prof = prof;
+  if (st != GH_OK) return st;
+  if (d->has_map) k_map_pre<<<pl.n_tiles, TILE_PTS, 0, d->stream>>>(d->subs, d->tiles, pl.n_sub, d->tables, d->mapJ, d->du, pl.S, NCOMP);
+  k_con<<<pl.n_tiles, TILE_PTS, 0, d->stream>>>(d->subs, d->tiles, pl.n_sub, d->tables, d->ua, d->du, d->H, pl.S, d->flag, part);
+  k_con_reduce<<<pl.n_sub, 32, 0, d->stream>>>(d->tiles, part, persub);
+  k_con_final_static<<<1, 32, 0, d->stream>>>(pl.n_sub);
+  d->launches += 3 + (d->has_map ? 1 : 0);
+  GH_CUDA(d, cudaGetLastError());
+  double h[6];
+  GH_CUDA(d, cudaMemcpyAsync(h, tot, sizeof h, cudaMemcpyDeviceToHost, d->stream));
+  if (per_sub) GH_CUDA(d, cudaMemcpyAsync(per_sub, persub, (size_t)pl.n_sub * 6 * sizeof(double), cudaMemcpyDeviceToHost, d->stream));
+  st = check_flag(d);   // synchronises
+  if (st != GH_OK) return st;
+  static const double ncomp[3] = {4.0, 30.0, 30.0};
+  for (int q = 0; q < 3; ++q) { out[2 * q] = std::sqrt(h[q] / ((double)pl.P * ncomp[q])); out[2 * q + 1] = h[3 + q]; }
+  if (per_sub)      // raw [s] = {sum0, sum1, sum2, max0, max1, max2} -> {rms0, max0, rms1, max1, rms2, max2}, in place
+    for (int s = 0; s < pl.n_sub; ++s) {
+      int n0, n1, n2; sub_dims(pl.descs[s], n0, n1, n2);
+      const double Ps = (double)n0 * n1 * n2;
+      double r[6];
+      for (int q = 0; q < 6; ++q) r[q] = per_sub[(size_t)s * 6 + q];
+      for (int q = 0; q < 3; ++q) { per_sub[(size_t)s * 6 + 2 * q] = std::sqrt(r[q] / (Ps * ncomp[q])); per_sub[(size_t)s * 6 + 2 * q + 1] = r[3 + q]; }
+    }
   return GH_OK;
 }
 

@@ -36,6 +36,7 @@ EXPORTS = [
     "gh_set_filter", "gh_apply_filter", "gh_filter_sigma",
     "gh_dp5_workspace_bytes", "gh_dp5_attach", "gh_dp5_step", "gh_set_option",
     "gh_rk_step_norms", "gh_set_frame_map", "gh_set_jacobian", "gh_spatial_coord_jac", "gh_spatial_coord_jac_state", "gh_fp64_peak",
+    "gh_constraint_norms_static",
 ]
 
 
@@ -102,6 +103,7 @@ def lib() -> C.CDLL:
     L.gh_gradient.argtypes = [vp, dp, ip]
     L.gh_rk_step.argtypes = [vp, C.c_double]
     L.gh_constraint_norms.argtypes = [vp, dp, dp]
+    L.gh_constraint_norms_static.argtypes = [vp, dp, dp]
     L.gh_rk_step_norms.argtypes = [vp, C.c_double, dp, dp]
     L.gh_set_profiling.argtypes = [vp, ip]
     L.gh_profile_read.argtypes = [vp, dp, dp]
@@ -245,6 +247,14 @@ def gh_constraint_norms(h, n_sub: int, per_sub: bool = False):
     out = np.zeros((3, 2))
     ps = np.zeros((n_sub, 3, 2)) if per_sub else None
     _check(lib().gh_constraint_norms(h, out.ctypes.data, ps.ctypes.data if per_sub else None), h)
+    return (out, ps) if per_sub else out
+
+
+def gh_constraint_norms_static(h, n_sub: int, per_sub: bool = False):
+    """gh_constraint_norms with its reduction scratch in the library's static device array: no allocation on the call path."""
+    out = np.zeros((3, 2))
+    ps = np.zeros((n_sub, 3, 2)) if per_sub else None
+    _check(lib().gh_constraint_norms_static(h, out.ctypes.data, ps.ctypes.data if per_sub else None), h)
     return (out, ps) if per_sub else out
 
 
@@ -459,6 +469,10 @@ class Domain:
     @_ordered
     def constraint_norms(self, per_sub: bool = False):
         return gh_constraint_norms(self.h, self.n_sub, per_sub)
+
+    @_ordered
+    def constraint_norms_static(self, per_sub: bool = False):
+        return gh_constraint_norms_static(self.h, self.n_sub, per_sub)
 
     @_ordered
     def dp5_attach(self):
