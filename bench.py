@@ -668,6 +668,8 @@ def run_sweep(args, dev):
 
     hbm_peak, _ = load_peaks()
     for label, cfg in sweep_members(args.sweep_max_points, args.sweep_paper_members):
+        if args.sweep_only and args.sweep_only not in label:
+            continue
         d = cfg["descs"][0]
         dom = gh.Domain([d], device=dev)
         P, S = dom.P, dom.S
@@ -757,6 +759,7 @@ def main():
     ap.add_argument("--profile-steps", type=int, default=10, help="steps of the second (per-launch events on) pass")
     ap.add_argument("--sweep-reps", type=int, default=20, help="c5: repetitions per member")
     ap.add_argument("--sweep-max-points", type=int, default=40_000_000, help="c5: skip members above this size")
+    ap.add_argument("--sweep-only", default="", help="c5: only the members whose label contains this text (e.g. 'block 160' for an ncu capture)")
     ap.add_argument("--sweep-paper-members", action="store_true", help="c5: also the paper's SingleBH / BBH shell prescriptions (PAPER.md:436)")
     ap.add_argument("--min-points", type=int, default=4_000_000, help="C4: replicate the base set until P >= this")
     ap.add_argument("--e2e-steps", type=int, default=5)

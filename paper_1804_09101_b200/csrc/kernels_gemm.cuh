@@ -34,6 +34,8 @@ struct GemmItem {
   int32_t mbs;                   // m-tiles per M-block (<= MB): the m-tiles are spread evenly over the fewest blocks
 };
 
+// 8 warps x 2 n-tiles.  Measured alternative, not kept: 16 warps x 1 n-tile (128 registers, four warps per scheduler to cover the
+// fixed DMMA issue waits) is 5 % slower on 160^3 / n = 128 - twice the shared-memory fragment loads per DMMA.
 constexpr int GEMM_TPB = 256, GEMM_KB = 8, GEMM_NST = 3, GEMM_NTW = 2;
 constexpr int GEMM_CT = (GEMM_TPB / 32) * 8 * GEMM_NTW;     // 128 columns per CTA
 __host__ __device__ constexpr size_t gemm_stage_doubles(int MB) { return (size_t)MB * GEMM_KB * 32; }
@@ -165,15 +167,29 @@ k_gemm(const GemmItem* __restrict__ items, const double* __restrict__ tables, co
     if (active) {
       const double* __restrict__ a_s = sm + (size_t)(t % NST) * STAGE_MAX + lane;
       const int mtn = min(mbs, MT - mb * mbs);    // m-tiles of this block that exist
+      // mtn < MBS only in the last block of a matrix whose m-tiles do not divide evenly (N = 320: 14 + 14 + 12).  The two cases
+      // are separate loops: a per-tile guard inside the unrolled loop costs a branch and a WARPSYNC per DMMA pair in EVERY block
+      // (ncu: 8 % of the issued instructions; 2.5 % of the kernel time on 160^3 and n = 128)
+      if (mtn == MBS) {
 #pragma unroll
-      for (int ks = 0; ks < KB; ++ks)
+        for (int ks = 0; ks < KB; ++ks)
 #pragma unroll
-        for (int mt = 0; mt < MBS; ++mt)
-          if (MBS == 1 || mt < mtn) {       // mtn < MBS only in the last block of a matrix whose m-tiles do not divide evenly
+          for (int mt = 0; mt < MBS; ++mt) {
             const double a = a_s[(mt * KB + ks) * 32];
 #pragma unroll
             for (int n = 0; n < NTW; ++n) dmma884(acc[mt][n][0], acc[mt][n][1], a, b[ks][n]);
           }
+      } else {
+#pragma unroll
+        for (int ks = 0; ks < KB; ++ks)
+#pragma unroll
+          for (int mt = 0; mt < MBS; ++mt)
+            if (mt < mtn) {
+              const double a = a_s[(mt * KB + ks) * 32];
+#pragma unroll
+              for (int n = 0; n < NTW; ++n) dmma884(acc[mt][n][0], acc[mt][n][1], a, b[ks][n]);
+            }
+      }
       if (kc == nKC - 1) {
         double* dst = out_ptr(t / per);
 #pragma unroll

@@ -687,8 +687,11 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
 // CBC: the domain has faces flagged CHARACTERISTIC (a second instantiation, so that domains without them do not pay for it).
 // NORMS: the constraint norms of the INPUT state as an epilogue (A8 fused into A5: C_a, the derivatives of psi and Phi and
 // Phi itself are on chip anyway; 0 extra bytes): per-tile partials part[tile][6] in the layout of K_con, folded by K_con_reduce.
+#ifndef GH_RHS_CTAS
+#define GH_RHS_CTAS 2      // resident CTAs per SM the register allocation aims at (3: a 170-register cap, measured slower - DESIGN.md §14)
+#endif
 template <int RK, bool CBC, bool NORMS = false>
-__global__ void __launch_bounds__(TILE_PTS, 2)
+__global__ void __launch_bounds__(TILE_PTS, GH_RHS_CTAS)
 k_rhs(const SubDev* __restrict__ subs, const int32_t* __restrict__ tile_first, int n_sub,
       const double* __restrict__ tables, const double* u, const double* __restrict__ du,
       const double* __restrict__ Hs, const double* __restrict__ dHs, double* k, RkArgs rk, int64_t S,
