@@ -54,6 +54,9 @@ __device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
 __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, unsigned bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(bytes) : "memory");
 }
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
+}
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity) {
   asm volatile(
       "{\n"
@@ -76,7 +79,7 @@ __global__ void __launch_bounds__(GEMM_TPB, 1)
 k_gemm(const GemmItem* __restrict__ items, const double* __restrict__ tables, const double* in, double* dub, int64_t S,
        int ncomp, CompMap cm) {
   extern __shared__ __align__(16) double sm[];      // GEMM_NST stages of MB x KB fragments (bulk copies need 16-byte alignment)
-  __shared__ __align__(8) uint64_t full[GEMM_NST];
+  __shared__ __align__(8) uint64_t full[GEMM_NST], empty[GEMM_NST];
   constexpr int KB = GEMM_KB, NST = GEMM_NST, NTW = GEMM_NTW;
   constexpr int STAGE_MAX = MB * KB * 32;
   const GemmItem it = items[blockIdx.x];
@@ -91,7 +94,7 @@ k_gemm(const GemmItem* __restrict__ items, const double* __restrict__ tables, co
 
   if (tid == 0) {
 #pragma unroll
-    for (int s = 0; s < NST; ++s) mbar_init(&full[s], 1);
+    for (int s = 0; s < NST; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], GEMM_TPB / 32); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
@@ -150,7 +153,15 @@ k_gemm(const GemmItem* __restrict__ items, const double* __restrict__ tables, co
 #pragma unroll 1
   for (int t = 0; t < total; ++t) {
     const int r = t % per, mb = r / nKC, kc = r - mb * nKC;
-    if (tid == 0 && t + NST - 1 < total) issue(t + NST - 1);     // into the slot every warp left before the last barrier
+    // Producer / consumer ring without a block barrier: the slot of stage t + NST - 1 is the one stage t - 1 used; the elected
+    // thread refills it once every warp has arrived on its `empty` barrier.  Only warp 0 waits for the slowest warp here; the
+    // others run up to NST - 1 stages apart, so their B-fragment loads, waits and epilogues no longer fall on the same cycles
+    // (with a __syncthreads per stage the pipe idled through them: 69 % busy, profiles/r02_ncu_k_gemm.md).
+    if (tid == 0 && t + NST - 1 < total) {
+      if (t >= 1) mbar_wait(&empty[(t - 1) % NST], (unsigned)(((t - 1) / NST) & 1));
+      issue(t + NST - 1);
+    }
+    __syncwarp();
     if (kc == 0) {
 #pragma unroll
       for (int mt = 0; mt < MBS; ++mt)
@@ -210,7 +221,8 @@ k_gemm(const GemmItem* __restrict__ items, const double* __restrict__ tables, co
         }
       }
     }
-    __syncthreads();
+    __syncwarp();                                   // every lane has its A fragments of this slot in registers
+    if (lane == 0) mbar_arrive(&empty[t % NST]);
   }
   };
 #define GH_GEMM_RUN(K) case K: run(std::integral_constant<int, (K <= MB ? K : MB)>{}); break;
