@@ -330,6 +330,7 @@ struct gh_domain {
   struct FBig { int N; size_t off; bool fourier; };     // large classes: one K_gemm filter matrix slot per (block, large axis) ...
   std::vector<FBig> f_big_blocks;
   std::map<int, std::vector<size_t>> f_big_L;   // ... and per large L the slots of its per-m filtered projectors
+  double gemm_stages[G_NLIST] = {};             // pipeline stages (m-blocks x k-chunks) of one component, summed over the list's items
   bool filt_blocks = false, filt_shells = false;
   // Dormand-Prince 5(4): seven stage derivatives in a separately attached workspace
   double* dpk[7] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
@@ -508,6 +509,8 @@ extern "C" gh_status gh_domain_create(const gh_subdomain_desc* descs, int32_t n_
     for (int64_t c0 = 0; c0 < cols; c0 += GEMM_CT) {
       GemmItem it = proto; it.col0 = (int)c0; it.ncols = (int)std::min<int64_t>(GEMM_CT, cols - c0);
       glist[list].push_back(it);
+      const int MT = (it.M + 7) / 8, KS = (it.K + 3) / 4;
+      d->gemm_stages[list] += (double)((MT + it.mbs - 1) / it.mbs) * ((KS + GEMM_KB - 1) / GEMM_KB);
     }
   };
   struct BigShellOff { int64_t FaQ, FsQ, FpQ; std::vector<int64_t> Th, Pr; };
@@ -968,9 +971,20 @@ void launch_gemm_list(gh_domain* d, int prof_cls, int l, const double* in, doubl
   if (!pl.n_gemm[l]) return;
   int first = 0;
   for (int k = 0; k < l; ++k) first += pl.n_gemm[k];
-  int gw = 1;     // components one CTA walks over: as many as still leave two CTAs per SM in the grid
-  for (int w = 10; w >= 1; --w)
-    if (nrun % w == 0 && (w == 1 || (int64_t)pl.n_gemm[l] * (nrun / w) >= 2 * d->n_sm)) { gw = w; break; }
+  // components one CTA walks over (one CTA per SM is resident): the divisor w of nrun with the best modelled efficiency
+  //   (fill of the last wave: CTAs / (waves x SMs))  x  (pipeline fill: w stages-per-component / (the same + 2 stages of ramp)).
+  // "As many as still leave two CTAs per SM" put 80^3 on 300 CTAs = 2.03 waves (a third, nearly empty wave: 68 %).
+  int gw = 1;
+  {
+    const double per = d->gemm_stages[l] / pl.n_gemm[l];
+    double best = -1.0;
+    for (int w = 1; w <= nrun && w <= 25; ++w) {
+      if (nrun % w) continue;
+      const int64_t ctas = (int64_t)pl.n_gemm[l] * (nrun / w), waves = (ctas + d->n_sm - 1) / d->n_sm;
+      const double eff = (double)ctas / (double)(waves * d->n_sm) * (w * per / (w * per + 2.0));
+      if (eff > best) { best = eff; gw = w; }
+    }
+  }
   ProfScope ps(d, prof_cls);
   k_gemm<GEMM_MB><<<dim3(pl.n_gemm[l], nrun / gw), GEMM_TPB, gemm_smem_bytes(GEMM_MB), d->stream>>>(d->gemm + first, d->tables, in, out, pl.S, nrun, cm);
 }

@@ -36,7 +36,10 @@ struct GemmItem {
 
 // 8 warps x 2 n-tiles.  Measured alternative, not kept: 16 warps x 1 n-tile (128 registers, four warps per scheduler to cover the
 // fixed DMMA issue waits) is 5 % slower on 160^3 / n = 128 - twice the shared-memory fragment loads per DMMA.
-constexpr int GEMM_TPB = 256, GEMM_KB = 8, GEMM_NST = 3, GEMM_NTW = 2;
+#ifndef GH_GEMM_NST
+#define GH_GEMM_NST 3
+#endif
+constexpr int GEMM_TPB = 256, GEMM_KB = 8, GEMM_NST = GH_GEMM_NST, GEMM_NTW = 2;
 constexpr int GEMM_CT = (GEMM_TPB / 32) * 8 * GEMM_NTW;     // 128 columns per CTA
 __host__ __device__ constexpr size_t gemm_stage_doubles(int MB) { return (size_t)MB * GEMM_KB * 32; }
 __host__ __device__ constexpr size_t gemm_smem_bytes(int MB) { return GEMM_NST * gemm_stage_doubles(MB) * sizeof(double); }
