@@ -407,18 +407,21 @@ def run_ours(args):
     t0 = time.perf_counter(); dom.get_fields(out_host); torch.cuda.synchronize(); d2h_s = time.perf_counter() - t0
     pcie = {"h2d_GBps": 50 * S * 8 / h2d_s / 1e9, "d2h_GBps": 50 * S * 8 / d2h_s / 1e9, "copies_only_ms": (h2d_s + d2h_s) * 1e3,
             "single_domain_ms_per_step": e2e_single_s * 1e3}
-    # The same e2e steps with TWO domains in flight (two handles of the same public API on two streams, driven by two host
-    # threads; every step still copies its own 1.94 GB in and out): one domain's H2D overlaps the other's D2H (PCIe is full
-    # duplex) and both overlap the kernels, so the step rate approaches max(H2D, D2H, compute) instead of their sum.
+    # The same e2e steps with SEVERAL domains in flight (handles of the same public API on their own streams, each driven by a host
+    # thread; every step still copies its own 1.94 GB in and out): one domain's H2D overlaps another's D2H (PCIe is full
+    # duplex) and both overlap the kernels.  One domain's chain is H2D + step + D2H (35 + 19 + 35 ms on C4): two in flight can reach
+    # half of that at best, three are bounded by one PCIe direction, max(H2D, D2H, compute).
     e2e_s, e2e_mode = e2e_single_s, "one domain: copy in, step, copy out, one after the other"
     if not args.no_e2e_overlap:
         try:
-            dom2 = gh.Domain(descs, device=dev)
-            if args.no_graph:
-                dom2.set_option(gh.GH_OPT_NO_GRAPH, 1)
-            dom2.set_gauge_source(H_host)
-            out_host2 = torch.empty(50, S, dtype=torch.float64).pin_memory()
-            doms = [(dom, out_host), (dom2, out_host2)]
+            doms = [(dom, out_host)]
+            for _ in range(max(1, args.e2e_domains) - 1):
+                dom2 = gh.Domain(descs, device=dev)
+                if args.no_graph:
+                    dom2.set_option(gh.GH_OPT_NO_GRAPH, 1)
+                dom2.set_gauge_source(H_host)
+                doms.append((dom2, torch.empty(50, S, dtype=torch.float64).pin_memory()))
+            nd = len(doms)
 
             def worker(dm, oh, n):
                 torch.cuda.set_device(local_rank)
@@ -441,16 +444,17 @@ def run_ours(args):
 
             run_pair(1)
             sync_all()
-            n_each = max(1, e2e_steps // 2 + e2e_steps % 2)
+            n_each = max(2, -(-e2e_steps // nd))
             t0 = time.perf_counter()
             run_pair(n_each)
-            e2e_s = (time.perf_counter() - t0) / (2 * n_each)
-            e2e_steps = 2 * n_each
-            e2e_mode = "two domains in flight on two streams (host threads): H2D, kernels and D2H of different steps overlap"
-            if not (bool(torch.isfinite(out_host2).all()) and torch.equal(out_host, out_host2)):
-                raise SystemExit("bench.py: the two e2e domains disagree")
-            dom2.close()
-            del dom2
+            e2e_s = (time.perf_counter() - t0) / (nd * n_each)
+            e2e_steps = nd * n_each
+            e2e_mode = f"{nd} domains in flight on {nd} streams (host threads): H2D, kernels and D2H of different steps overlap"
+            for dm, oh in doms[1:]:
+                if not (bool(torch.isfinite(oh).all()) and torch.equal(out_host, oh)):
+                    raise SystemExit("bench.py: the e2e domains disagree")
+                dm.close()
+            del doms
         except torch.OutOfMemoryError:
             pass
     pcie["mode"] = e2e_mode
@@ -762,12 +766,13 @@ def main():
     ap.add_argument("--sweep-only", default="", help="c5: only the members whose label contains this text (e.g. 'block 160' for an ncu capture)")
     ap.add_argument("--sweep-paper-members", action="store_true", help="c5: also the paper's SingleBH / BBH shell prescriptions (PAPER.md:436)")
     ap.add_argument("--min-points", type=int, default=4_000_000, help="C4: replicate the base set until P >= this")
-    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--e2e-steps", type=int, default=9)
     ap.add_argument("--cpu-points", type=int, default=1_300_000,
                     help="points in the cpu_baseline sample (default: the whole 64-subdomain base set, ~10 s on 16 cores)")
     ap.add_argument("--ref-points", type=int, default=60_000, help="points per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e-overlap", action="store_true", help="e2e leg with one domain only (no second domain in flight)")
+    ap.add_argument("--e2e-domains", type=int, default=3, help="domains in flight in the e2e leg (each with its own stream and host thread)")
     ap.add_argument("--no-graph", action="store_true", help="enqueue the step's kernels one by one instead of replaying the captured CUDA graph")
     ap.add_argument("--unfused-norms", action="store_true", help="step = gh_rk_step + stand-alone gh_constraint_norms (the round-1 path)")
     ap.add_argument("--no-extras", action="store_true", help="skip the spectral-filter and Dormand-Prince legs (run after the timed step)")
