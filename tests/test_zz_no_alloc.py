@@ -48,6 +48,14 @@ def test_static_scratch_matches_existing_path_twice(oracle):
     ref3 = d2.constraint_norms()
     assert _same(got3, ref3, 1e-11 * np.max(np.abs(us2[0]))) and np.array_equal(got3, ref3)
     assert torch.cuda.mem_get_info()[0] >= free1                              # no device memory was taken by the later calls
+    # dual frame set (K_map_pre runs inside both paths): still the same bits
+    S2 = d2.S
+    Jm = np.zeros((9, S2))
+    Jm[0], Jm[4], Jm[8], Jm[1] = 1 / 1.1, 1 / 1.05, 1.0, 0.02
+    d2.set_frame_map(Jm, np.zeros((3, S2)))
+    got4, ref4 = d2.constraint_norms_static(), d2.constraint_norms()
+    assert np.array_equal(got4, ref4) and not np.array_equal(got4, got3)
+    d2.set_frame_map(None, None)
     # the existing path is untouched by the static one
     assert np.array_equal(dom.constraint_norms(), ref2)
     for d, *_ in doms:
