@@ -35,7 +35,18 @@ constexpr int CHEB_NCLASS = 4;                    // register-tile classes: N <=
 inline int cheb_class(int N) { return N <= 24 ? 0 : N <= 32 ? 1 : N <= 48 ? 2 : 3; }
 inline int cheb_ct(int) { return CHEB_CT; }
 inline size_t cheb_frag_doubles(int N) { return (size_t)((N + 7) / 8) * ((N + 3) / 4) * 32; }   // D in fragment order
-constexpr int ANG_TPB0 = 256, ANG_TPB1 = 512;    // K_ang threads: class 0 (two CTAs per SM), class 1 (one CTA per SM)
+// K_ang threads per CTA.  192 x 2 CTAs and 384 x 1 CTA leave 168 registers per thread: no spills.  With 256 / 512 threads (128
+// registers, 104 B of stack) the spill reloads in the unit prologues went out to L2 - at ~200 KB of shared memory per SM there is
+// hardly any L1 left - and ~12 % of the warp-stall samples sat on integer address arithmetic waiting for them
+// (profiles/r02_ncu_k_ang.md section 4).  Measured on C4, per call: 256/512 2.90 ms, 192/384 2.77, 192/320 2.87, 192/448 3.15,
+// 192/256 2.88, 256/384 2.91, 192/512 3.05, 128 x 3 CTAs / 384 2.78.
+#ifndef GH_ANG_TPB0
+#define GH_ANG_TPB0 192
+#endif
+#ifndef GH_ANG_TPB1
+#define GH_ANG_TPB1 384
+#endif
+constexpr int ANG_TPB0 = GH_ANG_TPB0, ANG_TPB1 = GH_ANG_TPB1;    // K_ang threads: class 0 (two CTAs per SM), class 1 (one CTA per SM)
 constexpr size_t ANG_SMEM_2CTA = (GH_ANG_CTAS == 2 ? 113 : GH_ANG_CTAS == 3 ? 74 : 55) * 1024;     // K_ang shared memory that still lets GH_ANG_CTAS CTAs share an SM
 constexpr int ANG_NB_MAX = 8;                    // planes per K_ang CTA offered to the plan (S2 then has <= 2 column tiles per m)
 constexpr int ANG_NB_MAX_SMALL_L = 24;           // ... for L < 12, where a plane is a few tiles only (SingleBH k = 0: 5.96 -> 4.91 ms
