@@ -112,8 +112,14 @@ inline int ang_best_nch3(int NT3, int MT1, int NW) {
 // Modelled duration of one K_ang CTA (units: one DMMA slot of a warp) for `np_` planes of band limit L on NW warps: per stage
 // the number of rounds the warps need times the DMMAs of one unit (the k-steps and tiles the kernel really runs), plus a fixed
 // part for staging and barriers.  Used only to choose the planes per CTA and the CTA class of a shell.
-constexpr double ANG_FIX = 40.0;     // fixed part of a CTA (staging, barriers), in DMMA slots; 10-300 measured, flat optimum near 40
-constexpr double ANG_C0W = (double)GH_ANG_CTAS;      // class 0 runs GH_ANG_CTAS CTAs per SM
+#ifndef GH_ANG_FIX
+#define GH_ANG_FIX 40.0
+#endif
+constexpr double ANG_FIX = GH_ANG_FIX;     // fixed part of a CTA (staging, barriers), in DMMA slots; 10-300 measured, flat optimum near 40
+#ifndef GH_ANG_C0W
+#define GH_ANG_C0W ((double)GH_ANG_CTAS)
+#endif
+constexpr double ANG_C0W = GH_ANG_C0W;      // class 0 runs GH_ANG_CTAS CTAs per SM
 inline double ang_cta_cost(int L, int np_, int NW) {
   const int NT = ang_nt_class(L), nt = L + 1, h = nt, MT1 = (np_ * nt + 7) / 8;
   const int KSe1 = (h + 1 + 3) / 4, KSo1 = (L + 3) / 4, KSe3 = (h + 3) / 4, KSo3 = (L + 3) / 4, nt3 = (h + 1 + 7) / 8;

@@ -264,7 +264,10 @@ __device__ __forceinline__ void ang_s2_unit(const double* __restrict__ tm /* fra
 }
 
 // n-tiles of S2 one unit takes: the accumulators are 4 NT NTN doubles
-__host__ __device__ constexpr int c_ntn(int NT) { return NT == 1 ? 6 : NT == 2 ? 3 : NT == 3 ? 2 : 1; }
+#ifndef GH_ANG_NTN45
+#define GH_ANG_NTN45 1      // two column tiles per S2 unit for NT = 4, 5 measured no gain (2.783 against 2.775 ms per call on C4)
+#endif
+__host__ __device__ constexpr int c_ntn(int NT) { return NT == 1 ? 6 : NT == 2 ? 3 : NT == 3 ? 2 : NT <= 5 ? GH_ANG_NTN45 : 1; }
 
 // the three stages for a shell of class NT (everything that depends on NT at compile time)
 template <int NT, int NW, bool FILTER>
