@@ -443,7 +443,10 @@ __device__ __forceinline__ void rhs_store(double* out, const RkArgs& rk, int64_t
 // the loads of pairs s .. s+RHS_RING-1 are in flight while the algebra of stage 2 and the assembly of earlier pairs
 // run, which is what an HBM-bound kernel with 255 registers per thread (8 warps per SM) cannot get from the warp
 // scheduler alone.
-constexpr int RHS_RING = 3, RHS_RING_ROWS = 22, RHS_PHI_ROWS = 30;   // 15 derivatives + 2 gauge-source gradients + 5 u0 values (RK = 2)
+#ifndef GH_RHS_RING
+#define GH_RHS_RING 3
+#endif
+constexpr int RHS_RING = GH_RHS_RING, RHS_RING_ROWS = 22, RHS_PHI_ROWS = 30;   // 15 derivatives + 2 gauge-source gradients + 5 u0 values (RK = 2)
 constexpr size_t RHS_SMEM_BYTES = (size_t)(RHS_PHI_ROWS + RHS_RING * RHS_RING_ROWS) * TILE_PTS * sizeof(double);
 // NORMS (A8 as an epilogue of A5): this thread's partials {sum C_a^2, sum C_iab^2, sum C_ijab^2, max |C_a|,
 // max |C_iab|, max |C_ijab|} live in shared memory, not registers (the kernel already sits at the register limit): in rows 17..21
@@ -510,7 +513,7 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
   if (!skip) {
     rhs_prefetch<0, RK>(ring + 0 * SLOT, du, dHs, rk.u0, S, p);
     rhs_prefetch<1, RK>(ring + 1 * SLOT, du, dHs, rk.u0, S, p);
-    rhs_prefetch<2, RK>(ring + 2 * SLOT, du, dHs, rk.u0, S, p);
+    if (RHS_RING > 2) rhs_prefetch<2, RK>(ring + (RHS_RING > 2 ? 2 : 0) * SLOT, du, dHs, rk.u0, S, p);
   }
   const PhiSm Phi{phis};
   double psi[10], H[4], Pi[10];
@@ -672,13 +675,9 @@ __device__ __forceinline__ void rhs_point(const SubDev& sd, const double* __rest
       for (int i = 0; i < 3; ++i)
         rhs_store<RK>(k, rk, (int64_t)(20 + 10 * i + s) * S + p, o_Phi[i], Phi(i, s), RK == 2 ? slot[(19 + i) * TILE_PTS] : 0.0);
       // every value of the slot has been consumed: refill it with pair s + RHS_RING
-      if (s == 0) rhs_prefetch<3, RK>(ring + 0 * SLOT, du, dHs, rk.u0, S, p);
-      if (s == 1) rhs_prefetch<4, RK>(ring + 1 * SLOT, du, dHs, rk.u0, S, p);
-      if (s == 2) rhs_prefetch<5, RK>(ring + 2 * SLOT, du, dHs, rk.u0, S, p);
-      if (s == 3) rhs_prefetch<6, RK>(ring + 0 * SLOT, du, dHs, rk.u0, S, p);
-      if (s == 4) rhs_prefetch<7, RK>(ring + 1 * SLOT, du, dHs, rk.u0, S, p);
-      if (s == 5) rhs_prefetch<8, RK>(ring + 2 * SLOT, du, dHs, rk.u0, S, p);
-      if (s == 6) rhs_prefetch<9, RK>(ring + 0 * SLOT, du, dHs, rk.u0, S, p);
+#define GH_PF(K) if (s == K && K + RHS_RING < 10) rhs_prefetch<(K + RHS_RING < 10 ? K + RHS_RING : 9), RK>(ring + (K % RHS_RING) * SLOT, du, dHs, rk.u0, S, p);
+      GH_PF(0) GH_PF(1) GH_PF(2) GH_PF(3) GH_PF(4) GH_PF(5) GH_PF(6) GH_PF(7)
+#undef GH_PF
 
     }
 #undef GH_NACC
