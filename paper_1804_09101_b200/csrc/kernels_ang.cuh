@@ -177,7 +177,10 @@ __device__ __forceinline__ void ang_s3_unit(const double* __restrict__ a0p, cons
 // reflection like Pr_m): the filtered coefficients gamma +- delta replace C in Y; X is not written.
 // NTN: exact compile-time number of column tiles of this unit.  The k-steps and m-tiles need no run-time count: with nt = L+1,
 // hh = ceil(nt/2): ceil(hh/4) = ceil(nt/8) = NT k-steps, ceil(2 hh/8) = NT m-tiles (FILTER: ceil(hh/8) = ceil(NT/2)), always.
-__host__ __device__ constexpr int c_s2d(int NT) { return NT <= 3 ? NT : (NT % 2 == 0 ? 2 : 1); }   // ring depth: divides NT
+#ifndef GH_ANG_S2D4
+#define GH_ANG_S2D4 2      // depth 4 for NT = 4 (the whole mode ahead) spills 32 B at 168 registers: 2.839 against 2.769 ms per call on C4
+#endif
+__host__ __device__ constexpr int c_s2d(int NT) { return NT <= 3 ? NT : NT == 4 ? GH_ANG_S2D4 : (NT % 2 == 0 ? 2 : 1); }   // ring depth: divides NT
 
 template <int NT, int NTN, bool FILTER>
 __device__ __forceinline__ void ang_s2_unit(const double* __restrict__ tm /* fragments of mode m + lane */,
